@@ -1,0 +1,253 @@
+"""Pins the CPU oracle to things other than itself (CPU only; -m "not gpu").
+
+  * hand-computed worked examples T1-T5 (tests/golden/worked_examples.json)
+  * brute-force nested-loop join == hash-multimap join (definition 3)
+  * pandas / numpy group-by + merge as an independent third opinion (special cases reducing to library routines)
+  * invariants I1-I7 and closed-form pass fractions of the seeded generator
+  * adversarial inputs: duplicate build keys, dangling fks, sentinel-valued keys, wrapping products
+"""
+import numpy as np
+import pandas as pd
+import pytest
+
+import oracle
+import plans
+from golden_util import load, table
+from paper_2606_24647_b200 import datagen
+
+G = load()
+
+
+def _cols(res):
+    return [list(map(int, c)) for c in res.cols]
+
+
+def _rows(res):
+    return [list(map(int, r)) for r in zip(*res.cols)] if res.nrows else []
+
+
+# ------------------------------------------------------------------ worked examples
+def test_T1_filter_lowcard_groupby():
+    t = table(G["T1"]["cols"], G["T1"]["rows"])
+    f = dict(shipdate=t["shipdate"], quantity=t["qty"], price=t["price"], discount=t["disc"], tax=t["tax"],
+             flagA=t["flagA"], flagB=t["flagB"])
+    r = oracle.run_query(plans.plan_c1({"fact": f}))
+    assert _rows(r) == G["T1"]["expect"]
+    assert r.input_rows == G["T1"]["rows_passing"] == sum(row[-1] for row in _rows(r))
+    assert not r.overflow
+    for g, row in enumerate(_rows(r)):
+        assert oracle.avg(row[2], row[6]) == G["T1"]["expect_avg_qty"][g]
+        assert oracle.avg(row[3], row[6]) == G["T1"]["expect_avg_price"][g]
+
+
+def test_T2_selective_filter_global_sum():
+    t = table(G["T2"]["cols"], G["T2"]["rows"])
+    f = dict(shipdate=t["shipdate"], discount=t["disc"], quantity=t["qty"], price=t["price"])
+    r = oracle.run_query(plans.plan_c2({"fact": f}))
+    assert _rows(r) == G["T2"]["expect"]
+
+
+def _t3():
+    d = table(G["T3"]["dim_cols"], G["T3"]["dim"])
+    f = table(G["T3"]["fact_cols"], G["T3"]["fact"])
+    return {"dim": d, "fact": dict(fk=f["fk"], shipdate=f["shipdate"], price=f["price"], discount=f["disc"])}
+
+
+def test_T3_join_groupby_topk():
+    r = oracle.run_query(plans.plan_c3(_t3()))
+    assert _rows(r) == G["T3"]["expect"]
+    assert r.input_rows == G["T3"]["join_rows"]
+    r = oracle.run_query(plans.plan_c3(_t3(), topk=10))
+    assert _rows(r) == G["T3"]["expect_topk"]
+    r = oracle.run_query(plans.plan_c3(_t3(), topk=1))
+    assert _rows(r) == G["T3"]["expect_topk"][:1]
+
+
+def test_T4_chained_join():
+    c = table(G["T4"]["cust_cols"], G["T4"]["cust"])
+    o = table(G["T4"]["orders_cols"], G["T4"]["orders"])
+    f = table(G["T4"]["fact_cols"], G["T4"]["fact"])
+    t = {"cust": c, "orders": o, "fact": dict(fk=f["fk"], shipdate=f["shipdate"], price=f["price"], discount=f["disc"])}
+    r = oracle.run_query(plans.plan_c4(t))
+    assert _rows(r) == G["T4"]["expect"]
+    assert r.input_rows == G["T4"]["join_rows"]
+
+
+def test_T5_extreme_keys_min_max():
+    t = table(G["T5"]["cols"], G["T5"]["rows"])
+    f = dict(key=t["key"], shipdate=t["shipdate"], price=t["price"], quantity=t["qty"])
+    r = oracle.run_query(plans.plan_c5({"fact": f}))
+    assert _rows(r) == G["T5"]["expect"]
+    assert r.input_rows == G["T5"]["rows_passing"]
+
+
+# ------------------------------------------------------------------ joins: brute force, duplicates, dangling
+@pytest.mark.parametrize("seed", [1, 2, 3])
+def test_join_equals_bruteforce_with_duplicates_and_dangling(seed):
+    rng = np.random.default_rng(seed)
+    nb, npr = 700, 1500
+    bkey = rng.integers(0, 300, nb).astype(np.int64)        # duplicates on the build side (S3)
+    bval = rng.integers(0, 2406, nb).astype(np.int32)
+    pkey = rng.integers(-50, 400, npr).astype(np.int64)     # some fks match nothing (S4)
+    pval = rng.integers(0, 2526, npr).astype(np.int32)
+    a = oracle.join_pairs([bkey, bval], [(1, "lt", 1200)], 0, [pkey, pval], [(1, "gt", 1200)], 0)
+    b = oracle.join_pairs([bkey, bval], [(1, "lt", 1200)], 0, [pkey, pval], [(1, "gt", 1200)], 0, bruteforce=True)
+    assert a.nrows == b.nrows > 0
+    assert _cols(a) == _cols(b)
+    # third opinion: pandas merge cardinality (I2)
+    B = pd.DataFrame(dict(k=bkey, v=bval)).query("v < 1200")
+    P = pd.DataFrame(dict(k=pkey, v=pval)).query("v > 1200")
+    assert len(P.merge(B, on="k", how="inner")) == a.nrows
+    # the query path over the same join: COUNT(*) summed over groups == join cardinality
+    q = dict(builds=[dict(table=[bkey, bval], preds=[(1, "lt", 1200)], probes=[], key=0, payload=[1])],
+             table=[pkey, pval], preds=[(1, "gt", 1200)], probes=[(0, 0)], exprs=[[("col", 2)]], keys=[0],
+             aggs=[("count",), ("sum", 0)])
+    r = oracle.run_query(q)
+    assert r.input_rows == a.nrows == int(r.cols[1].sum())
+    M = P.merge(B, on="k", how="inner").groupby("k").agg(n=("v_y", "size"), s=("v_y", "sum")).sort_index()
+    assert list(M.index) == list(r.cols[0]) and list(M.n) == list(r.cols[1]) and list(M.s) == list(r.cols[2])
+
+
+# ------------------------------------------------------------------ third opinion on the configs (pandas / numpy)
+def test_c1_vs_pandas():
+    t = datagen.make_config(1, scale=0.2)
+    r = oracle.run_query(plans.plan_c1(t))
+    f = pd.DataFrame(t["fact"]).query("shipdate <= 2430")
+    f["dp"] = f.price * (100 - f.discount)
+    f["ch"] = f.dp * (100 + f.tax)
+    g = f.groupby(["flagA", "flagB"]).agg(q=("quantity", "sum"), p=("price", "sum"), dp=("dp", "sum"),
+                                          ch=("ch", "sum"), n=("price", "size")).sort_index().reset_index()
+    assert r.nrows == len(g) == 6
+    for c, name in enumerate(["flagA", "flagB", "q", "p", "dp", "ch", "n"]):
+        assert list(g[name]) == list(r.cols[c])
+    assert r.input_rows == len(f) and not r.overflow                          # I1
+    assert abs(len(f) / len(t["fact"]["price"]) - 2431 / 2526) < 5 * (0.0362 / 2e5) ** 0.5   # closed form, 5 sigma
+
+
+def test_c2_vs_numpy():
+    t = datagen.make_config(2, scale=0.02)
+    f = t["fact"]
+    r = oracle.run_query(plans.plan_c2(t))
+    m = (f["shipdate"] >= 730) & (f["shipdate"] < 1095) & (f["discount"] >= 5) & (f["discount"] <= 7) & (f["quantity"] < 24)
+    assert _rows(r) == [[int((f["price"][m] * f["discount"][m]).sum()), int(m.sum())]]
+    n = len(m)
+    p = (365 / 2526) * (3 / 11) * (23 / 50)
+    assert abs(m.sum() - n * p) < 5 * (n * p * (1 - p)) ** 0.5                  # closed form, 5 sigma
+
+
+def test_c3_vs_pandas_and_invariants():
+    t = datagen.make_config(3, scale=0.004)
+    r = oracle.run_query(plans.plan_c3(t))
+    D = pd.DataFrame(t["dim"]).query("orderdate < 1200")
+    F = pd.DataFrame(t["fact"]).query("shipdate > 1200")
+    M = F.merge(D, left_on="fk", right_on="key", how="inner")
+    M["dp"] = M.price * (100 - M.discount)
+    g = M.groupby("key").agg(s=("dp", "sum"), n=("dp", "size")).sort_index()
+    assert list(g.index) == list(r.cols[0]) and list(g.s) == list(r.cols[1]) and list(g.n) == list(r.cols[2])
+    assert r.input_rows == len(M) == int(r.cols[2].sum())                      # I1, I2
+    assert r.cols[2].min() >= 1 and r.cols[2].max() <= 7 and r.nrows <= len(D)  # I4
+    top = oracle.run_query(plans.plan_c3(t, topk=10))
+    exp = g.reset_index().sort_values(["s", "key"], ascending=[False, True]).head(10)
+    assert list(exp.key) == list(top.cols[0]) and list(exp.s) == list(top.cols[1])
+
+
+def test_c4_vs_pandas_and_invariants():
+    t = datagen.make_config(4, scale=0.004)
+    r = oracle.run_query(plans.plan_c4(t))
+    Cc = pd.DataFrame(t["cust"]).query("segment == 1")
+    O = pd.DataFrame(t["orders"]).query("orderdate < 1200").merge(Cc, left_on="custkey", right_on="key")
+    F = pd.DataFrame(t["fact"]).query("shipdate > 1200").merge(O, left_on="fk", right_on="orderkey")
+    F["dp"] = F.price * (100 - F.discount)
+    g = F.groupby(["orderkey", "orderdate"]).agg(s=("dp", "sum"), n=("dp", "size")).sort_index().reset_index()
+    assert r.nrows == len(g) > 0
+    for c, name in enumerate(["orderkey", "orderdate", "s", "n"]):
+        assert list(g[name]) == list(r.cols[c])
+    assert r.input_rows == len(F)
+    # I4: every emitted (orderkey, orderdate) is the orders table's pair
+    od = dict(zip(t["orders"]["orderkey"].tolist(), t["orders"]["orderdate"].tolist()))
+    assert all(od[int(k)] == int(d) for k, d in zip(r.cols[0], r.cols[1]))
+
+
+def test_c5_vs_pandas_and_invariants():
+    t = datagen.make_config(5, scale=0.0005)
+    r = oracle.run_query(plans.plan_c5(t))
+    F = pd.DataFrame(t["fact"]).query("shipdate < 2000")
+    g = F.groupby("key").agg(sp=("price", "sum"), sq=("quantity", "sum"), mn=("price", "min"), mx=("price", "max"),
+                             n=("price", "size")).sort_index().reset_index()
+    for c, name in enumerate(["key", "sp", "sq", "mn", "mx", "n"]):
+        assert list(g[name]) == list(r.cols[c])
+    # I3: MIN <= SUM/COUNT <= MAX, sums add up to the global sum
+    assert np.all(r.cols[3] * r.cols[5] <= r.cols[1]) and np.all(r.cols[1] <= r.cols[4] * r.cols[5])
+    assert int(r.cols[1].sum()) == int(F.price.sum()) and r.input_rows == len(F)
+
+
+# ------------------------------------------------------------------ invariants I5-I7, special cases
+def test_filter_true_false_and_empty():
+    t = datagen.make_config(2, scale=0.001)
+    f = t["fact"]
+    cols = [f["shipdate"], f["discount"], f["quantity"], f["price"]]
+    allp = oracle.run_query(dict(table=cols, preds=[], exprs=[[("col", 3)]], keys=[], aggs=[("sum", 0), ("count",)]))
+    assert _rows(allp) == [[int(f["price"].sum()), len(f["price"])]]                       # I5
+    none = oracle.run_query(dict(table=cols, preds=[(0, "lt", -1)], exprs=[[("col", 3)]], keys=[],
+                                 aggs=[("sum", 0), ("count",)]))
+    assert _rows(none) == [[0, 0]]                                                         # S9 global
+    noneg = oracle.run_query(dict(table=cols, preds=[(0, "lt", -1)], exprs=[[("col", 3)]], keys=[1],
+                                  aggs=[("sum", 0), ("count",)]))
+    assert noneg.nrows == 0                                                                # S9 grouped
+    empty = oracle.run_query(dict(table=[c[:0] for c in cols], preds=[], exprs=[[("col", 3)]], keys=[1],
+                                  aggs=[("sum", 0)]))
+    assert empty.nrows == 0
+
+
+def test_batch_split_permutation_and_partial_merge_invariance():
+    t = datagen.make_config(5, scale=0.0002)
+    base = oracle.run_query(plans.plan_c5(t))
+    n = len(t["fact"]["key"])
+    perm = np.random.default_rng(7).permutation(n)
+    tp = {"fact": {k: v[perm] for k, v in t["fact"].items()}}
+    assert _cols(oracle.run_query(plans.plan_c5(tp))) == _cols(base)                       # I7
+    # I6: aggregate the two halves separately, merge (Partial -> Final), compare
+    merged = {}
+    for lo, hi in [(0, n // 3), (n // 3, n)]:
+        part = oracle.run_query(plans.plan_c5({"fact": {k: v[lo:hi] for k, v in t["fact"].items()}}))
+        for row in _rows(part):
+            m = merged.setdefault(row[0], [0, 0, 2**63 - 1, -2**63, 0])
+            m[0] += row[1]; m[1] += row[2]; m[2] = min(m[2], row[3]); m[3] = max(m[3], row[4]); m[4] += row[5]
+    assert [[k] + v for k, v in sorted(merged.items())] == _rows(base)
+
+
+def test_bounds_inclusive_exclusive():
+    x = np.array([4, 5, 6, 7, 8], dtype=np.int32)
+    one = np.ones(5, dtype=np.int64)
+    def cnt(pred):
+        return int(oracle.run_query(dict(table=[x, one], preds=[pred], exprs=[], keys=[], aggs=[("count",)])).cols[0][0])
+    assert [cnt((0, "lt", 6)), cnt((0, "le", 6)), cnt((0, "gt", 6)), cnt((0, "ge", 6)), cnt((0, "eq", 6)),
+            cnt((0, "ne", 6)), cnt((0, "range_co", 5, 7)), cnt((0, "range_cc", 5, 7))] == [2, 3, 2, 3, 1, 4, 2, 3]
+
+
+def test_wrapping_products_flag_overflow():
+    a = np.array([2**62, -3, 5], dtype=np.int64)
+    b = np.array([4, 2**62, 7], dtype=np.int64)
+    r = oracle.filter_project([a, b], [], [[("col", 0), ("col", 1), ("mul",)], [("col", 0), ("col", 1), ("sub",)]])
+    assert r.overflow
+    def wrap(x):                                                                           # low 64 bits, two's complement
+        x %= 2**64
+        return x - 2**64 if x >= 2**63 else x
+    assert list(map(int, r.cols[0])) == [wrap(2**64), wrap(-3 * 2**62), 35] == [0, 2**62, 35]
+    assert list(map(int, r.cols[1])) == [2**62 - 4, -3 - 2**62, -2]
+    r2 = oracle.filter_project([a[2:], b[2:]], [], [[("col", 0), ("col", 1), ("mul",)]])
+    assert not r2.overflow
+
+
+def test_filter_project_keeps_input_order_and_signed_narrow_types():
+    d = np.array([-128, -1, 0, 127], dtype=np.int8)
+    v = np.array([10, 20, 30, 40], dtype=np.int32)
+    r = oracle.filter_project([d, v], [(0, "lt", 0)], [[("col", 1), ("col", 0), ("add",)]])
+    assert list(map(int, r.cols[0])) == [10 - 128, 19]                                      # S21 sign extension
+
+
+def test_no_overflow_in_configs():
+    # S6: the int128 shadow must stay silent on the config value ranges (max product 1.134e11 per row)
+    for cfg, sc in [(1, 0.05), (3, 0.001), (5, 0.0001)]:
+        t = datagen.make_config(cfg, scale=sc)
+        assert not oracle.run_query(plans.PLANS[cfg](t)).overflow
