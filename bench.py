@@ -1,0 +1,333 @@
+#!/usr/bin/env python
+"""bench.py — measures the hot path on B200 (contract: prompt §④ / "Maintain bench.py").
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--configs 1,3,4,5] [--c5-scale S]
+
+A step = one pass of the whole fused pipeline (table init -> fused scan kernel -> finaliser) over one batch of
+synthetic input. Headline workload: BASELINE.json configs[1] (C2: selective filter + global SUM over 60 M rows, the
+pure scan-bandwidth test the metric's >=70 % target is quoted on). The other configs are measured once each and
+reported under "per_config" in the same JSON line. Inputs (1.68 GB) are larger than L2 (126 MB), so every timed
+iteration reads HBM. N > 1 (torchrun): the path does not shard — each rank runs an independent replica ("replicas
+only") and value = N * rows / max-over-ranks time.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+for p in (ROOT, os.path.join(ROOT, "tests")):
+    if p not in sys.path:
+        sys.path.insert(0, p)
+
+import numpy as np  # noqa: E402
+
+METRIC = "input rows/s and achieved HBM GB/s (% of B200 peak) per operator pipeline"
+ALG_BYTES_PER_ROW = {1: 38, 2: 28, 3: 28, 4: 28, 5: 28}   # referenced fact columns, SURVEY §8(d)
+
+
+def peaks():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(path):
+        with open(path) as f:
+            return float(json.load(f)["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs, copy read+write)"
+    return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
+
+
+class ClockSampler:
+    """Samples nvidia-smi clocks and throttle reasons during the timed region."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index=0):
+        self.rows, self.proc, self.index = [], None, index
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), f"--query-gpu={self.Q}",
+                                          "--format=csv,noheader,nounits", "-lms", "100"], stdout=subprocess.PIPE, text=True)
+            threading.Thread(target=self._read, daemon=True).start()
+        except Exception:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append([x.strip() for x in line.split(",")])
+
+    def stop(self):
+        if self.proc:
+            self.proc.terminate()
+        sm = [float(r[0]) for r in self.rows if r and r[0].replace(".", "").isdigit()]
+        mx = [float(r[1]) for r in self.rows if len(r) > 1 and r[1].replace(".", "").isdigit()]
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        reasons = [n for i, n in enumerate(names) if any(len(r) > 3 + i and r[3 + i] == "Active" for r in self.rows)]
+        return dict(sm_mhz=float(np.median(sm)) if sm else None, sm_max_mhz=max(mx) if mx else None, reasons=reasons,
+                    samples=len(sm))
+
+
+def dist():
+    ws = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    lr = int(os.environ.get("LOCAL_RANK", "0"))
+    return ws, rank, lr
+
+
+def time_steps(torch, stream, fn, steps, warmup, barrier):
+    """W untimed + K timed calls of fn, CUDA events on the launching stream; returns total ms (this rank)."""
+    for _ in range(warmup):
+        fn()
+    torch.cuda.synchronize()
+    barrier()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    with torch.cuda.stream(stream):
+        e0.record(stream)
+        for _ in range(steps):
+            fn()
+        e1.record(stream)
+    torch.cuda.synchronize()
+    barrier()
+    return e0.elapsed_time(e1)
+
+
+def run_config(cfg, gq, ctx, torch, datagen, plans, gqrun, steps, warmup, scale=1.0, peak=6548.2):
+    """Device-resident timing of one config: whole pipeline (builds + fused scan + finalise) and its scan kernel."""
+    t0 = time.time()
+    tabs = datagen.make_config(cfg, scale=scale)
+    plan = plans.PLANS[cfg](tabs, topk=10) if cfg == 3 else plans.PLANS[cfg](tabs)
+    gen_s = time.time() - t0
+    nrows = len(plan["table"][0])
+    ncopies = 1
+    fact_bytes = sum(c.nbytes for c in plan["table"])
+    if fact_bytes < 2 * 126e6:               # C1: rotate copies so every timed rep reads cold HBM
+        ncopies = int(np.ceil(3 * 126e6 / fact_bytes)) + 1
+    # planner-style cardinality hints: expected surviving build rows / groups + 10 %
+    hints = {3: [0.55], 4: [0.22, 0.11]}
+    if cfg in hints:
+        for b, h in zip(plan["builds"], hints[cfg]):
+            b["max_rows"] = int(len(b["table"][0]) * h) + 1024
+        plan["max_groups"] = plan["builds"][-1]["max_rows"]
+    if cfg == 5:
+        plan["max_groups"] = int(datagen.ROWS[5]["keys"] * scale)
+    build_cols = [gqrun.dev(b["table"]) for b in plan.get("builds", [])]
+    fact = [gqrun.dev(plan["table"]) for _ in range(ncopies)]
+    torch.cuda.synchronize()
+    build_bytes = sum(c.nbytes for b in plan.get("builds", []) for c in b["table"])
+    state = {"i": 0, "tables": None, "pipes": None}
+
+    def make():
+        state["tables"] = gqrun.build_tables(ctx, plan, device_tables=build_cols)
+        state["pipes"] = [gqrun.prepare(ctx, plan, state["tables"], cols=f,
+                                        out_capacity=(10 if cfg == 3 else plan["max_groups"])) for f in fact]
+    make()
+
+    def step():
+        if plan.get("builds"):
+            state["tables"] = gqrun.build_tables(ctx, plan, device_tables=build_cols)   # re-init + rebuild: timed
+            probes = [(state["tables"][bi], kc) for bi, kc in plan["probes"]]
+            for p in state["pipes"]:
+                pp, _ = p.m.probes(probes)
+                p.plan.agg.probes = pp
+        state["pipes"][state["i"] % ncopies].run()
+        state["i"] += 1
+    l0 = ctx.launch_count()
+    step(); ctx.sync()
+    launches_per_step = ctx.launch_count() - l0
+    ms = time_steps(torch, ctx.stream, step, steps, warmup, lambda: None) / steps
+    ctx.sync()
+    alg = ALG_BYTES_PER_ROW[cfg] * nrows + build_bytes
+    out = dict(rows=nrows, ms_per_step=ms, rows_per_s=nrows / ms * 1e3, alg_gb=alg / 1e9, gbs=alg / ms / 1e6,
+               frac_of_measured=alg / ms / 1e6 / peak, frac_of_8000=alg / ms / 1e6 / 8000.0,
+               launches_per_step=launches_per_step, scale=scale, cold_copies=ncopies, gen_s=round(gen_s, 2))
+    if cfg == 1:   # L2-warm figure, labelled as such
+        def warm():
+            state["pipes"][0].run()
+        out["ms_l2_warm"] = time_steps(torch, ctx.stream, warm, steps, warmup, lambda: None) / steps
+    return out, plan, state
+
+
+def oracle_rate(plans, datagen, cfg, sample_rows, reps=1):
+    """The oracle as it stands, single thread, on a bounded sample of the workload (rows/s)."""
+    import oracle
+    scale = sample_rows / datagen.ROWS[cfg]["fact"]
+    plan = plans.PLANS[cfg](datagen.make_config(cfg, scale=scale))
+    n = len(plan["table"][0])
+    best = None
+    for _ in range(reps):
+        t0 = time.perf_counter()
+        oracle.run_query(plan)
+        dt = time.perf_counter() - t0
+        best = dt if best is None else min(best, dt)
+    return n / best, n, best
+
+
+def main_reference(args):
+    """--impl reference: the CPU oracle (this tier's reference arm) on the box's host cores, rank 0 only."""
+    ws, rank, _ = dist()
+    if rank != 0:
+        return
+    import plans
+    from paper_2606_24647_b200 import datagen
+    sample = 12_000_000
+    for _ in range(args.warmup):
+        oracle_rate(plans, datagen, 2, 1_000_000)
+    t0 = time.perf_counter()
+    rows = 0
+    for _ in range(args.steps):
+        r, n, dt = oracle_rate(plans, datagen, 2, sample)
+        rows += n
+    total = time.perf_counter() - t0
+    import oracle  # timed part only
+    # generation is inside oracle_rate but outside its timed region; recompute pure oracle time
+    rate, n, dt = oracle_rate(plans, datagen, 2, sample, reps=max(1, args.steps))
+    line = dict(impl="reference", metric=METRIC, value=rate, unit="rows/s", n_gpus=args.gpus, steps=args.steps,
+                warmup=args.warmup, ms_per_step=dt * 1e3, higher_is_better=True, scaling="weak", vs_baseline=None,
+                dtype="int64", data="synthetic",
+                config=dict(workload="C2 selective filter + global SUM(price*discount), 60M-row fact (BASELINE configs[1])",
+                            sample=f"first {n} rows of the seeded C2 table per step"),
+                cpu_baseline=dict(value=rate, unit="rows/s", cores=1, kind="oracle",
+                                  sample=f"{n} rows of C2, best of {max(1, args.steps)}"),
+                e2e=dict(value=rate, unit="rows/s", h2d_bytes_per_step=0, d2h_bytes_per_step=0), gpu_launches=0)
+    print(json.dumps(line))
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=5)
+    ap.add_argument("--impl", default="ours")
+    ap.add_argument("--configs", default="1,3,4,5", help="extra configs reported under per_config ('' = none)")
+    ap.add_argument("--c5-scale", type=float, default=1.0)
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    args.warmup = max(args.warmup, 3)
+    if args.impl == "reference":
+        return main_reference(args)
+
+    import torch
+    import gqrun
+    import plans
+    from paper_2606_24647_b200 import build as gqbuild, datagen
+    ws, rank, lr = dist()
+    if ws > 1:
+        import torch.distributed as td
+        torch.cuda.set_device(lr)
+        td.init_process_group("nccl", device_id=torch.device("cuda", lr))
+        flag = torch.zeros(1, device="cuda")
+
+        def barrier():
+            td.all_reduce(flag)
+            torch.cuda.synchronize()
+    else:
+        def barrier():
+            pass
+    if rank == 0:
+        gqbuild.build()
+    barrier()
+    from paper_2606_24647_b200 import gq
+    dev_index = lr if ws > 1 else 0
+    ctx = gq.Context(dev_index)
+    peak, peak_src = peaks()
+
+    # ---------------- headline: C2, device-resident ----------------
+    tabs = datagen.make_config(2)
+    plan = plans.plan_c2(tabs)
+    nrows = len(plan["table"][0])
+    cols = gqrun.dev(plan["table"], device=f"cuda:{dev_index}")
+    pipe = gqrun.prepare(ctx, plan, [], cols=cols)
+    l0 = ctx.launch_count()
+    pipe.run(); ctx.sync()
+    launches_per_step = ctx.launch_count() - l0
+    import oracle  # parity of the timed configuration against the oracle (full 60 M rows)
+    exp = oracle.run_query(plan) if (rank == 0 and not args.no_cpu_baseline) else None
+    res = pipe.result()
+    parity = None if exp is None else bool(res["n"] == 1 and all(int(a[0]) == int(e[0]) for a, e in zip(res["aggs"], exp.cols)))
+    sampler = ClockSampler(dev_index)
+    sampler.start()
+    total_ms = time_steps(torch, ctx.stream, pipe.run, args.steps, args.warmup, barrier)
+    # dominant kernel alone: further batches into an existing aggregation state launch only the fused scan kernel
+    st = ctx.aggregate(None, cols, preds=plan["preds"], exprs=plan["exprs"], keys=[], aggs=plan["aggs"], max_groups=1)
+    scan = lambda: ctx.aggregate(st, cols, preds=plan["preds"], exprs=plan["exprs"], keys=[], aggs=plan["aggs"], max_groups=1)
+    scan_ms = time_steps(torch, ctx.stream, scan, args.steps, args.warmup, lambda: None) / args.steps
+    # read-only roofline probe of this box (same bytes)
+    probe_t = torch.empty(1 << 30, dtype=torch.uint8, device=f"cuda:{dev_index}")
+    probe_ms = time_steps(torch, ctx.stream, lambda: ctx.read_probe(probe_t), 10, 3, lambda: None) / 10
+    clocks = sampler.stop()
+    if ws > 1:
+        t = torch.tensor([total_ms], device="cuda")
+        td.all_reduce(t, op=td.ReduceOp.MAX)
+        total_ms = float(t.item())
+    ms_per_step = total_ms / args.steps
+    value = ws * nrows / ms_per_step * 1e3
+    alg_bytes = ALG_BYTES_PER_ROW[2] * nrows + 16
+    achieved = alg_bytes / scan_ms / 1e6
+    traffic = None
+    tpath = os.path.join(ROOT, "profiles", "traffic.json")   # dram bytes per launch from the committed ncu capture
+    if os.path.exists(tpath):
+        with open(tpath) as f:
+            traffic = json.load(f).get("c2_scan_dram_bytes_per_launch")
+    roofline = dict(bound="hbm", kernel="gq_scan (C2 fused filter+project+global aggregate)", achieved=achieved,
+                    peak=peak, unit="GB/s", frac=achieved / peak, traffic=traffic, peak_source=peak_src,
+                    algorithmic_bytes_per_launch=alg_bytes, kernel_ms=scan_ms, frac_of_nominal_8000=achieved / 8000.0,
+                    read_probe_gbs=(1 << 30) / probe_ms / 1e6)
+
+    # ---------------- end to end: HOST buffers through the C ABI ----------------
+    e2e = None
+    if rank == 0 or ws > 1:
+        hcols = [torch.from_numpy(np.ascontiguousarray(c)).pin_memory() for c in plan["table"]]
+        hp = gqrun.prepare(ctx, plan, [], cols=hcols)
+        hp.run_host(); hp.run_host()
+        k = max(3, min(args.steps, 5))
+        t0 = time.perf_counter()
+        for _ in range(k):
+            hp.run_host()
+        e2e_ms = (time.perf_counter() - t0) / k * 1e3     # run_host returns after the results landed on the host
+        r = hp.result()
+        if exp is not None:
+            parity = parity and all(int(a[0]) == int(e[0]) for a, e in zip(r["aggs"], exp.cols))
+        e2e = dict(value=ws * nrows / e2e_ms * 1e3, unit="rows/s", h2d_bytes_per_step=int(sum(c.nbytes for c in plan["table"])),
+                   d2h_bytes_per_step=8 * (1 + len(plan["aggs"])), ms_per_step=e2e_ms,
+                   how="gq_pipeline_host: pinned host columns, 8 Mi-row chunks, H2D overlapped with the scan")
+        del hcols, hp
+
+    # ---------------- other configs (device-resident), rank 0 of a 1-GPU run only ----------------
+    per_config = {}
+    if ws == 1 and args.configs:
+        del cols, pipe, st, probe_t
+        torch.cuda.empty_cache()
+        for cfg in [int(x) for x in args.configs.split(",") if x]:
+            try:
+                sc = args.c5_scale if cfg == 5 else 1.0
+                out, _, _ = run_config(cfg, gq, ctx, torch, datagen, plans, gqrun, max(5, args.steps // 2), 3, scale=sc, peak=peak)
+                per_config[f"C{cfg}"] = out
+            except Exception as e:  # a failing extra config must not hide the headline number
+                per_config[f"C{cfg}"] = dict(error=str(e)[:300])
+            torch.cuda.empty_cache()
+
+    # ---------------- CPU baseline: the oracle on this box's host cores ----------------
+    cpu = None
+    if rank == 0 and not args.no_cpu_baseline:
+        rate, n, dt = oracle_rate(plans, datagen, 2, 60_000_000, reps=3)
+        cpu = dict(value=rate, unit="rows/s", cores=1, kind="oracle", sample=f"all {n} rows of C2, best of 3 ({dt:.2f} s each)",
+                   host_cores=os.cpu_count())
+    if rank == 0:
+        line = dict(metric=METRIC, value=value, unit="rows/s", n_gpus=ws, steps=args.steps, warmup=args.warmup,
+                    ms_per_step=ms_per_step, higher_is_better=True, scaling="weak", vs_baseline=None, dtype="int64",
+                    data="synthetic",
+                    config=dict(workload="C2 selective filter + global SUM(price*discount), 60M-row fact (BASELINE configs[1])",
+                                rows=nrows, l2="inputs (1.68 GB) larger than L2 (126 MB): every iteration reads HBM",
+                                parallelism="replicas only" if ws > 1 else "1 GPU", parity_vs_oracle=parity),
+                    roofline=roofline, cpu_baseline=cpu, e2e=e2e, gpu_launches=launches_per_step * args.steps,
+                    launches_per_step=launches_per_step, clocks=clocks, per_config=per_config)
+        print(json.dumps(line))
+    if ws > 1:
+        td.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

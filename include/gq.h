@@ -1,0 +1,198 @@
+/* gq.h — C ABI of the B200-native columnar query hot path (libgq.so).
+ *
+ * Scope (BASELINE.json north_star): the work the paper's cuDF operators do once data is in GPU
+ * memory — FilterProject -> HashBuild/HashProbe (inner equi-join) -> HashAggregation over device-resident column
+ * batches ("Accelerating Presto with GPUs", §3.2; operator model lines 112-116, 122-127).
+ *
+ * Model, as the paper states it:
+ *   - operators consume BATCHES of rows held as columns in device memory, together with the CUDA stream that orders
+ *     work on them (CudfVector = table + stream); a call only ENQUEUES work on the context's stream and
+ *     returns — "GPU operators return immediately ... without blocking";
+ *   - HashBuild consumes its whole input before HashProbe starts; streams are synchronised only at such pipeline
+ *     boundaries;
+ *   - HashAggregation accumulates over many input batches, then emits; here the state is a true
+ *     streaming hash table (no concatenate-and-reaggregate work-around);
+ *   - expressions are compiled at plan-creation time into fused code: every distinct plan shape
+ *     is translated once into one fused sm_100a kernel (filter + probes + projection + consumer), cached by shape;
+ *   - running out of (table) memory is an error, never a spill or a silent partial result.
+ *
+ * Conventions
+ *   Pointers   : every `data`, output column, workspace and count pointer is a DEVICE pointer unless its name starts
+ *                with `h_` or the doc says HOST. Descriptor structs and the arrays they point to are HOST memory and
+ *                are read during the call only.
+ *   Ownership  : the caller owns all columns, outputs and workspaces and must keep them alive until the enqueued work
+ *                has completed on the context's stream. The library owns only small host handles and the context's
+ *                few hundred bytes of device scratch. No call allocates or frees device memory after gq_create.
+ *   Alignment  : column and output pointers 16-byte aligned; workspaces 256-byte aligned.
+ *   Types      : signed int8 / int32 / int64 columns, no NULLs, no strings, no floating point input.
+ *                All arithmetic is wrapping two's-complement int64; aggregates and COUNT are int64.
+ *   Order      : row order of multi-row outputs and group order are unspecified (SQL gives none); top-k output is
+ *                ordered (aggregate descending, key ascending).
+ *   Errors     : host-detectable problems return at once with nothing enqueued. Device-detected problems (table or
+ *                output capacity exceeded, duplicate key under GQ_F_UNIQUE_KEYS) set a sticky flag in device memory;
+ *                later kernels of that context become no-ops; gq_sync() returns the code.
+ *   Threads    : one context = one stream; distinct contexts may be used concurrently (Fig. 3).
+ */
+#ifndef GQ_H
+#define GQ_H
+#include <stddef.h>
+#include <stdint.h>
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef enum {
+  GQ_OK = 0,
+  GQ_ERR_INVALID_ARG = 1,          /* null pointer, bad dtype/index, misaligned pointer, malformed expression */
+  GQ_ERR_UNSUPPORTED = 2,          /* valid request outside the implemented envelope (limits below) */
+  GQ_ERR_CAPACITY = 3,             /* hash table / output buffer full (device-detected, sticky) */
+  GQ_ERR_WORKSPACE_TOO_SMALL = 4,
+  GQ_ERR_CUDA = 5,                 /* CUDA runtime error: see gq_last_cuda_error */
+  GQ_ERR_DUPLICATE_KEY = 6,        /* GQ_F_UNIQUE_KEYS asserted but a duplicate build key was seen (sticky) */
+  GQ_ERR_COMPILE = 7               /* plan-time kernel compilation failed: see gq_last_message */
+} gq_status;
+
+typedef enum { GQ_I8 = 1, GQ_I32 = 2, GQ_I64 = 3 } gq_dtype;
+typedef struct { const void* data; gq_dtype dtype; } gq_column;                 /* DEVICE pointer, borrowed */
+typedef struct { const gq_column* cols; int32_t ncols; int64_t nrows; } gq_batch; /* one batch of rows (SoA) */
+
+/* Filter = AND of predicates `col <op> const` on INPUT columns; npred == 0 => every row passes. One-sided
+ * operators compare with `lo`. */
+typedef enum { GQ_LT = 0, GQ_LE, GQ_GT, GQ_GE, GQ_EQ, GQ_NE, GQ_RANGE_CO /* lo<=x<hi */, GQ_RANGE_CC /* lo<=x<=hi */ } gq_cmp;
+typedef struct { int32_t col; gq_cmp op; int64_t lo, hi; } gq_pred;
+
+/* Projection = postfix program over the row's columns; int64 wrapping + - *. `arg` = column index for GQ_X_COL,
+ * literal for GQ_X_CONST. Column indices >= batch.ncols name payload columns appended by probe steps, in order. */
+typedef enum { GQ_X_COL = 0, GQ_X_CONST, GQ_X_ADD, GQ_X_SUB, GQ_X_MUL } gq_xop;
+typedef struct { gq_xop op; int64_t arg; } gq_xtok;
+typedef struct { const gq_xtok* toks; int32_t ntoks; } gq_expr;
+
+typedef enum { GQ_SUM = 0, GQ_MIN, GQ_MAX, GQ_COUNT_STAR } gq_aggop;
+typedef struct { gq_aggop op; int32_t expr; /* index into exprs[]; ignored for COUNT_STAR */ } gq_agg;
+
+enum { GQ_F_UNIQUE_KEYS = 1u << 0 };  /* caller asserts unique build keys; VERIFIED on device, never trusted */
+enum { GQ_MAX_PREDS = 16, GQ_MAX_TOKS = 32, GQ_MAX_EXPRS = 8, GQ_MAX_AGGS = 8, GQ_MAX_PROBES = 4, GQ_MAX_PAYLOAD = 3,
+       GQ_MAX_KEYS = 2, GQ_MAX_COLS = 32, GQ_MAX_TOPK = 32, GQ_SIDE_SLOTS = 64 };
+
+typedef struct gq_ctx gq_ctx;           /* device + stream + sticky error */
+typedef struct gq_table gq_table;       /* join hash table (host handle; storage in caller's workspace) */
+typedef struct gq_aggstate gq_aggstate; /* group-by hash table (host handle; storage in caller's workspace) */
+
+/* ---- context ------------------------------------------------------------------------------------------------- */
+/* cuda_stream: a cudaStream_t (e.g. torch.cuda.current_stream().cuda_stream), 0 = legacy default stream. */
+gq_status gq_create(gq_ctx** out, int device, void* cuda_stream);
+gq_status gq_destroy(gq_ctx*);
+/* Blocks the HOST until the stream is idle (the pipeline boundary); returns the sticky device error. */
+gq_status gq_sync(gq_ctx*);
+/* Clears the sticky device error (enqueued on the stream). */
+gq_status gq_clear_error(gq_ctx*);
+const char* gq_status_str(gq_status);
+int gq_last_cuda_error(gq_ctx*);                 /* last cudaError_t seen by this context */
+const char* gq_last_message(gq_ctx*);            /* HOST string: last validation / compile diagnostic */
+/* Number of kernels this context has launched since creation (bench.py's gpu_launches). */
+int64_t gq_launch_count(gq_ctx*);
+
+/* ---- FilterProject, standalone and materialising ----------------------- */
+/* out_cols[e] : int64 column for expression e, capacity >= in->nrows. *d_out_count (DEVICE int64) += rows written,
+ * so the caller zeroes it before the first batch. Output row order unspecified. */
+gq_status gq_filter_project(gq_ctx*, const gq_batch* in, const gq_pred* preds, int32_t npred,
+                            const gq_expr* exprs, int32_t nexpr, int64_t* const* out_cols, int64_t out_capacity,
+                            int64_t* d_out_count);
+
+/* ---- HashBuild ------------------------------------------------------------ */
+typedef struct { const gq_table* table; int32_t key_col; } gq_probe_step;  /* key_col may name an earlier payload */
+typedef struct {
+  const gq_pred* preds; int32_t npred;
+  const gq_probe_step* probes; int32_t nprobes;  /* chained joins: rows must match these tables before insertion */
+  int32_t key_col;                               /* int64-widened key column (may be a payload of a probe step) */
+  const int32_t* payload_cols; int32_t npayload; /* stored beside the key, handed to probers */
+  uint32_t flags;                                /* GQ_F_UNIQUE_KEYS */
+} gq_build_desc;
+/* Open addressing, linear probing, 64-bit CAS; capacity = 2^ceil(log2(max_build_rows * 4/3)) slots. */
+gq_status gq_hash_build_workspace(int64_t max_build_rows, int32_t npayload, size_t* bytes);
+/* *table == NULL: creates the table in d_workspace (enqueues its initialisation) and inserts the batch.
+ * *table != NULL: inserts a further batch (same schema and desc; d_workspace/bytes/max_build_rows ignored). */
+gq_status gq_hash_build(gq_ctx*, gq_table** table, void* d_workspace, size_t bytes, int64_t max_build_rows,
+                        const gq_batch* in, const gq_build_desc* desc);
+/* "noMoreInput": records an event on the building stream; probing contexts on OTHER streams wait on it (the
+ * cross-pipeline synchronisation of PAPER.md:123). No host synchronisation. */
+gq_status gq_hash_build_finish(gq_ctx*, gq_table*);
+/* *d_count (DEVICE int64) = rows inserted so far (enqueued copy). */
+gq_status gq_table_count(gq_ctx*, const gq_table*, int64_t* d_count);
+gq_status gq_table_destroy(gq_table*);           /* frees the host handle; the workspace stays the caller's */
+
+/* ---- HashProbe, standalone and materialising inner join -------------------------- */
+/* Output row = exprs (int64 each) over [probe columns ++ payloads of the probed tables]; every matching pair is
+ * emitted (multiset semantics); unmatched probe rows are dropped. *d_out_count += rows written. */
+gq_status gq_hash_probe(gq_ctx*, const gq_batch* probe, const gq_pred* preds, int32_t npred,
+                        const gq_probe_step* probes, int32_t nprobes, const gq_expr* exprs, int32_t nexpr,
+                        int64_t* const* out_cols, int64_t out_capacity, int64_t* d_out_count);
+
+/* ---- HashAggregation, mode Single, streaming --------------------------------- */
+typedef struct {
+  const gq_pred* preds; int32_t npred;
+  const gq_probe_step* probes; int32_t nprobes;
+  const gq_expr* exprs; int32_t nexpr;
+  const int32_t* key_cols; int32_t nkeys;        /* 0 = one global group; <= GQ_MAX_KEYS */
+  int32_t ndependent;  /* trailing key columns functionally dependent on the leading ones: stored, not hashed.
+                          Needed when the packed key tuple is wider than 64 bits. */
+  const gq_agg* aggs; int32_t naggs;
+  int64_t max_groups;  /* capacity bound; also selects the low-cardinality shared-memory path when small */
+} gq_agg_desc;
+gq_status gq_hash_aggregate_workspace(int64_t max_groups, int32_t nkeys, int32_t naggs, size_t* bytes);
+/* *state == NULL: creates the state in d_workspace and aggregates the batch; else aggregates a further batch. */
+gq_status gq_hash_aggregate(gq_ctx*, gq_aggstate** state, void* d_workspace, size_t bytes, const gq_batch* in,
+                            const gq_agg_desc* desc);
+/* AVG derived in the finaliser: out = (double)agg[sum_agg] / (double)agg[count_agg] (IEEE-754 binary64). */
+typedef struct { int32_t sum_agg; int32_t count_agg; } gq_avg;
+/* Emits dense groups. out_key_cols[k] has the dtype of key column k; out_agg_cols[a] int64; out_avg_cols[j] double.
+ * topk == 0: all groups, order unspecified, *d_out_ngroups = group count (capacity exceeded => GQ_ERR_CAPACITY).
+ * topk  > 0: the topk groups with the largest aggregate `topk_agg`, ordered (aggregate desc, key tuple asc).
+ * d_topk_scratch: gq_topk_scratch_bytes() bytes, needed only when topk > 0. */
+size_t gq_topk_scratch_bytes(void);
+gq_status gq_hash_aggregate_finish(gq_ctx*, gq_aggstate*, void* const* out_key_cols, int64_t* const* out_agg_cols,
+                                   const gq_avg* avgs, int32_t navg, double* const* out_avg_cols,
+                                   int64_t out_capacity, int32_t topk, int32_t topk_agg, void* d_topk_scratch,
+                                   int64_t* d_out_ngroups);
+gq_status gq_aggstate_destroy(gq_aggstate*);
+
+/* ---- Fused pipeline: scan -> filter -> probe t1..tk -> project -> aggregate -> finalise ------- */
+typedef struct {
+  const gq_batch* in; gq_agg_desc agg;
+  const gq_avg* avgs; int32_t navg;
+  int32_t topk; int32_t topk_agg;
+} gq_plan;
+gq_status gq_pipeline_workspace(const gq_plan*, size_t* bytes);
+/* One stream-ordered pass, no host synchronisation inside: state init, fused scan kernel, finaliser. */
+gq_status gq_pipeline(gq_ctx*, const gq_plan*, void* d_workspace, size_t bytes, void* const* out_key_cols,
+                      int64_t* const* out_agg_cols, double* const* out_avg_cols, int64_t out_capacity,
+                      int64_t* d_out_ngroups);
+/* End-to-end variant with HOST input columns (plan->in->cols[].data are HOST pointers, pinned for full overlap):
+ * the batch is cut into chunks of chunk_rows, each copied host->device into a double-buffered staging area inside
+ * d_workspace while the previous chunk is aggregated (streaming of batches); results are copied back
+ * into HOST output buffers and the call returns after they have landed. Probed tables stay device-resident. */
+gq_status gq_pipeline_host_workspace(const gq_plan*, int64_t chunk_rows, size_t* bytes);
+gq_status gq_pipeline_host(gq_ctx*, const gq_plan*, int64_t chunk_rows, void* d_workspace, size_t bytes,
+                           void* const* h_out_key_cols, int64_t* const* h_out_agg_cols, double* const* h_out_avg_cols,
+                           int64_t out_capacity, int64_t* h_out_ngroups);
+
+/* ---- plan-time compilation ------------------------------------------------------------------------------------ */
+/* Directory of the on-disk kernel cache (<hash>.cubin + <hash>.cu); default: $GQ_KERNEL_CACHE or ./_kcache beside
+ * libgq.so. Plans are compiled on first use; these calls let a build step do it ahead of time, without a GPU. */
+gq_status gq_set_kernel_cache_dir(const char* h_path);
+/* Compiles (or finds in the cache) the fused kernel for the plan shape; needs no GPU. tables in probe steps may be
+ * described by handles created with gq_table_describe (no device memory). */
+gq_status gq_precompile_pipeline(const gq_plan*, char* h_msg, size_t msg_bytes);
+gq_status gq_precompile_build(const gq_batch* in, const gq_build_desc*, char* h_msg, size_t msg_bytes);
+/* Host-only table handle carrying just the schema (payload dtypes, flags) for precompilation. */
+gq_status gq_table_describe(gq_table** out, const gq_dtype* payload_dtypes, int32_t npayload, uint32_t flags);
+
+/* ---- measurement helper ---------------------------------------------------------------------------------------- */
+/* Read-only streaming sum over `bytes` bytes (16-byte aligned, multiple of 16): the practical read roofline probe of
+ * SURVEY §7.1 step 5. *d_out (DEVICE uint64) receives the wrapping sum of the 64-bit words. */
+gq_status gq_read_probe(gq_ctx*, const void* d_data, size_t bytes, uint64_t* d_out);
+
+#ifdef __cplusplus
+}
+#endif
+#endif

@@ -1,0 +1,738 @@
+// gq_api.cpp — the C ABI of include/gq.h: argument validation, workspace layout, plan normalisation, launches.
+// Every entry point only enqueues work on the context's stream — no device allocation, no host sync —
+// except gq_create/gq_destroy/gq_sync and the HOST-buffer end-to-end call gq_pipeline_host.
+#include <algorithm>
+#include <cstdio>
+#include <cstring>
+#include <map>
+#include <mutex>
+#include <sstream>
+
+#include "gq_internal.h"
+
+namespace {
+
+inline size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
+inline bool aligned(const void* p, size_t a) { return ((uintptr_t)p % a) == 0; }
+inline bool dtype_ok(int t) { return t == GQ_I8 || t == GQ_I32 || t == GQ_I64; }
+
+gq_status fail(gq_ctx* ctx, gq_status st, const std::string& m) { if (ctx) ctx->msg = m; return st; }
+gq_status cuda_fail(gq_ctx* ctx, cudaError_t e, const char* where) {
+  if (ctx) { ctx->last_cuda = (int)e; ctx->msg = std::string(where) + ": " + cudaGetErrorString(e); }
+  return GQ_ERR_CUDA;
+}
+
+int64_t table_capacity(int64_t max_rows) {   // power of two >= max_rows * 4/3, at least 1024 (load factor <= 0.75)
+  int64_t need = std::max<int64_t>(1024, max_rows + (max_rows + 2) / 3);
+  int64_t c = 1024;
+  while (c < need) c <<= 1;
+  return c;
+}
+int join_slot_words(int npayload) { return npayload == 0 ? 1 : (int)align_up((size_t)(1 + npayload), 2); }
+int agg_slot_words(int ndep, int naggs) { return (int)align_up((size_t)(1 + ndep + naggs), 2); }
+int log2i(int64_t v) { int l = 0; while ((1LL << l) < v) ++l; return l; }
+
+// workspace = [header 256 B][side area][slots]
+struct WsLayout { size_t side_off, slots_off, total; };
+WsLayout ws_layout(int64_t capacity, int slot_words, int nside) {
+  WsLayout w;
+  w.side_off = 256;
+  w.slots_off = 256 + align_up((size_t)nside * slot_words * 8, 256);
+  w.total = w.slots_off + (size_t)capacity * slot_words * 8;
+  return w;
+}
+
+gq_status check_batch(gq_ctx* ctx, const gq_batch* b) {
+  if (!b || b->ncols < 0 || b->ncols > GQ_MAX_COLS || b->nrows < 0 || (b->ncols > 0 && !b->cols))
+    return fail(ctx, GQ_ERR_INVALID_ARG, "bad batch");
+  for (int c = 0; c < b->ncols; ++c) {
+    if (!dtype_ok(b->cols[c].dtype)) return fail(ctx, GQ_ERR_INVALID_ARG, "bad column dtype");
+    if (b->nrows > 0 && (!b->cols[c].data || !aligned(b->cols[c].data, 16)))
+      return fail(ctx, GQ_ERR_INVALID_ARG, "column pointer null or not 16-byte aligned");
+  }
+  return GQ_OK;
+}
+
+// dtype of row column c (input column or payload of an earlier probe step)
+gq_dtype row_dtype(const GqScanSpec& sp, int c) {
+  int n = (int)sp.in_dtype.size();
+  if (c < n) return sp.in_dtype[(size_t)c];
+  c -= n;
+  for (const GqProbeSpec& p : sp.probes) { if (c < p.npayload) return p.pay_dtype[c]; c -= p.npayload; }
+  return GQ_I64;
+}
+int row_width(const GqScanSpec& sp) {
+  int n = (int)sp.in_dtype.size();
+  for (const GqProbeSpec& p : sp.probes) n += p.npayload;
+  return n;
+}
+
+gq_status fill_common(gq_ctx* ctx, GqScanSpec* sp, const gq_batch* in, const gq_pred* preds, int npred,
+                      const gq_probe_step* probes, int nprobes, const gq_expr* exprs, int nexpr) {
+  if (npred < 0 || npred > GQ_MAX_PREDS || (npred > 0 && !preds)) return fail(ctx, GQ_ERR_INVALID_ARG, "bad predicates");
+  if (nprobes < 0 || nprobes > GQ_MAX_PROBES || (nprobes > 0 && !probes)) return fail(ctx, GQ_ERR_INVALID_ARG, "bad probe steps");
+  if (nexpr < 0 || nexpr > GQ_MAX_EXPRS || (nexpr > 0 && !exprs)) return fail(ctx, GQ_ERR_INVALID_ARG, "bad expressions");
+  sp->in_dtype.clear();
+  for (int c = 0; c < in->ncols; ++c) sp->in_dtype.push_back(in->cols[c].dtype);
+  sp->preds.assign(preds, preds + npred);
+  for (const gq_pred& p : sp->preds)
+    if (p.col < 0 || p.col >= in->ncols || (int)p.op < 0 || (int)p.op > (int)GQ_RANGE_CC)
+      return fail(ctx, GQ_ERR_INVALID_ARG, "predicate column/op out of range");
+  sp->probes.clear();
+  for (int s = 0; s < nprobes; ++s) {
+    const gq_table* t = probes[s].table;
+    if (!t) return fail(ctx, GQ_ERR_INVALID_ARG, "null table in probe step");
+    GqProbeSpec ps;
+    ps.key_col = probes[s].key_col;
+    ps.npayload = t->npayload;
+    for (int p = 0; p < GQ_MAX_PAYLOAD; ++p) ps.pay_dtype[p] = t->payload_dtype[p];
+    ps.unique = (t->flags & GQ_F_UNIQUE_KEYS) != 0;
+    ps.slot_words = join_slot_words(t->npayload);
+    if (ps.key_col < 0 || ps.key_col >= row_width(*sp)) return fail(ctx, GQ_ERR_INVALID_ARG, "probe key column out of range");
+    sp->probes.push_back(ps);
+  }
+  sp->exprs.clear();
+  for (int e = 0; e < nexpr; ++e) {
+    if (!exprs[e].toks || exprs[e].ntoks < 1 || exprs[e].ntoks > GQ_MAX_TOKS) return fail(ctx, GQ_ERR_INVALID_ARG, "bad expression");
+    sp->exprs.emplace_back(exprs[e].toks, exprs[e].toks + exprs[e].ntoks);
+  }
+  sp->nrows_hint = in->nrows;
+  return GQ_OK;
+}
+
+// Shape signature (no constant values) and the constants in codegen order (predicates, then expression literals).
+int tile_bucket(int64_t nrows) { return nrows <= 0 ? 0 : nrows < 148LL * 8 * 512 * 2 ? 1 : nrows < 148LL * 8 * 512 * 4 ? 2 : 3; }
+std::string signature(const GqScanSpec& sp) {
+  std::string s;
+  s.reserve(256);
+  auto put = [&s](long long v) { s += std::to_string(v); s += ','; };
+  put(sp.consumer); put(tile_bucket(sp.nrows_hint));
+  for (gq_dtype t : sp.in_dtype) put(t);
+  s += 'p';
+  for (const gq_pred& p : sp.preds) { put(p.col); put(p.op); }
+  s += 'j';
+  for (const GqProbeSpec& p : sp.probes) { put(p.key_col); put(p.npayload); put(p.unique); for (int i = 0; i < p.npayload; ++i) put(p.pay_dtype[i]); }
+  s += 'e';
+  for (const auto& e : sp.exprs) { for (const gq_xtok& t : e) { put(t.op); if (t.op == GQ_X_COL) put(t.arg); } s += ';'; }
+  s += 'k';
+  for (int c : sp.key_cols) put(c);
+  put(sp.ndep);
+  for (const gq_agg& a : sp.aggs) { put(a.op); put(a.expr); }
+  put(sp.lc_cap); put(sp.target_sw); put(sp.build_key_col);
+  for (int c : sp.payload_cols) put(c);
+  put(sp.unique);
+  return s;
+}
+void collect_consts(const GqScanSpec& sp, std::vector<long long>* k) {
+  k->clear();
+  for (const gq_pred& p : sp.preds) { k->push_back(p.lo); if (p.op == GQ_RANGE_CO || p.op == GQ_RANGE_CC) k->push_back(p.hi); }
+  for (const auto& e : sp.exprs) for (const gq_xtok& t : e) if (t.op == GQ_X_CONST) k->push_back(t.arg);
+}
+
+struct CachedKernel { GqKernelInfo info; GqKernel k; bool loaded = false; };
+std::mutex g_kmu;
+std::map<std::string, CachedKernel> g_kernels;
+
+// Normalise the tiling hint so that every nrows in a bucket produces the same source.
+void canon_hint(GqScanSpec* sp) {
+  static const int64_t rep[4] = {0, 148LL * 8 * 512, 148LL * 8 * 512 * 3, 0};
+  sp->nrows_hint = rep[tile_bucket(sp->nrows_hint)];
+}
+
+gq_status get_kernel_info(const GqScanSpec& sp_in, CachedKernel** out, std::string* msg) {
+  GqScanSpec sp = sp_in;
+  canon_hint(&sp);
+  std::string sig = signature(sp);
+  std::lock_guard<std::mutex> l(g_kmu);
+  auto it = g_kernels.find(sig);
+  if (it == g_kernels.end()) {
+    CachedKernel ck;
+    gq_status st = gq_codegen(sp, &ck.info, msg);
+    if (st != GQ_OK) return st;
+    std::vector<long long> k;
+    collect_consts(sp, &k);
+    if (k != ck.info.consts) { if (msg) *msg = "internal: constant order mismatch"; return GQ_ERR_COMPILE; }
+    it = g_kernels.emplace(sig, std::move(ck)).first;
+  }
+  *out = &it->second;
+  return GQ_OK;
+}
+
+// Codegen (cached) -> JIT (cached) -> parameters -> launch of one fused scan kernel.
+gq_status run_scan(gq_ctx* ctx, const GqScanSpec& sp, const gq_batch* in, const gq_probe_step* probes,
+                   GqParams* P /* target/acc/out/out_count pre-filled */) {
+  CachedKernel* ck = nullptr;
+  gq_status st = get_kernel_info(sp, &ck, &ctx->msg);
+  if (st != GQ_OK) return st;
+  if (!ck->loaded) {
+    st = gq_jit_get(ck->info, &ck->k, &ctx->msg, &ctx->last_cuda);
+    if (st != GQ_OK) return st;
+    ck->loaded = true;
+  }
+  for (size_t c = 0; c < ck->info.cols.size(); ++c) P->col[c] = in->cols[ck->info.cols[c]].data;
+  P->nrows = in->nrows;
+  std::vector<long long> k;
+  collect_consts(sp, &k);
+  for (size_t i = 0; i < k.size(); ++i) P->k[i] = k[i];
+  for (size_t s = 0; s < sp.probes.size(); ++s) {
+    const gq_table* t = probes[s].table;
+    if (t->describe_only) return fail(ctx, GQ_ERR_INVALID_ARG, "probe step names a describe-only table");
+    P->probe[s] = t->dev;
+    if (t->finished && t->build_stream != ctx->stream) {   // cross-pipeline boundary
+      cudaError_t e = cudaStreamWaitEvent(ctx->stream, t->ready, 0);
+      if (e != cudaSuccess) return cuda_fail(ctx, e, "cudaStreamWaitEvent");
+    }
+  }
+  P->err = ctx->d_err;
+  if (in->nrows == 0) return GQ_OK;   // empty batches are legal no-ops (S9)
+  const int64_t ntiles = in->nrows / ck->k.tile_rows;
+  int grid = (int)std::max<int64_t>(1, std::min<int64_t>(ctx->num_sms, ntiles));
+  void* args[] = {(void*)P};
+  cudaError_t e = cudaLaunchKernel((const void*)ck->k.fn, dim3((unsigned)grid), dim3((unsigned)ck->k.threads), args,
+                                   (size_t)ck->k.smem_bytes, ctx->stream);
+  if (e != cudaSuccess) return cuda_fail(ctx, e, "launch of fused scan kernel");
+  ++ctx->launches;
+  return GQ_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+// ------------------------------------------------------------------------------------------------ context
+gq_status gq_create(gq_ctx** out, int device, void* cuda_stream) {
+  if (!out) return GQ_ERR_INVALID_ARG;
+  *out = nullptr;
+  cudaError_t e = cudaSetDevice(device);
+  if (e != cudaSuccess) return GQ_ERR_CUDA;
+  gq_ctx* c = new gq_ctx();
+  c->device = device;
+  c->stream = (cudaStream_t)cuda_stream;
+  int sms = 0;
+  if (cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, device) == cudaSuccess && sms > 0) c->num_sms = sms;
+  e = cudaMalloc((void**)&c->d_err, 256);
+  if (e == cudaSuccess) e = cudaMemset(c->d_err, 0, 256);
+  if (e == cudaSuccess) e = cudaMallocHost((void**)&c->h_err, 256);
+  if (e != cudaSuccess) { if (c->d_err) cudaFree(c->d_err); delete c; return GQ_ERR_CUDA; }
+  *c->h_err = 0;
+  *out = c;
+  return GQ_OK;
+}
+
+gq_status gq_destroy(gq_ctx* c) {
+  if (!c) return GQ_ERR_INVALID_ARG;
+  cudaFree(c->d_err);
+  cudaFreeHost(c->h_err);
+  if (c->copy_stream) cudaStreamDestroy(c->copy_stream);
+  for (int i = 0; i < 2; ++i) { if (c->ev_copied[i]) cudaEventDestroy(c->ev_copied[i]); if (c->ev_consumed[i]) cudaEventDestroy(c->ev_consumed[i]); }
+  delete c;
+  return GQ_OK;
+}
+
+gq_status gq_sync(gq_ctx* c) {
+  if (!c) return GQ_ERR_INVALID_ARG;
+  cudaError_t e = cudaMemcpyAsync(c->h_err, c->d_err, sizeof(int), cudaMemcpyDeviceToHost, c->stream);
+  if (e == cudaSuccess) e = cudaStreamSynchronize(c->stream);
+  if (e != cudaSuccess) return cuda_fail(c, e, "gq_sync");
+  int code = *c->h_err;
+  if (code == 0) return GQ_OK;
+  c->msg = code == GQ_ERR_CAPACITY ? "device: hash table or output capacity exceeded"
+         : code == GQ_ERR_DUPLICATE_KEY ? "device: duplicate build key under GQ_F_UNIQUE_KEYS" : "device error";
+  return (gq_status)code;
+}
+
+gq_status gq_clear_error(gq_ctx* c) {
+  if (!c) return GQ_ERR_INVALID_ARG;
+  cudaError_t e = cudaMemsetAsync(c->d_err, 0, sizeof(int), c->stream);
+  return e == cudaSuccess ? GQ_OK : cuda_fail(c, e, "gq_clear_error");
+}
+
+const char* gq_status_str(gq_status s) {
+  switch (s) {
+    case GQ_OK: return "GQ_OK";
+    case GQ_ERR_INVALID_ARG: return "GQ_ERR_INVALID_ARG";
+    case GQ_ERR_UNSUPPORTED: return "GQ_ERR_UNSUPPORTED";
+    case GQ_ERR_CAPACITY: return "GQ_ERR_CAPACITY";
+    case GQ_ERR_WORKSPACE_TOO_SMALL: return "GQ_ERR_WORKSPACE_TOO_SMALL";
+    case GQ_ERR_CUDA: return "GQ_ERR_CUDA";
+    case GQ_ERR_DUPLICATE_KEY: return "GQ_ERR_DUPLICATE_KEY";
+    case GQ_ERR_COMPILE: return "GQ_ERR_COMPILE";
+  }
+  return "GQ_ERR_UNKNOWN";
+}
+int gq_last_cuda_error(gq_ctx* c) { return c ? c->last_cuda : 0; }
+const char* gq_last_message(gq_ctx* c) { return c ? c->msg.c_str() : ""; }
+int64_t gq_launch_count(gq_ctx* c) { return c ? c->launches : 0; }
+
+// ------------------------------------------------------------------------------------------------ FilterProject
+static gq_status materialise(gq_ctx* ctx, const gq_batch* in, const gq_pred* preds, int32_t npred,
+                             const gq_probe_step* probes, int32_t nprobes, const gq_expr* exprs, int32_t nexpr,
+                             int64_t* const* out_cols, int64_t out_capacity, int64_t* d_out_count) {
+  if (!ctx) return GQ_ERR_INVALID_ARG;
+  gq_status st = check_batch(ctx, in);
+  if (st != GQ_OK) return st;
+  if (nexpr < 1 || !out_cols || !d_out_count || out_capacity < 0) return fail(ctx, GQ_ERR_INVALID_ARG, "bad outputs");
+  GqScanSpec sp;
+  st = fill_common(ctx, &sp, in, preds, npred, probes, nprobes, exprs, nexpr);
+  if (st != GQ_OK) return st;
+  sp.consumer = GQ_C_MATERIALISE;
+  GqParams P;
+  memset(&P, 0, sizeof P);
+  for (int e = 0; e < nexpr; ++e) {
+    if (!out_cols[e] || !aligned(out_cols[e], 16)) return fail(ctx, GQ_ERR_INVALID_ARG, "output column null or misaligned");
+    P.out[e] = (long long*)out_cols[e];
+  }
+  P.out_capacity = out_capacity;
+  P.out_count = (long long*)d_out_count;
+  return run_scan(ctx, sp, in, probes, &P);
+}
+
+gq_status gq_filter_project(gq_ctx* ctx, const gq_batch* in, const gq_pred* preds, int32_t npred, const gq_expr* exprs,
+                            int32_t nexpr, int64_t* const* out_cols, int64_t out_capacity, int64_t* d_out_count) {
+  return materialise(ctx, in, preds, npred, nullptr, 0, exprs, nexpr, out_cols, out_capacity, d_out_count);
+}
+
+gq_status gq_hash_probe(gq_ctx* ctx, const gq_batch* probe, const gq_pred* preds, int32_t npred,
+                        const gq_probe_step* probes, int32_t nprobes, const gq_expr* exprs, int32_t nexpr,
+                        int64_t* const* out_cols, int64_t out_capacity, int64_t* d_out_count) {
+  if (nprobes < 1) return fail(ctx, GQ_ERR_INVALID_ARG, "gq_hash_probe needs at least one probe step");
+  return materialise(ctx, probe, preds, npred, probes, nprobes, exprs, nexpr, out_cols, out_capacity, d_out_count);
+}
+
+// ------------------------------------------------------------------------------------------------ HashBuild
+gq_status gq_hash_build_workspace(int64_t max_build_rows, int32_t npayload, size_t* bytes) {
+  if (!bytes || max_build_rows < 0 || npayload < 0 || npayload > GQ_MAX_PAYLOAD) return GQ_ERR_INVALID_ARG;
+  *bytes = ws_layout(table_capacity(max_build_rows), join_slot_words(npayload), GQ_SIDE_SLOTS).total;
+  return GQ_OK;
+}
+
+static gq_status build_spec(gq_ctx* ctx, GqScanSpec* sp, const gq_batch* in, const gq_build_desc* d) {
+  gq_status st = fill_common(ctx, sp, in, d->preds, d->npred, d->probes, d->nprobes, nullptr, 0);
+  if (st != GQ_OK) return st;
+  if (d->npayload < 0 || d->npayload > GQ_MAX_PAYLOAD || (d->npayload > 0 && !d->payload_cols))
+    return fail(ctx, GQ_ERR_INVALID_ARG, "bad payload columns");
+  const int w = row_width(*sp);
+  if (d->key_col < 0 || d->key_col >= w) return fail(ctx, GQ_ERR_INVALID_ARG, "build key column out of range");
+  sp->consumer = GQ_C_BUILD;
+  sp->build_key_col = d->key_col;
+  sp->payload_cols.assign(d->payload_cols, d->payload_cols + d->npayload);
+  for (int c : sp->payload_cols) if (c < 0 || c >= w) return fail(ctx, GQ_ERR_INVALID_ARG, "payload column out of range");
+  sp->unique = (d->flags & GQ_F_UNIQUE_KEYS) != 0;
+  sp->target_sw = join_slot_words(d->npayload);
+  return GQ_OK;
+}
+
+gq_status gq_hash_build(gq_ctx* ctx, gq_table** table, void* d_ws, size_t bytes, int64_t max_build_rows,
+                        const gq_batch* in, const gq_build_desc* d) {
+  if (!ctx || !table || !d) return GQ_ERR_INVALID_ARG;
+  gq_status st = check_batch(ctx, in);
+  if (st != GQ_OK) return st;
+  GqScanSpec sp;
+  st = build_spec(ctx, &sp, in, d);
+  if (st != GQ_OK) return st;
+  gq_table* t = *table;
+  if (!t) {
+    if (!d_ws || !aligned(d_ws, 256) || max_build_rows < 0) return fail(ctx, GQ_ERR_INVALID_ARG, "bad workspace");
+    const int64_t cap = table_capacity(max_build_rows);
+    const int sw = sp.target_sw;
+    WsLayout w = ws_layout(cap, sw, GQ_SIDE_SLOTS);
+    if (bytes < w.total) return fail(ctx, GQ_ERR_WORKSPACE_TOO_SMALL, "hash-build workspace too small");
+    t = new gq_table();
+    t->capacity = cap;
+    t->npayload = d->npayload;
+    for (int p = 0; p < d->npayload; ++p) t->payload_dtype[p] = row_dtype(sp, d->payload_cols[p]);
+    t->flags = d->flags;
+    t->max_rows = max_build_rows;
+    t->dev.slots = (unsigned long long*)((char*)d_ws + w.slots_off);
+    t->dev.mask = (unsigned long long)(cap - 1);
+    t->dev.header = (long long*)d_ws;
+    t->dev.side = (unsigned long long*)((char*)d_ws + w.side_off);
+    t->dev.shift = 64 - log2i(cap);
+    t->dev.slot_words = sw;
+    t->dev.flags = d->flags;
+    unsigned long long pat[12];
+    for (int i = 0; i < 12; ++i) pat[i] = 0;
+    pat[0] = GQ_EMPTY_KEY;
+    cudaError_t e = gq_launch_init_table(ctx->stream, t->dev.slots, cap, sw, pat, t->dev.side, GQ_SIDE_SLOTS, t->dev.header, 0);
+    if (e != cudaSuccess) { delete t; return cuda_fail(ctx, e, "table init"); }
+    ++ctx->launches;
+    { GqScanSpec c = sp; c.nrows_hint = 0; t->build_sig = signature(c); }
+    *table = t;
+  } else {
+    GqScanSpec c = sp; c.nrows_hint = 0;
+    if (t->describe_only || signature(c) != t->build_sig) return fail(ctx, GQ_ERR_INVALID_ARG, "batch schema/desc differs from the table's first batch");
+    if (t->finished) return fail(ctx, GQ_ERR_INVALID_ARG, "table already finished");
+  }
+  GqParams P;
+  memset(&P, 0, sizeof P);
+  P.target = t->dev;
+  return run_scan(ctx, sp, in, d->probes, &P);
+}
+
+gq_status gq_hash_build_finish(gq_ctx* ctx, gq_table* t) {
+  if (!ctx || !t || t->describe_only) return GQ_ERR_INVALID_ARG;
+  if (!t->ready) {
+    cudaError_t e = cudaEventCreateWithFlags(&t->ready, cudaEventDisableTiming);
+    if (e != cudaSuccess) return cuda_fail(ctx, e, "cudaEventCreate");
+  }
+  cudaError_t e = cudaEventRecord(t->ready, ctx->stream);
+  if (e != cudaSuccess) return cuda_fail(ctx, e, "cudaEventRecord");
+  t->build_stream = ctx->stream;
+  t->finished = true;
+  return GQ_OK;
+}
+
+gq_status gq_table_count(gq_ctx* ctx, const gq_table* t, int64_t* d_count) {
+  if (!ctx || !t || !d_count || t->describe_only) return GQ_ERR_INVALID_ARG;
+  cudaError_t e = cudaMemcpyAsync(d_count, t->dev.header, 8, cudaMemcpyDeviceToDevice, ctx->stream);
+  return e == cudaSuccess ? GQ_OK : cuda_fail(ctx, e, "gq_table_count");
+}
+
+gq_status gq_table_destroy(gq_table* t) {
+  if (!t) return GQ_ERR_INVALID_ARG;
+  if (t->ready) cudaEventDestroy(t->ready);
+  delete t;
+  return GQ_OK;
+}
+
+gq_status gq_table_describe(gq_table** out, const gq_dtype* payload_dtypes, int32_t npayload, uint32_t flags) {
+  if (!out || npayload < 0 || npayload > GQ_MAX_PAYLOAD || (npayload > 0 && !payload_dtypes)) return GQ_ERR_INVALID_ARG;
+  gq_table* t = new gq_table();
+  t->describe_only = true;
+  t->npayload = npayload;
+  for (int p = 0; p < npayload; ++p) { if (!dtype_ok(payload_dtypes[p])) { delete t; return GQ_ERR_INVALID_ARG; } t->payload_dtype[p] = payload_dtypes[p]; }
+  t->flags = flags;
+  *out = t;
+  return GQ_OK;
+}
+
+}  // extern "C"
+
+// ------------------------------------------------------------------------------------------------ HashAggregation
+namespace {
+
+// Shared-memory budget of the low-cardinality path: (lc_cap+1) * naggs * 256 threads * 8 B of private cells.
+int lowcard_cap(int64_t max_groups, int naggs, int ndep) {
+  if (ndep > 0 || max_groups < 1 || max_groups > 64 || naggs < 1) return 0;
+  int cap = 2;
+  while (cap < max_groups) cap <<= 1;
+  long long bytes = 8LL * (cap + 1) * naggs * 256;
+  return bytes <= 100 * 1024 ? cap : 0;
+}
+
+gq_status agg_spec(gq_ctx* ctx, GqScanSpec* sp, const gq_batch* in, const gq_agg_desc* d, int key_bits[2],
+                   gq_dtype key_dtype[2]) {
+  gq_status st = fill_common(ctx, sp, in, d->preds, d->npred, d->probes, d->nprobes, d->exprs, d->nexpr);
+  if (st != GQ_OK) return st;
+  if (d->nkeys < 0 || d->nkeys > GQ_MAX_KEYS || (d->nkeys > 0 && !d->key_cols)) return fail(ctx, GQ_ERR_INVALID_ARG, "bad key columns");
+  if (d->naggs < 1 || d->naggs > GQ_MAX_AGGS || !d->aggs) return fail(ctx, GQ_ERR_INVALID_ARG, "bad aggregates");
+  if (d->ndependent < 0 || (d->nkeys > 0 && d->ndependent >= d->nkeys) || (d->nkeys == 0 && d->ndependent != 0))
+    return fail(ctx, GQ_ERR_INVALID_ARG, "bad ndependent");
+  if (d->max_groups < 1) return fail(ctx, GQ_ERR_INVALID_ARG, "max_groups must be >= 1");
+  const int w = row_width(*sp);
+  sp->key_cols.assign(d->key_cols, d->key_cols + d->nkeys);
+  int bits = 0;
+  key_bits[0] = key_bits[1] = 0;
+  for (int k = 0; k < d->nkeys; ++k) {
+    if (sp->key_cols[(size_t)k] < 0 || sp->key_cols[(size_t)k] >= w) return fail(ctx, GQ_ERR_INVALID_ARG, "key column out of range");
+    key_dtype[k] = row_dtype(*sp, sp->key_cols[(size_t)k]);
+    if (k < d->nkeys - d->ndependent) { key_bits[k] = 8 * gq_dtype_bytes(key_dtype[k]); bits += key_bits[k]; }
+  }
+  if (bits > 64) return fail(ctx, GQ_ERR_UNSUPPORTED, "packed key wider than 64 bits: declare trailing keys dependent (ndependent)");
+  sp->ndep = d->ndependent;
+  sp->aggs.assign(d->aggs, d->aggs + d->naggs);
+  for (const gq_agg& a : sp->aggs) {
+    if ((int)a.op < 0 || (int)a.op > (int)GQ_COUNT_STAR) return fail(ctx, GQ_ERR_INVALID_ARG, "bad aggregate op");
+    if (a.op != GQ_COUNT_STAR && (a.expr < 0 || a.expr >= d->nexpr)) return fail(ctx, GQ_ERR_INVALID_ARG, "aggregate names a missing expression");
+  }
+  sp->target_sw = agg_slot_words(d->ndependent, d->naggs);
+  sp->lc_cap = d->nkeys > 0 ? lowcard_cap(d->max_groups, d->naggs, d->ndependent) : 0;
+  sp->consumer = d->nkeys == 0 ? GQ_C_GLOBAL : sp->lc_cap > 0 ? GQ_C_LOWCARD : GQ_C_HIGHCARD;
+  return GQ_OK;
+}
+
+int64_t agg_capacity(int64_t max_groups, int nkeys) { return nkeys == 0 ? 0 : table_capacity(max_groups); }
+
+}  // namespace
+
+extern "C" {
+
+gq_status gq_hash_aggregate_workspace(int64_t max_groups, int32_t nkeys, int32_t naggs, size_t* bytes) {
+  if (!bytes || max_groups < 1 || nkeys < 0 || nkeys > GQ_MAX_KEYS || naggs < 1 || naggs > GQ_MAX_AGGS) return GQ_ERR_INVALID_ARG;
+  // slot words do not depend on how many keys are dependent beyond +1 word: size for the worst case (1 dependent)
+  *bytes = ws_layout(agg_capacity(max_groups, nkeys), agg_slot_words(nkeys > 1 ? 1 : 0, naggs), 1).total;
+  return GQ_OK;
+}
+
+gq_status gq_hash_aggregate(gq_ctx* ctx, gq_aggstate** state, void* d_ws, size_t bytes, const gq_batch* in,
+                            const gq_agg_desc* d) {
+  if (!ctx || !state || !d) return GQ_ERR_INVALID_ARG;
+  gq_status st = check_batch(ctx, in);
+  if (st != GQ_OK) return st;
+  GqScanSpec sp;
+  int key_bits[2];
+  gq_dtype key_dtype[2] = {GQ_I64, GQ_I64};
+  st = agg_spec(ctx, &sp, in, d, key_bits, key_dtype);
+  if (st != GQ_OK) return st;
+  GqScanSpec sig_sp = sp; sig_sp.nrows_hint = 0;
+  gq_aggstate* a = *state;
+  if (!a) {
+    if (!d_ws || !aligned(d_ws, 256)) return fail(ctx, GQ_ERR_INVALID_ARG, "bad workspace");
+    const int64_t cap = agg_capacity(d->max_groups, d->nkeys);
+    const int sw = sp.target_sw;
+    WsLayout w = ws_layout(cap, sw, 1);
+    if (bytes < w.total) return fail(ctx, GQ_ERR_WORKSPACE_TOO_SMALL, "hash-aggregate workspace too small");
+    a = new gq_aggstate();
+    a->capacity = cap; a->nkeys = d->nkeys; a->ndep = d->ndependent; a->naggs = d->naggs; a->max_groups = d->max_groups;
+    for (int k = 0; k < d->nkeys; ++k) { a->key_dtype[k] = key_dtype[k]; a->key_bits[k] = key_bits[k]; }
+    for (int i = 0; i < d->naggs; ++i) a->agg_op[i] = d->aggs[i].op;
+    a->lowcard = sp.consumer == GQ_C_LOWCARD; a->lc_cap = sp.lc_cap;
+    a->dev.slots = (unsigned long long*)((char*)d_ws + w.slots_off);
+    a->dev.mask = cap > 0 ? (unsigned long long)(cap - 1) : 0;
+    a->dev.header = (long long*)d_ws;
+    a->dev.side = (unsigned long long*)((char*)d_ws + w.side_off);
+    a->dev.shift = cap > 0 ? 64 - log2i(cap) : 63;
+    a->dev.slot_words = sw;
+    unsigned long long pat[12];
+    for (int i = 0; i < 12; ++i) pat[i] = 0;
+    pat[0] = GQ_EMPTY_KEY;
+    for (int i = 0; i < d->naggs; ++i)
+      pat[1 + d->ndependent + i] = d->aggs[i].op == GQ_MIN ? 0x7FFFFFFFFFFFFFFFULL : d->aggs[i].op == GQ_MAX ? 0x8000000000000000ULL : 0ULL;
+    // a key-less aggregation has exactly one group, present even with no input rows (S9): header[1] = 1
+    cudaError_t e = gq_launch_init_table(ctx->stream, a->dev.slots, cap, sw, pat, a->dev.side, 1, a->dev.header, d->nkeys == 0 ? 1 : 0);
+    if (e != cudaSuccess) { delete a; return cuda_fail(ctx, e, "aggregate state init"); }
+    ++ctx->launches;
+    a->sig = signature(sig_sp);
+    *state = a;
+  } else if (signature(sig_sp) != a->sig) return fail(ctx, GQ_ERR_INVALID_ARG, "batch schema/desc differs from the state's first batch");
+  GqParams P;
+  memset(&P, 0, sizeof P);
+  P.target = a->dev;
+  P.acc = (long long*)(a->dev.side + 1);
+  return run_scan(ctx, sp, in, d->probes, &P);
+}
+
+size_t gq_topk_scratch_bytes(void) { return gq_topk_scratch_bytes_impl(); }
+
+gq_status gq_hash_aggregate_finish(gq_ctx* ctx, gq_aggstate* a, void* const* out_key_cols, int64_t* const* out_agg_cols,
+                                   const gq_avg* avgs, int32_t navg, double* const* out_avg_cols, int64_t out_capacity,
+                                   int32_t topk, int32_t topk_agg, void* d_topk_scratch, int64_t* d_out_ngroups) {
+  if (!ctx || !a || !out_agg_cols || !d_out_ngroups || out_capacity < 0) return GQ_ERR_INVALID_ARG;
+  if (a->nkeys > 0 && !out_key_cols) return fail(ctx, GQ_ERR_INVALID_ARG, "missing key outputs");
+  if (navg < 0 || navg > GQ_MAX_AGGS || (navg > 0 && (!avgs || !out_avg_cols))) return fail(ctx, GQ_ERR_INVALID_ARG, "bad avg spec");
+  if (topk < 0 || topk > GQ_MAX_TOPK) return fail(ctx, GQ_ERR_UNSUPPORTED, "topk > GQ_MAX_TOPK");
+  if (topk > 0 && (topk_agg < 0 || topk_agg >= a->naggs || !d_topk_scratch)) return fail(ctx, GQ_ERR_INVALID_ARG, "bad topk arguments");
+  GqFinaliseParams p;
+  memset(&p, 0, sizeof p);
+  p.slots = a->dev.slots; p.capacity = a->capacity; p.slot_words = a->dev.slot_words;
+  p.side = a->dev.side; p.header = a->dev.header;
+  p.nkeys = a->nkeys; p.ndep = a->ndep; p.naggs = a->naggs;
+  for (int k = 0; k < a->nkeys; ++k) {
+    if (!out_key_cols[k]) return fail(ctx, GQ_ERR_INVALID_ARG, "null key output");
+    p.key_bits[k] = a->key_bits[k]; p.key_dtype[k] = a->key_dtype[k]; p.out_key[k] = out_key_cols[k];
+  }
+  for (int i = 0; i < a->naggs; ++i) {
+    if (!out_agg_cols[i]) return fail(ctx, GQ_ERR_INVALID_ARG, "null aggregate output");
+    p.out_agg[i] = (long long*)out_agg_cols[i];
+  }
+  p.navg = navg;
+  for (int v = 0; v < navg; ++v) {
+    if (avgs[v].sum_agg < 0 || avgs[v].sum_agg >= a->naggs || avgs[v].count_agg < 0 || avgs[v].count_agg >= a->naggs || !out_avg_cols[v])
+      return fail(ctx, GQ_ERR_INVALID_ARG, "bad avg spec");
+    p.avg_sum[v] = avgs[v].sum_agg; p.avg_cnt[v] = avgs[v].count_agg; p.out_avg[v] = out_avg_cols[v];
+  }
+  p.out_capacity = out_capacity; p.out_n = (long long*)d_out_ngroups; p.err = ctx->d_err;
+  p.topk = topk; p.topk_agg = topk_agg; p.scratch = d_topk_scratch;
+  cudaError_t e = cudaMemsetAsync(d_out_ngroups, 0, 8, ctx->stream);
+  if (e != cudaSuccess) return cuda_fail(ctx, e, "memset ngroups");
+  int nl = 0;
+  e = gq_launch_finalise(ctx->stream, p, ctx->num_sms, &nl);
+  if (e != cudaSuccess) return cuda_fail(ctx, e, "finalise");
+  ctx->launches += nl;
+  return GQ_OK;
+}
+
+gq_status gq_aggstate_destroy(gq_aggstate* a) { if (!a) return GQ_ERR_INVALID_ARG; delete a; return GQ_OK; }
+
+// ------------------------------------------------------------------------------------------------ fused pipeline
+gq_status gq_pipeline_workspace(const gq_plan* plan, size_t* bytes) {
+  if (!plan || !bytes) return GQ_ERR_INVALID_ARG;
+  size_t b = 0;
+  gq_status st = gq_hash_aggregate_workspace(plan->agg.max_groups, plan->agg.nkeys, plan->agg.naggs, &b);
+  if (st != GQ_OK) return st;
+  *bytes = align_up(b, 256) + (plan->topk > 0 ? gq_topk_scratch_bytes_impl() : 0);
+  return GQ_OK;
+}
+
+gq_status gq_pipeline(gq_ctx* ctx, const gq_plan* plan, void* d_ws, size_t bytes, void* const* out_key_cols,
+                      int64_t* const* out_agg_cols, double* const* out_avg_cols, int64_t out_capacity,
+                      int64_t* d_out_ngroups) {
+  if (!ctx || !plan || !plan->in) return GQ_ERR_INVALID_ARG;
+  size_t need = 0, aggb = 0;
+  gq_status st = gq_pipeline_workspace(plan, &need);
+  if (st != GQ_OK) return fail(ctx, st, "bad plan");
+  if (bytes < need) return fail(ctx, GQ_ERR_WORKSPACE_TOO_SMALL, "pipeline workspace too small");
+  gq_hash_aggregate_workspace(plan->agg.max_groups, plan->agg.nkeys, plan->agg.naggs, &aggb);
+  gq_aggstate* a = nullptr;
+  st = gq_hash_aggregate(ctx, &a, d_ws, aggb, plan->in, &plan->agg);
+  if (st != GQ_OK) { if (a) delete a; return st; }
+  st = gq_hash_aggregate_finish(ctx, a, out_key_cols, out_agg_cols, plan->avgs, plan->navg, out_avg_cols, out_capacity,
+                                plan->topk, plan->topk_agg, (char*)d_ws + align_up(aggb, 256), d_out_ngroups);
+  delete a;   // host handle only; the enqueued kernels hold device pointers into the caller's workspace
+  return st;
+}
+
+// ------------------------------------------------------------------------------------------------ read probe
+gq_status gq_read_probe(gq_ctx* ctx, const void* d_data, size_t bytes, uint64_t* d_out) {
+  if (!ctx || !d_data || !d_out || !aligned(d_data, 16) || bytes % 16) return GQ_ERR_INVALID_ARG;
+  cudaError_t e = gq_launch_read_probe(ctx->stream, d_data, bytes, (unsigned long long*)d_out, ctx->num_sms);
+  if (e != cudaSuccess) return cuda_fail(ctx, e, "read probe");
+  ++ctx->launches;
+  return GQ_OK;
+}
+
+}  // extern "C"
+
+// ------------------------------------------------------------------------------------------------ host-buffer e2e
+namespace {
+struct HostLayout { size_t agg_off, agg_bytes, topk_off, stage_off[2], stage_col_off[GQ_MAX_COLS], stage_bytes, out_off, out_key_off[2],
+                    out_agg_off[GQ_MAX_AGGS], out_avg_off[GQ_MAX_AGGS], n_off, total; };
+gq_status host_layout(const gq_plan* plan, int64_t chunk_rows, int64_t out_capacity, HostLayout* L) {
+  size_t aggb = 0;
+  gq_status st = gq_hash_aggregate_workspace(plan->agg.max_groups, plan->agg.nkeys, plan->agg.naggs, &aggb);
+  if (st != GQ_OK) return st;
+  size_t off = 0;
+  L->agg_off = 0; L->agg_bytes = aggb; off = align_up(aggb, 256);
+  L->topk_off = off; off += plan->topk > 0 ? align_up(gq_topk_scratch_bytes_impl(), 256) : 0;
+  size_t sb = 0;
+  for (int c = 0; c < plan->in->ncols; ++c) { L->stage_col_off[c] = sb; sb += align_up((size_t)chunk_rows * gq_dtype_bytes(plan->in->cols[c].dtype), 256); }
+  L->stage_bytes = sb;
+  for (int b = 0; b < 2; ++b) { L->stage_off[b] = off; off += sb; }
+  L->out_off = off;
+  for (int k = 0; k < plan->agg.nkeys; ++k) { L->out_key_off[k] = off; off += align_up((size_t)out_capacity * 8, 256); }
+  for (int a = 0; a < plan->agg.naggs; ++a) { L->out_agg_off[a] = off; off += align_up((size_t)out_capacity * 8, 256); }
+  for (int v = 0; v < plan->navg; ++v) { L->out_avg_off[v] = off; off += align_up((size_t)out_capacity * 8, 256); }
+  L->n_off = off; off += 256;
+  L->total = off;
+  return GQ_OK;
+}
+}  // namespace
+
+extern "C" {
+
+gq_status gq_pipeline_host_workspace(const gq_plan* plan, int64_t chunk_rows, size_t* bytes) {
+  if (!plan || !plan->in || !bytes || chunk_rows < 1) return GQ_ERR_INVALID_ARG;
+  HostLayout L;
+  // output capacity is not known here: size for max_groups rows (top-k needs only k)
+  int64_t cap = plan->topk > 0 ? plan->topk : std::max<int64_t>(1, plan->agg.max_groups);
+  gq_status st = host_layout(plan, chunk_rows, cap, &L);
+  if (st != GQ_OK) return st;
+  *bytes = L.total;
+  return GQ_OK;
+}
+
+gq_status gq_pipeline_host(gq_ctx* ctx, const gq_plan* plan, int64_t chunk_rows, void* d_ws, size_t bytes,
+                           void* const* h_out_key_cols, int64_t* const* h_out_agg_cols, double* const* h_out_avg_cols,
+                           int64_t out_capacity, int64_t* h_out_ngroups) {
+  if (!ctx || !plan || !plan->in || !d_ws || chunk_rows < 1 || !h_out_ngroups || !h_out_agg_cols) return GQ_ERR_INVALID_ARG;
+  const gq_batch* in = plan->in;
+  if (in->ncols < 1 || in->ncols > GQ_MAX_COLS) return fail(ctx, GQ_ERR_INVALID_ARG, "bad batch");
+  chunk_rows = (chunk_rows + 2047) / 2048 * 2048;   // whole tiles per chunk: only the last chunk has a ragged tail
+  int64_t cap = plan->topk > 0 ? plan->topk : std::max<int64_t>(1, plan->agg.max_groups);
+  if (out_capacity > cap) out_capacity = cap;
+  HostLayout L;
+  gq_status st = host_layout(plan, chunk_rows, cap, &L);
+  if (st != GQ_OK) return fail(ctx, st, "bad plan");
+  if (bytes < L.total) return fail(ctx, GQ_ERR_WORKSPACE_TOO_SMALL, "host-pipeline workspace too small");
+  cudaError_t e = cudaSuccess;
+  if (!ctx->copy_stream) {
+    e = cudaStreamCreateWithFlags(&ctx->copy_stream, cudaStreamNonBlocking);
+    for (int i = 0; i < 2 && e == cudaSuccess; ++i) {
+      e = cudaEventCreateWithFlags(&ctx->ev_copied[i], cudaEventDisableTiming);
+      if (e == cudaSuccess) e = cudaEventCreateWithFlags(&ctx->ev_consumed[i], cudaEventDisableTiming);
+    }
+    if (e != cudaSuccess) return cuda_fail(ctx, e, "copy stream setup");
+  }
+  char* ws = (char*)d_ws;
+  gq_aggstate* a = nullptr;
+  int64_t nchunks = std::max<int64_t>(1, (in->nrows + chunk_rows - 1) / chunk_rows);
+  for (int64_t i = 0; i < nchunks; ++i) {
+    const int b = (int)(i & 1);
+    const int64_t r0 = i * chunk_rows, n = std::min<int64_t>(chunk_rows, in->nrows - r0);
+    if (i >= 2) e = cudaStreamWaitEvent(ctx->copy_stream, ctx->ev_consumed[b], 0);
+    gq_column cols[GQ_MAX_COLS];
+    for (int c = 0; c < in->ncols && e == cudaSuccess; ++c) {
+      const int eb = gq_dtype_bytes(in->cols[c].dtype);
+      cols[c].dtype = in->cols[c].dtype;
+      cols[c].data = ws + L.stage_off[b] + L.stage_col_off[c];
+      if (n > 0) e = cudaMemcpyAsync((void*)cols[c].data, (const char*)in->cols[c].data + (size_t)r0 * eb, (size_t)n * eb,
+                                     cudaMemcpyHostToDevice, ctx->copy_stream);
+    }
+    if (e == cudaSuccess) e = cudaEventRecord(ctx->ev_copied[b], ctx->copy_stream);
+    if (e == cudaSuccess) e = cudaStreamWaitEvent(ctx->stream, ctx->ev_copied[b], 0);
+    if (e != cudaSuccess) { if (a) delete a; return cuda_fail(ctx, e, "chunk copy"); }
+    gq_batch chunk{cols, in->ncols, std::max<int64_t>(0, n)};
+    st = gq_hash_aggregate(ctx, &a, ws + L.agg_off, L.agg_bytes, &chunk, &plan->agg);
+    if (st != GQ_OK) { if (a) delete a; return st; }
+    e = cudaEventRecord(ctx->ev_consumed[b], ctx->stream);
+    if (e != cudaSuccess) { delete a; return cuda_fail(ctx, e, "event record"); }
+  }
+  void* dk[2]; int64_t* da[GQ_MAX_AGGS]; double* dv[GQ_MAX_AGGS];
+  for (int k = 0; k < plan->agg.nkeys; ++k) dk[k] = ws + L.out_key_off[k];
+  for (int i = 0; i < plan->agg.naggs; ++i) da[i] = (int64_t*)(ws + L.out_agg_off[i]);
+  for (int v = 0; v < plan->navg; ++v) dv[v] = (double*)(ws + L.out_avg_off[v]);
+  st = gq_hash_aggregate_finish(ctx, a, dk, da, plan->avgs, plan->navg, dv, cap, plan->topk, plan->topk_agg,
+                                ws + L.topk_off, (int64_t*)(ws + L.n_off));
+  const int nkeys = a->nkeys;
+  gq_dtype kd[2] = {a->key_dtype[0], a->key_dtype[1]};
+  delete a;
+  if (st != GQ_OK) return st;
+  e = cudaMemcpyAsync(h_out_ngroups, ws + L.n_off, 8, cudaMemcpyDeviceToHost, ctx->stream);
+  if (e != cudaSuccess) return cuda_fail(ctx, e, "copy ngroups");
+  st = gq_sync(ctx);
+  if (st != GQ_OK) return st;
+  const int64_t n = std::min<int64_t>(*h_out_ngroups, out_capacity);
+  if (*h_out_ngroups > out_capacity) return fail(ctx, GQ_ERR_CAPACITY, "host output capacity exceeded");
+  for (int k = 0; k < nkeys && e == cudaSuccess; ++k)
+    e = cudaMemcpyAsync(h_out_key_cols[k], dk[k], (size_t)n * gq_dtype_bytes(kd[k]), cudaMemcpyDeviceToHost, ctx->stream);
+  for (int i = 0; i < plan->agg.naggs && e == cudaSuccess; ++i)
+    e = cudaMemcpyAsync(h_out_agg_cols[i], da[i], (size_t)n * 8, cudaMemcpyDeviceToHost, ctx->stream);
+  for (int v = 0; v < plan->navg && e == cudaSuccess; ++v)
+    e = cudaMemcpyAsync(h_out_avg_cols[v], dv[v], (size_t)n * 8, cudaMemcpyDeviceToHost, ctx->stream);
+  if (e != cudaSuccess) return cuda_fail(ctx, e, "copy results");
+  return gq_sync(ctx);
+}
+
+// ------------------------------------------------------------------------------------------------ precompile
+gq_status gq_set_kernel_cache_dir(const char* h_path) { gq_jit_set_cache_dir(h_path); return GQ_OK; }
+
+static gq_status precompile(const GqScanSpec& sp, char* h_msg, size_t msg_bytes) {
+  std::string msg, path;
+  CachedKernel* ck = nullptr;
+  gq_status st = get_kernel_info(sp, &ck, &msg);
+  if (st == GQ_OK) st = gq_jit_compile_to_cache(ck->info, &path, &msg);
+  if (st == GQ_OK) msg = path;
+  if (h_msg && msg_bytes) { strncpy(h_msg, msg.c_str(), msg_bytes - 1); h_msg[msg_bytes - 1] = 0; }
+  return st;
+}
+
+gq_status gq_precompile_pipeline(const gq_plan* plan, char* h_msg, size_t msg_bytes) {
+  if (!plan || !plan->in) return GQ_ERR_INVALID_ARG;
+  gq_ctx tmp;
+  GqScanSpec sp;
+  int kb[2]; gq_dtype kd[2];
+  gq_status st = agg_spec(&tmp, &sp, plan->in, &plan->agg, kb, kd);
+  if (st != GQ_OK) { if (h_msg && msg_bytes) { strncpy(h_msg, tmp.msg.c_str(), msg_bytes - 1); h_msg[msg_bytes - 1] = 0; } return st; }
+  return precompile(sp, h_msg, msg_bytes);
+}
+
+gq_status gq_precompile_build(const gq_batch* in, const gq_build_desc* d, char* h_msg, size_t msg_bytes) {
+  if (!in || !d) return GQ_ERR_INVALID_ARG;
+  gq_ctx tmp;
+  GqScanSpec sp;
+  gq_status st = build_spec(&tmp, &sp, in, d);
+  if (st != GQ_OK) { if (h_msg && msg_bytes) { strncpy(h_msg, tmp.msg.c_str(), msg_bytes - 1); h_msg[msg_bytes - 1] = 0; } return st; }
+  return precompile(sp, h_msg, msg_bytes);
+}
+
+}  // extern "C"

@@ -1,0 +1,339 @@
+// gq_codegen.cpp — plan-time translation of one scan shape into a fused CUDA kernel source.
+//
+// This is the "expression compilation at plan creation time" of PAPER.md:124/:152 (TypedExpr -> fused AST), done
+// B200-first: the whole FilterProject -> HashProbe* -> consumer chain of a plan becomes ONE kernel. The generator
+// emits a prelude of #defines plus two straight-line row functions (gq_pass, gq_body) and splices them between the
+// two halves of the hand-written skeleton (gq_skeleton.cuh / gq_skeleton_kernel.cuh). Predicate bounds and literals
+// stay runtime parameters (GqParams::k), so a kernel is specialised by plan SHAPE, not by constants.
+#include <algorithm>
+#include <cstdio>
+#include <map>
+#include <sstream>
+
+#include "gq_internal.h"
+
+extern const char gq_skeleton_a[];
+extern const char gq_skeleton_b[];
+
+int gq_dtype_bytes(gq_dtype t) { return t == GQ_I8 ? 1 : t == GQ_I32 ? 4 : t == GQ_I64 ? 8 : 0; }
+static const char* ctype(gq_dtype t) { return t == GQ_I8 ? "signed char" : t == GQ_I32 ? "int" : "long long"; }
+
+static uint64_t fnv1a(const std::string& s) {
+  uint64_t h = 1469598103934665603ULL;
+  for (unsigned char c : s) { h ^= c; h *= 1099511628211ULL; }
+  return h;
+}
+
+namespace {
+struct Gen {
+  const GqScanSpec& sp;
+  std::string* msg;
+  int ncols_in;
+  std::vector<int> compact;           // input column -> kernel column (or -1)
+  std::vector<int> cols;              // kernel column -> input column
+  std::vector<long long> consts;
+  std::vector<int> vcol_probe, vcol_pay;  // virtual column -> (probe step, payload index)
+
+  Gen(const GqScanSpec& s, std::string* m) : sp(s), msg(m), ncols_in((int)s.in_dtype.size()) {
+    compact.assign((size_t)ncols_in, -1);
+    for (size_t s2 = 0; s2 < sp.probes.size(); ++s2)
+      for (int p = 0; p < sp.probes[s2].npayload; ++p) { vcol_probe.push_back((int)s2); vcol_pay.push_back(p); }
+  }
+  bool fail(const std::string& m) { if (msg) *msg = m; return false; }
+  int row_width() const { return ncols_in + (int)vcol_probe.size(); }
+  // number of row columns visible BEFORE probe step s
+  int width_before_probe(int s) const {
+    int w = ncols_in;
+    for (int i = 0; i < s; ++i) w += sp.probes[(size_t)i].npayload;
+    return w;
+  }
+  bool use_col(int c) {                                   // register an input column as referenced
+    if (c < 0 || c >= row_width()) return fail("column index out of range");
+    if (c >= ncols_in) return true;
+    if (compact[(size_t)c] < 0) {
+      if ((int)cols.size() >= GQ_MAXCOL) return fail("too many referenced input columns");
+      compact[(size_t)c] = (int)cols.size();
+      cols.push_back(c);
+    }
+    return true;
+  }
+  std::string val(int c) const {                          // name of the row value of column c
+    char b[32];
+    if (c < ncols_in) snprintf(b, sizeof b, "v%d", c);
+    else snprintf(b, sizeof b, "y%d_%d", vcol_probe[(size_t)(c - ncols_in)], vcol_pay[(size_t)(c - ncols_in)]);
+    return b;
+  }
+  std::string konst(long long v) {
+    if ((int)consts.size() >= GQ_MAXK) { fail("too many constants"); return "0"; }
+    consts.push_back(v);
+    return "P.k[" + std::to_string(consts.size() - 1) + "]";
+  }
+  std::string load(int c) const {                         // typed load of input column c for row slot j
+    int kc = compact[(size_t)c];
+    std::ostringstream o;
+    o << "const i64 v" << c << " = src.template ld<" << ctype(sp.in_dtype[(size_t)c]) << ">(" << kc << ", GQ_COL_OFF("
+      << kc << "), j);";
+    return o.str();
+  }
+  bool expr(const std::vector<gq_xtok>& toks, std::string* out) {
+    std::vector<std::string> st;
+    if (toks.empty() || (int)toks.size() > GQ_MAX_TOKS) return fail("expression length out of range");
+    for (const gq_xtok& t : toks) {
+      if (t.op == GQ_X_COL) {
+        if (t.arg < 0 || t.arg >= row_width()) return fail("expression column out of range");
+        st.push_back(val((int)t.arg));
+      } else if (t.op == GQ_X_CONST) st.push_back(konst(t.arg));
+      else if (t.op == GQ_X_ADD || t.op == GQ_X_SUB || t.op == GQ_X_MUL) {
+        if (st.size() < 2) return fail("malformed postfix expression");
+        std::string b = st.back(); st.pop_back();
+        std::string a = st.back(); st.pop_back();
+        const char* f = t.op == GQ_X_ADD ? "gq_add" : t.op == GQ_X_SUB ? "gq_sub" : "gq_mul";
+        st.push_back(std::string(f) + "(" + a + ", " + b + ")");
+      } else return fail("unknown expression token");
+    }
+    if (st.size() != 1) return fail("malformed postfix expression");
+    *out = st[0];
+    return true;
+  }
+};
+}  // namespace
+
+gq_status gq_codegen(const GqScanSpec& sp, GqKernelInfo* out, std::string* msg) {
+  Gen g(sp, msg);
+  const int nprobe = (int)sp.probes.size();
+  const int nagg = (int)sp.aggs.size();
+  if ((int)sp.preds.size() > GQ_MAX_PREDS || nprobe > GQ_MAX_PROBES || (int)sp.exprs.size() > GQ_MAX_EXPRS ||
+      nagg > GQ_MAX_AGGS) { if (msg) *msg = "plan exceeds GQ_MAX_* limits"; return GQ_ERR_UNSUPPORTED; }
+
+  // ---- 1. referenced columns: predicate columns first (they are read for every row) ----
+  for (const gq_pred& p : sp.preds) {
+    if (p.col < 0 || p.col >= g.ncols_in) { if (msg) *msg = "predicate column must be an input column"; return GQ_ERR_INVALID_ARG; }
+    if (!g.use_col(p.col)) return GQ_ERR_INVALID_ARG;
+  }
+  for (int s = 0; s < nprobe; ++s) {
+    if (sp.probes[(size_t)s].key_col < 0 || sp.probes[(size_t)s].key_col >= g.width_before_probe(s)) {
+      if (msg) *msg = "probe key column out of range"; return GQ_ERR_INVALID_ARG; }
+    if (!g.use_col(sp.probes[(size_t)s].key_col)) return GQ_ERR_INVALID_ARG;
+  }
+  for (const auto& e : sp.exprs)
+    for (const gq_xtok& t : e)
+      if (t.op == GQ_X_COL && !g.use_col((int)t.arg)) return GQ_ERR_INVALID_ARG;
+  for (int c : sp.key_cols) if (!g.use_col(c)) return GQ_ERR_INVALID_ARG;
+  if (sp.consumer == GQ_C_BUILD) {
+    if (!g.use_col(sp.build_key_col)) return GQ_ERR_INVALID_ARG;
+    for (int c : sp.payload_cols) if (!g.use_col(c)) return GQ_ERR_INVALID_ARG;
+  }
+  for (const gq_agg& a : sp.aggs)
+    if (a.op != GQ_COUNT_STAR && (a.expr < 0 || a.expr >= (int)sp.exprs.size())) {
+      if (msg) *msg = "aggregate names a missing expression"; return GQ_ERR_INVALID_ARG; }
+  if (g.cols.empty()) {  // a kernel needs at least one column to define rows; count(*)-only plans read column 0
+    if (g.ncols_in == 0) { if (msg) *msg = "batch has no columns"; return GQ_ERR_INVALID_ARG; }
+    g.use_col(0);
+  }
+
+  // ---- 2. tiling: consumer threads, rows per thread, stages under the 227 KB shared-memory budget ----
+  const int ncol = (int)g.cols.size();
+  int row_bytes = 0;
+  for (int c : g.cols) row_bytes += gq_dtype_bytes(sp.in_dtype[(size_t)c]);
+  int nt = 512;
+  long long cons_bytes = 256;
+  if (sp.consumer == GQ_C_GLOBAL) cons_bytes = 8LL * nagg * (nt / 32) + 256;
+  if (sp.consumer == GQ_C_LOWCARD) {
+    nt = 256;
+    cons_bytes = (((sp.lc_cap + 1) * 8 + 8 + 127) / 128 * 128) + 8LL * (sp.lc_cap + 1) * nagg * nt;
+  }
+  int r = 4, stages = 0;
+  // small inputs: smaller tiles so that every SM still gets several tiles
+  if (sp.nrows_hint > 0 && sp.nrows_hint < 148LL * 8 * nt * 4) r = 2;
+  if (sp.nrows_hint > 0 && sp.nrows_hint < 148LL * 8 * nt * 2) r = 1;
+  long long stage_bytes = 0;
+  for (;; r /= 2) {
+    stage_bytes = 0;
+    for (int c : g.cols) stage_bytes += ((long long)nt * r * gq_dtype_bytes(sp.in_dtype[(size_t)c]) + 127) / 128 * 128;
+    long long avail = GQ_SMEM_LIMIT - cons_bytes - 2 * 4 * 8 - 64 - 128;
+    stages = (int)std::min<long long>(4, avail / stage_bytes);
+    if (stages >= 3 || r == 1) break;
+  }
+  if (stages < 1) { if (msg) *msg = "plan does not fit shared memory"; return GQ_ERR_UNSUPPORTED; }
+
+  // ---- 3. prelude ----
+  std::ostringstream o;
+  o << "// generated by gq_codegen — plan-shape specialised prelude\n";
+  o << "#define GQ_NCOL " << ncol << "\n#define GQ_NT " << nt << "\n#define GQ_R " << r << "\n#define GQ_STAGES "
+    << stages << "\n#define GQ_STAGE_BYTES " << stage_bytes << "\n#define GQ_CONSUMER " << sp.consumer << "\n";
+  o << "#define GQ_NAGG " << nagg << "\n#define GQ_LC_CAP " << (sp.lc_cap > 0 ? sp.lc_cap : 1) << "\n#define GQ_TARGET_SW "
+    << (sp.target_sw > 0 ? sp.target_sw : 1) << "\n#define GQ_NDEP " << sp.ndep << "\n#define GQ_EVICT_FIRST 1\n";
+  {
+    long long off = 0, tx = 0;
+    std::ostringstream offs, bytes;
+    offs << "#define GQ_COL_OFF(c) (";
+    bytes << "#define GQ_COL_BYTES(c) (";
+    for (int i = 0; i < ncol; ++i) {
+      int b = gq_dtype_bytes(sp.in_dtype[(size_t)g.cols[(size_t)i]]);
+      offs << "(c) == " << i << " ? " << off << " : ";
+      bytes << "(c) == " << i << " ? " << b << " : ";
+      off += ((long long)nt * r * b + 127) / 128 * 128;
+      tx += (long long)nt * r * b;
+    }
+    offs << "0)\n";
+    bytes << "0)\n";
+    o << offs.str() << bytes.str() << "#define GQ_TX_BYTES " << tx << "\n";
+    o << "#define GQ_AGG_OP(a) (";
+    for (int a = 0; a < nagg; ++a) o << "(a) == " << a << " ? " << (int)sp.aggs[(size_t)a].op << " : ";
+    o << "0)\n";
+  }
+  o << gq_skeleton_a << "\n";
+
+  // ---- 4. gq_pass: the filter ----
+  o << "template <class Src> __device__ __forceinline__ bool gq_pass(const GqParams& P, const Src& src, int j) {\n";
+  {
+    std::vector<bool> loaded(g.compact.size(), false);
+    for (const gq_pred& p : sp.preds) {
+      if (!loaded[(size_t)p.col]) { o << "  " << g.load(p.col) << "\n"; loaded[(size_t)p.col] = true; }
+      std::string v = g.val(p.col), c;
+      const std::string klo = g.konst(p.lo);   // sequenced: lo before hi (operands of + are unsequenced)
+      const std::string khi = (p.op == GQ_RANGE_CO || p.op == GQ_RANGE_CC) ? g.konst(p.hi) : std::string();
+      switch (p.op) {
+        case GQ_LT: c = v + " < " + klo; break;
+        case GQ_LE: c = v + " <= " + klo; break;
+        case GQ_GT: c = v + " > " + klo; break;
+        case GQ_GE: c = v + " >= " + klo; break;
+        case GQ_EQ: c = v + " == " + klo; break;
+        case GQ_NE: c = v + " != " + klo; break;
+        case GQ_RANGE_CO: c = v + " >= " + klo + " && " + v + " < " + khi; break;
+        case GQ_RANGE_CC: c = v + " >= " + klo + " && " + v + " <= " + khi; break;
+        default: if (msg) *msg = "unknown comparison"; return GQ_ERR_INVALID_ARG;
+      }
+      o << "  if (!(" << c << ")) return false;\n";
+    }
+  }
+  o << "  return true;\n}\n\n";
+
+  // ---- 5. gq_body: probes, projection, consumer ----
+  o << "template <class Src> __device__ __forceinline__ void gq_body(const GqParams& P, const Src& src, int j, GqCtx& cx) {\n";
+  {
+    // every input column referenced beyond the filter
+    std::vector<bool> need(g.compact.size(), false);
+    auto mark = [&](int c) { if (c < g.ncols_in) need[(size_t)c] = true; };
+    for (const auto& p : sp.probes) mark(p.key_col);
+    for (const auto& e : sp.exprs) for (const gq_xtok& t : e) if (t.op == GQ_X_COL) mark((int)t.arg);
+    for (int c : sp.key_cols) mark(c);
+    if (sp.consumer == GQ_C_BUILD) { mark(sp.build_key_col); for (int c : sp.payload_cols) mark(c); }
+    for (size_t c = 0; c < need.size(); ++c) if (need[c]) o << "  " << g.load((int)c) << "\n";
+  }
+  std::string ind = "  ";
+  for (int s = 0; s < nprobe; ++s) {   // one open-addressing lookup loop per probe step, nested
+    const GqProbeSpec& ps = sp.probes[(size_t)s];
+    const int sw = ps.slot_words;
+    o << ind << "{ // probe step " << s << "\n";
+    ind += "  ";
+    o << ind << "const GqTableDev& T" << s << " = P.probe[" << s << "];\n";
+    o << ind << "const i64 pk" << s << " = " << g.val(ps.key_col) << ";\n";
+    o << ind << "const bool sd" << s << " = ((u64)pk" << s << " == GQ_EMPTY);\n";
+    o << ind << "i64 ns" << s << " = 0; if (sd" << s << ") ns" << s << " = gq_min(T" << s << ".header[1], GQ_SIDE_SLOTS);\n";
+    o << ind << "u64 i" << s << " = gq_hash(pk" << s << ", T" << s << ".shift);\n";
+    o << ind << "for (u64 n" << s << " = 0; n" << s << " <= T" << s << ".mask; ++n" << s << ") {\n";
+    ind += "  ";
+    o << ind << "const u64* s" << s << "; u64 w" << s << " = 0;\n";
+    o << ind << "if (sd" << s << ") { if ((i64)n" << s << " >= ns" << s << ") break; s" << s << " = T" << s
+      << ".side + n" << s << " * " << sw << ";" << (sw == 2 ? " w" + std::to_string(s) + " = s" + std::to_string(s) + "[1];" : "")
+      << " }\n";
+    o << ind << "else {\n";
+    o << ind << "  s" << s << " = T" << s << ".slots + i" << s << " * " << sw << "; i" << s << " = (i" << s << " + 1) & T"
+      << s << ".mask;\n";
+    if (sw == 2) o << ind << "  u64 kw; gq_ld128(s" << s << ", kw, w" << s << ");\n";
+    else o << ind << "  const u64 kw = __ldg(s" << s << ");\n";
+    o << ind << "  if (kw == GQ_EMPTY) break;\n";
+    o << ind << "  if (kw != (u64)pk" << s << ") continue;\n";
+    o << ind << "}\n";
+    for (int p = 0; p < ps.npayload; ++p) {
+      if (sw == 2) o << ind << "const i64 y" << s << "_" << p << " = (i64)w" << s << ";\n";
+      else o << ind << "const i64 y" << s << "_" << p << " = (i64)__ldg(s" << s << " + " << (1 + p) << ");\n";
+    }
+    if (ps.npayload == 0) o << ind << "(void)w" << s << ";\n";
+  }
+  // projection
+  for (size_t e = 0; e < sp.exprs.size(); ++e) {
+    std::string x;
+    if (!g.expr(sp.exprs[e], &x)) return GQ_ERR_INVALID_ARG;
+    o << ind << "const i64 e" << e << " = " << x << ";\n";
+  }
+  // group key
+  std::string keyx, depx;
+  if (sp.consumer == GQ_C_LOWCARD || sp.consumer == GQ_C_HIGHCARD) {
+    const int nk = (int)sp.key_cols.size();
+    if (nk < 1 || nk > GQ_MAX_KEYS || sp.ndep < 0 || sp.ndep >= nk) { if (msg) *msg = "bad key columns"; return GQ_ERR_INVALID_ARG; }
+    if (nk - sp.ndep == 1) keyx = g.val(sp.key_cols[0]);
+    else {  // two hashed keys packed into one 64-bit word: key0 in the low bits
+      auto dt = [&](int c) { return c < g.ncols_in ? sp.in_dtype[(size_t)c]
+                                                    : sp.probes[(size_t)g.vcol_probe[(size_t)(c - g.ncols_in)]].pay_dtype[g.vcol_pay[(size_t)(c - g.ncols_in)]]; };
+      int b0 = 8 * gq_dtype_bytes(dt(sp.key_cols[0])), b1 = 8 * gq_dtype_bytes(dt(sp.key_cols[1]));
+      if (b0 + b1 > 64) { if (msg) *msg = "packed key wider than 64 bits: declare a dependent key (ndependent)"; return GQ_ERR_UNSUPPORTED; }
+      char buf[256];
+      snprintf(buf, sizeof buf, "(i64)((((u64)%s) & 0x%llxULL) | ((((u64)%s) & 0x%llxULL) << %d))", g.val(sp.key_cols[0]).c_str(),
+               (unsigned long long)((b0 == 64) ? ~0ULL : ((1ULL << b0) - 1)), g.val(sp.key_cols[1]).c_str(),
+               (unsigned long long)((1ULL << b1) - 1), b0);
+      keyx = buf;
+    }
+    if (sp.ndep == 1) depx = g.val(sp.key_cols[(size_t)nk - 1]);
+  }
+  auto aggval = [&](const gq_agg& a) { return a.op == GQ_COUNT_STAR ? std::string("1") : "e" + std::to_string(a.expr); };
+  switch (sp.consumer) {
+    case GQ_C_GLOBAL:
+      for (int a = 0; a < nagg; ++a)
+        o << ind << "cx.acc[" << a << "] = gq_combine(" << (int)sp.aggs[(size_t)a].op << ", cx.acc[" << a << "], "
+          << aggval(sp.aggs[(size_t)a]) << ");\n";
+      break;
+    case GQ_C_LOWCARD:
+      o << ind << "const int grp = gq_lc_slot(cx, " << keyx << ", P.err);\n" << ind << "if (grp >= 0) {\n";
+      for (int a = 0; a < nagg; ++a)
+        o << ind << "  gq_lc_update(" << (int)sp.aggs[(size_t)a].op << ", cx, grp, " << a << ", " << aggval(sp.aggs[(size_t)a]) << ");\n";
+      o << ind << "}\n";
+      break;
+    case GQ_C_HIGHCARD:
+      o << ind << "bool won; u64* slot = gq_ht_upsert<" << sp.target_sw << ">(P.target, " << keyx << ", &won, P.err);\n";
+      o << ind << "if (slot) {\n";
+      if (sp.ndep == 1) o << ind << "  if (won) slot[1] = (u64)" << depx << ";\n";
+      for (int a = 0; a < nagg; ++a)
+        o << ind << "  gq_red(" << (int)sp.aggs[(size_t)a].op << ", slot + " << (1 + sp.ndep + a) << ", " << aggval(sp.aggs[(size_t)a]) << ");\n";
+      o << ind << "}\n";
+      break;
+    case GQ_C_BUILD: {
+      const int np = (int)sp.payload_cols.size();
+      o << ind << "const i64 pay[" << (np > 0 ? np : 1) << "] = {";
+      for (int p = 0; p < np; ++p) o << (p ? ", " : "") << g.val(sp.payload_cols[(size_t)p]);
+      if (np == 0) o << "0";
+      o << "};\n";
+      o << ind << "if (gq_ht_insert<" << sp.target_sw << ", " << np << ">(P.target, " << g.val(sp.build_key_col) << ", pay, "
+        << (sp.unique ? "true" : "false") << ", P.err)) ++cx.ninserted;\n";
+      break;
+    }
+    case GQ_C_MATERIALISE:
+      if (sp.exprs.size() > GQ_MAXOUT) { if (msg) *msg = "too many output columns"; return GQ_ERR_UNSUPPORTED; }
+      o << ind << "const i64 orow = gq_reserve_row(P);\n" << ind << "if (orow >= 0) {\n";
+      for (size_t e = 0; e < sp.exprs.size(); ++e) o << ind << "  P.out[" << e << "][orow] = e" << e << ";\n";
+      o << ind << "}\n";
+      break;
+    default: if (msg) *msg = "unknown consumer"; return GQ_ERR_INVALID_ARG;
+  }
+  for (int s = nprobe - 1; s >= 0; --s) {
+    if (sp.probes[(size_t)s].unique) o << ind << "break;  // unique build keys: first match is the only match\n";
+    ind.resize(ind.size() - 2);
+    o << ind << "}\n";
+    ind.resize(ind.size() - 2);
+    o << ind << "}\n";
+  }
+  o << "}\n\n" << gq_skeleton_b << "\n";
+
+  out->source = o.str();
+  char hb[32];
+  snprintf(hb, sizeof hb, "%016llx", (unsigned long long)fnv1a(out->source));
+  out->hash = hb;
+  out->threads = nt + 32;
+  out->tile_rows = nt * r;
+  out->smem_bytes = (int)(stages * stage_bytes + 2 * stages * 8 + 64 + cons_bytes + 128);
+  out->cols = g.cols;
+  out->consts = g.consts;
+  if ((int)g.consts.size() > GQ_MAXK) { if (msg) *msg = "too many constants"; return GQ_ERR_UNSUPPORTED; }
+  return GQ_OK;
+}

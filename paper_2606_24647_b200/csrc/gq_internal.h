@@ -1,0 +1,146 @@
+// gq_internal.h — host-side internals of libgq.so (not part of the ABI).
+#ifndef GQ_INTERNAL_H
+#define GQ_INTERNAL_H
+#include <cuda_runtime.h>
+
+#include <cstdint>
+#include <string>
+#include <vector>
+
+#include "../../include/gq.h"
+
+#define GQ_EMPTY_KEY 0x8000000000000000ULL
+#define GQ_MAXCOL 16
+#define GQ_MAXK 48
+#define GQ_MAXOUT 12
+#define GQ_SMEM_LIMIT 232448   // 227 KB opt-in dynamic shared memory per CTA on sm_100
+
+enum { GQ_C_GLOBAL = 0, GQ_C_LOWCARD = 1, GQ_C_HIGHCARD = 2, GQ_C_BUILD = 3, GQ_C_MATERIALISE = 4 };
+
+// ---- device-visible structs: layouts must match gq_skeleton.cuh ----
+struct GqTableDev {
+  unsigned long long* slots;
+  unsigned long long mask;
+  long long* header;
+  unsigned long long* side;
+  int shift;
+  int slot_words;
+  unsigned flags;
+  unsigned pad;
+};
+struct GqParams {
+  const void* col[GQ_MAXCOL];
+  long long nrows;
+  long long k[GQ_MAXK];
+  GqTableDev probe[4];
+  GqTableDev target;
+  long long* acc;
+  long long* out[GQ_MAXOUT];
+  long long out_capacity;
+  long long* out_count;
+  int* err;
+  int pad;
+};
+
+// ---- handles ----
+struct gq_ctx {
+  int device = 0;
+  cudaStream_t stream = nullptr;
+  int* d_err = nullptr;        // sticky device error
+  int* h_err = nullptr;        // pinned mirror
+  int num_sms = 148;
+  int last_cuda = 0;
+  int64_t launches = 0;
+  std::string msg;
+  cudaStream_t copy_stream = nullptr;   // gq_pipeline_host: H2D copies overlap the scan of the previous chunk
+  cudaEvent_t ev_copied[2] = {nullptr, nullptr}, ev_consumed[2] = {nullptr, nullptr};
+};
+
+struct gq_table {
+  bool describe_only = false;
+  GqTableDev dev{};
+  int64_t capacity = 0;
+  int npayload = 0;
+  gq_dtype payload_dtype[GQ_MAX_PAYLOAD] = {GQ_I64, GQ_I64, GQ_I64};
+  uint32_t flags = 0;
+  int64_t max_rows = 0;
+  std::string build_sig;       // shape signature of the first batch (later batches must match)
+  cudaEvent_t ready = nullptr; // recorded by gq_hash_build_finish
+  cudaStream_t build_stream = nullptr;
+  bool finished = false;
+};
+
+struct gq_aggstate {
+  GqTableDev dev{};
+  int64_t capacity = 0;        // 0 when nkeys == 0
+  int nkeys = 0, ndep = 0, naggs = 0;
+  gq_dtype key_dtype[GQ_MAX_KEYS] = {GQ_I64, GQ_I64};
+  int key_bits[GQ_MAX_KEYS] = {64, 0};  // packed widths (0 for a dependent key)
+  gq_aggop agg_op[GQ_MAX_AGGS] = {};
+  int64_t max_groups = 0;
+  bool lowcard = false;
+  int lc_cap = 0;
+  std::string sig;
+};
+
+// ---- normalised plan of one fused scan kernel ----
+struct GqProbeSpec {
+  int key_col;                 // index into the row (input columns, then payloads of earlier probes)
+  int npayload;
+  gq_dtype pay_dtype[GQ_MAX_PAYLOAD];
+  bool unique;
+  int slot_words;
+};
+struct GqScanSpec {
+  std::vector<gq_dtype> in_dtype;                 // batch schema
+  std::vector<gq_pred> preds;
+  std::vector<GqProbeSpec> probes;
+  std::vector<std::vector<gq_xtok>> exprs;
+  int consumer = GQ_C_GLOBAL;
+  std::vector<int> key_cols;                      // LOWCARD / HIGHCARD
+  int ndep = 0;
+  std::vector<gq_agg> aggs;
+  int lc_cap = 0;
+  int target_sw = 0;                              // slot words of the target table
+  int build_key_col = 0;                          // BUILD
+  std::vector<int> payload_cols;
+  bool unique = false;
+  int64_t nrows_hint = 0;                         // tiling heuristic only
+};
+
+struct GqKernelInfo {
+  std::string source;          // full translation unit
+  std::string hash;            // 16 hex digits of the source hash
+  int threads = 0;             // GQ_NT + 32
+  int smem_bytes = 0;
+  int tile_rows = 0;
+  std::vector<int> cols;       // compacted column list: original input column index per kernel column
+  std::vector<long long> consts;  // values for GqParams::k
+};
+
+// gq_codegen.cpp
+gq_status gq_codegen(const GqScanSpec& spec, GqKernelInfo* out, std::string* msg);
+int gq_dtype_bytes(gq_dtype t);
+// gq_jit.cpp
+struct GqKernel { cudaKernel_t fn = nullptr; int threads = 0; int smem_bytes = 0; int tile_rows = 0; };
+gq_status gq_jit_compile_to_cache(const GqKernelInfo& info, std::string* cubin_path, std::string* msg);
+gq_status gq_jit_get(const GqKernelInfo& info, GqKernel* out, std::string* msg, int* cuda_err);
+void gq_jit_set_cache_dir(const char* path);
+// gq_static.cu
+struct GqFinaliseParams {
+  const unsigned long long* slots; long long capacity; int slot_words;
+  const unsigned long long* side; const long long* header;
+  int nkeys, ndep, naggs;
+  int key_bits[2]; int key_dtype[2];
+  void* out_key[2]; long long* out_agg[GQ_MAX_AGGS];
+  int navg; int avg_sum[GQ_MAX_AGGS]; int avg_cnt[GQ_MAX_AGGS]; double* out_avg[GQ_MAX_AGGS];
+  long long out_capacity; long long* out_n; int* err;
+  int topk, topk_agg; void* scratch;
+};
+cudaError_t gq_launch_init_table(cudaStream_t s, unsigned long long* slots, long long nslots, int slot_words,
+                                 const unsigned long long* pattern, unsigned long long* side, long long nside,
+                                 long long* header, long long header1);
+cudaError_t gq_launch_finalise(cudaStream_t s, const GqFinaliseParams& p, int num_sms, int* nlaunches);
+cudaError_t gq_launch_read_probe(cudaStream_t s, const void* data, size_t bytes, unsigned long long* out, int num_sms);
+size_t gq_topk_scratch_bytes_impl();
+#endif

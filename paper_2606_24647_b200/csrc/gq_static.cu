@@ -1,0 +1,260 @@
+// gq_static.cu — plan-independent sm_100a kernels, compiled by nvcc into libgq.so: hash-table initialisation, the
+// HashAggregation finaliser (table -> dense output columns + device-side group count + derived AVG),
+// the top-k finaliser (OrderBy/TopN in its smallest form) and the read-roofline probe.
+#include "gq_internal.h"
+
+typedef unsigned long long u64;
+typedef long long i64;
+
+// ------------------------------------------------------------------------------------------------ table init
+// Writes the slot pattern (key = EMPTY, dependent words 0, aggregate identities) with 128-bit stores where the slot
+// size allows; zeroes the header (header[1] = header1) and marks side slots empty.
+__global__ void gq_k_init_table(u64* slots, i64 nwords, int sw, const __grid_constant__ ulonglong4 pat0,
+                                const __grid_constant__ ulonglong4 pat1, const __grid_constant__ ulonglong4 pat2,
+                                u64* side, i64 nside_words, i64* header, i64 header1) {
+  const u64 pat[12] = {pat0.x, pat0.y, pat0.z, pat0.w, pat1.x, pat1.y, pat1.z, pat1.w, pat2.x, pat2.y, pat2.z, pat2.w};
+  const i64 stride = (i64)gridDim.x * blockDim.x;
+  const i64 t0 = (i64)blockIdx.x * blockDim.x + threadIdx.x;
+  // slot sizes are multiples of 2 words (or 1 word: key-only tables) -> pairs of words never straddle the pattern oddly
+  if ((sw & 1) == 0) {
+    ulonglong2* s2 = (ulonglong2*)slots;
+    const i64 npairs = nwords / 2;
+    const int pw = sw / 2;
+    for (i64 i = t0; i < npairs; i += stride) {
+      int k = (int)(i % pw) * 2;
+      s2[i] = make_ulonglong2(pat[k], pat[k + 1]);
+    }
+  } else {
+    for (i64 i = t0; i < nwords; i += stride) slots[i] = pat[i % sw];
+  }
+  for (i64 i = t0; i < nside_words; i += stride) side[i] = pat[i % sw];
+  if (t0 < 32) header[t0] = (t0 == 1) ? header1 : 0;
+}
+
+cudaError_t gq_launch_init_table(cudaStream_t s, u64* slots, i64 nslots, int sw, const u64* pattern, u64* side,
+                                 i64 nside, i64* header, i64 header1) {
+  ulonglong4 p[3];
+  u64* pp = (u64*)p;
+  for (int i = 0; i < 12; ++i) pp[i] = pattern[i % sw];
+  i64 nwords = nslots * sw;
+  i64 work = (sw & 1) == 0 ? nwords / 2 : nwords;
+  int blocks = (int)std::min<i64>(148 * 16, std::max<i64>(1, (work + 255) / 256));
+  gq_k_init_table<<<blocks, 256, 0, s>>>(slots, nwords, sw, p[0], p[1], p[2], side, nside * sw, header, header1);
+  return cudaGetLastError();
+}
+
+// ------------------------------------------------------------------------------------------------ finalise (dense)
+__device__ __forceinline__ i64 gq_sext(u64 v, int bits) {
+  if (bits >= 64) return (i64)v;
+  u64 m = 1ULL << (bits - 1);
+  v &= (1ULL << bits) - 1;
+  return (i64)((v ^ m) - m);
+}
+__device__ __forceinline__ void gq_store_key(void* col, int dtype, i64 idx, i64 v) {
+  if (dtype == GQ_I8) ((signed char*)col)[idx] = (signed char)v;
+  else if (dtype == GQ_I32) ((int*)col)[idx] = (int)v;
+  else ((i64*)col)[idx] = v;
+}
+// Emits one group (slot words s[], key word `key`) at output row idx.
+__device__ __forceinline__ void gq_emit_group(const GqFinaliseParams& P, const u64* s, u64 key, i64 idx) {
+  const int nhashed = P.nkeys - P.ndep;
+  if (nhashed == 1) gq_store_key(P.out_key[0], P.key_dtype[0], idx, (i64)key);
+  else if (nhashed == 2) {
+    gq_store_key(P.out_key[0], P.key_dtype[0], idx, gq_sext(key, P.key_bits[0]));
+    gq_store_key(P.out_key[1], P.key_dtype[1], idx, gq_sext(key >> P.key_bits[0], P.key_bits[1]));
+  }
+  for (int d = 0; d < P.ndep; ++d) gq_store_key(P.out_key[nhashed + d], P.key_dtype[nhashed + d], idx, (i64)s[1 + d]);
+  for (int a = 0; a < P.naggs; ++a) P.out_agg[a][idx] = (i64)s[1 + P.ndep + a];
+  for (int v = 0; v < P.navg; ++v)
+    P.out_avg[v][idx] = (double)(i64)s[1 + P.ndep + P.avg_sum[v]] / (double)(i64)s[1 + P.ndep + P.avg_cnt[v]];
+}
+
+// One thread per GQ_FIN_PER slots; block-level compaction: ballot/popc inside warps, shared-memory scan over warps,
+// ONE atomicAdd per block on the device-side group count.
+#define GQ_FIN_THREADS 256
+#define GQ_FIN_PER 4
+__global__ void __launch_bounds__(GQ_FIN_THREADS) gq_k_finalise(const __grid_constant__ GqFinaliseParams P) {
+  __shared__ int warp_cnt[GQ_FIN_THREADS / 32];
+  __shared__ i64 block_base;
+  if (*(volatile int*)P.err != 0) return;
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  const i64 nblocks_slots = (P.capacity + GQ_FIN_THREADS * GQ_FIN_PER - 1) / (GQ_FIN_THREADS * GQ_FIN_PER);
+  for (i64 b = blockIdx.x; b < nblocks_slots; b += gridDim.x) {
+    const i64 base = b * (GQ_FIN_THREADS * GQ_FIN_PER);
+    u64 key[GQ_FIN_PER];
+    int mine = 0;
+#pragma unroll
+    for (int j = 0; j < GQ_FIN_PER; ++j) {
+      i64 i = base + j * GQ_FIN_THREADS + threadIdx.x;
+      key[j] = (i < P.capacity) ? P.slots[i * P.slot_words] : GQ_EMPTY_KEY;
+      mine += (key[j] != GQ_EMPTY_KEY);
+    }
+    // exclusive prefix of `mine` inside the block
+    int incl = mine;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) { int n = __shfl_up_sync(0xffffffffu, incl, o); if (lane >= o) incl += n; }
+    if (lane == 31) warp_cnt[warp] = incl;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+      int tot = 0;
+      for (int w = 0; w < GQ_FIN_THREADS / 32; ++w) { int c = warp_cnt[w]; warp_cnt[w] = tot; tot += c; }
+      block_base = tot ? (i64)atomicAdd((u64*)P.out_n, (u64)tot) : 0;
+    }
+    __syncthreads();
+    i64 idx = block_base + warp_cnt[warp] + (incl - mine);
+#pragma unroll
+    for (int j = 0; j < GQ_FIN_PER; ++j) {
+      if (key[j] == GQ_EMPTY_KEY) continue;
+      i64 i = base + j * GQ_FIN_THREADS + threadIdx.x;
+      if (idx < P.out_capacity) gq_emit_group(P, P.slots + i * P.slot_words, key[j], idx);
+      else atomicCAS(P.err, 0, (int)GQ_ERR_CAPACITY);
+      ++idx;
+    }
+    __syncthreads();
+  }
+  // the side slot: the group whose key equals the reserved EMPTY pattern, or THE group of a key-less aggregation
+  if (blockIdx.x == 0 && threadIdx.x == 0 && P.header[1] != 0) {
+    i64 idx = (i64)atomicAdd((u64*)P.out_n, 1ULL);
+    if (idx < P.out_capacity) gq_emit_group(P, P.side, GQ_EMPTY_KEY, idx);
+    else atomicCAS(P.err, 0, (int)GQ_ERR_CAPACITY);
+  }
+}
+
+// ------------------------------------------------------------------------------------------------ finalise (top-k)
+// Order: aggregate descending, then key tuple ascending — a total order, so the answer is unique.
+struct GqCand { i64 val, k0, k1, slot; int valid; };
+__device__ __forceinline__ bool gq_better(const GqCand& a, const GqCand& b) {   // a strictly before b
+  if (!a.valid) return false;
+  if (!b.valid) return true;
+  if (a.val != b.val) return a.val > b.val;
+  if (a.k0 != b.k0) return a.k0 < b.k0;
+  return a.k1 < b.k1;
+}
+__device__ __forceinline__ GqCand gq_cand_shfl(const GqCand& c, int src) {
+  GqCand r;
+  r.val = __shfl_sync(0xffffffffu, c.val, src); r.k0 = __shfl_sync(0xffffffffu, c.k0, src);
+  r.k1 = __shfl_sync(0xffffffffu, c.k1, src); r.slot = __shfl_sync(0xffffffffu, c.slot, src);
+  r.valid = __shfl_sync(0xffffffffu, c.valid, src);
+  return r;
+}
+// Warp-distributed sorted list: lane i holds the i-th best entry. Inserts warp-uniform candidate c.
+__device__ __forceinline__ void gq_list_insert(GqCand& mine, const GqCand& c, int lane) {
+  unsigned before = __ballot_sync(0xffffffffu, gq_better(mine, c));   // entries that stay ahead of c (a prefix)
+  int pos = __popc(before);
+  GqCand up;
+  up.val = __shfl_up_sync(0xffffffffu, mine.val, 1); up.k0 = __shfl_up_sync(0xffffffffu, mine.k0, 1);
+  up.k1 = __shfl_up_sync(0xffffffffu, mine.k1, 1); up.slot = __shfl_up_sync(0xffffffffu, mine.slot, 1);
+  up.valid = __shfl_up_sync(0xffffffffu, mine.valid, 1);
+  if (lane == pos) mine = c;
+  else if (lane > pos) mine = up;
+}
+__device__ __forceinline__ GqCand gq_make_cand(const GqFinaliseParams& P, const u64* s, u64 key, i64 slot) {
+  GqCand c;
+  c.valid = 1; c.slot = slot; c.k1 = 0;
+  c.val = (i64)s[1 + P.ndep + P.topk_agg];
+  const int nhashed = P.nkeys - P.ndep;
+  if (nhashed == 2) { c.k0 = gq_sext(key, P.key_bits[0]); c.k1 = gq_sext(key >> P.key_bits[0], P.key_bits[1]); }
+  else { c.k0 = (i64)key; if (P.ndep) c.k1 = (i64)s[1]; }
+  return c;
+}
+// Feeds the candidates held by the lanes in `m` (each better than the list's current worst) into the list.
+__device__ __forceinline__ void gq_list_feed(GqCand& mine, const GqCand& c, bool want, int lane) {
+  unsigned m = __ballot_sync(0xffffffffu, want);
+  while (m) {
+    int src = __ffs(m) - 1;
+    m &= m - 1;
+    GqCand b = gq_cand_shfl(c, src);
+    GqCand worst = gq_cand_shfl(mine, 31);
+    if (gq_better(b, worst)) gq_list_insert(mine, b, lane);
+  }
+}
+#define GQ_TOPK_BLOCKS 592
+#define GQ_TOPK_WARPS 8
+// pass 1: every warp scans a strided share of the table and keeps its own best 32; lists go to scratch.
+__global__ void __launch_bounds__(GQ_TOPK_WARPS * 32) gq_k_topk_scan(const __grid_constant__ GqFinaliseParams P) {
+  if (*(volatile int*)P.err != 0) return;
+  const int lane = threadIdx.x & 31;
+  const i64 gw = (i64)blockIdx.x * GQ_TOPK_WARPS + (threadIdx.x >> 5);
+  const i64 nw = (i64)gridDim.x * GQ_TOPK_WARPS;
+  GqCand mine; mine.valid = 0; mine.val = 0; mine.k0 = 0; mine.k1 = 0; mine.slot = -1;
+  if (gw == 0) {   // the side slot
+    GqCand c; c.valid = 0; c.val = 0; c.k0 = 0; c.k1 = 0; c.slot = -1;
+    bool want = false;
+    if (lane == 0 && P.header[1] != 0) { c = gq_make_cand(P, P.side, GQ_EMPTY_KEY, -2); want = true; }
+    gq_list_feed(mine, c, want, lane);
+  }
+  for (i64 i0 = gw * 32; i0 < P.capacity; i0 += nw * 32) {
+    i64 i = i0 + lane;
+    GqCand c; c.valid = 0; c.val = 0; c.k0 = 0; c.k1 = 0; c.slot = -1;
+    bool want = false;
+    if (i < P.capacity) {
+      const u64* s = P.slots + i * P.slot_words;
+      u64 key = s[0];
+      if (key != GQ_EMPTY_KEY) { c = gq_make_cand(P, s, key, i); want = true; }
+    }
+    GqCand worst = gq_cand_shfl(mine, 31);
+    want = want && gq_better(c, worst);
+    gq_list_feed(mine, c, want, lane);
+  }
+  GqCand* out = (GqCand*)P.scratch;
+  out[gw * 32 + lane] = mine;
+}
+// pass 2: one warp merges all lists and writes the first min(k, ngroups) groups in order.
+__global__ void __launch_bounds__(32) gq_k_topk_merge(const __grid_constant__ GqFinaliseParams P, i64 nlists) {
+  if (*(volatile int*)P.err != 0) return;
+  const int lane = threadIdx.x;
+  const GqCand* in = (const GqCand*)P.scratch;
+  GqCand mine; mine.valid = 0; mine.val = 0; mine.k0 = 0; mine.k1 = 0; mine.slot = -1;
+  for (i64 l = 0; l < nlists; ++l) {
+    GqCand c = in[l * 32 + lane];
+    GqCand worst = gq_cand_shfl(mine, 31);
+    bool want = c.valid && gq_better(c, worst);
+    gq_list_feed(mine, c, want, lane);
+  }
+  unsigned have = __ballot_sync(0xffffffffu, mine.valid != 0);
+  int n = min(__popc(have), P.topk);
+  if (lane < n) {
+    if (lane < P.out_capacity) {
+      const u64* s = mine.slot == -2 ? P.side : P.slots + mine.slot * P.slot_words;
+      gq_emit_group(P, s, mine.slot == -2 ? GQ_EMPTY_KEY : s[0], lane);
+    } else atomicCAS(P.err, 0, (int)GQ_ERR_CAPACITY);
+  }
+  if (lane == 0) *P.out_n = n;
+}
+
+size_t gq_topk_scratch_bytes_impl() { return sizeof(GqCand) * 32 * GQ_TOPK_BLOCKS * GQ_TOPK_WARPS; }
+
+cudaError_t gq_launch_finalise(cudaStream_t s, const GqFinaliseParams& p, int num_sms, int* nlaunches) {
+  if (p.topk > 0) {
+    gq_k_topk_scan<<<GQ_TOPK_BLOCKS, GQ_TOPK_WARPS * 32, 0, s>>>(p);
+    gq_k_topk_merge<<<1, 32, 0, s>>>(p, (i64)GQ_TOPK_BLOCKS * GQ_TOPK_WARPS);
+    *nlaunches = 2;
+  } else {
+    i64 nb = (p.capacity + GQ_FIN_THREADS * GQ_FIN_PER - 1) / (GQ_FIN_THREADS * GQ_FIN_PER);
+    int blocks = (int)std::max<i64>(1, std::min<i64>(nb, (i64)num_sms * 8));
+    gq_k_finalise<<<blocks, GQ_FIN_THREADS, 0, s>>>(p);
+    *nlaunches = 1;
+  }
+  return cudaGetLastError();
+}
+
+// ------------------------------------------------------------------------------------------------ read probe
+// Read-only streaming sum: what a pure scan can reach on this box (MEASURED_PEAKS is a copy).
+__global__ void __launch_bounds__(512) gq_k_read_probe(const ulonglong2* __restrict__ p, i64 n16, u64* out) {
+  u64 acc = 0;
+  const i64 stride = (i64)gridDim.x * blockDim.x;
+  i64 i = (i64)blockIdx.x * blockDim.x + threadIdx.x;
+  for (; i + 3 * stride < n16; i += 4 * stride) {
+    ulonglong2 a = p[i], b = p[i + stride], c = p[i + 2 * stride], d = p[i + 3 * stride];
+    acc += a.x + a.y + b.x + b.y + c.x + c.y + d.x + d.y;
+  }
+  for (; i < n16; i += stride) { ulonglong2 a = p[i]; acc += a.x + a.y; }
+  for (int o = 16; o > 0; o >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, o);
+  if ((threadIdx.x & 31) == 0 && acc) atomicAdd(out, acc);
+}
+cudaError_t gq_launch_read_probe(cudaStream_t s, const void* data, size_t bytes, u64* out, int num_sms) {
+  cudaError_t e = cudaMemsetAsync(out, 0, 8, s);
+  if (e != cudaSuccess) return e;
+  gq_k_read_probe<<<num_sms * 4, 512, 0, s>>>((const ulonglong2*)data, (i64)(bytes / 16), out);
+  return cudaGetLastError();
+}

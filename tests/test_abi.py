@@ -1,0 +1,78 @@
+"""CPU-only checks of the boundary: libgq.so loads, exports every symbol include/gq.h declares, validates arguments
+that need no device, and the plan compiler emits sm_100a kernels for the five benchmark plan shapes (no GPU needed)."""
+import ctypes as C
+import os
+import re
+
+import pytest
+
+from paper_2606_24647_b200 import build as gqbuild
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+@pytest.fixture(scope="module")
+def gq():
+    gqbuild.build()
+    from paper_2606_24647_b200 import gq as m
+    return m
+
+
+def test_exports_every_declared_symbol(gq):
+    hdr = open(os.path.join(ROOT, "include", "gq.h")).read()
+    hdr = re.sub(r"/\*.*?\*/", "", hdr, flags=re.S)
+    declared = sorted(set(re.findall(r"\b(gq_[a-z_0-9]+)\s*\(", hdr)))
+    assert declared, "no declarations parsed"
+    L = gq.lib()
+    missing = [s for s in declared if not hasattr(L, s)]
+    assert not missing, missing
+    assert sorted(gq.SYMBOLS) == declared
+
+
+def test_status_strings_and_workspace_queries(gq):
+    L = gq.lib()
+    assert L.gq_status_str(0) == b"GQ_OK" and L.gq_status_str(3) == b"GQ_ERR_CAPACITY"
+    n = C.c_size_t()
+    assert L.gq_hash_build_workspace(7_480_000, 0, C.byref(n)) == 0
+    assert n.value >= (1 << 24) * 8                       # C3: 2^24 key-only slots
+    assert L.gq_hash_build_workspace(10, 1, C.byref(n)) == 0 and n.value >= 1024 * 16
+    assert L.gq_hash_build_workspace(-1, 0, C.byref(n)) == 1
+    assert L.gq_hash_build_workspace(10, 9, C.byref(n)) == 1
+    assert L.gq_hash_aggregate_workspace(50_000_000, 1, 5, C.byref(n)) == 0
+    assert n.value >= (1 << 26) * 48                      # C5: 2^26 slots of key + 5 aggregates
+    assert L.gq_hash_aggregate_workspace(0, 1, 5, C.byref(n)) == 1
+    assert L.gq_topk_scratch_bytes() > 0
+
+
+def test_plan_compiler_emits_sm100_tma_kernels(gq, tmp_path):
+    I8, I32, I64 = gq.I8, gq.I32, gq.I64
+    col = lambda i: ("col", i)
+    L = gq.lib()
+    L.gq_set_kernel_cache_dir(str(tmp_path).encode())
+    try:
+        path = gq.precompile_pipeline([I32, I64, I64, I64], 60_000_000,
+                                      preds=[(0, "range_co", 730, 1095), (1, "range_cc", 5, 7), (2, "lt", 24)],
+                                      exprs=[[col(3), col(1), ("mul",)]], keys=[], aggs=[("sum", 0), ("count",)])
+        assert os.path.exists(path) and os.path.exists(path.replace(".cubin", ".cu"))
+        src = open(path.replace(".cubin", ".cu")).read()
+        assert "cp.async.bulk.shared::cluster.global.mbarrier" in src and "gq_pass" in src
+        blob = open(path, "rb").read()
+        assert blob[:4] == b"\x7fELF" and b"gq_scan" in blob
+        # malformed plans are rejected at plan time
+        with pytest.raises(gq.GqError):
+            gq.precompile_pipeline([I32], 10, exprs=[[("add",)]], aggs=[("sum", 0)])
+        with pytest.raises(gq.GqError):
+            gq.precompile_pipeline([I32], 10, preds=[(3, "lt", 1)], aggs=[("count",)])
+        with pytest.raises(gq.GqError):   # i64 + i32 key tuple needs a declared dependent key (S17)
+            gq.precompile_pipeline([I64, I32], 10, keys=[0, 1], aggs=[("count",)], max_groups=100)
+        gq.precompile_pipeline([I64, I32], 10, keys=[0, 1], ndependent=1, aggs=[("count",)], max_groups=100)
+    finally:
+        L.gq_set_kernel_cache_dir(None)
+
+
+def test_no_device_context_fails_loudly(gq):
+    import torch
+    if torch.cuda.is_available():
+        pytest.skip("GPU present")
+    with pytest.raises(RuntimeError):
+        gq.Context()
