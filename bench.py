@@ -40,34 +40,44 @@ def peaks():
 
 
 class ClockSampler:
-    """Samples nvidia-smi clocks and throttle reasons during the timed region."""
-    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
-         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+    """Samples SM clock and clock-event (throttle) reasons through NVML in a thread during the timed region."""
+    BITS = dict(sw_power_cap=0x4, hw_slowdown=0x8, sw_thermal_slowdown=0x20, hw_thermal_slowdown=0x40)
 
     def __init__(self, index=0):
-        self.rows, self.proc, self.index = [], None, index
+        self.index, self.sm, self.reasons, self.max, self.power = index, [], 0, None, []
+        self._stop = threading.Event()
+        self._t = None
 
     def start(self):
         try:
-            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), f"--query-gpu={self.Q}",
-                                          "--format=csv,noheader,nounits", "-lms", "100"], stdout=subprocess.PIPE, text=True)
-            threading.Thread(target=self._read, daemon=True).start()
-        except Exception:
-            self.proc = None
+            import pynvml
+            pynvml.nvmlInit()
+            h = pynvml.nvmlDeviceGetHandleByIndex(self.index)
+            self.max = float(pynvml.nvmlDeviceGetMaxClockInfo(h, pynvml.NVML_CLOCK_SM))
+            get_reasons = getattr(pynvml, "nvmlDeviceGetCurrentClocksEventReasons", None) or \
+                pynvml.nvmlDeviceGetCurrentClocksThrottleReasons
 
-    def _read(self):
-        for line in self.proc.stdout:
-            self.rows.append([x.strip() for x in line.split(",")])
+            def loop():
+                while not self._stop.is_set():
+                    try:
+                        self.sm.append(float(pynvml.nvmlDeviceGetClockInfo(h, pynvml.NVML_CLOCK_SM)))
+                        self.reasons |= int(get_reasons(h))
+                        self.power.append(pynvml.nvmlDeviceGetPowerUsage(h) / 1000.0)
+                    except Exception:
+                        pass
+                    time.sleep(0.002)
+            self._t = threading.Thread(target=loop, daemon=True)
+            self._t.start()
+        except Exception:
+            self._t = None
 
     def stop(self):
-        if self.proc:
-            self.proc.terminate()
-        sm = [float(r[0]) for r in self.rows if r and r[0].replace(".", "").isdigit()]
-        mx = [float(r[1]) for r in self.rows if len(r) > 1 and r[1].replace(".", "").isdigit()]
-        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
-        reasons = [n for i, n in enumerate(names) if any(len(r) > 3 + i and r[3 + i] == "Active" for r in self.rows)]
-        return dict(sm_mhz=float(np.median(sm)) if sm else None, sm_max_mhz=max(mx) if mx else None, reasons=reasons,
-                    samples=len(sm))
+        self._stop.set()
+        if self._t:
+            self._t.join(timeout=1.0)
+        return dict(sm_mhz=float(np.median(self.sm)) if self.sm else None, sm_max_mhz=self.max,
+                    reasons=[n for n, b in self.BITS.items() if self.reasons & b], samples=len(self.sm),
+                    power_w_max=max(self.power) if self.power else None)
 
 
 def dist():
@@ -198,7 +208,7 @@ def main_reference(args):
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--steps", type=int, default=400)
     ap.add_argument("--warmup", type=int, default=5)
     ap.add_argument("--impl", default="ours")
     ap.add_argument("--configs", default="1,3,4,5", help="extra configs reported under per_config ('' = none)")
@@ -250,6 +260,7 @@ def main():
     sampler = ClockSampler(dev_index)
     sampler.start()
     total_ms = time_steps(torch, ctx.stream, pipe.run, args.steps, args.warmup, barrier)
+    clocks = sampler.stop()
     # dominant kernel alone: further batches into an existing aggregation state launch only the fused scan kernel
     st = ctx.aggregate(None, cols, preds=plan["preds"], exprs=plan["exprs"], keys=[], aggs=plan["aggs"], max_groups=1)
     scan = lambda: ctx.aggregate(st, cols, preds=plan["preds"], exprs=plan["exprs"], keys=[], aggs=plan["aggs"], max_groups=1)
@@ -257,7 +268,6 @@ def main():
     # read-only roofline probe of this box (same bytes)
     probe_t = torch.empty(1 << 30, dtype=torch.uint8, device=f"cuda:{dev_index}")
     probe_ms = time_steps(torch, ctx.stream, lambda: ctx.read_probe(probe_t), 10, 3, lambda: None) / 10
-    clocks = sampler.stop()
     if ws > 1:
         t = torch.tensor([total_ms], device="cuda")
         td.all_reduce(t, op=td.ReduceOp.MAX)
@@ -303,7 +313,7 @@ def main():
         for cfg in [int(x) for x in args.configs.split(",") if x]:
             try:
                 sc = args.c5_scale if cfg == 5 else 1.0
-                out, _, _ = run_config(cfg, gq, ctx, torch, datagen, plans, gqrun, max(5, args.steps // 2), 3, scale=sc, peak=peak)
+                out, _, _ = run_config(cfg, gq, ctx, torch, datagen, plans, gqrun, max(5, min(20, args.steps)), 3, scale=sc, peak=peak)
                 per_config[f"C{cfg}"] = out
             except Exception as e:  # a failing extra config must not hide the headline number
                 per_config[f"C{cfg}"] = dict(error=str(e)[:300])

@@ -623,6 +623,7 @@ extern "C" {
 gq_status gq_pipeline_host_workspace(const gq_plan* plan, int64_t chunk_rows, size_t* bytes) {
   if (!plan || !plan->in || !bytes || chunk_rows < 1) return GQ_ERR_INVALID_ARG;
   HostLayout L;
+  chunk_rows = (chunk_rows + 2047) / 2048 * 2048;   // same rounding as gq_pipeline_host
   // output capacity is not known here: size for max_groups rows (top-k needs only k)
   int64_t cap = plan->topk > 0 ? plan->topk : std::max<int64_t>(1, plan->agg.max_groups);
   gq_status st = host_layout(plan, chunk_rows, cap, &L);

@@ -82,12 +82,13 @@ def test_config_small(ctx, cfg, scale):
         assert int(got["cols"][2].sum()) == exp.input_rows      # join cardinality = sum of COUNT (I2)
 
 
-def test_clustered_fact_same_result(ctx):
+def test_clustered_fact_variant(ctx):
     a = datagen.make_config(3, scale=0.01)
     b = datagen.make_config(3, scale=0.01, clustered=True)
-    _, ga = check(plans.plan_c3(a), ctx)
-    _, gb = check(plans.plan_c3(b), ctx)
-    assert np.array_equal(ga["cols"][0], gb["cols"][0]) and np.array_equal(ga["cols"][2], gb["cols"][2])
+    # same fk multiset in a different row order (the other fact columns are drawn by row index, so the two results
+    # differ from each other; each must equal the oracle's on its own table)
+    check(plans.plan_c3(a), ctx)
+    check(plans.plan_c3(b), ctx)
 
 
 # ------------------------------------------------------------------ standalone operators
@@ -106,8 +107,7 @@ def test_filter_project_sizes(ctx, n):
     preds = [(1, "range_co", 300, 2000), (0, "ne", 3)]
     exprs = [[("col", 2), ("col", 0), ("mul",), ("col", 1), ("add",)], [("col", 1)], [("const", 7), ("col", 2), ("sub",)]]
     exp = oracle.filter_project([a, b, c], preds, exprs)
-    outs, count = ctx.filter_project(gqrun.dev([a, b, c]) if n else [x.cuda() for x in map(__import__("torch").from_numpy, [a, b, c])],
-                                     preds, exprs)
+    outs, count = ctx.filter_project(gqrun.dev([a, b, c]), preds, exprs)
     ctx.sync()
     k = int(count.item())
     assert k == exp.nrows
