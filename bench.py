@@ -214,6 +214,7 @@ def main():
     ap.add_argument("--configs", default="1,3,4,5", help="extra configs reported under per_config ('' = none)")
     ap.add_argument("--c5-scale", type=float, default=1.0)
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-headline", action="store_true", help="profiling aid: only the --configs entries, printed as JSON")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3)
     if args.impl == "reference":
@@ -243,6 +244,15 @@ def main():
     dev_index = lr if ws > 1 else 0
     ctx = gq.Context(dev_index)
     peak, peak_src = peaks()
+
+    if args.no_headline:
+        per_config = {}
+        for cfg in [int(x) for x in args.configs.split(",") if x]:
+            sc = args.c5_scale if cfg == 5 else 1.0
+            out, _, _ = run_config(cfg, gq, ctx, torch, datagen, plans, gqrun, args.steps, args.warmup, scale=sc, peak=peak)
+            per_config[f"C{cfg}"] = out
+        print(json.dumps(dict(per_config=per_config)))
+        return
 
     # ---------------- headline: C2, device-resident ----------------
     tabs = datagen.make_config(2)

@@ -33,6 +33,7 @@ struct Gen {
   std::vector<int> cols;              // kernel column -> input column
   std::vector<long long> consts;
   std::vector<int> vcol_probe, vcol_pay;  // virtual column -> (probe step, payload index)
+  std::string sfx;                        // "" (one row at a time) or "[j]" (linear mode: GQ_R rows in register arrays)
 
   Gen(const GqScanSpec& s, std::string* m) : sp(s), msg(m), ncols_in((int)s.in_dtype.size()) {
     compact.assign((size_t)ncols_in, -1);
@@ -61,7 +62,7 @@ struct Gen {
     char b[32];
     if (c < ncols_in) snprintf(b, sizeof b, "v%d", c);
     else snprintf(b, sizeof b, "y%d_%d", vcol_probe[(size_t)(c - ncols_in)], vcol_pay[(size_t)(c - ncols_in)]);
-    return b;
+    return std::string(b) + sfx;
   }
   std::string konst(long long v) {
     if ((int)consts.size() >= GQ_MAXK) { fail("too many constants"); return "0"; }
@@ -71,8 +72,8 @@ struct Gen {
   std::string load(int c) const {                         // typed load of input column c for row slot j
     int kc = compact[(size_t)c];
     std::ostringstream o;
-    o << "const i64 v" << c << " = src.template ld<" << ctype(sp.in_dtype[(size_t)c]) << ">(" << kc << ", GQ_COL_OFF("
-      << kc << "), j);";
+    o << (sfx.empty() ? "const i64 v" : "v") << c << sfx << " = src.template ld<" << ctype(sp.in_dtype[(size_t)c]) << ">(" << kc
+      << ", GQ_COL_OFF(" << kc << "), j);";
     return o.str();
   }
   bool expr(const std::vector<gq_xtok>& toks, std::string* out) {
@@ -97,6 +98,170 @@ struct Gen {
   }
 };
 }  // namespace
+
+
+// ---- key expression shared by both modes: one hashed 64-bit word (+ optional dependent column) ----
+static gq_status key_exprs(Gen& g, const GqScanSpec& sp, std::string* keyx, std::string* depx, std::string* msg) {
+  const int nk = (int)sp.key_cols.size();
+  if (nk < 1 || nk > GQ_MAX_KEYS || sp.ndep < 0 || sp.ndep >= nk) { if (msg) *msg = "bad key columns"; return GQ_ERR_INVALID_ARG; }
+  if (nk - sp.ndep == 1) *keyx = g.val(sp.key_cols[0]);
+  else {  // two hashed keys packed into one 64-bit word: key0 in the low bits
+    auto dt = [&](int c) { return c < g.ncols_in ? sp.in_dtype[(size_t)c]
+                                                  : sp.probes[(size_t)g.vcol_probe[(size_t)(c - g.ncols_in)]].pay_dtype[g.vcol_pay[(size_t)(c - g.ncols_in)]]; };
+    int b0 = 8 * gq_dtype_bytes(dt(sp.key_cols[0])), b1 = 8 * gq_dtype_bytes(dt(sp.key_cols[1]));
+    if (b0 + b1 > 64) { if (msg) *msg = "packed key wider than 64 bits: declare a dependent key (ndependent)"; return GQ_ERR_UNSUPPORTED; }
+    char buf[256];
+    snprintf(buf, sizeof buf, "(i64)((((u64)%s) & 0x%llxULL) | ((((u64)%s) & 0x%llxULL) << %d))", g.val(sp.key_cols[0]).c_str(),
+             (unsigned long long)((b0 == 64) ? ~0ULL : ((1ULL << b0) - 1)), g.val(sp.key_cols[1]).c_str(),
+             (unsigned long long)((1ULL << b1) - 1), b0);
+    *keyx = buf;
+  }
+  if (sp.ndep == 1) *depx = g.val(sp.key_cols[(size_t)nk - 1]);
+  return GQ_OK;
+}
+
+// ---- linear mode: gq_tile processes the GQ_R rows of a thread step by step (see gq_codegen) ----
+static gq_status emit_linear(Gen& g, const GqScanSpec& sp, std::ostringstream& o, std::string* msg) {
+  g.sfx = "[j]";
+  const int nprobe = (int)sp.probes.size();
+  const int nagg = (int)sp.aggs.size();
+  const char* LOOP = "#pragma unroll\n  for (int j = 0; j < GQ_R; ++j) ";
+  o << "template <class Src> __device__ __forceinline__ void gq_tile(const GqParams& P, const Src& src, GqCtx& cx, int nvalid, bool full) {\n";
+  o << "  bool live[GQ_R];\n";
+  for (int c : g.cols) o << "  i64 v" << c << "[GQ_R];\n";
+  // ---- filter: all rows first, so the shared-memory loads of the GQ_R rows overlap ----
+  o << "  " << LOOP << "{\n    live[j] = full || j < nvalid;\n";
+  std::vector<bool> loaded(g.compact.size(), false);
+  for (const gq_pred& p : sp.preds) {
+    o << "    if (live[j]) { ";
+    if (!loaded[(size_t)p.col]) { o << g.load(p.col) << " "; loaded[(size_t)p.col] = true; }
+    std::string v = g.val(p.col), c;
+    const std::string klo = g.konst(p.lo);
+    const std::string khi = (p.op == GQ_RANGE_CO || p.op == GQ_RANGE_CC) ? g.konst(p.hi) : std::string();
+    switch (p.op) {
+      case GQ_LT: c = v + " < " + klo; break;
+      case GQ_LE: c = v + " <= " + klo; break;
+      case GQ_GT: c = v + " > " + klo; break;
+      case GQ_GE: c = v + " >= " + klo; break;
+      case GQ_EQ: c = v + " == " + klo; break;
+      case GQ_NE: c = v + " != " + klo; break;
+      case GQ_RANGE_CO: c = v + " >= " + klo + " && " + v + " < " + khi; break;
+      case GQ_RANGE_CC: c = v + " >= " + klo + " && " + v + " <= " + khi; break;
+      default: if (msg) *msg = "unknown comparison"; return GQ_ERR_INVALID_ARG;
+    }
+    o << "live[j] = (" << c << "); }\n";
+  }
+  o << "  }\n";
+  // ---- remaining input columns of surviving rows ----
+  {
+    bool any = false;
+    for (int c : g.cols) any = any || !loaded[(size_t)c];
+    if (any) {
+      o << "  " << LOOP << "if (live[j]) {\n";
+      for (int c : g.cols) if (!loaded[(size_t)c]) o << "    " << g.load(c) << "\n";
+      o << "  }\n";
+    }
+  }
+  // ---- probe steps: issue the first slot read of every row, then resolve ----
+  for (int s = 0; s < nprobe; ++s) {
+    const GqProbeSpec& ps = sp.probes[(size_t)s];
+    const int sw = ps.slot_words;
+    const std::string S = std::to_string(s), key = g.val(ps.key_col);
+    o << "  const GqTableDev& T" << S << " = P.probe[" << S << "];\n";
+    o << "  u64 pi" << S << "[GQ_R], pk" << S << "[GQ_R], pw" << S << "[GQ_R];\n";
+    for (int p = 0; p < ps.npayload; ++p) o << "  i64 y" << S << "_" << p << "[GQ_R];\n";
+    o << "  " << LOOP << "{\n    pi" << S << "[j] = 0; pk" << S << "[j] = GQ_EMPTY; pw" << S << "[j] = 0;\n";
+    o << "    if (live[j] && (u64)" << key << " != GQ_EMPTY) {\n";
+    o << "      pi" << S << "[j] = gq_hash(" << key << ", T" << S << ".shift);\n";
+    if (sw == 2) o << "      gq_ld128(T" << S << ".slots + pi" << S << "[j] * 2, pk" << S << "[j], pw" << S << "[j]);\n";
+    else o << "      pk" << S << "[j] = __ldg(T" << S << ".slots + pi" << S << "[j] * " << sw << ");\n";
+    o << "    }\n  }\n";
+    o << "  " << LOOP << "if (live[j]) {\n";
+    o << "    if ((u64)" << key << " == GQ_EMPTY) {   // reserved key pattern: unique table => at most one side entry (S14)\n";
+    o << "      if (T" << S << ".header[1] > 0) {";
+    for (int p = 0; p < ps.npayload; ++p) o << " y" << S << "_" << p << "[j] = (i64)T" << S << ".side[" << (1 + p) << "];";
+    o << " } else live[j] = false;\n    } else {\n";
+    o << "      u64 i = pi" << S << "[j], kw = pk" << S << "[j], w = pw" << S << "[j];\n";
+    o << "      for (u64 n = 0; kw != (u64)" << key << " && kw != GQ_EMPTY && n < T" << S << ".mask; ++n) {\n";
+    o << "        i = (i + 1) & T" << S << ".mask;\n";
+    if (sw == 2) o << "        gq_ld128(T" << S << ".slots + i * 2, kw, w);\n";
+    else o << "        kw = __ldg(T" << S << ".slots + i * " << sw << ");\n";
+    o << "      }\n";
+    o << "      if (kw != (u64)" << key << ") live[j] = false;\n      else {";
+    for (int p = 0; p < ps.npayload; ++p) {
+      if (sw == 2) o << " y" << S << "_" << p << "[j] = (i64)w;";
+      else o << " y" << S << "_" << p << "[j] = (i64)__ldg(T" << S << ".slots + i * " << sw << " + " << (1 + p) << ");";
+    }
+    o << " (void)w; }\n    }\n  }\n";
+  }
+  // ---- projection ----
+  if (!sp.exprs.empty()) {
+    for (size_t e = 0; e < sp.exprs.size(); ++e) o << "  i64 e" << e << "[GQ_R];\n";
+    o << "  " << LOOP << "if (live[j]) {\n";
+    for (size_t e = 0; e < sp.exprs.size(); ++e) {
+      std::string x;
+      if (!g.expr(sp.exprs[e], &x)) return GQ_ERR_INVALID_ARG;
+      o << "    e" << e << "[j] = " << x << ";\n";
+    }
+    o << "  }\n";
+  }
+  std::string keyx, depx;
+  if (sp.consumer == GQ_C_LOWCARD || sp.consumer == GQ_C_HIGHCARD) {
+    gq_status st = key_exprs(g, sp, &keyx, &depx, msg);
+    if (st != GQ_OK) return st;
+  }
+  auto aggval = [&](const gq_agg& a) { return a.op == GQ_COUNT_STAR ? std::string("1") : "e" + std::to_string(a.expr) + "[j]"; };
+  switch (sp.consumer) {
+    case GQ_C_GLOBAL:
+      o << "  " << LOOP << "if (live[j]) {\n";
+      for (int a = 0; a < nagg; ++a)
+        o << "    cx.acc[" << a << "] = gq_combine(" << (int)sp.aggs[(size_t)a].op << ", cx.acc[" << a << "], " << aggval(sp.aggs[(size_t)a]) << ");\n";
+      o << "  }\n";
+      break;
+    case GQ_C_LOWCARD:
+      o << "  " << LOOP << "if (live[j]) {\n    const int grp = gq_lc_slot(cx, " << keyx << ", P.err);\n    if (grp >= 0) {\n";
+      for (int a = 0; a < nagg; ++a)
+        o << "      gq_lc_update(" << (int)sp.aggs[(size_t)a].op << ", cx, grp, " << a << ", " << aggval(sp.aggs[(size_t)a]) << ");\n";
+      o << "    }\n  }\n";
+      break;
+    case GQ_C_HIGHCARD:
+      o << "  u64 ti[GQ_R], tk[GQ_R];\n";
+      o << "  " << LOOP << "{\n    ti[j] = 0; tk[j] = GQ_EMPTY;\n    if (live[j] && (u64)" << keyx << " != GQ_EMPTY) {\n";
+      o << "      ti[j] = gq_hash(" << keyx << ", P.target.shift);\n      tk[j] = gq_ld_relaxed(P.target.slots + ti[j] * " << sp.target_sw << ");\n    }\n  }\n";
+      o << "  " << LOOP << "if (live[j]) {\n";
+      o << "    bool won; u64* slot = gq_ht_upsert_pre<" << sp.target_sw << ">(P.target, " << keyx << ", ti[j], tk[j], &won, P.err);\n";
+      o << "    if (slot) {\n";
+      if (sp.ndep == 1) o << "      if (won) slot[1] = (u64)" << depx << ";\n";
+      for (int a = 0; a < nagg; ++a)
+        o << "      gq_red(" << (int)sp.aggs[(size_t)a].op << ", slot + " << (1 + sp.ndep + a) << ", " << aggval(sp.aggs[(size_t)a]) << ");\n";
+      o << "    }\n  }\n";
+      break;
+    case GQ_C_BUILD: {
+      const int np = (int)sp.payload_cols.size();
+      const std::string bk = g.val(sp.build_key_col);
+      o << "  u64 bi[GQ_R], bp[GQ_R];\n";
+      o << "  " << LOOP << "{\n    bi[j] = 0; bp[j] = 0;\n    if (live[j] && (u64)" << bk << " != GQ_EMPTY) {\n";
+      o << "      bi[j] = gq_hash(" << bk << ", P.target.shift);\n      bp[j] = atomicCAS(P.target.slots + bi[j] * " << sp.target_sw
+        << ", GQ_EMPTY, (u64)" << bk << ");\n    }\n  }\n";
+      o << "  " << LOOP << "if (live[j]) {\n    const i64 pay[" << (np > 0 ? np : 1) << "] = {";
+      for (int p = 0; p < np; ++p) o << (p ? ", " : "") << g.val(sp.payload_cols[(size_t)p]);
+      if (np == 0) o << "0";
+      o << "};\n    if (gq_ht_insert_pre<" << sp.target_sw << ", " << np << ">(P.target, " << bk << ", pay, " << (sp.unique ? "true" : "false")
+        << ", bi[j], bp[j], P.err)) ++cx.ninserted;\n  }\n";
+      break;
+    }
+    case GQ_C_MATERIALISE:
+      if (sp.exprs.size() > GQ_MAXOUT) { if (msg) *msg = "too many output columns"; return GQ_ERR_UNSUPPORTED; }
+      o << "  " << LOOP << "if (live[j]) {\n    const i64 orow = gq_reserve_row(P);\n    if (orow >= 0) {\n";
+      for (size_t e = 0; e < sp.exprs.size(); ++e) o << "      P.out[" << e << "][orow] = e" << e << "[j];\n";
+      o << "    }\n  }\n";
+      break;
+    default: if (msg) *msg = "unknown consumer"; return GQ_ERR_INVALID_ARG;
+  }
+  o << "}\n\n";
+  g.sfx.clear();
+  return GQ_OK;
+}
 
 gq_status gq_codegen(const GqScanSpec& sp, GqKernelInfo* out, std::string* msg) {
   Gen g(sp, msg);
@@ -184,146 +349,160 @@ gq_status gq_codegen(const GqScanSpec& sp, GqKernelInfo* out, std::string* msg) 
   }
   o << gq_skeleton_a << "\n";
 
-  // ---- 4. gq_pass: the filter ----
-  o << "template <class Src> __device__ __forceinline__ bool gq_pass(const GqParams& P, const Src& src, int j) {\n";
-  {
-    std::vector<bool> loaded(g.compact.size(), false);
-    for (const gq_pred& p : sp.preds) {
-      if (!loaded[(size_t)p.col]) { o << "  " << g.load(p.col) << "\n"; loaded[(size_t)p.col] = true; }
-      std::string v = g.val(p.col), c;
-      const std::string klo = g.konst(p.lo);   // sequenced: lo before hi (operands of + are unsequenced)
-      const std::string khi = (p.op == GQ_RANGE_CO || p.op == GQ_RANGE_CC) ? g.konst(p.hi) : std::string();
-      switch (p.op) {
-        case GQ_LT: c = v + " < " + klo; break;
-        case GQ_LE: c = v + " <= " + klo; break;
-        case GQ_GT: c = v + " > " + klo; break;
-        case GQ_GE: c = v + " >= " + klo; break;
-        case GQ_EQ: c = v + " == " + klo; break;
-        case GQ_NE: c = v + " != " + klo; break;
-        case GQ_RANGE_CO: c = v + " >= " + klo + " && " + v + " < " + khi; break;
-        case GQ_RANGE_CC: c = v + " >= " + klo + " && " + v + " <= " + khi; break;
-        default: if (msg) *msg = "unknown comparison"; return GQ_ERR_INVALID_ARG;
+  // Linear mode: every probed table has unique keys, so a row yields at most one output row and the GQ_R rows of a
+  // thread can advance through the steps together, with the first (usually only) slot access of every row issued
+  // before any is consumed (memory-level parallelism for the random accesses). Non-unique probes fan rows out and
+  // use the nested one-row-at-a-time form.
+  bool linear = true;
+  for (const GqProbeSpec& ps : sp.probes) linear = linear && ps.unique;
+  o << "#define GQ_LINEAR " << (linear ? 1 : 0) << "\n";
+  if (linear) {
+    gq_status lst = emit_linear(g, sp, o, msg);
+    if (lst != GQ_OK) return lst;
+  } else {
+    // ---- 4. gq_pass: the filter ----
+    o << "template <class Src> __device__ __forceinline__ bool gq_pass(const GqParams& P, const Src& src, int j) {\n";
+    {
+      std::vector<bool> loaded(g.compact.size(), false);
+      for (const gq_pred& p : sp.preds) {
+        if (!loaded[(size_t)p.col]) { o << "  " << g.load(p.col) << "\n"; loaded[(size_t)p.col] = true; }
+        std::string v = g.val(p.col), c;
+        const std::string klo = g.konst(p.lo);   // sequenced: lo before hi (operands of + are unsequenced)
+        const std::string khi = (p.op == GQ_RANGE_CO || p.op == GQ_RANGE_CC) ? g.konst(p.hi) : std::string();
+        switch (p.op) {
+          case GQ_LT: c = v + " < " + klo; break;
+          case GQ_LE: c = v + " <= " + klo; break;
+          case GQ_GT: c = v + " > " + klo; break;
+          case GQ_GE: c = v + " >= " + klo; break;
+          case GQ_EQ: c = v + " == " + klo; break;
+          case GQ_NE: c = v + " != " + klo; break;
+          case GQ_RANGE_CO: c = v + " >= " + klo + " && " + v + " < " + khi; break;
+          case GQ_RANGE_CC: c = v + " >= " + klo + " && " + v + " <= " + khi; break;
+          default: if (msg) *msg = "unknown comparison"; return GQ_ERR_INVALID_ARG;
+        }
+        o << "  if (!(" << c << ")) return false;\n";
       }
-      o << "  if (!(" << c << ")) return false;\n";
     }
-  }
-  o << "  return true;\n}\n\n";
+    o << "  return true;\n}\n\n";
 
-  // ---- 5. gq_body: probes, projection, consumer ----
-  o << "template <class Src> __device__ __forceinline__ void gq_body(const GqParams& P, const Src& src, int j, GqCtx& cx) {\n";
-  {
-    // every input column referenced beyond the filter
-    std::vector<bool> need(g.compact.size(), false);
-    auto mark = [&](int c) { if (c < g.ncols_in) need[(size_t)c] = true; };
-    for (const auto& p : sp.probes) mark(p.key_col);
-    for (const auto& e : sp.exprs) for (const gq_xtok& t : e) if (t.op == GQ_X_COL) mark((int)t.arg);
-    for (int c : sp.key_cols) mark(c);
-    if (sp.consumer == GQ_C_BUILD) { mark(sp.build_key_col); for (int c : sp.payload_cols) mark(c); }
-    for (size_t c = 0; c < need.size(); ++c) if (need[c]) o << "  " << g.load((int)c) << "\n";
-  }
-  std::string ind = "  ";
-  for (int s = 0; s < nprobe; ++s) {   // one open-addressing lookup loop per probe step, nested
-    const GqProbeSpec& ps = sp.probes[(size_t)s];
-    const int sw = ps.slot_words;
-    o << ind << "{ // probe step " << s << "\n";
-    ind += "  ";
-    o << ind << "const GqTableDev& T" << s << " = P.probe[" << s << "];\n";
-    o << ind << "const i64 pk" << s << " = " << g.val(ps.key_col) << ";\n";
-    o << ind << "const bool sd" << s << " = ((u64)pk" << s << " == GQ_EMPTY);\n";
-    o << ind << "i64 ns" << s << " = 0; if (sd" << s << ") ns" << s << " = gq_min(T" << s << ".header[1], GQ_SIDE_SLOTS);\n";
-    o << ind << "u64 i" << s << " = gq_hash(pk" << s << ", T" << s << ".shift);\n";
-    o << ind << "for (u64 n" << s << " = 0; n" << s << " <= T" << s << ".mask; ++n" << s << ") {\n";
-    ind += "  ";
-    o << ind << "const u64* s" << s << "; u64 w" << s << " = 0;\n";
-    o << ind << "if (sd" << s << ") { if ((i64)n" << s << " >= ns" << s << ") break; s" << s << " = T" << s
-      << ".side + n" << s << " * " << sw << ";" << (sw == 2 ? " w" + std::to_string(s) + " = s" + std::to_string(s) + "[1];" : "")
-      << " }\n";
-    o << ind << "else {\n";
-    o << ind << "  s" << s << " = T" << s << ".slots + i" << s << " * " << sw << "; i" << s << " = (i" << s << " + 1) & T"
-      << s << ".mask;\n";
-    if (sw == 2) o << ind << "  u64 kw; gq_ld128(s" << s << ", kw, w" << s << ");\n";
-    else o << ind << "  const u64 kw = __ldg(s" << s << ");\n";
-    o << ind << "  if (kw == GQ_EMPTY) break;\n";
-    o << ind << "  if (kw != (u64)pk" << s << ") continue;\n";
-    o << ind << "}\n";
-    for (int p = 0; p < ps.npayload; ++p) {
-      if (sw == 2) o << ind << "const i64 y" << s << "_" << p << " = (i64)w" << s << ";\n";
-      else o << ind << "const i64 y" << s << "_" << p << " = (i64)__ldg(s" << s << " + " << (1 + p) << ");\n";
+    // ---- 5. gq_body: probes, projection, consumer ----
+    o << "template <class Src> __device__ __forceinline__ void gq_body(const GqParams& P, const Src& src, int j, GqCtx& cx) {\n";
+    {
+      // every input column referenced beyond the filter
+      std::vector<bool> need(g.compact.size(), false);
+      auto mark = [&](int c) { if (c < g.ncols_in) need[(size_t)c] = true; };
+      for (const auto& p : sp.probes) mark(p.key_col);
+      for (const auto& e : sp.exprs) for (const gq_xtok& t : e) if (t.op == GQ_X_COL) mark((int)t.arg);
+      for (int c : sp.key_cols) mark(c);
+      if (sp.consumer == GQ_C_BUILD) { mark(sp.build_key_col); for (int c : sp.payload_cols) mark(c); }
+      for (size_t c = 0; c < need.size(); ++c) if (need[c]) o << "  " << g.load((int)c) << "\n";
     }
-    if (ps.npayload == 0) o << ind << "(void)w" << s << ";\n";
-  }
-  // projection
-  for (size_t e = 0; e < sp.exprs.size(); ++e) {
-    std::string x;
-    if (!g.expr(sp.exprs[e], &x)) return GQ_ERR_INVALID_ARG;
-    o << ind << "const i64 e" << e << " = " << x << ";\n";
-  }
-  // group key
-  std::string keyx, depx;
-  if (sp.consumer == GQ_C_LOWCARD || sp.consumer == GQ_C_HIGHCARD) {
-    const int nk = (int)sp.key_cols.size();
-    if (nk < 1 || nk > GQ_MAX_KEYS || sp.ndep < 0 || sp.ndep >= nk) { if (msg) *msg = "bad key columns"; return GQ_ERR_INVALID_ARG; }
-    if (nk - sp.ndep == 1) keyx = g.val(sp.key_cols[0]);
-    else {  // two hashed keys packed into one 64-bit word: key0 in the low bits
-      auto dt = [&](int c) { return c < g.ncols_in ? sp.in_dtype[(size_t)c]
-                                                    : sp.probes[(size_t)g.vcol_probe[(size_t)(c - g.ncols_in)]].pay_dtype[g.vcol_pay[(size_t)(c - g.ncols_in)]]; };
-      int b0 = 8 * gq_dtype_bytes(dt(sp.key_cols[0])), b1 = 8 * gq_dtype_bytes(dt(sp.key_cols[1]));
-      if (b0 + b1 > 64) { if (msg) *msg = "packed key wider than 64 bits: declare a dependent key (ndependent)"; return GQ_ERR_UNSUPPORTED; }
-      char buf[256];
-      snprintf(buf, sizeof buf, "(i64)((((u64)%s) & 0x%llxULL) | ((((u64)%s) & 0x%llxULL) << %d))", g.val(sp.key_cols[0]).c_str(),
-               (unsigned long long)((b0 == 64) ? ~0ULL : ((1ULL << b0) - 1)), g.val(sp.key_cols[1]).c_str(),
-               (unsigned long long)((1ULL << b1) - 1), b0);
-      keyx = buf;
+    std::string ind = "  ";
+    for (int s = 0; s < nprobe; ++s) {   // one open-addressing lookup loop per probe step, nested
+      const GqProbeSpec& ps = sp.probes[(size_t)s];
+      const int sw = ps.slot_words;
+      o << ind << "{ // probe step " << s << "\n";
+      ind += "  ";
+      o << ind << "const GqTableDev& T" << s << " = P.probe[" << s << "];\n";
+      o << ind << "const i64 pk" << s << " = " << g.val(ps.key_col) << ";\n";
+      o << ind << "const bool sd" << s << " = ((u64)pk" << s << " == GQ_EMPTY);\n";
+      o << ind << "i64 ns" << s << " = 0; if (sd" << s << ") ns" << s << " = gq_min(T" << s << ".header[1], GQ_SIDE_SLOTS);\n";
+      o << ind << "u64 i" << s << " = gq_hash(pk" << s << ", T" << s << ".shift);\n";
+      o << ind << "for (u64 n" << s << " = 0; n" << s << " <= T" << s << ".mask; ++n" << s << ") {\n";
+      ind += "  ";
+      o << ind << "const u64* s" << s << "; u64 w" << s << " = 0;\n";
+      o << ind << "if (sd" << s << ") { if ((i64)n" << s << " >= ns" << s << ") break; s" << s << " = T" << s
+        << ".side + n" << s << " * " << sw << ";" << (sw == 2 ? " w" + std::to_string(s) + " = s" + std::to_string(s) + "[1];" : "")
+        << " }\n";
+      o << ind << "else {\n";
+      o << ind << "  s" << s << " = T" << s << ".slots + i" << s << " * " << sw << "; i" << s << " = (i" << s << " + 1) & T"
+        << s << ".mask;\n";
+      if (sw == 2) o << ind << "  u64 kw; gq_ld128(s" << s << ", kw, w" << s << ");\n";
+      else o << ind << "  const u64 kw = __ldg(s" << s << ");\n";
+      o << ind << "  if (kw == GQ_EMPTY) break;\n";
+      o << ind << "  if (kw != (u64)pk" << s << ") continue;\n";
+      o << ind << "}\n";
+      for (int p = 0; p < ps.npayload; ++p) {
+        if (sw == 2) o << ind << "const i64 y" << s << "_" << p << " = (i64)w" << s << ";\n";
+        else o << ind << "const i64 y" << s << "_" << p << " = (i64)__ldg(s" << s << " + " << (1 + p) << ");\n";
+      }
+      if (ps.npayload == 0) o << ind << "(void)w" << s << ";\n";
     }
-    if (sp.ndep == 1) depx = g.val(sp.key_cols[(size_t)nk - 1]);
-  }
-  auto aggval = [&](const gq_agg& a) { return a.op == GQ_COUNT_STAR ? std::string("1") : "e" + std::to_string(a.expr); };
-  switch (sp.consumer) {
-    case GQ_C_GLOBAL:
-      for (int a = 0; a < nagg; ++a)
-        o << ind << "cx.acc[" << a << "] = gq_combine(" << (int)sp.aggs[(size_t)a].op << ", cx.acc[" << a << "], "
-          << aggval(sp.aggs[(size_t)a]) << ");\n";
-      break;
-    case GQ_C_LOWCARD:
-      o << ind << "const int grp = gq_lc_slot(cx, " << keyx << ", P.err);\n" << ind << "if (grp >= 0) {\n";
-      for (int a = 0; a < nagg; ++a)
-        o << ind << "  gq_lc_update(" << (int)sp.aggs[(size_t)a].op << ", cx, grp, " << a << ", " << aggval(sp.aggs[(size_t)a]) << ");\n";
-      o << ind << "}\n";
-      break;
-    case GQ_C_HIGHCARD:
-      o << ind << "bool won; u64* slot = gq_ht_upsert<" << sp.target_sw << ">(P.target, " << keyx << ", &won, P.err);\n";
-      o << ind << "if (slot) {\n";
-      if (sp.ndep == 1) o << ind << "  if (won) slot[1] = (u64)" << depx << ";\n";
-      for (int a = 0; a < nagg; ++a)
-        o << ind << "  gq_red(" << (int)sp.aggs[(size_t)a].op << ", slot + " << (1 + sp.ndep + a) << ", " << aggval(sp.aggs[(size_t)a]) << ");\n";
-      o << ind << "}\n";
-      break;
-    case GQ_C_BUILD: {
-      const int np = (int)sp.payload_cols.size();
-      o << ind << "const i64 pay[" << (np > 0 ? np : 1) << "] = {";
-      for (int p = 0; p < np; ++p) o << (p ? ", " : "") << g.val(sp.payload_cols[(size_t)p]);
-      if (np == 0) o << "0";
-      o << "};\n";
-      o << ind << "if (gq_ht_insert<" << sp.target_sw << ", " << np << ">(P.target, " << g.val(sp.build_key_col) << ", pay, "
-        << (sp.unique ? "true" : "false") << ", P.err)) ++cx.ninserted;\n";
-      break;
+    // projection
+    for (size_t e = 0; e < sp.exprs.size(); ++e) {
+      std::string x;
+      if (!g.expr(sp.exprs[e], &x)) return GQ_ERR_INVALID_ARG;
+      o << ind << "const i64 e" << e << " = " << x << ";\n";
     }
-    case GQ_C_MATERIALISE:
-      if (sp.exprs.size() > GQ_MAXOUT) { if (msg) *msg = "too many output columns"; return GQ_ERR_UNSUPPORTED; }
-      o << ind << "const i64 orow = gq_reserve_row(P);\n" << ind << "if (orow >= 0) {\n";
-      for (size_t e = 0; e < sp.exprs.size(); ++e) o << ind << "  P.out[" << e << "][orow] = e" << e << ";\n";
+    // group key
+    std::string keyx, depx;
+    if (sp.consumer == GQ_C_LOWCARD || sp.consumer == GQ_C_HIGHCARD) {
+      const int nk = (int)sp.key_cols.size();
+      if (nk < 1 || nk > GQ_MAX_KEYS || sp.ndep < 0 || sp.ndep >= nk) { if (msg) *msg = "bad key columns"; return GQ_ERR_INVALID_ARG; }
+      if (nk - sp.ndep == 1) keyx = g.val(sp.key_cols[0]);
+      else {  // two hashed keys packed into one 64-bit word: key0 in the low bits
+        auto dt = [&](int c) { return c < g.ncols_in ? sp.in_dtype[(size_t)c]
+                                                      : sp.probes[(size_t)g.vcol_probe[(size_t)(c - g.ncols_in)]].pay_dtype[g.vcol_pay[(size_t)(c - g.ncols_in)]]; };
+        int b0 = 8 * gq_dtype_bytes(dt(sp.key_cols[0])), b1 = 8 * gq_dtype_bytes(dt(sp.key_cols[1]));
+        if (b0 + b1 > 64) { if (msg) *msg = "packed key wider than 64 bits: declare a dependent key (ndependent)"; return GQ_ERR_UNSUPPORTED; }
+        char buf[256];
+        snprintf(buf, sizeof buf, "(i64)((((u64)%s) & 0x%llxULL) | ((((u64)%s) & 0x%llxULL) << %d))", g.val(sp.key_cols[0]).c_str(),
+                 (unsigned long long)((b0 == 64) ? ~0ULL : ((1ULL << b0) - 1)), g.val(sp.key_cols[1]).c_str(),
+                 (unsigned long long)((1ULL << b1) - 1), b0);
+        keyx = buf;
+      }
+      if (sp.ndep == 1) depx = g.val(sp.key_cols[(size_t)nk - 1]);
+    }
+    auto aggval = [&](const gq_agg& a) { return a.op == GQ_COUNT_STAR ? std::string("1") : "e" + std::to_string(a.expr); };
+    switch (sp.consumer) {
+      case GQ_C_GLOBAL:
+        for (int a = 0; a < nagg; ++a)
+          o << ind << "cx.acc[" << a << "] = gq_combine(" << (int)sp.aggs[(size_t)a].op << ", cx.acc[" << a << "], "
+            << aggval(sp.aggs[(size_t)a]) << ");\n";
+        break;
+      case GQ_C_LOWCARD:
+        o << ind << "const int grp = gq_lc_slot(cx, " << keyx << ", P.err);\n" << ind << "if (grp >= 0) {\n";
+        for (int a = 0; a < nagg; ++a)
+          o << ind << "  gq_lc_update(" << (int)sp.aggs[(size_t)a].op << ", cx, grp, " << a << ", " << aggval(sp.aggs[(size_t)a]) << ");\n";
+        o << ind << "}\n";
+        break;
+      case GQ_C_HIGHCARD:
+        o << ind << "bool won; u64* slot = gq_ht_upsert<" << sp.target_sw << ">(P.target, " << keyx << ", &won, P.err);\n";
+        o << ind << "if (slot) {\n";
+        if (sp.ndep == 1) o << ind << "  if (won) slot[1] = (u64)" << depx << ";\n";
+        for (int a = 0; a < nagg; ++a)
+          o << ind << "  gq_red(" << (int)sp.aggs[(size_t)a].op << ", slot + " << (1 + sp.ndep + a) << ", " << aggval(sp.aggs[(size_t)a]) << ");\n";
+        o << ind << "}\n";
+        break;
+      case GQ_C_BUILD: {
+        const int np = (int)sp.payload_cols.size();
+        o << ind << "const i64 pay[" << (np > 0 ? np : 1) << "] = {";
+        for (int p = 0; p < np; ++p) o << (p ? ", " : "") << g.val(sp.payload_cols[(size_t)p]);
+        if (np == 0) o << "0";
+        o << "};\n";
+        o << ind << "if (gq_ht_insert<" << sp.target_sw << ", " << np << ">(P.target, " << g.val(sp.build_key_col) << ", pay, "
+          << (sp.unique ? "true" : "false") << ", P.err)) ++cx.ninserted;\n";
+        break;
+      }
+      case GQ_C_MATERIALISE:
+        if (sp.exprs.size() > GQ_MAXOUT) { if (msg) *msg = "too many output columns"; return GQ_ERR_UNSUPPORTED; }
+        o << ind << "const i64 orow = gq_reserve_row(P);\n" << ind << "if (orow >= 0) {\n";
+        for (size_t e = 0; e < sp.exprs.size(); ++e) o << ind << "  P.out[" << e << "][orow] = e" << e << ";\n";
+        o << ind << "}\n";
+        break;
+      default: if (msg) *msg = "unknown consumer"; return GQ_ERR_INVALID_ARG;
+    }
+    for (int s = nprobe - 1; s >= 0; --s) {
+      if (sp.probes[(size_t)s].unique) o << ind << "break;  // unique build keys: first match is the only match\n";
+      ind.resize(ind.size() - 2);
       o << ind << "}\n";
-      break;
-    default: if (msg) *msg = "unknown consumer"; return GQ_ERR_INVALID_ARG;
+      ind.resize(ind.size() - 2);
+      o << ind << "}\n";
+    }
+    o << "}\n\n";
+
   }
-  for (int s = nprobe - 1; s >= 0; --s) {
-    if (sp.probes[(size_t)s].unique) o << ind << "break;  // unique build keys: first match is the only match\n";
-    ind.resize(ind.size() - 2);
-    o << ind << "}\n";
-    ind.resize(ind.size() - 2);
-    o << ind << "}\n";
-  }
-  o << "}\n\n" << gq_skeleton_b << "\n";
+  o << gq_skeleton_b << "\n";
 
   out->source = o.str();
   char hb[32];

@@ -195,6 +195,45 @@ __device__ __forceinline__ u64* gq_ht_upsert(const GqTableDev& T, i64 key, bool*
   return nullptr;
 }
 
+// Variants that continue from a first slot access already issued by the caller (linear mode: the first CAS / key read
+// of all GQ_R rows of a thread are in flight together before any of them is consumed).
+template <int SW, int NPAY>
+__device__ __forceinline__ bool gq_ht_insert_pre(const GqTableDev& T, i64 key, const i64* pay, bool unique, u64 i,
+                                                 u64 prev, int* err) {
+  if ((u64)key == GQ_EMPTY) return gq_ht_insert<SW, NPAY>(T, key, pay, unique, err);
+  for (u64 n = 0; n <= T.mask; ++n) {
+    u64* s = T.slots + i * SW;
+    if (prev == GQ_EMPTY) {
+#pragma unroll
+      for (int p = 0; p < NPAY; ++p) s[1 + p] = (u64)pay[p];
+      return true;
+    }
+    if (unique && prev == (u64)key) { gq_set_err(err, GQ_E_DUPLICATE); return false; }
+    i = (i + 1) & T.mask;
+    prev = atomicCAS(T.slots + i * SW, GQ_EMPTY, (u64)key);
+  }
+  gq_set_err(err, GQ_E_CAPACITY);
+  return false;
+}
+template <int SW>
+__device__ __forceinline__ u64* gq_ht_upsert_pre(const GqTableDev& T, i64 key, u64 i, u64 k, bool* won, int* err) {
+  if ((u64)key == GQ_EMPTY) return gq_ht_upsert<SW>(T, key, won, err);
+  *won = false;
+  for (u64 n = 0; n <= T.mask; ++n) {
+    u64* s = T.slots + i * SW;
+    if (k == (u64)key) return s;
+    if (k == GQ_EMPTY) {
+      u64 prev = atomicCAS(s, GQ_EMPTY, (u64)key);
+      if (prev == GQ_EMPTY) { *won = true; return s; }
+      if (prev == (u64)key) return s;
+    }
+    i = (i + 1) & T.mask;
+    k = gq_ld_relaxed(T.slots + i * SW);
+  }
+  gq_set_err(err, GQ_E_CAPACITY);
+  return nullptr;
+}
+
 // Aggregate update at L2 (RED.ADD / RED.MIN / RED.MAX .64 — results are not read back).
 __device__ __forceinline__ void gq_red(const int OP, u64* p, i64 v) {
   if (OP == GQ_OP_SUM || OP == GQ_OP_COUNT) atomicAdd(p, (u64)v);

@@ -7,6 +7,9 @@
 
 template <class Src>
 __device__ __forceinline__ void gq_process(const GqParams& P, const Src& src, GqCtx& cx, int nvalid_j, bool full) {
+#if GQ_LINEAR
+  gq_tile(P, src, cx, nvalid_j, full);   // generated: the GQ_R rows advance step by step, accesses issued before use
+#else
   // Evaluate the filter for all GQ_R rows first (independent shared-memory loads in flight together), then run the
   // body (probes, projection, consumer) only for passing rows.
   bool pass[GQ_R];
@@ -15,6 +18,7 @@ __device__ __forceinline__ void gq_process(const GqParams& P, const Src& src, Gq
 #pragma unroll
   for (int j = 0; j < GQ_R; ++j)
     if (pass[j]) gq_body(P, src, j, cx);
+#endif
 }
 
 extern "C" __global__ void __launch_bounds__(GQ_NT + 32, 1) gq_scan(const __grid_constant__ GqParams P) {
