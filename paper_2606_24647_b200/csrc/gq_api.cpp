@@ -120,7 +120,7 @@ std::string signature(const GqScanSpec& sp) {
   for (const gq_agg& a : sp.aggs) { put(a.op); put(a.expr); }
   put(sp.lc_cap); put(sp.target_sw); put(sp.build_key_col);
   for (int c : sp.payload_cols) put(c);
-  put(sp.unique);
+  put(sp.unique); put(sp.hot);
   return s;
 }
 void collect_consts(const GqScanSpec& sp, std::vector<long long>* k) {
@@ -420,6 +420,14 @@ int lowcard_cap(int64_t max_groups, int naggs, int ndep) {
   return bytes <= 100 * 1024 ? cap : 0;
 }
 
+// aggregation workspace = table workspace [+ hot list (4 KB) + heavy-hitter sample table] for keyed, non-tiny states
+bool agg_has_hot_area(int64_t max_groups, int nkeys) { return nkeys > 0 && max_groups > 64; }
+size_t agg_ws_bytes(int64_t cap, int sw, int64_t max_groups, int nkeys, size_t* hot_off) {
+  size_t base = align_up(ws_layout(cap, sw, 1).total, 256);
+  if (hot_off) *hot_off = base;
+  return base + (agg_has_hot_area(max_groups, nkeys) ? 4096 + (size_t)GQ_HOT_SLOTS * 16 : 0);
+}
+
 gq_status agg_spec(gq_ctx* ctx, GqScanSpec* sp, const gq_batch* in, const gq_agg_desc* d, int key_bits[2],
                    gq_dtype key_dtype[2]) {
   gq_status st = fill_common(ctx, sp, in, d->preds, d->npred, d->probes, d->nprobes, d->exprs, d->nexpr);
@@ -448,6 +456,9 @@ gq_status agg_spec(gq_ctx* ctx, GqScanSpec* sp, const gq_batch* in, const gq_agg
   sp->target_sw = agg_slot_words(d->ndependent, d->naggs);
   sp->lc_cap = d->nkeys > 0 ? lowcard_cap(d->max_groups, d->naggs, d->ndependent) : 0;
   sp->consumer = d->nkeys == 0 ? GQ_C_GLOBAL : sp->lc_cap > 0 ? GQ_C_LOWCARD : GQ_C_HIGHCARD;
+  // skew handling is compiled in when the group key is one plain input column (so that it can be sampled)
+  sp->hot = sp->consumer == GQ_C_HIGHCARD && d->nkeys == 1 && d->ndependent == 0 && sp->key_cols[0] < in->ncols &&
+            agg_has_hot_area(d->max_groups, d->nkeys);
   return GQ_OK;
 }
 
@@ -460,7 +471,7 @@ extern "C" {
 gq_status gq_hash_aggregate_workspace(int64_t max_groups, int32_t nkeys, int32_t naggs, size_t* bytes) {
   if (!bytes || max_groups < 1 || nkeys < 0 || nkeys > GQ_MAX_KEYS || naggs < 1 || naggs > GQ_MAX_AGGS) return GQ_ERR_INVALID_ARG;
   // slot words do not depend on how many keys are dependent beyond +1 word: size for the worst case (1 dependent)
-  *bytes = ws_layout(agg_capacity(max_groups, nkeys), agg_slot_words(nkeys > 1 ? 1 : 0, naggs), 1).total;
+  *bytes = agg_ws_bytes(agg_capacity(max_groups, nkeys), agg_slot_words(nkeys > 1 ? 1 : 0, naggs), max_groups, nkeys, nullptr);
   return GQ_OK;
 }
 
@@ -481,8 +492,14 @@ gq_status gq_hash_aggregate(gq_ctx* ctx, gq_aggstate** state, void* d_ws, size_t
     const int64_t cap = agg_capacity(d->max_groups, d->nkeys);
     const int sw = sp.target_sw;
     WsLayout w = ws_layout(cap, sw, 1);
-    if (bytes < w.total) return fail(ctx, GQ_ERR_WORKSPACE_TOO_SMALL, "hash-aggregate workspace too small");
+    size_t hot_off = 0;
+    if (bytes < agg_ws_bytes(cap, sw, d->max_groups, d->nkeys, &hot_off))
+      return fail(ctx, GQ_ERR_WORKSPACE_TOO_SMALL, "hash-aggregate workspace too small");
     a = new gq_aggstate();
+    if (agg_has_hot_area(d->max_groups, d->nkeys)) {
+      a->hot = (long long*)((char*)d_ws + hot_off);
+      a->hot_table = (unsigned long long*)((char*)d_ws + hot_off + 4096);
+    }
     a->capacity = cap; a->nkeys = d->nkeys; a->ndep = d->ndependent; a->naggs = d->naggs; a->max_groups = d->max_groups;
     for (int k = 0; k < d->nkeys; ++k) { a->key_dtype[k] = key_dtype[k]; a->key_bits[k] = key_bits[k]; }
     for (int i = 0; i < d->naggs; ++i) a->agg_op[i] = d->aggs[i].op;
@@ -509,6 +526,15 @@ gq_status gq_hash_aggregate(gq_ctx* ctx, gq_aggstate** state, void* d_ws, size_t
   memset(&P, 0, sizeof P);
   P.target = a->dev;
   P.acc = (long long*)(a->dev.side + 1);
+  if (sp.hot && a->hot && in->nrows >= GQ_HOT_MIN_ROWS) {   // heavy-hitter pass over a strided sample of the key column
+    int nl = 0;
+    const gq_column& kc = in->cols[sp.key_cols[0]];
+    cudaError_t e = gq_launch_hot_keys(ctx->stream, kc.data, (int)kc.dtype, in->nrows, a->hot_table, GQ_HOT_SLOTS, GQ_HOT_SAMPLE,
+                                       GQ_HOT_THRESHOLD, a->hot, GQ_HOT_MAX, &nl);
+    if (e != cudaSuccess) return cuda_fail(ctx, e, "heavy-hitter sampling");
+    ctx->launches += nl;
+    P.hot = a->hot;
+  }
   return run_scan(ctx, sp, in, d->probes, &P);
 }
 

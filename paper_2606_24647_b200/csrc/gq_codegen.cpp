@@ -225,6 +225,11 @@ static gq_status emit_linear(Gen& g, const GqScanSpec& sp, std::ostringstream& o
       o << "    }\n  }\n";
       break;
     case GQ_C_HIGHCARD:
+      o << "#if GQ_HOT\n  if (cx.nhot > 0) {\n  " << LOOP << "if (live[j]) {\n      const int hp = gq_hot_find(cx, " << keyx << ");\n"
+        << "      if (hp >= 0) {\n";
+      for (int a = 0; a < nagg; ++a)
+        o << "        gq_hot_update(" << (int)sp.aggs[(size_t)a].op << ", cx, hp, " << a << ", " << aggval(sp.aggs[(size_t)a]) << ");\n";
+      o << "        cx.hot_touched[hp] = 1;\n        live[j] = false;\n      }\n    }\n  }\n#endif\n";
       o << "  u64 ti[GQ_R], tk[GQ_R];\n";
       o << "  " << LOOP << "{\n    ti[j] = 0; tk[j] = GQ_EMPTY;\n    if (live[j] && (u64)" << keyx << " != GQ_EMPTY) {\n";
       o << "      ti[j] = gq_hash(" << keyx << ", P.target.shift);\n      tk[j] = gq_ld_relaxed(P.target.slots + ti[j] * " << sp.target_sw << ");\n    }\n  }\n";
@@ -307,6 +312,10 @@ gq_status gq_codegen(const GqScanSpec& sp, GqKernelInfo* out, std::string* msg) 
     nt = 256;
     cons_bytes = (((sp.lc_cap + 1) * 8 + 8 + 127) / 128 * 128) + 8LL * (sp.lc_cap + 1) * nagg * nt;
   }
+  bool all_unique = true;
+  for (const GqProbeSpec& ps : sp.probes) all_unique = all_unique && ps.unique;
+  const bool use_hot = sp.hot && sp.consumer == GQ_C_HIGHCARD && all_unique;   // linear mode only
+  if (use_hot) cons_bytes = 512 * 8 + 512LL * nagg * 8 + 512 * 4 + 256;
   int r = 4, stages = 0;
   // small inputs: smaller tiles so that every SM still gets several tiles
   if (sp.nrows_hint > 0 && sp.nrows_hint < 148LL * 8 * nt * 4) r = 2;
@@ -327,7 +336,7 @@ gq_status gq_codegen(const GqScanSpec& sp, GqKernelInfo* out, std::string* msg) 
   o << "#define GQ_NCOL " << ncol << "\n#define GQ_NT " << nt << "\n#define GQ_R " << r << "\n#define GQ_STAGES "
     << stages << "\n#define GQ_STAGE_BYTES " << stage_bytes << "\n#define GQ_CONSUMER " << sp.consumer << "\n";
   o << "#define GQ_NAGG " << nagg << "\n#define GQ_LC_CAP " << (sp.lc_cap > 0 ? sp.lc_cap : 1) << "\n#define GQ_TARGET_SW "
-    << (sp.target_sw > 0 ? sp.target_sw : 1) << "\n#define GQ_NDEP " << sp.ndep << "\n#define GQ_EVICT_FIRST 1\n";
+    << (sp.target_sw > 0 ? sp.target_sw : 1) << "\n#define GQ_NDEP " << sp.ndep << "\n#define GQ_EVICT_FIRST 1\n#define GQ_HOT " << (use_hot ? 1 : 0) << "\n";
   {
     long long off = 0, tx = 0;
     std::ostringstream offs, bytes;

@@ -38,6 +38,7 @@ struct GqParams {
   long long* out[GQ_MAXOUT];
   long long out_capacity;
   long long* out_count;
+  const long long* hot;        // HIGHCARD: hot list of this batch (hot[0] = count, hot[1..] = keys) or null
   int* err;
   int pad;
 };
@@ -80,6 +81,8 @@ struct gq_aggstate {
   int64_t max_groups = 0;
   bool lowcard = false;
   int lc_cap = 0;
+  long long* hot = nullptr;            // hot list (in the workspace)
+  unsigned long long* hot_table = nullptr;
   std::string sig;
 };
 
@@ -105,6 +108,7 @@ struct GqScanSpec {
   int build_key_col = 0;                          // BUILD
   std::vector<int> payload_cols;
   bool unique = false;
+  bool hot = false;                               // HIGHCARD: per-CTA shared-memory aggregation of hot keys
   int64_t nrows_hint = 0;                         // tiling heuristic only
 };
 
@@ -143,4 +147,12 @@ cudaError_t gq_launch_init_table(cudaStream_t s, unsigned long long* slots, long
 cudaError_t gq_launch_finalise(cudaStream_t s, const GqFinaliseParams& p, int num_sms, int* nlaunches);
 cudaError_t gq_launch_read_probe(cudaStream_t s, const void* data, size_t bytes, unsigned long long* out, int num_sms);
 size_t gq_topk_scratch_bytes_impl();
+cudaError_t gq_launch_hot_keys(cudaStream_t s, const void* keycol, int dtype, long long nrows, unsigned long long* table,
+                               long long nslots, long long nsample, unsigned long long threshold, long long* hot,
+                               int max_hot, int* nlaunches);
+#define GQ_HOT_MAX 256               // hot keys per batch (shared-memory set of 2*GQ_HOT_MAX positions per CTA)
+#define GQ_HOT_SAMPLE (1LL << 19)    // sampled rows
+#define GQ_HOT_SLOTS (1LL << 20)     // (key,count) sample table slots (16 B each)
+#define GQ_HOT_THRESHOLD 128         // sample count that makes a key hot (share >= 2^-12)
+#define GQ_HOT_MIN_ROWS (1LL << 22)  // batches smaller than this skip the heavy-hitter pass
 #endif

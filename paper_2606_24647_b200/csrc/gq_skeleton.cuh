@@ -68,6 +68,7 @@ struct GqParams {
   i64* out[GQ_MAXOUT];          // MATERIALISE: output columns
   i64 out_capacity;
   i64* out_count;
+  const i64* hot;               // HIGHCARD: hot list of this batch (hot[0] = count, hot[1..] = keys) or null
   int* err;                     // sticky device error
   int pad;
 };
@@ -282,6 +283,10 @@ struct GqCtx {
   i64* lc_acc;                          // LOWCARD: shared accumulators [(GQ_LC_CAP+1) * GQ_NAGG * GQ_NT], lane-private
   int* lc_side_used;
   i64 ninserted;                        // BUILD: rows inserted by this thread
+  i64* hot_keys;                        // HIGHCARD + GQ_HOT: shared set of this batch's hot keys [GQ_HOT_POS]
+  u64* hot_acc;                         //   CTA-shared accumulators [GQ_HOT_POS][GQ_NAGG]
+  int* hot_touched;                     //   entry received at least one row
+  int nhot;
   int t;
 };
 
@@ -307,6 +312,39 @@ __device__ __forceinline__ int gq_lc_slot(GqCtx& cx, i64 key, int* err) {
 __device__ __forceinline__ void gq_lc_update(const int OP, GqCtx& cx, int slot, int a, i64 v) {
   i64* cell = cx.lc_acc + ((slot * GQ_NAGG + a) * GQ_NT + cx.t);
   *cell = gq_combine(OP, *cell, v);
+}
+
+// Hot keys of a skewed high-cardinality group-by: rows whose key is in the batch's hot list
+// are accumulated in CTA-shared memory and flushed to the global table once per CTA, instead of hammering one L2
+// address with hundreds of millions of atomics. 64-bit shared atomics are CAS loops on sm_100 (ATOMS.CAST.SPIN), so
+// SUM/COUNT use two native 32-bit ATOMS.ADD with an explicit carry; MIN/MAX compare first and CAS only to improve.
+#define GQ_HOT_POS 512
+#define GQ_HOT_MAX 256
+__device__ __forceinline__ int gq_hot_find(const GqCtx& cx, i64 key) {
+  u32 i = (u32)gq_hash(key, 64 - 16) & (GQ_HOT_POS - 1);
+  for (int n = 0; n < GQ_HOT_POS; ++n, i = (i + 1) & (GQ_HOT_POS - 1)) {
+    const i64 k = cx.hot_keys[i];
+    if (k == key) return (int)i;
+    if ((u64)k == GQ_EMPTY) return -1;
+  }
+  return -1;
+}
+__device__ __forceinline__ void gq_hot_update(const int OP, GqCtx& cx, int pos, int a, i64 v) {
+  u64* cell = cx.hot_acc + pos * GQ_NAGG + a;
+  if (OP == GQ_OP_SUM || OP == GQ_OP_COUNT) {
+    u32* w = (u32*)cell;
+    const u32 lo = (u32)(u64)v, hi = (u32)((u64)v >> 32);
+    const u32 old = atomicAdd(w, lo);
+    const u32 up = hi + ((u32)(old + lo) < old ? 1u : 0u);   // carry out of the low word belongs to THIS addition
+    if (up) atomicAdd(w + 1, up);
+  } else {
+    i64 cur = *(volatile i64*)cell;
+    while (OP == GQ_OP_MIN ? v < cur : v > cur) {
+      const i64 prev = (i64)atomicCAS(cell, (u64)cur, (u64)v);
+      if (prev == cur) break;
+      cur = prev;
+    }
+  }
 }
 
 // MATERIALISE: ballot/popc compaction — the lanes that reach this point together reserve a contiguous

@@ -52,6 +52,28 @@ extern "C" __global__ void __launch_bounds__(GQ_NT + 32, 1) gq_scan(const __grid
 #pragma unroll
   for (int a = 0; a < GQ_NAGG; ++a) cx.acc[a] = gq_identity(GQ_AGG_OP(a));
 #endif
+#if GQ_HOT
+  cx.hot_keys = (i64*)(gq_smem + GQ_CONS_OFF);
+  cx.hot_acc = (u64*)(cx.hot_keys + GQ_HOT_POS);
+  cx.hot_touched = (int*)(cx.hot_acc + GQ_HOT_POS * GQ_NAGG);
+  cx.nhot = 0;
+  if (P.hot) { const i64 n = P.hot[0]; cx.nhot = (int)(n < GQ_HOT_MAX ? n : GQ_HOT_MAX); }
+  if (cx.nhot > 0) {
+    for (int i = tid; i < GQ_HOT_POS; i += GQ_NT + 32) {
+      cx.hot_keys[i] = (i64)GQ_EMPTY;
+      cx.hot_touched[i] = 0;
+#pragma unroll
+      for (int a = 0; a < GQ_NAGG; ++a) cx.hot_acc[i * GQ_NAGG + a] = (u64)gq_identity(GQ_AGG_OP(a));
+    }
+    __syncthreads();
+    if (tid < cx.nhot) {   // insert this batch's hot keys into the shared set (distinct by construction)
+      const i64 key = P.hot[1 + tid];
+      u32 i = (u32)gq_hash(key, 64 - 16) & (GQ_HOT_POS - 1);
+      for (int n = 0; n < GQ_HOT_POS; ++n, i = (i + 1) & (GQ_HOT_POS - 1))
+        if (atomicCAS((u64*)&cx.hot_keys[i], GQ_EMPTY, (u64)key) == GQ_EMPTY) break;
+    }
+  }
+#endif
   __syncthreads();
 
   if (tid >= GQ_NT) {
@@ -147,6 +169,19 @@ extern "C" __global__ void __launch_bounds__(GQ_NT + 32, 1) gq_scan(const __grid
           gq_red(GQ_AGG_OP(aa), slot + 1 + GQ_NDEP + aa, v);
         }
       }
+    }
+  }
+#endif
+#if GQ_HOT
+  if (cx.nhot > 0) {   // flush the CTA's hot-key partials into the global table (Partial -> Final)
+    gq_consumer_barrier();
+    for (int pos = tid; pos < GQ_HOT_POS; pos += GQ_NT) {
+      if (!cx.hot_touched[pos]) continue;
+      bool won;
+      u64* slot = gq_ht_upsert<GQ_TARGET_SW>(P.target, cx.hot_keys[pos], &won, P.err);
+      if (!slot) continue;
+#pragma unroll
+      for (int a = 0; a < GQ_NAGG; ++a) gq_red(GQ_AGG_OP(a), slot + 1 + GQ_NDEP + a, (i64)cx.hot_acc[pos * GQ_NAGG + a]);
     }
   }
 #endif

@@ -196,20 +196,40 @@ __global__ void __launch_bounds__(GQ_TOPK_WARPS * 32) gq_k_topk_scan(const __gri
     want = want && gq_better(c, worst);
     gq_list_feed(mine, c, want, lane);
   }
-  GqCand* out = (GqCand*)P.scratch;
-  out[gw * 32 + lane] = mine;
+  // merge the block's GQ_TOPK_WARPS lists into one (warp 0), so pass 2 sees one list per block
+  __shared__ GqCand sh[GQ_TOPK_WARPS][32];
+  sh[threadIdx.x >> 5][lane] = mine;
+  __syncthreads();
+  if ((threadIdx.x >> 5) == 0) {
+    for (int w = 1; w < GQ_TOPK_WARPS; ++w) {
+      GqCand c = sh[w][lane];
+      GqCand worst = gq_cand_shfl(mine, 31);
+      gq_list_feed(mine, c, c.valid && gq_better(c, worst), lane);
+    }
+    ((GqCand*)P.scratch)[(i64)blockIdx.x * 32 + lane] = mine;
+  }
 }
-// pass 2: one warp merges all lists and writes the first min(k, ngroups) groups in order.
-__global__ void __launch_bounds__(32) gq_k_topk_merge(const __grid_constant__ GqFinaliseParams P, i64 nlists) {
+// pass 2: one block; every warp merges a strided share of the per-block lists, warp 0 merges the warps' results and
+// writes the first min(k, ngroups) groups in order.
+#define GQ_TOPK_MERGE_WARPS 32
+__global__ void __launch_bounds__(GQ_TOPK_MERGE_WARPS * 32) gq_k_topk_merge(const __grid_constant__ GqFinaliseParams P, i64 nlists) {
   if (*(volatile int*)P.err != 0) return;
-  const int lane = threadIdx.x;
+  __shared__ GqCand sh[GQ_TOPK_MERGE_WARPS][32];
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   const GqCand* in = (const GqCand*)P.scratch;
   GqCand mine; mine.valid = 0; mine.val = 0; mine.k0 = 0; mine.k1 = 0; mine.slot = -1;
-  for (i64 l = 0; l < nlists; ++l) {
+  for (i64 l = warp; l < nlists; l += GQ_TOPK_MERGE_WARPS) {
     GqCand c = in[l * 32 + lane];
     GqCand worst = gq_cand_shfl(mine, 31);
-    bool want = c.valid && gq_better(c, worst);
-    gq_list_feed(mine, c, want, lane);
+    gq_list_feed(mine, c, c.valid && gq_better(c, worst), lane);
+  }
+  sh[warp][lane] = mine;
+  __syncthreads();
+  if (warp != 0) return;
+  for (int w = 1; w < GQ_TOPK_MERGE_WARPS; ++w) {
+    GqCand c = sh[w][lane];
+    GqCand worst = gq_cand_shfl(mine, 31);
+    gq_list_feed(mine, c, c.valid && gq_better(c, worst), lane);
   }
   unsigned have = __ballot_sync(0xffffffffu, mine.valid != 0);
   int n = min(__popc(have), P.topk);
@@ -222,12 +242,12 @@ __global__ void __launch_bounds__(32) gq_k_topk_merge(const __grid_constant__ Gq
   if (lane == 0) *P.out_n = n;
 }
 
-size_t gq_topk_scratch_bytes_impl() { return sizeof(GqCand) * 32 * GQ_TOPK_BLOCKS * GQ_TOPK_WARPS; }
+size_t gq_topk_scratch_bytes_impl() { return sizeof(GqCand) * 32 * GQ_TOPK_BLOCKS; }
 
 cudaError_t gq_launch_finalise(cudaStream_t s, const GqFinaliseParams& p, int num_sms, int* nlaunches) {
   if (p.topk > 0) {
     gq_k_topk_scan<<<GQ_TOPK_BLOCKS, GQ_TOPK_WARPS * 32, 0, s>>>(p);
-    gq_k_topk_merge<<<1, 32, 0, s>>>(p, (i64)GQ_TOPK_BLOCKS * GQ_TOPK_WARPS);
+    gq_k_topk_merge<<<1, GQ_TOPK_MERGE_WARPS * 32, 0, s>>>(p, (i64)GQ_TOPK_BLOCKS);
     *nlaunches = 2;
   } else {
     i64 nb = (p.capacity + GQ_FIN_THREADS * GQ_FIN_PER - 1) / (GQ_FIN_THREADS * GQ_FIN_PER);
@@ -256,5 +276,65 @@ cudaError_t gq_launch_read_probe(cudaStream_t s, const void* data, size_t bytes,
   cudaError_t e = cudaMemsetAsync(out, 0, 8, s);
   if (e != cudaSuccess) return e;
   gq_k_read_probe<<<num_sms * 4, 512, 0, s>>>((const ulonglong2*)data, (i64)(bytes / 16), out);
+  return cudaGetLastError();
+}
+
+// ------------------------------------------------------------------------------------------------ heavy hitters
+// Skew handling for high-cardinality group-by: before the fused scan of a large batch, a strided
+// sample of the group-key column is counted in a small (key,count) table; keys whose sample count reaches the
+// threshold form the batch's hot list. The scan kernel aggregates those keys per CTA in shared memory and flushes
+// them once, so the hottest keys no longer serialise hundreds of millions of same-address L2 atomics. The hot list
+// only steers WHERE an update is accumulated; results do not depend on it.
+__device__ __forceinline__ u64 gq_s_hash(i64 key, int shift) {
+  u64 x = (u64)key;
+  x ^= x >> 32;
+  return (x * 0x9E3779B97F4A7C15ULL) >> shift;
+}
+__global__ void gq_k_hot_sample(const void* keycol, int dtype, i64 nrows, i64 stride, i64 nsample, u64* table, u64 mask,
+                                int shift) {
+  const i64 t = (i64)blockIdx.x * blockDim.x + threadIdx.x;
+  if (t >= nsample) return;
+  const i64 r = t * stride;
+  if (r >= nrows) return;
+  i64 key = dtype == GQ_I8 ? (i64)((const signed char*)keycol)[r] : dtype == GQ_I32 ? (i64)((const int*)keycol)[r]
+                                                                                      : ((const i64*)keycol)[r];
+  if ((u64)key == GQ_EMPTY_KEY) return;
+  u64 i = gq_s_hash(key, shift);
+  for (u64 n = 0; n <= mask; ++n, i = (i + 1) & mask) {
+    u64* s = table + i * 2;
+    u64 k = *(volatile u64*)s;
+    if (k != (u64)key) {
+      if (k != GQ_EMPTY_KEY) continue;
+      u64 prev = atomicCAS(s, GQ_EMPTY_KEY, (u64)key);
+      if (prev != GQ_EMPTY_KEY && prev != (u64)key) continue;
+    }
+    atomicAdd(s + 1, 1ULL);
+    return;
+  }
+}
+// hot[0] = number of hot keys (<= max_hot), hot[1..] = keys
+__global__ void gq_k_hot_select(const u64* table, i64 nslots, u64 threshold, i64* hot, int max_hot) {
+  const i64 i = (i64)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= nslots) return;
+  const u64 k = table[i * 2];
+  if (k == GQ_EMPTY_KEY || table[i * 2 + 1] < threshold) return;
+  i64 idx = (i64)atomicAdd((u64*)hot, 1ULL);
+  if (idx < max_hot) hot[1 + idx] = (i64)k;
+}
+
+cudaError_t gq_launch_hot_keys(cudaStream_t s, const void* keycol, int dtype, i64 nrows, u64* table, i64 nslots,
+                               i64 nsample, u64 threshold, i64* hot, int max_hot, int* nlaunches) {
+  // (key,count) slots: key = EMPTY (0x80..0), count = 0
+  u64 pat[12];
+  for (int i = 0; i < 12; ++i) pat[i] = (i & 1) ? 0 : GQ_EMPTY_KEY;
+  cudaError_t e = gq_launch_init_table(s, table, nslots, 2, pat, table, 0, hot, 0);   // header := hot list head (zeroed)
+  if (e != cudaSuccess) return e;
+  int shift = 64;
+  for (i64 c = 1; c < nslots; c <<= 1) --shift;
+  const i64 stride = nrows / nsample > 0 ? nrows / nsample : 1;
+  gq_k_hot_sample<<<(unsigned)((nsample + 255) / 256), 256, 0, s>>>(keycol, dtype, nrows, stride, nsample, table,
+                                                                   (u64)(nslots - 1), shift);
+  gq_k_hot_select<<<(unsigned)((nslots + 255) / 256), 256, 0, s>>>(table, nslots, threshold, hot, max_hot);
+  *nlaunches = 3;
   return cudaGetLastError();
 }

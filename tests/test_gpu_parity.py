@@ -67,7 +67,7 @@ def test_golden_T1_to_T5(ctx):
 
 
 # ------------------------------------------------------------------ configs at sizes spanning many tiles + ragged tail
-@pytest.mark.parametrize("cfg,scale", [(1, 1.0), (1, 0.0371), (2, 0.0333333), (3, 0.02), (4, 0.02), (5, 0.003)])
+@pytest.mark.parametrize("cfg,scale", [(1, 1.0), (1, 0.0371), (2, 0.0333333), (3, 0.02), (4, 0.02), (5, 0.003), (5, 0.0101)])
 def test_config_small(ctx, cfg, scale):
     t = datagen.make_config(cfg, scale=scale)
     plan = plans.PLANS[cfg](t)
@@ -236,6 +236,22 @@ def test_colliding_keys_and_full_load(ctx):
     plan = dict(table=[keys, np.ones(3072, np.int64)], preds=[], exprs=[[("col", 1)]], keys=[0],
                 aggs=[("sum", 0)], max_groups=3072)
     check(plan, ctx)
+
+
+def test_hot_key_path_negative_values_and_filtered_hot_keys(ctx):
+    # >= 2^22 rows switches the heavy-hitter pass on: skewed keys, negative values (carry logic of the split 32-bit
+    # shared-memory adds), MIN/MAX, and one hot key whose rows are ALL filtered out (it must not appear as a group)
+    rng = np.random.default_rng(11)
+    n = (1 << 22) + 12_345
+    hot = np.array([7, -3, 2**40 + 1, 123456789, 99], dtype=np.int64)
+    keys = np.where(rng.random(n) < 0.6, hot[rng.integers(0, 5, n)], rng.integers(0, 3_000_000, n)).astype(np.int64)
+    v = rng.integers(-2**45, 2**45, n).astype(np.int64)
+    f = rng.integers(0, 100, n).astype(np.int32)
+    f[keys == 99] = 1000                                          # hot key 99 never passes the filter
+    plan = dict(table=[keys, v, f], preds=[(2, "lt", 90)], exprs=[[("col", 1)]], keys=[0],
+                aggs=[("sum", 0), ("min", 0), ("max", 0), ("count",)], max_groups=3_100_000)
+    exp, got = check(plan, ctx)
+    assert 99 not in set(got["cols"][0].tolist()) and 7 in set(got["cols"][0].tolist())
 
 
 def test_empty_and_filtered_out_inputs(ctx):
