@@ -140,6 +140,12 @@ typedef struct {
   int64_t max_groups;  /* capacity bound; also selects the low-cardinality shared-memory path when small */
 } gq_agg_desc;
 gq_status gq_hash_aggregate_workspace(int64_t max_groups, int32_t nkeys, int32_t naggs, size_t* bytes);
+/* Plan-aware size: at least the size above; larger when the plan qualifies for DIRECT aggregation — the single hashed
+ * group key is the key column of a probe step into a GQ_F_UNIQUE_KEYS table (and a dependent key, if any, is a payload
+ * of that table), so a row's group is the table slot it matched and the aggregates live in an array indexed by that
+ * slot (no second hash table; SURVEY §8(d) note on C3). gq_hash_aggregate takes that path when the workspace it is
+ * given is at least this large; the probed table's workspace must then stay alive until the state is finished. */
+gq_status gq_hash_aggregate_workspace_for(const gq_batch* in, const gq_agg_desc* desc, size_t* bytes);
 /* *state == NULL: creates the state in d_workspace and aggregates the batch; else aggregates a further batch. */
 gq_status gq_hash_aggregate(gq_ctx*, gq_aggstate** state, void* d_workspace, size_t bytes, const gq_batch* in,
                             const gq_agg_desc* desc);

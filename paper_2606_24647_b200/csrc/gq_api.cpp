@@ -100,6 +100,21 @@ gq_status fill_common(gq_ctx* ctx, GqScanSpec* sp, const gq_batch* in, const gq_
   return GQ_OK;
 }
 
+// Constants in codegen order (predicate bounds, then expression literals); equal values share one parameter slot
+// (so common subexpressions stay common in the generated code). idx receives the slot of every occurrence: WHICH
+// literals are equal is part of the plan shape, their values are not.
+void collect_consts(const GqScanSpec& sp, std::vector<long long>* k, std::vector<int>* idx = nullptr) {
+  k->clear();
+  auto put = [&](long long v) {
+    size_t i = 0;
+    while (i < k->size() && (*k)[i] != v) ++i;
+    if (i == k->size()) k->push_back(v);
+    if (idx) idx->push_back((int)i);
+  };
+  for (const gq_pred& p : sp.preds) { put(p.lo); if (p.op == GQ_RANGE_CO || p.op == GQ_RANGE_CC) put(p.hi); }
+  for (const auto& e : sp.exprs) for (const gq_xtok& t : e) if (t.op == GQ_X_CONST) put(t.arg);
+}
+
 // Shape signature (no constant values) and the constants in codegen order (predicates, then expression literals).
 int tile_bucket(int64_t nrows) { return nrows <= 0 ? 0 : nrows < 148LL * 8 * 512 * 2 ? 1 : nrows < 148LL * 8 * 512 * 4 ? 2 : 3; }
 std::string signature(const GqScanSpec& sp) {
@@ -118,17 +133,15 @@ std::string signature(const GqScanSpec& sp) {
   for (int c : sp.key_cols) put(c);
   put(sp.ndep);
   for (const gq_agg& a : sp.aggs) { put(a.op); put(a.expr); }
-  put(sp.lc_cap); put(sp.target_sw); put(sp.build_key_col);
+  put(sp.lc_cap); put(sp.lc_key_bits); put(sp.target_sw); put(sp.build_key_col);
   for (int c : sp.payload_cols) put(c);
-  put(sp.unique); put(sp.hot);
+  put(sp.unique); put(sp.hot); put(sp.fused_final); put(sp.direct_step); put(sp.direct_aw); put(sp.direct_touch);
+  s += 'c';
+  std::vector<long long> kv; std::vector<int> ki;
+  collect_consts(sp, &kv, &ki);
+  for (int i : ki) put(i);
   return s;
 }
-void collect_consts(const GqScanSpec& sp, std::vector<long long>* k) {
-  k->clear();
-  for (const gq_pred& p : sp.preds) { k->push_back(p.lo); if (p.op == GQ_RANGE_CO || p.op == GQ_RANGE_CC) k->push_back(p.hi); }
-  for (const auto& e : sp.exprs) for (const gq_xtok& t : e) if (t.op == GQ_X_CONST) k->push_back(t.arg);
-}
-
 struct CachedKernel { GqKernelInfo info; GqKernel k; bool loaded = false; };
 std::mutex g_kmu;
 std::map<std::string, CachedKernel> g_kernels;
@@ -350,6 +363,7 @@ gq_status gq_hash_build(gq_ctx* ctx, gq_table** table, void* d_ws, size_t bytes,
     t->dev.shift = 64 - log2i(cap);
     t->dev.slot_words = sw;
     t->dev.flags = d->flags;
+    t->dev.bshift = sw == 1 ? 2 : sw == 2 ? 1 : 0;   // slots per 32-byte bucket: 4 / 2 / 1
     unsigned long long pat[12];
     for (int i = 0; i < 12; ++i) pat[i] = 0;
     pat[0] = GQ_EMPTY_KEY;
@@ -411,13 +425,12 @@ gq_status gq_table_describe(gq_table** out, const gq_dtype* payload_dtypes, int3
 // ------------------------------------------------------------------------------------------------ HashAggregation
 namespace {
 
-// Shared-memory budget of the low-cardinality path: (lc_cap+1) * naggs * 256 threads * 8 B of private cells.
+// Low-cardinality path: max_groups group cells per consumer thread in shared memory (max_groups * naggs * 8 B per
+// thread); taken when at least 128 consumer threads fit beside a 3-stage ring (checked again by the plan compiler).
 int lowcard_cap(int64_t max_groups, int naggs, int ndep) {
   if (ndep > 0 || max_groups < 1 || max_groups > 64 || naggs < 1) return 0;
-  int cap = 2;
-  while (cap < max_groups) cap <<= 1;
-  long long bytes = 8LL * (cap + 1) * naggs * 256;
-  return bytes <= 100 * 1024 ? cap : 0;
+  long long bytes = 8LL * max_groups * naggs * 128;
+  return bytes <= 120 * 1024 ? (int)max_groups : 0;
 }
 
 // aggregation workspace = table workspace [+ hot list (4 KB) + heavy-hitter sample table] for keyed, non-tiny states
@@ -455,6 +468,7 @@ gq_status agg_spec(gq_ctx* ctx, GqScanSpec* sp, const gq_batch* in, const gq_agg
   }
   sp->target_sw = agg_slot_words(d->ndependent, d->naggs);
   sp->lc_cap = d->nkeys > 0 ? lowcard_cap(d->max_groups, d->naggs, d->ndependent) : 0;
+  sp->lc_key_bits = bits;
   sp->consumer = d->nkeys == 0 ? GQ_C_GLOBAL : sp->lc_cap > 0 ? GQ_C_LOWCARD : GQ_C_HIGHCARD;
   // skew handling is compiled in when the group key is one plain input column (so that it can be sampled)
   sp->hot = sp->consumer == GQ_C_HIGHCARD && d->nkeys == 1 && d->ndependent == 0 && sp->key_cols[0] < in->ncols &&
@@ -464,6 +478,40 @@ gq_status agg_spec(gq_ctx* ctx, GqScanSpec* sp, const gq_batch* in, const gq_agg
 
 int64_t agg_capacity(int64_t max_groups, int nkeys) { return nkeys == 0 ? 0 : table_capacity(max_groups); }
 
+// Direct aggregation (SURVEY §8(d) note on C3): when the single hashed group key is the key column of a probe step
+// into a table with unique keys, a surviving row's group IS the slot it matched, so the aggregate words live in an
+// array indexed by that slot: no second hash table, no key compare, no CAS. A dependent key must be a payload of the
+// same table (read back from it by the finaliser). Returns the probe step or -1.
+struct DirectPlan { int step = -1; int aw = 0; int touch = -1; int dep_pay = -1; int64_t cap = 0; size_t bytes = 0; };
+DirectPlan direct_plan(const GqScanSpec& sp, const gq_agg_desc* d, const gq_batch* in, bool schema_only = false) {
+  DirectPlan dp;
+  if (sp.consumer != GQ_C_HIGHCARD || d->nkeys - d->ndependent != 1 || d->nprobes < 1) return dp;
+  int step = -1;
+  for (int s = 0; s < d->nprobes; ++s)
+    if (d->probes[s].key_col == d->key_cols[0] && d->probes[s].table && (d->probes[s].table->flags & GQ_F_UNIQUE_KEYS) &&
+        (schema_only || !d->probes[s].table->describe_only)) step = s;
+  if (step < 0) return dp;
+  const gq_table* t = d->probes[step].table;
+  if (d->ndependent == 1) {
+    int first = in->ncols;
+    for (int s = 0; s < step; ++s) first += d->probes[s].table->npayload;
+    const int c = d->key_cols[1];
+    if (c < first || c >= first + t->npayload) return dp;
+    dp.dep_pay = c - first;
+  }
+  for (int i = 0; i < d->naggs; ++i) if (d->aggs[i].op == GQ_COUNT_STAR && dp.touch < 0) dp.touch = i;
+  const bool hidden = dp.touch < 0;
+  if (hidden) dp.touch = d->naggs;
+  dp.aw = (int)align_up((size_t)(d->naggs + (hidden ? 1 : 0)), 2);
+  dp.cap = t->capacity;
+  dp.bytes = 256 + (size_t)(dp.cap + 1) * dp.aw * 8;
+  // worthwhile unless the probed table is far larger than a hashed table of max_groups would be
+  const size_t hashed = (size_t)agg_capacity(d->max_groups, d->nkeys) * agg_slot_words(d->ndependent, d->naggs) * 8;
+  if (!schema_only && dp.bytes > 4 * hashed + (1u << 20)) return DirectPlan();
+  dp.step = step;
+  return dp;
+}
+
 }  // namespace
 
 extern "C" {
@@ -472,6 +520,20 @@ gq_status gq_hash_aggregate_workspace(int64_t max_groups, int32_t nkeys, int32_t
   if (!bytes || max_groups < 1 || nkeys < 0 || nkeys > GQ_MAX_KEYS || naggs < 1 || naggs > GQ_MAX_AGGS) return GQ_ERR_INVALID_ARG;
   // slot words do not depend on how many keys are dependent beyond +1 word: size for the worst case (1 dependent)
   *bytes = agg_ws_bytes(agg_capacity(max_groups, nkeys), agg_slot_words(nkeys > 1 ? 1 : 0, naggs), max_groups, nkeys, nullptr);
+  return GQ_OK;
+}
+
+gq_status gq_hash_aggregate_workspace_for(const gq_batch* in, const gq_agg_desc* d, size_t* bytes) {
+  if (!in || !d || !bytes) return GQ_ERR_INVALID_ARG;
+  gq_status st = gq_hash_aggregate_workspace(d->max_groups, d->nkeys, d->naggs, bytes);
+  if (st != GQ_OK) return st;
+  gq_ctx tmp;
+  GqScanSpec sp;
+  int kb[2]; gq_dtype kd[2] = {GQ_I64, GQ_I64};
+  st = agg_spec(&tmp, &sp, in, d, kb, kd);
+  if (st != GQ_OK) return st;
+  DirectPlan dp = direct_plan(sp, d, in);
+  if (dp.step >= 0) *bytes = std::max(*bytes, dp.bytes);
   return GQ_OK;
 }
 
@@ -485,47 +547,75 @@ gq_status gq_hash_aggregate(gq_ctx* ctx, gq_aggstate** state, void* d_ws, size_t
   gq_dtype key_dtype[2] = {GQ_I64, GQ_I64};
   st = agg_spec(ctx, &sp, in, d, key_bits, key_dtype);
   if (st != GQ_OK) return st;
-  GqScanSpec sig_sp = sp; sig_sp.nrows_hint = 0;
   gq_aggstate* a = *state;
   if (!a) {
     if (!d_ws || !aligned(d_ws, 256)) return fail(ctx, GQ_ERR_INVALID_ARG, "bad workspace");
-    const int64_t cap = agg_capacity(d->max_groups, d->nkeys);
-    const int sw = sp.target_sw;
-    WsLayout w = ws_layout(cap, sw, 1);
-    size_t hot_off = 0;
-    if (bytes < agg_ws_bytes(cap, sw, d->max_groups, d->nkeys, &hot_off))
-      return fail(ctx, GQ_ERR_WORKSPACE_TOO_SMALL, "hash-aggregate workspace too small");
+    DirectPlan dp = direct_plan(sp, d, in);
+    if (dp.step >= 0 && bytes < dp.bytes) dp = DirectPlan();   // workspace sized by the table-agnostic query: hashed path
     a = new gq_aggstate();
-    if (agg_has_hot_area(d->max_groups, d->nkeys)) {
-      a->hot = (long long*)((char*)d_ws + hot_off);
-      a->hot_table = (unsigned long long*)((char*)d_ws + hot_off + 4096);
-    }
-    a->capacity = cap; a->nkeys = d->nkeys; a->ndep = d->ndependent; a->naggs = d->naggs; a->max_groups = d->max_groups;
+    a->nkeys = d->nkeys; a->ndep = d->ndependent; a->naggs = d->naggs; a->max_groups = d->max_groups;
     for (int k = 0; k < d->nkeys; ++k) { a->key_dtype[k] = key_dtype[k]; a->key_bits[k] = key_bits[k]; }
     for (int i = 0; i < d->naggs; ++i) a->agg_op[i] = d->aggs[i].op;
-    a->lowcard = sp.consumer == GQ_C_LOWCARD; a->lc_cap = sp.lc_cap;
-    a->dev.slots = (unsigned long long*)((char*)d_ws + w.slots_off);
-    a->dev.mask = cap > 0 ? (unsigned long long)(cap - 1) : 0;
-    a->dev.header = (long long*)d_ws;
-    a->dev.side = (unsigned long long*)((char*)d_ws + w.side_off);
-    a->dev.shift = cap > 0 ? 64 - log2i(cap) : 63;
-    a->dev.slot_words = sw;
     unsigned long long pat[12];
     for (int i = 0; i < 12; ++i) pat[i] = 0;
-    pat[0] = GQ_EMPTY_KEY;
-    for (int i = 0; i < d->naggs; ++i)
-      pat[1 + d->ndependent + i] = d->aggs[i].op == GQ_MIN ? 0x7FFFFFFFFFFFFFFFULL : d->aggs[i].op == GQ_MAX ? 0x8000000000000000ULL : 0ULL;
-    // a key-less aggregation has exactly one group, present even with no input rows (S9): header[1] = 1
-    cudaError_t e = gq_launch_init_table(ctx->stream, a->dev.slots, cap, sw, pat, a->dev.side, 1, a->dev.header, d->nkeys == 0 ? 1 : 0);
+    cudaError_t e;
+    if (dp.step >= 0) {
+      a->direct = true; a->dtab = d->probes[dp.step].table->dev; a->dcap = dp.cap; a->daw = dp.aw; a->dtouch = dp.touch;
+      a->dep_pay = dp.dep_pay;
+      a->dev.header = (long long*)d_ws;
+      a->dacc = (unsigned long long*)((char*)d_ws + 256);
+      for (int i = 0; i < d->naggs; ++i)
+        pat[i] = d->aggs[i].op == GQ_MIN ? 0x7FFFFFFFFFFFFFFFULL : d->aggs[i].op == GQ_MAX ? 0x8000000000000000ULL : 0ULL;
+      e = gq_launch_init_table(ctx->stream, a->dacc, dp.cap + 1, dp.aw, pat, a->dacc, 0, a->dev.header, 0);
+    } else {
+      const int64_t cap = agg_capacity(d->max_groups, d->nkeys);
+      const int sw = sp.target_sw;
+      WsLayout w = ws_layout(cap, sw, 1);
+      size_t hot_off = 0;
+      if (bytes < agg_ws_bytes(cap, sw, d->max_groups, d->nkeys, &hot_off)) {
+        delete a;
+        return fail(ctx, GQ_ERR_WORKSPACE_TOO_SMALL, "hash-aggregate workspace too small");
+      }
+      if (agg_has_hot_area(d->max_groups, d->nkeys)) {
+        a->hot = (long long*)((char*)d_ws + hot_off);
+        a->hot_table = (unsigned long long*)((char*)d_ws + hot_off + 4096);
+      }
+      a->capacity = cap;
+      a->lowcard = sp.consumer == GQ_C_LOWCARD; a->lc_cap = sp.lc_cap;
+      a->dev.slots = (unsigned long long*)((char*)d_ws + w.slots_off);
+      a->dev.mask = cap > 0 ? (unsigned long long)(cap - 1) : 0;
+      a->dev.header = (long long*)d_ws;
+      a->dev.side = (unsigned long long*)((char*)d_ws + w.side_off);
+      a->dev.shift = cap > 0 ? 64 - log2i(cap) : 63;
+      a->dev.slot_words = sw;
+      pat[0] = GQ_EMPTY_KEY;
+      for (int i = 0; i < d->naggs; ++i)
+        pat[1 + d->ndependent + i] = d->aggs[i].op == GQ_MIN ? 0x7FFFFFFFFFFFFFFFULL : d->aggs[i].op == GQ_MAX ? 0x8000000000000000ULL : 0ULL;
+      // a key-less aggregation has exactly one group, present even with no input rows (S9): header[1] = 1
+      e = gq_launch_init_table(ctx->stream, a->dev.slots, cap, sw, pat, a->dev.side, 1, a->dev.header, d->nkeys == 0 ? 1 : 0);
+    }
     if (e != cudaSuccess) { delete a; return cuda_fail(ctx, e, "aggregate state init"); }
     ++ctx->launches;
-    a->sig = signature(sig_sp);
     *state = a;
-  } else if (signature(sig_sp) != a->sig) return fail(ctx, GQ_ERR_INVALID_ARG, "batch schema/desc differs from the state's first batch");
+  }
+  if (a->direct) {
+    DirectPlan dp = direct_plan(sp, d, in);
+    if (dp.step < 0 || d->probes[dp.step].table->dev.slots != a->dtab.slots || dp.aw != a->daw)
+      return fail(ctx, GQ_ERR_INVALID_ARG, "batch schema/desc differs from the state's first batch");
+    sp.consumer = GQ_C_DIRECT; sp.direct_step = dp.step; sp.direct_aw = dp.aw; sp.direct_touch = dp.touch == d->naggs;
+    sp.hot = false;
+  }
+  {
+    GqScanSpec sig_sp = sp; sig_sp.nrows_hint = 0;
+    const std::string sig = signature(sig_sp);
+    if (a->sig.empty()) a->sig = sig;
+    else if (sig != a->sig) return fail(ctx, GQ_ERR_INVALID_ARG, "batch schema/desc differs from the state's first batch");
+  }
   GqParams P;
   memset(&P, 0, sizeof P);
   P.target = a->dev;
   P.acc = (long long*)(a->dev.side + 1);
+  P.dacc = a->dacc;
   if (sp.hot && a->hot && in->nrows >= GQ_HOT_MIN_ROWS) {   // heavy-hitter pass over a strided sample of the key column
     int nl = 0;
     const gq_column& kc = in->cols[sp.key_cols[0]];
@@ -552,6 +642,10 @@ gq_status gq_hash_aggregate_finish(gq_ctx* ctx, gq_aggstate* a, void* const* out
   memset(&p, 0, sizeof p);
   p.slots = a->dev.slots; p.capacity = a->capacity; p.slot_words = a->dev.slot_words;
   p.side = a->dev.side; p.header = a->dev.header;
+  if (a->direct) {
+    p.direct = 1; p.capacity = a->dcap; p.dacc = a->dacc; p.daw = a->daw; p.dtouch = a->dtouch; p.dep_pay = a->dep_pay;
+    p.jslots = a->dtab.slots; p.jside = a->dtab.side; p.jsw = a->dtab.slot_words;
+  }
   p.nkeys = a->nkeys; p.ndep = a->ndep; p.naggs = a->naggs;
   for (int k = 0; k < a->nkeys; ++k) {
     if (!out_key_cols[k]) return fail(ctx, GQ_ERR_INVALID_ARG, "null key output");
@@ -581,12 +675,18 @@ gq_status gq_hash_aggregate_finish(gq_ctx* ctx, gq_aggstate* a, void* const* out
 gq_status gq_aggstate_destroy(gq_aggstate* a) { if (!a) return GQ_ERR_INVALID_ARG; delete a; return GQ_OK; }
 
 // ------------------------------------------------------------------------------------------------ fused pipeline
+// Scratch of the finaliser fused into the scan kernel: per-CTA partial groups + group counts (<= 256 CTAs).
+static size_t fused_scratch_bytes(const gq_agg_desc* d) {
+  const size_t g = d->nkeys == 0 ? 1 : (size_t)std::min<int64_t>(64, std::max<int64_t>(1, d->max_groups));
+  return align_up(256 * (g * (1 + (size_t)d->naggs) + 1) * 8, 256);
+}
+
 gq_status gq_pipeline_workspace(const gq_plan* plan, size_t* bytes) {
-  if (!plan || !bytes) return GQ_ERR_INVALID_ARG;
+  if (!plan || !plan->in || !bytes) return GQ_ERR_INVALID_ARG;
   size_t b = 0;
-  gq_status st = gq_hash_aggregate_workspace(plan->agg.max_groups, plan->agg.nkeys, plan->agg.naggs, &b);
+  gq_status st = gq_hash_aggregate_workspace_for(plan->in, &plan->agg, &b);
   if (st != GQ_OK) return st;
-  *bytes = align_up(b, 256) + (plan->topk > 0 ? gq_topk_scratch_bytes_impl() : 0);
+  *bytes = align_up(b, 256) + (plan->topk > 0 ? align_up(gq_topk_scratch_bytes_impl(), 256) : 0) + fused_scratch_bytes(&plan->agg);
   return GQ_OK;
 }
 
@@ -598,12 +698,55 @@ gq_status gq_pipeline(gq_ctx* ctx, const gq_plan* plan, void* d_ws, size_t bytes
   gq_status st = gq_pipeline_workspace(plan, &need);
   if (st != GQ_OK) return fail(ctx, st, "bad plan");
   if (bytes < need) return fail(ctx, GQ_ERR_WORKSPACE_TOO_SMALL, "pipeline workspace too small");
-  gq_hash_aggregate_workspace(plan->agg.max_groups, plan->agg.nkeys, plan->agg.naggs, &aggb);
+  if (!d_ws || !aligned(d_ws, 256)) return fail(ctx, GQ_ERR_INVALID_ARG, "bad workspace");
+  gq_hash_aggregate_workspace_for(plan->in, &plan->agg, &aggb);
+  const size_t topk_off = align_up(aggb, 256);
+  const size_t fused_off = topk_off + (plan->topk > 0 ? align_up(gq_topk_scratch_bytes_impl(), 256) : 0);
+
+  // One batch, key-less or low-cardinality, no top-k: ONE kernel — every CTA writes its partial groups, the last CTA
+  // to finish merges them and emits the dense result (no table-init and no finalise launch).
+  {
+    const gq_agg_desc* d = &plan->agg;
+    st = check_batch(ctx, plan->in);
+    if (st != GQ_OK) return st;
+    GqScanSpec sp;
+    int kb[2]; gq_dtype kd[2] = {GQ_I64, GQ_I64};
+    st = agg_spec(ctx, &sp, plan->in, d, kb, kd);
+    if (st != GQ_OK) return st;
+    if ((sp.consumer == GQ_C_GLOBAL || sp.consumer == GQ_C_LOWCARD) && plan->topk == 0 && plan->in->nrows > 0 &&
+        ctx->num_sms <= 256) {
+      if (!out_agg_cols || !d_out_ngroups || out_capacity < 0 || (d->nkeys > 0 && !out_key_cols)) return fail(ctx, GQ_ERR_INVALID_ARG, "missing outputs");
+      if (plan->navg < 0 || plan->navg > GQ_MAX_AGGS || (plan->navg > 0 && (!plan->avgs || !out_avg_cols))) return fail(ctx, GQ_ERR_INVALID_ARG, "bad avg spec");
+      sp.fused_final = true;
+      GqParams P;
+      memset(&P, 0, sizeof P);
+      GqFinal& F = P.fin;
+      F.part = (long long*)((char*)d_ws + fused_off);
+      F.ticket = (unsigned*)(ctx->d_err + 16);
+      F.nkeys = d->nkeys; F.navg = plan->navg;
+      for (int k = 0; k < d->nkeys; ++k) {
+        if (!out_key_cols[k]) return fail(ctx, GQ_ERR_INVALID_ARG, "null key output");
+        F.out_key[k] = out_key_cols[k]; F.key_bits[k] = kb[k]; F.key_dtype[k] = (int)kd[k];
+      }
+      for (int i = 0; i < d->naggs; ++i) {
+        if (!out_agg_cols[i]) return fail(ctx, GQ_ERR_INVALID_ARG, "null aggregate output");
+        F.out_agg[i] = (long long*)out_agg_cols[i];
+      }
+      for (int v = 0; v < plan->navg; ++v) {
+        if (plan->avgs[v].sum_agg < 0 || plan->avgs[v].sum_agg >= d->naggs || plan->avgs[v].count_agg < 0 ||
+            plan->avgs[v].count_agg >= d->naggs || !out_avg_cols[v]) return fail(ctx, GQ_ERR_INVALID_ARG, "bad avg spec");
+        F.avg_sum[v] = plan->avgs[v].sum_agg; F.avg_cnt[v] = plan->avgs[v].count_agg; F.out_avg[v] = out_avg_cols[v];
+      }
+      F.out_capacity = out_capacity; F.out_n = (long long*)d_out_ngroups;
+      return run_scan(ctx, sp, plan->in, d->probes, &P);
+    }
+  }
+
   gq_aggstate* a = nullptr;
   st = gq_hash_aggregate(ctx, &a, d_ws, aggb, plan->in, &plan->agg);
   if (st != GQ_OK) { if (a) delete a; return st; }
   st = gq_hash_aggregate_finish(ctx, a, out_key_cols, out_agg_cols, plan->avgs, plan->navg, out_avg_cols, out_capacity,
-                                plan->topk, plan->topk_agg, (char*)d_ws + align_up(aggb, 256), d_out_ngroups);
+                                plan->topk, plan->topk_agg, (char*)d_ws + topk_off, d_out_ngroups);
   delete a;   // host handle only; the enqueued kernels hold device pointers into the caller's workspace
   return st;
 }
@@ -750,6 +893,20 @@ gq_status gq_precompile_pipeline(const gq_plan* plan, char* h_msg, size_t msg_by
   int kb[2]; gq_dtype kd[2];
   gq_status st = agg_spec(&tmp, &sp, plan->in, &plan->agg, kb, kd);
   if (st != GQ_OK) { if (h_msg && msg_bytes) { strncpy(h_msg, tmp.msg.c_str(), msg_bytes - 1); h_msg[msg_bytes - 1] = 0; } return st; }
+  // every kernel variant this plan shape can launch: streaming (state in a global table), single-batch with the
+  // finaliser fused in (key-less / low-cardinality), and direct aggregation (group key = key of a unique probe)
+  if ((sp.consumer == GQ_C_GLOBAL || sp.consumer == GQ_C_LOWCARD) && plan->topk == 0) {
+    GqScanSpec f = sp; f.fused_final = true;
+    st = precompile(f, h_msg, msg_bytes);
+    if (st != GQ_OK) return st;
+  }
+  DirectPlan dp = direct_plan(sp, &plan->agg, plan->in, true);
+  if (dp.step >= 0) {
+    GqScanSpec f = sp;
+    f.consumer = GQ_C_DIRECT; f.direct_step = dp.step; f.direct_aw = dp.aw; f.direct_touch = dp.touch == plan->agg.naggs; f.hot = false;
+    st = precompile(f, h_msg, msg_bytes);
+    if (st != GQ_OK) return st;
+  }
   return precompile(sp, h_msg, msg_bytes);
 }
 

@@ -7,6 +7,7 @@
 // stay runtime parameters (GqParams::k), so a kernel is specialised by plan SHAPE, not by constants.
 #include <algorithm>
 #include <cstdio>
+#include <cstdlib>
 #include <map>
 #include <sstream>
 
@@ -34,6 +35,7 @@ struct Gen {
   std::vector<long long> consts;
   std::vector<int> vcol_probe, vcol_pay;  // virtual column -> (probe step, payload index)
   std::string sfx;                        // "" (one row at a time) or "[j]" (linear mode: GQ_R rows in register arrays)
+  bool linear = false;
 
   Gen(const GqScanSpec& s, std::string* m) : sp(s), msg(m), ncols_in((int)s.in_dtype.size()) {
     compact.assign((size_t)ncols_in, -1);
@@ -61,13 +63,20 @@ struct Gen {
   std::string val(int c) const {                          // name of the row value of column c
     char b[32];
     if (c < ncols_in) snprintf(b, sizeof b, "v%d", c);
-    else snprintf(b, sizeof b, "y%d_%d", vcol_probe[(size_t)(c - ncols_in)], vcol_pay[(size_t)(c - ncols_in)]);
+    else if (linear) {   // payload word of probe step s: py<s>[j][p]
+      snprintf(b, sizeof b, "py%d[j][%d]", vcol_probe[(size_t)(c - ncols_in)], vcol_pay[(size_t)(c - ncols_in)]);
+      return b;
+    } else snprintf(b, sizeof b, "y%d_%d", vcol_probe[(size_t)(c - ncols_in)], vcol_pay[(size_t)(c - ncols_in)]);
     return std::string(b) + sfx;
   }
-  std::string konst(long long v) {
-    if ((int)consts.size() >= GQ_MAXK) { fail("too many constants"); return "0"; }
-    consts.push_back(v);
-    return "P.k[" + std::to_string(consts.size() - 1) + "]";
+  std::string konst(long long v) {   // equal literals share one parameter slot, so common subexpressions stay common
+    size_t i = 0;
+    while (i < consts.size() && consts[i] != v) ++i;
+    if (i == consts.size()) {
+      if ((int)consts.size() >= GQ_MAXK) { fail("too many constants"); return "0"; }
+      consts.push_back(v);
+    }
+    return "P.k[" + std::to_string(i) + "]";
   }
   std::string load(int c) const {                         // typed load of input column c for row slot j
     int kc = compact[(size_t)c];
@@ -120,21 +129,34 @@ static gq_status key_exprs(Gen& g, const GqScanSpec& sp, std::string* keyx, std:
   return GQ_OK;
 }
 
-// ---- linear mode: gq_tile processes the GQ_R rows of a thread step by step (see gq_codegen) ----
+// ---- linear mode: gq_tile processes the GQ_R rows of a thread step by step. Every hash-table step hands all GQ_R
+// rows to one skeleton helper (gq_probe_rows / gq_upsert_rows / gq_insert_rows) that keeps their slot accesses in
+// flight together and resolves them in rounds.
 static gq_status emit_linear(Gen& g, const GqScanSpec& sp, std::ostringstream& o, std::string* msg) {
   g.sfx = "[j]";
+  g.linear = true;
   const int nprobe = (int)sp.probes.size();
   const int nagg = (int)sp.aggs.size();
   const char* LOOP = "#pragma unroll\n  for (int j = 0; j < GQ_R; ++j) ";
-  o << "template <class Src> __device__ __forceinline__ void gq_tile(const GqParams& P, const Src& src, GqCtx& cx, int nvalid, bool full) {\n";
+  // Dense form (low-cardinality consumer): in a full tile every load, expression and cell update is unconditional and
+  // a filtered-out row contributes the aggregate's identity to group 0 — straight-line code, so the compiler can
+  // interleave the GQ_R rows of a thread. The other consumers skip the work of filtered-out rows.
+  const bool dense = sp.consumer == GQ_C_LOWCARD;
+  const char* GUARD = dense ? "if (FULL || live[j]) " : "if (live[j]) ";
+  o << "template <class Src, bool FULL> __device__ __forceinline__ void gq_tile(const GqParams& P, const Src& src, GqCtx& cx, int nvalid) {\n";
   o << "  bool live[GQ_R];\n";
-  for (int c : g.cols) o << "  i64 v" << c << "[GQ_R];\n";
+  for (int c : g.cols) o << "  i64 v" << c << "[GQ_R]" << (dense ? " = {}" : "") << ";\n";
   // ---- filter: all rows first, so the shared-memory loads of the GQ_R rows overlap ----
-  o << "  " << LOOP << "{\n    live[j] = full || j < nvalid;\n";
+  o << "  " << LOOP << "{\n    live[j] = FULL || j < nvalid;\n";
   std::vector<bool> loaded(g.compact.size(), false);
   for (const gq_pred& p : sp.preds) {
-    o << "    if (live[j]) { ";
-    if (!loaded[(size_t)p.col]) { o << g.load(p.col) << " "; loaded[(size_t)p.col] = true; }
+    if (dense) {
+      if (!loaded[(size_t)p.col]) { o << "    " << GUARD << "{ " << g.load(p.col) << " }\n"; loaded[(size_t)p.col] = true; }
+      o << "    { ";
+    } else {
+      o << "    if (live[j]) { ";
+      if (!loaded[(size_t)p.col]) { o << g.load(p.col) << " "; loaded[(size_t)p.col] = true; }
+    }
     std::string v = g.val(p.col), c;
     const std::string klo = g.konst(p.lo);
     const std::string khi = (p.op == GQ_RANGE_CO || p.op == GQ_RANGE_CC) ? g.konst(p.hi) : std::string();
@@ -149,7 +171,7 @@ static gq_status emit_linear(Gen& g, const GqScanSpec& sp, std::ostringstream& o
       case GQ_RANGE_CC: c = v + " >= " + klo + " && " + v + " <= " + khi; break;
       default: if (msg) *msg = "unknown comparison"; return GQ_ERR_INVALID_ARG;
     }
-    o << "live[j] = (" << c << "); }\n";
+    o << "live[j] = " << (dense ? "live[j] && " : "") << "(" << c << "); }\n";
   }
   o << "  }\n";
   // ---- remaining input columns of surviving rows ----
@@ -157,47 +179,33 @@ static gq_status emit_linear(Gen& g, const GqScanSpec& sp, std::ostringstream& o
     bool any = false;
     for (int c : g.cols) any = any || !loaded[(size_t)c];
     if (any) {
-      o << "  " << LOOP << "if (live[j]) {\n";
+      o << "  " << LOOP << GUARD << "{\n";
       for (int c : g.cols) if (!loaded[(size_t)c]) o << "    " << g.load(c) << "\n";
       o << "  }\n";
     }
   }
-  // ---- probe steps: issue the first slot read of every row, then resolve ----
+  // a row column as a whole GQ_R array (input columns are arrays already; payloads are copied out)
+  int ntmp = 0;
+  auto as_array = [&](int c) -> std::string {
+    if (c < g.ncols_in) return "v" + std::to_string(c);
+    const std::string nm = "ka" + std::to_string(ntmp++);
+    o << "  i64 " << nm << "[GQ_R];\n  " << LOOP << nm << "[j] = " << g.val(c) << ";\n";
+    return nm;
+  };
+  // ---- probe steps ----
   for (int s = 0; s < nprobe; ++s) {
     const GqProbeSpec& ps = sp.probes[(size_t)s];
-    const int sw = ps.slot_words;
-    const std::string S = std::to_string(s), key = g.val(ps.key_col);
-    o << "  const GqTableDev& T" << S << " = P.probe[" << S << "];\n";
-    o << "  u64 pi" << S << "[GQ_R], pk" << S << "[GQ_R], pw" << S << "[GQ_R];\n";
-    for (int p = 0; p < ps.npayload; ++p) o << "  i64 y" << S << "_" << p << "[GQ_R];\n";
-    o << "  " << LOOP << "{\n    pi" << S << "[j] = 0; pk" << S << "[j] = GQ_EMPTY; pw" << S << "[j] = 0;\n";
-    o << "    if (live[j] && (u64)" << key << " != GQ_EMPTY) {\n";
-    o << "      pi" << S << "[j] = gq_hash(" << key << ", T" << S << ".shift);\n";
-    if (sw == 2) o << "      gq_ld128(T" << S << ".slots + pi" << S << "[j] * 2, pk" << S << "[j], pw" << S << "[j]);\n";
-    else o << "      pk" << S << "[j] = __ldg(T" << S << ".slots + pi" << S << "[j] * " << sw << ");\n";
-    o << "    }\n  }\n";
-    o << "  " << LOOP << "if (live[j]) {\n";
-    o << "    if ((u64)" << key << " == GQ_EMPTY) {   // reserved key pattern: unique table => at most one side entry (S14)\n";
-    o << "      if (T" << S << ".header[1] > 0) {";
-    for (int p = 0; p < ps.npayload; ++p) o << " y" << S << "_" << p << "[j] = (i64)T" << S << ".side[" << (1 + p) << "];";
-    o << " } else live[j] = false;\n    } else {\n";
-    o << "      u64 i = pi" << S << "[j], kw = pk" << S << "[j], w = pw" << S << "[j];\n";
-    o << "      for (u64 n = 0; kw != (u64)" << key << " && kw != GQ_EMPTY && n < T" << S << ".mask; ++n) {\n";
-    o << "        i = (i + 1) & T" << S << ".mask;\n";
-    if (sw == 2) o << "        gq_ld128(T" << S << ".slots + i * 2, kw, w);\n";
-    else o << "        kw = __ldg(T" << S << ".slots + i * " << sw << ");\n";
-    o << "      }\n";
-    o << "      if (kw != (u64)" << key << ") live[j] = false;\n      else {";
-    for (int p = 0; p < ps.npayload; ++p) {
-      if (sw == 2) o << " y" << S << "_" << p << "[j] = (i64)w;";
-      else o << " y" << S << "_" << p << "[j] = (i64)__ldg(T" << S << ".slots + i * " << sw << " + " << (1 + p) << ");";
-    }
-    o << " (void)w; }\n    }\n  }\n";
+    const std::string S = std::to_string(s);
+    const std::string karr = as_array(ps.key_col);
+    o << "  u64 pi" << S << "[GQ_R]; i64 py" << S << "[GQ_R][" << (ps.npayload > 0 ? ps.npayload : 1) << "];\n";
+    o << "  gq_probe_rows<" << ps.slot_words << ", " << ps.npayload << ">(P.probe[" << S << "], " << karr << ", live, pi" << S
+      << ", py" << S << ");\n";
+    o << "  (void)pi" << S << "; (void)py" << S << ";\n";
   }
   // ---- projection ----
   if (!sp.exprs.empty()) {
     for (size_t e = 0; e < sp.exprs.size(); ++e) o << "  i64 e" << e << "[GQ_R];\n";
-    o << "  " << LOOP << "if (live[j]) {\n";
+    o << "  " << LOOP << (dense ? "" : "if (live[j]) ") << "{\n";
     for (size_t e = 0; e < sp.exprs.size(); ++e) {
       std::string x;
       if (!g.expr(sp.exprs[e], &x)) return GQ_ERR_INVALID_ARG;
@@ -219,40 +227,58 @@ static gq_status emit_linear(Gen& g, const GqScanSpec& sp, std::ostringstream& o
       o << "  }\n";
       break;
     case GQ_C_LOWCARD:
-      o << "  " << LOOP << "if (live[j]) {\n    const int grp = gq_lc_slot(cx, " << keyx << ", P.err);\n    if (grp >= 0) {\n";
-      for (int a = 0; a < nagg; ++a)
-        o << "      gq_lc_update(" << (int)sp.aggs[(size_t)a].op << ", cx, grp, " << a << ", " << aggval(sp.aggs[(size_t)a]) << ");\n";
-      o << "    }\n  }\n";
+      // group id: one LDS on the fast path; first sights and collisions take the (rare, warp-converged) slow path
+      o << "  int grp[GQ_R]; i64 lk[GQ_R]; bool need[GQ_R]; bool anyneed = false;\n";
+      o << "  " << LOOP << "{\n    lk[j] = " << keyx << ";\n    const int g1 = gq_lc_find1(cx, lk[j]);\n"
+        << "    grp[j] = live[j] ? g1 : 0;\n    need[j] = live[j] && g1 < 0;\n    anyneed = anyneed || need[j];\n  }\n";
+      // (keys inserted while serving an earlier row are picked up by a second one-probe look before asking again)
+      o << "  if (__any_sync(0xffffffffu, anyneed)) {\n  " << LOOP << "{\n"
+        << "      if (need[j]) { const int g2 = gq_lc_find1(cx, lk[j]); if (g2 >= 0) { grp[j] = g2; need[j] = false; } }\n"
+        << "      if (__any_sync(0xffffffffu, need[j])) grp[j] = gq_lc_slow(cx, lk[j], need[j], grp[j], P.err);\n    }\n  }\n";
+      o << "  " << LOOP << "{\n";
+      for (int a = 0; a < nagg; ++a) {
+        const int op = (int)sp.aggs[(size_t)a].op;
+        o << "    gq_lc_update(" << op << ", cx, grp[j], " << a << ", live[j] ? " << aggval(sp.aggs[(size_t)a]) << " : gq_identity(" << op << "));\n";
+      }
+      o << "  }\n";
       break;
-    case GQ_C_HIGHCARD:
-      o << "#if GQ_HOT\n  if (cx.nhot > 0) {\n  " << LOOP << "if (live[j]) {\n      const int hp = gq_hot_find(cx, " << keyx << ");\n"
+    case GQ_C_HIGHCARD: {
+      o << "  i64 tkey[GQ_R];\n  " << LOOP << "tkey[j] = " << keyx << ";\n";
+      o << "#if GQ_HOT\n  if (cx.nhot > 0) {\n  " << LOOP << "if (live[j]) {\n      const int hp = gq_hot_find(cx, tkey[j]);\n"
         << "      if (hp >= 0) {\n";
       for (int a = 0; a < nagg; ++a)
         o << "        gq_hot_update(" << (int)sp.aggs[(size_t)a].op << ", cx, hp, " << a << ", " << aggval(sp.aggs[(size_t)a]) << ");\n";
       o << "        cx.hot_touched[hp] = 1;\n        live[j] = false;\n      }\n    }\n  }\n#endif\n";
-      o << "  u64 ti[GQ_R], tk[GQ_R];\n";
-      o << "  " << LOOP << "{\n    ti[j] = 0; tk[j] = GQ_EMPTY;\n    if (live[j] && (u64)" << keyx << " != GQ_EMPTY) {\n";
-      o << "      ti[j] = gq_hash(" << keyx << ", P.target.shift);\n      tk[j] = gq_ld_relaxed(P.target.slots + ti[j] * " << sp.target_sw << ");\n    }\n  }\n";
-      o << "  " << LOOP << "if (live[j]) {\n";
-      o << "    bool won; u64* slot = gq_ht_upsert_pre<" << sp.target_sw << ">(P.target, " << keyx << ", ti[j], tk[j], &won, P.err);\n";
-      o << "    if (slot) {\n";
-      if (sp.ndep == 1) o << "      if (won) slot[1] = (u64)" << depx << ";\n";
+      o << "  u64* slot[GQ_R]; bool won[GQ_R];\n";
+      o << "  gq_upsert_rows<" << sp.target_sw << ">(P.target, tkey, live, slot, won, P.err);\n";
+      o << "  " << LOOP << "if (live[j] && slot[j]) {\n";
+      if (sp.ndep == 1) o << "    if (won[j]) slot[j][1] = (u64)" << depx << ";\n";
       for (int a = 0; a < nagg; ++a)
-        o << "      gq_red(" << (int)sp.aggs[(size_t)a].op << ", slot + " << (1 + sp.ndep + a) << ", " << aggval(sp.aggs[(size_t)a]) << ");\n";
-      o << "    }\n  }\n";
+        o << "    gq_red(" << (int)sp.aggs[(size_t)a].op << ", slot[j] + " << (1 + sp.ndep + a) << ", " << aggval(sp.aggs[(size_t)a]) << ");\n";
+      o << "  }\n";
       break;
+    }
+    case GQ_C_DIRECT: {
+      // group == matched slot of probe step direct_step (SURVEY §8(d) note on C3): no key compare, no CAS
+      if (sp.direct_step < 0 || sp.direct_step >= nprobe || sp.direct_aw < nagg) { if (msg) *msg = "bad direct aggregation spec"; return GQ_ERR_INVALID_ARG; }
+      o << "  " << LOOP << "if (live[j]) {\n    u64* acc = P.dacc + pi" << sp.direct_step << "[j] * " << sp.direct_aw << ";\n";
+      for (int a = 0; a < nagg; ++a)
+        o << "    gq_red(" << (int)sp.aggs[(size_t)a].op << ", acc + " << a << ", " << aggval(sp.aggs[(size_t)a]) << ");\n";
+      if (sp.direct_touch) o << "    gq_red(3, acc + " << nagg << ", 1);\n";
+      o << "  }\n";
+      break;
+    }
     case GQ_C_BUILD: {
       const int np = (int)sp.payload_cols.size();
-      const std::string bk = g.val(sp.build_key_col);
-      o << "  u64 bi[GQ_R], bp[GQ_R];\n";
-      o << "  " << LOOP << "{\n    bi[j] = 0; bp[j] = 0;\n    if (live[j] && (u64)" << bk << " != GQ_EMPTY) {\n";
-      o << "      bi[j] = gq_hash(" << bk << ", P.target.shift);\n      bp[j] = atomicCAS(P.target.slots + bi[j] * " << sp.target_sw
-        << ", GQ_EMPTY, (u64)" << bk << ");\n    }\n  }\n";
-      o << "  " << LOOP << "if (live[j]) {\n    const i64 pay[" << (np > 0 ? np : 1) << "] = {";
-      for (int p = 0; p < np; ++p) o << (p ? ", " : "") << g.val(sp.payload_cols[(size_t)p]);
-      if (np == 0) o << "0";
-      o << "};\n    if (gq_ht_insert_pre<" << sp.target_sw << ", " << np << ">(P.target, " << bk << ", pay, " << (sp.unique ? "true" : "false")
-        << ", bi[j], bp[j], P.err)) ++cx.ninserted;\n  }\n";
+      const std::string karr = as_array(sp.build_key_col);
+      o << "  i64 bpay[GQ_R][" << (np > 0 ? np : 1) << "];\n";
+      if (np > 0) {
+        o << "  " << LOOP << "if (live[j]) {\n";
+        for (int p = 0; p < np; ++p) o << "    bpay[j][" << p << "] = " << g.val(sp.payload_cols[(size_t)p]) << ";\n";
+        o << "  }\n";
+      }
+      o << "  cx.ninserted += gq_insert_rows<" << sp.target_sw << ", " << np << ">(P.target, " << karr << ", live, bpay, "
+        << (sp.unique ? "true" : "false") << ", P.err);\n";
       break;
     }
     case GQ_C_MATERIALISE:
@@ -265,6 +291,7 @@ static gq_status emit_linear(Gen& g, const GqScanSpec& sp, std::ostringstream& o
   }
   o << "}\n\n";
   g.sfx.clear();
+  g.linear = false;
   return GQ_OK;
 }
 
@@ -305,12 +332,21 @@ gq_status gq_codegen(const GqScanSpec& sp, GqKernelInfo* out, std::string* msg) 
   const int ncol = (int)g.cols.size();
   int row_bytes = 0;
   for (int c : g.cols) row_bytes += gq_dtype_bytes(sp.in_dtype[(size_t)c]);
+  auto env_int = [](const char* name) { const char* e = getenv(name); return e ? atoi(e) : 0; };   // tuning sweeps only
   int nt = 512;
   long long cons_bytes = 256;
+  int lc_kt = 64, lc_key32 = 0;
   if (sp.consumer == GQ_C_GLOBAL) cons_bytes = 8LL * nagg * (nt / 32) + 256;
   if (sp.consumer == GQ_C_LOWCARD) {
-    nt = 256;
-    cons_bytes = (((sp.lc_cap + 1) * 8 + 8 + 127) / 128 * 128) + 8LL * (sp.lc_cap + 1) * nagg * nt;
+    if (sp.lc_cap < 1 || sp.lc_cap > 64) { if (msg) *msg = "low-cardinality path needs 1..64 groups"; return GQ_ERR_INVALID_ARG; }
+    lc_kt = sp.lc_cap <= 16 ? 64 : sp.lc_cap <= 32 ? 128 : 256;
+    lc_key32 = sp.lc_key_bits > 0 && sp.lc_key_bits < 32;
+    const long long head = (lc_kt * 12LL + sp.lc_cap * 8LL + 16 + 8LL * sp.lc_cap * nagg + 127) / 128 * 128;
+    // thread-private cells: as many consumer threads as leave room for a 3-stage ring of one-row-per-thread tiles
+    for (nt = 256; nt > 128; nt /= 2)   // 8 warps x GQ_R independent rows per thread; cells cost 8 B x groups x aggregates per thread
+      if (head + 8LL * sp.lc_cap * nagg * nt + 3LL * ((row_bytes * nt + 127) / 128 * 128 + 128 * ncol) + 1024 <= GQ_SMEM_LIMIT) break;
+    if (env_int("GQ_TUNE_LC_NT")) nt = env_int("GQ_TUNE_LC_NT");
+    cons_bytes = head + 8LL * sp.lc_cap * nagg * nt;
   }
   bool all_unique = true;
   for (const GqProbeSpec& ps : sp.probes) all_unique = all_unique && ps.unique;
@@ -320,6 +356,8 @@ gq_status gq_codegen(const GqScanSpec& sp, GqKernelInfo* out, std::string* msg) 
   // small inputs: smaller tiles so that every SM still gets several tiles
   if (sp.nrows_hint > 0 && sp.nrows_hint < 148LL * 8 * nt * 4) r = 2;
   if (sp.nrows_hint > 0 && sp.nrows_hint < 148LL * 8 * nt * 2) r = 1;
+  if (sp.consumer == GQ_C_LOWCARD) r = (sp.nrows_hint > 0 && sp.nrows_hint < 148LL * nt * 4) ? 1 : 4;   // straight-line rows: ILP
+  if (env_int("GQ_TUNE_R")) r = env_int("GQ_TUNE_R");
   long long stage_bytes = 0;
   for (;; r /= 2) {
     stage_bytes = 0;
@@ -328,6 +366,7 @@ gq_status gq_codegen(const GqScanSpec& sp, GqKernelInfo* out, std::string* msg) 
     stages = (int)std::min<long long>(4, avail / stage_bytes);
     if (stages >= 3 || r == 1) break;
   }
+  if (env_int("GQ_TUNE_STAGES") && env_int("GQ_TUNE_STAGES") < stages) stages = env_int("GQ_TUNE_STAGES");
   if (stages < 1) { if (msg) *msg = "plan does not fit shared memory"; return GQ_ERR_UNSUPPORTED; }
 
   // ---- 3. prelude ----
@@ -335,8 +374,10 @@ gq_status gq_codegen(const GqScanSpec& sp, GqKernelInfo* out, std::string* msg) 
   o << "// generated by gq_codegen — plan-shape specialised prelude\n";
   o << "#define GQ_NCOL " << ncol << "\n#define GQ_NT " << nt << "\n#define GQ_R " << r << "\n#define GQ_STAGES "
     << stages << "\n#define GQ_STAGE_BYTES " << stage_bytes << "\n#define GQ_CONSUMER " << sp.consumer << "\n";
-  o << "#define GQ_NAGG " << nagg << "\n#define GQ_LC_CAP " << (sp.lc_cap > 0 ? sp.lc_cap : 1) << "\n#define GQ_TARGET_SW "
-    << (sp.target_sw > 0 ? sp.target_sw : 1) << "\n#define GQ_NDEP " << sp.ndep << "\n#define GQ_EVICT_FIRST 1\n#define GQ_HOT " << (use_hot ? 1 : 0) << "\n";
+  o << "#define GQ_NAGG " << nagg << "\n#define GQ_LC_G " << (sp.lc_cap > 0 ? sp.lc_cap : 1) << "\n#define GQ_LC_KT " << lc_kt
+    << "\n#define GQ_LC_KEY32 " << lc_key32 << "\n#define GQ_TARGET_SW "
+    << (sp.target_sw > 0 ? sp.target_sw : 1) << "\n#define GQ_NDEP " << sp.ndep << "\n#define GQ_EVICT_FIRST " << (getenv("GQ_TUNE_NO_EVICT_FIRST") ? 0 : 1) << "\n#define GQ_HOT " << (use_hot ? 1 : 0)
+    << "\n#define GQ_FUSED_FINAL " << (sp.fused_final ? 1 : 0) << "\n#define GQ_DIRECT_AW " << (sp.direct_aw > 0 ? sp.direct_aw : 1) << "\n";
   {
     long long off = 0, tx = 0;
     std::ostringstream offs, bytes;
@@ -416,7 +457,7 @@ gq_status gq_codegen(const GqScanSpec& sp, GqKernelInfo* out, std::string* msg) 
       o << ind << "const i64 pk" << s << " = " << g.val(ps.key_col) << ";\n";
       o << ind << "const bool sd" << s << " = ((u64)pk" << s << " == GQ_EMPTY);\n";
       o << ind << "i64 ns" << s << " = 0; if (sd" << s << ") ns" << s << " = gq_min(T" << s << ".header[1], GQ_SIDE_SLOTS);\n";
-      o << ind << "u64 i" << s << " = gq_hash(pk" << s << ", T" << s << ".shift);\n";
+      o << ind << "u64 i" << s << " = gq_slot0(T" << s << ", pk" << s << ");\n";
       o << ind << "for (u64 n" << s << " = 0; n" << s << " <= T" << s << ".mask; ++n" << s << ") {\n";
       ind += "  ";
       o << ind << "const u64* s" << s << "; u64 w" << s << " = 0;\n";

@@ -15,7 +15,7 @@
 #define GQ_MAXOUT 12
 #define GQ_SMEM_LIMIT 232448   // 227 KB opt-in dynamic shared memory per CTA on sm_100
 
-enum { GQ_C_GLOBAL = 0, GQ_C_LOWCARD = 1, GQ_C_HIGHCARD = 2, GQ_C_BUILD = 3, GQ_C_MATERIALISE = 4 };
+enum { GQ_C_GLOBAL = 0, GQ_C_LOWCARD = 1, GQ_C_HIGHCARD = 2, GQ_C_BUILD = 3, GQ_C_MATERIALISE = 4, GQ_C_DIRECT = 5 };
 
 // ---- device-visible structs: layouts must match gq_skeleton.cuh ----
 struct GqTableDev {
@@ -26,7 +26,19 @@ struct GqTableDev {
   int shift;
   int slot_words;
   unsigned flags;
-  unsigned pad;
+  unsigned bshift;             // log2(slots per 32-byte bucket) for join tables, 0 for aggregation tables
+};
+struct GqFinal {
+  long long* part;
+  unsigned* ticket;
+  void* out_key[2];
+  long long* out_agg[8];
+  double* out_avg[8];
+  int avg_sum[8], avg_cnt[8];
+  int navg, nkeys;
+  int key_bits[2], key_dtype[2];
+  long long out_capacity;
+  long long* out_n;
 };
 struct GqParams {
   const void* col[GQ_MAXCOL];
@@ -41,13 +53,15 @@ struct GqParams {
   const long long* hot;        // HIGHCARD: hot list of this batch (hot[0] = count, hot[1..] = keys) or null
   int* err;
   int pad;
+  unsigned long long* dacc;    // DIRECT: aggregate words indexed by slot of the probed unique table
+  GqFinal fin;
 };
 
 // ---- handles ----
 struct gq_ctx {
   int device = 0;
   cudaStream_t stream = nullptr;
-  int* d_err = nullptr;        // sticky device error
+  int* d_err = nullptr;        // sticky device error; d_err + 16 = ticket counter of the fused finaliser
   int* h_err = nullptr;        // pinned mirror
   int num_sms = 148;
   int last_cuda = 0;
@@ -81,6 +95,11 @@ struct gq_aggstate {
   int64_t max_groups = 0;
   bool lowcard = false;
   int lc_cap = 0;
+  bool direct = false;         // aggregate words indexed by the slot of a probed unique table (no keys stored)
+  GqTableDev dtab{};           //   that table
+  int64_t dcap = 0;            //   its capacity (the accumulator array has dcap + 1 slots: the last is the side entry)
+  int daw = 0, dtouch = -1, dep_pay = -1;   // words per accumulator slot, word that marks a touched slot, payload = dep key
+  unsigned long long* dacc = nullptr;
   long long* hot = nullptr;            // hot list (in the workspace)
   unsigned long long* hot_table = nullptr;
   std::string sig;
@@ -103,7 +122,12 @@ struct GqScanSpec {
   std::vector<int> key_cols;                      // LOWCARD / HIGHCARD
   int ndep = 0;
   std::vector<gq_agg> aggs;
-  int lc_cap = 0;
+  int lc_cap = 0;                                 // LOWCARD: number of group cells (= max_groups)
+  int lc_key_bits = 0;                            // LOWCARD: packed key width
+  bool fused_final = false;                       // LOWCARD / GLOBAL: finaliser fused into the scan kernel
+  int direct_step = -1;                           // DIRECT: probe step whose matched slot is the group
+  int direct_aw = 0;                              // DIRECT: words per accumulator slot
+  bool direct_touch = false;                      // DIRECT: hidden COUNT word marks touched slots
   int target_sw = 0;                              // slot words of the target table
   int build_key_col = 0;                          // BUILD
   std::vector<int> payload_cols;
@@ -134,6 +158,9 @@ void gq_jit_set_cache_dir(const char* path);
 struct GqFinaliseParams {
   const unsigned long long* slots; long long capacity; int slot_words;
   const unsigned long long* side; const long long* header;
+  // direct mode: groups = touched accumulator slots; keys / dependent key come from the join table
+  int direct; const unsigned long long* dacc; int daw, dtouch, dep_pay;
+  const unsigned long long* jslots; const unsigned long long* jside; int jsw;
   int nkeys, ndep, naggs;
   int key_bits[2]; int key_dtype[2];
   void* out_key[2]; long long* out_agg[GQ_MAX_AGGS];

@@ -33,7 +33,7 @@ struct Nvrtc {
 
 bool load_nvrtc(std::string* msg) {
   if (g_nvrtc.h) return true;
-  const char* names[] = {"libnvrtc.so.12", "/usr/local/cuda/lib64/libnvrtc.so.12", "libnvrtc.so", nullptr};
+  const char* names[] = {"/usr/local/cuda/lib64/libnvrtc.so.12", "libnvrtc.so.12", "libnvrtc.so", nullptr};   // the toolkit's own NVRTC first: an older one bundled with a Python package may already be in the process
   for (int i = 0; names[i] && !g_nvrtc.h; ++i) g_nvrtc.h = dlopen(names[i], RTLD_NOW | RTLD_LOCAL);
   if (!g_nvrtc.h) { if (msg) *msg = "cannot dlopen libnvrtc.so.12"; return false; }
   g_nvrtc.create = (fn_create)dlsym(g_nvrtc.h, "nvrtcCreateProgram");

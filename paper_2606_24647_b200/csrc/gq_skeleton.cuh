@@ -17,7 +17,8 @@
 //   tail  = the < GQ_TILE leftover rows are read straight from global memory by one CTA (same row functions).
 //
 // Prelude macros expected: GQ_NCOL, GQ_NT, GQ_R, GQ_STAGES, GQ_STAGE_BYTES, GQ_COL_OFF(c), GQ_COL_BYTES(c) (bytes per
-// element), GQ_CONSUMER, GQ_NAGG, GQ_AGG_OP(a), GQ_LC_CAP, GQ_TARGET_SW, GQ_NDEP, GQ_EVICT_FIRST.
+// element), GQ_CONSUMER, GQ_NAGG, GQ_AGG_OP(a), GQ_LC_G (group cells), GQ_LC_KT (key-table slots), GQ_LC_KEY32,
+// GQ_TARGET_SW, GQ_NDEP, GQ_EVICT_FIRST, GQ_HOT, GQ_FUSED_FINAL, GQ_DIRECT_AW.
 
 typedef unsigned long long u64;
 typedef long long i64;
@@ -36,6 +37,7 @@ typedef unsigned int u32;
 #define GQ_C_HIGHCARD 2
 #define GQ_C_BUILD 3
 #define GQ_C_MATERIALISE 4
+#define GQ_C_DIRECT 5
 
 #define GQ_E_CAPACITY 3
 #define GQ_E_DUPLICATE 6
@@ -54,7 +56,23 @@ struct GqTableDev {
   int shift;         // 64 - log2(capacity)
   int slot_words;
   u32 flags;
-  u32 pad;
+  u32 bshift;        // log2(slots per 32-byte bucket): probe sequences start on a bucket boundary (join tables)
+};
+
+// Outputs of the finaliser fused into the scan kernel (gq_pipeline over one batch, LOWCARD / GLOBAL consumers): every
+// CTA writes its partial groups to `part`, takes a ticket, and the last CTA merges all partials and emits the dense
+// result (keys, aggregates, AVG, group count) — no separate init / finalise launches. Must match gq_internal.h.
+struct GqFinal {
+  i64* part;                    // [grid][G][1 + NAGG] (LOWCARD) or [grid][NAGG] (GLOBAL), then [grid] group counts
+  u32* ticket;                  // context-owned counter, zero between kernels (reset by the last CTA)
+  void* out_key[2];
+  i64* out_agg[8];
+  double* out_avg[8];
+  int avg_sum[8], avg_cnt[8];
+  int navg, nkeys;
+  int key_bits[2], key_dtype[2];
+  i64 out_capacity;
+  i64* out_n;
 };
 
 // Kernel parameters: one fixed layout for every generated kernel. Must match gq_internal.h:GqParams.
@@ -71,6 +89,8 @@ struct GqParams {
   const i64* hot;               // HIGHCARD: hot list of this batch (hot[0] = count, hot[1..] = keys) or null
   int* err;                     // sticky device error
   int pad;
+  u64* dacc;                    // DIRECT: aggregate words indexed by the slot of the probed unique table
+  GqFinal fin;                  // GQ_FUSED_FINAL: outputs of the in-kernel finaliser
 };
 
 // ---------------------------------------------------------------------------------------------- PTX wrappers
@@ -134,15 +154,30 @@ __device__ __forceinline__ void gq_set_err(int* err, int code) { atomicCAS(err, 
 
 // ---------------------------------------------------------------------------------------------- hash tables
 // Open addressing, linear probing, 64-bit CAS on the key word (north_star). Fibonacci hashing of the folded key.
+// Join tables are read one 32-byte sector at a time (LDG.256): a "bucket" holds 4 key-only slots, 2 key+payload
+// slots or 1 wide slot, and every probe sequence starts on a bucket boundary (T.bshift), so the first fetch examines
+// a whole bucket. Slots of a bucket fill in order (an inserter only skips a slot it has seen occupied), hence a
+// lookup may stop at the first EMPTY slot.
 __device__ __forceinline__ u64 gq_hash(i64 key, int shift) {
   u64 x = (u64)key;
   x ^= x >> 32;
   return (x * 0x9E3779B97F4A7C15ULL) >> shift;
 }
+__device__ __forceinline__ u64 gq_slot0(const GqTableDev& T, i64 key) {
+  return (gq_hash(key, T.shift) >> T.bshift) << T.bshift;
+}
+__device__ __forceinline__ void gq_ld256(const u64* p, u64 (&w)[4]) {   // one 32-byte sector, read-only path
+  asm volatile("ld.global.nc.v4.u64 {%0, %1, %2, %3}, [%4];" : "=l"(w[0]), "=l"(w[1]), "=l"(w[2]), "=l"(w[3]) : "l"(p));
+}
+__device__ __forceinline__ void gq_ld256_relaxed(const u64* p, u64 (&w)[4]) {   // sees concurrent CAS results (L2)
+  asm volatile("ld.relaxed.gpu.global.v2.u64 {%0, %1}, [%2];" : "=l"(w[0]), "=l"(w[1]) : "l"(p) : "memory");
+  asm volatile("ld.relaxed.gpu.global.v2.u64 {%0, %1}, [%2];" : "=l"(w[2]), "=l"(w[3]) : "l"(p + 2) : "memory");
+}
 
-// HashBuild insert: duplicates are kept as separate slots (multiset, S3) unless `unique` is asserted,
-// in which case an equal key sets the sticky GQ_E_DUPLICATE. Payload words are written by the CAS winner; probes only
-// run after the building kernel has finished (pipeline boundary), so no reader can see them half-written.
+// HashBuild insert of one row: duplicates are kept as separate slots (multiset, S3) unless `unique`
+// is asserted, in which case an equal key sets the sticky GQ_E_DUPLICATE. Payload words are written by the CAS
+// winner; probes only run after the building kernel has finished (pipeline boundary), so no reader can
+// see them half-written.
 template <int SW, int NPAY>
 __device__ __forceinline__ bool gq_ht_insert(const GqTableDev& T, i64 key, const i64* pay, bool unique, int* err) {
   if ((u64)key == GQ_EMPTY) {                     // reserved bit pattern: side area (S14)
@@ -155,7 +190,7 @@ __device__ __forceinline__ bool gq_ht_insert(const GqTableDev& T, i64 key, const
     for (int p = 0; p < NPAY; ++p) s[1 + p] = (u64)pay[p];
     return true;
   }
-  u64 i = gq_hash(key, T.shift);
+  u64 i = gq_slot0(T, key);
   for (u64 n = 0; n <= T.mask; ++n, i = (i + 1) & T.mask) {
     u64* s = T.slots + i * SW;
     u64 prev = atomicCAS(s, GQ_EMPTY, (u64)key);
@@ -170,9 +205,9 @@ __device__ __forceinline__ bool gq_ht_insert(const GqTableDev& T, i64 key, const
   return false;
 }
 
-// HashAggregation insert-or-update: returns the slot of `key`, claiming a free one by CAS if the key is
-// new. Aggregate words already hold their identities (table-init kernel), so there is no claimed-but-uninitialised
-// window. *won tells the caller it created the group (it then stores the dependent key columns).
+// HashAggregation insert-or-update of one row: returns the slot of `key`, claiming a free one by CAS
+// if the key is new. Aggregate words already hold their identities (table-init kernel), so there is no
+// claimed-but-uninitialised window. *won tells the caller it created the group.
 template <int SW>
 __device__ __forceinline__ u64* gq_ht_upsert(const GqTableDev& T, i64 key, bool* won, int* err) {
   *won = false;
@@ -181,7 +216,7 @@ __device__ __forceinline__ u64* gq_ht_upsert(const GqTableDev& T, i64 key, bool*
     *won = (prev == 0);
     return T.side;
   }
-  u64 i = gq_hash(key, T.shift);
+  u64 i = gq_slot0(T, key);
   for (u64 n = 0; n <= T.mask; ++n, i = (i + 1) & T.mask) {
     u64* s = T.slots + i * SW;
     u64 k = gq_ld_relaxed(s);
@@ -196,43 +231,154 @@ __device__ __forceinline__ u64* gq_ht_upsert(const GqTableDev& T, i64 key, bool*
   return nullptr;
 }
 
-// Variants that continue from a first slot access already issued by the caller (linear mode: the first CAS / key read
-// of all GQ_R rows of a thread are in flight together before any of them is consumed).
+// ---- GQ_R rows of a thread at once ("linear mode"): the slot accesses of all rows are issued together and resolved
+// in rounds, so a thread keeps up to GQ_R random accesses in flight and a round costs ONE memory latency however many
+// rows are still unresolved (memory-level parallelism is what bounds the hash phases, not bandwidth).
+
+// HashProbe of a table with unique keys. live[j] is cleared for rows without a match; idx[j] receives
+// the matching slot index (capacity = the side entry), pay[j][] its payload words.
 template <int SW, int NPAY>
-__device__ __forceinline__ bool gq_ht_insert_pre(const GqTableDev& T, i64 key, const i64* pay, bool unique, u64 i,
-                                                 u64 prev, int* err) {
-  if ((u64)key == GQ_EMPTY) return gq_ht_insert<SW, NPAY>(T, key, pay, unique, err);
-  for (u64 n = 0; n <= T.mask; ++n) {
-    u64* s = T.slots + i * SW;
-    if (prev == GQ_EMPTY) {
+__device__ __forceinline__ void gq_probe_rows(const GqTableDev& T, const i64 (&key)[GQ_R], bool (&live)[GQ_R],
+                                              u64 (&idx)[GQ_R], i64 (&pay)[GQ_R][NPAY > 0 ? NPAY : 1]) {
+  constexpr int B = SW == 1 ? 4 : SW == 2 ? 2 : 1;   // slots per 32-byte bucket
+  u64 w[GQ_R][4];
+  u32 pend = 0;
 #pragma unroll
-      for (int p = 0; p < NPAY; ++p) s[1 + p] = (u64)pay[p];
-      return true;
+  for (int j = 0; j < GQ_R; ++j) {
+    idx[j] = 0;
+    if (live[j]) {
+      if ((u64)key[j] == GQ_EMPTY) {   // reserved key pattern: unique table => at most one side entry (S14)
+        if (T.header[1] > 0) {
+#pragma unroll
+          for (int p = 0; p < NPAY; ++p) pay[j][p] = (i64)T.side[1 + p];
+          idx[j] = T.mask + 1;
+        } else live[j] = false;
+      } else {
+        idx[j] = gq_slot0(T, key[j]);
+        gq_ld256(T.slots + idx[j] * SW, w[j]);
+        pend |= 1u << j;
+      }
     }
-    if (unique && prev == (u64)key) { gq_set_err(err, GQ_E_DUPLICATE); return false; }
-    i = (i + 1) & T.mask;
-    prev = atomicCAS(T.slots + i * SW, GQ_EMPTY, (u64)key);
   }
-  gq_set_err(err, GQ_E_CAPACITY);
-  return false;
+  for (u64 round = 0; pend != 0; ++round) {
+#pragma unroll
+    for (int j = 0; j < GQ_R; ++j) {
+      if (pend & (1u << j)) {
+        bool done = false;
+#pragma unroll
+        for (int b = 0; b < B; ++b) {
+          const u64 kw = w[j][b * SW];
+          if (!done && kw == (u64)key[j]) {
+            done = true;
+            idx[j] += b;
+#pragma unroll
+            for (int p = 0; p < NPAY; ++p) pay[j][p] = (i64)w[j][b * SW + 1 + p];
+          } else if (!done && kw == GQ_EMPTY) { done = true; live[j] = false; }
+        }
+        if (!done && round * B > T.mask) { done = true; live[j] = false; }   // full table without the key
+        if (done) pend &= ~(1u << j);
+        else {
+          idx[j] = (idx[j] + B) & T.mask;
+          gq_ld256(T.slots + idx[j] * SW, w[j]);
+        }
+      }
+    }
+  }
 }
-template <int SW>
-__device__ __forceinline__ u64* gq_ht_upsert_pre(const GqTableDev& T, i64 key, u64 i, u64 k, bool* won, int* err) {
-  if ((u64)key == GQ_EMPTY) return gq_ht_upsert<SW>(T, key, won, err);
-  *won = false;
-  for (u64 n = 0; n <= T.mask; ++n) {
-    u64* s = T.slots + i * SW;
-    if (k == (u64)key) return s;
-    if (k == GQ_EMPTY) {
-      u64 prev = atomicCAS(s, GQ_EMPTY, (u64)key);
-      if (prev == GQ_EMPTY) { *won = true; return s; }
-      if (prev == (u64)key) return s;
+
+// HashBuild insert of GQ_R rows: read the bucket, CAS the first EMPTY slot seen, re-examine on a lost race.
+template <int SW, int NPAY>
+__device__ __forceinline__ int gq_insert_rows(const GqTableDev& T, const i64 (&key)[GQ_R], const bool (&live)[GQ_R],
+                                              const i64 (&pay)[GQ_R][NPAY > 0 ? NPAY : 1], bool unique, int* err) {
+  constexpr int B = SW == 1 ? 4 : SW == 2 ? 2 : 1;
+  u64 w[GQ_R][4];
+  u64 idx[GQ_R];
+  u32 pend = 0;
+  int ninserted = 0;
+#pragma unroll
+  for (int j = 0; j < GQ_R; ++j) {
+    idx[j] = 0;
+    if (live[j]) {
+      if ((u64)key[j] == GQ_EMPTY) { if (gq_ht_insert<SW, NPAY>(T, key[j], pay[j], unique, err)) ++ninserted; }
+      else {
+        idx[j] = gq_slot0(T, key[j]);
+        gq_ld256_relaxed(T.slots + idx[j] * SW, w[j]);
+        pend |= 1u << j;
+      }
     }
-    i = (i + 1) & T.mask;
-    k = gq_ld_relaxed(T.slots + i * SW);
   }
-  gq_set_err(err, GQ_E_CAPACITY);
-  return nullptr;
+  for (u64 round = 0; pend != 0; ++round) {
+#pragma unroll
+    for (int j = 0; j < GQ_R; ++j) {
+      if (pend & (1u << j)) {
+        int fb = -1;          // first EMPTY slot of the bucket
+        bool dup = false;
+#pragma unroll
+        for (int b = 0; b < B; ++b) {
+          const u64 kw = w[j][b * SW];
+          if (fb < 0 && kw == GQ_EMPTY) fb = b;
+          if (fb < 0 && kw == (u64)key[j]) dup = true;   // an equal key stored before the first free slot
+        }
+        if (unique && dup) { gq_set_err(err, GQ_E_DUPLICATE); pend &= ~(1u << j); }
+        else if (fb >= 0) {
+          u64* s = T.slots + (idx[j] + fb) * SW;
+          const u64 prev = atomicCAS(s, GQ_EMPTY, (u64)key[j]);
+          if (prev == GQ_EMPTY) {
+#pragma unroll
+            for (int p = 0; p < NPAY; ++p) s[1 + p] = (u64)pay[j][p];
+            ++ninserted;
+            pend &= ~(1u << j);
+          } else {
+#pragma unroll
+            for (int b = 0; b < B; ++b) if (b == fb) w[j][b * SW] = prev;   // lost the race: look at the bucket again
+          }
+        } else if (round > 2 * (T.mask + 1)) { gq_set_err(err, GQ_E_CAPACITY); pend &= ~(1u << j); }
+        else {
+          idx[j] = (idx[j] + B) & T.mask;
+          gq_ld256_relaxed(T.slots + idx[j] * SW, w[j]);
+        }
+      }
+    }
+  }
+  return ninserted;
+}
+
+// HashAggregation insert-or-update of GQ_R rows: slot[j] = the group's slot (null on error), won[j] = created it.
+template <int SW>
+__device__ __forceinline__ void gq_upsert_rows(const GqTableDev& T, const i64 (&key)[GQ_R], const bool (&live)[GQ_R],
+                                               u64* (&slot)[GQ_R], bool (&won)[GQ_R], int* err) {
+  u64 k[GQ_R], idx[GQ_R];
+  u32 pend = 0;
+#pragma unroll
+  for (int j = 0; j < GQ_R; ++j) {
+    slot[j] = nullptr; won[j] = false; idx[j] = 0; k[j] = GQ_EMPTY;
+    if (live[j]) {
+      if ((u64)key[j] == GQ_EMPTY) slot[j] = gq_ht_upsert<SW>(T, key[j], &won[j], err);
+      else {
+        idx[j] = gq_slot0(T, key[j]);
+        k[j] = gq_ld_relaxed(T.slots + idx[j] * SW);
+        pend |= 1u << j;
+      }
+    }
+  }
+  for (u64 round = 0; pend != 0; ++round) {
+#pragma unroll
+    for (int j = 0; j < GQ_R; ++j) {
+      if (pend & (1u << j)) {
+        u64* s = T.slots + idx[j] * SW;
+        if (k[j] == (u64)key[j]) { slot[j] = s; pend &= ~(1u << j); }
+        else if (k[j] == GQ_EMPTY) {
+          const u64 prev = atomicCAS(s, GQ_EMPTY, (u64)key[j]);
+          if (prev == GQ_EMPTY) { won[j] = true; slot[j] = s; pend &= ~(1u << j); }
+          else k[j] = prev;                         // somebody else claimed it: same key => next round returns it
+        } else if (round > 2 * (T.mask + 1)) { gq_set_err(err, GQ_E_CAPACITY); pend &= ~(1u << j); }
+        else {
+          idx[j] = (idx[j] + 1) & T.mask;
+          k[j] = gq_ld_relaxed(T.slots + idx[j] * SW);
+        }
+      }
+    }
+  }
 }
 
 // Aggregate update at L2 (RED.ADD / RED.MIN / RED.MAX .64 — results are not read back).
@@ -279,9 +425,11 @@ struct GqSrcGlobal {
 // Per-thread consumer context. Only the members the selected GQ_CONSUMER uses survive dead-code elimination.
 struct GqCtx {
   i64 acc[GQ_NAGG > 0 ? GQ_NAGG : 1];   // GLOBAL: register accumulators
-  i64* lc_keys;                         // LOWCARD: shared key table [GQ_LC_CAP + 1]
-  i64* lc_acc;                          // LOWCARD: shared accumulators [(GQ_LC_CAP+1) * GQ_NAGG * GQ_NT], lane-private
-  int* lc_side_used;
+  u64* lc_tab;                          // LOWCARD: shared key table [GQ_LC_KT]: {key32, gid} packed, or 64-bit keys
+  u32* lc_gid;                          //   group ids of the 64-bit key table [GQ_LC_KT]
+  i64* lc_gkey;                         //   key of every group id [GQ_LC_G]
+  int* lc_n;                            //   [0] groups so far, [1] insert lock, [2] gid of the reserved-pattern key + 1
+  i64* lc_acc;                          //   accumulators [GQ_LC_G][GQ_NAGG][GQ_NT], thread-private cells
   i64 ninserted;                        // BUILD: rows inserted by this thread
   i64* hot_keys;                        // HIGHCARD + GQ_HOT: shared set of this batch's hot keys [GQ_HOT_POS]
   u64* hot_acc;                         //   CTA-shared accumulators [GQ_HOT_POS][GQ_NAGG]
@@ -290,27 +438,130 @@ struct GqCtx {
   int t;
 };
 
-// Low-cardinality group-by: the CTA keeps a tiny open-addressing key table in shared memory (CAS only
-// the first time a key is seen); each consumer thread owns a PRIVATE accumulator cell per (group, aggregate), laid
-// out [group][agg][thread] so a warp's 32 cells are 32 consecutive 8-byte words: plain conflict-free LDS/add/STS,
-// no atomics, no shuffles on the per-row path. Cells are reduced over threads once, at the end, and flushed into the
-// global group-by table (the Partial -> Final merge of PAPER.md:154 inside one kernel).
-__device__ __forceinline__ int gq_lc_slot(GqCtx& cx, i64 key, int* err) {
-  if ((u64)key == GQ_EMPTY) { *cx.lc_side_used = 1; return GQ_LC_CAP; }
-  u32 i = (u32)gq_hash(key, 64 - 16) & (GQ_LC_CAP - 1);
-  for (int n = 0; n < GQ_LC_CAP; ++n, i = (i + 1) & (GQ_LC_CAP - 1)) {
-    i64 k = ((volatile i64*)cx.lc_keys)[i];
-    if (k == key) return (int)i;
-    if ((u64)k == GQ_EMPTY) {
-      u64 prev = atomicCAS((u64*)&cx.lc_keys[i], GQ_EMPTY, (u64)key);
-      if (prev == GQ_EMPTY || prev == (u64)key) return (int)i;
-    }
+// Low-cardinality group-by. The CTA keeps a small key table in shared memory that maps a packed key
+// to a dense group id (assigned the first time the key is seen, under a CTA lock — at most GQ_LC_G times per CTA).
+// Each consumer thread owns a PRIVATE accumulator cell per (group, aggregate), laid out [group][agg][thread] so a
+// warp's 32 cells are 32 consecutive 8-byte words: plain conflict-free LDS / add / STS, no atomics and no shuffles
+// on the per-row path. Cells are reduced over threads once, at the end (Partial -> Final of PAPER.md:154 inside one
+// kernel). Packed keys narrower than 32 bits use {key32, gid} entries fetched with one LDS.64.
+#define GQ_LC_LOG2KT (GQ_LC_KT == 64 ? 6 : GQ_LC_KT == 128 ? 7 : 8)
+__device__ __forceinline__ u32 gq_lc_hash(i64 key) {
+#if GQ_LC_KEY32
+  return ((u32)key * 0x9E3779B1u) >> (32 - GQ_LC_LOG2KT);
+#else
+  return (u32)gq_hash(key, 64 - GQ_LC_LOG2KT);
+#endif
+}
+// Fast path: walk the probe sequence until the key or an empty position (almost always the first position: the table
+// has >= 4x more positions than groups). Returns the group id, or -1 if the key is not in the table yet.
+__device__ __forceinline__ int gq_lc_find(const GqCtx& cx, i64 key) {
+  u32 h = gq_lc_hash(key);
+#if GQ_LC_KEY32
+  for (int n = 0; n < GQ_LC_KT; ++n, h = (h + 1) & (GQ_LC_KT - 1)) {
+    const u64 e = ((volatile u64*)cx.lc_tab)[h];
+    if ((u32)(e >> 32) == (u32)key) return (int)(u32)e;
+    if (e == ~0ULL) return -1;
   }
-  gq_set_err(err, GQ_E_CAPACITY);   // more distinct keys than max_groups
+#else
+  if ((u64)key == GQ_EMPTY) return ((volatile int*)cx.lc_n)[2] - 1;   // reserved bit pattern: id kept aside
+  for (int n = 0; n < GQ_LC_KT; ++n, h = (h + 1) & (GQ_LC_KT - 1)) {
+    const u64 k = ((volatile u64*)cx.lc_tab)[h];
+    if (k == (u64)key) return (int)((volatile u32*)cx.lc_gid)[h];
+    if (k == GQ_EMPTY) return -1;
+  }
+#endif
   return -1;
 }
-__device__ __forceinline__ void gq_lc_update(const int OP, GqCtx& cx, int slot, int a, i64 v) {
-  i64* cell = cx.lc_acc + ((slot * GQ_NAGG + a) * GQ_NT + cx.t);
+// One-probe form for the per-row path: group id if the first position holds the key, else -1 (then gq_lc_slow decides).
+__device__ __forceinline__ int gq_lc_find1(const GqCtx& cx, i64 key) {
+  const u32 h = gq_lc_hash(key);
+#if GQ_LC_KEY32
+  const u64 e = ((volatile u64*)cx.lc_tab)[h];
+  return (u32)(e >> 32) == (u32)key ? (int)(u32)e : -1;
+#else
+  const u64 k = ((volatile u64*)cx.lc_tab)[h];
+  return (k == (u64)key && k != GQ_EMPTY) ? (int)((volatile u32*)cx.lc_gid)[h] : -1;
+#endif
+}
+// Slow path (collision, or first sight of a key): the warp handles its needy lanes one key at a time; lane 0 takes
+// the CTA lock, walks the probe sequence and inserts the key with the next group id if it is absent. Must be called
+// by all 32 lanes of the warp (converged); `need` selects the lanes that want an answer.
+__device__ __forceinline__ int gq_lc_slow_body(GqCtx& cx, i64 key, bool need, int grp, int* err) {
+  u32 m = __ballot_sync(0xffffffffu, need);
+  const int lane = threadIdx.x & 31;
+  while (m) {
+    const int l = __ffs(m) - 1;
+    const i64 k = __shfl_sync(0xffffffffu, key, l);
+    int g = 0;
+    if (lane == 0) g = gq_lc_find(cx, k);          // another warp may have inserted it meanwhile: no lock needed
+    g = __shfl_sync(0xffffffffu, g, 0);
+    if (g < 0) {
+    if (lane == 0) {
+      bool locked = false;                      // wait for the lock OR for the key to appear (inserted by its holder)
+      while (g < 0 && !locked) { if (atomicCAS(&cx.lc_n[1], 0, 1) == 0) locked = true; else g = gq_lc_find(cx, k); }
+      if (locked) {
+      __threadfence_block();
+      if ((u64)k == GQ_EMPTY && !GQ_LC_KEY32) {        // reserved bit pattern: its group id lives in lc_n[2]
+        g = ((volatile int*)cx.lc_n)[2] - 1;
+        if (g < 0) {
+          g = ((volatile int*)cx.lc_n)[0];
+          if (g >= GQ_LC_G) { gq_set_err(err, GQ_E_CAPACITY); g = 0; }
+          else { cx.lc_gkey[g] = k; ((volatile int*)cx.lc_n)[0] = g + 1; ((volatile int*)cx.lc_n)[2] = g + 1; }
+        }
+      } else {
+        u32 i = gq_lc_hash(k);
+        g = -1;
+        for (int n = 0; n < GQ_LC_KT && g < 0; ++n, i = (i + 1) & (GQ_LC_KT - 1)) {
+#if GQ_LC_KEY32
+          const u64 e = ((volatile u64*)cx.lc_tab)[i];
+          if ((u32)(e >> 32) == (u32)k) g = (int)(u32)e;
+          else if (e == ~0ULL) {
+            g = ((volatile int*)cx.lc_n)[0];
+            if (g >= GQ_LC_G) { gq_set_err(err, GQ_E_CAPACITY); g = 0; }
+            else {
+              cx.lc_gkey[g] = k; ((volatile int*)cx.lc_n)[0] = g + 1;
+              ((volatile u64*)cx.lc_tab)[i] = ((u64)(u32)k << 32) | (u32)g;
+            }
+          }
+#else
+          const u64 e = ((volatile u64*)cx.lc_tab)[i];
+          if (e == (u64)k) g = (int)((volatile u32*)cx.lc_gid)[i];
+          else if (e == GQ_EMPTY) {
+            g = ((volatile int*)cx.lc_n)[0];
+            if (g >= GQ_LC_G) { gq_set_err(err, GQ_E_CAPACITY); g = 0; }
+            else {
+              cx.lc_gkey[g] = k; ((volatile int*)cx.lc_n)[0] = g + 1;
+              ((volatile u32*)cx.lc_gid)[i] = (u32)g;
+              __threadfence_block();                    // readers match the key first, then read the id
+              ((volatile u64*)cx.lc_tab)[i] = (u64)k;
+            }
+          }
+#endif
+        }
+        if (g < 0) { gq_set_err(err, GQ_E_CAPACITY); g = 0; }   // key table full (more distinct keys than max_groups)
+      }
+      __threadfence_block();
+      atomicExch(&cx.lc_n[1], 0);
+      }
+    }
+    g = __shfl_sync(0xffffffffu, g, 0);
+    }
+    if (need && key == k) { grp = g; need = false; }   // every lane waiting for this key is served at once
+    m = __ballot_sync(0xffffffffu, need);
+  }
+  return grp;
+}
+// Out of line: the per-row code only carries a call, not four inlined copies of the insert protocol.
+__device__ __noinline__ int gq_lc_slow_call(u64* tab, u32* gid, i64* gkey, int* n, i64 key, bool need, int grp, int* err) {
+  GqCtx c;
+  c.lc_tab = tab; c.lc_gid = gid; c.lc_gkey = gkey; c.lc_n = n;
+  return gq_lc_slow_body(c, key, need, grp, err);
+}
+__device__ __forceinline__ int gq_lc_slow(GqCtx& cx, i64 key, bool need, int grp, int* err) {
+  return gq_lc_slow_call(cx.lc_tab, cx.lc_gid, cx.lc_gkey, cx.lc_n, key, need, grp, err);
+}
+__device__ __forceinline__ void gq_lc_update(const int OP, GqCtx& cx, int grp, int a, i64 v) {
+  i64* cell = cx.lc_acc + ((grp * GQ_NAGG + a) * GQ_NT + cx.t);
   *cell = gq_combine(OP, *cell, v);
 }
 

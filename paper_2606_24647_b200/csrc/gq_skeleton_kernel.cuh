@@ -1,14 +1,21 @@
-// gq_skeleton_kernel.cuh — second half of the fused scan kernel (follows the generated gq_pass / gq_body).
+// gq_skeleton_kernel.cuh — second half of the fused scan kernel (follows the generated row functions).
 
 // Shared-memory layout (dynamic): [GQ_STAGES stages][full/empty mbarriers][consumer area]
 #define GQ_BAR_OFF (GQ_STAGES * GQ_STAGE_BYTES)
 #define GQ_CONS_OFF (GQ_BAR_OFF + 2 * GQ_STAGES * 8 + 64)
-#define GQ_LC_KEYS_BYTES (((GQ_LC_CAP + 1) * 8 + 8 + 127) / 128 * 128)
+// LOWCARD consumer area: key table, group ids, group keys, counters, final values, then the private cells
+#define GQ_LC_GID_OFF (GQ_LC_KT * 8)
+#define GQ_LC_GKEY_OFF (GQ_LC_KT * 12)
+#define GQ_LC_N_OFF (GQ_LC_GKEY_OFF + GQ_LC_G * 8)
+#define GQ_LC_FIN_OFF (GQ_LC_N_OFF + 16)
+#define GQ_LC_HEAD_BYTES ((GQ_LC_FIN_OFF + GQ_LC_G * GQ_NAGG * 8 + 127) / 128 * 128)
 
 template <class Src>
 __device__ __forceinline__ void gq_process(const GqParams& P, const Src& src, GqCtx& cx, int nvalid_j, bool full) {
 #if GQ_LINEAR
-  gq_tile(P, src, cx, nvalid_j, full);   // generated: the GQ_R rows advance step by step, accesses issued before use
+  // generated: the GQ_R rows advance step by step, accesses issued before use
+  if (full) gq_tile<Src, true>(P, src, cx, nvalid_j);
+  else gq_tile<Src, false>(P, src, cx, nvalid_j);
 #else
   // Evaluate the filter for all GQ_R rows first (independent shared-memory loads in flight together), then run the
   // body (probes, projection, consumer) only for passing rows.
@@ -21,13 +28,63 @@ __device__ __forceinline__ void gq_process(const GqParams& P, const Src& src, Gq
 #endif
 }
 
+__device__ __forceinline__ i64 gq_ldcg(const i64* p) { return __ldcg(p); }
+
+#if GQ_FUSED_FINAL
+__device__ __forceinline__ i64 gq_fin_sext(u64 v, int bits) {
+  if (bits >= 64) return (i64)v;
+  const u64 m = 1ULL << (bits - 1);
+  v &= (1ULL << bits) - 1;
+  return (i64)((v ^ m) - m);
+}
+__device__ __forceinline__ void gq_fin_store_key(void* col, int dtype, i64 idx, i64 v) {
+  if (dtype == 1) ((signed char*)col)[idx] = (signed char)v;
+  else if (dtype == 2) ((int*)col)[idx] = (int)v;
+  else ((i64*)col)[idx] = v;
+}
+// One output row: keys unpacked from the packed key word, aggregates, derived AVG = double(sum) / double(count).
+__device__ __forceinline__ void gq_fin_emit(const GqFinal& F, i64 row, i64 key, const i64* vals) {
+  if (F.nkeys == 1) gq_fin_store_key(F.out_key[0], F.key_dtype[0], row, key);
+  else if (F.nkeys == 2) {
+    gq_fin_store_key(F.out_key[0], F.key_dtype[0], row, gq_fin_sext((u64)key, F.key_bits[0]));
+    gq_fin_store_key(F.out_key[1], F.key_dtype[1], row, gq_fin_sext((u64)key >> F.key_bits[0], F.key_bits[1]));
+  }
+#pragma unroll
+  for (int a = 0; a < GQ_NAGG; ++a) F.out_agg[a][row] = vals[a];
+  for (int v = 0; v < F.navg; ++v) F.out_avg[v][row] = (double)vals[F.avg_sum[v]] / (double)vals[F.avg_cnt[v]];
+}
+#endif
+
+#if GQ_CONSUMER == GQ_C_LOWCARD
+// Reduces the GQ_NT private cells of pair p = group * GQ_NAGG + a over the warp's lanes; every lane gets the result.
+__device__ __forceinline__ i64 gq_lc_reduce_pair(const GqCtx& cx, int p, int a, int lane) {
+  i64 v = 0;
+  const i64* cells = cx.lc_acc + (size_t)p * GQ_NT;
+#pragma unroll
+  for (int aa = 0; aa < GQ_NAGG; ++aa) {
+    if (aa == a) {   // the aggregate's op is a compile-time property of aa
+      v = gq_identity(GQ_AGG_OP(aa));
+#pragma unroll 4
+      for (int i = lane; i < GQ_NT; i += 32) v = gq_combine(GQ_AGG_OP(aa), v, cells[i]);
+      v = gq_warp_reduce(GQ_AGG_OP(aa), v);
+    }
+  }
+  return v;
+}
+#endif
+
 extern "C" __global__ void __launch_bounds__(GQ_NT + 32, 1) gq_scan(const __grid_constant__ GqParams P) {
   extern __shared__ __align__(128) unsigned char gq_smem[];
   u64* full_bar = (u64*)(gq_smem + GQ_BAR_OFF);
   u64* empty_bar = full_bar + GQ_STAGES;
   const int tid = threadIdx.x;
   const i64 ntiles = P.nrows / GQ_TILE;                  // full tiles; the remainder is the tail
-  if (*(volatile int*)P.err != 0) return;                // sticky error: later kernels are no-ops (gq.h "Errors")
+  if (*(volatile int*)P.err != 0) {                      // sticky error: later kernels are no-ops (gq.h "Errors")
+#if GQ_FUSED_FINAL
+    if (tid == 0) { const u32 t = atomicAdd(P.fin.ticket, 1u); if (t == gridDim.x - 1) *P.fin.ticket = 0; }
+#endif
+    return;
+  }
 
   if (tid == 0) {
     for (int s = 0; s < GQ_STAGES; ++s) { gq_mbar_init(&full_bar[s], 1); gq_mbar_init(&empty_bar[s], GQ_NWARP); }
@@ -37,15 +94,17 @@ extern "C" __global__ void __launch_bounds__(GQ_NT + 32, 1) gq_scan(const __grid
   cx.t = tid;
   cx.ninserted = 0;
 #if GQ_CONSUMER == GQ_C_LOWCARD
-  cx.lc_keys = (i64*)(gq_smem + GQ_CONS_OFF);
-  cx.lc_side_used = (int*)(cx.lc_keys + GQ_LC_CAP + 1);
-  cx.lc_acc = (i64*)(gq_smem + GQ_CONS_OFF + GQ_LC_KEYS_BYTES);
+  cx.lc_tab = (u64*)(gq_smem + GQ_CONS_OFF);
+  cx.lc_gid = (u32*)(gq_smem + GQ_CONS_OFF + GQ_LC_GID_OFF);
+  cx.lc_gkey = (i64*)(gq_smem + GQ_CONS_OFF + GQ_LC_GKEY_OFF);
+  cx.lc_n = (int*)(gq_smem + GQ_CONS_OFF + GQ_LC_N_OFF);
+  cx.lc_acc = (i64*)(gq_smem + GQ_CONS_OFF + GQ_LC_HEAD_BYTES);
   if (tid < GQ_NT) {
-    for (int i = tid; i <= GQ_LC_CAP; i += GQ_NT) cx.lc_keys[i] = (i64)GQ_EMPTY;
-    if (tid == 0) *cx.lc_side_used = 0;
+    for (int i = tid; i < GQ_LC_KT; i += GQ_NT) cx.lc_tab[i] = GQ_LC_KEY32 ? ~0ULL : GQ_EMPTY;
+    if (tid < 4) cx.lc_n[tid] = 0;
 #pragma unroll
     for (int a = 0; a < GQ_NAGG; ++a)
-      for (int g = 0; g <= GQ_LC_CAP; ++g) cx.lc_acc[(g * GQ_NAGG + a) * GQ_NT + tid] = gq_identity(GQ_AGG_OP(a));
+      for (int g = 0; g < GQ_LC_G; ++g) cx.lc_acc[(g * GQ_NAGG + a) * GQ_NT + tid] = gq_identity(GQ_AGG_OP(a));
   }
 #endif
 #if GQ_CONSUMER == GQ_C_GLOBAL
@@ -125,14 +184,17 @@ extern "C" __global__ void __launch_bounds__(GQ_NT + 32, 1) gq_scan(const __grid
   }
 
   // -------------------------------------------------------------------- consumer epilogues
+  const int lane = tid & 31, warp = tid >> 5;
+  (void)lane; (void)warp;
 #if GQ_CONSUMER == GQ_C_GLOBAL
   {
-    // warp shuffle -> shared -> one atomic per CTA per aggregate
-    i64* red = (i64*)(gq_smem + GQ_CONS_OFF);            // [GQ_NAGG][GQ_NWARP]
+    // warp shuffle -> shared -> one value per CTA per aggregate
+    i64* red = (i64*)(gq_smem + GQ_CONS_OFF);            // [GQ_NAGG][GQ_NWARP], then [4] flags
+    int* flag = (int*)(red + GQ_NAGG * GQ_NWARP);
 #pragma unroll
     for (int a = 0; a < GQ_NAGG; ++a) {
       i64 v = gq_warp_reduce(GQ_AGG_OP(a), cx.acc[a]);
-      if ((tid & 31) == 0) red[a * GQ_NWARP + (tid >> 5)] = v;
+      if (lane == 0) red[a * GQ_NWARP + warp] = v;
     }
     gq_consumer_barrier();
     if (tid < 32) {
@@ -141,35 +203,123 @@ extern "C" __global__ void __launch_bounds__(GQ_NT + 32, 1) gq_scan(const __grid
         i64 v = gq_identity(GQ_AGG_OP(a));
         for (int w = tid; w < GQ_NWARP; w += 32) v = gq_combine(GQ_AGG_OP(a), v, red[a * GQ_NWARP + w]);
         v = gq_warp_reduce(GQ_AGG_OP(a), v);
+#if GQ_FUSED_FINAL
+        if (tid == 0) P.fin.part[(i64)blockIdx.x * GQ_NAGG + a] = v;
+#else
         if (tid == 0) gq_red(GQ_AGG_OP(a), (u64*)&P.acc[a], v);
+#endif
       }
     }
+#if GQ_FUSED_FINAL
+    // last CTA to finish merges the per-CTA partials and writes the single output row
+    if (tid == 0) { __threadfence(); flag[0] = (atomicAdd(P.fin.ticket, 1u) == gridDim.x - 1); }
+    gq_consumer_barrier();
+    if (flag[0]) {
+      __threadfence();
+#pragma unroll
+      for (int a = 0; a < GQ_NAGG; ++a) {
+        i64 v = gq_identity(GQ_AGG_OP(a));
+        for (int b = tid; b < (int)gridDim.x; b += GQ_NT) v = gq_combine(GQ_AGG_OP(a), v, gq_ldcg(P.fin.part + (i64)b * GQ_NAGG + a));
+        v = gq_warp_reduce(GQ_AGG_OP(a), v);
+        if (lane == 0) red[a * GQ_NWARP + warp] = v;
+      }
+      gq_consumer_barrier();
+      if (tid == 0) {
+        i64 vals[GQ_NAGG];
+#pragma unroll
+        for (int a = 0; a < GQ_NAGG; ++a) {
+          i64 v = gq_identity(GQ_AGG_OP(a));
+          for (int w = 0; w < GQ_NWARP; ++w) v = gq_combine(GQ_AGG_OP(a), v, red[a * GQ_NWARP + w]);
+          vals[a] = v;
+        }
+        if (P.fin.out_capacity >= 1) gq_fin_emit(P.fin, 0, 0, vals);
+        else gq_set_err(P.err, GQ_E_CAPACITY);
+        *P.fin.out_n = 1;
+        *P.fin.ticket = 0;
+      }
+    }
+#endif
   }
 #endif
 #if GQ_CONSUMER == GQ_C_LOWCARD
   {
     gq_consumer_barrier();
-    // one thread per (group position, aggregate): reduce the GQ_NT private cells, merge into the global table
-    for (int pa = tid; pa < (GQ_LC_CAP + 1) * GQ_NAGG; pa += GQ_NT) {
-      const int g = pa / GQ_NAGG, a = pa % GQ_NAGG;
-      const bool used = g < GQ_LC_CAP ? ((u64)cx.lc_keys[g] != GQ_EMPTY) : (*cx.lc_side_used != 0);
-      if (!used) continue;
-      const i64 key = g < GQ_LC_CAP ? cx.lc_keys[g] : (i64)GQ_EMPTY;
-      const i64* cells = cx.lc_acc + (size_t)pa * GQ_NT;
-      i64 v = 0;
-      bool won;
-      u64* slot = gq_ht_upsert<GQ_TARGET_SW>(P.target, key, &won, P.err);
-      if (!slot) continue;
-      // the aggregate's op is only known per `a` at compile time: dispatch over the (few) aggregates
+    const int ng = ((volatile int*)cx.lc_n)[0];
+#if !GQ_FUSED_FINAL
+    // one warp per (group, aggregate): reduce the GQ_NT private cells, merge into the global table
+    for (int p = warp; p < ng * GQ_NAGG; p += GQ_NWARP) {
+      const int g = p / GQ_NAGG, a = p % GQ_NAGG;
+      const i64 v = gq_lc_reduce_pair(cx, p, a, lane);
+      if (lane == 0) {
+        bool won;
+        u64* slot = gq_ht_upsert<GQ_TARGET_SW>(P.target, cx.lc_gkey[g], &won, P.err);
+        if (slot) {
 #pragma unroll
-      for (int aa = 0; aa < GQ_NAGG; ++aa) {
-        if (aa == a) {
-          v = gq_identity(GQ_AGG_OP(aa));
-          for (int i = 0; i < GQ_NT; ++i) v = gq_combine(GQ_AGG_OP(aa), v, cells[(i + tid) % GQ_NT]);
-          gq_red(GQ_AGG_OP(aa), slot + 1 + GQ_NDEP + aa, v);
+          for (int aa = 0; aa < GQ_NAGG; ++aa)
+            if (aa == a) gq_red(GQ_AGG_OP(aa), slot + 1 + GQ_NDEP + aa, v);
         }
       }
     }
+#else
+    // ---- finaliser fused into the scan: partials -> global scratch -> ticket -> last CTA merges and emits
+    constexpr int PW = 1 + GQ_NAGG;                      // words per partial group: key, aggregates
+    i64* mypart = P.fin.part + (i64)blockIdx.x * GQ_LC_G * PW;
+    i64* pn = P.fin.part + (i64)gridDim.x * GQ_LC_G * PW;
+    i64* fin = (i64*)(gq_smem + GQ_CONS_OFF + GQ_LC_FIN_OFF);
+    for (int p = warp; p < ng * GQ_NAGG; p += GQ_NWARP) {
+      const int g = p / GQ_NAGG, a = p % GQ_NAGG;
+      const i64 v = gq_lc_reduce_pair(cx, p, a, lane);
+      if (lane == 0) { mypart[g * PW + 1 + a] = v; if (a == 0) mypart[g * PW] = cx.lc_gkey[g]; }
+    }
+    if (tid == 0) pn[blockIdx.x] = ng;
+    gq_consumer_barrier();
+    if (tid == 0) { __threadfence(); cx.lc_n[3] = (atomicAdd(P.fin.ticket, 1u) == gridDim.x - 1); }
+    gq_consumer_barrier();
+    if (((volatile int*)cx.lc_n)[3]) {
+      __threadfence();
+#pragma unroll
+      for (int a = 0; a < GQ_NAGG; ++a)
+        for (int g = 0; g < GQ_LC_G; ++g) cx.lc_acc[(g * GQ_NAGG + a) * GQ_NT + tid] = gq_identity(GQ_AGG_OP(a));
+      // fold every CTA's partial groups into this CTA's private cells: one (CTA, group) pair per thread and round,
+      // the loads of four rounds issued together (group ids are those of THIS CTA's key table)
+      const int npairs = (int)gridDim.x * GQ_LC_G;
+      for (int p0 = 0; p0 < npairs; p0 += 4 * GQ_NT) {   // uniform bounds: the slow path needs converged warps
+        i64 w[4][PW];
+        i64 nb[4];
+#pragma unroll
+        for (int u = 0; u < 4; ++u) {
+          const int p = p0 + u * GQ_NT + tid;
+          const int pc = p < npairs ? p : 0;
+          nb[u] = gq_ldcg(pn + pc / GQ_LC_G);
+#pragma unroll
+          for (int i = 0; i < PW; ++i) w[u][i] = gq_ldcg(P.fin.part + (i64)pc * PW + i);   // stale beyond the CTA's count
+        }
+#pragma unroll
+        for (int u = 0; u < 4; ++u) {
+          const int p = p0 + u * GQ_NT + tid;
+          const bool have = p < npairs && (p % GQ_LC_G) < (int)nb[u];
+          int grp = have ? gq_lc_find(cx, w[u][0]) : 0;
+          if (__any_sync(0xffffffffu, have && grp < 0)) grp = gq_lc_slow(cx, w[u][0], have && grp < 0, grp, P.err);
+          if (have) {
+#pragma unroll
+            for (int a = 0; a < GQ_NAGG; ++a) gq_lc_update(GQ_AGG_OP(a), cx, grp, a, w[u][1 + a]);
+          }
+        }
+      }
+      gq_consumer_barrier();
+      const int ng2 = ((volatile int*)cx.lc_n)[0];
+      for (int p = warp; p < ng2 * GQ_NAGG; p += GQ_NWARP) {
+        const i64 v = gq_lc_reduce_pair(cx, p, p % GQ_NAGG, lane);
+        if (lane == 0) fin[p] = v;
+      }
+      gq_consumer_barrier();
+      if (tid < ng2) {
+        if (tid < P.fin.out_capacity) gq_fin_emit(P.fin, tid, cx.lc_gkey[tid], fin + tid * GQ_NAGG);
+        else gq_set_err(P.err, GQ_E_CAPACITY);
+      }
+      if (tid == 0) { *P.fin.out_n = ng2; *P.fin.ticket = 0; }
+    }
+#endif
   }
 #endif
 #if GQ_HOT
@@ -188,7 +338,7 @@ extern "C" __global__ void __launch_bounds__(GQ_NT + 32, 1) gq_scan(const __grid
 #if GQ_CONSUMER == GQ_C_BUILD
   {
     i64 v = gq_warp_reduce(GQ_OP_SUM, cx.ninserted);
-    if ((tid & 31) == 0 && v != 0) atomicAdd((u64*)&P.target.header[0], (u64)v);
+    if (lane == 0 && v != 0) atomicAdd((u64*)&P.target.header[0], (u64)v);
   }
 #endif
 }

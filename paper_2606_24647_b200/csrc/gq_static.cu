@@ -55,18 +55,38 @@ __device__ __forceinline__ void gq_store_key(void* col, int dtype, i64 idx, i64 
   else if (dtype == GQ_I32) ((int*)col)[idx] = (int)v;
   else ((i64*)col)[idx] = v;
 }
-// Emits one group (slot words s[], key word `key`) at output row idx.
-__device__ __forceinline__ void gq_emit_group(const GqFinaliseParams& P, const u64* s, u64 key, i64 idx) {
-  const int nhashed = P.nkeys - P.ndep;
-  if (nhashed == 1) gq_store_key(P.out_key[0], P.key_dtype[0], idx, (i64)key);
-  else if (nhashed == 2) {
-    gq_store_key(P.out_key[0], P.key_dtype[0], idx, gq_sext(key, P.key_bits[0]));
-    gq_store_key(P.out_key[1], P.key_dtype[1], idx, gq_sext(key >> P.key_bits[0], P.key_bits[1]));
+// A group as the finalisers see it. Hashed state: slot i of the group-by table (key word, dependent words, aggregate
+// words). Direct state: accumulator slot i is a group iff its touch word (a COUNT) is non-zero; key and dependent key
+// come from slot i of the join table the scan probed. Index `capacity` (direct) / -2 (hashed) names the side entry.
+struct GqGroupRef { u64 key; const u64* dep; const u64* agg; };
+__device__ __forceinline__ bool gq_group_at(const GqFinaliseParams& P, i64 i, GqGroupRef* g) {
+  if (P.direct) {
+    const u64* acc = P.dacc + i * P.daw;
+    if (acc[P.dtouch] == 0) return false;
+    const u64* js = i < P.capacity ? P.jslots + i * P.jsw : P.jside;
+    g->key = i < P.capacity ? js[0] : GQ_EMPTY_KEY;
+    g->dep = js + 1 + (P.dep_pay > 0 ? P.dep_pay : 0);
+    g->agg = acc;
+    return true;
   }
-  for (int d = 0; d < P.ndep; ++d) gq_store_key(P.out_key[nhashed + d], P.key_dtype[nhashed + d], idx, (i64)s[1 + d]);
-  for (int a = 0; a < P.naggs; ++a) P.out_agg[a][idx] = (i64)s[1 + P.ndep + a];
+  const u64* s = i == -2 ? P.side : P.slots + i * P.slot_words;
+  g->key = i == -2 ? GQ_EMPTY_KEY : s[0];
+  g->dep = s + 1;
+  g->agg = s + 1 + P.ndep;
+  return i == -2 ? P.header[1] != 0 : g->key != GQ_EMPTY_KEY;
+}
+// Emits one group at output row idx.
+__device__ __forceinline__ void gq_emit_group(const GqFinaliseParams& P, const GqGroupRef& g, i64 idx) {
+  const int nhashed = P.nkeys - P.ndep;
+  if (nhashed == 1) gq_store_key(P.out_key[0], P.key_dtype[0], idx, (i64)g.key);
+  else if (nhashed == 2) {
+    gq_store_key(P.out_key[0], P.key_dtype[0], idx, gq_sext(g.key, P.key_bits[0]));
+    gq_store_key(P.out_key[1], P.key_dtype[1], idx, gq_sext(g.key >> P.key_bits[0], P.key_bits[1]));
+  }
+  for (int d = 0; d < P.ndep; ++d) gq_store_key(P.out_key[nhashed + d], P.key_dtype[nhashed + d], idx, (i64)g.dep[d]);
+  for (int a = 0; a < P.naggs; ++a) P.out_agg[a][idx] = (i64)g.agg[a];
   for (int v = 0; v < P.navg; ++v)
-    P.out_avg[v][idx] = (double)(i64)s[1 + P.ndep + P.avg_sum[v]] / (double)(i64)s[1 + P.ndep + P.avg_cnt[v]];
+    P.out_avg[v][idx] = (double)(i64)g.agg[P.avg_sum[v]] / (double)(i64)g.agg[P.avg_cnt[v]];
 }
 
 // One thread per GQ_FIN_PER slots; block-level compaction: ballot/popc inside warps, shared-memory scan over warps,
@@ -81,13 +101,14 @@ __global__ void __launch_bounds__(GQ_FIN_THREADS) gq_k_finalise(const __grid_con
   const i64 nblocks_slots = (P.capacity + GQ_FIN_THREADS * GQ_FIN_PER - 1) / (GQ_FIN_THREADS * GQ_FIN_PER);
   for (i64 b = blockIdx.x; b < nblocks_slots; b += gridDim.x) {
     const i64 base = b * (GQ_FIN_THREADS * GQ_FIN_PER);
-    u64 key[GQ_FIN_PER];
+    GqGroupRef grp[GQ_FIN_PER];
+    bool have[GQ_FIN_PER];
     int mine = 0;
 #pragma unroll
     for (int j = 0; j < GQ_FIN_PER; ++j) {
       i64 i = base + j * GQ_FIN_THREADS + threadIdx.x;
-      key[j] = (i < P.capacity) ? P.slots[i * P.slot_words] : GQ_EMPTY_KEY;
-      mine += (key[j] != GQ_EMPTY_KEY);
+      have[j] = (i < P.capacity) && gq_group_at(P, i, &grp[j]);
+      mine += have[j];
     }
     // exclusive prefix of `mine` inside the block
     int incl = mine;
@@ -104,18 +125,18 @@ __global__ void __launch_bounds__(GQ_FIN_THREADS) gq_k_finalise(const __grid_con
     i64 idx = block_base + warp_cnt[warp] + (incl - mine);
 #pragma unroll
     for (int j = 0; j < GQ_FIN_PER; ++j) {
-      if (key[j] == GQ_EMPTY_KEY) continue;
-      i64 i = base + j * GQ_FIN_THREADS + threadIdx.x;
-      if (idx < P.out_capacity) gq_emit_group(P, P.slots + i * P.slot_words, key[j], idx);
+      if (!have[j]) continue;
+      if (idx < P.out_capacity) gq_emit_group(P, grp[j], idx);
       else atomicCAS(P.err, 0, (int)GQ_ERR_CAPACITY);
       ++idx;
     }
     __syncthreads();
   }
   // the side slot: the group whose key equals the reserved EMPTY pattern, or THE group of a key-less aggregation
-  if (blockIdx.x == 0 && threadIdx.x == 0 && P.header[1] != 0) {
+  GqGroupRef sg;
+  if (blockIdx.x == 0 && threadIdx.x == 0 && gq_group_at(P, P.direct ? P.capacity : -2, &sg)) {
     i64 idx = (i64)atomicAdd((u64*)P.out_n, 1ULL);
-    if (idx < P.out_capacity) gq_emit_group(P, P.side, GQ_EMPTY_KEY, idx);
+    if (idx < P.out_capacity) gq_emit_group(P, sg, idx);
     else atomicCAS(P.err, 0, (int)GQ_ERR_CAPACITY);
   }
 }
@@ -148,13 +169,13 @@ __device__ __forceinline__ void gq_list_insert(GqCand& mine, const GqCand& c, in
   if (lane == pos) mine = c;
   else if (lane > pos) mine = up;
 }
-__device__ __forceinline__ GqCand gq_make_cand(const GqFinaliseParams& P, const u64* s, u64 key, i64 slot) {
+__device__ __forceinline__ GqCand gq_make_cand(const GqFinaliseParams& P, const GqGroupRef& g, i64 slot) {
   GqCand c;
   c.valid = 1; c.slot = slot; c.k1 = 0;
-  c.val = (i64)s[1 + P.ndep + P.topk_agg];
+  c.val = (i64)g.agg[P.topk_agg];
   const int nhashed = P.nkeys - P.ndep;
-  if (nhashed == 2) { c.k0 = gq_sext(key, P.key_bits[0]); c.k1 = gq_sext(key >> P.key_bits[0], P.key_bits[1]); }
-  else { c.k0 = (i64)key; if (P.ndep) c.k1 = (i64)s[1]; }
+  if (nhashed == 2) { c.k0 = gq_sext(g.key, P.key_bits[0]); c.k1 = gq_sext(g.key >> P.key_bits[0], P.key_bits[1]); }
+  else { c.k0 = (i64)g.key; if (P.ndep) c.k1 = (i64)g.dep[0]; }
   return c;
 }
 // Feeds the candidates held by the lanes in `m` (each better than the list's current worst) into the list.
@@ -180,18 +201,17 @@ __global__ void __launch_bounds__(GQ_TOPK_WARPS * 32) gq_k_topk_scan(const __gri
   if (gw == 0) {   // the side slot
     GqCand c; c.valid = 0; c.val = 0; c.k0 = 0; c.k1 = 0; c.slot = -1;
     bool want = false;
-    if (lane == 0 && P.header[1] != 0) { c = gq_make_cand(P, P.side, GQ_EMPTY_KEY, -2); want = true; }
+    GqGroupRef g;
+    const i64 si = P.direct ? P.capacity : -2;
+    if (lane == 0 && gq_group_at(P, si, &g)) { c = gq_make_cand(P, g, si); want = true; }
     gq_list_feed(mine, c, want, lane);
   }
   for (i64 i0 = gw * 32; i0 < P.capacity; i0 += nw * 32) {
     i64 i = i0 + lane;
     GqCand c; c.valid = 0; c.val = 0; c.k0 = 0; c.k1 = 0; c.slot = -1;
     bool want = false;
-    if (i < P.capacity) {
-      const u64* s = P.slots + i * P.slot_words;
-      u64 key = s[0];
-      if (key != GQ_EMPTY_KEY) { c = gq_make_cand(P, s, key, i); want = true; }
-    }
+    GqGroupRef g;
+    if (i < P.capacity && gq_group_at(P, i, &g)) { c = gq_make_cand(P, g, i); want = true; }
     GqCand worst = gq_cand_shfl(mine, 31);
     want = want && gq_better(c, worst);
     gq_list_feed(mine, c, want, lane);
@@ -234,10 +254,9 @@ __global__ void __launch_bounds__(GQ_TOPK_MERGE_WARPS * 32) gq_k_topk_merge(cons
   unsigned have = __ballot_sync(0xffffffffu, mine.valid != 0);
   int n = min(__popc(have), P.topk);
   if (lane < n) {
-    if (lane < P.out_capacity) {
-      const u64* s = mine.slot == -2 ? P.side : P.slots + mine.slot * P.slot_words;
-      gq_emit_group(P, s, mine.slot == -2 ? GQ_EMPTY_KEY : s[0], lane);
-    } else atomicCAS(P.err, 0, (int)GQ_ERR_CAPACITY);
+    GqGroupRef g;
+    if (lane < P.out_capacity) { gq_group_at(P, mine.slot, &g); gq_emit_group(P, g, lane); }
+    else atomicCAS(P.err, 0, (int)GQ_ERR_CAPACITY);
   }
   if (lane == 0) *P.out_n = n;
 }

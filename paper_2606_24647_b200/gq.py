@@ -34,7 +34,7 @@ STATUS = ["GQ_OK", "GQ_ERR_INVALID_ARG", "GQ_ERR_UNSUPPORTED", "GQ_ERR_CAPACITY"
 SYMBOLS = ["gq_create", "gq_destroy", "gq_sync", "gq_clear_error", "gq_status_str", "gq_last_cuda_error",
            "gq_last_message", "gq_launch_count", "gq_filter_project", "gq_hash_build_workspace", "gq_hash_build",
            "gq_hash_build_finish", "gq_table_count", "gq_table_destroy", "gq_hash_probe",
-           "gq_hash_aggregate_workspace", "gq_hash_aggregate", "gq_topk_scratch_bytes", "gq_hash_aggregate_finish",
+           "gq_hash_aggregate_workspace", "gq_hash_aggregate_workspace_for", "gq_hash_aggregate", "gq_topk_scratch_bytes", "gq_hash_aggregate_finish",
            "gq_aggstate_destroy", "gq_pipeline_workspace", "gq_pipeline", "gq_pipeline_host_workspace",
            "gq_pipeline_host", "gq_set_kernel_cache_dir", "gq_precompile_pipeline", "gq_precompile_build",
            "gq_table_describe", "gq_read_probe"]
@@ -124,6 +124,7 @@ def lib():
         L.gq_hash_probe.argtypes = [C.c_void_p, C.POINTER(_Batch), C.POINTER(_Pred), C.c_int32, C.POINTER(_Probe),
                                     C.c_int32, C.POINTER(_Expr), C.c_int32, C.POINTER(C.c_void_p), C.c_int64, C.c_void_p]
         L.gq_hash_aggregate_workspace.argtypes = [C.c_int64, C.c_int32, C.c_int32, C.POINTER(C.c_size_t)]
+        L.gq_hash_aggregate_workspace_for.argtypes = [C.POINTER(_Batch), C.POINTER(_AggDesc), C.POINTER(C.c_size_t)]
         L.gq_hash_aggregate.argtypes = [C.c_void_p, C.POINTER(C.c_void_p), C.c_void_p, C.c_size_t, C.POINTER(_Batch),
                                         C.POINTER(_AggDesc)]
         L.gq_hash_aggregate_finish.argtypes = [C.c_void_p, C.c_void_p, C.POINTER(C.c_void_p), C.POINTER(C.c_void_p),
@@ -384,14 +385,19 @@ class Context:
         return out
 
     # ---- HashAggregation (streaming) ----
-    def aggregate(self, state, cols, preds=(), probes=(), exprs=(), keys=(), ndependent=0, aggs=(), max_groups=1):
+    def aggregate(self, state, cols, preds=(), probes=(), exprs=(), keys=(), ndependent=0, aggs=(), max_groups=1,
+                  plan_aware_workspace=False):
+        """plan_aware_workspace: size the state with gq_hash_aggregate_workspace_for (enables direct aggregation)."""
         with torch.cuda.stream(self.stream):
             m = _M()
             b = m.batch(cols)
             d = m.agg_desc(preds, probes, exprs, keys, ndependent, aggs, max_groups)
             if state is None:
                 nbytes = C.c_size_t()
-                self._check(self.L.gq_hash_aggregate_workspace(int(max_groups), len(keys), len(aggs), C.byref(nbytes)))
+                if plan_aware_workspace:
+                    self._check(self.L.gq_hash_aggregate_workspace_for(C.byref(b), C.byref(d), C.byref(nbytes)))
+                else:
+                    self._check(self.L.gq_hash_aggregate_workspace(int(max_groups), len(keys), len(aggs), C.byref(nbytes)))
                 ws = self._ws(nbytes.value)
                 dts = _row_dtypes(cols, probes)
                 h = C.c_void_p()
