@@ -104,6 +104,18 @@ def time_steps(torch, stream, fn, steps, warmup, barrier):
     return e0.elapsed_time(e1)
 
 
+def parse_configs(text, c5_scale):
+    """'1,1x64,3' -> [(label, cfg, scale)]; 'NxS' = config N at S times its row count (supplementary steady-state rows)."""
+    out = []
+    for tok in [t for t in text.split(",") if t]:
+        if "x" in tok:
+            c, sc = tok.split("x")
+            out.append((f"C{c}x{sc}", int(c), float(sc)))
+        else:
+            out.append((f"C{tok}", int(tok), c5_scale if int(tok) == 5 else 1.0))
+    return out
+
+
 def run_config(cfg, gq, ctx, torch, datagen, plans, gqrun, steps, warmup, scale=1.0, peak=6548.2):
     """Device-resident timing of one config: whole pipeline (builds + fused scan + finalise) and its scan kernel."""
     t0 = time.time()
@@ -131,13 +143,14 @@ def run_config(cfg, gq, ctx, torch, datagen, plans, gqrun, steps, warmup, scale=
 
     def make():
         state["tables"] = gqrun.build_tables(ctx, plan, device_tables=build_cols)
+        state["ws"] = [t.workspace for t in state["tables"]]      # table workspaces are reused by every timed step
         state["pipes"] = [gqrun.prepare(ctx, plan, state["tables"], cols=f,
                                         out_capacity=(10 if cfg == 3 else plan["max_groups"])) for f in fact]
     make()
 
     def step():
         if plan.get("builds"):
-            state["tables"] = gqrun.build_tables(ctx, plan, device_tables=build_cols)   # re-init + rebuild: timed
+            state["tables"] = gqrun.build_tables(ctx, plan, device_tables=build_cols, workspaces=state["ws"])   # re-init + rebuild: timed
             probes = [(state["tables"][bi], kc) for bi, kc in plan["probes"]]
             for p in state["pipes"]:
                 pp, _ = p.m.probes(probes)
@@ -211,7 +224,8 @@ def main():
     ap.add_argument("--steps", type=int, default=400)
     ap.add_argument("--warmup", type=int, default=5)
     ap.add_argument("--impl", default="ours")
-    ap.add_argument("--configs", default="1,3,4,5", help="extra configs reported under per_config ('' = none)")
+    ap.add_argument("--configs", default="1,1x64,3,4,5", help="extra configs reported under per_config ('' = none); "
+                    "NxS = config N at S times its rows (C1x64: the low-cardinality pipeline at steady state)")
     ap.add_argument("--c5-scale", type=float, default=1.0)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-headline", action="store_true", help="profiling aid: only the --configs entries, printed as JSON")
@@ -247,10 +261,9 @@ def main():
 
     if args.no_headline:
         per_config = {}
-        for cfg in [int(x) for x in args.configs.split(",") if x]:
-            sc = args.c5_scale if cfg == 5 else 1.0
+        for label, cfg, sc in parse_configs(args.configs, args.c5_scale):
             out, _, _ = run_config(cfg, gq, ctx, torch, datagen, plans, gqrun, args.steps, args.warmup, scale=sc, peak=peak)
-            per_config[f"C{cfg}"] = out
+            per_config[label] = out
         print(json.dumps(dict(per_config=per_config)))
         return
 
@@ -320,13 +333,12 @@ def main():
     if ws == 1 and args.configs:
         del cols, pipe, st, probe_t
         torch.cuda.empty_cache()
-        for cfg in [int(x) for x in args.configs.split(",") if x]:
+        for label, cfg, sc in parse_configs(args.configs, args.c5_scale):
             try:
-                sc = args.c5_scale if cfg == 5 else 1.0
                 out, _, _ = run_config(cfg, gq, ctx, torch, datagen, plans, gqrun, max(5, min(20, args.steps)), 3, scale=sc, peak=peak)
-                per_config[f"C{cfg}"] = out
+                per_config[label] = out
             except Exception as e:  # a failing extra config must not hide the headline number
-                per_config[f"C{cfg}"] = dict(error=str(e)[:300])
+                per_config[label] = dict(error=str(e)[:300])
             torch.cuda.empty_cache()
 
     # ---------------- CPU baseline: the oracle on this box's host cores ----------------

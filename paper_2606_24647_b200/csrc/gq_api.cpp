@@ -3,6 +3,7 @@
 // except gq_create/gq_destroy/gq_sync and the HOST-buffer end-to-end call gq_pipeline_host.
 #include <algorithm>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <map>
 #include <mutex>
@@ -27,6 +28,15 @@ int64_t table_capacity(int64_t max_rows) {   // power of two >= max_rows * 4/3, 
   int64_t c = 1024;
   while (c < need) c <<= 1;
   return c;
+}
+// Join tables: max_rows / 0.65 slots rounded up to a multiple of 1024 — NOT to a power of two: the slot index comes
+// from a multiply-shift range reduction, so the table (and a direct-aggregation array indexed by its slots) is as
+// small as the hint allows and has the best chance of staying L2-resident.
+int64_t join_capacity(int64_t max_rows) {
+  int load = 50;                                       // percent; GQ_TUNE_JOIN_LOAD overrides (tuning sweeps only)
+  if (const char* e = getenv("GQ_TUNE_JOIN_LOAD")) { int v = atoi(e); if (v >= 10 && v <= 90) load = v; }
+  int64_t need = std::max<int64_t>(1024, (max_rows * 100 + load - 1) / load);
+  return (need + 1023) / 1024 * 1024;
 }
 int join_slot_words(int npayload) { return npayload == 0 ? 1 : (int)align_up((size_t)(1 + npayload), 2); }
 int agg_slot_words(int ndep, int naggs) { return (int)align_up((size_t)(1 + ndep + naggs), 2); }
@@ -315,7 +325,7 @@ gq_status gq_hash_probe(gq_ctx* ctx, const gq_batch* probe, const gq_pred* preds
 // ------------------------------------------------------------------------------------------------ HashBuild
 gq_status gq_hash_build_workspace(int64_t max_build_rows, int32_t npayload, size_t* bytes) {
   if (!bytes || max_build_rows < 0 || npayload < 0 || npayload > GQ_MAX_PAYLOAD) return GQ_ERR_INVALID_ARG;
-  *bytes = ws_layout(table_capacity(max_build_rows), join_slot_words(npayload), GQ_SIDE_SLOTS).total;
+  *bytes = ws_layout(join_capacity(max_build_rows), join_slot_words(npayload), GQ_SIDE_SLOTS).total;
   return GQ_OK;
 }
 
@@ -346,7 +356,7 @@ gq_status gq_hash_build(gq_ctx* ctx, gq_table** table, void* d_ws, size_t bytes,
   gq_table* t = *table;
   if (!t) {
     if (!d_ws || !aligned(d_ws, 256) || max_build_rows < 0) return fail(ctx, GQ_ERR_INVALID_ARG, "bad workspace");
-    const int64_t cap = table_capacity(max_build_rows);
+    const int64_t cap = join_capacity(max_build_rows);
     const int sw = sp.target_sw;
     WsLayout w = ws_layout(cap, sw, GQ_SIDE_SLOTS);
     if (bytes < w.total) return fail(ctx, GQ_ERR_WORKSPACE_TOO_SMALL, "hash-build workspace too small");

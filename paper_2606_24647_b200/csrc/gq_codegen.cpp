@@ -465,8 +465,7 @@ gq_status gq_codegen(const GqScanSpec& sp, GqKernelInfo* out, std::string* msg) 
         << ".side + n" << s << " * " << sw << ";" << (sw == 2 ? " w" + std::to_string(s) + " = s" + std::to_string(s) + "[1];" : "")
         << " }\n";
       o << ind << "else {\n";
-      o << ind << "  s" << s << " = T" << s << ".slots + i" << s << " * " << sw << "; i" << s << " = (i" << s << " + 1) & T"
-        << s << ".mask;\n";
+      o << ind << "  s" << s << " = T" << s << ".slots + i" << s << " * " << sw << "; i" << s << " = gq_next(T" << s << ", i" << s << ", 1);\n";
       if (sw == 2) o << ind << "  u64 kw; gq_ld128(s" << s << ", kw, w" << s << ");\n";
       else o << ind << "  const u64 kw = __ldg(s" << s << ");\n";
       o << ind << "  if (kw == GQ_EMPTY) break;\n";

@@ -50,7 +50,7 @@ typedef unsigned int u32;
 // Device view of a hash table (join table or group-by table). Layout must match gq_internal.h:GqTableDev.
 struct GqTableDev {
   u64* slots;        // capacity * slot_words words; word 0 of a slot = key (GQ_EMPTY when free)
-  u64 mask;          // capacity - 1 (capacity is a power of two)
+  u64 mask;          // capacity - 1 (capacity: any multiple of 4; a power of two for group-by tables)
   i64* header;       // [0] rows inserted, [1] entries in the side area, [2..] reserved
   u64* side;         // GQ_SIDE_SLOTS slots for rows whose key == GQ_EMPTY (join) / 1 slot (group-by)
   int shift;         // 64 - log2(capacity)
@@ -163,8 +163,15 @@ __device__ __forceinline__ u64 gq_hash(i64 key, int shift) {
   x ^= x >> 32;
   return (x * 0x9E3779B97F4A7C15ULL) >> shift;
 }
+// First slot of a key's probe sequence: the top bits of the hash scaled to the capacity (multiply-shift range
+// reduction — the capacity need not be a power of two, so a table is sized to its row-count hint, not the next power
+// of two above it), aligned down to a bucket boundary.
 __device__ __forceinline__ u64 gq_slot0(const GqTableDev& T, i64 key) {
-  return (gq_hash(key, T.shift) >> T.bshift) << T.bshift;
+  return (__umul64hi(gq_hash(key, 0), T.mask + 1) >> T.bshift) << T.bshift;
+}
+__device__ __forceinline__ u64 gq_next(const GqTableDev& T, u64 i, u64 step) {   // capacity is a multiple of step
+  i += step;
+  return i > T.mask ? 0 : i;
 }
 __device__ __forceinline__ void gq_ld256(const u64* p, u64 (&w)[4]) {   // one 32-byte sector, read-only path
   asm volatile("ld.global.nc.v4.u64 {%0, %1, %2, %3}, [%4];" : "=l"(w[0]), "=l"(w[1]), "=l"(w[2]), "=l"(w[3]) : "l"(p));
@@ -191,7 +198,7 @@ __device__ __forceinline__ bool gq_ht_insert(const GqTableDev& T, i64 key, const
     return true;
   }
   u64 i = gq_slot0(T, key);
-  for (u64 n = 0; n <= T.mask; ++n, i = (i + 1) & T.mask) {
+  for (u64 n = 0; n <= T.mask; ++n, i = gq_next(T, i, 1)) {
     u64* s = T.slots + i * SW;
     u64 prev = atomicCAS(s, GQ_EMPTY, (u64)key);
     if (prev == GQ_EMPTY) {
@@ -217,7 +224,7 @@ __device__ __forceinline__ u64* gq_ht_upsert(const GqTableDev& T, i64 key, bool*
     return T.side;
   }
   u64 i = gq_slot0(T, key);
-  for (u64 n = 0; n <= T.mask; ++n, i = (i + 1) & T.mask) {
+  for (u64 n = 0; n <= T.mask; ++n, i = gq_next(T, i, 1)) {
     u64* s = T.slots + i * SW;
     u64 k = gq_ld_relaxed(s);
     if (k == (u64)key) return s;
@@ -278,7 +285,7 @@ __device__ __forceinline__ void gq_probe_rows(const GqTableDev& T, const i64 (&k
         if (!done && round * B > T.mask) { done = true; live[j] = false; }   // full table without the key
         if (done) pend &= ~(1u << j);
         else {
-          idx[j] = (idx[j] + B) & T.mask;
+          idx[j] = gq_next(T, idx[j], B);
           gq_ld256(T.slots + idx[j] * SW, w[j]);
         }
       }
@@ -334,7 +341,7 @@ __device__ __forceinline__ int gq_insert_rows(const GqTableDev& T, const i64 (&k
           }
         } else if (round > 2 * (T.mask + 1)) { gq_set_err(err, GQ_E_CAPACITY); pend &= ~(1u << j); }
         else {
-          idx[j] = (idx[j] + B) & T.mask;
+          idx[j] = gq_next(T, idx[j], B);
           gq_ld256_relaxed(T.slots + idx[j] * SW, w[j]);
         }
       }
@@ -373,7 +380,7 @@ __device__ __forceinline__ void gq_upsert_rows(const GqTableDev& T, const i64 (&
           else k[j] = prev;                         // somebody else claimed it: same key => next round returns it
         } else if (round > 2 * (T.mask + 1)) { gq_set_err(err, GQ_E_CAPACITY); pend &= ~(1u << j); }
         else {
-          idx[j] = (idx[j] + 1) & T.mask;
+          idx[j] = gq_next(T, idx[j], 1);
           k[j] = gq_ld_relaxed(T.slots + idx[j] * SW);
         }
       }

@@ -356,7 +356,8 @@ class Context:
 
     # ---- HashBuild ----
     def hash_build(self, cols, preds=(), probes=(), key=0, payload=(), unique=False, max_rows=None, table=None,
-                   finish=True):
+                   finish=True, workspace=None):
+        """workspace: a uint8 CUDA tensor to (re)use for the table instead of allocating one."""
         with torch.cuda.stream(self.stream):
             m = _M()
             b = m.batch(cols)
@@ -365,7 +366,9 @@ class Context:
                 max_rows = int(b.nrows if max_rows is None else max_rows)
                 nbytes = C.c_size_t()
                 self._check(self.L.gq_hash_build_workspace(max_rows, len(payload), C.byref(nbytes)))
-                ws = self._ws(nbytes.value)
+                ws = workspace if workspace is not None else self._ws(nbytes.value)
+                if ws.numel() < nbytes.value + 256:
+                    raise ValueError("workspace tensor too small")
                 dts = _row_dtypes(cols, probes)
                 h = C.c_void_p()
                 st = self.L.gq_hash_build(self.h, C.byref(h), self._ws_ptr(ws), nbytes.value, max_rows, C.byref(b), C.byref(d))

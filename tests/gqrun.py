@@ -12,15 +12,16 @@ def dev(cols, device="cuda"):
     return [torch.from_numpy(np.ascontiguousarray(c)).to(device) for c in cols]
 
 
-def build_tables(ctx, plan, device_tables=None):
+def build_tables(ctx, plan, device_tables=None, workspaces=None):
     """HashBuild for every plan['builds'] entry, in order (each may probe earlier ones)."""
     tables = []
     for i, b in enumerate(plan.get("builds", [])):
+        ws = workspaces[i] if workspaces is not None else None
         cols = device_tables[i] if device_tables is not None else dev(b["table"])
         probes = [(tables[bi], kc) for bi, kc in b.get("probes", [])]
         tables.append(ctx.hash_build(cols, preds=b.get("preds", []), probes=probes, key=b["key"],
                                      payload=b.get("payload", []), unique=b.get("unique", False),
-                                     max_rows=b.get("max_rows")))
+                                     max_rows=b.get("max_rows"), workspace=ws))
     return tables
 
 
