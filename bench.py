@@ -87,6 +87,21 @@ def dist():
     return ws, rank, lr
 
 
+def whole_job_value(local_total_ms, rows_per_rank, steps, td=None, device=None):
+    """Replicas-only multi-GPU accounting: every rank runs the same pipeline on its own copy of the
+    workload; the job's time is the MAX over ranks and value = world_size * rows / that time. td = torch.distributed
+    (initialised) or None for a single process. Returns (ms_per_step, rows_per_s)."""
+    ws, total = 1, float(local_total_ms)
+    if td is not None and td.is_initialized() and td.get_world_size() > 1:
+        import torch
+        ws = td.get_world_size()
+        t = torch.tensor([total], dtype=torch.float64, device=device or "cpu")
+        td.all_reduce(t, op=td.ReduceOp.MAX)
+        total = float(t.item())
+    ms_per_step = total / steps
+    return ms_per_step, ws * rows_per_rank / ms_per_step * 1e3
+
+
 def time_steps(torch, stream, fn, steps, warmup, barrier):
     """W untimed + K timed calls of fn, CUDA events on the launching stream; returns total ms (this rank)."""
     for _ in range(warmup):
@@ -291,12 +306,7 @@ def main():
     # read-only roofline probe of this box (same bytes)
     probe_t = torch.empty(1 << 30, dtype=torch.uint8, device=f"cuda:{dev_index}")
     probe_ms = time_steps(torch, ctx.stream, lambda: ctx.read_probe(probe_t), 10, 3, lambda: None) / 10
-    if ws > 1:
-        t = torch.tensor([total_ms], device="cuda")
-        td.all_reduce(t, op=td.ReduceOp.MAX)
-        total_ms = float(t.item())
-    ms_per_step = total_ms / args.steps
-    value = ws * nrows / ms_per_step * 1e3
+    ms_per_step, value = whole_job_value(total_ms, nrows, args.steps, td if ws > 1 else None, "cuda")
     alg_bytes = ALG_BYTES_PER_ROW[2] * nrows + 16
     achieved = alg_bytes / scan_ms / 1e6
     traffic = None

@@ -1,0 +1,167 @@
+"""Parity of the specialised kernel paths against the CPU oracle (-m gpu): direct (slot-indexed) aggregation, the
+finaliser fused into the scan kernel, low-cardinality key tables with 64-bit keys, join tables at full load."""
+import numpy as np
+import pytest
+
+import oracle
+import plans
+from paper_2606_24647_b200 import datagen
+
+pytestmark = pytest.mark.gpu
+I64_MIN = np.iinfo(np.int64).min
+
+
+@pytest.fixture(scope="module")
+def ctx():
+    from paper_2606_24647_b200 import build as gqbuild
+    gqbuild.build()
+    from paper_2606_24647_b200 import gq
+    return gq.Context()
+
+
+def run(plan, ctx, **kw):
+    import gqrun
+    exp = oracle.run_query(plan)
+    got = gqrun.run_query(plan, ctx=ctx, **kw)
+    assert got["n"] == exp.nrows
+    for c, (g, e) in enumerate(zip(got["cols"], exp.cols)):
+        assert np.array_equal(g, e), f"column {c} differs"
+    return exp, got
+
+
+def _join_plan(nb, nf, rng, aggs, with_dep=False, extra_keys=()):
+    """dim(key unique [, attr]) JOIN fact(fk, v) GROUP BY fk [, attr]."""
+    bkeys = np.concatenate([rng.permutation(4 * nb)[:nb].astype(np.int64) - nb, np.array(extra_keys, np.int64)])
+    attr = rng.integers(-1000, 1000, len(bkeys)).astype(np.int32)
+    bsel = rng.integers(0, 2, len(bkeys)).astype(np.int8)
+    fk = rng.choice(np.concatenate([bkeys, np.array([7 * nb + 1, 7 * nb + 2], np.int64)]), nf).astype(np.int64)
+    v = rng.integers(-5000, 5000, nf).astype(np.int64)
+    fsel = rng.integers(0, 4, nf).astype(np.int32)
+    build = dict(table=[bkeys, attr, bsel], preds=[(2, "eq", 1)], key=0, payload=[1] if with_dep else [], unique=True)
+    return dict(builds=[build], table=[fk, v, fsel], preds=[(2, "lt", 3)], probes=[(0, 0)], exprs=[[("col", 1)]],
+                keys=[0, 3] if with_dep else [0], ndependent=1 if with_dep else 0, aggs=aggs, max_groups=len(bkeys))
+
+
+@pytest.mark.parametrize("with_dep", [False, True])
+@pytest.mark.parametrize("aggs", [[("sum", 0), ("count",)], [("min", 0), ("max", 0), ("sum", 0)]])
+def test_direct_aggregation_pipeline(ctx, with_dep, aggs):
+    # group key = key of a unique-key probe step: the pipeline aggregates into an array indexed by the matched slot.
+    # Second aggregate list has no COUNT(*): a hidden touch word marks the groups. INT64_MIN is a build key (S14).
+    rng = np.random.default_rng(5)
+    plan = _join_plan(20_000, 300_000, rng, aggs, with_dep, extra_keys=[I64_MIN, np.iinfo(np.int64).max])
+    run(plan, ctx)
+
+
+def test_direct_equals_hashed_standalone_and_streams(ctx):
+    import gqrun
+    rng = np.random.default_rng(6)
+    plan = _join_plan(5_000, 120_000, rng, [("sum", 0), ("count",)])
+    exp = oracle.run_query(plan)
+    tables = gqrun.build_tables(ctx, plan)
+    cols = gqrun.dev(plan["table"])
+    n = len(plan["table"][0])
+    for aware in (False, True):                    # hashed state vs direct state, three batches each
+        st = None
+        for lo, hi in ((0, 40_000), (40_000, 40_016), (40_016, n)):
+            st = ctx.aggregate(st, [c[lo:hi] for c in cols], preds=plan["preds"], probes=[(tables[0], 0)],
+                               exprs=plan["exprs"], keys=plan["keys"], aggs=plan["aggs"], max_groups=plan["max_groups"],
+                               plan_aware_workspace=aware)
+        r = ctx.aggregate_finish(st, capacity=exp.nrows + 3)
+        ctx.sync()
+        ng = int(r["n"].item())
+        assert ng == exp.nrows
+        got = gqrun.sort_rows([r["keys"][0][:ng].cpu().numpy()] + [a[:ng].cpu().numpy() for a in r["aggs"]], 1)
+        for g, e in zip(got, exp.cols):
+            assert np.array_equal(g, e)
+
+
+def test_direct_topk(ctx):
+    rng = np.random.default_rng(7)
+    plan = _join_plan(3_000, 50_000, rng, [("sum", 0), ("count",)])
+    plan["topk"], plan["topk_agg"] = 10, 0
+    run(plan, ctx, out_capacity=10)
+
+
+def test_join_table_at_full_load_and_all_misses(ctx):
+    rng = np.random.default_rng(8)
+    nb = 50_000
+    bkeys = rng.permutation(1 << 22)[:nb].astype(np.int64)
+    fk = np.concatenate([bkeys, bkeys + (1 << 23)])           # second half matches nothing
+    v = np.ones(len(fk), np.int64)
+    build = dict(table=[bkeys], preds=[], key=0, payload=[], unique=True, max_rows=nb)   # exactly the hinted rows
+    plan = dict(builds=[build], table=[fk, v], preds=[], probes=[(0, 0)], exprs=[[("col", 1)]], keys=[0],
+                aggs=[("sum", 0), ("count",)], max_groups=nb)
+    exp, got = run(plan, ctx)
+    assert exp.nrows == nb and int(got["cols"][2].sum()) == nb
+
+
+@pytest.mark.parametrize("n", [1, 255, 1024, 1025, 5000, 200_003])
+def test_fused_finaliser_lowcard_sizes(ctx, n):
+    # one-kernel pipeline (scan + in-kernel finaliser): tail-only inputs, one CTA, many CTAs
+    plan = plans.plan_c1(datagen.make_config(1, scale=n / 1_000_000))
+    exp, got = run(plan, ctx, avgs=[(0, 4), (1, 4)])
+    for a, (s, c) in zip(got["avgs"], [(2, 6), (3, 6)]):
+        ref = np.array([oracle.avg(int(x), int(y)) for x, y in zip(exp.cols[s], exp.cols[c])])
+        assert np.allclose(a, ref, rtol=1e-12, atol=0)
+
+
+def test_fused_finaliser_global_no_passing_rows_and_repeat(ctx):
+    import gqrun
+    plan = plans.plan_c2(datagen.make_config(2, scale=0.002))
+    plan["preds"] = [(0, "lt", -5)]                           # nothing passes: one row (0, 0)   (S9)
+    exp, got = run(plan, ctx)
+    assert [int(c[0]) for c in got["cols"]] == [0, 0]
+    plan = plans.plan_c2(datagen.make_config(2, scale=0.01))
+    p = gqrun.prepare(ctx, plan, [])
+    exp = oracle.run_query(plan)
+    for _ in range(5):                                        # the ticket counter must return to zero every run
+        p.run()
+        ctx.sync()
+        r = p.result()
+        assert r["n"] == 1 and [int(a[0]) for a in r["aggs"]] == [int(c[0]) for c in exp.cols]
+
+
+def test_lowcard_wide_keys_reserved_pattern_and_many_groups(ctx):
+    rng = np.random.default_rng(9)
+    n = 70_000
+    pool = np.array([I64_MIN, -1, 0, 1, 1 << 40, np.iinfo(np.int64).max, 12345678901234], np.int64)
+    k = pool[rng.integers(0, len(pool), n)]
+    v = rng.integers(-100, 100, n).astype(np.int64)
+    plan = dict(table=[k, v], preds=[(1, "ne", 3)], exprs=[[("col", 1)]], keys=[0],
+                aggs=[("sum", 0), ("min", 0), ("max", 0), ("count",)], max_groups=len(pool))
+    run(plan, ctx)
+    # 24 groups over two packed narrow keys; also streamed in batches into a (non-fused) low-cardinality state
+    a = rng.integers(-3, 3, n).astype(np.int8)
+    b = rng.integers(10, 14, n).astype(np.int32)
+    plan = dict(table=[a, b, v], preds=[], exprs=[[("col", 2)]], keys=[0, 1], aggs=[("sum", 0), ("count",)], max_groups=24)
+    exp, _ = run(plan, ctx)
+    import gqrun
+    cols = gqrun.dev(plan["table"])
+    st = None
+    for lo, hi in ((0, 4096), (4096, 4112), (4112, n)):
+        st = ctx.aggregate(st, [c[lo:hi] for c in cols], exprs=plan["exprs"], keys=plan["keys"], aggs=plan["aggs"], max_groups=24)
+    r = ctx.aggregate_finish(st, capacity=30)
+    ctx.sync()
+    ng = int(r["n"].item())
+    got = gqrun.sort_rows([kk[:ng].cpu().numpy().astype(np.int64) for kk in r["keys"]] + [x[:ng].cpu().numpy() for x in r["aggs"]], 2)
+    for g, e in zip(got, exp.cols):
+        assert np.array_equal(g, e)
+
+
+def test_lowcard_more_groups_than_declared_is_an_error():
+    from paper_2606_24647_b200 import gq
+    import gqrun
+    c = gq.Context()
+    k = (np.arange(5000) % 9).astype(np.int8)
+    plan = dict(table=[k, np.ones(5000, np.int64)], preds=[], exprs=[[("col", 1)]], keys=[0], aggs=[("sum", 0)], max_groups=6)
+    p = gqrun.prepare(c, plan, [])
+    p.run()
+    with pytest.raises(gq.GqError) as e:
+        c.sync()
+    assert e.value.status == 3                                 # GQ_ERR_CAPACITY, sticky
+    c.clear_error()
+    plan["max_groups"] = 9
+    p = gqrun.prepare(c, plan, [])
+    p.run()
+    c.sync()                                                   # and the ticket counter survived the failed run
+    assert p.result()["n"] == 9
