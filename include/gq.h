@@ -198,6 +198,10 @@ gq_status gq_table_describe(gq_table** out, const gq_dtype* payload_dtypes, int3
 /* Read-only streaming sum over `bytes` bytes (16-byte aligned, multiple of 16): the practical read roofline probe of
  * SURVEY §7.1 step 5. *d_out (DEVICE uint64) receives the wrapping sum of the 64-bit words. */
 gq_status gq_read_probe(gq_ctx*, const void* d_data, size_t bytes, uint64_t* d_out);
+/* Random-access rate probe: what bounds the hash phases (SURVEY §8(d) "secondary limiters"). Enqueues naccesses
+ * pseudo-random 8-byte accesses over d_table (bytes = a power of two >= 4096, 32-byte aligned, CONTENTS ARE MODIFIED by
+ * modes 1-3): mode 0 loads, 1 RED.ADD.64, 2 load + two REDs in one 32-byte slot (insert-or-update), 3 CAS. */
+gq_status gq_random_probe(gq_ctx*, void* d_table, size_t bytes, int64_t naccesses, int32_t mode, uint64_t* d_out);
 
 #ifdef __cplusplus
 }

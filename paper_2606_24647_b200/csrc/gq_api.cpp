@@ -373,7 +373,7 @@ gq_status gq_hash_build(gq_ctx* ctx, gq_table** table, void* d_ws, size_t bytes,
     t->dev.shift = 64 - log2i(cap);
     t->dev.slot_words = sw;
     t->dev.flags = d->flags;
-    t->dev.bshift = sw == 1 ? 2 : sw == 2 ? 1 : 0;   // slots per 32-byte bucket: 4 / 2 / 1
+    t->dev.bshift = (sw == 1 ? 2 : sw == 2 ? 1 : 0);   // slots per 32-byte bucket: 4 / 2 / 1
     unsigned long long pat[12];
     for (int i = 0; i < 12; ++i) pat[i] = 0;
     pat[0] = GQ_EMPTY_KEY;
@@ -770,6 +770,15 @@ gq_status gq_read_probe(gq_ctx* ctx, const void* d_data, size_t bytes, uint64_t*
   return GQ_OK;
 }
 
+gq_status gq_random_probe(gq_ctx* ctx, void* d_table, size_t bytes, int64_t naccesses, int32_t mode, uint64_t* d_out) {
+  if (!ctx || !d_table || !d_out || !aligned(d_table, 32) || bytes < 4096 || (bytes & (bytes - 1)) || naccesses < 0 || mode < 0 || mode > 3)
+    return GQ_ERR_INVALID_ARG;
+  cudaError_t e = gq_launch_random_probe(ctx->stream, d_table, bytes, naccesses, mode, (unsigned long long*)d_out, ctx->num_sms);
+  if (e != cudaSuccess) return cuda_fail(ctx, e, "random probe");
+  ++ctx->launches;
+  return GQ_OK;
+}
+
 }  // extern "C"
 
 // ------------------------------------------------------------------------------------------------ host-buffer e2e
@@ -802,7 +811,7 @@ extern "C" {
 gq_status gq_pipeline_host_workspace(const gq_plan* plan, int64_t chunk_rows, size_t* bytes) {
   if (!plan || !plan->in || !bytes || chunk_rows < 1) return GQ_ERR_INVALID_ARG;
   HostLayout L;
-  chunk_rows = (chunk_rows + 2047) / 2048 * 2048;   // same rounding as gq_pipeline_host
+  chunk_rows = (chunk_rows + 7679) / 7680 * 7680;   // same rounding as gq_pipeline_host
   // output capacity is not known here: size for max_groups rows (top-k needs only k)
   int64_t cap = plan->topk > 0 ? plan->topk : std::max<int64_t>(1, plan->agg.max_groups);
   gq_status st = host_layout(plan, chunk_rows, cap, &L);
@@ -817,7 +826,7 @@ gq_status gq_pipeline_host(gq_ctx* ctx, const gq_plan* plan, int64_t chunk_rows,
   if (!ctx || !plan || !plan->in || !d_ws || chunk_rows < 1 || !h_out_ngroups || !h_out_agg_cols) return GQ_ERR_INVALID_ARG;
   const gq_batch* in = plan->in;
   if (in->ncols < 1 || in->ncols > GQ_MAX_COLS) return fail(ctx, GQ_ERR_INVALID_ARG, "bad batch");
-  chunk_rows = (chunk_rows + 2047) / 2048 * 2048;   // whole tiles per chunk: only the last chunk has a ragged tail
+  chunk_rows = (chunk_rows + 7679) / 7680 * 7680;   // whole tiles (1280 / 1536 / 1024 rows) per chunk: only the last chunk has a ragged tail
   int64_t cap = plan->topk > 0 ? plan->topk : std::max<int64_t>(1, plan->agg.max_groups);
   if (out_capacity > cap) out_capacity = cap;
   HostLayout L;

@@ -333,7 +333,13 @@ gq_status gq_codegen(const GqScanSpec& sp, GqKernelInfo* out, std::string* msg) 
   int row_bytes = 0;
   for (int c : g.cols) row_bytes += gq_dtype_bytes(sp.in_dtype[(size_t)c]);
   auto env_int = [](const char* name) { const char* e = getenv(name); return e ? atoi(e) : 0; };   // tuning sweeps only
-  int nt = 512;
+  // Hash phases are bound by memory latency, not bandwidth (profiles/r1_hash_phases.md): 24 consumer warps x 2 rows
+  // hide more of it than 16 x 4 (C4 1.56 -> 1.13 ms). Pure scans: 20 warps x 2 rows (C2 0.242 -> 0.238 ms).
+  const bool hashing = nprobe > 0 || sp.consumer == GQ_C_BUILD || sp.consumer == GQ_C_HIGHCARD || sp.consumer == GQ_C_DIRECT;
+  int nt = hashing ? 768 : 640;
+  const bool tablebound = sp.consumer == GQ_C_HIGHCARD && nprobe == 0;   // DRAM-random bound (C5): 16 warps x 4 rows measured best
+  if (tablebound) nt = 512;
+  if (env_int("GQ_TUNE_NT") && sp.consumer != GQ_C_LOWCARD) nt = env_int("GQ_TUNE_NT");
   long long cons_bytes = 256;
   int lc_kt = 64, lc_key32 = 0;
   if (sp.consumer == GQ_C_GLOBAL) cons_bytes = 8LL * nagg * (nt / 32) + 256;
@@ -352,9 +358,8 @@ gq_status gq_codegen(const GqScanSpec& sp, GqKernelInfo* out, std::string* msg) 
   for (const GqProbeSpec& ps : sp.probes) all_unique = all_unique && ps.unique;
   const bool use_hot = sp.hot && sp.consumer == GQ_C_HIGHCARD && all_unique;   // linear mode only
   if (use_hot) cons_bytes = 512 * 8 + 512LL * nagg * 8 + 512 * 4 + 256;
-  int r = 4, stages = 0;
+  int r = tablebound ? 4 : 2, stages = 0;
   // small inputs: smaller tiles so that every SM still gets several tiles
-  if (sp.nrows_hint > 0 && sp.nrows_hint < 148LL * 8 * nt * 4) r = 2;
   if (sp.nrows_hint > 0 && sp.nrows_hint < 148LL * 8 * nt * 2) r = 1;
   if (sp.consumer == GQ_C_LOWCARD) r = (sp.nrows_hint > 0 && sp.nrows_hint < 148LL * nt * 4) ? 1 : 4;   // straight-line rows: ILP
   if (env_int("GQ_TUNE_R")) r = env_int("GQ_TUNE_R");

@@ -50,7 +50,7 @@ struct GqParams {
   long long* out[GQ_MAXOUT];
   long long out_capacity;
   long long* out_count;
-  const long long* hot;        // HIGHCARD: hot list of this batch (hot[0] = count, hot[1..] = keys) or null
+  const long long* hot;        // HIGHCARD: hot list of this batch (hot[0] = count, hot[32..] = keys) or null
   int* err;
   int pad;
   unsigned long long* dacc;    // DIRECT: aggregate words indexed by slot of the probed unique table
@@ -173,6 +173,7 @@ cudaError_t gq_launch_init_table(cudaStream_t s, unsigned long long* slots, long
                                  long long* header, long long header1);
 cudaError_t gq_launch_finalise(cudaStream_t s, const GqFinaliseParams& p, int num_sms, int* nlaunches);
 cudaError_t gq_launch_read_probe(cudaStream_t s, const void* data, size_t bytes, unsigned long long* out, int num_sms);
+cudaError_t gq_launch_random_probe(cudaStream_t s, void* table, size_t bytes, long long n, int mode, unsigned long long* out, int num_sms);
 size_t gq_topk_scratch_bytes_impl();
 cudaError_t gq_launch_hot_keys(cudaStream_t s, const void* keycol, int dtype, long long nrows, unsigned long long* table,
                                long long nslots, long long nsample, unsigned long long threshold, long long* hot,

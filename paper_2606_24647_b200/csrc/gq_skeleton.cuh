@@ -86,7 +86,7 @@ struct GqParams {
   i64* out[GQ_MAXOUT];          // MATERIALISE: output columns
   i64 out_capacity;
   i64* out_count;
-  const i64* hot;               // HIGHCARD: hot list of this batch (hot[0] = count, hot[1..] = keys) or null
+  const i64* hot;               // HIGHCARD: hot list of this batch (hot[0] = count, hot[32..] = keys) or null
   int* err;                     // sticky device error
   int pad;
   u64* dacc;                    // DIRECT: aggregate words indexed by the slot of the probed unique table

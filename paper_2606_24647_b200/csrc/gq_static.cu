@@ -179,22 +179,27 @@ __device__ __forceinline__ GqCand gq_make_cand(const GqFinaliseParams& P, const 
   return c;
 }
 // Feeds the candidates held by the lanes in `m` (each better than the list's current worst) into the list.
-__device__ __forceinline__ void gq_list_feed(GqCand& mine, const GqCand& c, bool want, int lane) {
+// `kth` = topk - 1: only the first topk entries matter, so admission compares with entry kth (entries behind it are
+// pushed-down leftovers that stay sorted and are never read).
+__device__ __forceinline__ void gq_list_feed(GqCand& mine, const GqCand& c, bool want, int lane, int kth) {
   unsigned m = __ballot_sync(0xffffffffu, want);
   while (m) {
     int src = __ffs(m) - 1;
     m &= m - 1;
     GqCand b = gq_cand_shfl(c, src);
-    GqCand worst = gq_cand_shfl(mine, 31);
+    GqCand worst = gq_cand_shfl(mine, kth);
     if (gq_better(b, worst)) gq_list_insert(mine, b, lane);
   }
 }
 #define GQ_TOPK_BLOCKS 592
 #define GQ_TOPK_WARPS 8
-// pass 1: every warp scans a strided share of the table and keeps its own best 32; lists go to scratch.
+#define GQ_TOPK_UNROLL 4
+// pass 1: every warp scans a strided share of the table (GQ_TOPK_UNROLL chunks of 32 slots in flight) and keeps its
+// own best list; lists go to scratch.
 __global__ void __launch_bounds__(GQ_TOPK_WARPS * 32) gq_k_topk_scan(const __grid_constant__ GqFinaliseParams P) {
   if (*(volatile int*)P.err != 0) return;
   const int lane = threadIdx.x & 31;
+  const int kth = P.topk - 1;
   const i64 gw = (i64)blockIdx.x * GQ_TOPK_WARPS + (threadIdx.x >> 5);
   const i64 nw = (i64)gridDim.x * GQ_TOPK_WARPS;
   GqCand mine; mine.valid = 0; mine.val = 0; mine.k0 = 0; mine.k1 = 0; mine.slot = -1;
@@ -204,17 +209,37 @@ __global__ void __launch_bounds__(GQ_TOPK_WARPS * 32) gq_k_topk_scan(const __gri
     GqGroupRef g;
     const i64 si = P.direct ? P.capacity : -2;
     if (lane == 0 && gq_group_at(P, si, &g)) { c = gq_make_cand(P, g, si); want = true; }
-    gq_list_feed(mine, c, want, lane);
+    gq_list_feed(mine, c, want, lane, kth);
   }
-  for (i64 i0 = gw * 32; i0 < P.capacity; i0 += nw * 32) {
-    i64 i = i0 + lane;
-    GqCand c; c.valid = 0; c.val = 0; c.k0 = 0; c.k1 = 0; c.slot = -1;
-    bool want = false;
-    GqGroupRef g;
-    if (i < P.capacity && gq_group_at(P, i, &g)) { c = gq_make_cand(P, g, i); want = true; }
-    GqCand worst = gq_cand_shfl(mine, 31);
-    want = want && gq_better(c, worst);
-    gq_list_feed(mine, c, want, lane);
+  for (i64 i0 = gw * 32; i0 < P.capacity; i0 += nw * 32 * GQ_TOPK_UNROLL) {
+    // validity word and ordering aggregate of GQ_TOPK_UNROLL slots, loaded unconditionally (all in flight together);
+    // the full candidate (keys) is only built for the few slots that can still enter the list
+    u64 tv[GQ_TOPK_UNROLL];
+    i64 vv[GQ_TOPK_UNROLL];
+#pragma unroll
+    for (int u = 0; u < GQ_TOPK_UNROLL; ++u) {
+      const i64 i = i0 + (i64)u * nw * 32 + lane;
+      const i64 ii = i < P.capacity ? i : 0;
+      if (P.direct) { tv[u] = P.dacc[ii * P.daw + P.dtouch]; vv[u] = (i64)P.dacc[ii * P.daw + P.topk_agg]; }
+      else {
+        const u64* sl = P.slots + ii * P.slot_words;
+        tv[u] = sl[0] != GQ_EMPTY_KEY; vv[u] = (i64)sl[1 + P.ndep + P.topk_agg];
+      }
+      if (i >= P.capacity) tv[u] = 0;
+    }
+#pragma unroll
+    for (int u = 0; u < GQ_TOPK_UNROLL; ++u) {
+      const i64 i = i0 + (i64)u * nw * 32 + lane;
+      const GqCand worst = gq_cand_shfl(mine, kth);
+      bool want = tv[u] != 0 && (!worst.valid || vv[u] >= worst.val);
+      GqCand c; c.valid = 0; c.val = 0; c.k0 = 0; c.k1 = 0; c.slot = -1;
+      if (want) {
+        GqGroupRef g;
+        want = gq_group_at(P, i, &g);
+        if (want) { c = gq_make_cand(P, g, i); want = gq_better(c, worst); }
+      }
+      gq_list_feed(mine, c, want, lane, kth);
+    }
   }
   // merge the block's GQ_TOPK_WARPS lists into one (warp 0), so pass 2 sees one list per block
   __shared__ GqCand sh[GQ_TOPK_WARPS][32];
@@ -223,33 +248,39 @@ __global__ void __launch_bounds__(GQ_TOPK_WARPS * 32) gq_k_topk_scan(const __gri
   if ((threadIdx.x >> 5) == 0) {
     for (int w = 1; w < GQ_TOPK_WARPS; ++w) {
       GqCand c = sh[w][lane];
-      GqCand worst = gq_cand_shfl(mine, 31);
-      gq_list_feed(mine, c, c.valid && gq_better(c, worst), lane);
+      GqCand worst = gq_cand_shfl(mine, kth);
+      gq_list_feed(mine, c, c.valid && gq_better(c, worst), lane, kth);
     }
     ((GqCand*)P.scratch)[(i64)blockIdx.x * 32 + lane] = mine;
   }
 }
-// pass 2: one block; every warp merges a strided share of the per-block lists, warp 0 merges the warps' results and
-// writes the first min(k, ngroups) groups in order.
+// pass 2: one block; every warp merges a strided share of the per-block lists (two lists in flight), warp 0 merges the
+// warps' results and writes the first min(k, ngroups) groups in order.
 #define GQ_TOPK_MERGE_WARPS 32
 __global__ void __launch_bounds__(GQ_TOPK_MERGE_WARPS * 32) gq_k_topk_merge(const __grid_constant__ GqFinaliseParams P, i64 nlists) {
   if (*(volatile int*)P.err != 0) return;
   __shared__ GqCand sh[GQ_TOPK_MERGE_WARPS][32];
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  const int kth = P.topk - 1;
   const GqCand* in = (const GqCand*)P.scratch;
   GqCand mine; mine.valid = 0; mine.val = 0; mine.k0 = 0; mine.k1 = 0; mine.slot = -1;
-  for (i64 l = warp; l < nlists; l += GQ_TOPK_MERGE_WARPS) {
-    GqCand c = in[l * 32 + lane];
-    GqCand worst = gq_cand_shfl(mine, 31);
-    gq_list_feed(mine, c, c.valid && gq_better(c, worst), lane);
+  for (i64 l = warp; l < nlists; l += 2 * GQ_TOPK_MERGE_WARPS) {
+    const i64 l2 = l + GQ_TOPK_MERGE_WARPS;
+    GqCand c0 = in[l * 32 + lane], c1;
+    c1.valid = 0; c1.val = 0; c1.k0 = 0; c1.k1 = 0; c1.slot = -1;
+    if (l2 < nlists) c1 = in[l2 * 32 + lane];
+    GqCand worst = gq_cand_shfl(mine, kth);
+    gq_list_feed(mine, c0, c0.valid && gq_better(c0, worst), lane, kth);
+    worst = gq_cand_shfl(mine, kth);
+    gq_list_feed(mine, c1, c1.valid && gq_better(c1, worst), lane, kth);
   }
   sh[warp][lane] = mine;
   __syncthreads();
   if (warp != 0) return;
   for (int w = 1; w < GQ_TOPK_MERGE_WARPS; ++w) {
     GqCand c = sh[w][lane];
-    GqCand worst = gq_cand_shfl(mine, 31);
-    gq_list_feed(mine, c, c.valid && gq_better(c, worst), lane);
+    GqCand worst = gq_cand_shfl(mine, kth);
+    gq_list_feed(mine, c, c.valid && gq_better(c, worst), lane, kth);
   }
   unsigned have = __ballot_sync(0xffffffffu, mine.valid != 0);
   int n = min(__popc(have), P.topk);
@@ -298,6 +329,52 @@ cudaError_t gq_launch_read_probe(cudaStream_t s, const void* data, size_t bytes,
   return cudaGetLastError();
 }
 
+// ------------------------------------------------------------------------------------------------ random-access probe
+// What the hash phases can reach on this box: n pseudo-random 8-byte accesses spread over a table of `bytes` bytes
+// (a power of two), 4 independent accesses in flight per thread. mode 0 = read-only loads, 1 = RED.ADD.64,
+// 2 = load + two REDs in the same 32-byte slot (an insert-or-update), 3 = CAS.
+__device__ __forceinline__ u64 gq_p_mix(u64 x) {
+  x ^= x >> 33; x *= 0xff51afd7ed558ccdULL; x ^= x >> 33; x *= 0xc4ceb9fe1a85ec53ULL; x ^= x >> 33;
+  return x;
+}
+template <int MODE>
+__global__ void __launch_bounds__(512) gq_k_random_probe(u64* tab, u64 mask, i64 n, u64* out) {
+  u64 acc = 0;
+  const i64 nthreads = (i64)gridDim.x * blockDim.x;
+  for (i64 i0 = (i64)blockIdx.x * blockDim.x + threadIdx.x; i0 < n; i0 += nthreads * 4) {
+    u64 idx[4], v[4];
+#pragma unroll
+    for (int j = 0; j < 4; ++j) idx[j] = gq_p_mix((u64)(i0 + j * nthreads)) & mask;
+    if (MODE == 0) {
+#pragma unroll
+      for (int j = 0; j < 4; ++j) v[j] = __ldg(tab + idx[j]);
+    } else if (MODE == 1) {
+#pragma unroll
+      for (int j = 0; j < 4; ++j) { atomicAdd(tab + idx[j], 1ULL); v[j] = 0; }
+    } else if (MODE == 2) {
+#pragma unroll
+      for (int j = 0; j < 4; ++j) v[j] = *(volatile u64*)(tab + (idx[j] & ~3ULL));
+#pragma unroll
+      for (int j = 0; j < 4; ++j) { atomicAdd(tab + (idx[j] & ~3ULL) + 1, 1ULL); atomicAdd(tab + (idx[j] & ~3ULL) + 2, 1ULL); }
+    } else {
+#pragma unroll
+      for (int j = 0; j < 4; ++j) v[j] = atomicCAS(tab + idx[j], ~0ULL, 5ULL);
+    }
+#pragma unroll
+    for (int j = 0; j < 4; ++j) acc += v[j];
+  }
+  if (acc == 0x123456789ULL) *out = acc;   // keeps the loads alive
+}
+cudaError_t gq_launch_random_probe(cudaStream_t s, void* table, size_t bytes, i64 n, int mode, u64* out, int num_sms) {
+  const u64 mask = (u64)(bytes / 8) - 1;
+  dim3 g((unsigned)num_sms * 4), b(512);
+  if (mode == 0) gq_k_random_probe<0><<<g, b, 0, s>>>((u64*)table, mask, n, out);
+  else if (mode == 1) gq_k_random_probe<1><<<g, b, 0, s>>>((u64*)table, mask, n, out);
+  else if (mode == 2) gq_k_random_probe<2><<<g, b, 0, s>>>((u64*)table, mask, n, out);
+  else gq_k_random_probe<3><<<g, b, 0, s>>>((u64*)table, mask, n, out);
+  return cudaGetLastError();
+}
+
 // ------------------------------------------------------------------------------------------------ heavy hitters
 // Skew handling for high-cardinality group-by: before the fused scan of a large batch, a strided
 // sample of the group-key column is counted in a small (key,count) table; keys whose sample count reaches the
@@ -331,14 +408,34 @@ __global__ void gq_k_hot_sample(const void* keycol, int dtype, i64 nrows, i64 st
     return;
   }
 }
-// hot[0] = number of hot keys (<= max_hot), hot[1..] = keys
+// hot[0] = number of hot keys (<= max_hot), hot[1..31] = histogram of sample counts by floor(log2), hot[32..] = keys.
+// The hot list must hold the MOST frequent keys: when more than max_hot keys reach the base threshold, the threshold
+// is raised to the smallest power of two that leaves at most max_hot of them.
+__global__ void gq_k_hot_hist(const u64* table, i64 nslots, u64 threshold, i64* hot) {
+  const i64 i = (i64)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= nslots) return;
+  const u64 c = table[i * 2 + 1];
+  if (table[i * 2] == GQ_EMPTY_KEY || c < threshold) return;
+  int b = 63 - __clzll((long long)c);
+  if (b > 31) b = 31;
+  if (b < 1) b = 1;
+  atomicAdd((u64*)&hot[b], 1ULL);
+}
 __global__ void gq_k_hot_select(const u64* table, i64 nslots, u64 threshold, i64* hot, int max_hot) {
   const i64 i = (i64)blockIdx.x * blockDim.x + threadIdx.x;
   if (i >= nslots) return;
   const u64 k = table[i * 2];
-  if (k == GQ_EMPTY_KEY || table[i * 2 + 1] < threshold) return;
+  const u64 c = table[i * 2 + 1];
+  if (k == GQ_EMPTY_KEY || c < threshold) return;
+  u64 t = threshold;                          // every thread derives the same raised threshold from the histogram
+  i64 above = 0;
+  for (int b = 31; b >= 1; --b) {
+    above += hot[b];
+    if (above > max_hot) { const u64 tb = 1ULL << (b + 1); if (tb > t) t = tb; break; }
+  }
+  if (c < t) return;
   i64 idx = (i64)atomicAdd((u64*)hot, 1ULL);
-  if (idx < max_hot) hot[1 + idx] = (i64)k;
+  if (idx < max_hot) hot[32 + idx] = (i64)k;
 }
 
 cudaError_t gq_launch_hot_keys(cudaStream_t s, const void* keycol, int dtype, i64 nrows, u64* table, i64 nslots,
@@ -353,7 +450,8 @@ cudaError_t gq_launch_hot_keys(cudaStream_t s, const void* keycol, int dtype, i6
   const i64 stride = nrows / nsample > 0 ? nrows / nsample : 1;
   gq_k_hot_sample<<<(unsigned)((nsample + 255) / 256), 256, 0, s>>>(keycol, dtype, nrows, stride, nsample, table,
                                                                    (u64)(nslots - 1), shift);
+  gq_k_hot_hist<<<(unsigned)((nslots + 255) / 256), 256, 0, s>>>(table, nslots, threshold, hot);
   gq_k_hot_select<<<(unsigned)((nslots + 255) / 256), 256, 0, s>>>(table, nslots, threshold, hot, max_hot);
-  *nlaunches = 3;
+  *nlaunches = 4;
   return cudaGetLastError();
 }

@@ -37,7 +37,7 @@ SYMBOLS = ["gq_create", "gq_destroy", "gq_sync", "gq_clear_error", "gq_status_st
            "gq_hash_aggregate_workspace", "gq_hash_aggregate_workspace_for", "gq_hash_aggregate", "gq_topk_scratch_bytes", "gq_hash_aggregate_finish",
            "gq_aggstate_destroy", "gq_pipeline_workspace", "gq_pipeline", "gq_pipeline_host_workspace",
            "gq_pipeline_host", "gq_set_kernel_cache_dir", "gq_precompile_pipeline", "gq_precompile_build",
-           "gq_table_describe", "gq_read_probe"]
+           "gq_table_describe", "gq_read_probe", "gq_random_probe"]
 
 
 class GqError(RuntimeError):
@@ -143,6 +143,7 @@ def lib():
         L.gq_precompile_build.argtypes = [C.POINTER(_Batch), C.POINTER(_BuildDesc), C.c_char_p, C.c_size_t]
         L.gq_table_describe.argtypes = [C.POINTER(C.c_void_p), C.POINTER(C.c_int), C.c_int32, C.c_uint32]
         L.gq_read_probe.argtypes = [C.c_void_p, C.c_void_p, C.c_size_t, C.c_void_p]
+        L.gq_random_probe.argtypes = [C.c_void_p, C.c_void_p, C.c_size_t, C.c_int64, C.c_int32, C.c_void_p]
         _lib = L
     return _lib
 
@@ -439,6 +440,15 @@ class Context:
         with torch.cuda.stream(self.stream):
             self._check(self.L.gq_read_probe(self.h, t.data_ptr(), nbytes, out.data_ptr()))
         return out
+
+
+    def random_probe(self, table: torch.Tensor, naccesses: int, mode: int) -> None:
+        """Enqueue gq_random_probe over a uint8/int64 CUDA tensor whose byte size is a power of two."""
+        out = torch.zeros(1, dtype=torch.int64, device=self.device)
+        with torch.cuda.stream(self.stream):
+            self._check(self.L.gq_random_probe(self.h, table.data_ptr(), table.numel() * table.element_size(),
+                                               int(naccesses), int(mode), out.data_ptr()))
+        self._keep_probe_out = out
 
 
 class Pipeline:
