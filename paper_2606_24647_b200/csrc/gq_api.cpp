@@ -146,6 +146,7 @@ std::string signature(const GqScanSpec& sp) {
   put(sp.lc_cap); put(sp.lc_key_bits); put(sp.target_sw); put(sp.build_key_col);
   for (int c : sp.payload_cols) put(c);
   put(sp.unique); put(sp.hot); put(sp.fused_final); put(sp.direct_step); put(sp.direct_aw); put(sp.direct_touch);
+  put(sp.part_rw); for (int e : sp.part_exprs) put(e);
   s += 'c';
   std::vector<long long> kv; std::vector<int> ki;
   collect_consts(sp, &kv, &ki);
@@ -522,6 +523,39 @@ DirectPlan direct_plan(const GqScanSpec& sp, const gq_agg_desc* d, const gq_batc
   return dp;
 }
 
+// Radix-clustered aggregation: for a high-cardinality state whose table is far larger than L2,
+// pass A (PARTITION consumer of the scan kernel) appends every surviving row to the record buffer of its key's table
+// partition and pass B (gq_k_part_upsert) applies the records partition by partition, so every insert-or-update hits
+// an L2-resident table slice. Worth it only for big tables and big batches; thresholds overridable for tests.
+struct PartPlan { bool on = false; int npart = 0, pshift = 0, rw = 0; int64_t pcap = 0; size_t bytes = 0; std::vector<int> exprs; int src[GQ_MAX_AGGS]; };
+int64_t env_i64(const char* name, int64_t dflt) { const char* e = getenv(name); return e ? atoll(e) : dflt; }
+PartPlan part_plan(const GqScanSpec& sp, const gq_agg_desc* d, int64_t nrows) {
+  PartPlan pp;
+  if (sp.consumer != GQ_C_HIGHCARD) return pp;
+  for (const GqProbeSpec& ps : sp.probes) if (!ps.unique) return pp;
+  const int64_t cap = agg_capacity(d->max_groups, d->nkeys);
+  const int sw = sp.target_sw;
+  const int64_t table_bytes = cap * sw * 8;
+  if (table_bytes < env_i64("GQ_TUNE_PART_MIN_TABLE_MB", 256) * (1 << 20) || nrows < env_i64("GQ_TUNE_PART_MIN_ROWS", 1 << 24)) return pp;
+  int64_t np = 16;
+  while (np < 4096 && table_bytes / np > (4 << 20) && np * 2 <= cap / 64) np <<= 1;
+  pp.npart = (int)np;
+  pp.pshift = log2i(cap) - log2i(np);
+  for (int a = 0; a < d->naggs; ++a) {
+    pp.src[a] = -1;
+    if (d->aggs[a].op == GQ_COUNT_STAR) continue;
+    size_t i = 0;
+    while (i < pp.exprs.size() && pp.exprs[i] != d->aggs[a].expr) ++i;
+    if (i == pp.exprs.size()) pp.exprs.push_back(d->aggs[a].expr);
+    pp.src[a] = 1 + d->ndependent + (int)i;
+  }
+  pp.rw = (int)align_up((size_t)(1 + d->ndependent + pp.exprs.size()), 4);
+  pp.pcap = nrows / np + nrows / (4 * np) + 1024;
+  pp.bytes = align_up((size_t)np * 8 * GQ_PART_CURSOR_STRIDE, 256) + (size_t)np * (size_t)pp.pcap * pp.rw * 8;
+  pp.on = true;
+  return pp;
+}
+
 }  // namespace
 
 extern "C" {
@@ -544,6 +578,10 @@ gq_status gq_hash_aggregate_workspace_for(const gq_batch* in, const gq_agg_desc*
   if (st != GQ_OK) return st;
   DirectPlan dp = direct_plan(sp, d, in);
   if (dp.step >= 0) *bytes = std::max(*bytes, dp.bytes);
+  else {
+    PartPlan pp = part_plan(sp, d, in->nrows);
+    if (pp.on) *bytes = align_up(*bytes, 256) + pp.bytes;
+  }
   return GQ_OK;
 }
 
@@ -590,6 +628,15 @@ gq_status gq_hash_aggregate(gq_ctx* ctx, gq_aggstate** state, void* d_ws, size_t
         a->hot = (long long*)((char*)d_ws + hot_off);
         a->hot_table = (unsigned long long*)((char*)d_ws + hot_off + 4096);
       }
+      {
+        PartPlan pp = part_plan(sp, d, in->nrows);
+        const size_t base = align_up(agg_ws_bytes(cap, sw, d->max_groups, d->nkeys, nullptr), 256);
+        if (pp.on && bytes >= base + pp.bytes) {   // the plan-aware workspace query made room for the record buffers
+          a->pcur = (unsigned long long*)((char*)d_ws + base);
+          a->part = (unsigned long long*)((char*)d_ws + base + align_up((size_t)pp.npart * 8 * GQ_PART_CURSOR_STRIDE, 256));
+          a->pcap = pp.pcap; a->npart = pp.npart; a->pshift = pp.pshift; a->part_rw = pp.rw; a->part_rows = in->nrows;
+        }
+      }
       a->capacity = cap;
       a->lowcard = sp.consumer == GQ_C_LOWCARD; a->lc_cap = sp.lc_cap;
       a->dev.slots = (unsigned long long*)((char*)d_ws + w.slots_off);
@@ -634,6 +681,27 @@ gq_status gq_hash_aggregate(gq_ctx* ctx, gq_aggstate** state, void* d_ws, size_t
     if (e != cudaSuccess) return cuda_fail(ctx, e, "heavy-hitter sampling");
     ctx->launches += nl;
     P.hot = a->hot;
+  }
+  if (a->part && !a->direct && in->nrows >= env_i64("GQ_TUNE_PART_MIN_ROWS", 1 << 24) / 4) {
+    // radix-clustered: pass A appends records per table partition, pass B applies them partition by partition
+    PartPlan pp = part_plan(sp, d, a->part_rows);
+    if (!pp.on || pp.rw != a->part_rw || pp.npart != a->npart) return fail(ctx, GQ_ERR_INVALID_ARG, "batch schema/desc differs from the state's first batch");
+    sp.consumer = GQ_C_PARTITION; sp.part_rw = pp.rw; sp.part_exprs = pp.exprs;
+    P.part = a->part; P.pcur = a->pcur; P.pcap = a->pcap; P.pshift = a->pshift;
+    cudaError_t e = cudaMemsetAsync(a->pcur, 0, (size_t)a->npart * 8 * GQ_PART_CURSOR_STRIDE, ctx->stream);
+    if (e != cudaSuccess) return cuda_fail(ctx, e, "partition cursors");
+    gq_status st2 = run_scan(ctx, sp, in, d->probes, &P);
+    if (st2 != GQ_OK) return st2;
+    GqPartParams pb;
+    memset(&pb, 0, sizeof pb);
+    pb.part = a->part; pb.pcur = a->pcur; pb.pcap = a->pcap; pb.npart = a->npart; pb.rw = a->part_rw;
+    pb.slots = a->dev.slots; pb.mask = a->dev.mask; pb.sw = a->dev.slot_words; pb.ndep = a->ndep; pb.naggs = a->naggs;
+    for (int i = 0; i < a->naggs; ++i) { pb.op[i] = (int)a->agg_op[i]; pb.src[i] = pp.src[i]; }
+    pb.err = ctx->d_err;
+    e = gq_launch_part_upsert(ctx->stream, pb, ctx->num_sms);
+    if (e != cudaSuccess) return cuda_fail(ctx, e, "partitioned upsert");
+    ++ctx->launches;
+    return GQ_OK;
   }
   return run_scan(ctx, sp, in, d->probes, &P);
 }
@@ -918,6 +986,15 @@ gq_status gq_precompile_pipeline(const gq_plan* plan, char* h_msg, size_t msg_by
     GqScanSpec f = sp; f.fused_final = true;
     st = precompile(f, h_msg, msg_bytes);
     if (st != GQ_OK) return st;
+  }
+  {
+    PartPlan pp = part_plan(sp, &plan->agg, plan->in->nrows);
+    if (pp.on) {
+      GqScanSpec f = sp;
+      f.consumer = GQ_C_PARTITION; f.part_rw = pp.rw; f.part_exprs = pp.exprs;
+      st = precompile(f, h_msg, msg_bytes);
+      if (st != GQ_OK) return st;
+    }
   }
   DirectPlan dp = direct_plan(sp, &plan->agg, plan->in, true);
   if (dp.step >= 0) {

@@ -214,7 +214,7 @@ static gq_status emit_linear(Gen& g, const GqScanSpec& sp, std::ostringstream& o
     o << "  }\n";
   }
   std::string keyx, depx;
-  if (sp.consumer == GQ_C_LOWCARD || sp.consumer == GQ_C_HIGHCARD) {
+  if (sp.consumer == GQ_C_LOWCARD || sp.consumer == GQ_C_HIGHCARD || sp.consumer == GQ_C_PARTITION) {
     gq_status st = key_exprs(g, sp, &keyx, &depx, msg);
     if (st != GQ_OK) return st;
   }
@@ -242,6 +242,7 @@ static gq_status emit_linear(Gen& g, const GqScanSpec& sp, std::ostringstream& o
       }
       o << "  }\n";
       break;
+    case GQ_C_PARTITION:
     case GQ_C_HIGHCARD: {
       o << "  i64 tkey[GQ_R];\n  " << LOOP << "tkey[j] = " << keyx << ";\n";
       o << "#if GQ_HOT\n  if (cx.nhot > 0) {\n  " << LOOP << "if (live[j]) {\n      const int hp = gq_hot_find(cx, tkey[j]);\n"
@@ -249,6 +250,24 @@ static gq_status emit_linear(Gen& g, const GqScanSpec& sp, std::ostringstream& o
       for (int a = 0; a < nagg; ++a)
         o << "        gq_hot_update(" << (int)sp.aggs[(size_t)a].op << ", cx, hp, " << a << ", " << aggval(sp.aggs[(size_t)a]) << ");\n";
       o << "        cx.hot_touched[hp] = 1;\n        live[j] = false;\n      }\n    }\n  }\n#endif\n";
+      if (sp.consumer == GQ_C_PARTITION) {
+        // pass A of the radix-clustered aggregation: append (key, dependent key, aggregate inputs) to the record
+        // buffer of the key's table partition; rows that do not fit (or carry the reserved key pattern) fall through
+        // to the ordinary insert-or-update below, so any skew stays correct
+        const int rw = sp.part_rw;
+        o << "  u64 pidx[GQ_R], ppart[GQ_R];\n";
+        o << "  " << LOOP << "{\n    pidx[j] = ~0ULL; ppart[j] = 0;\n    if (live[j] && (u64)tkey[j] != GQ_EMPTY) {\n"
+          << "      ppart[j] = gq_slot0(P.target, tkey[j]) >> P.pshift;\n      pidx[j] = atomicAdd(P.pcur + ppart[j] * 16, 1ULL);\n    }\n  }\n";
+        o << "  " << LOOP << "if (live[j] && pidx[j] < (u64)P.pcap) {\n    u64* rec = P.part + (ppart[j] * (u64)P.pcap + pidx[j]) * " << rw << ";\n";
+        std::vector<std::string> words;
+        words.push_back("(u64)tkey[j]");
+        if (sp.ndep == 1) words.push_back("(u64)" + depx);
+        for (int e : sp.part_exprs) words.push_back("(u64)e" + std::to_string(e) + "[j]");
+        while ((int)words.size() < rw) words.push_back("0ULL");
+        for (int w = 0; w < rw; w += 4)
+          o << "    gq_st256(rec + " << w << ", " << words[(size_t)w] << ", " << words[(size_t)w + 1] << ", " << words[(size_t)w + 2] << ", " << words[(size_t)w + 3] << ");\n";
+        o << "    live[j] = false;\n  }\n";
+      }
       o << "  u64* slot[GQ_R]; bool won[GQ_R];\n";
       o << "  gq_upsert_rows<" << sp.target_sw << ">(P.target, tkey, live, slot, won, P.err);\n";
       o << "  " << LOOP << "if (live[j] && slot[j]) {\n";
@@ -335,7 +354,8 @@ gq_status gq_codegen(const GqScanSpec& sp, GqKernelInfo* out, std::string* msg) 
   auto env_int = [](const char* name) { const char* e = getenv(name); return e ? atoi(e) : 0; };   // tuning sweeps only
   // Hash phases are bound by memory latency, not bandwidth (profiles/r1_hash_phases.md): 24 consumer warps x 2 rows
   // hide more of it than 16 x 4 (C4 1.56 -> 1.13 ms). Pure scans: 20 warps x 2 rows (C2 0.242 -> 0.238 ms).
-  const bool hashing = nprobe > 0 || sp.consumer == GQ_C_BUILD || sp.consumer == GQ_C_HIGHCARD || sp.consumer == GQ_C_DIRECT;
+  const bool hashing = nprobe > 0 || sp.consumer == GQ_C_BUILD || sp.consumer == GQ_C_HIGHCARD || sp.consumer == GQ_C_DIRECT ||
+                       sp.consumer == GQ_C_PARTITION;
   int nt = hashing ? 768 : 640;
   const bool tablebound = sp.consumer == GQ_C_HIGHCARD && nprobe == 0;   // DRAM-random bound (C5): 16 warps x 4 rows measured best
   if (tablebound) nt = 512;
@@ -356,7 +376,7 @@ gq_status gq_codegen(const GqScanSpec& sp, GqKernelInfo* out, std::string* msg) 
   }
   bool all_unique = true;
   for (const GqProbeSpec& ps : sp.probes) all_unique = all_unique && ps.unique;
-  const bool use_hot = sp.hot && sp.consumer == GQ_C_HIGHCARD && all_unique;   // linear mode only
+  const bool use_hot = sp.hot && (sp.consumer == GQ_C_HIGHCARD || sp.consumer == GQ_C_PARTITION) && all_unique;   // linear mode only
   if (use_hot) cons_bytes = 512 * 8 + 512LL * nagg * 8 + 512 * 4 + 256;
   int r = tablebound ? 4 : 2, stages = 0;
   // small inputs: smaller tiles so that every SM still gets several tiles

@@ -15,7 +15,7 @@
 #define GQ_MAXOUT 12
 #define GQ_SMEM_LIMIT 232448   // 227 KB opt-in dynamic shared memory per CTA on sm_100
 
-enum { GQ_C_GLOBAL = 0, GQ_C_LOWCARD = 1, GQ_C_HIGHCARD = 2, GQ_C_BUILD = 3, GQ_C_MATERIALISE = 4, GQ_C_DIRECT = 5 };
+enum { GQ_C_GLOBAL = 0, GQ_C_LOWCARD = 1, GQ_C_HIGHCARD = 2, GQ_C_BUILD = 3, GQ_C_MATERIALISE = 4, GQ_C_DIRECT = 5, GQ_C_PARTITION = 6 };
 
 // ---- device-visible structs: layouts must match gq_skeleton.cuh ----
 struct GqTableDev {
@@ -54,6 +54,10 @@ struct GqParams {
   int* err;
   int pad;
   unsigned long long* dacc;    // DIRECT: aggregate words indexed by slot of the probed unique table
+  unsigned long long* part;    // PARTITION: record buffers
+  unsigned long long* pcur;    // PARTITION: append cursors
+  long long pcap;
+  long long pshift;
   GqFinal fin;
 };
 
@@ -100,6 +104,10 @@ struct gq_aggstate {
   int64_t dcap = 0;            //   its capacity (the accumulator array has dcap + 1 slots: the last is the side entry)
   int daw = 0, dtouch = -1, dep_pay = -1;   // words per accumulator slot, word that marks a touched slot, payload = dep key
   unsigned long long* dacc = nullptr;
+  unsigned long long* part = nullptr;  // radix-clustered mode: record buffers and cursors (in the workspace)
+  unsigned long long* pcur = nullptr;
+  int64_t pcap = 0; int npart = 0, pshift = 0, part_rw = 0;
+  int64_t part_rows = 0;               //   rows the buffers were sized for
   long long* hot = nullptr;            // hot list (in the workspace)
   unsigned long long* hot_table = nullptr;
   std::string sig;
@@ -128,6 +136,8 @@ struct GqScanSpec {
   int direct_step = -1;                           // DIRECT: probe step whose matched slot is the group
   int direct_aw = 0;                              // DIRECT: words per accumulator slot
   bool direct_touch = false;                      // DIRECT: hidden COUNT word marks touched slots
+  int part_rw = 0;                                // PARTITION: words per record (multiple of 4)
+  std::vector<int> part_exprs;                    // PARTITION: expressions stored in a record, in word order
   int target_sw = 0;                              // slot words of the target table
   int build_key_col = 0;                          // BUILD
   std::vector<int> payload_cols;
@@ -174,6 +184,14 @@ cudaError_t gq_launch_init_table(cudaStream_t s, unsigned long long* slots, long
 cudaError_t gq_launch_finalise(cudaStream_t s, const GqFinaliseParams& p, int num_sms, int* nlaunches);
 cudaError_t gq_launch_read_probe(cudaStream_t s, const void* data, size_t bytes, unsigned long long* out, int num_sms);
 cudaError_t gq_launch_random_probe(cudaStream_t s, void* table, size_t bytes, long long n, int mode, unsigned long long* out, int num_sms);
+#define GQ_PART_CURSOR_STRIDE 16   // one append cursor per 128-byte line: atomics to one line serialise at L2
+struct GqPartParams {
+  const unsigned long long* part; const unsigned long long* pcur; long long pcap; int npart; int rw;
+  unsigned long long* slots; unsigned long long mask; int sw; int ndep; int naggs;
+  int op[GQ_MAX_AGGS]; int src[GQ_MAX_AGGS];   // src = record word of the aggregate's input, -1 = COUNT(*)
+  int* err;
+};
+cudaError_t gq_launch_part_upsert(cudaStream_t s, const GqPartParams& p, int num_sms);
 size_t gq_topk_scratch_bytes_impl();
 cudaError_t gq_launch_hot_keys(cudaStream_t s, const void* keycol, int dtype, long long nrows, unsigned long long* table,
                                long long nslots, long long nsample, unsigned long long threshold, long long* hot,

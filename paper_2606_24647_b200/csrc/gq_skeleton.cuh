@@ -38,6 +38,7 @@ typedef unsigned int u32;
 #define GQ_C_BUILD 3
 #define GQ_C_MATERIALISE 4
 #define GQ_C_DIRECT 5
+#define GQ_C_PARTITION 6
 
 #define GQ_E_CAPACITY 3
 #define GQ_E_DUPLICATE 6
@@ -90,6 +91,10 @@ struct GqParams {
   int* err;                     // sticky device error
   int pad;
   u64* dacc;                    // DIRECT: aggregate words indexed by the slot of the probed unique table
+  u64* part;                    // PARTITION: record buffers, [npart][pcap] records of GQ_PART_RW words
+  u64* pcur;                    // PARTITION: per-partition append cursors
+  i64 pcap;                     // PARTITION: records per partition
+  i64 pshift;                   // PARTITION: partition = first slot of the key in the target table >> pshift
   GqFinal fin;                  // GQ_FUSED_FINAL: outputs of the in-kernel finaliser
 };
 
@@ -408,6 +413,14 @@ __device__ __forceinline__ i64 gq_warp_reduce(const int OP, i64 v) {
 #pragma unroll
   for (int o = 16; o > 0; o >>= 1) v = gq_combine(OP, v, __shfl_xor_sync(0xffffffffu, v, o));
   return v;
+}
+
+// Radix-clustered aggregation, pass A: a surviving row is appended to the record buffer of the
+// partition its key's first table slot falls in; pass B (gq_k_part_upsert) then applies the records partition by
+// partition, so the slice of the group-by table being updated stays L2-resident. One record = GQ_PART_RW words (key,
+// dependent key, aggregate inputs), a multiple of 4 words so that it is written with 32-byte stores.
+__device__ __forceinline__ void gq_st256(u64* p, u64 a, u64 b, u64 c, u64 d) {
+  asm volatile("st.global.v4.u64 [%0], {%1, %2, %3, %4};" ::"l"(p), "l"(a), "l"(b), "l"(c), "l"(d) : "memory");
 }
 
 // ---------------------------------------------------------------------------------------------- row sources

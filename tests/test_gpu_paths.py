@@ -165,3 +165,53 @@ def test_lowcard_more_groups_than_declared_is_an_error():
     p.run()
     c.sync()                                                   # and the ticket counter survived the failed run
     assert p.result()["n"] == 9
+
+
+# ------------------------------------------------------------------ radix-clustered (partitioned) aggregation
+@pytest.fixture
+def force_partition(monkeypatch):
+    # thresholds that switch the partitioned path on for tables and batches the oracle can check in seconds
+    monkeypatch.setenv("GQ_TUNE_PART_MIN_TABLE_MB", "0")
+    monkeypatch.setenv("GQ_TUNE_PART_MIN_ROWS", "4096")
+
+
+@pytest.mark.parametrize("scale", [0.003, 0.0101])
+def test_partitioned_aggregation_c5_shape(ctx, force_partition, scale):
+    plan = plans.plan_c5(datagen.make_config(5, scale=scale))
+    l0 = ctx.launch_count()
+    run(plan, ctx)
+    assert ctx.launch_count() - l0 >= 4          # init, scan (pass A), partitioned upsert (pass B), finalise
+
+
+def test_partitioned_aggregation_skew_overflow_reserved_key_and_dependent_key(ctx, force_partition):
+    rng = np.random.default_rng(11)
+    n = 300_000
+    # one key owns 60 % of the rows (its partition overflows -> in-kernel fallback), plus the reserved bit pattern
+    k = rng.integers(0, 50_000, n).astype(np.int64) * 7919
+    k[rng.random(n) < 0.6] = 123456789
+    k[::1000] = I64_MIN
+    dep = (k % 1000).astype(np.int32)              # functionally dependent on the key
+    v = rng.integers(-1000, 1000, n).astype(np.int64)
+    w = rng.integers(0, 5, n).astype(np.int64)
+    plan = dict(table=[k, dep, v, w], preds=[(3, "lt", 4)], exprs=[[("col", 2)], [("col", 3)]], keys=[0, 1], ndependent=1,
+                aggs=[("sum", 0), ("min", 0), ("max", 1), ("count",), ("sum", 1)], max_groups=60_000)
+    run(plan, ctx)
+
+
+def test_partitioned_aggregation_streams_batches(ctx, force_partition):
+    import gqrun
+    plan = plans.plan_c5(datagen.make_config(5, scale=0.004))
+    exp = oracle.run_query(plan)
+    cols = gqrun.dev(plan["table"])
+    n = len(plan["table"][0])
+    st = None
+    for lo, hi in ((0, n // 2 // 16 * 16), (n // 2 // 16 * 16, n - 160), (n - 160, n)):   # last batch takes the plain path
+        st = ctx.aggregate(st, [c[lo:hi] for c in cols], preds=plan["preds"], exprs=plan["exprs"], keys=plan["keys"],
+                           aggs=plan["aggs"], max_groups=plan["max_groups"], plan_aware_workspace=True)
+    r = ctx.aggregate_finish(st, capacity=exp.nrows + 5)
+    ctx.sync()
+    ng = int(r["n"].item())
+    assert ng == exp.nrows
+    got = gqrun.sort_rows([r["keys"][0][:ng].cpu().numpy()] + [a[:ng].cpu().numpy() for a in r["aggs"]], 1)
+    for g, e in zip(got, exp.cols):
+        assert np.array_equal(g, e)
