@@ -539,6 +539,7 @@ PartPlan part_plan(const GqScanSpec& sp, const gq_agg_desc* d, int64_t nrows) {
   if (table_bytes < env_i64("GQ_TUNE_PART_MIN_TABLE_MB", 256) * (1 << 20) || nrows < env_i64("GQ_TUNE_PART_MIN_ROWS", 1 << 24)) return pp;
   int64_t np = 16;
   while (np < 4096 && table_bytes / np > (4 << 20) && np * 2 <= cap / 64) np <<= 1;
+  if (env_i64("GQ_TUNE_PART_NPART", 0) > 0) np = env_i64("GQ_TUNE_PART_NPART", 0);
   pp.npart = (int)np;
   pp.pshift = log2i(cap) - log2i(np);
   for (int a = 0; a < d->naggs; ++a) {
