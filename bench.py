@@ -122,7 +122,7 @@ def time_steps(torch, stream, fn, steps, warmup, barrier):
 def parse_configs(text, c5_scale):
     """'1,1x64,3' -> [(label, cfg, scale)]; 'NxS' = config N at S times its row count (supplementary steady-state rows)."""
     out = []
-    for tok in [t for t in text.split(",") if t]:
+    for tok in [t for t in text.split(",") if t and t != "ops"]:
         if "x" in tok:
             c, sc = tok.split("x")
             out.append((f"C{c}x{sc}", int(c), float(sc)))
@@ -186,6 +186,59 @@ def run_config(cfg, gq, ctx, torch, datagen, plans, gqrun, steps, warmup, scale=
             state["pipes"][0].run()
         out["ms_l2_warm"] = time_steps(torch, ctx.stream, warm, steps, warmup, lambda: None) / steps
     return out, plan, state
+
+
+def run_standalone_ops(gq, ctx, torch, datagen, plans, gqrun, steps, warmup):
+    """The standalone, materialising entry points on the C2 / C3 tables: gq_filter_project
+    (ballot/popc compaction), gq_hash_build, gq_hash_probe (inner join materialised as output columns)."""
+    out = {}
+    t2 = datagen.make_config(2)
+    p2 = plans.plan_c2(t2)
+    cols = gqrun.dev(p2["table"])
+    n = len(p2["table"][0])
+    exprs = [[("col", 3), ("col", 1), ("mul",)], [("col", 0)]]
+    cap = n // 20
+    outs = [torch.empty(cap, dtype=torch.int64, device="cuda") for _ in exprs]
+    count = torch.zeros(1, dtype=torch.int64, device="cuda")
+
+    def fp():
+        count.zero_()
+        ctx.filter_project(cols, p2["preds"], exprs, capacity=cap, outs=outs, count=count)
+    ms = time_steps(torch, ctx.stream, fp, steps, warmup, lambda: None) / steps
+    ctx.sync()
+    out["filter_project_c2"] = dict(rows=n, out_rows=int(count.item()), ms=ms, rows_per_s=n / ms * 1e3,
+                                    gbs=(28 * n + 16 * int(count.item())) / ms / 1e6)
+    del cols, outs
+    torch.cuda.empty_cache()
+    t3 = datagen.make_config(3)
+    p3 = plans.plan_c3(t3)
+    b = p3["builds"][0]
+    bcols = gqrun.dev(b["table"])
+    nb = len(b["table"][0])
+    hint = int(nb * 0.55) + 1024
+    tb = ctx.hash_build(bcols, preds=b["preds"], key=0, unique=True, max_rows=hint)
+    ws = tb.workspace
+
+    def build():
+        ctx.hash_build(bcols, preds=b["preds"], key=0, unique=True, max_rows=hint, workspace=ws)
+    ms = time_steps(torch, ctx.stream, build, steps, warmup, lambda: None) / steps
+    out["hash_build_c3_dim"] = dict(rows=nb, ms=ms, rows_per_s=nb / ms * 1e3, gbs=12 * nb / ms / 1e6,
+                                    note="table init + scan + CAS inserts (7.48 M of 15 M rows pass the filter)")
+    tb = ctx.hash_build(bcols, preds=b["preds"], key=0, unique=True, max_rows=hint, workspace=ws)
+    fcols = gqrun.dev(p3["table"])
+    nf = len(p3["table"][0])
+    pexprs = [[("col", 0)], p3["exprs"][0]]
+    pcap = nf // 3
+    pouts = [torch.empty(pcap, dtype=torch.int64, device="cuda") for _ in pexprs]
+
+    def probe():
+        count.zero_()
+        ctx.hash_probe(fcols, p3["preds"], [(tb, 0)], pexprs, capacity=pcap, outs=pouts, count=count)
+    ms = time_steps(torch, ctx.stream, probe, steps, warmup, lambda: None) / steps
+    ctx.sync()
+    out["hash_probe_c3_fact"] = dict(rows=nf, out_rows=int(count.item()), ms=ms, rows_per_s=nf / ms * 1e3,
+                                     gbs=(28 * nf + 16 * int(count.item())) / ms / 1e6)
+    return out
 
 
 def oracle_rate(plans, datagen, cfg, sample_rows, reps=1):
@@ -260,7 +313,8 @@ def main():
     ap.add_argument("--steps", type=int, default=400)
     ap.add_argument("--warmup", type=int, default=5)
     ap.add_argument("--impl", default="ours")
-    ap.add_argument("--configs", default="1,1x64,3,4,5", help="extra configs reported under per_config ('' = none); "
+    ap.add_argument("--configs", default="1,1x64,3,4,5,ops", help="extra configs reported under per_config ('' = none); "
+                    "ops = the standalone materialising entry points (filter_project, hash_build, hash_probe); "
                     "NxS = config N at S times its rows (C1x64: the low-cardinality pipeline at steady state)")
     ap.add_argument("--c5-scale", type=float, default=1.0)
     ap.add_argument("--no-cpu-baseline", action="store_true")
@@ -303,6 +357,8 @@ def main():
         for label, cfg, sc in parse_configs(args.configs, args.c5_scale):
             out, _, _ = run_config(cfg, gq, ctx, torch, datagen, plans, gqrun, args.steps, args.warmup, scale=sc, peak=peak)
             per_config[label] = out
+        if "ops" in args.configs.split(","):
+            per_config["standalone_ops"] = run_standalone_ops(gq, ctx, torch, datagen, plans, gqrun, args.steps, args.warmup)
         print(json.dumps(dict(per_config=per_config)))
         return
 
@@ -373,6 +429,13 @@ def main():
                 per_config[label] = out
             except Exception as e:  # a failing extra config must not hide the headline number
                 per_config[label] = dict(error=str(e)[:300])
+            torch.cuda.empty_cache()
+
+        if "ops" in args.configs.split(","):
+            try:
+                per_config["standalone_ops"] = run_standalone_ops(gq, ctx, torch, datagen, plans, gqrun, 10, 3)
+            except Exception as e:
+                per_config["standalone_ops"] = dict(error=str(e)[:300])
             torch.cuda.empty_cache()
 
     # ---------------- CPU baseline: the oracle on this box's host cores ----------------

@@ -191,6 +191,9 @@ gq_status gq_set_kernel_cache_dir(const char* h_path);
  * described by handles created with gq_table_describe (no device memory). */
 gq_status gq_precompile_pipeline(const gq_plan*, char* h_msg, size_t msg_bytes);
 gq_status gq_precompile_build(const gq_batch* in, const gq_build_desc*, char* h_msg, size_t msg_bytes);
+/* The materialising kernel of gq_filter_project (nprobes == 0) / gq_hash_probe for this shape. */
+gq_status gq_precompile_materialise(const gq_batch* in, const gq_pred* preds, int32_t npred, const gq_probe_step* probes,
+                                    int32_t nprobes, const gq_expr* exprs, int32_t nexpr, char* h_msg, size_t msg_bytes);
 /* Host-only table handle carrying just the schema (payload dtypes, flags) for precompilation. */
 gq_status gq_table_describe(gq_table** out, const gq_dtype* payload_dtypes, int32_t npayload, uint32_t flags);
 

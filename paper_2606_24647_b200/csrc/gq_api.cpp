@@ -1007,6 +1007,17 @@ gq_status gq_precompile_pipeline(const gq_plan* plan, char* h_msg, size_t msg_by
   return precompile(sp, h_msg, msg_bytes);
 }
 
+gq_status gq_precompile_materialise(const gq_batch* in, const gq_pred* preds, int32_t npred, const gq_probe_step* probes,
+                                    int32_t nprobes, const gq_expr* exprs, int32_t nexpr, char* h_msg, size_t msg_bytes) {
+  if (!in || nexpr < 1) return GQ_ERR_INVALID_ARG;
+  gq_ctx tmp;
+  GqScanSpec sp;
+  gq_status st = fill_common(&tmp, &sp, in, preds, npred, probes, nprobes, exprs, nexpr);
+  if (st != GQ_OK) { if (h_msg && msg_bytes) { strncpy(h_msg, tmp.msg.c_str(), msg_bytes - 1); h_msg[msg_bytes - 1] = 0; } return st; }
+  sp.consumer = GQ_C_MATERIALISE;
+  return precompile(sp, h_msg, msg_bytes);
+}
+
 gq_status gq_precompile_build(const gq_batch* in, const gq_build_desc* d, char* h_msg, size_t msg_bytes) {
   if (!in || !d) return GQ_ERR_INVALID_ARG;
   gq_ctx tmp;

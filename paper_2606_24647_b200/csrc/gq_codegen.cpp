@@ -302,9 +302,10 @@ static gq_status emit_linear(Gen& g, const GqScanSpec& sp, std::ostringstream& o
     }
     case GQ_C_MATERIALISE:
       if (sp.exprs.size() > GQ_MAXOUT) { if (msg) *msg = "too many output columns"; return GQ_ERR_UNSUPPORTED; }
-      o << "  " << LOOP << "if (live[j]) {\n    const i64 orow = gq_reserve_row(P);\n    if (orow >= 0) {\n";
-      for (size_t e = 0; e < sp.exprs.size(); ++e) o << "      P.out[" << e << "][orow] = e" << e << "[j];\n";
-      o << "    }\n  }\n";
+      o << "  i64 orow[GQ_R];\n  gq_materialise_offsets(P, cx, live, orow);\n";
+      o << "  " << LOOP << "if (orow[j] >= 0) {\n";
+      for (size_t e = 0; e < sp.exprs.size(); ++e) o << "    P.out[" << e << "][orow[j]] = e" << e << "[j];\n";
+      o << "  }\n";
       break;
     default: if (msg) *msg = "unknown consumer"; return GQ_ERR_INVALID_ARG;
   }
@@ -382,6 +383,7 @@ gq_status gq_codegen(const GqScanSpec& sp, GqKernelInfo* out, std::string* msg) 
   // small inputs: smaller tiles so that every SM still gets several tiles
   if (sp.nrows_hint > 0 && sp.nrows_hint < 148LL * 8 * nt * 2) r = 1;
   if (sp.consumer == GQ_C_LOWCARD) r = (sp.nrows_hint > 0 && sp.nrows_hint < 148LL * nt * 4) ? 1 : 4;   // straight-line rows: ILP
+  if (sp.consumer == GQ_C_MATERIALISE && !hashing && !(sp.nrows_hint > 0 && sp.nrows_hint < 148LL * 8 * nt * 2)) r = 4;   // two CTA barriers per tile: bigger tiles
   if (env_int("GQ_TUNE_R")) r = env_int("GQ_TUNE_R");
   long long stage_bytes = 0;
   for (;; r /= 2) {

@@ -450,6 +450,7 @@ struct GqCtx {
   i64* lc_gkey;                         //   key of every group id [GQ_LC_G]
   int* lc_n;                            //   [0] groups so far, [1] insert lock, [2] gid of the reserved-pattern key + 1
   i64* lc_acc;                          //   accumulators [GQ_LC_G][GQ_NAGG][GQ_NT], thread-private cells
+  int* mat;                             // MATERIALISE: shared [0] rows of the tile so far, [2..3] the tile's output base
   i64 ninserted;                        // BUILD: rows inserted by this thread
   i64* hot_keys;                        // HIGHCARD + GQ_HOT: shared set of this batch's hot keys [GQ_HOT_POS]
   u64* hot_acc;                         //   CTA-shared accumulators [GQ_HOT_POS][GQ_NAGG]
@@ -630,6 +631,38 @@ __device__ __forceinline__ i64 gq_reserve_row(const GqParams& P) {
   i64 idx = base + __popc(m & ((1u << lane) - 1u));
   if (idx >= P.out_capacity) { gq_set_err(P.err, GQ_E_CAPACITY); return -1; }
   return idx;
+}
+
+// MATERIALISE, linear mode: one global reservation per CTA and tile. Ballot/popc gives each row its rank inside the
+// warp, a shared-memory add gives the warp its offset inside the tile, and thread 0 reserves the tile's output range
+// with ONE atomic on the device-side row count (per-warp reservations serialise on that single address: 1.2 ms for
+// the 1.09 M output rows of the C2 filter; per-tile ones do not).
+__device__ __forceinline__ void gq_materialise_offsets(const GqParams& P, GqCtx& cx, const bool (&live)[GQ_R], i64 (&orow)[GQ_R]) {
+  const int lane = threadIdx.x & 31;
+  int pre[GQ_R];
+  int wtot = 0;
+#pragma unroll
+  for (int j = 0; j < GQ_R; ++j) {
+    const u32 m = __ballot_sync(0xffffffffu, live[j]);
+    pre[j] = wtot + __popc(m & ((1u << lane) - 1u));
+    wtot += __popc(m);
+  }
+  int woff = 0;
+  if (lane == 0 && wtot) woff = atomicAdd(&cx.mat[0], wtot);
+  woff = __shfl_sync(0xffffffffu, woff, 0);
+  gq_consumer_barrier();                                  // every warp has added its rows
+  if (threadIdx.x == 0) {
+    const int tot = ((volatile int*)cx.mat)[0];
+    *(volatile i64*)(cx.mat + 2) = tot ? (i64)atomicAdd((u64*)P.out_count, (u64)tot) : 0;
+    ((volatile int*)cx.mat)[0] = 0;
+  }
+  gq_consumer_barrier();                                  // base published, tile counter reset
+  const i64 base = *(volatile i64*)(cx.mat + 2);
+#pragma unroll
+  for (int j = 0; j < GQ_R; ++j) {
+    orow[j] = live[j] ? base + woff + pre[j] : -1;
+    if (orow[j] >= P.out_capacity) { gq_set_err(P.err, GQ_E_CAPACITY); orow[j] = -1; }
+  }
 }
 
 //@@ROW_FUNCTIONS@@

@@ -111,6 +111,10 @@ extern "C" __global__ void __launch_bounds__(GQ_NT + 32, 1) gq_scan(const __grid
 #pragma unroll
   for (int a = 0; a < GQ_NAGG; ++a) cx.acc[a] = gq_identity(GQ_AGG_OP(a));
 #endif
+#if GQ_CONSUMER == GQ_C_MATERIALISE
+  cx.mat = (int*)(gq_smem + GQ_CONS_OFF);
+  if (tid < 4) cx.mat[tid] = 0;
+#endif
 #if GQ_HOT
   cx.hot_keys = (i64*)(gq_smem + GQ_CONS_OFF);
   cx.hot_acc = (u64*)(cx.hot_keys + GQ_HOT_POS);

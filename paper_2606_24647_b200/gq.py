@@ -36,7 +36,7 @@ SYMBOLS = ["gq_create", "gq_destroy", "gq_sync", "gq_clear_error", "gq_status_st
            "gq_hash_build_finish", "gq_table_count", "gq_table_destroy", "gq_hash_probe",
            "gq_hash_aggregate_workspace", "gq_hash_aggregate_workspace_for", "gq_hash_aggregate", "gq_topk_scratch_bytes", "gq_hash_aggregate_finish",
            "gq_aggstate_destroy", "gq_pipeline_workspace", "gq_pipeline", "gq_pipeline_host_workspace",
-           "gq_pipeline_host", "gq_set_kernel_cache_dir", "gq_precompile_pipeline", "gq_precompile_build",
+           "gq_pipeline_host", "gq_set_kernel_cache_dir", "gq_precompile_pipeline", "gq_precompile_build", "gq_precompile_materialise",
            "gq_table_describe", "gq_read_probe", "gq_random_probe"]
 
 
@@ -141,6 +141,8 @@ def lib():
         L.gq_set_kernel_cache_dir.argtypes = [C.c_char_p]
         L.gq_precompile_pipeline.argtypes = [C.POINTER(_Plan), C.c_char_p, C.c_size_t]
         L.gq_precompile_build.argtypes = [C.POINTER(_Batch), C.POINTER(_BuildDesc), C.c_char_p, C.c_size_t]
+        L.gq_precompile_materialise.argtypes = [C.POINTER(_Batch), C.POINTER(_Pred), C.c_int32, C.POINTER(_Probe), C.c_int32,
+                                                C.POINTER(_Expr), C.c_int32, C.c_char_p, C.c_size_t]
         L.gq_table_describe.argtypes = [C.POINTER(C.c_void_p), C.POINTER(C.c_int), C.c_int32, C.c_uint32]
         L.gq_read_probe.argtypes = [C.c_void_p, C.c_void_p, C.c_size_t, C.c_void_p]
         L.gq_random_probe.argtypes = [C.c_void_p, C.c_void_p, C.c_size_t, C.c_int64, C.c_int32, C.c_void_p]
@@ -335,13 +337,16 @@ class Context:
         return (ws.data_ptr() + 255) // 256 * 256
 
     # ---- FilterProject / HashProbe (materialising) ----
-    def filter_project(self, cols, preds, exprs, capacity=None, probes=()):
+    def filter_project(self, cols, preds, exprs, capacity=None, probes=(), outs=None, count=None):
+        """outs / count: optional pre-allocated int64 output columns and a ZEROED int64[1] counter to reuse."""
         with torch.cuda.stream(self.stream):
             m = _M()
             b = m.batch(cols)
             cap = int(capacity) if capacity is not None else int(b.nrows)
-            outs = [self._empty(cap, torch.int64) for _ in exprs]
-            count = torch.zeros(1, dtype=torch.int64, device=self.device)
+            if outs is None:
+                outs = [self._empty(cap, torch.int64) for _ in exprs]
+            if count is None:
+                count = torch.zeros(1, dtype=torch.int64, device=self.device)
             pr, npr = m.preds(preds)
             ee, ne = m.exprs(exprs)
             if probes:
@@ -352,8 +357,8 @@ class Context:
             self._check(st)
         return outs, count
 
-    def hash_probe(self, cols, preds, probes, exprs, capacity):
-        return self.filter_project(cols, preds, exprs, capacity=capacity, probes=probes)
+    def hash_probe(self, cols, preds, probes, exprs, capacity, outs=None, count=None):
+        return self.filter_project(cols, preds, exprs, capacity=capacity, probes=probes, outs=outs, count=count)
 
     # ---- HashBuild ----
     def hash_build(self, cols, preds=(), probes=(), key=0, payload=(), unique=False, max_rows=None, table=None,
@@ -514,6 +519,20 @@ def precompile_pipeline(col_dtypes, nrows, preds=(), probes=(), exprs=(), keys=(
     plan = _Plan(C.pointer(b), m.agg_desc(preds, probes, exprs, keys, ndependent, aggs, max_groups), None, 0, 0, 0)
     buf = C.create_string_buffer(8192)
     st = lib().gq_precompile_pipeline(C.byref(plan), buf, 8192)
+    if st:
+        raise GqError(st, buf.value.decode(errors="replace"))
+    return buf.value.decode()
+
+
+def precompile_materialise(col_dtypes, nrows, preds=(), probes=(), exprs=()):
+    """Kernel of filter_project / hash_probe for this shape; needs no GPU. Returns the cubin path."""
+    m = _M()
+    b = m.batch([None] * len(col_dtypes), dtypes=list(col_dtypes), nrows=int(nrows))
+    pr, npr = m.preds(preds)
+    pb, npb = m.probes(probes)
+    ee, ne = m.exprs(exprs)
+    buf = C.create_string_buffer(8192)
+    st = lib().gq_precompile_materialise(C.byref(b), pr, npr, pb, npb, ee, ne, buf, 8192)
     if st:
         raise GqError(st, buf.value.decode(errors="replace"))
     return buf.value.decode()
