@@ -404,7 +404,7 @@ gq_status gq_codegen(const GqScanSpec& sp, GqKernelInfo* out, std::string* msg) 
   o << "#define GQ_NAGG " << nagg << "\n#define GQ_LC_G " << (sp.lc_cap > 0 ? sp.lc_cap : 1) << "\n#define GQ_LC_KT " << lc_kt
     << "\n#define GQ_LC_KEY32 " << lc_key32 << "\n#define GQ_TARGET_SW "
     << (sp.target_sw > 0 ? sp.target_sw : 1) << "\n#define GQ_NDEP " << sp.ndep << "\n#define GQ_EVICT_FIRST " << (getenv("GQ_TUNE_NO_EVICT_FIRST") ? 0 : 1) << "\n#define GQ_HOT " << (use_hot ? 1 : 0)
-    << "\n#define GQ_FUSED_FINAL " << (sp.fused_final ? 1 : 0) << "\n#define GQ_DIRECT_AW " << (sp.direct_aw > 0 ? sp.direct_aw : 1) << "\n";
+    << "\n#define GQ_STAMPS " << (getenv("GQ_TUNE_STAMPS") ? 1 : 0) << "\n#define GQ_FUSED_FINAL " << (sp.fused_final ? 1 : 0) << "\n#define GQ_DIRECT_AW " << (sp.direct_aw > 0 ? sp.direct_aw : 1) << "\n";
   {
     long long off = 0, tx = 0;
     std::ostringstream offs, bytes;

@@ -466,6 +466,7 @@ struct GqCtx {
 // on the per-row path. Cells are reduced over threads once, at the end (Partial -> Final of PAPER.md:154 inside one
 // kernel). Packed keys narrower than 32 bits use {key32, gid} entries fetched with one LDS.64.
 #define GQ_LC_LOG2KT (GQ_LC_KT == 64 ? 6 : GQ_LC_KT == 128 ? 7 : 8)
+#define GQ_LC_PENDING 0xFFFFFFFEu   // group id of a key-table position that is claimed but not published yet
 __device__ __forceinline__ u32 gq_lc_hash(i64 key) {
 #if GQ_LC_KEY32
   return ((u32)key * 0x9E3779B1u) >> (32 - GQ_LC_LOG2KT);
@@ -480,14 +481,14 @@ __device__ __forceinline__ int gq_lc_find(const GqCtx& cx, i64 key) {
 #if GQ_LC_KEY32
   for (int n = 0; n < GQ_LC_KT; ++n, h = (h + 1) & (GQ_LC_KT - 1)) {
     const u64 e = ((volatile u64*)cx.lc_tab)[h];
-    if ((u32)(e >> 32) == (u32)key) return (int)(u32)e;
+    if ((u32)(e >> 32) == (u32)key) return (u32)e == GQ_LC_PENDING ? -1 : (int)(u32)e;
     if (e == ~0ULL) return -1;
   }
 #else
-  if ((u64)key == GQ_EMPTY) return ((volatile int*)cx.lc_n)[2] - 1;   // reserved bit pattern: id kept aside
+  if ((u64)key == GQ_EMPTY) { const int v = ((volatile int*)cx.lc_n)[2]; return v > 0 ? v - 1 : -1; }   // reserved bit pattern: id kept aside
   for (int n = 0; n < GQ_LC_KT; ++n, h = (h + 1) & (GQ_LC_KT - 1)) {
     const u64 k = ((volatile u64*)cx.lc_tab)[h];
-    if (k == (u64)key) return (int)((volatile u32*)cx.lc_gid)[h];
+    if (k == (u64)key) { const u32 g = ((volatile u32*)cx.lc_gid)[h]; return g == GQ_LC_PENDING ? -1 : (int)g; }
     if (k == GQ_EMPTY) return -1;
   }
 #endif
@@ -498,15 +499,85 @@ __device__ __forceinline__ int gq_lc_find1(const GqCtx& cx, i64 key) {
   const u32 h = gq_lc_hash(key);
 #if GQ_LC_KEY32
   const u64 e = ((volatile u64*)cx.lc_tab)[h];
-  return (u32)(e >> 32) == (u32)key ? (int)(u32)e : -1;
+  return ((u32)(e >> 32) == (u32)key && (u32)e != GQ_LC_PENDING) ? (int)(u32)e : -1;
 #else
   const u64 k = ((volatile u64*)cx.lc_tab)[h];
-  return (k == (u64)key && k != GQ_EMPTY) ? (int)((volatile u32*)cx.lc_gid)[h] : -1;
+  if (k != (u64)key || k == GQ_EMPTY) return -1;
+  const u32 g = ((volatile u32*)cx.lc_gid)[h];
+  return g == GQ_LC_PENDING ? -1 : (int)g;
 #endif
 }
 // Slow path (collision, or first sight of a key): the warp handles its needy lanes one key at a time; lane 0 takes
 // the CTA lock, walks the probe sequence and inserts the key with the next group id if it is absent. Must be called
 // by all 32 lanes of the warp (converged); `need` selects the lanes that want an answer.
+// Lock-free insert-or-find of one key by ONE thread: the table position is claimed by CAS with a "pending" group id,
+// the winner then draws the next dense id and publishes it; a thread that meets a pending entry of its key waits for
+// the id (the winner is always another warp, or this very thread).
+__device__ __forceinline__ int gq_lc_new_group(GqCtx& cx, i64 k, int* err) {
+  int g = atomicAdd(&cx.lc_n[0], 1);
+  if (g >= GQ_LC_G) { gq_set_err(err, GQ_E_CAPACITY); g = 0; }   // more distinct keys than max_groups
+  else cx.lc_gkey[g] = k;
+  return g;
+}
+__device__ __forceinline__ int gq_lc_insert_or_find(GqCtx& cx, i64 k, int* err) {
+#if !GQ_LC_KEY32
+  if ((u64)k == GQ_EMPTY) {                               // reserved bit pattern: its id lives in lc_n[2] (id + 1)
+    for (;;) {
+      const int v = ((volatile int*)cx.lc_n)[2];
+      if (v > 0) return v - 1;
+      if (v == 0 && atomicCAS(&cx.lc_n[2], 0, -1) == 0) {
+        const int g = gq_lc_new_group(cx, k, err);
+        __threadfence_block();
+        ((volatile int*)cx.lc_n)[2] = g + 1;
+        return g;
+      }
+    }
+  }
+#endif
+  u32 i = gq_lc_hash(k);
+  for (int adv = 0; adv < GQ_LC_KT;) {                     // `continue` re-examines the same position
+#if GQ_LC_KEY32
+    const u64 e = ((volatile u64*)cx.lc_tab)[i];
+    if ((u32)(e >> 32) == (u32)k) {
+      if ((u32)e != GQ_LC_PENDING) return (int)(u32)e;
+      continue;                                           // id not published yet: look again
+    }
+    if (e == ~0ULL) {
+      const u64 prev = atomicCAS(&cx.lc_tab[i], ~0ULL, ((u64)(u32)k << 32) | GQ_LC_PENDING);
+      if (prev == ~0ULL) {
+        const int g = gq_lc_new_group(cx, k, err);
+        __threadfence_block();
+        ((volatile u64*)cx.lc_tab)[i] = ((u64)(u32)k << 32) | (u32)g;
+        return g;
+      }
+      continue;                                           // somebody claimed this position: re-examine it
+    }
+#else
+    const u64 e = ((volatile u64*)cx.lc_tab)[i];
+    if (e == (u64)k) {
+      const u32 g = ((volatile u32*)cx.lc_gid)[i];
+      if (g != GQ_LC_PENDING) return (int)g;
+      continue;
+    }
+    if (e == GQ_EMPTY) {
+      const u64 prev = atomicCAS(&cx.lc_tab[i], GQ_EMPTY, (u64)k);   // lc_gid[i] holds GQ_LC_PENDING until published
+      if (prev == GQ_EMPTY) {
+        const int g = gq_lc_new_group(cx, k, err);
+        __threadfence_block();
+        ((volatile u32*)cx.lc_gid)[i] = (u32)g;
+        return g;
+      }
+      continue;
+    }
+#endif
+    i = (i + 1) & (GQ_LC_KT - 1);
+    ++adv;
+  }
+  gq_set_err(err, GQ_E_CAPACITY);                         // key table full
+  return 0;
+}
+// Slow path (collision, or first sight of a key): the warp serves its needy lanes one KEY at a time — lane 0 inserts
+// or finds it, every lane waiting for that key takes the answer. Must be called by all 32 lanes (converged).
 __device__ __forceinline__ int gq_lc_slow_body(GqCtx& cx, i64 key, bool need, int grp, int* err) {
   u32 m = __ballot_sync(0xffffffffu, need);
   const int lane = threadIdx.x & 31;
@@ -514,60 +585,9 @@ __device__ __forceinline__ int gq_lc_slow_body(GqCtx& cx, i64 key, bool need, in
     const int l = __ffs(m) - 1;
     const i64 k = __shfl_sync(0xffffffffu, key, l);
     int g = 0;
-    if (lane == 0) g = gq_lc_find(cx, k);          // another warp may have inserted it meanwhile: no lock needed
+    if (lane == 0) g = gq_lc_insert_or_find(cx, k, err);
     g = __shfl_sync(0xffffffffu, g, 0);
-    if (g < 0) {
-    if (lane == 0) {
-      bool locked = false;                      // wait for the lock OR for the key to appear (inserted by its holder)
-      while (g < 0 && !locked) { if (atomicCAS(&cx.lc_n[1], 0, 1) == 0) locked = true; else g = gq_lc_find(cx, k); }
-      if (locked) {
-      __threadfence_block();
-      if ((u64)k == GQ_EMPTY && !GQ_LC_KEY32) {        // reserved bit pattern: its group id lives in lc_n[2]
-        g = ((volatile int*)cx.lc_n)[2] - 1;
-        if (g < 0) {
-          g = ((volatile int*)cx.lc_n)[0];
-          if (g >= GQ_LC_G) { gq_set_err(err, GQ_E_CAPACITY); g = 0; }
-          else { cx.lc_gkey[g] = k; ((volatile int*)cx.lc_n)[0] = g + 1; ((volatile int*)cx.lc_n)[2] = g + 1; }
-        }
-      } else {
-        u32 i = gq_lc_hash(k);
-        g = -1;
-        for (int n = 0; n < GQ_LC_KT && g < 0; ++n, i = (i + 1) & (GQ_LC_KT - 1)) {
-#if GQ_LC_KEY32
-          const u64 e = ((volatile u64*)cx.lc_tab)[i];
-          if ((u32)(e >> 32) == (u32)k) g = (int)(u32)e;
-          else if (e == ~0ULL) {
-            g = ((volatile int*)cx.lc_n)[0];
-            if (g >= GQ_LC_G) { gq_set_err(err, GQ_E_CAPACITY); g = 0; }
-            else {
-              cx.lc_gkey[g] = k; ((volatile int*)cx.lc_n)[0] = g + 1;
-              ((volatile u64*)cx.lc_tab)[i] = ((u64)(u32)k << 32) | (u32)g;
-            }
-          }
-#else
-          const u64 e = ((volatile u64*)cx.lc_tab)[i];
-          if (e == (u64)k) g = (int)((volatile u32*)cx.lc_gid)[i];
-          else if (e == GQ_EMPTY) {
-            g = ((volatile int*)cx.lc_n)[0];
-            if (g >= GQ_LC_G) { gq_set_err(err, GQ_E_CAPACITY); g = 0; }
-            else {
-              cx.lc_gkey[g] = k; ((volatile int*)cx.lc_n)[0] = g + 1;
-              ((volatile u32*)cx.lc_gid)[i] = (u32)g;
-              __threadfence_block();                    // readers match the key first, then read the id
-              ((volatile u64*)cx.lc_tab)[i] = (u64)k;
-            }
-          }
-#endif
-        }
-        if (g < 0) { gq_set_err(err, GQ_E_CAPACITY); g = 0; }   // key table full (more distinct keys than max_groups)
-      }
-      __threadfence_block();
-      atomicExch(&cx.lc_n[1], 0);
-      }
-    }
-    g = __shfl_sync(0xffffffffu, g, 0);
-    }
-    if (need && key == k) { grp = g; need = false; }   // every lane waiting for this key is served at once
+    if (need && key == k) { grp = g; need = false; }
     m = __ballot_sync(0xffffffffu, need);
   }
   return grp;

@@ -30,6 +30,14 @@ __device__ __forceinline__ void gq_process(const GqParams& P, const Src& src, Gq
 
 __device__ __forceinline__ i64 gq_ldcg(const i64* p) { return __ldcg(p); }
 
+// Tuning aid (GQ_TUNE_STAMPS): thread 0 of the LAST CTA records globaltimer values at phase boundaries behind a magic
+// word at the end of the partials scratch, so that the fixed costs of a one-launch pipeline can be read back.
+#if GQ_STAMPS && GQ_FUSED_FINAL
+#define GQ_STAMP(i) do { if (threadIdx.x == 0) { unsigned long long t_; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t_)); gq_stamp[i] = t_; } } while (0)
+#else
+#define GQ_STAMP(i) do { } while (0)
+#endif
+
 #if GQ_FUSED_FINAL
 __device__ __forceinline__ i64 gq_fin_sext(u64 v, int bits) {
   if (bits >= 64) return (i64)v;
@@ -78,6 +86,11 @@ extern "C" __global__ void __launch_bounds__(GQ_NT + 32, 1) gq_scan(const __grid
   u64* full_bar = (u64*)(gq_smem + GQ_BAR_OFF);
   u64* empty_bar = full_bar + GQ_STAGES;
   const int tid = threadIdx.x;
+#if GQ_STAMPS && GQ_FUSED_FINAL
+  unsigned long long gq_stamp[12];
+  for (int i = 0; i < 12; ++i) gq_stamp[i] = 0;
+#endif
+  GQ_STAMP(0);
   const i64 ntiles = P.nrows / GQ_TILE;                  // full tiles; the remainder is the tail
   if (*(volatile int*)P.err != 0) {                      // sticky error: later kernels are no-ops (gq.h "Errors")
 #if GQ_FUSED_FINAL
@@ -100,7 +113,7 @@ extern "C" __global__ void __launch_bounds__(GQ_NT + 32, 1) gq_scan(const __grid
   cx.lc_n = (int*)(gq_smem + GQ_CONS_OFF + GQ_LC_N_OFF);
   cx.lc_acc = (i64*)(gq_smem + GQ_CONS_OFF + GQ_LC_HEAD_BYTES);
   if (tid < GQ_NT) {
-    for (int i = tid; i < GQ_LC_KT; i += GQ_NT) cx.lc_tab[i] = GQ_LC_KEY32 ? ~0ULL : GQ_EMPTY;
+    for (int i = tid; i < GQ_LC_KT; i += GQ_NT) { cx.lc_tab[i] = GQ_LC_KEY32 ? ~0ULL : GQ_EMPTY; cx.lc_gid[i] = 0xFFFFFFFEu; }
     if (tid < 4) cx.lc_n[tid] = 0;
 #pragma unroll
     for (int a = 0; a < GQ_NAGG; ++a)
@@ -138,6 +151,7 @@ extern "C" __global__ void __launch_bounds__(GQ_NT + 32, 1) gq_scan(const __grid
   }
 #endif
   __syncthreads();
+  GQ_STAMP(1);
 
   if (tid >= GQ_NT) {
     // ------------------------------------------------------------------ producer warp: TMA bulk copies
@@ -168,8 +182,10 @@ extern "C" __global__ void __launch_bounds__(GQ_NT + 32, 1) gq_scan(const __grid
       const int s = (int)(it % GQ_STAGES);
       const u32 ph = (u32)((it / GQ_STAGES) & 1);
       gq_mbar_wait(&full_bar[s], ph);                    // the tile's bytes have landed
+      if (it == 0) GQ_STAMP(2);
       src.stage = gq_smem + (size_t)s * GQ_STAGE_BYTES;
       gq_process(P, src, cx, GQ_R, true);
+      if (it == 0) GQ_STAMP(3);
       __syncwarp();
       if ((tid & 31) == 0) gq_mbar_arrive(&empty_bar[s]);  // this warp is done with the stage
     }
@@ -188,6 +204,7 @@ extern "C" __global__ void __launch_bounds__(GQ_NT + 32, 1) gq_scan(const __grid
   }
 
   // -------------------------------------------------------------------- consumer epilogues
+  GQ_STAMP(4);
   const int lane = tid & 31, warp = tid >> 5;
   (void)lane; (void)warp;
 #if GQ_CONSUMER == GQ_C_GLOBAL
@@ -248,7 +265,7 @@ extern "C" __global__ void __launch_bounds__(GQ_NT + 32, 1) gq_scan(const __grid
 #if GQ_CONSUMER == GQ_C_LOWCARD
   {
     gq_consumer_barrier();
-    const int ng = ((volatile int*)cx.lc_n)[0];
+    const int ng = min(((volatile int*)cx.lc_n)[0], GQ_LC_G);   // the counter overshoots when the plan's max_groups is exceeded
 #if !GQ_FUSED_FINAL
     // one warp per (group, aggregate): reduce the GQ_NT private cells, merge into the global table
     for (int p = warp; p < ng * GQ_NAGG; p += GQ_NWARP) {
@@ -277,9 +294,11 @@ extern "C" __global__ void __launch_bounds__(GQ_NT + 32, 1) gq_scan(const __grid
     }
     if (tid == 0) pn[blockIdx.x] = ng;
     gq_consumer_barrier();
+    GQ_STAMP(5);
     if (tid == 0) { __threadfence(); cx.lc_n[3] = (atomicAdd(P.fin.ticket, 1u) == gridDim.x - 1); }
     gq_consumer_barrier();
     if (((volatile int*)cx.lc_n)[3]) {
+      GQ_STAMP(6);
       __threadfence();
 #pragma unroll
       for (int a = 0; a < GQ_NAGG; ++a)
@@ -311,7 +330,8 @@ extern "C" __global__ void __launch_bounds__(GQ_NT + 32, 1) gq_scan(const __grid
         }
       }
       gq_consumer_barrier();
-      const int ng2 = ((volatile int*)cx.lc_n)[0];
+      GQ_STAMP(7);
+      const int ng2 = min(((volatile int*)cx.lc_n)[0], GQ_LC_G);
       for (int p = warp; p < ng2 * GQ_NAGG; p += GQ_NWARP) {
         const i64 v = gq_lc_reduce_pair(cx, p, p % GQ_NAGG, lane);
         if (lane == 0) fin[p] = v;
@@ -321,6 +341,14 @@ extern "C" __global__ void __launch_bounds__(GQ_NT + 32, 1) gq_scan(const __grid
         if (tid < P.fin.out_capacity) gq_fin_emit(P.fin, tid, cx.lc_gkey[tid], fin + tid * GQ_NAGG);
         else gq_set_err(P.err, GQ_E_CAPACITY);
       }
+      GQ_STAMP(8);
+#if GQ_STAMPS
+      if (tid == 0) {
+        unsigned long long* dbg = (unsigned long long*)(pn + gridDim.x + 8);
+        dbg[0] = 0x57414D5053544D50ULL;
+        for (int i = 0; i < 12; ++i) dbg[1 + i] = gq_stamp[i];
+      }
+#endif
       if (tid == 0) { *P.fin.out_n = ng2; *P.fin.ticket = 0; }
     }
 #endif
