@@ -576,21 +576,20 @@ __device__ __forceinline__ int gq_lc_insert_or_find(GqCtx& cx, i64 k, int* err) 
   gq_set_err(err, GQ_E_CAPACITY);                         // key table full
   return 0;
 }
-// Slow path (collision, or first sight of a key): the warp serves its needy lanes one KEY at a time — lane 0 inserts
-// or finds it, every lane waiting for that key takes the answer. Must be called by all 32 lanes (converged).
+// Slow path (collision, or first sight of a key): the needy lanes of the warp are grouped by key (MATCH.ANY); the
+// first lane of every group inserts or finds its key — all groups at once, they touch different table positions —
+// and hands the id to its group. Must be called by all 32 lanes of the warp (converged).
 __device__ __forceinline__ int gq_lc_slow_body(GqCtx& cx, i64 key, bool need, int grp, int* err) {
-  u32 m = __ballot_sync(0xffffffffu, need);
   const int lane = threadIdx.x & 31;
-  while (m) {
-    const int l = __ffs(m) - 1;
-    const i64 k = __shfl_sync(0xffffffffu, key, l);
-    int g = 0;
-    if (lane == 0) g = gq_lc_insert_or_find(cx, k, err);
-    g = __shfl_sync(0xffffffffu, g, 0);
-    if (need && key == k) { grp = g; need = false; }
-    m = __ballot_sync(0xffffffffu, need);
+  const u32 needmask = __ballot_sync(0xffffffffu, need);
+  int src = lane, g = 0;
+  if (need) {
+    const u32 m = __match_any_sync(needmask, key);
+    src = __ffs(m) - 1;
+    if (src == lane) g = gq_lc_insert_or_find(cx, key, err);
   }
-  return grp;
+  g = __shfl_sync(0xffffffffu, g, src);
+  return need ? g : grp;
 }
 // Out of line: the per-row code only carries a call, not four inlined copies of the insert protocol.
 __device__ __noinline__ int gq_lc_slow_call(u64* tab, u32* gid, i64* gkey, int* n, i64 key, bool need, int grp, int* err) {

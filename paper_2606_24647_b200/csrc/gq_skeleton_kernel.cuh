@@ -64,20 +64,30 @@ __device__ __forceinline__ void gq_fin_emit(const GqFinal& F, i64 row, i64 key, 
 #endif
 
 #if GQ_CONSUMER == GQ_C_LOWCARD
-// Reduces the GQ_NT private cells of pair p = group * GQ_NAGG + a over the warp's lanes; every lane gets the result.
-__device__ __forceinline__ i64 gq_lc_reduce_pair(const GqCtx& cx, int p, int a, int lane) {
-  i64 v = 0;
-  const i64* cells = cx.lc_acc + (size_t)p * GQ_NT;
+// Reduces the GQ_NT private cells of up to four pairs p = group * GQ_NAGG + a (p0, p0 + GQ_NWARP, ...) over the warp's
+// lanes, the four chains interleaved (the loads of one pair alone are a dependent LDS/combine chain); every lane gets
+// the results.
+__device__ __forceinline__ void gq_lc_reduce4(const GqCtx& cx, int p0, int np, int lane, i64 (&v)[4]) {
+  int op[4];
+  const i64* cells[4];
 #pragma unroll
-  for (int aa = 0; aa < GQ_NAGG; ++aa) {
-    if (aa == a) {   // the aggregate's op is a compile-time property of aa
-      v = gq_identity(GQ_AGG_OP(aa));
-#pragma unroll 4
-      for (int i = lane; i < GQ_NT; i += 32) v = gq_combine(GQ_AGG_OP(aa), v, cells[i]);
-      v = gq_warp_reduce(GQ_AGG_OP(aa), v);
-    }
+  for (int u = 0; u < 4; ++u) {
+    const int p = p0 + u * GQ_NWARP;
+    const int pc = p < np ? p : p0;
+    op[u] = GQ_AGG_OP(pc % GQ_NAGG);
+    cells[u] = cx.lc_acc + (size_t)pc * GQ_NT;
+    v[u] = gq_identity(op[u]);
   }
-  return v;
+#pragma unroll 2
+  for (int i = lane; i < GQ_NT; i += 32) {
+#pragma unroll
+    for (int u = 0; u < 4; ++u) v[u] = gq_combine(op[u], v[u], cells[u][i]);
+  }
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) {
+#pragma unroll
+    for (int u = 0; u < 4; ++u) v[u] = gq_combine(op[u], v[u], __shfl_xor_sync(0xffffffffu, v[u], o));
+  }
 }
 #endif
 
@@ -236,7 +246,6 @@ extern "C" __global__ void __launch_bounds__(GQ_NT + 32, 1) gq_scan(const __grid
     if (tid == 0) { __threadfence(); flag[0] = (atomicAdd(P.fin.ticket, 1u) == gridDim.x - 1); }
     gq_consumer_barrier();
     if (flag[0]) {
-      __threadfence();
 #pragma unroll
       for (int a = 0; a < GQ_NAGG; ++a) {
         i64 v = gq_identity(GQ_AGG_OP(a));
@@ -268,16 +277,17 @@ extern "C" __global__ void __launch_bounds__(GQ_NT + 32, 1) gq_scan(const __grid
     const int ng = min(((volatile int*)cx.lc_n)[0], GQ_LC_G);   // the counter overshoots when the plan's max_groups is exceeded
 #if !GQ_FUSED_FINAL
     // one warp per (group, aggregate): reduce the GQ_NT private cells, merge into the global table
-    for (int p = warp; p < ng * GQ_NAGG; p += GQ_NWARP) {
-      const int g = p / GQ_NAGG, a = p % GQ_NAGG;
-      const i64 v = gq_lc_reduce_pair(cx, p, a, lane);
-      if (lane == 0) {
-        bool won;
-        u64* slot = gq_ht_upsert<GQ_TARGET_SW>(P.target, cx.lc_gkey[g], &won, P.err);
-        if (slot) {
+    for (int p0 = warp; p0 < ng * GQ_NAGG; p0 += 4 * GQ_NWARP) {
+      i64 v[4];
+      gq_lc_reduce4(cx, p0, ng * GQ_NAGG, lane, v);
 #pragma unroll
-          for (int aa = 0; aa < GQ_NAGG; ++aa)
-            if (aa == a) gq_red(GQ_AGG_OP(aa), slot + 1 + GQ_NDEP + aa, v);
+      for (int u = 0; u < 4; ++u) {
+        const int p = p0 + u * GQ_NWARP;
+        if (lane == 0 && p < ng * GQ_NAGG) {
+          const int g = p / GQ_NAGG, a = p % GQ_NAGG;
+          bool won;
+          u64* slot = gq_ht_upsert<GQ_TARGET_SW>(P.target, cx.lc_gkey[g], &won, P.err);
+          if (slot) gq_red(GQ_AGG_OP(a), slot + 1 + GQ_NDEP + a, v[u]);
         }
       }
     }
@@ -287,10 +297,18 @@ extern "C" __global__ void __launch_bounds__(GQ_NT + 32, 1) gq_scan(const __grid
     i64* mypart = P.fin.part + (i64)blockIdx.x * GQ_LC_G * PW;
     i64* pn = P.fin.part + (i64)gridDim.x * GQ_LC_G * PW;
     i64* fin = (i64*)(gq_smem + GQ_CONS_OFF + GQ_LC_FIN_OFF);
-    for (int p = warp; p < ng * GQ_NAGG; p += GQ_NWARP) {
-      const int g = p / GQ_NAGG, a = p % GQ_NAGG;
-      const i64 v = gq_lc_reduce_pair(cx, p, a, lane);
-      if (lane == 0) { mypart[g * PW + 1 + a] = v; if (a == 0) mypart[g * PW] = cx.lc_gkey[g]; }
+    for (int p0 = warp; p0 < ng * GQ_NAGG; p0 += 4 * GQ_NWARP) {
+      i64 v[4];
+      gq_lc_reduce4(cx, p0, ng * GQ_NAGG, lane, v);
+#pragma unroll
+      for (int u = 0; u < 4; ++u) {
+        const int p = p0 + u * GQ_NWARP;
+        if (lane == 0 && p < ng * GQ_NAGG) {
+          const int g = p / GQ_NAGG, a = p % GQ_NAGG;
+          mypart[g * PW + 1 + a] = v[u];
+          if (a == 0) mypart[g * PW] = cx.lc_gkey[g];
+        }
+      }
     }
     if (tid == 0) pn[blockIdx.x] = ng;
     gq_consumer_barrier();
@@ -299,7 +317,7 @@ extern "C" __global__ void __launch_bounds__(GQ_NT + 32, 1) gq_scan(const __grid
     gq_consumer_barrier();
     if (((volatile int*)cx.lc_n)[3]) {
       GQ_STAMP(6);
-      __threadfence();
+      // (writers fenced before taking their ticket; the partials are read with ld.cg after the CTA barrier above)
 #pragma unroll
       for (int a = 0; a < GQ_NAGG; ++a)
         for (int g = 0; g < GQ_LC_G; ++g) cx.lc_acc[(g * GQ_NAGG + a) * GQ_NT + tid] = gq_identity(GQ_AGG_OP(a));
@@ -332,9 +350,12 @@ extern "C" __global__ void __launch_bounds__(GQ_NT + 32, 1) gq_scan(const __grid
       gq_consumer_barrier();
       GQ_STAMP(7);
       const int ng2 = min(((volatile int*)cx.lc_n)[0], GQ_LC_G);
-      for (int p = warp; p < ng2 * GQ_NAGG; p += GQ_NWARP) {
-        const i64 v = gq_lc_reduce_pair(cx, p, p % GQ_NAGG, lane);
-        if (lane == 0) fin[p] = v;
+      for (int p0 = warp; p0 < ng2 * GQ_NAGG; p0 += 4 * GQ_NWARP) {
+        i64 v[4];
+        gq_lc_reduce4(cx, p0, ng2 * GQ_NAGG, lane, v);
+#pragma unroll
+        for (int u = 0; u < 4; ++u)
+          if (lane == 0 && p0 + u * GQ_NWARP < ng2 * GQ_NAGG) fin[p0 + u * GQ_NWARP] = v[u];
       }
       gq_consumer_barrier();
       if (tid < ng2) {
