@@ -108,8 +108,9 @@ typedef struct {
   const int32_t* payload_cols; int32_t npayload; /* stored beside the key, handed to probers */
   uint32_t flags;                                /* GQ_F_UNIQUE_KEYS */
 } gq_build_desc;
-/* Open addressing, linear probing, 64-bit CAS; capacity = max_build_rows / 0.65 slots rounded up to a multiple of
- * 1024 (not to a power of two: slot = multiply-shift range reduction of the hash), read in 32-byte buckets. */
+/* Open addressing, linear probing, 64-bit CAS; capacity = max_build_rows / load slots rounded up to a multiple of
+ * 1024 (not to a power of two: slot = multiply-shift range reduction of the hash), load = 0.4 for tables that fit L2 and
+ * 0.7 for larger ones; read in 32-byte (key-only) or 64-byte (key + payload) buckets. */
 gq_status gq_hash_build_workspace(int64_t max_build_rows, int32_t npayload, size_t* bytes);
 /* *table == NULL: creates the table in d_workspace (enqueues its initialisation) and inserts the batch.
  * *table != NULL: inserts a further batch (same schema and desc; d_workspace/bytes/max_build_rows ignored). */

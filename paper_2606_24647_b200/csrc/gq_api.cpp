@@ -29,12 +29,14 @@ int64_t table_capacity(int64_t max_rows) {   // power of two >= max_rows * 4/3, 
   while (c < need) c <<= 1;
   return c;
 }
-// Join tables: max_rows / 0.65 slots rounded up to a multiple of 1024 — NOT to a power of two: the slot index comes
-// from a multiply-shift range reduction, so the table (and a direct-aggregation array indexed by its slots) is as
-// small as the hint allows and has the best chance of staying L2-resident.
-int64_t join_capacity(int64_t max_rows) {
-  int load = 50;                                       // percent; GQ_TUNE_JOIN_LOAD overrides (tuning sweeps only)
-  if (const char* e = getenv("GQ_TUNE_JOIN_LOAD")) { int v = atoi(e); if (v >= 10 && v <= 90) load = v; }
+// Join tables: capacity = max_rows / load rounded up to a multiple of 1024 — NOT to a power of two: the slot index
+// comes from a multiply-shift range reduction, so the table (and a direct-aggregation array indexed by its slots) is
+// as small as the hint allows. Load factor (measured, C3/C4 sweeps 0.3-0.75): a table that fits L2 even at load 0.4
+// takes 0.4 — its probes are latency-bound and sparse buckets save dependent rounds (C4 1.06 -> 0.98 ms); a larger
+// one is bound by random DRAM sectors and takes 0.7 to shrink its footprint (C3 1.77 -> 1.60 ms).
+int64_t join_capacity(int64_t max_rows, int slot_words = 1) {
+  int load = (max_rows * slot_words * 8 * 10 / 4 <= (80LL << 20)) ? 40 : 70;
+  if (const char* e = getenv("GQ_TUNE_JOIN_LOAD")) { int v = atoi(e); if (v >= 10 && v <= 90) load = v; }   // tuning sweeps only
   int64_t need = std::max<int64_t>(1024, (max_rows * 100 + load - 1) / load);
   return (need + 1023) / 1024 * 1024;
 }
@@ -326,7 +328,7 @@ gq_status gq_hash_probe(gq_ctx* ctx, const gq_batch* probe, const gq_pred* preds
 // ------------------------------------------------------------------------------------------------ HashBuild
 gq_status gq_hash_build_workspace(int64_t max_build_rows, int32_t npayload, size_t* bytes) {
   if (!bytes || max_build_rows < 0 || npayload < 0 || npayload > GQ_MAX_PAYLOAD) return GQ_ERR_INVALID_ARG;
-  *bytes = ws_layout(join_capacity(max_build_rows), join_slot_words(npayload), GQ_SIDE_SLOTS).total;
+  *bytes = ws_layout(join_capacity(max_build_rows, join_slot_words(npayload)), join_slot_words(npayload), GQ_SIDE_SLOTS).total;
   return GQ_OK;
 }
 
@@ -357,8 +359,8 @@ gq_status gq_hash_build(gq_ctx* ctx, gq_table** table, void* d_ws, size_t bytes,
   gq_table* t = *table;
   if (!t) {
     if (!d_ws || !aligned(d_ws, 256) || max_build_rows < 0) return fail(ctx, GQ_ERR_INVALID_ARG, "bad workspace");
-    const int64_t cap = join_capacity(max_build_rows);
     const int sw = sp.target_sw;
+    const int64_t cap = join_capacity(max_build_rows, sw);
     WsLayout w = ws_layout(cap, sw, GQ_SIDE_SLOTS);
     if (bytes < w.total) return fail(ctx, GQ_ERR_WORKSPACE_TOO_SMALL, "hash-build workspace too small");
     t = new gq_table();
@@ -374,7 +376,7 @@ gq_status gq_hash_build(gq_ctx* ctx, gq_table** table, void* d_ws, size_t bytes,
     t->dev.shift = 64 - log2i(cap);
     t->dev.slot_words = sw;
     t->dev.flags = d->flags;
-    t->dev.bshift = (sw == 1 ? 2 : sw == 2 ? 1 : 0);   // slots per 32-byte bucket: 4 / 2 / 1
+    t->dev.bshift = (sw == 1 ? 2 : sw == 2 ? 2 : 0);   // slots per 32-byte bucket: 4 / 2 / 1
     unsigned long long pat[12];
     for (int i = 0; i < 12; ++i) pat[i] = 0;
     pat[0] = GQ_EMPTY_KEY;

@@ -186,6 +186,15 @@ __device__ __forceinline__ void gq_ld256_relaxed(const u64* p, u64 (&w)[4]) {   
   asm volatile("ld.relaxed.gpu.global.v2.u64 {%0, %1}, [%2];" : "=l"(w[2]), "=l"(w[3]) : "l"(p + 2) : "memory");
 }
 
+template <int NW> __device__ __forceinline__ void gq_ld_bucket(const u64* p, u64 (&w)[NW]) {
+  gq_ld256(p, *(u64(*)[4])&w[0]);
+  if (NW == 8) gq_ld256(p + 4, *(u64(*)[4])&w[NW - 4]);
+}
+template <int NW> __device__ __forceinline__ void gq_ld_bucket_relaxed(const u64* p, u64 (&w)[NW]) {
+  gq_ld256_relaxed(p, *(u64(*)[4])&w[0]);
+  if (NW == 8) gq_ld256_relaxed(p + 4, *(u64(*)[4])&w[NW - 4]);
+}
+
 // HashBuild insert of one row: duplicates are kept as separate slots (multiset, S3) unless `unique`
 // is asserted, in which case an equal key sets the sticky GQ_E_DUPLICATE. Payload words are written by the CAS
 // winner; probes only run after the building kernel has finished (pipeline boundary), so no reader can
@@ -252,8 +261,9 @@ __device__ __forceinline__ u64* gq_ht_upsert(const GqTableDev& T, i64 key, bool*
 template <int SW, int NPAY>
 __device__ __forceinline__ void gq_probe_rows(const GqTableDev& T, const i64 (&key)[GQ_R], bool (&live)[GQ_R],
                                               u64 (&idx)[GQ_R], i64 (&pay)[GQ_R][NPAY > 0 ? NPAY : 1]) {
-  constexpr int B = SW == 1 ? 4 : SW == 2 ? 2 : 1;   // slots per 32-byte bucket
-  u64 w[GQ_R][4];
+  constexpr int B = SW == 1 ? 4 : SW == 2 ? 4 : 1;   // slots per bucket: 32 bytes, or 64 bytes for key+payload slots
+  constexpr int NW = B * SW;                         // words per bucket fetch (4 or 8: one or two LDG.256)
+  u64 w[GQ_R][NW];
   u32 pend = 0;
 #pragma unroll
   for (int j = 0; j < GQ_R; ++j) {
@@ -267,7 +277,7 @@ __device__ __forceinline__ void gq_probe_rows(const GqTableDev& T, const i64 (&k
         } else live[j] = false;
       } else {
         idx[j] = gq_slot0(T, key[j]);
-        gq_ld256(T.slots + idx[j] * SW, w[j]);
+        gq_ld_bucket<NW>(T.slots + idx[j] * SW, w[j]);
         pend |= 1u << j;
       }
     }
@@ -291,7 +301,7 @@ __device__ __forceinline__ void gq_probe_rows(const GqTableDev& T, const i64 (&k
         if (done) pend &= ~(1u << j);
         else {
           idx[j] = gq_next(T, idx[j], B);
-          gq_ld256(T.slots + idx[j] * SW, w[j]);
+          gq_ld_bucket<NW>(T.slots + idx[j] * SW, w[j]);
         }
       }
     }
@@ -302,8 +312,9 @@ __device__ __forceinline__ void gq_probe_rows(const GqTableDev& T, const i64 (&k
 template <int SW, int NPAY>
 __device__ __forceinline__ int gq_insert_rows(const GqTableDev& T, const i64 (&key)[GQ_R], const bool (&live)[GQ_R],
                                               const i64 (&pay)[GQ_R][NPAY > 0 ? NPAY : 1], bool unique, int* err) {
-  constexpr int B = SW == 1 ? 4 : SW == 2 ? 2 : 1;
-  u64 w[GQ_R][4];
+  constexpr int B = SW == 1 ? 4 : SW == 2 ? 4 : 1;
+  constexpr int NW = B * SW;
+  u64 w[GQ_R][NW];
   u64 idx[GQ_R];
   u32 pend = 0;
   int ninserted = 0;
@@ -314,7 +325,7 @@ __device__ __forceinline__ int gq_insert_rows(const GqTableDev& T, const i64 (&k
       if ((u64)key[j] == GQ_EMPTY) { if (gq_ht_insert<SW, NPAY>(T, key[j], pay[j], unique, err)) ++ninserted; }
       else {
         idx[j] = gq_slot0(T, key[j]);
-        gq_ld256_relaxed(T.slots + idx[j] * SW, w[j]);
+        gq_ld_bucket_relaxed<NW>(T.slots + idx[j] * SW, w[j]);
         pend |= 1u << j;
       }
     }
@@ -347,7 +358,7 @@ __device__ __forceinline__ int gq_insert_rows(const GqTableDev& T, const i64 (&k
         } else if (round > 2 * (T.mask + 1)) { gq_set_err(err, GQ_E_CAPACITY); pend &= ~(1u << j); }
         else {
           idx[j] = gq_next(T, idx[j], B);
-          gq_ld256_relaxed(T.slots + idx[j] * SW, w[j]);
+          gq_ld_bucket_relaxed<NW>(T.slots + idx[j] * SW, w[j]);
         }
       }
     }
