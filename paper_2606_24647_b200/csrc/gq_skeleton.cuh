@@ -286,18 +286,27 @@ __device__ __forceinline__ void gq_probe_rows(const GqTableDev& T, const i64 (&k
 #pragma unroll
     for (int j = 0; j < GQ_R; ++j) {
       if (pend & (1u << j)) {
-        bool done = false;
+        // slots of a bucket fill in order, so a match can never sit behind an EMPTY slot: look for the key in all B
+        // slots first, and only without a match ask whether the bucket has a free slot (= the key is absent)
+        int hb = -1;
+        bool emp = false;
 #pragma unroll
         for (int b = 0; b < B; ++b) {
           const u64 kw = w[j][b * SW];
-          if (!done && kw == (u64)key[j]) {
-            done = true;
-            idx[j] += b;
-#pragma unroll
-            for (int p = 0; p < NPAY; ++p) pay[j][p] = (i64)w[j][b * SW + 1 + p];
-          } else if (!done && kw == GQ_EMPTY) { done = true; live[j] = false; }
+          if (kw == (u64)key[j]) hb = b;
+          emp = emp || kw == GQ_EMPTY;
         }
-        if (!done && round * B > T.mask) { done = true; live[j] = false; }   // full table without the key
+        bool done = true;
+        if (hb >= 0) {
+          idx[j] += hb;
+#pragma unroll
+          for (int b = 0; b < B; ++b)
+            if (b == hb) {
+#pragma unroll
+              for (int p = 0; p < NPAY; ++p) pay[j][p] = (i64)w[j][b * SW + 1 + p];
+            }
+        } else if (emp || round * B > T.mask) live[j] = false;   // free slot seen, or a full table without the key
+        else done = false;
         if (done) pend &= ~(1u << j);
         else {
           idx[j] = gq_next(T, idx[j], B);
