@@ -347,13 +347,11 @@ __device__ __forceinline__ u64 gq_p_ld_relaxed(const u64* p) {
 // of 26 GB of DRAM reads) but takes 173 ms, because a partition's most frequent key then serialises its same-address
 // REDs at L2 with nothing else to overlap (barrier every 16 / 64 / 256 partitions: 96 / 71 / 56 ms); combining equal
 // keys of a warp in registers before touching the table costs more issue slots than the REDs it saves (78 ms).
-#define GQ_PART_GROUPS 1
 __global__ void __launch_bounds__(GQ_PART_THREADS) gq_k_part_upsert(const __grid_constant__ GqPartParams P) {
   if (*(volatile int*)P.err != 0) return;
   const u64 cap = P.mask + 1;
-  const int group = blockIdx.x % GQ_PART_GROUPS, rank = blockIdx.x / GQ_PART_GROUPS;
-  const int nrank = (gridDim.x - group + GQ_PART_GROUPS - 1) / GQ_PART_GROUPS;   // CTAs of this group
-  for (int p = group; p < P.npart; p += GQ_PART_GROUPS) {
+  const int rank = blockIdx.x, nrank = gridDim.x;
+  for (int p = 0; p < P.npart; ++p) {
     i64 n = (i64)P.pcur[(i64)p * GQ_PART_CURSOR_STRIDE];
     if (n > P.pcap) n = P.pcap;
     const u64* base = P.part + (u64)p * (u64)P.pcap * P.rw;
