@@ -41,6 +41,9 @@ int64_t join_capacity(int64_t max_rows, int slot_words = 1) {
   return (need + 1023) / 1024 * 1024;
 }
 int join_slot_words(int npayload) { return npayload == 0 ? 1 : (int)align_up((size_t)(1 + npayload), 2); }
+// Group-by slot = key + dependent word + aggregates, padded to an even word count (16-byte multiple). Padding to a
+// power of two (64-byte slots for C5, never straddling a DRAM burst) was measured: radix-clustered 35.3 -> 34.3 ms but
+// single-pass 47.9 -> 49.9 ms and a 3.2 -> 4.3 GB table; not adopted.
 int agg_slot_words(int ndep, int naggs) { return (int)align_up((size_t)(1 + ndep + naggs), 2); }
 int log2i(int64_t v) { int l = 0; while ((1LL << l) < v) ++l; return l; }
 
@@ -377,8 +380,8 @@ gq_status gq_hash_build(gq_ctx* ctx, gq_table** table, void* d_ws, size_t bytes,
     t->dev.slot_words = sw;
     t->dev.flags = d->flags;
     t->dev.bshift = (sw == 1 ? 2 : sw == 2 ? 2 : 0);   // slots per 32-byte bucket: 4 / 2 / 1
-    unsigned long long pat[12];
-    for (int i = 0; i < 12; ++i) pat[i] = 0;
+    unsigned long long pat[16];
+    for (int i = 0; i < 16; ++i) pat[i] = 0;
     pat[0] = GQ_EMPTY_KEY;
     cudaError_t e = gq_launch_init_table(ctx->stream, t->dev.slots, cap, sw, pat, t->dev.side, GQ_SIDE_SLOTS, t->dev.header, 0);
     if (e != cudaSuccess) { delete t; return cuda_fail(ctx, e, "table init"); }
@@ -607,8 +610,8 @@ gq_status gq_hash_aggregate(gq_ctx* ctx, gq_aggstate** state, void* d_ws, size_t
     a->nkeys = d->nkeys; a->ndep = d->ndependent; a->naggs = d->naggs; a->max_groups = d->max_groups;
     for (int k = 0; k < d->nkeys; ++k) { a->key_dtype[k] = key_dtype[k]; a->key_bits[k] = key_bits[k]; }
     for (int i = 0; i < d->naggs; ++i) a->agg_op[i] = d->aggs[i].op;
-    unsigned long long pat[12];
-    for (int i = 0; i < 12; ++i) pat[i] = 0;
+    unsigned long long pat[16];
+    for (int i = 0; i < 16; ++i) pat[i] = 0;
     cudaError_t e;
     if (dp.step >= 0) {
       a->direct = true; a->dtab = d->probes[dp.step].table->dev; a->dcap = dp.cap; a->daw = dp.aw; a->dtouch = dp.touch;

@@ -11,8 +11,9 @@ typedef long long i64;
 // size allows; zeroes the header (header[1] = header1) and marks side slots empty.
 __global__ void gq_k_init_table(u64* slots, i64 nwords, int sw, const __grid_constant__ ulonglong4 pat0,
                                 const __grid_constant__ ulonglong4 pat1, const __grid_constant__ ulonglong4 pat2,
-                                u64* side, i64 nside_words, i64* header, i64 header1) {
-  const u64 pat[12] = {pat0.x, pat0.y, pat0.z, pat0.w, pat1.x, pat1.y, pat1.z, pat1.w, pat2.x, pat2.y, pat2.z, pat2.w};
+                                const __grid_constant__ ulonglong4 pat3, u64* side, i64 nside_words, i64* header, i64 header1) {
+  const u64 pat[16] = {pat0.x, pat0.y, pat0.z, pat0.w, pat1.x, pat1.y, pat1.z, pat1.w,
+                       pat2.x, pat2.y, pat2.z, pat2.w, pat3.x, pat3.y, pat3.z, pat3.w};
   const i64 stride = (i64)gridDim.x * blockDim.x;
   const i64 t0 = (i64)blockIdx.x * blockDim.x + threadIdx.x;
   // slot sizes are multiples of 2 words (or 1 word: key-only tables) -> pairs of words never straddle the pattern oddly
@@ -33,13 +34,13 @@ __global__ void gq_k_init_table(u64* slots, i64 nwords, int sw, const __grid_con
 
 cudaError_t gq_launch_init_table(cudaStream_t s, u64* slots, i64 nslots, int sw, const u64* pattern, u64* side,
                                  i64 nside, i64* header, i64 header1) {
-  ulonglong4 p[3];
+  ulonglong4 p[4];
   u64* pp = (u64*)p;
-  for (int i = 0; i < 12; ++i) pp[i] = pattern[i % sw];
+  for (int i = 0; i < 16; ++i) pp[i] = pattern[i % sw];
   i64 nwords = nslots * sw;
   i64 work = (sw & 1) == 0 ? nwords / 2 : nwords;
   int blocks = (int)std::min<i64>(148 * 16, std::max<i64>(1, (work + 255) / 256));
-  gq_k_init_table<<<blocks, 256, 0, s>>>(slots, nwords, sw, p[0], p[1], p[2], side, nside * sw, header, header1);
+  gq_k_init_table<<<blocks, 256, 0, s>>>(slots, nwords, sw, p[0], p[1], p[2], p[3], side, nside * sw, header, header1);
   return cudaGetLastError();
 }
 
@@ -528,8 +529,8 @@ __global__ void gq_k_hot_select(const u64* table, i64 nslots, u64 threshold, i64
 cudaError_t gq_launch_hot_keys(cudaStream_t s, const void* keycol, int dtype, i64 nrows, u64* table, i64 nslots,
                                i64 nsample, u64 threshold, i64* hot, int max_hot, int* nlaunches) {
   // (key,count) slots: key = EMPTY (0x80..0), count = 0
-  u64 pat[12];
-  for (int i = 0; i < 12; ++i) pat[i] = (i & 1) ? 0 : GQ_EMPTY_KEY;
+  u64 pat[16];
+  for (int i = 0; i < 16; ++i) pat[i] = (i & 1) ? 0 : GQ_EMPTY_KEY;
   cudaError_t e = gq_launch_init_table(s, table, nslots, 2, pat, table, 0, hot, 0);   // header := hot list head (zeroed)
   if (e != cudaSuccess) return e;
   int shift = 64;
