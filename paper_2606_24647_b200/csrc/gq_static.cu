@@ -1,6 +1,8 @@
 // gq_static.cu — plan-independent sm_100a kernels, compiled by nvcc into libgq.so: hash-table initialisation, the
 // HashAggregation finaliser (table -> dense output columns + device-side group count + derived AVG),
 // the top-k finaliser (OrderBy/TopN in its smallest form) and the read-roofline probe.
+#include <cstdlib>
+
 #include "gq_internal.h"
 
 typedef unsigned long long u64;
@@ -413,7 +415,9 @@ __global__ void __launch_bounds__(GQ_PART_THREADS) gq_k_part_upsert(const __grid
   }
 }
 cudaError_t gq_launch_part_upsert(cudaStream_t s, const GqPartParams& p, int num_sms) {
-  gq_k_part_upsert<<<num_sms * 2, GQ_PART_THREADS, 0, s>>>(p);
+  int per_sm = 2;
+  if (const char* e = getenv("GQ_TUNE_PART_CTAS_PER_SM")) { int v = atoi(e); if (v >= 1 && v <= 4) per_sm = v; }   // tuning sweeps only
+  gq_k_part_upsert<<<num_sms * per_sm, GQ_PART_THREADS, 0, s>>>(p);
   return cudaGetLastError();
 }
 
