@@ -556,7 +556,7 @@ PartPlan part_plan(const GqScanSpec& sp, const gq_agg_desc* d, int64_t nrows) {
     pp.src[a] = 1 + d->ndependent + (int)i;
   }
   pp.rw = (int)align_up((size_t)(1 + d->ndependent + pp.exprs.size()), 4);
-  pp.pcap = nrows / np + nrows / (4 * np) + 1024;
+  pp.pcap = (nrows / np + nrows / (4 * np) + 1024 + GQ_PART_CHUNK - 1) / GQ_PART_CHUNK * GQ_PART_CHUNK;   // whole chunks
   pp.bytes = align_up((size_t)np * 8 * GQ_PART_CURSOR_STRIDE, 256) + (size_t)np * (size_t)pp.pcap * pp.rw * 8;
   pp.on = true;
   return pp;
@@ -693,7 +693,7 @@ gq_status gq_hash_aggregate(gq_ctx* ctx, gq_aggstate** state, void* d_ws, size_t
     PartPlan pp = part_plan(sp, d, a->part_rows);
     if (!pp.on || pp.rw != a->part_rw || pp.npart != a->npart) return fail(ctx, GQ_ERR_INVALID_ARG, "batch schema/desc differs from the state's first batch");
     sp.consumer = GQ_C_PARTITION; sp.part_rw = pp.rw; sp.part_exprs = pp.exprs;
-    P.part = a->part; P.pcur = a->pcur; P.pcap = a->pcap; P.pshift = a->pshift;
+    P.part = a->part; P.pcur = a->pcur; P.pcap = a->pcap; P.pshift = a->pshift; P.npart = a->npart;
     cudaError_t e = cudaMemsetAsync(a->pcur, 0, (size_t)a->npart * 8 * GQ_PART_CURSOR_STRIDE, ctx->stream);
     if (e != cudaSuccess) return cuda_fail(ctx, e, "partition cursors");
     gq_status st2 = run_scan(ctx, sp, in, d->probes, &P);

@@ -192,6 +192,21 @@ static gq_status emit_linear(Gen& g, const GqScanSpec& sp, std::ostringstream& o
     o << "  i64 " << nm << "[GQ_R];\n  " << LOOP << nm << "[j] = " << g.val(c) << ";\n";
     return nm;
   };
+  // ---- projection, emitted after the probe steps ----
+  bool projected = false;
+  auto emit_projection = [&]() -> bool {
+    projected = true;
+    if (sp.exprs.empty()) return true;
+    for (size_t e = 0; e < sp.exprs.size(); ++e) o << "  i64 e" << e << "[GQ_R];\n";
+    o << "  " << LOOP << (dense ? "" : "if (live[j]) ") << "{\n";
+    for (size_t e = 0; e < sp.exprs.size(); ++e) {
+      std::string x;
+      if (!g.expr(sp.exprs[e], &x)) return false;
+      o << "    e" << e << "[j] = " << x << ";\n";
+    }
+    o << "  }\n";
+    return true;
+  };
   // ---- probe steps ----
   for (int s = 0; s < nprobe; ++s) {
     const GqProbeSpec& ps = sp.probes[(size_t)s];
@@ -202,17 +217,7 @@ static gq_status emit_linear(Gen& g, const GqScanSpec& sp, std::ostringstream& o
       << ", py" << S << ");\n";
     o << "  (void)pi" << S << "; (void)py" << S << ";\n";
   }
-  // ---- projection ----
-  if (!sp.exprs.empty()) {
-    for (size_t e = 0; e < sp.exprs.size(); ++e) o << "  i64 e" << e << "[GQ_R];\n";
-    o << "  " << LOOP << (dense ? "" : "if (live[j]) ") << "{\n";
-    for (size_t e = 0; e < sp.exprs.size(); ++e) {
-      std::string x;
-      if (!g.expr(sp.exprs[e], &x)) return GQ_ERR_INVALID_ARG;
-      o << "    e" << e << "[j] = " << x << ";\n";
-    }
-    o << "  }\n";
-  }
+  if (!projected && !emit_projection()) return GQ_ERR_INVALID_ARG;
   std::string keyx, depx;
   if (sp.consumer == GQ_C_LOWCARD || sp.consumer == GQ_C_HIGHCARD || sp.consumer == GQ_C_PARTITION) {
     gq_status st = key_exprs(g, sp, &keyx, &depx, msg);
@@ -257,8 +262,8 @@ static gq_status emit_linear(Gen& g, const GqScanSpec& sp, std::ostringstream& o
         const int rw = sp.part_rw;
         o << "  u64 pidx[GQ_R], ppart[GQ_R];\n";
         o << "  " << LOOP << "{\n    pidx[j] = ~0ULL; ppart[j] = 0;\n    if (live[j] && (u64)tkey[j] != GQ_EMPTY) {\n"
-          << "      ppart[j] = gq_slot0(P.target, tkey[j]) >> P.pshift;\n      pidx[j] = atomicAdd(P.pcur + ppart[j] * 16, 1ULL);\n    }\n  }\n";
-        o << "  " << LOOP << "if (live[j] && pidx[j] < (u64)P.pcap) {\n    u64* rec = P.part + (ppart[j] * (u64)P.pcap + pidx[j]) * " << rw << ";\n";
+          << "      ppart[j] = gq_slot0(P.target, tkey[j]) >> P.pshift;\n      pidx[j] = (u64)gq_part_reserve(P, cx.part_st, ppart[j]);\n    }\n  }\n";
+        o << "  " << LOOP << "if (live[j] && pidx[j] != ~0ULL) {\n    u64* rec = P.part + (ppart[j] * (u64)P.pcap + pidx[j]) * " << rw << ";\n";
         std::vector<std::string> words;
         words.push_back("(u64)tkey[j]");
         if (sp.ndep == 1) words.push_back("(u64)" + depx);
@@ -379,6 +384,8 @@ gq_status gq_codegen(const GqScanSpec& sp, GqKernelInfo* out, std::string* msg) 
   for (const GqProbeSpec& ps : sp.probes) all_unique = all_unique && ps.unique;
   const bool use_hot = sp.hot && (sp.consumer == GQ_C_HIGHCARD || sp.consumer == GQ_C_PARTITION) && all_unique;   // linear mode only
   if (use_hot) cons_bytes = 512 * 8 + 512LL * nagg * 8 + 512 * 4 + 256;
+  long long part_state_off = 0;
+  if (sp.part_rw > 0) { part_state_off = (cons_bytes + 127) / 128 * 128; cons_bytes = part_state_off + 4096 * 4; }   // <= 4096 partitions
   int r = tablebound ? 4 : 2, stages = 0;
   // small inputs: smaller tiles so that every SM still gets several tiles
   if (sp.nrows_hint > 0 && sp.nrows_hint < 148LL * 8 * nt * 2) r = 1;
@@ -404,7 +411,7 @@ gq_status gq_codegen(const GqScanSpec& sp, GqKernelInfo* out, std::string* msg) 
   o << "#define GQ_NAGG " << nagg << "\n#define GQ_LC_G " << (sp.lc_cap > 0 ? sp.lc_cap : 1) << "\n#define GQ_LC_KT " << lc_kt
     << "\n#define GQ_LC_KEY32 " << lc_key32 << "\n#define GQ_TARGET_SW "
     << (sp.target_sw > 0 ? sp.target_sw : 1) << "\n#define GQ_NDEP " << sp.ndep << "\n#define GQ_EVICT_FIRST " << (getenv("GQ_TUNE_NO_EVICT_FIRST") ? 0 : 1) << "\n#define GQ_HOT " << (use_hot ? 1 : 0)
-    << "\n#define GQ_STAMPS " << (getenv("GQ_TUNE_STAMPS") ? 1 : 0) << "\n#define GQ_FUSED_FINAL " << (sp.fused_final ? 1 : 0) << "\n#define GQ_DIRECT_AW " << (sp.direct_aw > 0 ? sp.direct_aw : 1) << "\n";
+    << "\n#define GQ_PART_RW " << sp.part_rw << "\n#define GQ_PART_STATE_OFF " << part_state_off << "\n#define GQ_STAMPS " << (getenv("GQ_TUNE_STAMPS") ? 1 : 0) << "\n#define GQ_FUSED_FINAL " << (sp.fused_final ? 1 : 0) << "\n#define GQ_DIRECT_AW " << (sp.direct_aw > 0 ? sp.direct_aw : 1) << "\n";
   {
     long long off = 0, tx = 0;
     std::ostringstream offs, bytes;

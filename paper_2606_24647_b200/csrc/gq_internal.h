@@ -58,6 +58,7 @@ struct GqParams {
   unsigned long long* pcur;    // PARTITION: append cursors
   long long pcap;
   long long pshift;
+  long long npart;
   GqFinal fin;
 };
 
@@ -184,6 +185,7 @@ cudaError_t gq_launch_init_table(cudaStream_t s, unsigned long long* slots, long
 cudaError_t gq_launch_finalise(cudaStream_t s, const GqFinaliseParams& p, int num_sms, int* nlaunches);
 cudaError_t gq_launch_read_probe(cudaStream_t s, const void* data, size_t bytes, unsigned long long* out, int num_sms);
 cudaError_t gq_launch_random_probe(cudaStream_t s, void* table, size_t bytes, long long n, int mode, unsigned long long* out, int num_sms);
+#define GQ_PART_CHUNK 32            // records per CTA-private append chunk (cursors count chunks)
 #define GQ_PART_CURSOR_STRIDE 16   // one append cursor per 128-byte line: atomics to one line serialise at L2
 struct GqPartParams {
   const unsigned long long* part; const unsigned long long* pcur; long long pcap; int npart; int rw;

@@ -95,6 +95,7 @@ struct GqParams {
   u64* pcur;                    // PARTITION: per-partition append cursors
   i64 pcap;                     // PARTITION: records per partition
   i64 pshift;                   // PARTITION: partition = first slot of the key in the target table >> pshift
+  i64 npart;                    // number of partitions
   GqFinal fin;                  // GQ_FUSED_FINAL: outputs of the in-kernel finaliser
 };
 
@@ -443,6 +444,36 @@ __device__ __forceinline__ void gq_st256(u64* p, u64 a, u64 b, u64 c, u64 d) {
   asm volatile("st.global.v4.u64 [%0], {%1, %2, %3, %4};" ::"l"(p), "l"(a), "l"(b), "l"(c), "l"(d) : "memory");
 }
 
+// Appending is done in CTA-private chunks of GQ_PART_CHUNK records: a shared-memory counter hands out the slots of the
+// CTA's open chunk of a partition (ATOMS), and only the thread that finds the chunk exhausted draws the next chunk from
+// the partition's global cursor — one global atomic per 32 records instead of one per record (a returned global
+// atomic per row caps the scan at ~35 G rows/s). Unused slots of the last chunks are padded with EMPTY-key records at
+// the end of the kernel; pass B skips them. Returns the record index inside the partition buffer, or -1 when the
+// partition's buffer is full (the caller then processes the row in place).
+#define GQ_PART_CHUNK 32u
+__device__ __forceinline__ i64 gq_part_reserve(const GqParams& P, u32* st, u64 p) {
+  for (;;) {
+    const u32 v0 = ((volatile u32*)st)[p];
+    if ((v0 & 0xFFFFu) > GQ_PART_CHUNK) {                 // being refilled by another thread, or full
+      if ((v0 >> 16) == 0xFFFFu) return -1;
+      continue;
+    }
+    const u32 v = atomicAdd(&st[p], 1u);
+    const u32 used = v & 0xFFFFu;
+    if (used < GQ_PART_CHUNK) return (i64)(v >> 16) * GQ_PART_CHUNK + used;
+    if (used == GQ_PART_CHUNK) {                          // this thread opens the next chunk and takes its first slot
+      const u64 c = atomicAdd(P.pcur + p * 16, 1ULL);
+      if (c >= (u64)P.pcap / GQ_PART_CHUNK || c >= 0xFFFFull) {
+        ((volatile u32*)st)[p] = 0xFFFF0000u | (GQ_PART_CHUNK + 1u);
+        return -1;
+      }
+      __threadfence_block();
+      ((volatile u32*)st)[p] = ((u32)c << 16) | 1u;
+      return (i64)c * GQ_PART_CHUNK;
+    }
+  }
+}
+
 // ---------------------------------------------------------------------------------------------- row sources
 // A tile staged in shared memory by the producer, or the ragged tail read from global memory.
 struct GqSrcSmem {
@@ -470,6 +501,7 @@ struct GqCtx {
   i64* lc_gkey;                         //   key of every group id [GQ_LC_G]
   int* lc_n;                            //   [0] groups so far, [1] insert lock, [2] gid of the reserved-pattern key + 1
   i64* lc_acc;                          //   accumulators [GQ_LC_G][GQ_NAGG][GQ_NT], thread-private cells
+  u32* part_st;                         // record append: per-partition {chunk id : 16, used : 16} of this CTA's open chunk
   int* mat;                             // MATERIALISE: shared [0] rows of the tile so far, [2..3] the tile's output base
   i64 ninserted;                        // BUILD: rows inserted by this thread
   i64* hot_keys;                        // HIGHCARD + GQ_HOT: shared set of this batch's hot keys [GQ_HOT_POS]

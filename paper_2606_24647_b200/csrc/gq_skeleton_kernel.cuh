@@ -138,6 +138,10 @@ extern "C" __global__ void __launch_bounds__(GQ_NT + 32, 1) gq_scan(const __grid
   cx.mat = (int*)(gq_smem + GQ_CONS_OFF);
   if (tid < 4) cx.mat[tid] = 0;
 #endif
+#if GQ_PART_RW
+  cx.part_st = (u32*)(gq_smem + GQ_CONS_OFF + GQ_PART_STATE_OFF);
+  for (int i = tid; i < (int)P.npart; i += GQ_NT + 32) cx.part_st[i] = GQ_PART_CHUNK;   // no open chunk yet
+#endif
 #if GQ_HOT
   cx.hot_keys = (i64*)(gq_smem + GQ_CONS_OFF);
   cx.hot_acc = (u64*)(cx.hot_keys + GQ_HOT_POS);
@@ -385,6 +389,18 @@ extern "C" __global__ void __launch_bounds__(GQ_NT + 32, 1) gq_scan(const __grid
       if (!slot) continue;
 #pragma unroll
       for (int a = 0; a < GQ_NAGG; ++a) gq_red(GQ_AGG_OP(a), slot + 1 + GQ_NDEP + a, (i64)cx.hot_acc[pos * GQ_NAGG + a]);
+    }
+  }
+#endif
+#if GQ_PART_RW
+  {   // pad the unused slots of this CTA's open chunks with EMPTY-key records (pass B skips them)
+    gq_consumer_barrier();
+    for (int p = tid; p < (int)P.npart; p += GQ_NT) {
+      const u32 v = cx.part_st[p];
+      const u32 used = v & 0xFFFFu, chunk = v >> 16;
+      if (chunk == 0xFFFFu || used >= GQ_PART_CHUNK || (chunk == 0 && v == GQ_PART_CHUNK)) continue;
+      u64* rec = P.part + ((u64)p * (u64)P.pcap + (u64)chunk * GQ_PART_CHUNK) * GQ_PART_RW;
+      for (u32 i = used; i < GQ_PART_CHUNK; ++i) rec[(u64)i * GQ_PART_RW] = GQ_EMPTY;
     }
   }
 #endif

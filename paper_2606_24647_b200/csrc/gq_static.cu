@@ -355,7 +355,7 @@ __global__ void __launch_bounds__(GQ_PART_THREADS) gq_k_part_upsert(const __grid
   const u64 cap = P.mask + 1;
   const int rank = blockIdx.x, nrank = gridDim.x;
   for (int p = 0; p < P.npart; ++p) {
-    i64 n = (i64)P.pcur[(i64)p * GQ_PART_CURSOR_STRIDE];
+    i64 n = (i64)P.pcur[(i64)p * GQ_PART_CURSOR_STRIDE] * GQ_PART_CHUNK;   // cursors count chunks of GQ_PART_CHUNK records
     if (n > P.pcap) n = P.pcap;
     const u64* base = P.part + (u64)p * (u64)P.pcap * P.rw;
     const i64 step = (i64)nrank * GQ_PART_THREADS * GQ_PART_U;
@@ -373,6 +373,7 @@ __global__ void __launch_bounds__(GQ_PART_THREADS) gq_k_part_upsert(const __grid
         asm volatile("ld.global.nc.L1::no_allocate.v4.u64 {%0, %1, %2, %3}, [%4];"
                      : "=l"(w[u][0]), "=l"(w[u][1]), "=l"(w[u][2]), "=l"(w[u][3]) : "l"(rec));
         key[u] = w[u][0];
+        live[u] = live[u] && key[u] != GQ_EMPTY_KEY;       // padding of a partly used chunk
       }
 #pragma unroll
       for (int u = 0; u < GQ_PART_U; ++u) {
