@@ -146,7 +146,10 @@ gq_status gq_hash_aggregate_workspace(int64_t max_groups, int32_t nkeys, int32_t
  * group key is the key column of a probe step into a GQ_F_UNIQUE_KEYS table (and a dependent key, if any, is a payload
  * of that table), so a row's group is the table slot it matched and the aggregates live in an array indexed by that
  * slot (no second hash table; SURVEY §8(d) note on C3). gq_hash_aggregate takes that path when the workspace it is
- * given is at least this large; the probed table's workspace must then stay alive until the state is finished. */
+ * given is at least this large; the probed table's workspace must then stay alive until the state is finished.
+ * It also adds the record buffers of the RADIX-CLUSTERED path taken by high-cardinality states whose table is >= 256 MB
+ * when the first batch has >= 16 Mi rows (32-byte records, sized for every row of that batch: e.g. 24 GB for C5): the
+ * scan appends surviving rows per table partition and a second kernel applies them partition by partition. */
 gq_status gq_hash_aggregate_workspace_for(const gq_batch* in, const gq_agg_desc* desc, size_t* bytes);
 /* *state == NULL: creates the state in d_workspace and aggregates the batch; else aggregates a further batch. */
 gq_status gq_hash_aggregate(gq_ctx*, gq_aggstate** state, void* d_workspace, size_t bytes, const gq_batch* in,
