@@ -199,7 +199,7 @@ __device__ __forceinline__ void gq_list_feed(GqCand& mine, const GqCand& c, bool
 #define GQ_TOPK_UNROLL 4
 // pass 1: every warp scans a strided share of the table (GQ_TOPK_UNROLL chunks of 32 slots in flight) and keeps its
 // own best list; lists go to scratch.
-__global__ void __launch_bounds__(GQ_TOPK_WARPS * 32) gq_k_topk_scan(const __grid_constant__ GqFinaliseParams P) {
+__global__ void __launch_bounds__(GQ_TOPK_WARPS * 32, 4) gq_k_topk_scan(const __grid_constant__ GqFinaliseParams P) {
   if (*(volatile int*)P.err != 0) return;
   const int lane = threadIdx.x & 31;
   const int kth = P.topk - 1;
