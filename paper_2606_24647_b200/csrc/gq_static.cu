@@ -252,7 +252,7 @@ __global__ void __launch_bounds__(GQ_TOPK_WARPS * 32, 4) gq_k_topk_scan(const __
     for (int w = 1; w < GQ_TOPK_WARPS; ++w) {
       GqCand c = sh[w][lane];
       GqCand worst = gq_cand_shfl(mine, kth);
-      gq_list_feed(mine, c, c.valid && gq_better(c, worst), lane, kth);
+      gq_list_feed(mine, c, c.valid && lane <= kth && gq_better(c, worst), lane, kth);   // entries behind the k-th of a sorted list cannot matter
     }
     ((GqCand*)P.scratch)[(i64)blockIdx.x * 32 + lane] = mine;
   }
@@ -273,9 +273,9 @@ __global__ void __launch_bounds__(GQ_TOPK_MERGE_WARPS * 32) gq_k_topk_merge(cons
     c1.valid = 0; c1.val = 0; c1.k0 = 0; c1.k1 = 0; c1.slot = -1;
     if (l2 < nlists) c1 = in[l2 * 32 + lane];
     GqCand worst = gq_cand_shfl(mine, kth);
-    gq_list_feed(mine, c0, c0.valid && gq_better(c0, worst), lane, kth);
+    gq_list_feed(mine, c0, c0.valid && lane <= kth && gq_better(c0, worst), lane, kth);
     worst = gq_cand_shfl(mine, kth);
-    gq_list_feed(mine, c1, c1.valid && gq_better(c1, worst), lane, kth);
+    gq_list_feed(mine, c1, c1.valid && lane <= kth && gq_better(c1, worst), lane, kth);
   }
   sh[warp][lane] = mine;
   __syncthreads();
@@ -283,7 +283,7 @@ __global__ void __launch_bounds__(GQ_TOPK_MERGE_WARPS * 32) gq_k_topk_merge(cons
   for (int w = 1; w < GQ_TOPK_MERGE_WARPS; ++w) {
     GqCand c = sh[w][lane];
     GqCand worst = gq_cand_shfl(mine, kth);
-    gq_list_feed(mine, c, c.valid && gq_better(c, worst), lane, kth);
+    gq_list_feed(mine, c, c.valid && lane <= kth && gq_better(c, worst), lane, kth);   // entries behind the k-th of a sorted list cannot matter
   }
   unsigned have = __ballot_sync(0xffffffffu, mine.valid != 0);
   int n = min(__popc(have), P.topk);
