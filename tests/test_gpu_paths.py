@@ -215,3 +215,38 @@ def test_partitioned_aggregation_streams_batches(ctx, force_partition):
     got = gqrun.sort_rows([r["keys"][0][:ng].cpu().numpy()] + [a[:ng].cpu().numpy() for a in r["aggs"]], 1)
     for g, e in zip(got, exp.cols):
         assert np.array_equal(g, e)
+
+
+def test_pipeline_is_cuda_graph_capturable():
+    # every call only enqueues on the context's stream (no allocation, no host sync): a whole build + pipeline sequence
+    # can be captured into a CUDA graph and replayed (operators return immediately)
+    import torch
+    import gqrun
+    from paper_2606_24647_b200 import gq
+    s = torch.cuda.Stream()
+    with torch.cuda.stream(s):
+        c = gq.Context(0, stream=s)
+        plan = plans.plan_c3(datagen.make_config(3, scale=0.01))
+        exp = oracle.run_query(plan)
+        bcols = [gqrun.dev(b["table"]) for b in plan["builds"]]
+        tables = gqrun.build_tables(c, plan, device_tables=bcols)      # warm-up run compiles / loads the kernels
+        ws = [t.workspace for t in tables]
+        p = gqrun.prepare(c, plan, tables)
+        p.run()
+        c.sync()
+        g = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(g, stream=s):
+            tables = gqrun.build_tables(c, plan, device_tables=bcols, workspaces=ws)
+            pr, _ = p.m.probes([(tables[bi], kc) for bi, kc in plan["probes"]])
+            p.plan.agg.probes = pr
+            p.run()
+        for _ in range(3):
+            for a in p.aggs:
+                a.zero_()
+            g.replay()
+            torch.cuda.synchronize()
+            r = p.result()
+            got = gqrun.sort_rows([r["keys"][0].cpu().numpy()] + [a.cpu().numpy() for a in r["aggs"]], 1)
+            assert r["n"] == exp.nrows
+            for x, e in zip(got, exp.cols):
+                assert np.array_equal(x, e)
