@@ -102,14 +102,11 @@ extern "C" __global__ void __launch_bounds__(GQ_NT + 32, 1) gq_scan(const __grid
 #endif
   GQ_STAMP(0);
   const i64 ntiles = P.nrows / GQ_TILE;                  // full tiles; the remainder is the tail
-  if (*(volatile int*)P.err != 0) {                      // sticky error: later kernels are no-ops (gq.h "Errors")
-#if GQ_FUSED_FINAL
-    if (tid == 0) { const u32 t = atomicAdd(P.fin.ticket, 1u); if (t == gridDim.x - 1) *P.fin.ticket = 0; }
-#endif
-    return;
-  }
-
+  // Sticky error: later kernels are no-ops (gq.h "Errors"). Thread 0 reads the flag once, the CTA decides after the
+  // set-up barrier below: every thread sees the same value, and the round trip overlaps the shared-memory set-up.
+  volatile int* err_seen = (volatile int*)(gq_smem + GQ_BAR_OFF + 2 * GQ_STAGES * 8);
   if (tid == 0) {
+    *err_seen = *(volatile int*)P.err;
     for (int s = 0; s < GQ_STAGES; ++s) { gq_mbar_init(&full_bar[s], 1); gq_mbar_init(&empty_bar[s], GQ_NWARP); }
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
@@ -165,6 +162,12 @@ extern "C" __global__ void __launch_bounds__(GQ_NT + 32, 1) gq_scan(const __grid
   }
 #endif
   __syncthreads();
+  if (*err_seen != 0) {
+#if GQ_FUSED_FINAL
+    if (tid == 0) { const u32 t = atomicAdd(P.fin.ticket, 1u); if (t == gridDim.x - 1) *P.fin.ticket = 0; }
+#endif
+    return;
+  }
   GQ_STAMP(1);
 
   if (tid >= GQ_NT) {
