@@ -139,7 +139,8 @@ typedef struct {
   int32_t ndependent;  /* trailing key columns functionally dependent on the leading ones: stored, not hashed.
                           Needed when the packed key tuple is wider than 64 bits. */
   const gq_agg* aggs; int32_t naggs;
-  int64_t max_groups;  /* capacity bound; also selects the low-cardinality shared-memory path when small */
+  int64_t max_groups;  /* capacity bound (exceeding it => GQ_ERR_CAPACITY); <= 64 selects the low-cardinality path
+                          (per-thread cells in shared memory) */
 } gq_agg_desc;
 gq_status gq_hash_aggregate_workspace(int64_t max_groups, int32_t nkeys, int32_t naggs, size_t* bytes);
 /* Plan-aware size: at least the size above; larger when the plan qualifies for DIRECT aggregation — the single hashed
@@ -174,7 +175,10 @@ typedef struct {
   int32_t topk; int32_t topk_agg;
 } gq_plan;
 gq_status gq_pipeline_workspace(const gq_plan*, size_t* bytes);
-/* One stream-ordered pass, no host synchronisation inside: state init, fused scan kernel, finaliser. */
+/* One stream-ordered pass, no host synchronisation inside: state init, fused scan kernel, finaliser.
+ * Key-less and low-cardinality plans (max_groups <= 64) without top-k run as ONE kernel: every CTA writes its partial
+ * groups to the workspace and the last CTA to finish merges them and writes the result. The calls can be captured into
+ * a CUDA graph. */
 gq_status gq_pipeline(gq_ctx*, const gq_plan*, void* d_workspace, size_t bytes, void* const* out_key_cols,
                       int64_t* const* out_agg_cols, double* const* out_avg_cols, int64_t out_capacity,
                       int64_t* d_out_ngroups);
