@@ -456,6 +456,7 @@ __device__ __forceinline__ i64 gq_part_reserve(const GqParams& P, u32* st, u64 p
     const u32 v0 = ((volatile u32*)st)[p];
     if ((v0 & 0xFFFFu) > GQ_PART_CHUNK) {                 // being refilled by another thread, or full
       if ((v0 >> 16) == 0xFFFFu) return -1;
+      __nanosleep(64);                                    // the refill is a global atomic away: do not burn issue slots
       continue;
     }
     const u32 v = atomicAdd(&st[p], 1u);
