@@ -1,7 +1,8 @@
 // gq_skeleton.cuh — hand-written sm_100a device code of the fused scan kernel (one translation unit per plan shape).
 //
-// The plan compiler (gq_codegen.cpp) emits a small prelude of #defines + two row functions (gq_pass / gq_body) and
-// splices them at the //@@ROW_FUNCTIONS@@ marker below; everything else — the TMA bulk-copy pipeline, the hash-table
+// The plan compiler (gq_codegen.cpp) emits a small prelude of #defines + the row code (gq_tile: the GQ_R rows of a
+// thread step by step through filter, probes, projection and consumer; or gq_pass / gq_body when a probed table may
+// hold duplicate keys) and splices it at the //@@ROW_FUNCTIONS@@ marker below; everything else — the TMA bulk-copy pipeline, the hash-table
 // primitives, the shared-memory low-cardinality aggregation, the reductions — is this file, compiled as-is by NVRTC
 // (no headers needed) or by nvcc (build-time check). This is the fused FilterProject -> HashProbe* -> consumer step
 // of SURVEY.md §8(a1-a8): predicate and projection are evaluated in registers inside the consuming kernel
