@@ -49,7 +49,8 @@ typedef enum {
   GQ_ERR_WORKSPACE_TOO_SMALL = 4,
   GQ_ERR_CUDA = 5,                 /* CUDA runtime error: see gq_last_cuda_error */
   GQ_ERR_DUPLICATE_KEY = 6,        /* GQ_F_UNIQUE_KEYS asserted but a duplicate build key was seen (sticky) */
-  GQ_ERR_COMPILE = 7               /* plan-time kernel compilation failed: see gq_last_message */
+  GQ_ERR_COMPILE = 7,              /* plan-time kernel compilation failed: see gq_last_message */
+  GQ_ERR_DEPENDENT_KEY = 8         /* GQ_F_CHECK_DEPENDENT: a key declared dependent took two values in one group (sticky) */
 } gq_status;
 
 typedef enum { GQ_I8 = 1, GQ_I32 = 2, GQ_I64 = 3 } gq_dtype;
@@ -70,7 +71,12 @@ typedef struct { const gq_xtok* toks; int32_t ntoks; } gq_expr;
 typedef enum { GQ_SUM = 0, GQ_MIN, GQ_MAX, GQ_COUNT_STAR } gq_aggop;
 typedef struct { gq_aggop op; int32_t expr; /* index into exprs[]; ignored for COUNT_STAR */ } gq_agg;
 
-enum { GQ_F_UNIQUE_KEYS = 1u << 0 };  /* caller asserts unique build keys; VERIFIED on device, never trusted */
+enum {
+  GQ_F_UNIQUE_KEYS = 1u << 0,      /* gq_build_desc: caller asserts unique build keys; VERIFIED on device, never trusted */
+  GQ_F_CHECK_DEPENDENT = 1u << 1   /* gq_agg_desc: debug check of `ndependent`: every row compares its
+                                      dependent key with the one stored for its group; a mismatch sets the sticky
+                                      GQ_ERR_DEPENDENT_KEY instead of silently merging two groups */
+};
 enum { GQ_MAX_PREDS = 16, GQ_MAX_TOKS = 32, GQ_MAX_EXPRS = 8, GQ_MAX_AGGS = 8, GQ_MAX_PROBES = 4, GQ_MAX_PAYLOAD = 3,
        GQ_MAX_KEYS = 2, GQ_MAX_COLS = 32, GQ_MAX_TOPK = 32, GQ_SIDE_SLOTS = 64 };
 
@@ -141,6 +147,7 @@ typedef struct {
   const gq_agg* aggs; int32_t naggs;
   int64_t max_groups;  /* capacity bound (exceeding it => GQ_ERR_CAPACITY); <= 64 selects the low-cardinality path
                           (per-thread cells in shared memory) */
+  uint32_t flags;      /* GQ_F_CHECK_DEPENDENT */
 } gq_agg_desc;
 gq_status gq_hash_aggregate_workspace(int64_t max_groups, int32_t nkeys, int32_t naggs, size_t* bytes);
 /* Plan-aware size: at least the size above; larger when the plan qualifies for DIRECT aggregation — the single hashed
@@ -209,10 +216,14 @@ gq_status gq_table_describe(gq_table** out, const gq_dtype* payload_dtypes, int3
 /* Read-only streaming sum over `bytes` bytes (16-byte aligned, multiple of 16): the practical read roofline probe of
  * SURVEY §7.1 step 5. *d_out (DEVICE uint64) receives the wrapping sum of the 64-bit words. */
 gq_status gq_read_probe(gq_ctx*, const void* d_data, size_t bytes, uint64_t* d_out);
-/* Random-access rate probe: what bounds the hash phases (SURVEY §8(d) "secondary limiters"). Enqueues naccesses
- * pseudo-random 8-byte accesses over d_table (bytes = a power of two >= 4096, 32-byte aligned, CONTENTS ARE MODIFIED by
- * modes 1-3): mode 0 loads, 1 RED.ADD.64, 2 load + two REDs in one 32-byte slot (insert-or-update), 3 CAS. */
-gq_status gq_random_probe(gq_ctx*, void* d_table, size_t bytes, int64_t naccesses, int32_t mode, uint64_t* d_out);
+
+/* ---- planner knobs --------------------------------------------------------------------------------------------- */
+/* Process-wide thresholds a planner may override ("the query planner should choose the operator
+ * implementation based on both the expected input and the available resources"). Names:
+ *   "part_min_table_mb"  group-by tables at least this large take the radix-partitioned path (default 256)
+ *   "part_min_rows"      ... when the first batch has at least this many rows (default 16 Mi)
+ * Unknown names return GQ_ERR_INVALID_ARG. A negative value restores the default. */
+gq_status gq_set_option(const char* h_name, int64_t value);
 
 #ifdef __cplusplus
 }

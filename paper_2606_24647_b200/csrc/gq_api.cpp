@@ -2,6 +2,7 @@
 // Every entry point only enqueues work on the context's stream — no device allocation, no host sync —
 // except gq_create/gq_destroy/gq_sync and the HOST-buffer end-to-end call gq_pipeline_host.
 #include <algorithm>
+#include <atomic>
 #include <cstdio>
 #include <cstdlib>
 #include <cstring>
@@ -35,8 +36,7 @@ int64_t table_capacity(int64_t max_rows) {   // power of two >= max_rows * 4/3, 
 // takes 0.4 — its probes are latency-bound and sparse buckets save dependent rounds (C4 1.06 -> 0.98 ms); a larger
 // one is bound by random DRAM sectors and takes 0.7 to shrink its footprint (C3 1.77 -> 1.60 ms).
 int64_t join_capacity(int64_t max_rows, int slot_words = 1) {
-  int load = (max_rows * slot_words * 8 * 10 / 4 <= (80LL << 20)) ? 40 : 70;
-  if (const char* e = getenv("GQ_TUNE_JOIN_LOAD")) { int v = atoi(e); if (v >= 10 && v <= 90) load = v; }   // tuning sweeps only
+  const int load = (max_rows * slot_words * 8 * 10 / 4 <= (80LL << 20)) ? 40 : 70;
   int64_t need = std::max<int64_t>(1024, (max_rows * 100 + load - 1) / load);
   return (need + 1023) / 1024 * 1024;
 }
@@ -57,7 +57,12 @@ WsLayout ws_layout(int64_t capacity, int slot_words, int nside) {
   return w;
 }
 
+// Every entry point that enqueues work makes the context's device current first (a process may hold contexts on
+// several GPUs; cudaSetDevice is a no-op when nothing changes).
+inline void use_device(gq_ctx* ctx) { if (ctx) cudaSetDevice(ctx->device); }
+
 gq_status check_batch(gq_ctx* ctx, const gq_batch* b) {
+  use_device(ctx);
   if (!b || b->ncols < 0 || b->ncols > GQ_MAX_COLS || b->nrows < 0 || (b->ncols > 0 && !b->cols))
     return fail(ctx, GQ_ERR_INVALID_ARG, "bad batch");
   for (int c = 0; c < b->ncols; ++c) {
@@ -112,6 +117,7 @@ gq_status fill_common(gq_ctx* ctx, GqScanSpec* sp, const gq_batch* in, const gq_
     sp->exprs.emplace_back(exprs[e].toks, exprs[e].toks + exprs[e].ntoks);
   }
   sp->nrows_hint = in->nrows;
+  if (ctx && ctx->num_sms > 0) sp->num_sms = ctx->num_sms;
   return GQ_OK;
 }
 
@@ -131,12 +137,12 @@ void collect_consts(const GqScanSpec& sp, std::vector<long long>* k, std::vector
 }
 
 // Shape signature (no constant values) and the constants in codegen order (predicates, then expression literals).
-int tile_bucket(int64_t nrows) { return nrows <= 0 ? 0 : nrows < 148LL * 8 * 512 * 2 ? 1 : nrows < 148LL * 8 * 512 * 4 ? 2 : 3; }
+int tile_bucket(int64_t nrows, int sms) { return nrows <= 0 ? 0 : nrows < (int64_t)sms * 8 * 512 * 2 ? 1 : nrows < (int64_t)sms * 8 * 512 * 4 ? 2 : 3; }
 std::string signature(const GqScanSpec& sp) {
   std::string s;
   s.reserve(256);
   auto put = [&s](long long v) { s += std::to_string(v); s += ','; };
-  put(sp.consumer); put(tile_bucket(sp.nrows_hint));
+  put(sp.consumer); put(tile_bucket(sp.nrows_hint, sp.num_sms)); put(sp.num_sms);
   for (gq_dtype t : sp.in_dtype) put(t);
   s += 'p';
   for (const gq_pred& p : sp.preds) { put(p.col); put(p.op); }
@@ -150,7 +156,7 @@ std::string signature(const GqScanSpec& sp) {
   for (const gq_agg& a : sp.aggs) { put(a.op); put(a.expr); }
   put(sp.lc_cap); put(sp.lc_key_bits); put(sp.target_sw); put(sp.build_key_col);
   for (int c : sp.payload_cols) put(c);
-  put(sp.unique); put(sp.hot); put(sp.fused_final); put(sp.direct_step); put(sp.direct_aw); put(sp.direct_touch);
+  put(sp.unique); put(sp.hot); put(sp.check_dep); put(sp.fused_final); put(sp.direct_step); put(sp.direct_aw); put(sp.direct_touch);
   put(sp.part_rw); for (int e : sp.part_exprs) put(e);
   s += 'c';
   std::vector<long long> kv; std::vector<int> ki;
@@ -158,14 +164,15 @@ std::string signature(const GqScanSpec& sp) {
   for (int i : ki) put(i);
   return s;
 }
-struct CachedKernel { GqKernelInfo info; GqKernel k; bool loaded = false; };
+struct CachedKernel { GqKernelInfo info; GqKernel k; bool loaded = false; int device = -1; };
 std::mutex g_kmu;
 std::map<std::string, CachedKernel> g_kernels;
 
 // Normalise the tiling hint so that every nrows in a bucket produces the same source.
 void canon_hint(GqScanSpec* sp) {
-  static const int64_t rep[4] = {0, 148LL * 8 * 512, 148LL * 8 * 512 * 3, 0};
-  sp->nrows_hint = rep[tile_bucket(sp->nrows_hint)];
+  const int64_t unit = (int64_t)sp->num_sms * 8 * 512;
+  const int64_t rep[4] = {0, unit, unit * 3, 0};
+  sp->nrows_hint = rep[tile_bucket(sp->nrows_hint, sp->num_sms)];
 }
 
 gq_status get_kernel_info(const GqScanSpec& sp_in, CachedKernel** out, std::string* msg) {
@@ -193,10 +200,17 @@ gq_status run_scan(gq_ctx* ctx, const GqScanSpec& sp, const gq_batch* in, const 
   CachedKernel* ck = nullptr;
   gq_status st = get_kernel_info(sp, &ck, &ctx->msg);
   if (st != GQ_OK) return st;
-  if (!ck->loaded) {
-    st = gq_jit_get(ck->info, &ck->k, &ctx->msg, &ctx->last_cuda);
-    if (st != GQ_OK) return st;
-    ck->loaded = true;
+  GqKernel kern;
+  {   // distinct contexts may launch the same plan shape for the first time concurrently (gq.h "Threads")
+    std::lock_guard<std::mutex> l(g_kmu);
+    if (!ck->loaded || ck->device != ctx->device) {
+      cudaSetDevice(ctx->device);
+      st = gq_jit_get(ck->info, ctx->device, &ck->k, &ctx->msg, &ctx->last_cuda);
+      if (st != GQ_OK) return st;
+      ck->loaded = true;
+      ck->device = ctx->device;
+    }
+    kern = ck->k;
   }
   for (size_t c = 0; c < ck->info.cols.size(); ++c) P->col[c] = in->cols[ck->info.cols[c]].data;
   P->nrows = in->nrows;
@@ -214,11 +228,11 @@ gq_status run_scan(gq_ctx* ctx, const GqScanSpec& sp, const gq_batch* in, const 
   }
   P->err = ctx->d_err;
   if (in->nrows == 0) return GQ_OK;   // empty batches are legal no-ops (S9)
-  const int64_t ntiles = in->nrows / ck->k.tile_rows;
+  const int64_t ntiles = in->nrows / kern.tile_rows;
   int grid = (int)std::max<int64_t>(1, std::min<int64_t>(ctx->num_sms, ntiles));
   void* args[] = {(void*)P};
-  cudaError_t e = cudaLaunchKernel((const void*)ck->k.fn, dim3((unsigned)grid), dim3((unsigned)ck->k.threads), args,
-                                   (size_t)ck->k.smem_bytes, ctx->stream);
+  cudaError_t e = cudaLaunchKernel((const void*)kern.fn, dim3((unsigned)grid), dim3((unsigned)kern.threads), args,
+                                   (size_t)kern.smem_bytes, ctx->stream);
   if (e != cudaSuccess) return cuda_fail(ctx, e, "launch of fused scan kernel");
   ++ctx->launches;
   return GQ_OK;
@@ -253,6 +267,7 @@ gq_status gq_destroy(gq_ctx* c) {
   cudaFree(c->d_err);
   cudaFreeHost(c->h_err);
   if (c->copy_stream) cudaStreamDestroy(c->copy_stream);
+  if (c->ev_start) cudaEventDestroy(c->ev_start);
   for (int i = 0; i < 2; ++i) { if (c->ev_copied[i]) cudaEventDestroy(c->ev_copied[i]); if (c->ev_consumed[i]) cudaEventDestroy(c->ev_consumed[i]); }
   delete c;
   return GQ_OK;
@@ -260,18 +275,21 @@ gq_status gq_destroy(gq_ctx* c) {
 
 gq_status gq_sync(gq_ctx* c) {
   if (!c) return GQ_ERR_INVALID_ARG;
+  use_device(c);
   cudaError_t e = cudaMemcpyAsync(c->h_err, c->d_err, sizeof(int), cudaMemcpyDeviceToHost, c->stream);
   if (e == cudaSuccess) e = cudaStreamSynchronize(c->stream);
   if (e != cudaSuccess) return cuda_fail(c, e, "gq_sync");
   int code = *c->h_err;
   if (code == 0) return GQ_OK;
   c->msg = code == GQ_ERR_CAPACITY ? "device: hash table or output capacity exceeded"
-         : code == GQ_ERR_DUPLICATE_KEY ? "device: duplicate build key under GQ_F_UNIQUE_KEYS" : "device error";
+         : code == GQ_ERR_DUPLICATE_KEY ? "device: duplicate build key under GQ_F_UNIQUE_KEYS"
+         : code == GQ_ERR_DEPENDENT_KEY ? "device: a key declared dependent (ndependent) took two values within one group" : "device error";
   return (gq_status)code;
 }
 
 gq_status gq_clear_error(gq_ctx* c) {
   if (!c) return GQ_ERR_INVALID_ARG;
+  use_device(c);
   cudaError_t e = cudaMemsetAsync(c->d_err, 0, sizeof(int), c->stream);
   return e == cudaSuccess ? GQ_OK : cuda_fail(c, e, "gq_clear_error");
 }
@@ -286,6 +304,7 @@ const char* gq_status_str(gq_status s) {
     case GQ_ERR_CUDA: return "GQ_ERR_CUDA";
     case GQ_ERR_DUPLICATE_KEY: return "GQ_ERR_DUPLICATE_KEY";
     case GQ_ERR_COMPILE: return "GQ_ERR_COMPILE";
+    case GQ_ERR_DEPENDENT_KEY: return "GQ_ERR_DEPENDENT_KEY";
   }
   return "GQ_ERR_UNKNOWN";
 }
@@ -383,7 +402,7 @@ gq_status gq_hash_build(gq_ctx* ctx, gq_table** table, void* d_ws, size_t bytes,
     unsigned long long pat[16];
     for (int i = 0; i < 16; ++i) pat[i] = 0;
     pat[0] = GQ_EMPTY_KEY;
-    cudaError_t e = gq_launch_init_table(ctx->stream, t->dev.slots, cap, sw, pat, t->dev.side, GQ_SIDE_SLOTS, t->dev.header, 0);
+    cudaError_t e = gq_launch_init_table(ctx->stream, t->dev.slots, cap, sw, pat, t->dev.side, GQ_SIDE_SLOTS, t->dev.header, 0, ctx->num_sms);
     if (e != cudaSuccess) { delete t; return cuda_fail(ctx, e, "table init"); }
     ++ctx->launches;
     { GqScanSpec c = sp; c.nrows_hint = 0; t->build_sig = signature(c); }
@@ -401,6 +420,7 @@ gq_status gq_hash_build(gq_ctx* ctx, gq_table** table, void* d_ws, size_t bytes,
 
 gq_status gq_hash_build_finish(gq_ctx* ctx, gq_table* t) {
   if (!ctx || !t || t->describe_only) return GQ_ERR_INVALID_ARG;
+  use_device(ctx);
   if (!t->ready) {
     cudaError_t e = cudaEventCreateWithFlags(&t->ready, cudaEventDisableTiming);
     if (e != cudaSuccess) return cuda_fail(ctx, e, "cudaEventCreate");
@@ -414,6 +434,7 @@ gq_status gq_hash_build_finish(gq_ctx* ctx, gq_table* t) {
 
 gq_status gq_table_count(gq_ctx* ctx, const gq_table* t, int64_t* d_count) {
   if (!ctx || !t || !d_count || t->describe_only) return GQ_ERR_INVALID_ARG;
+  use_device(ctx);
   cudaError_t e = cudaMemcpyAsync(d_count, t->dev.header, 8, cudaMemcpyDeviceToDevice, ctx->stream);
   return e == cudaSuccess ? GQ_OK : cuda_fail(ctx, e, "gq_table_count");
 }
@@ -487,8 +508,12 @@ gq_status agg_spec(gq_ctx* ctx, GqScanSpec* sp, const gq_batch* in, const gq_agg
   sp->lc_key_bits = bits;
   sp->consumer = d->nkeys == 0 ? GQ_C_GLOBAL : sp->lc_cap > 0 ? GQ_C_LOWCARD : GQ_C_HIGHCARD;
   // skew handling is compiled in when the group key is one plain input column (so that it can be sampled)
+  bool all_unique = true;
+  for (const GqProbeSpec& ps : sp->probes) all_unique = all_unique && ps.unique;
   sp->hot = sp->consumer == GQ_C_HIGHCARD && d->nkeys == 1 && d->ndependent == 0 && sp->key_cols[0] < in->ncols &&
-            agg_has_hot_area(d->max_groups, d->nkeys);
+            agg_has_hot_area(d->max_groups, d->nkeys) && all_unique;
+  if (d->flags & ~(uint32_t)GQ_F_CHECK_DEPENDENT) return fail(ctx, GQ_ERR_INVALID_ARG, "unknown gq_agg_desc flags");
+  sp->check_dep = (d->flags & GQ_F_CHECK_DEPENDENT) != 0 && d->ndependent > 0;
   return GQ_OK;
 }
 
@@ -502,6 +527,7 @@ struct DirectPlan { int step = -1; int aw = 0; int touch = -1; int dep_pay = -1;
 DirectPlan direct_plan(const GqScanSpec& sp, const gq_agg_desc* d, const gq_batch* in, bool schema_only = false) {
   DirectPlan dp;
   if (sp.consumer != GQ_C_HIGHCARD || d->nkeys - d->ndependent != 1 || d->nprobes < 1) return dp;
+  for (const GqProbeSpec& ps : sp.probes) if (!ps.unique) return dp;   // rows fan out: the one-row-at-a-time code has no direct form
   int step = -1;
   for (int s = 0; s < d->nprobes; ++s)
     if (d->probes[s].key_col == d->key_cols[0] && d->probes[s].table && (d->probes[s].table->flags & GQ_F_UNIQUE_KEYS) &&
@@ -533,7 +559,8 @@ DirectPlan direct_plan(const GqScanSpec& sp, const gq_agg_desc* d, const gq_batc
 // partition and pass B (gq_k_part_upsert) applies the records partition by partition, so every insert-or-update hits
 // an L2-resident table slice. Worth it only for big tables and big batches; thresholds overridable for tests.
 struct PartPlan { bool on = false; int npart = 0, pshift = 0, rw = 0; int64_t pcap = 0; size_t bytes = 0; std::vector<int> exprs; int src[GQ_MAX_AGGS]; };
-int64_t env_i64(const char* name, int64_t dflt) { const char* e = getenv(name); return e ? atoll(e) : dflt; }
+// planner knobs (gq_set_option)
+std::atomic<int64_t> g_part_min_table_mb{256}, g_part_min_rows{1 << 24};
 PartPlan part_plan(const GqScanSpec& sp, const gq_agg_desc* d, int64_t nrows) {
   PartPlan pp;
   if (sp.consumer != GQ_C_HIGHCARD) return pp;
@@ -541,10 +568,9 @@ PartPlan part_plan(const GqScanSpec& sp, const gq_agg_desc* d, int64_t nrows) {
   const int64_t cap = agg_capacity(d->max_groups, d->nkeys);
   const int sw = sp.target_sw;
   const int64_t table_bytes = cap * sw * 8;
-  if (table_bytes < env_i64("GQ_TUNE_PART_MIN_TABLE_MB", 256) * (1 << 20) || nrows < env_i64("GQ_TUNE_PART_MIN_ROWS", 1 << 24)) return pp;
+  if (table_bytes < g_part_min_table_mb.load() * (1 << 20) || nrows < g_part_min_rows.load()) return pp;
   int64_t np = 16;
   while (np < 4096 && table_bytes / np > (4 << 20) && np * 2 <= cap / 64) np <<= 1;
-  if (env_i64("GQ_TUNE_PART_NPART", 0) > 0) np = env_i64("GQ_TUNE_PART_NPART", 0);
   pp.npart = (int)np;
   pp.pshift = log2i(cap) - log2i(np);
   for (int a = 0; a < d->naggs; ++a) {
@@ -620,7 +646,7 @@ gq_status gq_hash_aggregate(gq_ctx* ctx, gq_aggstate** state, void* d_ws, size_t
       a->dacc = (unsigned long long*)((char*)d_ws + 256);
       for (int i = 0; i < d->naggs; ++i)
         pat[i] = d->aggs[i].op == GQ_MIN ? 0x7FFFFFFFFFFFFFFFULL : d->aggs[i].op == GQ_MAX ? 0x8000000000000000ULL : 0ULL;
-      e = gq_launch_init_table(ctx->stream, a->dacc, dp.cap + 1, dp.aw, pat, a->dacc, 0, a->dev.header, 0);
+      e = gq_launch_init_table(ctx->stream, a->dacc, dp.cap + 1, dp.aw, pat, a->dacc, 0, a->dev.header, 0, ctx->num_sms);
     } else {
       const int64_t cap = agg_capacity(d->max_groups, d->nkeys);
       const int sw = sp.target_sw;
@@ -652,10 +678,12 @@ gq_status gq_hash_aggregate(gq_ctx* ctx, gq_aggstate** state, void* d_ws, size_t
       a->dev.shift = cap > 0 ? 64 - log2i(cap) : 63;
       a->dev.slot_words = sw;
       pat[0] = GQ_EMPTY_KEY;
+      a->check_dep = sp.check_dep;
+      if (sp.check_dep) pat[1] = GQ_DEP_UNSET;
       for (int i = 0; i < d->naggs; ++i)
         pat[1 + d->ndependent + i] = d->aggs[i].op == GQ_MIN ? 0x7FFFFFFFFFFFFFFFULL : d->aggs[i].op == GQ_MAX ? 0x8000000000000000ULL : 0ULL;
       // a key-less aggregation has exactly one group, present even with no input rows (S9): header[1] = 1
-      e = gq_launch_init_table(ctx->stream, a->dev.slots, cap, sw, pat, a->dev.side, 1, a->dev.header, d->nkeys == 0 ? 1 : 0);
+      e = gq_launch_init_table(ctx->stream, a->dev.slots, cap, sw, pat, a->dev.side, 1, a->dev.header, d->nkeys == 0 ? 1 : 0, ctx->num_sms);
     }
     if (e != cudaSuccess) { delete a; return cuda_fail(ctx, e, "aggregate state init"); }
     ++ctx->launches;
@@ -683,12 +711,12 @@ gq_status gq_hash_aggregate(gq_ctx* ctx, gq_aggstate** state, void* d_ws, size_t
     int nl = 0;
     const gq_column& kc = in->cols[sp.key_cols[0]];
     cudaError_t e = gq_launch_hot_keys(ctx->stream, kc.data, (int)kc.dtype, in->nrows, a->hot_table, GQ_HOT_SLOTS, GQ_HOT_SAMPLE,
-                                       GQ_HOT_THRESHOLD, a->hot, GQ_HOT_MAX, &nl);
+                                       GQ_HOT_THRESHOLD, a->hot, GQ_HOT_MAX, ctx->num_sms, &nl);
     if (e != cudaSuccess) return cuda_fail(ctx, e, "heavy-hitter sampling");
     ctx->launches += nl;
     P.hot = a->hot;
   }
-  if (a->part && !a->direct && in->nrows >= env_i64("GQ_TUNE_PART_MIN_ROWS", 1 << 24) / 4) {
+  if (a->part && !a->direct && in->nrows >= g_part_min_rows.load() / 4) {
     // radix-clustered: pass A appends records per table partition, pass B applies them partition by partition
     PartPlan pp = part_plan(sp, d, a->part_rows);
     if (!pp.on || pp.rw != a->part_rw || pp.npart != a->npart) return fail(ctx, GQ_ERR_INVALID_ARG, "batch schema/desc differs from the state's first batch");
@@ -703,6 +731,7 @@ gq_status gq_hash_aggregate(gq_ctx* ctx, gq_aggstate** state, void* d_ws, size_t
     pb.part = a->part; pb.pcur = a->pcur; pb.pcap = a->pcap; pb.npart = a->npart; pb.rw = a->part_rw;
     pb.slots = a->dev.slots; pb.mask = a->dev.mask; pb.sw = a->dev.slot_words; pb.ndep = a->ndep; pb.naggs = a->naggs;
     for (int i = 0; i < a->naggs; ++i) { pb.op[i] = (int)a->agg_op[i]; pb.src[i] = pp.src[i]; }
+    pb.check_dep = a->check_dep ? 1 : 0;
     pb.err = ctx->d_err;
     e = gq_launch_part_upsert(ctx->stream, pb, ctx->num_sms);
     if (e != cudaSuccess) return cuda_fail(ctx, e, "partitioned upsert");
@@ -718,6 +747,7 @@ gq_status gq_hash_aggregate_finish(gq_ctx* ctx, gq_aggstate* a, void* const* out
                                    const gq_avg* avgs, int32_t navg, double* const* out_avg_cols, int64_t out_capacity,
                                    int32_t topk, int32_t topk_agg, void* d_topk_scratch, int64_t* d_out_ngroups) {
   if (!ctx || !a || !out_agg_cols || !d_out_ngroups || out_capacity < 0) return GQ_ERR_INVALID_ARG;
+  use_device(ctx);
   if (a->nkeys > 0 && !out_key_cols) return fail(ctx, GQ_ERR_INVALID_ARG, "missing key outputs");
   if (navg < 0 || navg > GQ_MAX_AGGS || (navg > 0 && (!avgs || !out_avg_cols))) return fail(ctx, GQ_ERR_INVALID_ARG, "bad avg spec");
   if (topk < 0 || topk > GQ_MAX_TOPK) return fail(ctx, GQ_ERR_UNSUPPORTED, "topk > GQ_MAX_TOPK");
@@ -838,18 +868,19 @@ gq_status gq_pipeline(gq_ctx* ctx, const gq_plan* plan, void* d_ws, size_t bytes
 // ------------------------------------------------------------------------------------------------ read probe
 gq_status gq_read_probe(gq_ctx* ctx, const void* d_data, size_t bytes, uint64_t* d_out) {
   if (!ctx || !d_data || !d_out || !aligned(d_data, 16) || bytes % 16) return GQ_ERR_INVALID_ARG;
+  use_device(ctx);
   cudaError_t e = gq_launch_read_probe(ctx->stream, d_data, bytes, (unsigned long long*)d_out, ctx->num_sms);
   if (e != cudaSuccess) return cuda_fail(ctx, e, "read probe");
   ++ctx->launches;
   return GQ_OK;
 }
 
-gq_status gq_random_probe(gq_ctx* ctx, void* d_table, size_t bytes, int64_t naccesses, int32_t mode, uint64_t* d_out) {
-  if (!ctx || !d_table || !d_out || !aligned(d_table, 32) || bytes < 4096 || (bytes & (bytes - 1)) || naccesses < 0 || mode < 0 || mode > 3)
-    return GQ_ERR_INVALID_ARG;
-  cudaError_t e = gq_launch_random_probe(ctx->stream, d_table, bytes, naccesses, mode, (unsigned long long*)d_out, ctx->num_sms);
-  if (e != cudaSuccess) return cuda_fail(ctx, e, "random probe");
-  ++ctx->launches;
+gq_status gq_set_option(const char* h_name, int64_t value) {
+  if (!h_name) return GQ_ERR_INVALID_ARG;
+  const std::string n = h_name;
+  if (n == "part_min_table_mb") g_part_min_table_mb = value < 0 ? 256 : value;
+  else if (n == "part_min_rows") g_part_min_rows = value < 0 ? (1 << 24) : value;
+  else return GQ_ERR_INVALID_ARG;
   return GQ_OK;
 }
 
@@ -857,6 +888,7 @@ gq_status gq_random_probe(gq_ctx* ctx, void* d_table, size_t bytes, int64_t nacc
 
 // ------------------------------------------------------------------------------------------------ host-buffer e2e
 namespace {
+const int64_t GQ_HOST_CHUNK_ALIGN = 30720;   // lcm of the tile sizes the plan compiler picks
 struct HostLayout { size_t agg_off, agg_bytes, topk_off, stage_off[2], stage_col_off[GQ_MAX_COLS], stage_bytes, out_off, out_key_off[2],
                     out_agg_off[GQ_MAX_AGGS], out_avg_off[GQ_MAX_AGGS], n_off, total; };
 gq_status host_layout(const gq_plan* plan, int64_t chunk_rows, int64_t out_capacity, HostLayout* L) {
@@ -885,7 +917,7 @@ extern "C" {
 gq_status gq_pipeline_host_workspace(const gq_plan* plan, int64_t chunk_rows, size_t* bytes) {
   if (!plan || !plan->in || !bytes || chunk_rows < 1) return GQ_ERR_INVALID_ARG;
   HostLayout L;
-  chunk_rows = (chunk_rows + 7679) / 7680 * 7680;   // same rounding as gq_pipeline_host
+  chunk_rows = (chunk_rows + GQ_HOST_CHUNK_ALIGN - 1) / GQ_HOST_CHUNK_ALIGN * GQ_HOST_CHUNK_ALIGN;   // same rounding as gq_pipeline_host
   // output capacity is not known here: size for max_groups rows (top-k needs only k)
   int64_t cap = plan->topk > 0 ? plan->topk : std::max<int64_t>(1, plan->agg.max_groups);
   gq_status st = host_layout(plan, chunk_rows, cap, &L);
@@ -899,8 +931,10 @@ gq_status gq_pipeline_host(gq_ctx* ctx, const gq_plan* plan, int64_t chunk_rows,
                            int64_t out_capacity, int64_t* h_out_ngroups) {
   if (!ctx || !plan || !plan->in || !d_ws || chunk_rows < 1 || !h_out_ngroups || !h_out_agg_cols) return GQ_ERR_INVALID_ARG;
   const gq_batch* in = plan->in;
+  use_device(ctx);
   if (in->ncols < 1 || in->ncols > GQ_MAX_COLS) return fail(ctx, GQ_ERR_INVALID_ARG, "bad batch");
-  chunk_rows = (chunk_rows + 7679) / 7680 * 7680;   // whole tiles (1280 / 1536 / 1024 rows) per chunk: only the last chunk has a ragged tail
+  // whole tiles of every kernel shape (1024 / 1280 / 1536 / 2048 rows) per chunk: only the last chunk has a ragged tail
+  chunk_rows = (chunk_rows + GQ_HOST_CHUNK_ALIGN - 1) / GQ_HOST_CHUNK_ALIGN * GQ_HOST_CHUNK_ALIGN;
   int64_t cap = plan->topk > 0 ? plan->topk : std::max<int64_t>(1, plan->agg.max_groups);
   if (out_capacity > cap) out_capacity = cap;
   HostLayout L;
@@ -916,6 +950,11 @@ gq_status gq_pipeline_host(gq_ctx* ctx, const gq_plan* plan, int64_t chunk_rows,
     }
     if (e != cudaSuccess) return cuda_fail(ctx, e, "copy stream setup");
   }
+  // the staging areas may still be in use by earlier work on the context's stream
+  if (!ctx->ev_start) e = cudaEventCreateWithFlags(&ctx->ev_start, cudaEventDisableTiming);
+  if (e == cudaSuccess) e = cudaEventRecord(ctx->ev_start, ctx->stream);
+  if (e == cudaSuccess) e = cudaStreamWaitEvent(ctx->copy_stream, ctx->ev_start, 0);
+  if (e != cudaSuccess) return cuda_fail(ctx, e, "copy stream ordering");
   char* ws = (char*)d_ws;
   gq_aggstate* a = nullptr;
   int64_t nchunks = std::max<int64_t>(1, (in->nrows + chunk_rows - 1) / chunk_rows);

@@ -109,6 +109,25 @@ struct Gen {
 }  // namespace
 
 
+// ---- filter condition of one predicate, shared by both modes ----
+static bool pred_cond(Gen& g, const gq_pred& p, std::string* c) {
+  const std::string v = g.val(p.col);
+  const std::string klo = g.konst(p.lo);   // sequenced: lo before hi (operands of + are unsequenced)
+  const std::string khi = (p.op == GQ_RANGE_CO || p.op == GQ_RANGE_CC) ? g.konst(p.hi) : std::string();
+  switch (p.op) {
+    case GQ_LT: *c = v + " < " + klo; break;
+    case GQ_LE: *c = v + " <= " + klo; break;
+    case GQ_GT: *c = v + " > " + klo; break;
+    case GQ_GE: *c = v + " >= " + klo; break;
+    case GQ_EQ: *c = v + " == " + klo; break;
+    case GQ_NE: *c = v + " != " + klo; break;
+    case GQ_RANGE_CO: *c = v + " >= " + klo + " && " + v + " < " + khi; break;
+    case GQ_RANGE_CC: *c = v + " >= " + klo + " && " + v + " <= " + khi; break;
+    default: return g.fail("unknown comparison");
+  }
+  return true;
+}
+
 // ---- key expression shared by both modes: one hashed 64-bit word (+ optional dependent column) ----
 static gq_status key_exprs(Gen& g, const GqScanSpec& sp, std::string* keyx, std::string* depx, std::string* msg) {
   const int nk = (int)sp.key_cols.size();
@@ -157,20 +176,8 @@ static gq_status emit_linear(Gen& g, const GqScanSpec& sp, std::ostringstream& o
       o << "    if (live[j]) { ";
       if (!loaded[(size_t)p.col]) { o << g.load(p.col) << " "; loaded[(size_t)p.col] = true; }
     }
-    std::string v = g.val(p.col), c;
-    const std::string klo = g.konst(p.lo);
-    const std::string khi = (p.op == GQ_RANGE_CO || p.op == GQ_RANGE_CC) ? g.konst(p.hi) : std::string();
-    switch (p.op) {
-      case GQ_LT: c = v + " < " + klo; break;
-      case GQ_LE: c = v + " <= " + klo; break;
-      case GQ_GT: c = v + " > " + klo; break;
-      case GQ_GE: c = v + " >= " + klo; break;
-      case GQ_EQ: c = v + " == " + klo; break;
-      case GQ_NE: c = v + " != " + klo; break;
-      case GQ_RANGE_CO: c = v + " >= " + klo + " && " + v + " < " + khi; break;
-      case GQ_RANGE_CC: c = v + " >= " + klo + " && " + v + " <= " + khi; break;
-      default: if (msg) *msg = "unknown comparison"; return GQ_ERR_INVALID_ARG;
-    }
+    std::string c;
+    if (!pred_cond(g, p, &c)) return GQ_ERR_INVALID_ARG;
     o << "live[j] = " << (dense ? "live[j] && " : "") << "(" << c << "); }\n";
   }
   o << "  }\n";
@@ -276,7 +283,7 @@ static gq_status emit_linear(Gen& g, const GqScanSpec& sp, std::ostringstream& o
       o << "  u64* slot[GQ_R]; bool won[GQ_R];\n";
       o << "  gq_upsert_rows<" << sp.target_sw << ">(P.target, tkey, live, slot, won, P.err);\n";
       o << "  " << LOOP << "if (live[j] && slot[j]) {\n";
-      if (sp.ndep == 1) o << "    if (won[j]) slot[j][1] = (u64)" << depx << ";\n";
+      if (sp.ndep == 1) o << "    gq_dep_store(slot[j] + 1, " << depx << ", won[j], P.err);\n";
       for (int a = 0; a < nagg; ++a)
         o << "    gq_red(" << (int)sp.aggs[(size_t)a].op << ", slot[j] + " << (1 + sp.ndep + a) << ", " << aggval(sp.aggs[(size_t)a]) << ");\n";
       o << "  }\n";
@@ -357,7 +364,6 @@ gq_status gq_codegen(const GqScanSpec& sp, GqKernelInfo* out, std::string* msg) 
   const int ncol = (int)g.cols.size();
   int row_bytes = 0;
   for (int c : g.cols) row_bytes += gq_dtype_bytes(sp.in_dtype[(size_t)c]);
-  auto env_int = [](const char* name) { const char* e = getenv(name); return e ? atoi(e) : 0; };   // tuning sweeps only
   // Hash phases are bound by memory latency, not bandwidth (profiles/r1_hash_phases.md): 24 consumer warps x 2 rows
   // hide more of it than 16 x 4 (C4 1.56 -> 1.13 ms). Pure scans: 20 warps x 2 rows (C2 0.242 -> 0.238 ms).
   const bool hashing = nprobe > 0 || sp.consumer == GQ_C_BUILD || sp.consumer == GQ_C_HIGHCARD || sp.consumer == GQ_C_DIRECT ||
@@ -365,7 +371,6 @@ gq_status gq_codegen(const GqScanSpec& sp, GqKernelInfo* out, std::string* msg) 
   int nt = hashing ? 768 : 640;
   const bool tablebound = sp.consumer == GQ_C_HIGHCARD && nprobe == 0;   // DRAM-random bound (C5): 16 warps x 4 rows measured best
   if (tablebound) nt = 512;
-  if (env_int("GQ_TUNE_NT") && sp.consumer != GQ_C_LOWCARD) nt = env_int("GQ_TUNE_NT");
   long long cons_bytes = 256;
   int lc_kt = 64, lc_key32 = 0;
   if (sp.consumer == GQ_C_GLOBAL) cons_bytes = 8LL * nagg * (nt / 32) + 256;
@@ -377,7 +382,6 @@ gq_status gq_codegen(const GqScanSpec& sp, GqKernelInfo* out, std::string* msg) 
     // thread-private cells: as many consumer threads as leave room for a 3-stage ring of one-row-per-thread tiles
     for (nt = 256; nt > 128; nt /= 2)   // 8 warps x GQ_R independent rows per thread; cells cost 8 B x groups x aggregates per thread
       if (head + 8LL * sp.lc_cap * nagg * nt + 3LL * ((row_bytes * nt + 127) / 128 * 128 + 128 * ncol) + 1024 <= GQ_SMEM_LIMIT) break;
-    if (env_int("GQ_TUNE_LC_NT")) nt = env_int("GQ_TUNE_LC_NT");
     cons_bytes = head + 8LL * sp.lc_cap * nagg * nt;
   }
   bool all_unique = true;
@@ -388,10 +392,9 @@ gq_status gq_codegen(const GqScanSpec& sp, GqKernelInfo* out, std::string* msg) 
   if (sp.part_rw > 0) { part_state_off = (cons_bytes + 127) / 128 * 128; cons_bytes = part_state_off + 4096 * 4; }   // <= 4096 partitions
   int r = tablebound ? 4 : 2, stages = 0;
   // small inputs: smaller tiles so that every SM still gets several tiles
-  if (sp.nrows_hint > 0 && sp.nrows_hint < 148LL * 8 * nt * 2) r = 1;
-  if (sp.consumer == GQ_C_LOWCARD) r = (sp.nrows_hint > 0 && sp.nrows_hint < 148LL * nt * 4) ? 1 : 4;   // straight-line rows: ILP
-  if (sp.consumer == GQ_C_MATERIALISE && !hashing && !(sp.nrows_hint > 0 && sp.nrows_hint < 148LL * 8 * nt * 2)) r = 4;   // two CTA barriers per tile: bigger tiles
-  if (env_int("GQ_TUNE_R")) r = env_int("GQ_TUNE_R");
+  if (sp.nrows_hint > 0 && sp.nrows_hint < (long long)sp.num_sms * 8 * nt * 2) r = 1;
+  if (sp.consumer == GQ_C_LOWCARD) r = (sp.nrows_hint > 0 && sp.nrows_hint < (long long)sp.num_sms * nt * 4) ? 1 : 4;   // straight-line rows: ILP
+  if (sp.consumer == GQ_C_MATERIALISE && !hashing && !(sp.nrows_hint > 0 && sp.nrows_hint < (long long)sp.num_sms * 8 * nt * 2)) r = 4;   // two CTA barriers per tile: bigger tiles
   long long stage_bytes = 0;
   for (;; r /= 2) {
     stage_bytes = 0;
@@ -400,7 +403,6 @@ gq_status gq_codegen(const GqScanSpec& sp, GqKernelInfo* out, std::string* msg) 
     stages = (int)std::min<long long>(4, avail / stage_bytes);
     if (stages >= 3 || r == 1) break;
   }
-  if (env_int("GQ_TUNE_STAGES") && env_int("GQ_TUNE_STAGES") < stages) stages = env_int("GQ_TUNE_STAGES");
   if (stages < 1) { if (msg) *msg = "plan does not fit shared memory"; return GQ_ERR_UNSUPPORTED; }
 
   // ---- 3. prelude ----
@@ -410,8 +412,8 @@ gq_status gq_codegen(const GqScanSpec& sp, GqKernelInfo* out, std::string* msg) 
     << stages << "\n#define GQ_STAGE_BYTES " << stage_bytes << "\n#define GQ_CONSUMER " << sp.consumer << "\n";
   o << "#define GQ_NAGG " << nagg << "\n#define GQ_LC_G " << (sp.lc_cap > 0 ? sp.lc_cap : 1) << "\n#define GQ_LC_KT " << lc_kt
     << "\n#define GQ_LC_KEY32 " << lc_key32 << "\n#define GQ_TARGET_SW "
-    << (sp.target_sw > 0 ? sp.target_sw : 1) << "\n#define GQ_NDEP " << sp.ndep << "\n#define GQ_EVICT_FIRST " << (getenv("GQ_TUNE_NO_EVICT_FIRST") ? 0 : 1) << "\n#define GQ_HOT " << (use_hot ? 1 : 0)
-    << "\n#define GQ_PART_RW " << sp.part_rw << "\n#define GQ_PART_STATE_OFF " << part_state_off << "\n#define GQ_STAMPS " << (getenv("GQ_TUNE_STAMPS") ? 1 : 0) << "\n#define GQ_FUSED_FINAL " << (sp.fused_final ? 1 : 0) << "\n#define GQ_DIRECT_AW " << (sp.direct_aw > 0 ? sp.direct_aw : 1) << "\n";
+    << (sp.target_sw > 0 ? sp.target_sw : 1) << "\n#define GQ_NDEP " << sp.ndep << "\n#define GQ_CHECK_DEP " << (sp.check_dep ? 1 : 0) << "\n#define GQ_LC_KEY_BITS " << (lc_key32 ? sp.lc_key_bits : 1) << "\n#define GQ_HOT " << (use_hot ? 1 : 0)
+    << "\n#define GQ_PART_RW " << sp.part_rw << "\n#define GQ_PART_STATE_OFF " << part_state_off << "\n#define GQ_FUSED_FINAL " << (sp.fused_final ? 1 : 0) << "\n#define GQ_DIRECT_AW " << (sp.direct_aw > 0 ? sp.direct_aw : 1) << "\n";
   {
     long long off = 0, tx = 0;
     std::ostringstream offs, bytes;
@@ -450,20 +452,8 @@ gq_status gq_codegen(const GqScanSpec& sp, GqKernelInfo* out, std::string* msg) 
       std::vector<bool> loaded(g.compact.size(), false);
       for (const gq_pred& p : sp.preds) {
         if (!loaded[(size_t)p.col]) { o << "  " << g.load(p.col) << "\n"; loaded[(size_t)p.col] = true; }
-        std::string v = g.val(p.col), c;
-        const std::string klo = g.konst(p.lo);   // sequenced: lo before hi (operands of + are unsequenced)
-        const std::string khi = (p.op == GQ_RANGE_CO || p.op == GQ_RANGE_CC) ? g.konst(p.hi) : std::string();
-        switch (p.op) {
-          case GQ_LT: c = v + " < " + klo; break;
-          case GQ_LE: c = v + " <= " + klo; break;
-          case GQ_GT: c = v + " > " + klo; break;
-          case GQ_GE: c = v + " >= " + klo; break;
-          case GQ_EQ: c = v + " == " + klo; break;
-          case GQ_NE: c = v + " != " + klo; break;
-          case GQ_RANGE_CO: c = v + " >= " + klo + " && " + v + " < " + khi; break;
-          case GQ_RANGE_CC: c = v + " >= " + klo + " && " + v + " <= " + khi; break;
-          default: if (msg) *msg = "unknown comparison"; return GQ_ERR_INVALID_ARG;
-        }
+        std::string c;
+        if (!pred_cond(g, p, &c)) return GQ_ERR_INVALID_ARG;
         o << "  if (!(" << c << ")) return false;\n";
       }
     }
@@ -520,21 +510,8 @@ gq_status gq_codegen(const GqScanSpec& sp, GqKernelInfo* out, std::string* msg) 
     // group key
     std::string keyx, depx;
     if (sp.consumer == GQ_C_LOWCARD || sp.consumer == GQ_C_HIGHCARD) {
-      const int nk = (int)sp.key_cols.size();
-      if (nk < 1 || nk > GQ_MAX_KEYS || sp.ndep < 0 || sp.ndep >= nk) { if (msg) *msg = "bad key columns"; return GQ_ERR_INVALID_ARG; }
-      if (nk - sp.ndep == 1) keyx = g.val(sp.key_cols[0]);
-      else {  // two hashed keys packed into one 64-bit word: key0 in the low bits
-        auto dt = [&](int c) { return c < g.ncols_in ? sp.in_dtype[(size_t)c]
-                                                      : sp.probes[(size_t)g.vcol_probe[(size_t)(c - g.ncols_in)]].pay_dtype[g.vcol_pay[(size_t)(c - g.ncols_in)]]; };
-        int b0 = 8 * gq_dtype_bytes(dt(sp.key_cols[0])), b1 = 8 * gq_dtype_bytes(dt(sp.key_cols[1]));
-        if (b0 + b1 > 64) { if (msg) *msg = "packed key wider than 64 bits: declare a dependent key (ndependent)"; return GQ_ERR_UNSUPPORTED; }
-        char buf[256];
-        snprintf(buf, sizeof buf, "(i64)((((u64)%s) & 0x%llxULL) | ((((u64)%s) & 0x%llxULL) << %d))", g.val(sp.key_cols[0]).c_str(),
-                 (unsigned long long)((b0 == 64) ? ~0ULL : ((1ULL << b0) - 1)), g.val(sp.key_cols[1]).c_str(),
-                 (unsigned long long)((1ULL << b1) - 1), b0);
-        keyx = buf;
-      }
-      if (sp.ndep == 1) depx = g.val(sp.key_cols[(size_t)nk - 1]);
+      gq_status kst = key_exprs(g, sp, &keyx, &depx, msg);
+      if (kst != GQ_OK) return kst;
     }
     auto aggval = [&](const gq_agg& a) { return a.op == GQ_COUNT_STAR ? std::string("1") : "e" + std::to_string(a.expr); };
     switch (sp.consumer) {
@@ -552,7 +529,7 @@ gq_status gq_codegen(const GqScanSpec& sp, GqKernelInfo* out, std::string* msg) 
       case GQ_C_HIGHCARD:
         o << ind << "bool won; u64* slot = gq_ht_upsert<" << sp.target_sw << ">(P.target, " << keyx << ", &won, P.err);\n";
         o << ind << "if (slot) {\n";
-        if (sp.ndep == 1) o << ind << "  if (won) slot[1] = (u64)" << depx << ";\n";
+        if (sp.ndep == 1) o << ind << "  gq_dep_store(slot + 1, " << depx << ", won, P.err);\n";
         for (int a = 0; a < nagg; ++a)
           o << ind << "  gq_red(" << (int)sp.aggs[(size_t)a].op << ", slot + " << (1 + sp.ndep + a) << ", " << aggval(sp.aggs[(size_t)a]) << ");\n";
         o << ind << "}\n";
@@ -573,7 +550,7 @@ gq_status gq_codegen(const GqScanSpec& sp, GqKernelInfo* out, std::string* msg) 
         for (size_t e = 0; e < sp.exprs.size(); ++e) o << ind << "  P.out[" << e << "][orow] = e" << e << ";\n";
         o << ind << "}\n";
         break;
-      default: if (msg) *msg = "unknown consumer"; return GQ_ERR_INVALID_ARG;
+      default: if (msg) *msg = "consumer not available for plans that probe a table with duplicate keys"; return GQ_ERR_UNSUPPORTED;
     }
     for (int s = nprobe - 1; s >= 0; --s) {
       if (sp.probes[(size_t)s].unique) o << ind << "break;  // unique build keys: first match is the only match\n";

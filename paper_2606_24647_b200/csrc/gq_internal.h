@@ -14,6 +14,8 @@
 #define GQ_MAXK 48
 #define GQ_MAXOUT 12
 #define GQ_SMEM_LIMIT 232448   // 227 KB opt-in dynamic shared memory per CTA on sm_100
+#define GQ_DEFAULT_SMS 148     // B200; used only when a plan is compiled ahead of time without a device attached
+#define GQ_DEP_UNSET 0x8000000000000001ULL   // dependent-key word of a slot nobody has stored yet (GQ_F_CHECK_DEPENDENT)
 
 enum { GQ_C_GLOBAL = 0, GQ_C_LOWCARD = 1, GQ_C_HIGHCARD = 2, GQ_C_BUILD = 3, GQ_C_MATERIALISE = 4, GQ_C_DIRECT = 5, GQ_C_PARTITION = 6 };
 
@@ -68,12 +70,12 @@ struct gq_ctx {
   cudaStream_t stream = nullptr;
   int* d_err = nullptr;        // sticky device error; d_err + 16 = ticket counter of the fused finaliser
   int* h_err = nullptr;        // pinned mirror
-  int num_sms = 148;
+  int num_sms = GQ_DEFAULT_SMS;
   int last_cuda = 0;
   int64_t launches = 0;
   std::string msg;
   cudaStream_t copy_stream = nullptr;   // gq_pipeline_host: H2D copies overlap the scan of the previous chunk
-  cudaEvent_t ev_copied[2] = {nullptr, nullptr}, ev_consumed[2] = {nullptr, nullptr};
+  cudaEvent_t ev_copied[2] = {nullptr, nullptr}, ev_consumed[2] = {nullptr, nullptr}, ev_start = nullptr;
 };
 
 struct gq_table {
@@ -100,6 +102,7 @@ struct gq_aggstate {
   int64_t max_groups = 0;
   bool lowcard = false;
   int lc_cap = 0;
+  bool check_dep = false;      // GQ_F_CHECK_DEPENDENT
   bool direct = false;         // aggregate words indexed by the slot of a probed unique table (no keys stored)
   GqTableDev dtab{};           //   that table
   int64_t dcap = 0;            //   its capacity (the accumulator array has dcap + 1 slots: the last is the side entry)
@@ -144,6 +147,8 @@ struct GqScanSpec {
   std::vector<int> payload_cols;
   bool unique = false;
   bool hot = false;                               // HIGHCARD: per-CTA shared-memory aggregation of hot keys
+  bool check_dep = false;                         // GQ_F_CHECK_DEPENDENT: every row verifies the dependent key
+  int num_sms = GQ_DEFAULT_SMS;                   // tiling heuristics: SM count of the context's device
   int64_t nrows_hint = 0;                         // tiling heuristic only
 };
 
@@ -163,7 +168,7 @@ int gq_dtype_bytes(gq_dtype t);
 // gq_jit.cpp
 struct GqKernel { cudaKernel_t fn = nullptr; int threads = 0; int smem_bytes = 0; int tile_rows = 0; };
 gq_status gq_jit_compile_to_cache(const GqKernelInfo& info, std::string* cubin_path, std::string* msg);
-gq_status gq_jit_get(const GqKernelInfo& info, GqKernel* out, std::string* msg, int* cuda_err);
+gq_status gq_jit_get(const GqKernelInfo& info, int device, GqKernel* out, std::string* msg, int* cuda_err);
 void gq_jit_set_cache_dir(const char* path);
 // gq_static.cu
 struct GqFinaliseParams {
@@ -181,23 +186,23 @@ struct GqFinaliseParams {
 };
 cudaError_t gq_launch_init_table(cudaStream_t s, unsigned long long* slots, long long nslots, int slot_words,
                                  const unsigned long long* pattern, unsigned long long* side, long long nside,
-                                 long long* header, long long header1);
+                                 long long* header, long long header1, int num_sms);
 cudaError_t gq_launch_finalise(cudaStream_t s, const GqFinaliseParams& p, int num_sms, int* nlaunches);
 cudaError_t gq_launch_read_probe(cudaStream_t s, const void* data, size_t bytes, unsigned long long* out, int num_sms);
-cudaError_t gq_launch_random_probe(cudaStream_t s, void* table, size_t bytes, long long n, int mode, unsigned long long* out, int num_sms);
 #define GQ_PART_CHUNK 32            // records per CTA-private append chunk (cursors count chunks)
 #define GQ_PART_CURSOR_STRIDE 16   // one append cursor per 128-byte line: atomics to one line serialise at L2
 struct GqPartParams {
   const unsigned long long* part; const unsigned long long* pcur; long long pcap; int npart; int rw;
   unsigned long long* slots; unsigned long long mask; int sw; int ndep; int naggs;
   int op[GQ_MAX_AGGS]; int src[GQ_MAX_AGGS];   // src = record word of the aggregate's input, -1 = COUNT(*)
+  int check_dep;
   int* err;
 };
 cudaError_t gq_launch_part_upsert(cudaStream_t s, const GqPartParams& p, int num_sms);
 size_t gq_topk_scratch_bytes_impl();
 cudaError_t gq_launch_hot_keys(cudaStream_t s, const void* keycol, int dtype, long long nrows, unsigned long long* table,
                                long long nslots, long long nsample, unsigned long long threshold, long long* hot,
-                               int max_hot, int* nlaunches);
+                               int max_hot, int num_sms, int* nlaunches);
 #define GQ_HOT_MAX 256               // hot keys per batch (shared-memory set of 2*GQ_HOT_MAX positions per CTA)
 #define GQ_HOT_SAMPLE (1LL << 19)    // sampled rows
 #define GQ_HOT_SLOTS (1LL << 20)     // (key,count) sample table slots (16 B each)

@@ -19,7 +19,7 @@
 namespace {
 std::mutex g_mu;
 std::string g_cache_dir;
-std::map<std::string, GqKernel> g_loaded;   // hash -> loaded kernel (per process; single device assumed)
+std::map<std::string, GqKernel> g_loaded;   // hash@device -> loaded kernel (the shared-memory attribute is per device)
 
 typedef int (*fn_create)(void**, const char*, const char*, int, const char* const*, const char* const*);
 typedef int (*fn_compile)(void*, int, const char* const*);
@@ -116,9 +116,10 @@ gq_status gq_jit_compile_to_cache(const GqKernelInfo& info, std::string* cubin_p
   return get_cubin(info, &cubin, cubin_path, msg);
 }
 
-gq_status gq_jit_get(const GqKernelInfo& info, GqKernel* out, std::string* msg, int* cuda_err) {
+gq_status gq_jit_get(const GqKernelInfo& info, int device, GqKernel* out, std::string* msg, int* cuda_err) {
   std::lock_guard<std::mutex> l(g_mu);
-  auto it = g_loaded.find(info.hash);
+  const std::string lkey = info.hash + "@" + std::to_string(device);
+  auto it = g_loaded.find(lkey);
   if (it != g_loaded.end()) { *out = it->second; return GQ_OK; }
   std::string cubin;
   gq_status st = get_cubin(info, &cubin, nullptr, msg);
@@ -134,7 +135,7 @@ gq_status gq_jit_get(const GqKernelInfo& info, GqKernel* out, std::string* msg, 
     return GQ_ERR_CUDA;
   }
   GqKernel k; k.fn = fn; k.threads = info.threads; k.smem_bytes = info.smem_bytes; k.tile_rows = info.tile_rows;
-  g_loaded[info.hash] = k;
+  g_loaded[lkey] = k;
   *out = k;
   return GQ_OK;
 }

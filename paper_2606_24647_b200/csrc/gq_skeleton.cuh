@@ -19,7 +19,7 @@
 //
 // Prelude macros expected: GQ_NCOL, GQ_NT, GQ_R, GQ_STAGES, GQ_STAGE_BYTES, GQ_COL_OFF(c), GQ_COL_BYTES(c) (bytes per
 // element), GQ_CONSUMER, GQ_NAGG, GQ_AGG_OP(a), GQ_LC_G (group cells), GQ_LC_KT (key-table slots), GQ_LC_KEY32,
-// GQ_TARGET_SW, GQ_NDEP, GQ_EVICT_FIRST, GQ_HOT, GQ_FUSED_FINAL, GQ_DIRECT_AW.
+// GQ_LC_KEY_BITS, GQ_TARGET_SW, GQ_NDEP, GQ_CHECK_DEP, GQ_HOT, GQ_FUSED_FINAL, GQ_DIRECT_AW.
 
 typedef unsigned long long u64;
 typedef long long i64;
@@ -43,6 +43,7 @@ typedef unsigned int u32;
 
 #define GQ_E_CAPACITY 3
 #define GQ_E_DUPLICATE 6
+#define GQ_E_DEPENDENT 8
 
 #define GQ_OP_SUM 0
 #define GQ_OP_MIN 1
@@ -129,14 +130,9 @@ __device__ __forceinline__ u64 gq_policy_evict_first() {
 }
 // 1-D bulk copy global -> shared, completion counted in bytes on an mbarrier (TMA engine; SASS: UBLKCP).
 __device__ __forceinline__ void gq_bulk_g2s(void* dst, const void* src, u32 bytes, u64* bar, u64 pol) {
-#if GQ_EVICT_FIRST
   asm volatile(
       "cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes.L2::cache_hint [%0], [%1], %2, [%3], %4;" ::
           "r"(gq_smem_addr(dst)), "l"(src), "r"(bytes), "r"(gq_smem_addr(bar)), "l"(pol) : "memory");
-#else
-  asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::
-                   "r"(gq_smem_addr(dst)), "l"(src), "r"(bytes), "r"(gq_smem_addr(bar)) : "memory");
-#endif
 }
 __device__ __forceinline__ void gq_consumer_barrier() {   // named barrier 1: the GQ_NT consumer threads only
   asm volatile("bar.sync 1, %0;" ::"n"(GQ_NT) : "memory");
@@ -415,6 +411,20 @@ __device__ __forceinline__ void gq_upsert_rows(const GqTableDev& T, const i64 (&
   }
 }
 
+// Dependent key word of a group slot: a trailing key column declared functionally dependent on the
+// hashed key is stored, not hashed. Normally the row that created the group stores it. With GQ_F_CHECK_DEPENDENT the
+// word starts as GQ_DEP_UNSET and EVERY row CASes its value in: a row that finds a different value stored proves the
+// declaration false and sets the sticky GQ_E_DEPENDENT.
+#define GQ_DEP_UNSET 0x8000000000000001ULL
+__device__ __forceinline__ void gq_dep_store(u64* w, i64 dep, bool won, int* err) {
+#if GQ_CHECK_DEP
+  const u64 prev = atomicCAS(w, GQ_DEP_UNSET, (u64)dep);
+  if (prev != GQ_DEP_UNSET && prev != (u64)dep) gq_set_err(err, GQ_E_DEPENDENT);
+#else
+  if (won) *w = (u64)dep;
+#endif
+}
+
 // Aggregate update at L2 (RED.ADD / RED.MIN / RED.MAX .64 — results are not read back).
 __device__ __forceinline__ void gq_red(const int OP, u64* p, i64 v) {
   if (OP == GQ_OP_SUM || OP == GQ_OP_COUNT) atomicAdd(p, (u64)v);
@@ -521,9 +531,12 @@ struct GqCtx {
 // kernel). Packed keys narrower than 32 bits use {key32, gid} entries fetched with one LDS.64.
 #define GQ_LC_LOG2KT (GQ_LC_KT == 64 ? 6 : GQ_LC_KT == 128 ? 7 : 8)
 #define GQ_LC_PENDING 0xFFFFFFFEu   // group id of a key-table position that is claimed but not published yet
+// {key32, gid} entries hold the key masked to the packed key width (< 32 bits): a sign-extended single key such as -1
+// would otherwise equal the high half of an EMPTY entry (~0). Distinct keys of that width stay distinct when masked.
+#define GQ_LC_K32(key) ((u32)(key) & ((1u << GQ_LC_KEY_BITS) - 1u))
 __device__ __forceinline__ u32 gq_lc_hash(i64 key) {
 #if GQ_LC_KEY32
-  return ((u32)key * 0x9E3779B1u) >> (32 - GQ_LC_LOG2KT);
+  return (GQ_LC_K32(key) * 0x9E3779B1u) >> (32 - GQ_LC_LOG2KT);
 #else
   return (u32)gq_hash(key, 64 - GQ_LC_LOG2KT);
 #endif
@@ -535,7 +548,7 @@ __device__ __forceinline__ int gq_lc_find(const GqCtx& cx, i64 key) {
 #if GQ_LC_KEY32
   for (int n = 0; n < GQ_LC_KT; ++n, h = (h + 1) & (GQ_LC_KT - 1)) {
     const u64 e = ((volatile u64*)cx.lc_tab)[h];
-    if ((u32)(e >> 32) == (u32)key) return (u32)e == GQ_LC_PENDING ? -1 : (int)(u32)e;
+    if ((u32)(e >> 32) == GQ_LC_K32(key)) return (u32)e == GQ_LC_PENDING ? -1 : (int)(u32)e;
     if (e == ~0ULL) return -1;
   }
 #else
@@ -553,7 +566,7 @@ __device__ __forceinline__ int gq_lc_find1(const GqCtx& cx, i64 key) {
   const u32 h = gq_lc_hash(key);
 #if GQ_LC_KEY32
   const u64 e = ((volatile u64*)cx.lc_tab)[h];
-  return ((u32)(e >> 32) == (u32)key && (u32)e != GQ_LC_PENDING) ? (int)(u32)e : -1;
+  return ((u32)(e >> 32) == GQ_LC_K32(key) && (u32)e != GQ_LC_PENDING) ? (int)(u32)e : -1;
 #else
   const u64 k = ((volatile u64*)cx.lc_tab)[h];
   if (k != (u64)key || k == GQ_EMPTY) return -1;
@@ -592,16 +605,16 @@ __device__ __forceinline__ int gq_lc_insert_or_find(GqCtx& cx, i64 k, int* err) 
   for (int adv = 0; adv < GQ_LC_KT;) {                     // `continue` re-examines the same position
 #if GQ_LC_KEY32
     const u64 e = ((volatile u64*)cx.lc_tab)[i];
-    if ((u32)(e >> 32) == (u32)k) {
+    if ((u32)(e >> 32) == GQ_LC_K32(k)) {
       if ((u32)e != GQ_LC_PENDING) return (int)(u32)e;
       continue;                                           // id not published yet: look again
     }
     if (e == ~0ULL) {
-      const u64 prev = atomicCAS(&cx.lc_tab[i], ~0ULL, ((u64)(u32)k << 32) | GQ_LC_PENDING);
+      const u64 prev = atomicCAS(&cx.lc_tab[i], ~0ULL, ((u64)GQ_LC_K32(k) << 32) | GQ_LC_PENDING);
       if (prev == ~0ULL) {
         const int g = gq_lc_new_group(cx, k, err);
         __threadfence_block();
-        ((volatile u64*)cx.lc_tab)[i] = ((u64)(u32)k << 32) | (u32)g;
+        ((volatile u64*)cx.lc_tab)[i] = ((u64)GQ_LC_K32(k) << 32) | (u32)g;
         return g;
       }
       continue;                                           // somebody claimed this position: re-examine it
@@ -629,6 +642,14 @@ __device__ __forceinline__ int gq_lc_insert_or_find(GqCtx& cx, i64 k, int* err) 
   }
   gq_set_err(err, GQ_E_CAPACITY);                         // key table full
   return 0;
+}
+// One row at a time (row code of plans that probe a table with duplicate keys: rows fan out, so the lanes of a warp
+// are not converged here): look the key up, insert it on first sight. gq_lc_insert_or_find is a single-thread,
+// lock-free protocol, so it needs no warp cooperation; a lane that meets an entry another lane is still publishing
+// re-reads it (independent thread scheduling guarantees the publisher makes progress).
+__device__ __forceinline__ int gq_lc_slot(GqCtx& cx, i64 key, int* err) {
+  const int g = gq_lc_find(cx, key);
+  return g >= 0 ? g : gq_lc_insert_or_find(cx, key, err);
 }
 // Slow path (collision, or first sight of a key): the needy lanes of the warp are grouped by key (MATCH.ANY); the
 // first lane of every group inserts or finds its key — all groups at once, they touch different table positions —

@@ -30,14 +30,6 @@ __device__ __forceinline__ void gq_process(const GqParams& P, const Src& src, Gq
 
 __device__ __forceinline__ i64 gq_ldcg(const i64* p) { return __ldcg(p); }
 
-// Tuning aid (GQ_TUNE_STAMPS): thread 0 of the LAST CTA records globaltimer values at phase boundaries behind a magic
-// word at the end of the partials scratch, so that the fixed costs of a one-launch pipeline can be read back.
-#if GQ_STAMPS && GQ_FUSED_FINAL
-#define GQ_STAMP(i) do { if (threadIdx.x == 0) { unsigned long long t_; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t_)); gq_stamp[i] = t_; } } while (0)
-#else
-#define GQ_STAMP(i) do { } while (0)
-#endif
-
 #if GQ_FUSED_FINAL
 __device__ __forceinline__ i64 gq_fin_sext(u64 v, int bits) {
   if (bits >= 64) return (i64)v;
@@ -96,11 +88,6 @@ extern "C" __global__ void __launch_bounds__(GQ_NT + 32, 1) gq_scan(const __grid
   u64* full_bar = (u64*)(gq_smem + GQ_BAR_OFF);
   u64* empty_bar = full_bar + GQ_STAGES;
   const int tid = threadIdx.x;
-#if GQ_STAMPS && GQ_FUSED_FINAL
-  unsigned long long gq_stamp[12];
-  for (int i = 0; i < 12; ++i) gq_stamp[i] = 0;
-#endif
-  GQ_STAMP(0);
   const i64 ntiles = P.nrows / GQ_TILE;                  // full tiles; the remainder is the tail
   // Sticky error: later kernels are no-ops (gq.h "Errors"). Thread 0 reads the flag once, the CTA decides after the
   // set-up barrier below: every thread sees the same value, and the round trip overlaps the shared-memory set-up.
@@ -168,7 +155,6 @@ extern "C" __global__ void __launch_bounds__(GQ_NT + 32, 1) gq_scan(const __grid
 #endif
     return;
   }
-  GQ_STAMP(1);
 
   if (tid >= GQ_NT) {
     // ------------------------------------------------------------------ producer warp: TMA bulk copies
@@ -199,10 +185,8 @@ extern "C" __global__ void __launch_bounds__(GQ_NT + 32, 1) gq_scan(const __grid
       const int s = (int)(it % GQ_STAGES);
       const u32 ph = (u32)((it / GQ_STAGES) & 1);
       gq_mbar_wait(&full_bar[s], ph);                    // the tile's bytes have landed
-      if (it == 0) GQ_STAMP(2);
       src.stage = gq_smem + (size_t)s * GQ_STAGE_BYTES;
       gq_process(P, src, cx, GQ_R, true);
-      if (it == 0) GQ_STAMP(3);
       __syncwarp();
       if ((tid & 31) == 0) gq_mbar_arrive(&empty_bar[s]);  // this warp is done with the stage
     }
@@ -221,7 +205,6 @@ extern "C" __global__ void __launch_bounds__(GQ_NT + 32, 1) gq_scan(const __grid
   }
 
   // -------------------------------------------------------------------- consumer epilogues
-  GQ_STAMP(4);
   const int lane = tid & 31, warp = tid >> 5;
   (void)lane; (void)warp;
 #if GQ_CONSUMER == GQ_C_GLOBAL
@@ -319,11 +302,9 @@ extern "C" __global__ void __launch_bounds__(GQ_NT + 32, 1) gq_scan(const __grid
     }
     if (tid == 0) pn[blockIdx.x] = ng;
     gq_consumer_barrier();
-    GQ_STAMP(5);
     if (tid == 0) { __threadfence(); cx.lc_n[3] = (atomicAdd(P.fin.ticket, 1u) == gridDim.x - 1); }
     gq_consumer_barrier();
     if (((volatile int*)cx.lc_n)[3]) {
-      GQ_STAMP(6);
       // (writers fenced before taking their ticket; the partials are read with ld.cg after the CTA barrier above)
 #pragma unroll
       for (int a = 0; a < GQ_NAGG; ++a)
@@ -355,7 +336,6 @@ extern "C" __global__ void __launch_bounds__(GQ_NT + 32, 1) gq_scan(const __grid
         }
       }
       gq_consumer_barrier();
-      GQ_STAMP(7);
       const int ng2 = min(((volatile int*)cx.lc_n)[0], GQ_LC_G);
       for (int p0 = warp; p0 < ng2 * GQ_NAGG; p0 += 4 * GQ_NWARP) {
         i64 v[4];
@@ -369,14 +349,6 @@ extern "C" __global__ void __launch_bounds__(GQ_NT + 32, 1) gq_scan(const __grid
         if (tid < P.fin.out_capacity) gq_fin_emit(P.fin, tid, cx.lc_gkey[tid], fin + tid * GQ_NAGG);
         else gq_set_err(P.err, GQ_E_CAPACITY);
       }
-      GQ_STAMP(8);
-#if GQ_STAMPS
-      if (tid == 0) {
-        unsigned long long* dbg = (unsigned long long*)(pn + gridDim.x + 8);
-        dbg[0] = 0x57414D5053544D50ULL;
-        for (int i = 0; i < 12; ++i) dbg[1 + i] = gq_stamp[i];
-      }
-#endif
       if (tid == 0) { *P.fin.out_n = ng2; *P.fin.ticket = 0; }
     }
 #endif

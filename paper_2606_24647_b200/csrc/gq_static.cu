@@ -1,7 +1,7 @@
 // gq_static.cu — plan-independent sm_100a kernels, compiled by nvcc into libgq.so: hash-table initialisation, the
 // HashAggregation finaliser (table -> dense output columns + device-side group count + derived AVG),
 // the top-k finaliser (OrderBy/TopN in its smallest form) and the read-roofline probe.
-#include <cstdlib>
+#include <algorithm>
 
 #include "gq_internal.h"
 
@@ -35,13 +35,13 @@ __global__ void gq_k_init_table(u64* slots, i64 nwords, int sw, const __grid_con
 }
 
 cudaError_t gq_launch_init_table(cudaStream_t s, u64* slots, i64 nslots, int sw, const u64* pattern, u64* side,
-                                 i64 nside, i64* header, i64 header1) {
+                                 i64 nside, i64* header, i64 header1, int num_sms) {
   ulonglong4 p[4];
   u64* pp = (u64*)p;
   for (int i = 0; i < 16; ++i) pp[i] = pattern[i % sw];
   i64 nwords = nslots * sw;
   i64 work = (sw & 1) == 0 ? nwords / 2 : nwords;
-  int blocks = (int)std::min<i64>(148 * 16, std::max<i64>(1, (work + 255) / 256));
+  int blocks = (int)std::min<i64>((i64)num_sms * 16, std::max<i64>(1, (work + 255) / 256));
   gq_k_init_table<<<blocks, 256, 0, s>>>(slots, nwords, sw, p[0], p[1], p[2], p[3], side, nside * sw, header, header1);
   return cudaGetLastError();
 }
@@ -402,7 +402,12 @@ __global__ void __launch_bounds__(GQ_PART_THREADS) gq_k_part_upsert(const __grid
         }
         if (!slot) { atomicCAS(P.err, 0, (int)GQ_ERR_CAPACITY); continue; }
         const u64* rec = base + r * P.rw;
-        if (won && P.ndep) slot[1] = w[u][1];
+        if (P.ndep) {   // dependent key word (see gq_dep_store in the scan skeleton)
+          if (P.check_dep) {
+            const u64 prev = atomicCAS(slot + 1, GQ_DEP_UNSET, w[u][1]);
+            if (prev != GQ_DEP_UNSET && prev != w[u][1]) atomicCAS(P.err, 0, (int)GQ_ERR_DEPENDENT_KEY);
+          } else if (won) slot[1] = w[u][1];
+        }
         for (int a = 0; a < P.naggs; ++a) {
           const int sa = P.src[a];
           const i64 v = sa < 0 ? 1 : sa == 1 ? (i64)w[u][1] : sa == 2 ? (i64)w[u][2] : sa == 3 ? (i64)w[u][3] : (i64)__ldg(rec + sa);
@@ -416,55 +421,7 @@ __global__ void __launch_bounds__(GQ_PART_THREADS) gq_k_part_upsert(const __grid
   }
 }
 cudaError_t gq_launch_part_upsert(cudaStream_t s, const GqPartParams& p, int num_sms) {
-  int per_sm = 2;
-  if (const char* e = getenv("GQ_TUNE_PART_CTAS_PER_SM")) { int v = atoi(e); if (v >= 1 && v <= 4) per_sm = v; }   // tuning sweeps only
-  gq_k_part_upsert<<<num_sms * per_sm, GQ_PART_THREADS, 0, s>>>(p);
-  return cudaGetLastError();
-}
-
-// ------------------------------------------------------------------------------------------------ random-access probe
-// What the hash phases can reach on this box: n pseudo-random 8-byte accesses spread over a table of `bytes` bytes
-// (a power of two), 4 independent accesses in flight per thread. mode 0 = read-only loads, 1 = RED.ADD.64,
-// 2 = load + two REDs in the same 32-byte slot (an insert-or-update), 3 = CAS.
-__device__ __forceinline__ u64 gq_p_mix(u64 x) {
-  x ^= x >> 33; x *= 0xff51afd7ed558ccdULL; x ^= x >> 33; x *= 0xc4ceb9fe1a85ec53ULL; x ^= x >> 33;
-  return x;
-}
-template <int MODE>
-__global__ void __launch_bounds__(512) gq_k_random_probe(u64* tab, u64 mask, i64 n, u64* out) {
-  u64 acc = 0;
-  const i64 nthreads = (i64)gridDim.x * blockDim.x;
-  for (i64 i0 = (i64)blockIdx.x * blockDim.x + threadIdx.x; i0 < n; i0 += nthreads * 4) {
-    u64 idx[4], v[4];
-#pragma unroll
-    for (int j = 0; j < 4; ++j) idx[j] = gq_p_mix((u64)(i0 + j * nthreads)) & mask;
-    if (MODE == 0) {
-#pragma unroll
-      for (int j = 0; j < 4; ++j) v[j] = __ldg(tab + idx[j]);
-    } else if (MODE == 1) {
-#pragma unroll
-      for (int j = 0; j < 4; ++j) { atomicAdd(tab + idx[j], 1ULL); v[j] = 0; }
-    } else if (MODE == 2) {
-#pragma unroll
-      for (int j = 0; j < 4; ++j) v[j] = *(volatile u64*)(tab + (idx[j] & ~3ULL));
-#pragma unroll
-      for (int j = 0; j < 4; ++j) { atomicAdd(tab + (idx[j] & ~3ULL) + 1, 1ULL); atomicAdd(tab + (idx[j] & ~3ULL) + 2, 1ULL); }
-    } else {
-#pragma unroll
-      for (int j = 0; j < 4; ++j) v[j] = atomicCAS(tab + idx[j], ~0ULL, 5ULL);
-    }
-#pragma unroll
-    for (int j = 0; j < 4; ++j) acc += v[j];
-  }
-  if (acc == 0x123456789ULL) *out = acc;   // keeps the loads alive
-}
-cudaError_t gq_launch_random_probe(cudaStream_t s, void* table, size_t bytes, i64 n, int mode, u64* out, int num_sms) {
-  const u64 mask = (u64)(bytes / 8) - 1;
-  dim3 g((unsigned)num_sms * 4), b(512);
-  if (mode == 0) gq_k_random_probe<0><<<g, b, 0, s>>>((u64*)table, mask, n, out);
-  else if (mode == 1) gq_k_random_probe<1><<<g, b, 0, s>>>((u64*)table, mask, n, out);
-  else if (mode == 2) gq_k_random_probe<2><<<g, b, 0, s>>>((u64*)table, mask, n, out);
-  else gq_k_random_probe<3><<<g, b, 0, s>>>((u64*)table, mask, n, out);
+  gq_k_part_upsert<<<num_sms * 2, GQ_PART_THREADS, 0, s>>>(p);
   return cudaGetLastError();
 }
 
@@ -532,11 +489,11 @@ __global__ void gq_k_hot_select(const u64* table, i64 nslots, u64 threshold, i64
 }
 
 cudaError_t gq_launch_hot_keys(cudaStream_t s, const void* keycol, int dtype, i64 nrows, u64* table, i64 nslots,
-                               i64 nsample, u64 threshold, i64* hot, int max_hot, int* nlaunches) {
+                               i64 nsample, u64 threshold, i64* hot, int max_hot, int num_sms, int* nlaunches) {
   // (key,count) slots: key = EMPTY (0x80..0), count = 0
   u64 pat[16];
   for (int i = 0; i < 16; ++i) pat[i] = (i & 1) ? 0 : GQ_EMPTY_KEY;
-  cudaError_t e = gq_launch_init_table(s, table, nslots, 2, pat, table, 0, hot, 0);   // header := hot list head (zeroed)
+  cudaError_t e = gq_launch_init_table(s, table, nslots, 2, pat, table, 0, hot, 0, num_sms);   // header := hot list head (zeroed)
   if (e != cudaSuccess) return e;
   int shift = 64;
   for (i64 c = 1; c < nslots; c <<= 1) --shift;

@@ -27,8 +27,9 @@ _CMP = dict(lt=0, le=1, gt=2, ge=3, eq=4, ne=5, range_co=6, range_cc=7)
 _XOP = dict(col=0, const=1, add=2, sub=3, mul=4)
 _AGG = dict(sum=0, min=1, max=2, count=3)
 F_UNIQUE_KEYS = 1
+F_CHECK_DEPENDENT = 2
 STATUS = ["GQ_OK", "GQ_ERR_INVALID_ARG", "GQ_ERR_UNSUPPORTED", "GQ_ERR_CAPACITY", "GQ_ERR_WORKSPACE_TOO_SMALL",
-          "GQ_ERR_CUDA", "GQ_ERR_DUPLICATE_KEY", "GQ_ERR_COMPILE"]
+          "GQ_ERR_CUDA", "GQ_ERR_DUPLICATE_KEY", "GQ_ERR_COMPILE", "GQ_ERR_DEPENDENT_KEY"]
 
 # every symbol include/gq.h declares (tests check that the library exports all of them)
 SYMBOLS = ["gq_create", "gq_destroy", "gq_sync", "gq_clear_error", "gq_status_str", "gq_last_cuda_error",
@@ -37,7 +38,7 @@ SYMBOLS = ["gq_create", "gq_destroy", "gq_sync", "gq_clear_error", "gq_status_st
            "gq_hash_aggregate_workspace", "gq_hash_aggregate_workspace_for", "gq_hash_aggregate", "gq_topk_scratch_bytes", "gq_hash_aggregate_finish",
            "gq_aggstate_destroy", "gq_pipeline_workspace", "gq_pipeline", "gq_pipeline_host_workspace",
            "gq_pipeline_host", "gq_set_kernel_cache_dir", "gq_precompile_pipeline", "gq_precompile_build", "gq_precompile_materialise",
-           "gq_table_describe", "gq_read_probe", "gq_random_probe"]
+           "gq_table_describe", "gq_read_probe", "gq_set_option"]
 
 
 class GqError(RuntimeError):
@@ -84,7 +85,7 @@ class _AggDesc(C.Structure):
     _fields_ = [("preds", C.POINTER(_Pred)), ("npred", C.c_int32), ("probes", C.POINTER(_Probe)),
                 ("nprobes", C.c_int32), ("exprs", C.POINTER(_Expr)), ("nexpr", C.c_int32),
                 ("key_cols", C.POINTER(C.c_int32)), ("nkeys", C.c_int32), ("ndependent", C.c_int32),
-                ("aggs", C.POINTER(_Agg)), ("naggs", C.c_int32), ("max_groups", C.c_int64)]
+                ("aggs", C.POINTER(_Agg)), ("naggs", C.c_int32), ("max_groups", C.c_int64), ("flags", C.c_uint32)]
 
 
 class _Avg(C.Structure):
@@ -145,7 +146,7 @@ def lib():
                                                 C.POINTER(_Expr), C.c_int32, C.c_char_p, C.c_size_t]
         L.gq_table_describe.argtypes = [C.POINTER(C.c_void_p), C.POINTER(C.c_int), C.c_int32, C.c_uint32]
         L.gq_read_probe.argtypes = [C.c_void_p, C.c_void_p, C.c_size_t, C.c_void_p]
-        L.gq_random_probe.argtypes = [C.c_void_p, C.c_void_p, C.c_size_t, C.c_int64, C.c_int32, C.c_void_p]
+        L.gq_set_option.argtypes = [C.c_char_p, C.c_int64]
         _lib = L
     return _lib
 
@@ -211,7 +212,7 @@ class _M:
         self.keep += [a, list(tensors)]
         return a
 
-    def agg_desc(self, preds, probes, exprs, keys, ndependent, aggs, max_groups):
+    def agg_desc(self, preds, probes, exprs, keys, ndependent, aggs, max_groups, check_dependent=False):
         pr, npr = self.preds(preds)
         pb, npb = self.probes(probes)
         ee, ne = self.exprs(exprs)
@@ -220,7 +221,8 @@ class _M:
         for i, a in enumerate(aggs):
             aa[i] = _Agg(_AGG[a[0]], int(a[1]) if len(a) > 1 and a[1] is not None else 0)
         self.keep.append(aa)
-        return _AggDesc(pr, npr, pb, npb, ee, ne, kk, nk, int(ndependent), aa, len(aggs), int(max_groups))
+        return _AggDesc(pr, npr, pb, npb, ee, ne, kk, nk, int(ndependent), aa, len(aggs), int(max_groups),
+                        F_CHECK_DEPENDENT if check_dependent else 0)
 
     def build_desc(self, preds, probes, key, payload, unique):
         pr, npr = self.preds(preds)
@@ -395,12 +397,12 @@ class Context:
 
     # ---- HashAggregation (streaming) ----
     def aggregate(self, state, cols, preds=(), probes=(), exprs=(), keys=(), ndependent=0, aggs=(), max_groups=1,
-                  plan_aware_workspace=False):
+                  plan_aware_workspace=False, check_dependent=False):
         """plan_aware_workspace: size the state with gq_hash_aggregate_workspace_for (enables direct aggregation)."""
         with torch.cuda.stream(self.stream):
             m = _M()
             b = m.batch(cols)
-            d = m.agg_desc(preds, probes, exprs, keys, ndependent, aggs, max_groups)
+            d = m.agg_desc(preds, probes, exprs, keys, ndependent, aggs, max_groups, check_dependent)
             if state is None:
                 nbytes = C.c_size_t()
                 if plan_aware_workspace:
@@ -435,9 +437,9 @@ class Context:
 
     # ---- fused pipeline ----
     def prepare_pipeline(self, cols, preds=(), probes=(), exprs=(), keys=(), ndependent=0, aggs=(), max_groups=1,
-                         avgs=(), topk=0, topk_agg=0, out_capacity=None):
+                         avgs=(), topk=0, topk_agg=0, out_capacity=None, check_dependent=False):
         return Pipeline(self, cols, preds, probes, exprs, keys, ndependent, aggs, max_groups, avgs, topk, topk_agg,
-                        out_capacity)
+                        out_capacity, check_dependent)
 
     def read_probe(self, t: torch.Tensor) -> torch.Tensor:
         out = torch.zeros(1, dtype=torch.int64, device=self.device)
@@ -447,26 +449,19 @@ class Context:
         return out
 
 
-    def random_probe(self, table: torch.Tensor, naccesses: int, mode: int) -> None:
-        """Enqueue gq_random_probe over a uint8/int64 CUDA tensor whose byte size is a power of two."""
-        out = torch.zeros(1, dtype=torch.int64, device=self.device)
-        with torch.cuda.stream(self.stream):
-            self._check(self.L.gq_random_probe(self.h, table.data_ptr(), table.numel() * table.element_size(),
-                                               int(naccesses), int(mode), out.data_ptr()))
-        self._keep_probe_out = out
-
 
 class Pipeline:
     """A marshalled gq_plan with its workspace and outputs pre-allocated: run() is one gq_pipeline call (enqueue only)."""
 
     def __init__(self, ctx, cols, preds, probes, exprs, keys, ndependent, aggs, max_groups, avgs, topk, topk_agg,
-                 out_capacity):
+                 out_capacity, check_dependent=False):
         self.ctx, L = ctx, ctx.L
         m = self.m = _M()
         self.host = not cols[0].is_cuda
         self.batch = m.batch(cols)
         aa, na = m.avgs(avgs)
-        self.plan = _Plan(C.pointer(self.batch), m.agg_desc(preds, probes, exprs, keys, ndependent, aggs, max_groups),
+        self.plan = _Plan(C.pointer(self.batch),
+                          m.agg_desc(preds, probes, exprs, keys, ndependent, aggs, max_groups, check_dependent),
                           aa, na, int(topk), int(topk_agg))
         dts = _row_dtypes(cols, probes)
         cap = int(out_capacity if out_capacity is not None else (topk if topk > 0 else max(1, max_groups)))
@@ -512,11 +507,20 @@ class Pipeline:
         return dict(n=n, keys=[k[:n] for k in self.keys], aggs=[a[:n] for a in self.aggs], avgs=[v[:n] for v in self.avgs])
 
 
-def precompile_pipeline(col_dtypes, nrows, preds=(), probes=(), exprs=(), keys=(), ndependent=0, aggs=(), max_groups=1):
+def set_option(name: str, value: int) -> None:
+    """Planner knob (gq_set_option): e.g. "part_min_rows"; a negative value restores the default."""
+    st = lib().gq_set_option(name.encode(), int(value))
+    if st:
+        raise GqError(st, f"unknown option {name}")
+
+
+def precompile_pipeline(col_dtypes, nrows, preds=(), probes=(), exprs=(), keys=(), ndependent=0, aggs=(), max_groups=1,
+                        check_dependent=False):
     """Compile (or find cached) the fused kernel of a plan shape; needs no GPU. Returns the cubin path."""
     m = _M()
     b = m.batch([None] * len(col_dtypes), dtypes=list(col_dtypes), nrows=int(nrows))
-    plan = _Plan(C.pointer(b), m.agg_desc(preds, probes, exprs, keys, ndependent, aggs, max_groups), None, 0, 0, 0)
+    plan = _Plan(C.pointer(b), m.agg_desc(preds, probes, exprs, keys, ndependent, aggs, max_groups, check_dependent),
+                 None, 0, 0, 0)
     buf = C.create_string_buffer(8192)
     st = lib().gq_precompile_pipeline(C.byref(plan), buf, 8192)
     if st:

@@ -70,6 +70,28 @@ def test_plan_compiler_emits_sm100_tma_kernels(gq, tmp_path):
         L.gq_set_kernel_cache_dir(None)
 
 
+def test_plan_compiler_covers_probes_of_duplicate_key_tables(gq):
+    # one-row-at-a-time row code (a probed table may hold duplicate keys): every consumer compiles (no GPU needed)
+    I8, I32, I64 = gq.I8, gq.I32, gq.I64
+    col = lambda i: ("col", i)
+    multi, uniq = gq.describe_table([I32], unique=False), gq.describe_table([I32], unique=True)
+    ex, ag = [[col(2), col(3), ("mul",)]], [("sum", 0), ("count",)]
+    for kw in (dict(keys=[], max_groups=1), dict(keys=[1], max_groups=6), dict(keys=[0], max_groups=100_000),
+               dict(keys=[0, 3], ndependent=1, max_groups=100_000, check_dependent=True)):
+        assert os.path.exists(gq.precompile_pipeline([I64, I8, I64], 1_000_000, probes=[(multi, 0)], exprs=ex, aggs=ag, **kw))
+    # multiset step followed by a unique step whose key is the group key: hashed group-by, not direct aggregation
+    assert os.path.exists(gq.precompile_pipeline([I64, I64, I64], 1_000_000, probes=[(multi, 0), (uniq, 1)], exprs=ex,
+                                                 keys=[1], aggs=ag, max_groups=100_000))
+    assert os.path.exists(gq.precompile_build([I64, I64], 1_000_000, probes=[(multi, 0)], key=1, payload=[2]))
+    assert os.path.exists(gq.precompile_materialise([I64, I64], 1_000_000, probes=[(multi, 0)], exprs=[[col(2)], [col(1)]]))
+
+
+def test_options(gq):
+    L = gq.lib()
+    assert L.gq_set_option(b"part_min_rows", 4096) == 0 and L.gq_set_option(b"part_min_rows", -1) == 0
+    assert L.gq_set_option(b"no_such_option", 1) == 1 and L.gq_set_option(None, 1) == 1
+
+
 def test_no_device_context_fails_loudly(gq):
     import torch
     if torch.cuda.is_available():

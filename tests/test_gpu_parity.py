@@ -66,6 +66,59 @@ def test_golden_T1_to_T5(ctx):
     assert [list(map(int, r)) for r in zip(*got["cols"])] == G["T5"]["expect"]
 
 
+def _rows(cols):
+    return [list(map(int, r)) for r in zip(*cols)]
+
+
+def test_golden_T6_topk_ties(ctx):
+    # S11 ties through every top-k route: direct (slot-indexed) state, hashed state, packed two-key state (signed
+    # second key), and a low-cardinality state finished with top-k
+    import gqrun
+    from test_oracle_pins import t6_plans
+    t, pair = t6_plans()
+    for k in (3, 4, 10):
+        exp, got = check(plans.plan_c3(t, topk=k), ctx, out_capacity=k)
+        assert _rows(got["cols"]) == G["T6"][f"expect_top{k}"]
+    plan = plans.plan_c3(t)
+    tables = gqrun.build_tables(ctx, plan)
+    st = ctx.aggregate(None, gqrun.dev(plan["table"]), preds=plan["preds"], probes=[(tables[0], 0)], exprs=plan["exprs"],
+                       keys=plan["keys"], aggs=plan["aggs"], max_groups=100)          # hashed route (table-agnostic workspace)
+    r = ctx.aggregate_finish(st, capacity=3, topk=3, topk_agg=0)
+    ctx.sync()
+    assert int(r["n"].item()) == 3
+    assert _rows([r["keys"][0].cpu().numpy()] + [a.cpu().numpy() for a in r["aggs"]])[:3] == G["T6"]["expect_top3"]
+    for k in (3, 5):
+        for mg in (5000, 6):
+            exp, got = check(dict(pair(k), max_groups=mg), ctx, out_capacity=k)
+            assert _rows(got["cols"]) == G["T6"][f"expect_pair_top{k}"]
+
+
+def test_golden_T7_wrapping_sums(ctx):
+    # S6: running sums wrap modulo 2^64 on every aggregation route (RED.ADD at L2, thread-private cells, registers)
+    from test_oracle_pins import t7_plan
+    rows = G["T7"]["rows"]
+    for mg in (5000, 4):                                          # high-cardinality table / low-cardinality fused finaliser
+        exp, got = check(t7_plan(rows, max_groups=mg), ctx)
+        assert _rows(got["cols"]) == G["T7"]["expect"] and exp.overflow
+    exp, got = check(t7_plan(rows, keys=()), ctx)                 # key-less: registers -> shuffle -> last-CTA merge
+    assert _rows(got["cols"]) == G["T7"]["expect_global"]
+    t = table(G["T7"]["cols"], rows)                              # direct aggregation: group key = key of a unique probe
+    dim = dict(table=[np.array([4, 2, 1, 3, 9], np.int64)], preds=[], probes=[], key=0, payload=[], unique=True)
+    plan = dict(builds=[dim], table=[t["key"], t["v"]], preds=[], probes=[(0, 0)], exprs=[[("col", 1)]], keys=[0],
+                aggs=[("sum", 0), ("min", 0), ("max", 0), ("count",)], max_groups=5)
+    exp, got = check(plan, ctx)
+    assert _rows(got["cols"]) == G["T7"]["expect"]
+    # many rows: 2^20 + 3 rows of 2^62 on one key wrap the sum 2^18 times; hot-key / warp-level paths included
+    n = (1 << 22) + 3
+    k = np.where(np.arange(n) % 4 == 0, 1, np.arange(n) % 1000 + 2).astype(np.int64)
+    v = np.where(k == 1, 1 << 62, 3).astype(np.int64)
+    for mg in (2000, 0):
+        plan = dict(table=[k, v], preds=[], exprs=[[("col", 1)]], keys=[0] if mg else [], aggs=[("sum", 0), ("count",)],
+                    max_groups=max(mg, 1))
+        exp, got = check(plan, ctx)
+        assert exp.overflow
+
+
 # ------------------------------------------------------------------ configs at sizes spanning many tiles + ragged tail
 @pytest.mark.parametrize("cfg,scale", [(1, 1.0), (1, 0.0371), (2, 0.0333333), (3, 0.02), (4, 0.02), (5, 0.003), (5, 0.0101)])
 def test_config_small(ctx, cfg, scale):

@@ -167,12 +167,138 @@ def test_lowcard_more_groups_than_declared_is_an_error():
     assert p.result()["n"] == 9
 
 
+def test_lowcard_single_int8_key_with_negative_values(ctx):
+    # {key32, gid} entries of the shared-memory key table: a sign-extended -1 must not be mistaken for an EMPTY entry
+    import gqrun
+    rng = np.random.default_rng(21)
+    n = 90_001
+    k = rng.choice(np.array([-128, -1, 0, 5, 127], np.int8), n)
+    v = rng.integers(-1000, 1000, n).astype(np.int64)
+    plan = dict(table=[k, v], preds=[], exprs=[[("col", 1)]], keys=[0], aggs=[("sum", 0), ("min", 0), ("max", 0), ("count",)],
+                max_groups=5)
+    exp, got = run(plan, ctx)                                  # fused one-kernel pipeline
+    assert set(got["cols"][0].tolist()) == {-128, -1, 0, 5, 127}
+    cols = gqrun.dev(plan["table"])
+    st = None
+    for lo, hi in ((0, 4096), (4096, n)):                      # streaming state (global table behind the shared cells)
+        st = ctx.aggregate(st, [c[lo:hi] for c in cols], exprs=plan["exprs"], keys=[0], aggs=plan["aggs"], max_groups=5)
+    r = ctx.aggregate_finish(st, capacity=8)
+    ctx.sync()
+    ng = int(r["n"].item())
+    got = gqrun.sort_rows([r["keys"][0][:ng].cpu().numpy().astype(np.int64)] + [a[:ng].cpu().numpy() for a in r["aggs"]], 1)
+    for g, e in zip(got, exp.cols):
+        assert np.array_equal(g, e)
+    # only -1 present: the one key that used to vanish
+    plan = dict(table=[np.full(5000, -1, np.int8), np.ones(5000, np.int64)], preds=[], exprs=[[("col", 1)]], keys=[0],
+                aggs=[("sum", 0)], max_groups=3)
+    exp, got = run(plan, ctx)
+    assert got["n"] == 1 and int(got["cols"][1][0]) == 5000
+
+
+# ------------------------------------------------------------------ probes of tables with duplicate keys (multiset, S3)
+def _multiset_plan(rng, nb, nf, keys, aggs, max_groups, ndependent=0, dup=4):
+    """fact(fk, grp8, v) JOIN build(key with duplicates, attr) — every matching pair counts (inner join)."""
+    bkey = rng.integers(0, nb // dup, nb).astype(np.int64) * 3 - 100          # ~dup rows per key, some keys absent
+    attr = (bkey % 17).astype(np.int32)                                       # functionally dependent on the key
+    bsel = rng.integers(0, 3, nb).astype(np.int8)
+    fk = (rng.integers(-20, nb // dup + 20, nf).astype(np.int64)) * 3 - 100   # dangling fks too (S4)
+    grp = rng.integers(-2, 3, nf).astype(np.int8)
+    v = rng.integers(-10**9, 10**9, nf).astype(np.int64)
+    build = dict(table=[bkey, attr, bsel], preds=[(2, "ne", 0)], probes=[], key=0, payload=[1], unique=False)
+    return dict(builds=[build], table=[fk, grp, v], preds=[(2, "gt", -900_000_000)], probes=[(0, 0)],
+                exprs=[[("col", 2), ("col", 3), ("mul",)], [("col", 3)]], keys=keys, ndependent=ndependent, aggs=aggs,
+                max_groups=max_groups)
+
+
+@pytest.mark.parametrize("consumer", ["global", "lowcard", "highcard", "highcard_dep"])
+def test_fused_pipeline_over_duplicate_key_build(ctx, consumer):
+    rng = np.random.default_rng(31)
+    aggs = [("sum", 0), ("min", 1), ("max", 0), ("count",)]
+    keys, mg, ndep = {"global": ([], 1, 0), "lowcard": ([1], 5, 0), "highcard": ([0], 30_000, 0),
+                      "highcard_dep": ([0, 3], 30_000, 1)}[consumer]
+    plan = _multiset_plan(rng, 40_000, 250_003, keys, aggs, mg, ndep)
+    exp, got = run(plan, ctx)
+    assert exp.input_rows > 250_003                              # rows really fan out
+    assert int(got["cols"][-1].sum()) == exp.input_rows          # I2: join cardinality
+
+
+def test_fused_pipeline_over_duplicate_key_build_large_and_chained(ctx):
+    import gqrun
+    rng = np.random.default_rng(32)
+    # >= 2^22 fact rows: the size at which unique-probe plans switch the heavy-hitter pass on (it must stay off here)
+    plan = _multiset_plan(rng, 60_000, (1 << 22) + 777, [0], [("sum", 0), ("count",)], 40_000, dup=3)
+    exp, got = run(plan, ctx)
+    assert int(got["cols"][-1].sum()) == exp.input_rows
+    # chained join THROUGH a multiset table: orders-like build probes the duplicate-key table, fact probes the result
+    nb = 20_000
+    ckey = rng.integers(0, 3000, nb).astype(np.int64)                          # duplicates
+    cval = rng.integers(0, 5, nb).astype(np.int8)
+    okey = rng.permutation(50_000).astype(np.int64)
+    ocust = rng.integers(-10, 3100, 50_000).astype(np.int64)
+    fk = rng.integers(0, 52_000, 300_001).astype(np.int64)
+    v = rng.integers(0, 10**6, 300_001).astype(np.int64)
+    b0 = dict(table=[ckey, cval], preds=[(1, "lt", 2)], probes=[], key=0, payload=[1], unique=False)
+    b1 = dict(table=[okey, ocust], preds=[], probes=[(0, 1)], key=0, payload=[2], unique=False,   # fans out: NOT unique,
+              max_rows=400_000)                                     # and more rows are inserted than the batch has
+    plan = dict(builds=[b0, b1], table=[fk, v], preds=[], probes=[(1, 0)], exprs=[[("col", 1), ("col", 2), ("add",)]],
+                keys=[0], aggs=[("sum", 0), ("count",)], max_groups=60_000)
+    exp, got = run(plan, ctx)
+    assert exp.input_rows > 0 and int(got["cols"][-1].sum()) == exp.input_rows
+    # and a unique dimension joined after the multiset step, grouped by the dimension's key (no direct aggregation here)
+    dkey = np.arange(-2, 3, dtype=np.int64)
+    plan = _multiset_plan(rng, 30_000, 200_000, [1], [("sum", 0), ("count",)], 10_000)
+    plan["builds"].append(dict(table=[dkey], preds=[], probes=[], key=0, payload=[], unique=True))
+    plan["probes"].append((1, 1))
+    run(plan, ctx)
+
+
+def test_check_dependent_flag_catches_a_false_declaration(ctx):
+    # S17: a key declared functionally dependent is stored, not hashed. With GQ_F_CHECK_DEPENDENT a false declaration
+    # is a sticky error instead of silently merged groups; a true one gives the oracle's tuple-grouped result.
+    import gqrun
+    from paper_2606_24647_b200 import gq
+    rng = np.random.default_rng(41)
+    n = 120_000
+    k = rng.integers(0, 5000, n).astype(np.int64)
+    dep_true = (k * 7 % 1000).astype(np.int32)
+    v = rng.integers(0, 100, n).astype(np.int64)
+    plan = dict(table=[k, dep_true, v], preds=[], exprs=[[("col", 2)]], keys=[0, 1], ndependent=1,
+                aggs=[("sum", 0), ("count",)], max_groups=6000)
+    exp = oracle.run_query(plan)
+    for force_part in (False, True):
+        if force_part:
+            gq.set_option("part_min_table_mb", 0); gq.set_option("part_min_rows", 4096)
+        try:
+            c = gq.Context()
+            p2 = c.prepare_pipeline(gqrun.dev(plan["table"]), exprs=plan["exprs"], keys=[0, 1], ndependent=1, aggs=plan["aggs"],
+                                    max_groups=6000, check_dependent=True)
+            p2.run(); c.sync()
+            r = p2.result()
+            got = gqrun.sort_rows([x.cpu().numpy().astype(np.int64) for x in r["keys"]] + [a.cpu().numpy() for a in r["aggs"]], 2)
+            assert r["n"] == exp.nrows and all(np.array_equal(g, e) for g, e in zip(got, exp.cols))
+            dep_false = dep_true.copy()
+            dep_false[n // 2] += 1                                  # ONE row breaks the dependency
+            p3 = c.prepare_pipeline(gqrun.dev([k, dep_false, v]), exprs=plan["exprs"], keys=[0, 1], ndependent=1,
+                                    aggs=plan["aggs"], max_groups=6000, check_dependent=True)
+            p3.run()
+            with pytest.raises(gq.GqError) as e:
+                c.sync()
+            assert e.value.status == 8                              # GQ_ERR_DEPENDENT_KEY
+            c.clear_error(); c.sync()
+        finally:
+            gq.set_option("part_min_table_mb", -1); gq.set_option("part_min_rows", -1)
+
+
 # ------------------------------------------------------------------ radix-clustered (partitioned) aggregation
 @pytest.fixture
-def force_partition(monkeypatch):
-    # thresholds that switch the partitioned path on for tables and batches the oracle can check in seconds
-    monkeypatch.setenv("GQ_TUNE_PART_MIN_TABLE_MB", "0")
-    monkeypatch.setenv("GQ_TUNE_PART_MIN_ROWS", "4096")
+def force_partition():
+    # planner thresholds that switch the partitioned path on for tables and batches the oracle can check in seconds
+    from paper_2606_24647_b200 import gq
+    gq.set_option("part_min_table_mb", 0)
+    gq.set_option("part_min_rows", 4096)
+    yield
+    gq.set_option("part_min_table_mb", -1)
+    gq.set_option("part_min_rows", -1)
 
 
 @pytest.mark.parametrize("scale", [0.003, 0.0101])

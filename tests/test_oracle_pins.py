@@ -81,6 +81,43 @@ def test_T5_extreme_keys_min_max():
     assert r.input_rows == G["T5"]["rows_passing"]
 
 
+def t6_plans():
+    d, f = table(G["T6"]["dim_cols"], G["T6"]["dim"]), table(G["T6"]["fact_cols"], G["T6"]["fact"])
+    t = {"dim": d, "fact": dict(fk=f["fk"], shipdate=f["shipdate"], price=f["price"], discount=f["disc"])}
+    p = table(G["T6"]["pair_cols"], G["T6"]["pair_rows"])
+    pair = lambda k: dict(table=[p["a"], p["b"], p["v"]], preds=[], exprs=[[("col", 2)]], keys=[0, 1],
+                          aggs=[("sum", 0)], topk=k, topk_agg=0, max_groups=5000)
+    return t, pair
+
+
+def test_T6_topk_ties_are_decided_by_the_key():
+    # S11: (aggregate desc, key tuple asc). Keys 3, 5, 9 tie at 1000 and k = 3 cuts through the tie; reversing the
+    # oracle's tie-break (or comparing keys unsigned) changes these lists.
+    t, pair = t6_plans()
+    r = oracle.run_query(plans.plan_c3(t))
+    assert _rows(r) == G["T6"]["expect"] and r.input_rows == G["T6"]["join_rows"]
+    for k in (3, 4, 10):
+        assert _rows(oracle.run_query(plans.plan_c3(t, topk=k))) == G["T6"][f"expect_top{k}"]
+    for k in (3, 5):
+        assert _rows(oracle.run_query(pair(k))) == G["T6"][f"expect_pair_top{k}"]
+
+
+def t7_plan(rows, keys=(0,), max_groups=5000):
+    t = table(G["T7"]["cols"], rows)
+    aggs = [("sum", 0), ("min", 0), ("max", 0), ("count",)] if keys else [("sum", 0), ("count",)]
+    return dict(table=[t["key"], t["v"]], preds=[], exprs=[[("col", 1)]], keys=list(keys), aggs=aggs, max_groups=max_groups)
+
+
+def test_T7_running_sum_wraps_and_is_flagged():
+    # S6: the running SUM wraps modulo 2^64 and the __int128 shadow raises the flag; no single value overflows here
+    r = oracle.run_query(t7_plan(G["T7"]["rows"]))
+    assert _rows(r) == G["T7"]["expect"] and r.overflow == bool(G["T7"]["expect_overflow"])
+    g = oracle.run_query(t7_plan(G["T7"]["rows"], keys=()))
+    assert _rows(g) == G["T7"]["expect_global"] and g.overflow
+    n = oracle.run_query(t7_plan(G["T7"]["rows_no_wrap"]))
+    assert _rows(n) == G["T7"]["expect_no_wrap"] and not n.overflow      # INT64_MAX reached exactly: no wrap, no flag
+
+
 # ------------------------------------------------------------------ joins: brute force, duplicates, dangling
 @pytest.mark.parametrize("seed", [1, 2, 3])
 def test_join_equals_bruteforce_with_duplicates_and_dangling(seed):
