@@ -1,8 +1,27 @@
-"""Full-size parity (-m gpu): BASELINE.json's C3, C4 and C5 at their full row counts, in the launch configuration
-bench.py times (same cardinality hints, same pipelines). The oracle cannot evaluate 60-600 M rows in test time, so the
-check is (a) invariants that hold at any size, computed from the inputs with plain numpy selections and wrapping sums
-(SURVEY §8(c) I1/I3), and (b) SAMPLED groups compared one by one, bit-exactly, with the oracle run on exactly the input
-rows that can contribute to them (selecting rows is input preparation; all arithmetic is the oracle's)."""
+"""Full-size parity (-m gpu): BASELINE.json's C2-C5 at their full row counts, in the launch configuration bench.py
+times (same cardinality hints, same pipelines). The WHOLE result table is compared with the oracle's through the digests
+of tests/golden/fullsize_digests.json (written by tests/golden/make_fullsize_digests.py from oracle/ + datagen only: group
+count, rows fed to GROUP BY, and per output column in key order the wrapping sum, xor and SHA-256 — SURVEY §8(c) "full
+table exact"). When a digest differs, the older checks localise it: (a) invariants computed from the inputs with plain
+numpy selections and wrapping sums (I1/I3), (b) SAMPLED groups compared one by one with the oracle run on exactly the
+input rows that can contribute to them (selecting rows is input preparation; all arithmetic is the oracle's)."""
+import json
+import os
+
+from golden_util import digest_columns
+
+with open(os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden", "fullsize_digests.json")) as _f:
+    DIGESTS = json.load(_f)
+
+
+def _check_digest(cfg, got):
+    d = DIGESTS[f"C{cfg}"]
+    assert got["n"] == d["ngroups"], f"C{cfg}: {got['n']} groups, the oracle has {d['ngroups']}"
+    mine = digest_columns(got["cols"])
+    for c, (a, b) in enumerate(zip(mine, d["columns"])):
+        assert a == b, f"C{cfg}: output column {c} differs from the oracle's full table (digest)"
+    assert len(mine) == len(d["columns"])
+
 import numpy as np
 import pytest
 
@@ -46,6 +65,13 @@ def _sample_check(plan, got, nkeys_out, rows_of, rng, nsample=48):
     assert not exp.overflow
 
 
+def test_c2_full_size(ctx):
+    plan = plans.plan_c2(datagen.make_config(2))
+    got = _gpu(plan, ctx)
+    _check_digest(2, got)
+    assert int(got["cols"][1][0]) == DIGESTS["C2"]["input_rows"]
+
+
 def test_c3_full_size(ctx):
     t = datagen.make_config(3)
     plan = plans.plan_c3(t)
@@ -53,6 +79,7 @@ def test_c3_full_size(ctx):
     plan["max_groups"] = plan["builds"][0]["max_rows"]
     got = _gpu(plan, ctx)
     d, f = t["dim"], t["fact"]
+    assert int(got["cols"][2].sum()) == DIGESTS["C3"]["input_rows"]
     dkeys = d["key"][d["orderdate"] < 1200]
     live = (f["shipdate"] > 1200) & np.isin(f["fk"], dkeys)
     assert int(got["cols"][2].sum()) == int(live.sum())                               # I1/I2: sum of COUNT = join cardinality
@@ -65,11 +92,13 @@ def test_c3_full_size(ctx):
         sub = plans.plan_c3({"dim": {k: v[dm] for k, v in d.items()}, "fact": {k: v[fm] for k, v in f.items()}})
         return sub
     _sample_check(plan, got, 1, rows_of, np.random.default_rng(3))
-    # top-10 through the top-k finaliser = first 10 of the full result ordered by (sum desc, key asc)
+    _check_digest(3, got)                                                              # the whole 6.5 M-row table
+    # top-10 through the top-k finaliser = the oracle's top-10 (sum desc, key asc), in order
     top = _gpu(dict(plan, topk=10, topk_agg=0), ctx, out_capacity=10)
-    order = np.lexsort((got["cols"][0], -got["cols"][1]))[:10]
-    for c in range(3):
-        assert np.array_equal(top["cols"][c], got["cols"][c][order])
+    assert [[int(c[i]) for c in top["cols"]] for i in range(top["n"])] == DIGESTS["C3"]["top10"]
+    # and with the build side sized from its INPUT row count (no selectivity knowledge): same table
+    plan_ub = plans.plan_c3(t)
+    _check_digest(3, _gpu(plan_ub, ctx))
 
 
 def test_c4_full_size(ctx):
@@ -97,6 +126,8 @@ def test_c4_full_size(ctx):
         return plans.plan_c4({"cust": {k: v[cm] for k, v in c.items()}, "orders": {k: v[omk] for k, v in o.items()},
                               "fact": {k: v[fm] for k, v in f.items()}})
     _sample_check(plan, got, 2, rows_of, np.random.default_rng(4))
+    _check_digest(4, got)                                                              # the whole 1.3 M-row table
+    _check_digest(4, _gpu(plans.plan_c4(t), ctx))                                      # upper-bound sizing: same table
 
 
 def test_c5_full_size(ctx):
@@ -124,3 +155,4 @@ def test_c5_full_size(ctx):
     assert exp.nrows == int(sel.sum())
     for c in range(len(exp.cols)):
         assert np.array_equal(got["cols"][c][sel], exp.cols[c]), f"sampled groups: column {c} differs"
+    _check_digest(5, got)                                                              # the whole 34.2 M-row table
