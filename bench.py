@@ -256,27 +256,6 @@ def oracle_rate(plans, datagen, cfg, sample_rows, reps=1):
     return n / best, n, best
 
 
-def main_random_probe():
-    """--random-probe: random 8-byte access rates over tables of growing size (what bounds the hash phases)."""
-    import torch
-    from paper_2606_24647_b200 import build as gqbuild
-    gqbuild.build()
-    from paper_2606_24647_b200 import gq
-    ctx = gq.Context(0)
-    n = 64 << 20
-    modes = {0: "load", 1: "red", 2: "load+2red/slot", 3: "cas"}
-    rows = []
-    for mb in (16, 64, 128, 256, 1024, 4096):
-        tab = torch.zeros(mb << 17, dtype=torch.int64, device="cuda")      # mb MiB
-        for mode, name in modes.items():
-            ctx.random_probe(tab, n, mode)
-            ms = time_steps(torch, ctx.stream, lambda: ctx.random_probe(tab, n, mode), 3, 1, lambda: None) / 3
-            rows.append(dict(table_mib=mb, op=name, ms=ms, g_accesses_per_s=n / ms / 1e6))
-        del tab
-        torch.cuda.empty_cache()
-    print(json.dumps(dict(random_probe=rows, accesses=n)))
-
-
 def main_reference(args):
     """--impl reference: the CPU oracle (this tier's reference arm) on the box's host cores, rank 0 only."""
     ws, rank, _ = dist()
@@ -318,14 +297,11 @@ def main():
                     "NxS = config N at S times its rows (C1x64: the low-cardinality pipeline at steady state)")
     ap.add_argument("--c5-scale", type=float, default=1.0)
     ap.add_argument("--no-cpu-baseline", action="store_true")
-    ap.add_argument("--random-probe", action="store_true", help="measurement aid: random-access rates vs table size")
     ap.add_argument("--no-headline", action="store_true", help="profiling aid: only the --configs entries, printed as JSON")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3)
     if args.impl == "reference":
         return main_reference(args)
-    if args.random_probe:
-        return main_random_probe()
 
     import torch
     import gqrun

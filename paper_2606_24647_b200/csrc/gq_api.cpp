@@ -157,7 +157,7 @@ std::string signature(const GqScanSpec& sp) {
   put(sp.lc_cap); put(sp.lc_key_bits); put(sp.target_sw); put(sp.build_key_col);
   for (int c : sp.payload_cols) put(c);
   put(sp.unique); put(sp.hot); put(sp.check_dep); put(sp.fused_final); put(sp.direct_step); put(sp.direct_aw); put(sp.direct_touch);
-  put(sp.part_rw); for (int e : sp.part_exprs) put(e);
+  put(sp.part_rw); put(sp.part_states); for (int e : sp.part_exprs) put(e);
   s += 'c';
   std::vector<long long> kv; std::vector<int> ki;
   collect_consts(sp, &kv, &ki);
@@ -194,6 +194,37 @@ gq_status get_kernel_info(const GqScanSpec& sp_in, CachedKernel** out, std::stri
   return GQ_OK;
 }
 
+// JIT (cached) of a generated kernel for the context's device.
+gq_status load_kernel(gq_ctx* ctx, CachedKernel* ck, GqKernel* kern) {
+  std::lock_guard<std::mutex> l(g_kmu);   // distinct contexts may launch the same plan shape for the first time concurrently (gq.h "Threads")
+  if (!ck->loaded || ck->device != ctx->device) {
+    cudaSetDevice(ctx->device);
+    gq_status st = gq_jit_get(ck->info, ctx->device, &ck->k, &ctx->msg, &ctx->last_cuda);
+    if (st != GQ_OK) return st;
+    ck->loaded = true;
+    ck->device = ctx->device;
+  }
+  *kern = ck->k;
+  return GQ_OK;
+}
+
+// Pass B kernel of the partitioned shared-memory aggregation for this plan shape (cached by shape).
+gq_status get_psa_kernel_info(const GqScanSpec& sp, int log2slots, const int* src, CachedKernel** out, std::string* msg) {
+  std::string sig = "psa:" + std::to_string(log2slots) + "," + std::to_string(sp.target_sw) + "," + std::to_string(sp.part_rw) + "," +
+                    std::to_string(sp.ndep) + "," + std::to_string(sp.check_dep) + ";";
+  for (size_t a = 0; a < sp.aggs.size(); ++a) sig += std::to_string((int)sp.aggs[a].op) + ":" + std::to_string(src[a]) + ",";
+  std::lock_guard<std::mutex> l(g_kmu);
+  auto it = g_kernels.find(sig);
+  if (it == g_kernels.end()) {
+    CachedKernel ck;
+    gq_status st = gq_codegen_psa(sp, log2slots, src, &ck.info, msg);
+    if (st != GQ_OK) return st;
+    it = g_kernels.emplace(sig, std::move(ck)).first;
+  }
+  *out = &it->second;
+  return GQ_OK;
+}
+
 // Codegen (cached) -> JIT (cached) -> parameters -> launch of one fused scan kernel.
 gq_status run_scan(gq_ctx* ctx, const GqScanSpec& sp, const gq_batch* in, const gq_probe_step* probes,
                    GqParams* P /* target/acc/out/out_count pre-filled */) {
@@ -201,17 +232,8 @@ gq_status run_scan(gq_ctx* ctx, const GqScanSpec& sp, const gq_batch* in, const 
   gq_status st = get_kernel_info(sp, &ck, &ctx->msg);
   if (st != GQ_OK) return st;
   GqKernel kern;
-  {   // distinct contexts may launch the same plan shape for the first time concurrently (gq.h "Threads")
-    std::lock_guard<std::mutex> l(g_kmu);
-    if (!ck->loaded || ck->device != ctx->device) {
-      cudaSetDevice(ctx->device);
-      st = gq_jit_get(ck->info, ctx->device, &ck->k, &ctx->msg, &ctx->last_cuda);
-      if (st != GQ_OK) return st;
-      ck->loaded = true;
-      ck->device = ctx->device;
-    }
-    kern = ck->k;
-  }
+  st = load_kernel(ctx, ck, &kern);
+  if (st != GQ_OK) return st;
   for (size_t c = 0; c < ck->info.cols.size(); ++c) P->col[c] = in->cols[ck->info.cols[c]].data;
   P->nrows = in->nrows;
   std::vector<long long> k;
@@ -588,6 +610,71 @@ PartPlan part_plan(const GqScanSpec& sp, const gq_agg_desc* d, int64_t nrows) {
   return pp;
 }
 
+// Partitioned shared-memory aggregation (gq_psa_kernel.cuh): the single-batch path of gq_pipeline for
+// high-cardinality group-bys whose table would be far larger than L2. Pass A (SCATTER consumer) appends one record per
+// surviving row to CTA-private chunks of the key's partition; pass B aggregates every partition in a shared-memory
+// table and writes the dense result. No global group-by table, no global atomics on the per-row path.
+struct PsaPlan {
+  bool on = false;
+  int npart = 0, log2npart = 0, log2slots = 0, rw = 0;
+  std::vector<int> exprs; int src[GQ_MAX_AGGS];
+  int64_t chunks_bound = 0, merge_cap = 0;
+  uint32_t seg_chunks = 0, max_items = 0;
+  size_t off_zero = 0, zero_bytes = 0, off_pcount = 0, off_pfill = 0, off_pstart = 0, off_items = 0, off_itemseg = 0, off_ncta = 0,
+         off_info = 0, off_plist = 0, off_merge = 0, merge_bytes = 0, off_rec = 0, bytes = 0;
+};
+const int64_t GQ_PSA_MAX_TILE = 4096;   // upper bound of the scan kernel's tile (rows): bounds a CTA's share of the rows
+PsaPlan psa_plan(const GqScanSpec& sp, const gq_agg_desc* d, int64_t nrows, int topk) {
+  PsaPlan pp;
+  if (sp.consumer != GQ_C_HIGHCARD || topk != 0 || d->nkeys < 1) return pp;
+  for (const GqProbeSpec& ps : sp.probes) if (!ps.unique) return pp;
+  const int sw = sp.target_sw;
+  if ((int64_t)agg_capacity(d->max_groups, d->nkeys) * sw * 8 < g_part_min_table_mb.load() * (1 << 20) || nrows < g_part_min_rows.load()) return pp;
+  int L = 6;
+  while ((((1LL << (L + 1)) + 1) * sw + 2 * 66) * 8 + 64 <= GQ_SMEM_LIMIT) ++L;
+  if ((((1LL << L) + 1) * sw + 2 * 66) * 8 + 64 > GQ_SMEM_LIMIT) return pp;
+  pp.log2slots = L;
+  const int64_t slots = 1LL << L, limit = slots - slots / 8 - 512;
+  if (limit < 32) return pp;
+  int lp = 6;                                               // 64 .. 16384 partitions; more groups than that: the key
+  while (lp < 14 && (d->max_groups + limit - 1) / limit > (1LL << lp)) ++lp;   // ranges are halved in pass B instead
+  pp.log2npart = lp; pp.npart = 1 << lp;
+  for (int a = 0; a < d->naggs; ++a) {
+    pp.src[a] = -1;
+    if (d->aggs[a].op == GQ_COUNT_STAR) continue;
+    size_t i = 0;
+    while (i < pp.exprs.size() && pp.exprs[i] != d->aggs[a].expr) ++i;
+    if (i == pp.exprs.size()) pp.exprs.push_back(d->aggs[a].expr);
+    pp.src[a] = 1 + d->ndependent + (int)i;
+  }
+  pp.rw = (int)align_up((size_t)(1 + d->ndependent + pp.exprs.size()), 4);
+  // every pass-A CTA owns a private range of chunk ids: its share of the rows / 32, plus one part-filled chunk per partition
+  pp.chunks_bound = nrows / GQ_PART_CHUNK + (int64_t)GQ_MAX_SMS * (pp.npart + 2 * GQ_PSA_MAX_TILE / GQ_PART_CHUNK + 2);
+  if (pp.chunks_bound >= (1LL << GQ_PSA_GID_BITS) || nrows / GQ_PART_CHUNK + pp.npart + 300 >= (1LL << 20)* GQ_MAX_SMS) return pp;
+  // a partition is "heavy" (cut into segments for several CTAs) when it is far above the average AND a sizeable share of all work
+  pp.seg_chunks = (uint32_t)std::max<int64_t>(std::max<int64_t>(64, pp.chunks_bound / 512), 4 * pp.chunks_bound / pp.npart);
+  pp.max_items = (uint32_t)(pp.npart + 2 * (pp.chunks_bound / pp.seg_chunks) + 2);
+  pp.merge_cap = table_capacity(std::min<int64_t>(std::max<int64_t>(1, d->max_groups), (pp.chunks_bound / pp.seg_chunks + 1) * limit));
+  size_t off = 0;
+  auto take = [&off](size_t b) { size_t o = off; off += align_up(b, 256); return o; };
+  pp.off_zero = take(256);                                   // [0] work cursor, [1] item count
+  pp.off_pcount = take((size_t)pp.npart * 4);
+  pp.off_pfill = take((size_t)pp.npart * 4);
+  pp.zero_bytes = off;                                       // zeroed before every run
+  pp.off_pstart = take((size_t)(pp.npart + 1) * 4);
+  pp.off_items = take((size_t)pp.max_items * 4);
+  pp.off_itemseg = take((size_t)pp.max_items * 4);
+  pp.off_ncta = take((size_t)GQ_MAX_SMS * 4);
+  pp.off_info = take((size_t)pp.chunks_bound * 4);
+  pp.off_plist = take((size_t)pp.chunks_bound * 4);
+  pp.merge_bytes = ws_layout(pp.merge_cap, sw, 1).total;
+  pp.off_merge = take(pp.merge_bytes);
+  pp.off_rec = take((size_t)pp.chunks_bound * GQ_PART_CHUNK * pp.rw * 8);
+  pp.bytes = off;
+  pp.on = true;
+  return pp;
+}
+
 }  // namespace
 
 extern "C" {
@@ -720,7 +807,7 @@ gq_status gq_hash_aggregate(gq_ctx* ctx, gq_aggstate** state, void* d_ws, size_t
     // radix-clustered: pass A appends records per table partition, pass B applies them partition by partition
     PartPlan pp = part_plan(sp, d, a->part_rows);
     if (!pp.on || pp.rw != a->part_rw || pp.npart != a->npart) return fail(ctx, GQ_ERR_INVALID_ARG, "batch schema/desc differs from the state's first batch");
-    sp.consumer = GQ_C_PARTITION; sp.part_rw = pp.rw; sp.part_exprs = pp.exprs;
+    sp.consumer = GQ_C_PARTITION; sp.part_rw = pp.rw; sp.part_exprs = pp.exprs; sp.part_states = 4096;
     P.part = a->part; P.pcur = a->pcur; P.pcap = a->pcap; P.pshift = a->pshift; P.npart = a->npart;
     cudaError_t e = cudaMemsetAsync(a->pcur, 0, (size_t)a->npart * 8 * GQ_PART_CURSOR_STRIDE, ctx->stream);
     if (e != cudaSuccess) return cuda_fail(ctx, e, "partition cursors");
@@ -795,12 +882,143 @@ static size_t fused_scratch_bytes(const gq_agg_desc* d) {
   return align_up(256 * (g * (1 + (size_t)d->naggs) + 1) * 8, 256);
 }
 
+// Offsets inside a pipeline workspace: [aggregation state][top-k scratch][fused-finaliser scratch][partitioned aggregation]
+struct PipeLayout { size_t aggb = 0, topk_off = 0, fused_off = 0, psa_off = 0, total = 0; PsaPlan psa; };
+static gq_status pipe_layout(gq_ctx* ctx, const gq_plan* plan, GqScanSpec* sp, int kb[2], gq_dtype kd[2], PipeLayout* L) {
+  gq_status st = agg_spec(ctx, sp, plan->in, &plan->agg, kb, kd);
+  if (st != GQ_OK) return st;
+  DirectPlan dp = direct_plan(*sp, &plan->agg, plan->in, true);
+  if (dp.step < 0) L->psa = psa_plan(*sp, &plan->agg, plan->in->nrows, plan->topk);
+  if (L->psa.on) st = gq_hash_aggregate_workspace(plan->agg.max_groups, plan->agg.nkeys, plan->agg.naggs, &L->aggb);   // single-pass fallback state
+  else st = gq_hash_aggregate_workspace_for(plan->in, &plan->agg, &L->aggb);
+  if (st != GQ_OK) return st;
+  L->topk_off = align_up(L->aggb, 256);
+  L->fused_off = L->topk_off + (plan->topk > 0 ? align_up(gq_topk_scratch_bytes_impl(), 256) : 0);
+  L->psa_off = L->fused_off + fused_scratch_bytes(&plan->agg);
+  L->total = L->psa_off + (L->psa.on ? L->psa.bytes : 0);
+  return GQ_OK;
+}
+
 gq_status gq_pipeline_workspace(const gq_plan* plan, size_t* bytes) {
   if (!plan || !plan->in || !bytes) return GQ_ERR_INVALID_ARG;
-  size_t b = 0;
-  gq_status st = gq_hash_aggregate_workspace_for(plan->in, &plan->agg, &b);
+  gq_ctx tmp;
+  GqScanSpec sp;
+  int kb[2]; gq_dtype kd[2] = {GQ_I64, GQ_I64};
+  PipeLayout L;
+  gq_status st = pipe_layout(&tmp, plan, &sp, kb, kd, &L);
   if (st != GQ_OK) return st;
-  *bytes = align_up(b, 256) + (plan->topk > 0 ? align_up(gq_topk_scratch_bytes_impl(), 256) : 0) + fused_scratch_bytes(&plan->agg);
+  *bytes = L.total;
+  return GQ_OK;
+}
+
+// Outputs of a finaliser that runs inside a generated kernel (fused scan finaliser, pass B of the partitioned aggregation).
+static gq_status fill_final(gq_ctx* ctx, const gq_plan* plan, const int kb[2], const gq_dtype kd[2], void* const* out_key_cols,
+                            int64_t* const* out_agg_cols, double* const* out_avg_cols, int64_t out_capacity, int64_t* d_out_ngroups,
+                            GqFinal* F) {
+  const gq_agg_desc* d = &plan->agg;
+  if (!out_agg_cols || !d_out_ngroups || out_capacity < 0 || (d->nkeys > 0 && !out_key_cols)) return fail(ctx, GQ_ERR_INVALID_ARG, "missing outputs");
+  if (plan->navg < 0 || plan->navg > GQ_MAX_AGGS || (plan->navg > 0 && (!plan->avgs || !out_avg_cols))) return fail(ctx, GQ_ERR_INVALID_ARG, "bad avg spec");
+  F->nkeys = d->nkeys; F->navg = plan->navg;
+  for (int k = 0; k < d->nkeys; ++k) {
+    if (!out_key_cols[k]) return fail(ctx, GQ_ERR_INVALID_ARG, "null key output");
+    F->out_key[k] = out_key_cols[k]; F->key_bits[k] = kb[k]; F->key_dtype[k] = (int)kd[k];
+  }
+  for (int i = 0; i < d->naggs; ++i) {
+    if (!out_agg_cols[i]) return fail(ctx, GQ_ERR_INVALID_ARG, "null aggregate output");
+    F->out_agg[i] = (long long*)out_agg_cols[i];
+  }
+  for (int v = 0; v < plan->navg; ++v) {
+    if (plan->avgs[v].sum_agg < 0 || plan->avgs[v].sum_agg >= d->naggs || plan->avgs[v].count_agg < 0 ||
+        plan->avgs[v].count_agg >= d->naggs || !out_avg_cols[v]) return fail(ctx, GQ_ERR_INVALID_ARG, "bad avg spec");
+    F->avg_sum[v] = plan->avgs[v].sum_agg; F->avg_cnt[v] = plan->avgs[v].count_agg; F->out_avg[v] = out_avg_cols[v];
+  }
+  F->out_capacity = out_capacity; F->out_n = (long long*)d_out_ngroups;
+  return GQ_OK;
+}
+
+// The partitioned shared-memory aggregation: zero the counters -> pass A (scan + scatter) -> directory -> pass B ->
+// emit the merge table of split partitions. Five kernels, stream-ordered, no host synchronisation.
+static gq_status run_psa(gq_ctx* ctx, const gq_plan* plan, GqScanSpec sp, const PsaPlan& pp, char* ws, const GqFinal& F) {
+  const gq_agg_desc* d = &plan->agg;
+  const gq_batch* in = plan->in;
+  sp.consumer = GQ_C_SCATTER; sp.hot = false; sp.part_rw = pp.rw; sp.part_exprs = pp.exprs; sp.part_states = pp.npart;
+  CachedKernel* ck = nullptr;
+  gq_status st = get_kernel_info(sp, &ck, &ctx->msg);
+  if (st != GQ_OK) return st;
+  const int64_t tile = ck->info.tile_rows;
+  if (tile > GQ_PSA_MAX_TILE || ctx->num_sms > GQ_MAX_SMS) return fail(ctx, GQ_ERR_UNSUPPORTED, "internal: scatter tile/grid exceeds the workspace bound");
+  const int64_t grid = std::max<int64_t>(1, std::min<int64_t>(ctx->num_sms, in->nrows / tile));
+  const int64_t slab = (in->nrows / grid + 2 * tile) / GQ_PART_CHUNK + pp.npart + 2;
+  if (grid * slab > pp.chunks_bound || slab >= (1LL << 20)) return fail(ctx, GQ_ERR_UNSUPPORTED, "internal: chunk range bound");
+  cudaError_t e = cudaMemsetAsync(ws + pp.off_zero, 0, pp.zero_bytes, ctx->stream);
+  if (e == cudaSuccess) e = cudaMemsetAsync(F.out_n, 0, 8, ctx->stream);
+  if (e != cudaSuccess) return cuda_fail(ctx, e, "partitioned aggregation: memset");
+  // merge table of split (heavy) partitions: ordinary group-by table protocol
+  GqTableDev mt{};
+  {
+    WsLayout w = ws_layout(pp.merge_cap, sp.target_sw, 1);
+    mt.slots = (unsigned long long*)(ws + pp.off_merge + w.slots_off);
+    mt.mask = (unsigned long long)(pp.merge_cap - 1);
+    mt.header = (long long*)(ws + pp.off_merge);
+    mt.side = (unsigned long long*)(ws + pp.off_merge + w.side_off);
+    mt.shift = 64 - log2i(pp.merge_cap);
+    mt.slot_words = sp.target_sw;
+    unsigned long long pat[16];
+    for (int i = 0; i < 16; ++i) pat[i] = 0;
+    pat[0] = GQ_EMPTY_KEY;
+    if (sp.check_dep) pat[1] = GQ_DEP_UNSET;
+    for (int i = 0; i < d->naggs; ++i)
+      pat[1 + d->ndependent + i] = d->aggs[i].op == GQ_MIN ? 0x7FFFFFFFFFFFFFFFULL : d->aggs[i].op == GQ_MAX ? 0x8000000000000000ULL : 0ULL;
+    e = gq_launch_init_table(ctx->stream, mt.slots, pp.merge_cap, sp.target_sw, pat, mt.side, 1, mt.header, 0, ctx->num_sms);
+    if (e != cudaSuccess) return cuda_fail(ctx, e, "merge table init");
+    ++ctx->launches;
+  }
+  auto U = [&](size_t off) { return (unsigned*)(ws + off); };
+  GqParams P;
+  memset(&P, 0, sizeof P);
+  P.part = (unsigned long long*)(ws + pp.off_rec);
+  P.pshift = 64 - pp.log2npart; P.npart = pp.npart;
+  P.sc_info = U(pp.off_info); P.sc_count = U(pp.off_pcount); P.sc_ncta = U(pp.off_ncta); P.sc_slab = slab;
+  e = cudaMemsetAsync(P.sc_ncta, 0, GQ_MAX_SMS * 4, ctx->stream);
+  if (e != cudaSuccess) return cuda_fail(ctx, e, "partitioned aggregation: memset");
+  st = run_scan(ctx, sp, in, d->probes, &P);
+  if (st != GQ_OK) return st;
+  GqPsaDirParams dp{};
+  dp.pcount = U(pp.off_pcount); dp.pstart = U(pp.off_pstart); dp.items = U(pp.off_items); dp.item_seg = U(pp.off_itemseg);
+  dp.nitems = U(pp.off_zero) + 1; dp.npart = pp.npart; dp.seg_chunks = pp.seg_chunks; dp.err = ctx->d_err; dp.max_items = pp.max_items;
+  e = gq_launch_psa_dir(ctx->stream, dp);
+  if (e == cudaSuccess) e = gq_launch_psa_fill(ctx->stream, U(pp.off_info), U(pp.off_ncta), (int)grid, slab, U(pp.off_pstart), U(pp.off_pfill), U(pp.off_plist));
+  if (e != cudaSuccess) return cuda_fail(ctx, e, "partition directory");
+  ctx->launches += 2;
+  CachedKernel* pk = nullptr;
+  st = get_psa_kernel_info(sp, pp.log2slots, pp.src, &pk, &ctx->msg);
+  if (st != GQ_OK) return st;
+  GqKernel kern;
+  st = load_kernel(ctx, pk, &kern);
+  if (st != GQ_OK) return st;
+  GqPsaParams B;
+  memset(&B, 0, sizeof B);
+  B.rec = P.part; B.plist = U(pp.off_plist); B.pstart = U(pp.off_pstart); B.items = U(pp.off_items); B.item_seg = U(pp.off_itemseg);
+  B.nitems = U(pp.off_zero) + 1; B.work = U(pp.off_zero); B.err = ctx->d_err; B.merge = mt; B.seg_chunks = pp.seg_chunks;
+  B.hshift = 64 - pp.log2npart; B.fin = F;
+  void* args[] = {(void*)&B};
+  e = cudaLaunchKernel((const void*)kern.fn, dim3((unsigned)ctx->num_sms), dim3((unsigned)kern.threads), args, (size_t)kern.smem_bytes, ctx->stream);
+  if (e != cudaSuccess) return cuda_fail(ctx, e, "launch of the partitioned aggregation kernel");
+  ++ctx->launches;
+  // groups of split partitions: appended to the same dense output
+  GqFinaliseParams fp;
+  memset(&fp, 0, sizeof fp);
+  fp.slots = mt.slots; fp.capacity = pp.merge_cap; fp.slot_words = sp.target_sw; fp.side = mt.side; fp.header = mt.header;
+  fp.nkeys = d->nkeys; fp.ndep = d->ndependent; fp.naggs = d->naggs;
+  for (int k = 0; k < d->nkeys; ++k) { fp.key_bits[k] = F.key_bits[k]; fp.key_dtype[k] = F.key_dtype[k]; fp.out_key[k] = F.out_key[k]; }
+  for (int i = 0; i < d->naggs; ++i) fp.out_agg[i] = F.out_agg[i];
+  fp.navg = F.navg;
+  for (int v = 0; v < F.navg; ++v) { fp.avg_sum[v] = F.avg_sum[v]; fp.avg_cnt[v] = F.avg_cnt[v]; fp.out_avg[v] = F.out_avg[v]; }
+  fp.out_capacity = F.out_capacity; fp.out_n = F.out_n; fp.err = ctx->d_err;
+  int nl = 0;
+  e = gq_launch_finalise(ctx->stream, fp, ctx->num_sms, &nl);
+  if (e != cudaSuccess) return cuda_fail(ctx, e, "merge table finalise");
+  ctx->launches += nl;
   return GQ_OK;
 }
 
@@ -808,59 +1026,43 @@ gq_status gq_pipeline(gq_ctx* ctx, const gq_plan* plan, void* d_ws, size_t bytes
                       int64_t* const* out_agg_cols, double* const* out_avg_cols, int64_t out_capacity,
                       int64_t* d_out_ngroups) {
   if (!ctx || !plan || !plan->in) return GQ_ERR_INVALID_ARG;
-  size_t need = 0, aggb = 0;
-  gq_status st = gq_pipeline_workspace(plan, &need);
-  if (st != GQ_OK) return fail(ctx, st, "bad plan");
-  if (bytes < need) return fail(ctx, GQ_ERR_WORKSPACE_TOO_SMALL, "pipeline workspace too small");
+  gq_status st = check_batch(ctx, plan->in);
+  if (st != GQ_OK) return st;
+  GqScanSpec sp;
+  int kb[2]; gq_dtype kd[2] = {GQ_I64, GQ_I64};
+  PipeLayout L;
+  st = pipe_layout(ctx, plan, &sp, kb, kd, &L);
+  if (st != GQ_OK) return st;
+  if (bytes < L.total) return fail(ctx, GQ_ERR_WORKSPACE_TOO_SMALL, "pipeline workspace too small");
   if (!d_ws || !aligned(d_ws, 256)) return fail(ctx, GQ_ERR_INVALID_ARG, "bad workspace");
-  gq_hash_aggregate_workspace_for(plan->in, &plan->agg, &aggb);
-  const size_t topk_off = align_up(aggb, 256);
-  const size_t fused_off = topk_off + (plan->topk > 0 ? align_up(gq_topk_scratch_bytes_impl(), 256) : 0);
+  const gq_agg_desc* d = &plan->agg;
 
   // One batch, key-less or low-cardinality, no top-k: ONE kernel — every CTA writes its partial groups, the last CTA
   // to finish merges them and emits the dense result (no table-init and no finalise launch).
-  {
-    const gq_agg_desc* d = &plan->agg;
-    st = check_batch(ctx, plan->in);
+  if ((sp.consumer == GQ_C_GLOBAL || sp.consumer == GQ_C_LOWCARD) && plan->topk == 0 && plan->in->nrows > 0 && ctx->num_sms <= 256) {
+    sp.fused_final = true;
+    GqParams P;
+    memset(&P, 0, sizeof P);
+    st = fill_final(ctx, plan, kb, kd, out_key_cols, out_agg_cols, out_avg_cols, out_capacity, d_out_ngroups, &P.fin);
     if (st != GQ_OK) return st;
-    GqScanSpec sp;
-    int kb[2]; gq_dtype kd[2] = {GQ_I64, GQ_I64};
-    st = agg_spec(ctx, &sp, plan->in, d, kb, kd);
+    P.fin.part = (long long*)((char*)d_ws + L.fused_off);
+    P.fin.ticket = (unsigned*)(ctx->d_err + 16);
+    return run_scan(ctx, sp, plan->in, d->probes, &P);
+  }
+  // One large batch into a group-by table far larger than L2: partitioned shared-memory aggregation
+  if (L.psa.on && ctx->num_sms <= GQ_MAX_SMS) {
+    GqFinal F;
+    memset(&F, 0, sizeof F);
+    st = fill_final(ctx, plan, kb, kd, out_key_cols, out_agg_cols, out_avg_cols, out_capacity, d_out_ngroups, &F);
     if (st != GQ_OK) return st;
-    if ((sp.consumer == GQ_C_GLOBAL || sp.consumer == GQ_C_LOWCARD) && plan->topk == 0 && plan->in->nrows > 0 &&
-        ctx->num_sms <= 256) {
-      if (!out_agg_cols || !d_out_ngroups || out_capacity < 0 || (d->nkeys > 0 && !out_key_cols)) return fail(ctx, GQ_ERR_INVALID_ARG, "missing outputs");
-      if (plan->navg < 0 || plan->navg > GQ_MAX_AGGS || (plan->navg > 0 && (!plan->avgs || !out_avg_cols))) return fail(ctx, GQ_ERR_INVALID_ARG, "bad avg spec");
-      sp.fused_final = true;
-      GqParams P;
-      memset(&P, 0, sizeof P);
-      GqFinal& F = P.fin;
-      F.part = (long long*)((char*)d_ws + fused_off);
-      F.ticket = (unsigned*)(ctx->d_err + 16);
-      F.nkeys = d->nkeys; F.navg = plan->navg;
-      for (int k = 0; k < d->nkeys; ++k) {
-        if (!out_key_cols[k]) return fail(ctx, GQ_ERR_INVALID_ARG, "null key output");
-        F.out_key[k] = out_key_cols[k]; F.key_bits[k] = kb[k]; F.key_dtype[k] = (int)kd[k];
-      }
-      for (int i = 0; i < d->naggs; ++i) {
-        if (!out_agg_cols[i]) return fail(ctx, GQ_ERR_INVALID_ARG, "null aggregate output");
-        F.out_agg[i] = (long long*)out_agg_cols[i];
-      }
-      for (int v = 0; v < plan->navg; ++v) {
-        if (plan->avgs[v].sum_agg < 0 || plan->avgs[v].sum_agg >= d->naggs || plan->avgs[v].count_agg < 0 ||
-            plan->avgs[v].count_agg >= d->naggs || !out_avg_cols[v]) return fail(ctx, GQ_ERR_INVALID_ARG, "bad avg spec");
-        F.avg_sum[v] = plan->avgs[v].sum_agg; F.avg_cnt[v] = plan->avgs[v].count_agg; F.out_avg[v] = out_avg_cols[v];
-      }
-      F.out_capacity = out_capacity; F.out_n = (long long*)d_out_ngroups;
-      return run_scan(ctx, sp, plan->in, d->probes, &P);
-    }
+    return run_psa(ctx, plan, sp, L.psa, (char*)d_ws + L.psa_off, F);
   }
 
   gq_aggstate* a = nullptr;
-  st = gq_hash_aggregate(ctx, &a, d_ws, aggb, plan->in, &plan->agg);
+  st = gq_hash_aggregate(ctx, &a, d_ws, L.aggb, plan->in, &plan->agg);
   if (st != GQ_OK) { if (a) delete a; return st; }
   st = gq_hash_aggregate_finish(ctx, a, out_key_cols, out_agg_cols, plan->avgs, plan->navg, out_avg_cols, out_capacity,
-                                plan->topk, plan->topk_agg, (char*)d_ws + topk_off, d_out_ngroups);
+                                plan->topk, plan->topk_agg, (char*)d_ws + L.topk_off, d_out_ngroups);
   delete a;   // host handle only; the enqueued kernels hold device pointers into the caller's workspace
   return st;
 }
@@ -1036,12 +1238,26 @@ gq_status gq_precompile_pipeline(const gq_plan* plan, char* h_msg, size_t msg_by
     PartPlan pp = part_plan(sp, &plan->agg, plan->in->nrows);
     if (pp.on) {
       GqScanSpec f = sp;
-      f.consumer = GQ_C_PARTITION; f.part_rw = pp.rw; f.part_exprs = pp.exprs;
+      f.consumer = GQ_C_PARTITION; f.part_rw = pp.rw; f.part_exprs = pp.exprs; f.part_states = 4096;
       st = precompile(f, h_msg, msg_bytes);
       if (st != GQ_OK) return st;
     }
   }
   DirectPlan dp = direct_plan(sp, &plan->agg, plan->in, true);
+  if (dp.step < 0) {
+    PsaPlan pa = psa_plan(sp, &plan->agg, plan->in->nrows, plan->topk);
+    if (pa.on) {
+      GqScanSpec f = sp;
+      f.consumer = GQ_C_SCATTER; f.hot = false; f.part_rw = pa.rw; f.part_exprs = pa.exprs; f.part_states = pa.npart;
+      st = precompile(f, h_msg, msg_bytes);
+      if (st != GQ_OK) return st;
+      std::string msg, path;
+      CachedKernel* pk = nullptr;
+      st = get_psa_kernel_info(f, pa.log2slots, pa.src, &pk, &msg);
+      if (st == GQ_OK) st = gq_jit_compile_to_cache(pk->info, &path, &msg);
+      if (st != GQ_OK) { if (h_msg && msg_bytes) { strncpy(h_msg, msg.c_str(), msg_bytes - 1); h_msg[msg_bytes - 1] = 0; } return st; }
+    }
+  }
   if (dp.step >= 0) {
     GqScanSpec f = sp;
     f.consumer = GQ_C_DIRECT; f.direct_step = dp.step; f.direct_aw = dp.aw; f.direct_touch = dp.touch == plan->agg.naggs; f.hot = false;

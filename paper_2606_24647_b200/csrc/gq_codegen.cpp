@@ -15,6 +15,7 @@
 
 extern const char gq_skeleton_a[];
 extern const char gq_skeleton_b[];
+extern const char gq_skeleton_psa[];
 
 int gq_dtype_bytes(gq_dtype t) { return t == GQ_I8 ? 1 : t == GQ_I32 ? 4 : t == GQ_I64 ? 8 : 0; }
 static const char* ctype(gq_dtype t) { return t == GQ_I8 ? "signed char" : t == GQ_I32 ? "int" : "long long"; }
@@ -226,7 +227,7 @@ static gq_status emit_linear(Gen& g, const GqScanSpec& sp, std::ostringstream& o
   }
   if (!projected && !emit_projection()) return GQ_ERR_INVALID_ARG;
   std::string keyx, depx;
-  if (sp.consumer == GQ_C_LOWCARD || sp.consumer == GQ_C_HIGHCARD || sp.consumer == GQ_C_PARTITION) {
+  if (sp.consumer == GQ_C_LOWCARD || sp.consumer == GQ_C_HIGHCARD || sp.consumer == GQ_C_PARTITION || sp.consumer == GQ_C_SCATTER) {
     gq_status st = key_exprs(g, sp, &keyx, &depx, msg);
     if (st != GQ_OK) return st;
   }
@@ -286,6 +287,24 @@ static gq_status emit_linear(Gen& g, const GqScanSpec& sp, std::ostringstream& o
       if (sp.ndep == 1) o << "    gq_dep_store(slot[j] + 1, " << depx << ", won[j], P.err);\n";
       for (int a = 0; a < nagg; ++a)
         o << "    gq_red(" << (int)sp.aggs[(size_t)a].op << ", slot[j] + " << (1 + sp.ndep + a) << ", " << aggval(sp.aggs[(size_t)a]) << ");\n";
+      o << "  }\n";
+      break;
+    }
+    case GQ_C_SCATTER: {
+      // pass A of the partitioned shared-memory aggregation: one record per surviving row, appended to a CTA-private
+      // chunk of the partition the key hashes to (P.pshift = 64 - log2(partitions)); no table is touched here
+      const int rw = sp.part_rw;
+      o << "  u64 ridx[GQ_R];\n";
+      o << "  " << LOOP << "{\n    ridx[j] = ~0ULL;\n    if (live[j]) ridx[j] = gq_scatter_reserve(P, cx.part_st, cx.sc_next, (u32)(gq_hash("
+        << keyx << ", 0) >> P.pshift));\n  }\n";
+      o << "  " << LOOP << "if (ridx[j] != ~0ULL) {\n    u64* rec = P.part + ridx[j] * " << rw << ";\n";
+      std::vector<std::string> words;
+      words.push_back("(u64)(" + keyx + ")");
+      if (sp.ndep == 1) words.push_back("(u64)" + depx);
+      for (int e : sp.part_exprs) words.push_back("(u64)e" + std::to_string(e) + "[j]");
+      while ((int)words.size() < rw) words.push_back("0ULL");
+      for (int w = 0; w < rw; w += 4)
+        o << "    gq_st256(rec + " << w << ", " << words[(size_t)w] << ", " << words[(size_t)w + 1] << ", " << words[(size_t)w + 2] << ", " << words[(size_t)w + 3] << ");\n";
       o << "  }\n";
       break;
     }
@@ -367,7 +386,7 @@ gq_status gq_codegen(const GqScanSpec& sp, GqKernelInfo* out, std::string* msg) 
   // Hash phases are bound by memory latency, not bandwidth (profiles/r1_hash_phases.md): 24 consumer warps x 2 rows
   // hide more of it than 16 x 4 (C4 1.56 -> 1.13 ms). Pure scans: 20 warps x 2 rows (C2 0.242 -> 0.238 ms).
   const bool hashing = nprobe > 0 || sp.consumer == GQ_C_BUILD || sp.consumer == GQ_C_HIGHCARD || sp.consumer == GQ_C_DIRECT ||
-                       sp.consumer == GQ_C_PARTITION;
+                       sp.consumer == GQ_C_PARTITION || sp.consumer == GQ_C_SCATTER;
   int nt = hashing ? 768 : 640;
   const bool tablebound = sp.consumer == GQ_C_HIGHCARD && nprobe == 0;   // DRAM-random bound (C5): 16 warps x 4 rows measured best
   if (tablebound) nt = 512;
@@ -389,7 +408,11 @@ gq_status gq_codegen(const GqScanSpec& sp, GqKernelInfo* out, std::string* msg) 
   const bool use_hot = sp.hot && (sp.consumer == GQ_C_HIGHCARD || sp.consumer == GQ_C_PARTITION) && all_unique;   // linear mode only
   if (use_hot) cons_bytes = 512 * 8 + 512LL * nagg * 8 + 512 * 4 + 256;
   long long part_state_off = 0;
-  if (sp.part_rw > 0) { part_state_off = (cons_bytes + 127) / 128 * 128; cons_bytes = part_state_off + 4096 * 4; }   // <= 4096 partitions
+  if (sp.part_rw > 0) {   // partition state words (+ the CTA's chunk counter)
+    if (sp.part_states < 1 || sp.part_states > 16384) { if (msg) *msg = "bad partition count"; return GQ_ERR_INVALID_ARG; }
+    part_state_off = (cons_bytes + 127) / 128 * 128;
+    cons_bytes = part_state_off + sp.part_states * 4LL + 64;
+  }
   int r = tablebound ? 4 : 2, stages = 0;
   // small inputs: smaller tiles so that every SM still gets several tiles
   if (sp.nrows_hint > 0 && sp.nrows_hint < (long long)sp.num_sms * 8 * nt * 2) r = 1;
@@ -408,6 +431,9 @@ gq_status gq_codegen(const GqScanSpec& sp, GqKernelInfo* out, std::string* msg) 
   // ---- 3. prelude ----
   std::ostringstream o;
   o << "// generated by gq_codegen — plan-shape specialised prelude\n";
+  // (part of the source, hence of the kernel's identity: two plans that differ only in their shared-memory carve-up,
+  // e.g. in the number of partition state words, must not share a cached kernel and its launch configuration)
+  o << "#define GQ_SMEM_BYTES " << (stages * stage_bytes + 2 * stages * 8 + 64 + cons_bytes + 128) << "\n";
   o << "#define GQ_NCOL " << ncol << "\n#define GQ_NT " << nt << "\n#define GQ_R " << r << "\n#define GQ_STAGES "
     << stages << "\n#define GQ_STAGE_BYTES " << stage_bytes << "\n#define GQ_CONSUMER " << sp.consumer << "\n";
   o << "#define GQ_NAGG " << nagg << "\n#define GQ_LC_G " << (sp.lc_cap > 0 ? sp.lc_cap : 1) << "\n#define GQ_LC_KT " << lc_kt
@@ -574,5 +600,37 @@ gq_status gq_codegen(const GqScanSpec& sp, GqKernelInfo* out, std::string* msg) 
   out->cols = g.cols;
   out->consts = g.consts;
   if ((int)g.consts.size() > GQ_MAXK) { if (msg) *msg = "too many constants"; return GQ_ERR_UNSUPPORTED; }
+  return GQ_OK;
+}
+
+// Pass B of the partitioned shared-memory aggregation (gq_psa_kernel.cuh), specialised by the plan's aggregate list,
+// record layout and table slot layout. `src[a]` = record word holding the input of aggregate a (unused for COUNT).
+gq_status gq_codegen_psa(const GqScanSpec& sp, int log2slots, const int* src, GqKernelInfo* out, std::string* msg) {
+  const int nagg = (int)sp.aggs.size();
+  if (nagg < 1 || nagg > GQ_MAX_AGGS || sp.part_rw < 4 || sp.part_rw % 4 || sp.target_sw < 2 || log2slots < 6 || log2slots > 16) {
+    if (msg) *msg = "bad partitioned-aggregation spec"; return GQ_ERR_INVALID_ARG; }
+  std::ostringstream o;
+  o << "// generated by gq_codegen_psa — plan-shape specialised prelude\n";
+  // the scan skeleton's macros: only its types and hash-table primitives are used here
+  o << "#define GQ_NCOL 1\n#define GQ_NT 512\n#define GQ_R 1\n#define GQ_STAGES 1\n#define GQ_STAGE_BYTES 128\n#define GQ_CONSUMER 2\n"
+    << "#define GQ_LC_G 1\n#define GQ_LC_KT 64\n#define GQ_LC_KEY32 0\n#define GQ_LC_KEY_BITS 1\n#define GQ_HOT 0\n#define GQ_PART_STATE_OFF 0\n"
+    << "#define GQ_FUSED_FINAL 0\n#define GQ_DIRECT_AW 1\n#define GQ_COL_OFF(c) 0\n#define GQ_COL_BYTES(c) 8\n#define GQ_TX_BYTES 0\n";
+  o << "#define GQ_NAGG " << nagg << "\n#define GQ_TARGET_SW " << sp.target_sw << "\n#define GQ_NDEP " << sp.ndep << "\n#define GQ_CHECK_DEP "
+    << (sp.check_dep ? 1 : 0) << "\n#define GQ_PART_RW " << sp.part_rw << "\n#define GQ_PSA_LOG2SLOTS " << log2slots << "\n";
+  o << "#define GQ_AGG_OP(a) (";
+  for (int a = 0; a < nagg; ++a) o << "(a) == " << a << " ? " << (int)sp.aggs[(size_t)a].op << " : ";
+  o << "0)\n#define GQ_AGG_SRC(a) (";
+  for (int a = 0; a < nagg; ++a) o << "(a) == " << a << " ? " << (src[a] < 0 ? 0 : src[a]) << " : ";
+  o << "0)\n";
+  o << gq_skeleton_a << "\n" << gq_skeleton_psa << "\n";
+  out->source = o.str();
+  char hb[32];
+  snprintf(hb, sizeof hb, "%016llx", (unsigned long long)fnv1a(out->source));
+  out->hash = hb;
+  out->entry = "gq_psa";
+  out->threads = 512;
+  out->tile_rows = 0;
+  out->smem_bytes = (int)((((1LL << log2slots) + 1) * sp.target_sw + 2 * 66) * 8 + 64);
+  if (out->smem_bytes > GQ_SMEM_LIMIT) { if (msg) *msg = "partitioned-aggregation table does not fit shared memory"; return GQ_ERR_UNSUPPORTED; }
   return GQ_OK;
 }

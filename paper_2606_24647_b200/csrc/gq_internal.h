@@ -17,7 +17,7 @@
 #define GQ_DEFAULT_SMS 148     // B200; used only when a plan is compiled ahead of time without a device attached
 #define GQ_DEP_UNSET 0x8000000000000001ULL   // dependent-key word of a slot nobody has stored yet (GQ_F_CHECK_DEPENDENT)
 
-enum { GQ_C_GLOBAL = 0, GQ_C_LOWCARD = 1, GQ_C_HIGHCARD = 2, GQ_C_BUILD = 3, GQ_C_MATERIALISE = 4, GQ_C_DIRECT = 5, GQ_C_PARTITION = 6 };
+enum { GQ_C_GLOBAL = 0, GQ_C_LOWCARD = 1, GQ_C_HIGHCARD = 2, GQ_C_BUILD = 3, GQ_C_MATERIALISE = 4, GQ_C_DIRECT = 5, GQ_C_PARTITION = 6, GQ_C_SCATTER = 7 };
 
 // ---- device-visible structs: layouts must match gq_skeleton.cuh ----
 struct GqTableDev {
@@ -61,6 +61,10 @@ struct GqParams {
   long long pcap;
   long long pshift;
   long long npart;
+  unsigned* sc_info;           // SCATTER (pass A of the partitioned shared-memory aggregation): see gq_skeleton.cuh
+  unsigned* sc_count;
+  unsigned* sc_ncta;
+  long long sc_slab;
   GqFinal fin;
 };
 
@@ -140,7 +144,8 @@ struct GqScanSpec {
   int direct_step = -1;                           // DIRECT: probe step whose matched slot is the group
   int direct_aw = 0;                              // DIRECT: words per accumulator slot
   bool direct_touch = false;                      // DIRECT: hidden COUNT word marks touched slots
-  int part_rw = 0;                                // PARTITION: words per record (multiple of 4)
+  int part_states = 0;                            // PARTITION / SCATTER: partition state words in shared memory
+  int part_rw = 0;                                // PARTITION / SCATTER: words per record (multiple of 4)
   std::vector<int> part_exprs;                    // PARTITION: expressions stored in a record, in word order
   int target_sw = 0;                              // slot words of the target table
   int build_key_col = 0;                          // BUILD
@@ -153,6 +158,7 @@ struct GqScanSpec {
 };
 
 struct GqKernelInfo {
+  std::string entry = "gq_scan";   // kernel name
   std::string source;          // full translation unit
   std::string hash;            // 16 hex digits of the source hash
   int threads = 0;             // GQ_NT + 32
@@ -164,6 +170,7 @@ struct GqKernelInfo {
 
 // gq_codegen.cpp
 gq_status gq_codegen(const GqScanSpec& spec, GqKernelInfo* out, std::string* msg);
+gq_status gq_codegen_psa(const GqScanSpec& spec, int log2slots, const int* src, GqKernelInfo* out, std::string* msg);
 int gq_dtype_bytes(gq_dtype t);
 // gq_jit.cpp
 struct GqKernel { cudaKernel_t fn = nullptr; int threads = 0; int smem_bytes = 0; int tile_rows = 0; };
@@ -203,6 +210,20 @@ size_t gq_topk_scratch_bytes_impl();
 cudaError_t gq_launch_hot_keys(cudaStream_t s, const void* keycol, int dtype, long long nrows, unsigned long long* table,
                                long long nslots, long long nsample, unsigned long long threshold, long long* hot,
                                int max_hot, int num_sms, int* nlaunches);
+// ---- partitioned shared-memory aggregation (gq_psa_kernel.cuh, gq_psa.cu) ----
+#define GQ_MAX_SMS 160               // workspace sizing bound for the per-CTA chunk ranges of pass A
+#define GQ_PSA_GID_BITS 26           // directory entry = chunk id | records used << 26
+struct GqPsaParams {                 // must match gq_psa_kernel.cuh
+  const unsigned long long* rec; const unsigned* plist; const unsigned* pstart; const unsigned* items; const unsigned* item_seg;
+  const unsigned* nitems; unsigned* work; int* err; GqTableDev merge; unsigned seg_chunks; int hshift; GqFinal fin;
+};
+struct GqPsaDirParams {
+  const unsigned* pcount; unsigned* pstart; unsigned* items; unsigned* item_seg; unsigned* nitems; int npart; unsigned seg_chunks;
+  int* err; unsigned max_items;
+};
+cudaError_t gq_launch_psa_dir(cudaStream_t s, const GqPsaDirParams& p);
+cudaError_t gq_launch_psa_fill(cudaStream_t s, const unsigned* info, const unsigned* ncta, int nctas, long long slab,
+                               const unsigned* pstart, unsigned* pfill, unsigned* plist);
 #define GQ_HOT_MAX 256               // hot keys per batch (shared-memory set of 2*GQ_HOT_MAX positions per CTA)
 #define GQ_HOT_SAMPLE (1LL << 19)    // sampled rows
 #define GQ_HOT_SLOTS (1LL << 20)     // (key,count) sample table slots (16 B each)

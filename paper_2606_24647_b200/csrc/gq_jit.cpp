@@ -127,7 +127,7 @@ gq_status gq_jit_get(const GqKernelInfo& info, int device, GqKernel* out, std::s
   cudaLibrary_t lib;
   cudaError_t e = cudaLibraryLoadData(&lib, cubin.data(), nullptr, nullptr, 0, nullptr, nullptr, 0);
   cudaKernel_t fn = nullptr;
-  if (e == cudaSuccess) e = cudaLibraryGetKernel(&fn, lib, "gq_scan");
+  if (e == cudaSuccess) e = cudaLibraryGetKernel(&fn, lib, info.entry.c_str());
   if (e == cudaSuccess) e = cudaFuncSetAttribute((const void*)fn, cudaFuncAttributeMaxDynamicSharedMemorySize, info.smem_bytes);
   if (e != cudaSuccess) {
     if (cuda_err) *cuda_err = (int)e;

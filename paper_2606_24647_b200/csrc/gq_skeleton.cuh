@@ -40,6 +40,7 @@ typedef unsigned int u32;
 #define GQ_C_MATERIALISE 4
 #define GQ_C_DIRECT 5
 #define GQ_C_PARTITION 6
+#define GQ_C_SCATTER 7
 
 #define GQ_E_CAPACITY 3
 #define GQ_E_DUPLICATE 6
@@ -98,6 +99,10 @@ struct GqParams {
   i64 pcap;                     // PARTITION: records per partition
   i64 pshift;                   // PARTITION: partition = first slot of the key in the target table >> pshift
   i64 npart;                    // number of partitions
+  u32* sc_info;                 // SCATTER: per chunk (partition << 8) | records used
+  u32* sc_count;                // SCATTER: chunks per partition (RED)
+  u32* sc_ncta;                 // SCATTER: chunks allocated by every CTA
+  i64 sc_slab;                  // SCATTER: chunk ids of CTA b are [b * sc_slab, (b + 1) * sc_slab)
   GqFinal fin;                  // GQ_FUSED_FINAL: outputs of the in-kernel finaliser
 };
 
@@ -486,6 +491,35 @@ __device__ __forceinline__ i64 gq_part_reserve(const GqParams& P, u32* st, u64 p
   }
 }
 
+// Partitioned shared-memory aggregation, pass A (SCATTER consumer): a surviving row becomes one record
+// (key, dependent key, aggregate inputs) appended to a chunk of GQ_PART_CHUNK records that belongs to the partition
+// its key hashes to. Chunks are CTA-private and are handed out from a CTA-private range of chunk ids by a
+// shared-memory counter, so the per-row path has NO global atomic: one ATOMS on the partition's {chunk : 20, used : 12}
+// state word hands out the slots of the open chunk; the thread that finds it exhausted opens the next chunk (one
+// ATOMS on the CTA's chunk counter, one fire-and-forget RED on the partition's chunk count, one 4-byte store of the
+// chunk's partition). Pass B (gq_psa) finds a partition's chunks through a directory built from those words.
+// Returns the record index (chunk id * GQ_PART_CHUNK + slot), or ~0 when the CTA's chunk range is exhausted (cannot
+// happen for a range sized rows / GQ_PART_CHUNK + partitions; reported as a capacity error).
+__device__ __forceinline__ u64 gq_scatter_reserve(const GqParams& P, u32* st, u32* next, u32 p) {
+  for (;;) {
+    const u32 v0 = ((volatile u32*)st)[p];
+    if ((v0 & 0xFFFu) > GQ_PART_CHUNK) { __nanosleep(20); continue; }   // the next chunk is being opened (a few cycles)
+    const u32 v = atomicAdd(&st[p], 1u);
+    const u32 used = v & 0xFFFu;
+    if (used < GQ_PART_CHUNK) return ((u64)blockIdx.x * (u64)P.sc_slab + (v >> 12)) * GQ_PART_CHUNK + used;
+    if (used == GQ_PART_CHUNK) {                           // this thread opens the next chunk and takes its first slot
+      const u32 c = atomicAdd(next, 1u);
+      if ((i64)c >= P.sc_slab) { gq_set_err(P.err, GQ_E_CAPACITY); ((volatile u32*)st)[p] = v & ~0xFFFu; return ~0ULL; }
+      const u64 gid = (u64)blockIdx.x * (u64)P.sc_slab + c;
+      P.sc_info[gid] = (p << 8) | GQ_PART_CHUNK;           // assumed full; part-filled chunks are fixed up at the end
+      atomicAdd(P.sc_count + p, 1u);
+      __threadfence_block();
+      ((volatile u32*)st)[p] = (c << 12) | 1u;
+      return gid * GQ_PART_CHUNK;
+    }
+  }
+}
+
 // ---------------------------------------------------------------------------------------------- row sources
 // A tile staged in shared memory by the producer, or the ragged tail read from global memory.
 struct GqSrcSmem {
@@ -513,7 +547,8 @@ struct GqCtx {
   i64* lc_gkey;                         //   key of every group id [GQ_LC_G]
   int* lc_n;                            //   [0] groups so far, [1] insert lock, [2] gid of the reserved-pattern key + 1
   i64* lc_acc;                          //   accumulators [GQ_LC_G][GQ_NAGG][GQ_NT], thread-private cells
-  u32* part_st;                         // record append: per-partition {chunk id : 16, used : 16} of this CTA's open chunk
+  u32* part_st;                         // record append: per-partition {chunk id, used} of this CTA's open chunk
+  u32* sc_next;                         // SCATTER: next free chunk of this CTA's chunk range
   int* mat;                             // MATERIALISE: shared [0] rows of the tile so far, [2..3] the tile's output base
   i64 ninserted;                        // BUILD: rows inserted by this thread
   i64* hot_keys;                        // HIGHCARD + GQ_HOT: shared set of this batch's hot keys [GQ_HOT_POS]

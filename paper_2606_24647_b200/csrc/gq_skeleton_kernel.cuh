@@ -125,6 +125,10 @@ extern "C" __global__ void __launch_bounds__(GQ_NT + 32, 1) gq_scan(const __grid
 #if GQ_PART_RW
   cx.part_st = (u32*)(gq_smem + GQ_CONS_OFF + GQ_PART_STATE_OFF);
   for (int i = tid; i < (int)P.npart; i += GQ_NT + 32) cx.part_st[i] = GQ_PART_CHUNK;   // no open chunk yet
+#if GQ_CONSUMER == GQ_C_SCATTER
+  cx.sc_next = cx.part_st + P.npart;
+  if (tid == 0) *cx.sc_next = 0;
+#endif
 #endif
 #if GQ_HOT
   cx.hot_keys = (i64*)(gq_smem + GQ_CONS_OFF);
@@ -367,7 +371,17 @@ extern "C" __global__ void __launch_bounds__(GQ_NT + 32, 1) gq_scan(const __grid
     }
   }
 #endif
-#if GQ_PART_RW
+#if GQ_CONSUMER == GQ_C_SCATTER
+  {   // record how far this CTA's part-filled chunks got, and how many chunks it opened
+    gq_consumer_barrier();
+    for (int p = tid; p < (int)P.npart; p += GQ_NT) {
+      const u32 v = cx.part_st[p];
+      const u32 used = v & 0xFFFu;
+      if (used < GQ_PART_CHUNK) P.sc_info[(u64)blockIdx.x * (u64)P.sc_slab + (v >> 12)] = ((u32)p << 8) | used;
+    }
+    if (tid == 0) { const u32 n = *cx.sc_next; P.sc_ncta[blockIdx.x] = n < (u32)P.sc_slab ? n : (u32)P.sc_slab; }
+  }
+#elif GQ_PART_RW
   {   // pad the unused slots of this CTA's open chunks with EMPTY-key records (pass B skips them)
     gq_consumer_barrier();
     for (int p = tid; p < (int)P.npart; p += GQ_NT) {

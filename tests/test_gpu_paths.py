@@ -324,6 +324,56 @@ def test_partitioned_aggregation_skew_overflow_reserved_key_and_dependent_key(ct
     run(plan, ctx)
 
 
+def test_partitioned_shared_memory_aggregation_shapes(ctx, force_partition):
+    # gq_pipeline's single-batch path (scatter -> directory -> shared-memory aggregation per partition): packed two-key
+    # groups with signed narrow keys, AVG, a probe step in front, and a batch that is only a ragged tail
+    rng = np.random.default_rng(12)
+    n = 260_007
+    a = rng.integers(-300, 300, n).astype(np.int32)
+    b = rng.integers(-100, 100, n).astype(np.int8)
+    v = rng.integers(-10**11, 10**11, n).astype(np.int64)
+    plan = dict(table=[a, b, v], preds=[(2, "ne", 5)], exprs=[[("col", 2)], [("col", 2), ("col", 0), ("mul",)]], keys=[0, 1],
+                aggs=[("sum", 0), ("count",), ("min", 1), ("max", 0)], max_groups=130_000)
+    l0 = ctx.launch_count()
+    exp, got = run(plan, ctx, avgs=[(0, 1)])
+    assert ctx.launch_count() - l0 == 6          # merge-table init, scan+scatter, directory x2, shared-memory aggregation, merge emit
+    ref = np.array([oracle.avg(int(x), int(y)) for x, y in zip(exp.cols[2], exp.cols[3])])
+    assert np.array_equal(got["avgs"][0], ref)
+    rngj = np.random.default_rng(13)
+    plan = _join_plan(9_000, 200_000, rngj, [("sum", 0), ("count",)])
+    plan["keys"] = [1]; plan["max_groups"] = 20_000                      # group by a non-join column: hashed, partitioned
+    run(plan, ctx)
+    plan = plans.plan_c5(datagen.make_config(5, scale=0.00001))          # 6000 rows: tail-only batches still work
+    plan["max_groups"] = 10_000
+    run(plan, ctx)
+
+
+def test_partitioned_shared_memory_aggregation_heavy_keys_and_many_groups(ctx, force_partition):
+    rng = np.random.default_rng(14)
+    # (a) heavy partitions are cut into segments whose partial groups meet in the global merge table: one key owns 55 %
+    # of 1.5 M rows, another 20 %, plus the reserved bit pattern and a dependent key
+    n = 1_500_000
+    k = rng.integers(0, 40_000, n).astype(np.int64) * 104729
+    u = rng.random(n)
+    k[u < 0.55] = 987654321
+    k[(u >= 0.55) & (u < 0.75)] = -5
+    k[::997] = I64_MIN
+    dep = (k % 1000).astype(np.int32)
+    v = rng.integers(-10**6, 10**6, n).astype(np.int64)
+    plan = dict(table=[k, dep, v], preds=[], exprs=[[("col", 2)]], keys=[0, 1], ndependent=1,
+                aggs=[("sum", 0), ("min", 0), ("max", 0), ("count",)], max_groups=45_000)
+    exp, got = run(plan, ctx)
+    assert int(got["cols"][-1].max()) > 800_000
+    # (b) far more distinct keys than max_groups promised: partitions overflow their shared-memory table and their key
+    # range is halved (second hash) until it fits -- slower, never wrong
+    n = 700_000
+    k = rng.permutation(5_000_000)[:n].astype(np.int64) - 2_000_000
+    plan = dict(table=[k, np.ones(n, np.int64)], preds=[], exprs=[[("col", 1)]], keys=[0], aggs=[("sum", 0), ("count",)],
+                max_groups=100_000)
+    exp, got = run(plan, ctx, out_capacity=n)
+    assert got["n"] == n
+
+
 def test_partitioned_aggregation_streams_batches(ctx, force_partition):
     import gqrun
     plan = plans.plan_c5(datagen.make_config(5, scale=0.004))
