@@ -209,15 +209,15 @@ gq_status load_kernel(gq_ctx* ctx, CachedKernel* ck, GqKernel* kern) {
 }
 
 // Pass B kernel of the partitioned shared-memory aggregation for this plan shape (cached by shape).
-gq_status get_psa_kernel_info(const GqScanSpec& sp, int log2slots, const int* src, CachedKernel** out, std::string* msg) {
-  std::string sig = "psa:" + std::to_string(log2slots) + "," + std::to_string(sp.target_sw) + "," + std::to_string(sp.part_rw) + "," +
+gq_status get_psa_kernel_info(const GqScanSpec& sp, int log2slots, const int* src, int threads, CachedKernel** out, std::string* msg) {
+  std::string sig = "psa:" + std::to_string(log2slots) + "," + std::to_string(threads) + "," + std::to_string(sp.target_sw) + "," + std::to_string(sp.part_rw) + "," +
                     std::to_string(sp.ndep) + "," + std::to_string(sp.check_dep) + ";";
   for (size_t a = 0; a < sp.aggs.size(); ++a) sig += std::to_string((int)sp.aggs[a].op) + ":" + std::to_string(src[a]) + ",";
   std::lock_guard<std::mutex> l(g_kmu);
   auto it = g_kernels.find(sig);
   if (it == g_kernels.end()) {
     CachedKernel ck;
-    gq_status st = gq_codegen_psa(sp, log2slots, src, &ck.info, msg);
+    gq_status st = gq_codegen_psa(sp, log2slots, src, threads, &ck.info, msg);
     if (st != GQ_OK) return st;
     it = g_kernels.emplace(sig, std::move(ck)).first;
   }
@@ -582,7 +582,7 @@ DirectPlan direct_plan(const GqScanSpec& sp, const gq_agg_desc* d, const gq_batc
 // an L2-resident table slice. Worth it only for big tables and big batches; thresholds overridable for tests.
 struct PartPlan { bool on = false; int npart = 0, pshift = 0, rw = 0; int64_t pcap = 0; size_t bytes = 0; std::vector<int> exprs; int src[GQ_MAX_AGGS]; };
 // planner knobs (gq_set_option)
-std::atomic<int64_t> g_part_min_table_mb{256}, g_part_min_rows{1 << 24};
+std::atomic<int64_t> g_part_min_table_mb{256}, g_part_min_rows{1 << 24}, g_hot_min_rows{GQ_HOT_MIN_ROWS}, g_psa_max_log2part{GQ_PSA_MAX_LOG2PART}, g_psa_threads{0};
 PartPlan part_plan(const GqScanSpec& sp, const gq_agg_desc* d, int64_t nrows) {
   PartPlan pp;
   if (sp.consumer != GQ_C_HIGHCARD) return pp;
@@ -616,12 +616,13 @@ PartPlan part_plan(const GqScanSpec& sp, const gq_agg_desc* d, int64_t nrows) {
 // table and writes the dense result. No global group-by table, no global atomics on the per-row path.
 struct PsaPlan {
   bool on = false;
-  int npart = 0, log2npart = 0, log2slots = 0, rw = 0;
+  int npart = 0, log2npart = 0, log2sub = 0, log2slots = 0, rw = 0, threads = 512;
+  bool hot = false;
   std::vector<int> exprs; int src[GQ_MAX_AGGS];
   int64_t chunks_bound = 0, merge_cap = 0;
   uint32_t seg_chunks = 0, max_items = 0;
   size_t off_zero = 0, zero_bytes = 0, off_pcount = 0, off_pfill = 0, off_pstart = 0, off_items = 0, off_itemseg = 0, off_ncta = 0,
-         off_info = 0, off_plist = 0, off_merge = 0, merge_bytes = 0, off_rec = 0, bytes = 0;
+         off_info = 0, off_plist = 0, off_merge = 0, merge_bytes = 0, off_hot = 0, off_rec = 0, bytes = 0;
 };
 const int64_t GQ_PSA_MAX_TILE = 4096;   // upper bound of the scan kernel's tile (rows): bounds a CTA's share of the rows
 PsaPlan psa_plan(const GqScanSpec& sp, const gq_agg_desc* d, int64_t nrows, int topk) {
@@ -634,11 +635,26 @@ PsaPlan psa_plan(const GqScanSpec& sp, const gq_agg_desc* d, int64_t nrows, int 
   while ((((1LL << (L + 1)) + 1) * sw + 2 * 66) * 8 + 64 <= GQ_SMEM_LIMIT) ++L;
   if ((((1LL << L) + 1) * sw + 2 * 66) * 8 + 64 > GQ_SMEM_LIMIT) return pp;
   pp.log2slots = L;
-  const int64_t slots = 1LL << L, limit = slots - slots / 8 - 512;
+  // groups a shared-memory table takes (gq_psa_kernel.cuh GQ_PSA_LIMIT), less 5 % for the spread of a hash partitioning
+  const int64_t slots = 1LL << L;
+  auto limit_for = [slots](int threads) { return (slots - slots / 16 - threads) * 19 / 20; };
+  int64_t limit = limit_for(512);
   if (limit < 32) return pp;
-  int lp = 6;                                               // 64 .. 16384 partitions; more groups than that: the key
+  int lp = 6;                                               // 64 .. 16384 key ranges; more groups than that: the key
   while (lp < 14 && (d->max_groups + limit - 1) / limit > (1LL << lp)) ++lp;   // ranges are halved in pass B instead
-  pp.log2npart = lp; pp.npart = 1 << lp;
+  // 32 warps hide more of the table's dependent shared-memory round trips than 16; taken when the tables still hold the plan's groups
+  const int64_t want = g_psa_threads.load();   // 0 = decide here, 512 / 1024 = the planner's choice
+  pp.threads = want == 512 ? 512 : want == 1024 ? 1024
+             : (limit_for(1024) >= 32 && (d->max_groups + limit_for(1024) - 1) / limit_for(1024) <= (1LL << lp)) ? 1024 : 512;
+  if (limit_for(pp.threads) < 32) return pp;
+  limit = limit_for(pp.threads);
+  // Pass A scatters into at most 2^psa_max_log2part partitions: every (CTA, partition) pair has an open 128-byte line of
+  // records, and those lines must stay in L2 until they are full, or every record becomes a random 32-byte DRAM write.
+  // The remaining key-range bits are resolved in pass B: 2^log2sub sub-passes per partition, one per work item.
+  pp.log2npart = (int)std::min<int64_t>(lp, std::max<int64_t>(6, g_psa_max_log2part.load()));
+  pp.log2sub = std::min(3, lp - pp.log2npart);
+  pp.npart = 1 << pp.log2npart;
+  pp.hot = sp.hot;
   for (int a = 0; a < d->naggs; ++a) {
     pp.src[a] = -1;
     if (d->aggs[a].op == GQ_COUNT_STAR) continue;
@@ -653,8 +669,8 @@ PsaPlan psa_plan(const GqScanSpec& sp, const gq_agg_desc* d, int64_t nrows, int 
   if (pp.chunks_bound >= (1LL << GQ_PSA_GID_BITS) || nrows / GQ_PART_CHUNK + pp.npart + 300 >= (1LL << 20)* GQ_MAX_SMS) return pp;
   // a partition is "heavy" (cut into segments for several CTAs) when it is far above the average AND a sizeable share of all work
   pp.seg_chunks = (uint32_t)std::max<int64_t>(std::max<int64_t>(64, pp.chunks_bound / 512), 4 * pp.chunks_bound / pp.npart);
-  pp.max_items = (uint32_t)(pp.npart + 2 * (pp.chunks_bound / pp.seg_chunks) + 2);
-  pp.merge_cap = table_capacity(std::min<int64_t>(std::max<int64_t>(1, d->max_groups), (pp.chunks_bound / pp.seg_chunks + 1) * limit));
+  pp.max_items = (uint32_t)((pp.npart + 2 * (pp.chunks_bound / pp.seg_chunks) + 2) << pp.log2sub);
+  pp.merge_cap = table_capacity(std::min<int64_t>(std::max<int64_t>(1, d->max_groups), (pp.chunks_bound / pp.seg_chunks + 1) * limit) + GQ_HOT_MAX);
   size_t off = 0;
   auto take = [&off](size_t b) { size_t o = off; off += align_up(b, 256); return o; };
   pp.off_zero = take(256);                                   // [0] work cursor, [1] item count
@@ -669,6 +685,7 @@ PsaPlan psa_plan(const GqScanSpec& sp, const gq_agg_desc* d, int64_t nrows, int 
   pp.off_plist = take((size_t)pp.chunks_bound * 4);
   pp.merge_bytes = ws_layout(pp.merge_cap, sw, 1).total;
   pp.off_merge = take(pp.merge_bytes);
+  if (pp.hot) pp.off_hot = take(4096 + (size_t)GQ_HOT_SLOTS * 16);   // hot list + heavy-hitter sample table
   pp.off_rec = take((size_t)pp.chunks_bound * GQ_PART_CHUNK * pp.rw * 8);
   pp.bytes = off;
   pp.on = true;
@@ -794,7 +811,7 @@ gq_status gq_hash_aggregate(gq_ctx* ctx, gq_aggstate** state, void* d_ws, size_t
   P.target = a->dev;
   P.acc = (long long*)(a->dev.side + 1);
   P.dacc = a->dacc;
-  if (sp.hot && a->hot && in->nrows >= GQ_HOT_MIN_ROWS) {   // heavy-hitter pass over a strided sample of the key column
+  if (sp.hot && a->hot && in->nrows >= g_hot_min_rows.load()) {   // heavy-hitter pass over a strided sample of the key column
     int nl = 0;
     const gq_column& kc = in->cols[sp.key_cols[0]];
     cudaError_t e = gq_launch_hot_keys(ctx->stream, kc.data, (int)kc.dtype, in->nrows, a->hot_table, GQ_HOT_SLOTS, GQ_HOT_SAMPLE,
@@ -941,7 +958,7 @@ static gq_status fill_final(gq_ctx* ctx, const gq_plan* plan, const int kb[2], c
 static gq_status run_psa(gq_ctx* ctx, const gq_plan* plan, GqScanSpec sp, const PsaPlan& pp, char* ws, const GqFinal& F) {
   const gq_agg_desc* d = &plan->agg;
   const gq_batch* in = plan->in;
-  sp.consumer = GQ_C_SCATTER; sp.hot = false; sp.part_rw = pp.rw; sp.part_exprs = pp.exprs; sp.part_states = pp.npart;
+  sp.consumer = GQ_C_SCATTER; sp.hot = pp.hot; sp.part_rw = pp.rw; sp.part_exprs = pp.exprs; sp.part_states = pp.npart;
   CachedKernel* ck = nullptr;
   gq_status st = get_kernel_info(sp, &ck, &ctx->msg);
   if (st != GQ_OK) return st;
@@ -981,17 +998,30 @@ static gq_status run_psa(gq_ctx* ctx, const gq_plan* plan, GqScanSpec sp, const 
   P.sc_info = U(pp.off_info); P.sc_count = U(pp.off_pcount); P.sc_ncta = U(pp.off_ncta); P.sc_slab = slab;
   e = cudaMemsetAsync(P.sc_ncta, 0, GQ_MAX_SMS * 4, ctx->stream);
   if (e != cudaSuccess) return cuda_fail(ctx, e, "partitioned aggregation: memset");
+  if (pp.hot && in->nrows >= g_hot_min_rows.load()) {
+    // skewed batches: the most frequent keys (strided sample of the key column) are aggregated per CTA in shared memory
+    // by pass A and flushed into the merge table; they never become records
+    int nl = 0;
+    const gq_column& kc = in->cols[sp.key_cols[0]];
+    long long* hot = (long long*)(ws + pp.off_hot);
+    e = gq_launch_hot_keys(ctx->stream, kc.data, (int)kc.dtype, in->nrows, (unsigned long long*)(ws + pp.off_hot + 4096), GQ_HOT_SLOTS,
+                           GQ_HOT_SAMPLE, GQ_HOT_THRESHOLD, hot, GQ_HOT_MAX, ctx->num_sms, &nl);
+    if (e != cudaSuccess) return cuda_fail(ctx, e, "heavy-hitter sampling");
+    ctx->launches += nl;
+    P.hot = hot;
+    P.target = mt;
+  }
   st = run_scan(ctx, sp, in, d->probes, &P);
   if (st != GQ_OK) return st;
   GqPsaDirParams dp{};
   dp.pcount = U(pp.off_pcount); dp.pstart = U(pp.off_pstart); dp.items = U(pp.off_items); dp.item_seg = U(pp.off_itemseg);
-  dp.nitems = U(pp.off_zero) + 1; dp.npart = pp.npart; dp.seg_chunks = pp.seg_chunks; dp.err = ctx->d_err; dp.max_items = pp.max_items;
+  dp.nitems = U(pp.off_zero) + 1; dp.npart = pp.npart; dp.seg_chunks = pp.seg_chunks; dp.err = ctx->d_err; dp.max_items = pp.max_items; dp.nsub = 1u << pp.log2sub;
   e = gq_launch_psa_dir(ctx->stream, dp);
   if (e == cudaSuccess) e = gq_launch_psa_fill(ctx->stream, U(pp.off_info), U(pp.off_ncta), (int)grid, slab, U(pp.off_pstart), U(pp.off_pfill), U(pp.off_plist));
   if (e != cudaSuccess) return cuda_fail(ctx, e, "partition directory");
   ctx->launches += 2;
   CachedKernel* pk = nullptr;
-  st = get_psa_kernel_info(sp, pp.log2slots, pp.src, &pk, &ctx->msg);
+  st = get_psa_kernel_info(sp, pp.log2slots, pp.src, pp.threads, &pk, &ctx->msg);
   if (st != GQ_OK) return st;
   GqKernel kern;
   st = load_kernel(ctx, pk, &kern);
@@ -1000,7 +1030,7 @@ static gq_status run_psa(gq_ctx* ctx, const gq_plan* plan, GqScanSpec sp, const 
   memset(&B, 0, sizeof B);
   B.rec = P.part; B.plist = U(pp.off_plist); B.pstart = U(pp.off_pstart); B.items = U(pp.off_items); B.item_seg = U(pp.off_itemseg);
   B.nitems = U(pp.off_zero) + 1; B.work = U(pp.off_zero); B.err = ctx->d_err; B.merge = mt; B.seg_chunks = pp.seg_chunks;
-  B.hshift = 64 - pp.log2npart; B.fin = F;
+  B.hshift = 64 - pp.log2npart; B.log2sub = pp.log2sub; B.fin = F;
   void* args[] = {(void*)&B};
   e = cudaLaunchKernel((const void*)kern.fn, dim3((unsigned)ctx->num_sms), dim3((unsigned)kern.threads), args, (size_t)kern.smem_bytes, ctx->stream);
   if (e != cudaSuccess) return cuda_fail(ctx, e, "launch of the partitioned aggregation kernel");
@@ -1082,6 +1112,9 @@ gq_status gq_set_option(const char* h_name, int64_t value) {
   const std::string n = h_name;
   if (n == "part_min_table_mb") g_part_min_table_mb = value < 0 ? 256 : value;
   else if (n == "part_min_rows") g_part_min_rows = value < 0 ? (1 << 24) : value;
+  else if (n == "hot_min_rows") g_hot_min_rows = value < 0 ? GQ_HOT_MIN_ROWS : value;
+  else if (n == "psa_threads") g_psa_threads = (value == 512 || value == 1024) ? value : 0;
+  else if (n == "psa_max_log2_partitions") g_psa_max_log2part = value < 0 ? GQ_PSA_MAX_LOG2PART : value;
   else return GQ_ERR_INVALID_ARG;
   return GQ_OK;
 }
@@ -1248,12 +1281,12 @@ gq_status gq_precompile_pipeline(const gq_plan* plan, char* h_msg, size_t msg_by
     PsaPlan pa = psa_plan(sp, &plan->agg, plan->in->nrows, plan->topk);
     if (pa.on) {
       GqScanSpec f = sp;
-      f.consumer = GQ_C_SCATTER; f.hot = false; f.part_rw = pa.rw; f.part_exprs = pa.exprs; f.part_states = pa.npart;
+      f.consumer = GQ_C_SCATTER; f.hot = pa.hot; f.part_rw = pa.rw; f.part_exprs = pa.exprs; f.part_states = pa.npart;
       st = precompile(f, h_msg, msg_bytes);
       if (st != GQ_OK) return st;
       std::string msg, path;
       CachedKernel* pk = nullptr;
-      st = get_psa_kernel_info(f, pa.log2slots, pa.src, &pk, &msg);
+      st = get_psa_kernel_info(f, pa.log2slots, pa.src, pa.threads, &pk, &msg);
       if (st == GQ_OK) st = gq_jit_compile_to_cache(pk->info, &path, &msg);
       if (st != GQ_OK) { if (h_msg && msg_bytes) { strncpy(h_msg, msg.c_str(), msg_bytes - 1); h_msg[msg_bytes - 1] = 0; } return st; }
     }

@@ -232,6 +232,15 @@ static gq_status emit_linear(Gen& g, const GqScanSpec& sp, std::ostringstream& o
     if (st != GQ_OK) return st;
   }
   auto aggval = [&](const gq_agg& a) { return a.op == GQ_COUNT_STAR ? std::string("1") : "e" + std::to_string(a.expr) + "[j]"; };
+  // hot keys of a skewed batch (DESIGN 5.4): rows whose key is in the batch's hot list are aggregated in CTA-shared
+  // memory and leave the row set; the CTA flushes its partial groups once, at the end of the kernel
+  auto emit_hot = [&]() {
+    o << "#if GQ_HOT\n  if (cx.nhot > 0) {\n  " << LOOP << "if (live[j]) {\n      const int hp = gq_hot_find(cx, tkey[j]);\n"
+      << "      if (hp >= 0) {\n";
+    for (int a = 0; a < nagg; ++a)
+      o << "        gq_hot_update(" << (int)sp.aggs[(size_t)a].op << ", cx, hp, " << a << ", " << aggval(sp.aggs[(size_t)a]) << ");\n";
+    o << "        cx.hot_touched[hp] = 1;\n        live[j] = false;\n      }\n    }\n  }\n#endif\n";
+  };
   switch (sp.consumer) {
     case GQ_C_GLOBAL:
       o << "  " << LOOP << "if (live[j]) {\n";
@@ -258,11 +267,7 @@ static gq_status emit_linear(Gen& g, const GqScanSpec& sp, std::ostringstream& o
     case GQ_C_PARTITION:
     case GQ_C_HIGHCARD: {
       o << "  i64 tkey[GQ_R];\n  " << LOOP << "tkey[j] = " << keyx << ";\n";
-      o << "#if GQ_HOT\n  if (cx.nhot > 0) {\n  " << LOOP << "if (live[j]) {\n      const int hp = gq_hot_find(cx, tkey[j]);\n"
-        << "      if (hp >= 0) {\n";
-      for (int a = 0; a < nagg; ++a)
-        o << "        gq_hot_update(" << (int)sp.aggs[(size_t)a].op << ", cx, hp, " << a << ", " << aggval(sp.aggs[(size_t)a]) << ");\n";
-      o << "        cx.hot_touched[hp] = 1;\n        live[j] = false;\n      }\n    }\n  }\n#endif\n";
+      emit_hot();
       if (sp.consumer == GQ_C_PARTITION) {
         // pass A of the radix-clustered aggregation: append (key, dependent key, aggregate inputs) to the record
         // buffer of the key's table partition; rows that do not fit (or carry the reserved key pattern) fall through
@@ -294,12 +299,14 @@ static gq_status emit_linear(Gen& g, const GqScanSpec& sp, std::ostringstream& o
       // pass A of the partitioned shared-memory aggregation: one record per surviving row, appended to a CTA-private
       // chunk of the partition the key hashes to (P.pshift = 64 - log2(partitions)); no table is touched here
       const int rw = sp.part_rw;
+      o << "  i64 tkey[GQ_R];\n  " << LOOP << "tkey[j] = " << keyx << ";\n";
+      emit_hot();
       o << "  u64 ridx[GQ_R];\n";
       o << "  " << LOOP << "{\n    ridx[j] = ~0ULL;\n    if (live[j]) ridx[j] = gq_scatter_reserve(P, cx.part_st, cx.sc_next, (u32)(gq_hash("
-        << keyx << ", 0) >> P.pshift));\n  }\n";
+        << "tkey[j], 0) >> P.pshift));\n  }\n";
       o << "  " << LOOP << "if (ridx[j] != ~0ULL) {\n    u64* rec = P.part + ridx[j] * " << rw << ";\n";
       std::vector<std::string> words;
-      words.push_back("(u64)(" + keyx + ")");
+      words.push_back("(u64)tkey[j]");
       if (sp.ndep == 1) words.push_back("(u64)" + depx);
       for (int e : sp.part_exprs) words.push_back("(u64)e" + std::to_string(e) + "[j]");
       while ((int)words.size() < rw) words.push_back("0ULL");
@@ -405,7 +412,7 @@ gq_status gq_codegen(const GqScanSpec& sp, GqKernelInfo* out, std::string* msg) 
   }
   bool all_unique = true;
   for (const GqProbeSpec& ps : sp.probes) all_unique = all_unique && ps.unique;
-  const bool use_hot = sp.hot && (sp.consumer == GQ_C_HIGHCARD || sp.consumer == GQ_C_PARTITION) && all_unique;   // linear mode only
+  const bool use_hot = sp.hot && (sp.consumer == GQ_C_HIGHCARD || sp.consumer == GQ_C_PARTITION || sp.consumer == GQ_C_SCATTER) && all_unique;   // linear mode only
   if (use_hot) cons_bytes = 512 * 8 + 512LL * nagg * 8 + 512 * 4 + 256;
   long long part_state_off = 0;
   if (sp.part_rw > 0) {   // partition state words (+ the CTA's chunk counter)
@@ -605,9 +612,10 @@ gq_status gq_codegen(const GqScanSpec& sp, GqKernelInfo* out, std::string* msg) 
 
 // Pass B of the partitioned shared-memory aggregation (gq_psa_kernel.cuh), specialised by the plan's aggregate list,
 // record layout and table slot layout. `src[a]` = record word holding the input of aggregate a (unused for COUNT).
-gq_status gq_codegen_psa(const GqScanSpec& sp, int log2slots, const int* src, GqKernelInfo* out, std::string* msg) {
+gq_status gq_codegen_psa(const GqScanSpec& sp, int log2slots, const int* src, int threads, GqKernelInfo* out, std::string* msg) {
   const int nagg = (int)sp.aggs.size();
-  if (nagg < 1 || nagg > GQ_MAX_AGGS || sp.part_rw < 4 || sp.part_rw % 4 || sp.target_sw < 2 || log2slots < 6 || log2slots > 16) {
+  if (nagg < 1 || nagg > GQ_MAX_AGGS || sp.part_rw < 4 || sp.part_rw % 4 || sp.target_sw < 2 || log2slots < 6 || log2slots > 16 ||
+      (threads != 512 && threads != 1024)) {
     if (msg) *msg = "bad partitioned-aggregation spec"; return GQ_ERR_INVALID_ARG; }
   std::ostringstream o;
   o << "// generated by gq_codegen_psa — plan-shape specialised prelude\n";
@@ -616,7 +624,8 @@ gq_status gq_codegen_psa(const GqScanSpec& sp, int log2slots, const int* src, Gq
     << "#define GQ_LC_G 1\n#define GQ_LC_KT 64\n#define GQ_LC_KEY32 0\n#define GQ_LC_KEY_BITS 1\n#define GQ_HOT 0\n#define GQ_PART_STATE_OFF 0\n"
     << "#define GQ_FUSED_FINAL 0\n#define GQ_DIRECT_AW 1\n#define GQ_COL_OFF(c) 0\n#define GQ_COL_BYTES(c) 8\n#define GQ_TX_BYTES 0\n";
   o << "#define GQ_NAGG " << nagg << "\n#define GQ_TARGET_SW " << sp.target_sw << "\n#define GQ_NDEP " << sp.ndep << "\n#define GQ_CHECK_DEP "
-    << (sp.check_dep ? 1 : 0) << "\n#define GQ_PART_RW " << sp.part_rw << "\n#define GQ_PSA_LOG2SLOTS " << log2slots << "\n";
+    << (sp.check_dep ? 1 : 0) << "\n#define GQ_PART_RW " << sp.part_rw << "\n#define GQ_PSA_LOG2SLOTS " << log2slots << "\n#define GQ_PSA_THREADS " << threads
+    << "\n#define GQ_PSA_U " << (threads == 1024 ? 2 : 4) << "\n";
   o << "#define GQ_AGG_OP(a) (";
   for (int a = 0; a < nagg; ++a) o << "(a) == " << a << " ? " << (int)sp.aggs[(size_t)a].op << " : ";
   o << "0)\n#define GQ_AGG_SRC(a) (";
@@ -628,7 +637,7 @@ gq_status gq_codegen_psa(const GqScanSpec& sp, int log2slots, const int* src, Gq
   snprintf(hb, sizeof hb, "%016llx", (unsigned long long)fnv1a(out->source));
   out->hash = hb;
   out->entry = "gq_psa";
-  out->threads = 512;
+  out->threads = threads;
   out->tile_rows = 0;
   out->smem_bytes = (int)((((1LL << log2slots) + 1) * sp.target_sw + 2 * 66) * 8 + 64);
   if (out->smem_bytes > GQ_SMEM_LIMIT) { if (msg) *msg = "partitioned-aggregation table does not fit shared memory"; return GQ_ERR_UNSUPPORTED; }

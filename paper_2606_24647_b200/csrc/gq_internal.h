@@ -170,7 +170,7 @@ struct GqKernelInfo {
 
 // gq_codegen.cpp
 gq_status gq_codegen(const GqScanSpec& spec, GqKernelInfo* out, std::string* msg);
-gq_status gq_codegen_psa(const GqScanSpec& spec, int log2slots, const int* src, GqKernelInfo* out, std::string* msg);
+gq_status gq_codegen_psa(const GqScanSpec& spec, int log2slots, const int* src, int threads, GqKernelInfo* out, std::string* msg);
 int gq_dtype_bytes(gq_dtype t);
 // gq_jit.cpp
 struct GqKernel { cudaKernel_t fn = nullptr; int threads = 0; int smem_bytes = 0; int tile_rows = 0; };
@@ -212,14 +212,15 @@ cudaError_t gq_launch_hot_keys(cudaStream_t s, const void* keycol, int dtype, lo
                                int max_hot, int num_sms, int* nlaunches);
 // ---- partitioned shared-memory aggregation (gq_psa_kernel.cuh, gq_psa.cu) ----
 #define GQ_MAX_SMS 160               // workspace sizing bound for the per-CTA chunk ranges of pass A
+#define GQ_PSA_MAX_LOG2PART 14        // default cap on pass-A partitions (planner knob "psa_max_log2_partitions")
 #define GQ_PSA_GID_BITS 26           // directory entry = chunk id | records used << 26
 struct GqPsaParams {                 // must match gq_psa_kernel.cuh
   const unsigned long long* rec; const unsigned* plist; const unsigned* pstart; const unsigned* items; const unsigned* item_seg;
-  const unsigned* nitems; unsigned* work; int* err; GqTableDev merge; unsigned seg_chunks; int hshift; GqFinal fin;
+  const unsigned* nitems; unsigned* work; int* err; GqTableDev merge; unsigned seg_chunks; int hshift; int log2sub; int pad; GqFinal fin;
 };
 struct GqPsaDirParams {
   const unsigned* pcount; unsigned* pstart; unsigned* items; unsigned* item_seg; unsigned* nitems; int npart; unsigned seg_chunks;
-  int* err; unsigned max_items;
+  int* err; unsigned max_items; unsigned nsub;
 };
 cudaError_t gq_launch_psa_dir(cudaStream_t s, const GqPsaDirParams& p);
 cudaError_t gq_launch_psa_fill(cudaStream_t s, const unsigned* info, const unsigned* ncta, int nctas, long long slab,

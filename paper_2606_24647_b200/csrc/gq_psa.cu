@@ -37,7 +37,7 @@ __global__ void __launch_bounds__(GQ_DIR_THREADS) gq_k_psa_dir(const __grid_cons
   auto cls = [&](u32 n) { return n > P.seg_chunks ? 0 : n > big ? 1 : 2; };
   for (int p = lo; p < hi; ++p) {
     const u32 n = P.pcount[p];
-    if (n) atomicAdd(&cls_n[cls(n)], n > P.seg_chunks ? (n + P.seg_chunks - 1) / P.seg_chunks : 1u);
+    if (n) atomicAdd(&cls_n[cls(n)], (n > P.seg_chunks ? (n + P.seg_chunks - 1) / P.seg_chunks : 1u) * P.nsub);
   }
   __syncthreads();
   if (t == 0) {
@@ -51,8 +51,10 @@ __global__ void __launch_bounds__(GQ_DIR_THREADS) gq_k_psa_dir(const __grid_cons
     const u32 n = P.pcount[p];
     if (!n) continue;
     const u32 k = n > P.seg_chunks ? (n + P.seg_chunks - 1) / P.seg_chunks : 1u;
-    const u32 at = atomicAdd(&cls_cur[cls(n)], k);
-    for (u32 i = 0; i < k; ++i) { P.items[at + i] = (u32)p; P.item_seg[at + i] = i; }
+    const u32 at = atomicAdd(&cls_cur[cls(n)], k * P.nsub);   // the sub-passes of a segment are neighbours in the queue: the
+    for (u32 i = 0; i < k * P.nsub; ++i) {                     // CTAs that draw them stream the same chunks at the same time (L2)
+      P.items[at + i] = (u32)p; P.item_seg[at + i] = (i / P.nsub) | ((i % P.nsub) << 24);
+    }
   }
 }
 cudaError_t gq_launch_psa_dir(cudaStream_t s, const GqPsaDirParams& p) {

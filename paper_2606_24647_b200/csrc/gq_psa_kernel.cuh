@@ -9,7 +9,10 @@
 //   - the CTA streams the item's chunks from HBM exactly once (coalesced 32-byte records, GQ_PSA_U chunks in flight
 //     per warp) and aggregates them in its shared-memory table: open addressing, linear probing, ATOMS.CAS.64 to
 //     claim a key, SUM/COUNT as 32-bit ATOMS.ADD pairs with explicit carry (64-bit shared atomics are CAS loops on
-//     sm_100), MIN/MAX as compare-then-CAS — no global atomic and no global table on the per-row path;
+//     sm_100), MIN/MAX as compare-then-CAS — no global atomic and no global table on the per-row path. The 32 records
+//     of a chunk go through the table TOGETHER (gq_psa_row: warp-converged probe rounds, straight-line updates): with
+//     one data-dependent loop per lane the warp executed every lane's path in turn (12 of 32 lanes active, 490
+//     warp instructions per chunk);
 //   - then writes its groups straight into the dense output columns (ONE global atomic per item reserves the rows).
 // Heavy partitions (hot keys) are cut into segments handled by different CTAs; a segment flushes its partial groups
 // into a small global merge table with the ordinary insert-or-update protocol, emitted afterwards by gq_k_finalise.
@@ -17,13 +20,13 @@
 // is halved (by a second, bijective hash) and the chunks are streamed again for each half, recursively.
 //
 // Prelude macros used: GQ_NAGG, GQ_AGG_OP(a), GQ_AGG_SRC(a) (record word of the aggregate's input; unused for COUNT),
-// GQ_NDEP, GQ_CHECK_DEP, GQ_TARGET_SW (words per table slot), GQ_PART_RW (words per record), GQ_PSA_LOG2SLOTS.
+// GQ_NDEP, GQ_CHECK_DEP, GQ_TARGET_SW (words per table slot), GQ_PART_RW (words per record), GQ_PSA_LOG2SLOTS,
+// GQ_PSA_THREADS, GQ_PSA_U (chunks in flight per warp).
 
-#define GQ_PSA_THREADS 512
-#define GQ_PSA_NW (GQ_PSA_THREADS / 32)
-#define GQ_PSA_U 4                                   // chunks in flight per warp
+#define GQ_PSA_NW (GQ_PSA_THREADS / 32)            // GQ_PSA_THREADS, GQ_PSA_U (chunks in flight per warp): prelude
 #define GQ_PSA_SLOTS (1 << GQ_PSA_LOG2SLOTS)
-#define GQ_PSA_LIMIT (GQ_PSA_SLOTS - GQ_PSA_SLOTS / 8 - GQ_PSA_THREADS)   // groups a table takes before it gives up
+// groups a table takes before it gives up: every thread may have one more claim in flight when the count is checked
+#define GQ_PSA_LIMIT (GQ_PSA_SLOTS - GQ_PSA_SLOTS / 16 - GQ_PSA_THREADS)
 #define GQ_PSA_SW GQ_TARGET_SW
 #define GQ_PSA_RW GQ_PART_RW
 #define GQ_PSA_TABW ((GQ_PSA_SLOTS + 1) * GQ_PSA_SW)  // + the side slot (key == the reserved EMPTY pattern, S14)
@@ -35,13 +38,15 @@ struct GqPsaParams {
   const u32* plist;      // directory: chunk entries grouped by partition
   const u32* pstart;     // [partitions + 1] first directory entry of every partition
   const u32* items;      // work items: partition | segment << 16 ... see item_seg
-  const u32* item_seg;   // segment index of the item inside its partition (0 for unsplit partitions)
+  const u32* item_seg;   // segment index of the item inside its partition (0 for unsplit partitions) | sub-pass << 24
   const u32* nitems;     // device scalar
   u32* work;             // queue cursor (zero before the launch)
   int* err;
   GqTableDev merge;      // global merge table for the segments of split partitions
   u32 seg_chunks;        // chunks per segment (partitions with more chunks are split)
   int hshift;            // partition = hash >> hshift
+  int log2sub;           // every partition is aggregated in 2^log2sub sub-passes (work items), one per value of the next hash bits
+  int pad;
   GqFinal fin;
 };
 
@@ -51,21 +56,6 @@ __device__ __forceinline__ u64 gq_psa_mix(u64 x) {   // bijective finaliser: dis
   x ^= x >> 33; x *= 0xff51afd7ed558ccdULL; x ^= x >> 33; x *= 0xc4ceb9fe1a85ec53ULL; x ^= x >> 33;
   return x;
 }
-__device__ __forceinline__ void gq_psa_add(u64* cell, i64 v) {
-  u32* w = (u32*)cell;
-  const u32 lo = (u32)(u64)v, hi = (u32)((u64)v >> 32);
-  const u32 old = atomicAdd(w, lo);
-  const u32 up = hi + ((u32)(old + lo) < old ? 1u : 0u);     // the carry out of the low word belongs to THIS addition
-  if (up) atomicAdd(w + 1, up);
-}
-__device__ __forceinline__ void gq_psa_minmax(const int OP, u64* cell, i64 v) {
-  i64 cur = *(volatile i64*)cell;
-  while (OP == GQ_OP_MIN ? v < cur : v > cur) {
-    const i64 prev = (i64)atomicCAS(cell, (u64)cur, (u64)v);
-    if (prev == cur) break;
-    cur = prev;
-  }
-}
 __device__ __forceinline__ u64 gq_psa_init_word(int q) {    // word q of an empty slot
   if (q == 0) return GQ_EMPTY;
   u64 v = GQ_CHECK_DEP ? GQ_DEP_UNSET : 0ULL;
@@ -74,42 +64,75 @@ __device__ __forceinline__ u64 gq_psa_init_word(int q) {    // word q of an empt
   return v;
 }
 
-// Slot of `key` in the shared table (claimed on first sight); nullptr once the table has given up.
-__device__ __forceinline__ u64* gq_psa_find(u64* tab, u32* ctl, u64 key, u64 h, int hshift, bool* won) {
-  *won = false;
-  if (key == GQ_EMPTY) {
-    *won = atomicExch(&ctl[GQ_PSA_SIDE], 1u) == 0u;
-    return tab + (size_t)GQ_PSA_SLOTS * GQ_PSA_SW;
+// One record per lane, all 32 lanes of the warp together (converged): finds or claims the slot of every active
+// lane's key and applies the record's aggregate inputs. The probe loop runs until no lane is pending, so the warp
+// executes it once per round, not once per lane; new groups are counted with one atomic per warp; the updates are
+// straight-line code (SUM/COUNT: a 32-bit ATOMS.ADD and, only when there is a carry or a high word, a second one;
+// MIN/MAX: compare first, CAS only to improve).
+__device__ __forceinline__ void gq_psa_row(u64* tab, u32* ctl, const u64 (&w)[GQ_PSA_RW], bool act, u64 h, int tshift, int* err) {
+  const u64 key = w[0];
+  u64* slot = nullptr;
+  bool won = false, side_won = false;
+  if (act && key == GQ_EMPTY) {                         // reserved bit pattern (S14): the side slot, counted by GQ_PSA_SIDE
+    side_won = atomicExch(&ctl[GQ_PSA_SIDE], 1u) == 0u;
+    slot = tab + (size_t)GQ_PSA_SLOTS * GQ_PSA_SW;
   }
-  u32 i = (u32)(h >> (hshift - GQ_PSA_LOG2SLOTS)) & (GQ_PSA_SLOTS - 1);
-  for (u32 n = 0; n < GQ_PSA_SLOTS; ++n, i = (i + 1) & (GQ_PSA_SLOTS - 1)) {
-    u64* s = tab + (size_t)i * GQ_PSA_SW;
-    const u64 k = *(volatile u64*)s;
-    if (k == key) return s;
-    if (k == GQ_EMPTY) {
-      if (((volatile u32*)ctl)[GQ_PSA_OVF]) return nullptr;
-      const u64 prev = atomicCAS(s, GQ_EMPTY, key);
-      if (prev == GQ_EMPTY) {
-        *won = true;
-        if (atomicAdd(&ctl[GQ_PSA_NG], 1u) >= (u32)GQ_PSA_LIMIT) ((volatile u32*)ctl)[GQ_PSA_OVF] = 1u;
-        return s;
-      }
-      if (prev == key) return s;
+  bool pend = act && slot == nullptr;
+  u32 i = (u32)(h >> (tshift - GQ_PSA_LOG2SLOTS)) & (GQ_PSA_SLOTS - 1);
+  for (int n = 0; __any_sync(0xffffffffu, pend); ++n) {
+    if (pend) {
+      u64* s = tab + (size_t)i * GQ_PSA_SW;
+      const u64 k = *(volatile u64*)s;
+      if (k == key) { slot = s; pend = false; }
+      else if (k == GQ_EMPTY) {
+        if (((volatile u32*)ctl)[GQ_PSA_OVF]) pend = false;                 // the table has given up: the item is redone
+        else {
+          const u64 prev = atomicCAS(s, GQ_EMPTY, key);
+          if (prev == GQ_EMPTY) { slot = s; won = true; pend = false; }
+          else if (prev == key) { slot = s; pend = false; }
+          else i = (i + 1) & (GQ_PSA_SLOTS - 1);
+        }
+      } else i = (i + 1) & (GQ_PSA_SLOTS - 1);
+      if (n > GQ_PSA_SLOTS) { ((volatile u32*)ctl)[GQ_PSA_OVF] = 1u; pend = false; }
     }
   }
-  ((volatile u32*)ctl)[GQ_PSA_OVF] = 1u;
-  return nullptr;
-}
-
-__device__ __forceinline__ void gq_psa_dep(u64* w, u64 dep, bool won, int* err) {
+  const u32 wm = __ballot_sync(0xffffffffu, won);
+  if (wm != 0u && (threadIdx.x & 31) == (u32)(__ffs(wm) - 1)) {
+    const u32 c = (u32)__popc(wm);
+    if (atomicAdd(&ctl[GQ_PSA_NG], c) + c > (u32)GQ_PSA_LIMIT) ((volatile u32*)ctl)[GQ_PSA_OVF] = 1u;
+  }
+  if (slot != nullptr) {
 #if GQ_NDEP
 #if GQ_CHECK_DEP
-  const u64 prev = atomicCAS(w, GQ_DEP_UNSET, dep);
-  if (prev != GQ_DEP_UNSET && prev != dep) gq_set_err(err, GQ_E_DEPENDENT);
+    { const u64 prev = atomicCAS(slot + 1, GQ_DEP_UNSET, w[1]); if (prev != GQ_DEP_UNSET && prev != w[1]) gq_set_err(err, GQ_E_DEPENDENT); }
 #else
-  if (won) *(volatile u64*)w = dep;
+    if (won || side_won) *(volatile u64*)(slot + 1) = w[1];
 #endif
 #endif
+#pragma unroll
+    for (int a = 0; a < GQ_NAGG; ++a) {
+      const int op = GQ_AGG_OP(a);
+      u64* cell = slot + 1 + GQ_NDEP + a;
+      if (op == GQ_OP_COUNT) {
+        const u32 old = atomicAdd((u32*)cell, 1u);
+        if (old == 0xFFFFFFFFu) atomicAdd((u32*)cell + 1, 1u);
+      } else if (op == GQ_OP_SUM) {
+        const u64 v = w[GQ_AGG_SRC(a)];
+        const u32 lo = (u32)v, hi = (u32)(v >> 32);
+        const u32 old = atomicAdd((u32*)cell, lo);
+        const u32 up = hi + ((u32)(old + lo) < old ? 1u : 0u);   // the carry out of the low word belongs to THIS addition
+        if (up) atomicAdd((u32*)cell + 1, up);
+      } else {
+        const i64 v = (i64)w[GQ_AGG_SRC(a)];
+        i64 cur = *(volatile i64*)cell;
+        while (op == GQ_OP_MIN ? v < cur : v > cur) {
+          const i64 prev = (i64)atomicCAS(cell, (u64)cur, (u64)v);
+          if (prev == cur) break;
+          cur = prev;
+        }
+      }
+    }
+  }
 }
 
 __device__ __forceinline__ i64 gq_psa_sext(u64 v, int bits) {
@@ -159,7 +182,8 @@ extern "C" __global__ void __launch_bounds__(GQ_PSA_THREADS, 1) gq_psa(const __g
     __syncthreads();
     const u32 item = ctl[GQ_PSA_ITEM];
     if (item >= nitems) break;
-    const u32 part = P.items[item], seg = P.item_seg[item];
+    const u32 part = P.items[item], seg = P.item_seg[item] & 0xFFFFFFu, sub = P.item_seg[item] >> 24;
+    const int tshift = P.hshift - P.log2sub;            // the table index comes from the hash bits below partition and sub-pass
     const u32 p0 = P.pstart[part], p1 = P.pstart[part + 1];
     const bool split = (p1 - p0) > P.seg_chunks;      // this item is one segment of a heavy partition
     const u32 c0 = split ? p0 + seg * P.seg_chunks : p0;
@@ -196,23 +220,12 @@ extern "C" __global__ void __launch_bounds__(GQ_PSA_THREADS, 1) gq_psa(const __g
         }
 #pragma unroll
         for (int u = 0; u < GQ_PSA_U; ++u) {
-          if (!live[u]) continue;
           const u64 key = w[u][0];
-          if (filt) { const u64 h2 = gq_psa_mix(key); if (h2 < lo || h2 > hi) continue; }
-          bool won;
-          u64* slot = gq_psa_find(tab, ctl, key, gq_hash((i64)key, 0), P.hshift, &won);
-          if (!slot) continue;
-#if GQ_NDEP
-          gq_psa_dep(slot + 1, w[u][1], won, P.err);
-#endif
-#pragma unroll
-          for (int a = 0; a < GQ_NAGG; ++a) {
-            const int op = GQ_AGG_OP(a);
-            const i64 v = op == GQ_OP_COUNT ? 1 : (i64)w[u][op == GQ_OP_COUNT ? 0 : GQ_AGG_SRC(a)];
-            u64* cell = slot + 1 + GQ_NDEP + a;
-            if (op == GQ_OP_SUM || op == GQ_OP_COUNT) gq_psa_add(cell, v);
-            else gq_psa_minmax(op, cell, v);
-          }
+          const u64 h = gq_hash((i64)key, 0);
+          bool act = live[u];
+          if (P.log2sub) act = act && (u32)((h >> tshift) & ((1u << P.log2sub) - 1u)) == sub;   // another sub-pass owns this key
+          if (filt) { const u64 h2 = gq_psa_mix(key); act = act && h2 >= lo && h2 <= hi; }
+          gq_psa_row(tab, ctl, w[u], act, h, tshift, P.err);
         }
       }
       __syncthreads();
