@@ -632,22 +632,18 @@ PsaPlan psa_plan(const GqScanSpec& sp, const gq_agg_desc* d, int64_t nrows, int 
   const int sw = sp.target_sw;
   if ((int64_t)agg_capacity(d->max_groups, d->nkeys) * sw * 8 < g_part_min_table_mb.load() * (1 << 20) || nrows < g_part_min_rows.load()) return pp;
   int L = 6;
-  while ((((1LL << (L + 1)) + 1) * sw + 2 * 66) * 8 + 64 <= GQ_SMEM_LIMIT) ++L;
-  if ((((1LL << L) + 1) * sw + 2 * 66) * 8 + 64 > GQ_SMEM_LIMIT) return pp;
+  auto psa_smem = [sw](int l) { return (((1LL << l) + 1) * sw + 2 * 66) * 8 + 64; };   // as gq_codegen_psa sizes it
+  while (psa_smem(L + 1) <= GQ_SMEM_LIMIT) ++L;
+  if (psa_smem(L) > GQ_SMEM_LIMIT) return pp;
   pp.log2slots = L;
   // groups a shared-memory table takes (gq_psa_kernel.cuh GQ_PSA_LIMIT), less 5 % for the spread of a hash partitioning
   const int64_t slots = 1LL << L;
-  auto limit_for = [slots](int threads) { return (slots - slots / 16 - threads) * 19 / 20; };
-  int64_t limit = limit_for(512);
+  const int64_t limit = (slots - slots / 4) * 19 / 20;
   if (limit < 32) return pp;
   int lp = 6;                                               // 64 .. 16384 key ranges; more groups than that: the key
   while (lp < 14 && (d->max_groups + limit - 1) / limit > (1LL << lp)) ++lp;   // ranges are halved in pass B instead
-  // 32 warps hide more of the table's dependent shared-memory round trips than 16; taken when the tables still hold the plan's groups
-  const int64_t want = g_psa_threads.load();   // 0 = decide here, 512 / 1024 = the planner's choice
-  pp.threads = want == 512 ? 512 : want == 1024 ? 1024
-             : (limit_for(1024) >= 32 && (d->max_groups + limit_for(1024) - 1) / limit_for(1024) <= (1LL << lp)) ? 1024 : 512;
-  if (limit_for(pp.threads) < 32) return pp;
-  limit = limit_for(pp.threads);
+  // 32 warps hide more of the table's dependent shared-memory round trips than 16 (C5 pass B 6.95 -> 5.27 ms)
+  pp.threads = g_psa_threads.load() == 512 ? 512 : 1024;
   // Pass A scatters into at most 2^psa_max_log2part partitions: every (CTA, partition) pair has an open 128-byte line of
   // records, and those lines must stay in L2 until they are full, or every record becomes a random 32-byte DRAM write.
   // The remaining key-range bits are resolved in pass B: 2^log2sub sub-passes per partition, one per work item.

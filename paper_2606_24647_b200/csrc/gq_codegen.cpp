@@ -304,6 +304,7 @@ static gq_status emit_linear(Gen& g, const GqScanSpec& sp, std::ostringstream& o
       o << "  u64 ridx[GQ_R];\n";
       o << "  " << LOOP << "{\n    ridx[j] = ~0ULL;\n    if (live[j]) ridx[j] = gq_scatter_reserve(P, cx.part_st, cx.sc_next, (u32)(gq_hash("
         << "tkey[j], 0) >> P.pshift));\n  }\n";
+      o << "  const u64 keep = gq_policy_evict_last();\n";
       o << "  " << LOOP << "if (ridx[j] != ~0ULL) {\n    u64* rec = P.part + ridx[j] * " << rw << ";\n";
       std::vector<std::string> words;
       words.push_back("(u64)tkey[j]");
@@ -311,7 +312,7 @@ static gq_status emit_linear(Gen& g, const GqScanSpec& sp, std::ostringstream& o
       for (int e : sp.part_exprs) words.push_back("(u64)e" + std::to_string(e) + "[j]");
       while ((int)words.size() < rw) words.push_back("0ULL");
       for (int w = 0; w < rw; w += 4)
-        o << "    gq_st256(rec + " << w << ", " << words[(size_t)w] << ", " << words[(size_t)w + 1] << ", " << words[(size_t)w + 2] << ", " << words[(size_t)w + 3] << ");\n";
+        o << "    gq_st256_keep(rec + " << w << ", " << words[(size_t)w] << ", " << words[(size_t)w + 1] << ", " << words[(size_t)w + 2] << ", " << words[(size_t)w + 3] << ", keep);\n";
       o << "  }\n";
       break;
     }
@@ -639,7 +640,7 @@ gq_status gq_codegen_psa(const GqScanSpec& sp, int log2slots, const int* src, in
   out->entry = "gq_psa";
   out->threads = threads;
   out->tile_rows = 0;
-  out->smem_bytes = (int)((((1LL << log2slots) + 1) * sp.target_sw + 2 * 66) * 8 + 64);
+  out->smem_bytes = (int)((((1LL << log2slots) + 1) * sp.target_sw + 2 * 66) * 8 + 64);   // table, range stack, control words
   if (out->smem_bytes > GQ_SMEM_LIMIT) { if (msg) *msg = "partitioned-aggregation table does not fit shared memory"; return GQ_ERR_UNSUPPORTED; }
   return GQ_OK;
 }

@@ -25,8 +25,9 @@
 
 #define GQ_PSA_NW (GQ_PSA_THREADS / 32)            // GQ_PSA_THREADS, GQ_PSA_U (chunks in flight per warp): prelude
 #define GQ_PSA_SLOTS (1 << GQ_PSA_LOG2SLOTS)
-// groups a table takes before it gives up: every thread may have one more claim in flight when the count is checked
-#define GQ_PSA_LIMIT (GQ_PSA_SLOTS - GQ_PSA_SLOTS / 16 - GQ_PSA_THREADS)
+// Groups a table takes before it gives up (load 0.75). The count is checked once per warp and row, so up to
+// GQ_PSA_THREADS further claims may be in flight: a table that fills up completely is caught by the probe loop's guard.
+#define GQ_PSA_LIMIT (GQ_PSA_SLOTS - GQ_PSA_SLOTS / 4)
 #define GQ_PSA_SW GQ_TARGET_SW
 #define GQ_PSA_RW GQ_PART_RW
 #define GQ_PSA_TABW ((GQ_PSA_SLOTS + 1) * GQ_PSA_SW)  // + the side slot (key == the reserved EMPTY pattern, S14)
@@ -197,7 +198,10 @@ extern "C" __global__ void __launch_bounds__(GQ_PSA_THREADS, 1) gq_psa(const __g
       const bool filt = !(lo == 0ULL && hi == ~0ULL);
       __syncthreads();
       // ---- empty table
-      for (int i = tid; i < GQ_PSA_TABW; i += GQ_PSA_THREADS) tab[i] = gq_psa_init_word(i % GQ_PSA_SW);
+      for (int i = tid; i <= GQ_PSA_SLOTS; i += GQ_PSA_THREADS) {
+#pragma unroll
+        for (int q = 0; q < GQ_PSA_SW; ++q) tab[(size_t)i * GQ_PSA_SW + q] = gq_psa_init_word(q);   // constants after unrolling
+      }
       if (tid == 0) { ctl[GQ_PSA_NG] = 0; ctl[GQ_PSA_OVF] = 0; ctl[GQ_PSA_CUR] = 0; ctl[GQ_PSA_SIDE] = 0; ctl[GQ_PSA_SP] = sp - 1; }
       __syncthreads();
       // ---- stream the item's chunks: GQ_PSA_U chunks of 32 records per warp in flight

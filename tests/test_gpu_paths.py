@@ -374,6 +374,32 @@ def test_partitioned_shared_memory_aggregation_heavy_keys_and_many_groups(ctx, f
     assert got["n"] == n
 
 
+def test_partitioned_shared_memory_aggregation_hot_keys_and_sub_passes(ctx, force_partition):
+    # pass A aggregates the batch's most frequent keys in shared memory (they never become records; their groups reach
+    # the output through the merge table), and with fewer pass-A partitions than key ranges pass B runs sub-passes
+    from paper_2606_24647_b200 import gq
+    rng = np.random.default_rng(15)
+    n = 900_000
+    k = (rng.zipf(1.3, n) % 300_000).astype(np.int64) * 7 - 1000          # a few very hot keys, a long tail
+    k[::5000] = I64_MIN
+    v = rng.integers(-10**9, 10**9, n).astype(np.int64)
+    w = rng.integers(0, 50, n).astype(np.int64)
+    plan = dict(table=[k, v, w], preds=[(2, "lt", 45)], exprs=[[("col", 1)], [("col", 2)]], keys=[0],
+                aggs=[("sum", 0), ("sum", 1), ("min", 0), ("max", 0), ("count",)], max_groups=300_000)
+    try:
+        gq.set_option("hot_min_rows", 4096)
+        for lp in (14, 6, 5):
+            gq.set_option("psa_max_log2_partitions", lp)
+            for th in (512, 1024):
+                gq.set_option("psa_threads", th)
+                l0 = ctx.launch_count()
+                exp, got = run(plan, ctx)
+                assert ctx.launch_count() - l0 == 10     # + table init and three kernels of the heavy-hitter sampling
+                assert int(got["cols"][-1].max()) > 100_000
+    finally:
+        gq.set_option("hot_min_rows", -1); gq.set_option("psa_max_log2_partitions", -1); gq.set_option("psa_threads", 0)
+
+
 def test_partitioned_aggregation_streams_batches(ctx, force_partition):
     import gqrun
     plan = plans.plan_c5(datagen.make_config(5, scale=0.004))
