@@ -1,21 +1,21 @@
 #!/usr/bin/env python
 """bench.py — measures the hot path on B200 (contract: prompt §④ / "Maintain bench.py").
 
-    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--configs 1,3,4,5] [--c5-scale S]
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--configs 1,1x64,3,4,5,ops]
 
-A step = one pass of the whole fused pipeline (table init -> fused scan kernel -> finaliser) over one batch of
-synthetic input. Headline workload: BASELINE.json configs[1] (C2: selective filter + global SUM over 60 M rows, the
-pure scan-bandwidth test the metric's >=70 % target is quoted on). The other configs are measured once each and
-reported under "per_config" in the same JSON line. Inputs (1.68 GB) are larger than L2 (126 MB), so every timed
-iteration reads HBM. N > 1 (torchrun): the path does not shard — each rank runs an independent replica ("replicas
-only") and value = N * rows / max-over-ranks time.
+A step = one pass of the whole fused pipeline (table init -> builds -> fused scan kernel -> finaliser) over one batch
+of synthetic input. Headline workload: BASELINE.json configs[1] (C2: selective filter + global SUM over 60 M rows, the
+pure scan-bandwidth test the metric's >= 70 % target is quoted on). Every other config is measured in the same run and
+reported under "per_config" with the same record: pipeline ms, per-kernel device times (gq_profile), the dominant
+kernel's roofline, parity against the oracle (stored oracle-written digests at full size), clocks. Inputs are larger
+than L2 (C1: rotated copies), so every timed iteration reads HBM. N > 1 (torchrun): the path does not shard — each
+rank runs an independent replica ("replicas only") and value = N * rows / max-over-ranks time.
 """
 from __future__ import annotations
 
 import argparse
 import json
 import os
-import subprocess
 import sys
 import threading
 import time
@@ -28,7 +28,10 @@ for p in (ROOT, os.path.join(ROOT, "tests")):
 import numpy as np  # noqa: E402
 
 METRIC = "input rows/s and achieved HBM GB/s (% of B200 peak) per operator pipeline"
+WORKLOAD = "C2 selective filter + global SUM(price*discount), 60M-row fact (BASELINE configs[1])"
 ALG_BYTES_PER_ROW = {1: 38, 2: 28, 3: 28, 4: 28, 5: 28}   # referenced fact columns, SURVEY §8(d)
+L2_NOTE = "inputs (1.68 GB) are larger than L2: every timed iteration reads HBM (no flush needed)"
+MIN_LOAD_MS = 120.0                                      # the clock sampler sees at least this much load per loop
 
 
 def peaks():
@@ -39,8 +42,26 @@ def peaks():
     return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
 
 
+def host_info():
+    model, mem = None, None
+    try:
+        with open("/proc/cpuinfo") as f:
+            for line in f:
+                if line.startswith("model name"):
+                    model = line.split(":", 1)[1].strip()
+                    break
+        with open("/proc/meminfo") as f:
+            for line in f:
+                if line.startswith("MemTotal"):
+                    mem = line.split(":", 1)[1].strip()
+                    break
+    except OSError:
+        pass
+    return dict(nproc=os.cpu_count(), cpu_model=model, mem_total=mem)
+
+
 class ClockSampler:
-    """Samples SM clock and clock-event (throttle) reasons through NVML in a thread during the timed region."""
+    """Samples SM clock and clock-event (throttle) reasons through NVML in a thread while a loop runs."""
     BITS = dict(sw_power_cap=0x4, hw_slowdown=0x8, sw_thermal_slowdown=0x20, hw_thermal_slowdown=0x40)
 
     def __init__(self, index=0):
@@ -70,6 +91,7 @@ class ClockSampler:
             self._t.start()
         except Exception:
             self._t = None
+        return self
 
     def stop(self):
         self._stop.set()
@@ -77,7 +99,7 @@ class ClockSampler:
             self._t.join(timeout=1.0)
         return dict(sm_mhz=float(np.median(self.sm)) if self.sm else None, sm_max_mhz=self.max,
                     reasons=[n for n, b in self.BITS.items() if self.reasons & b], samples=len(self.sm),
-                    power_w_max=max(self.power) if self.power else None)
+                    span="sampled every 2 ms across warm-up + timed loop", power_w_max=max(self.power) if self.power else None)
 
 
 def dist():
@@ -102,13 +124,24 @@ def whole_job_value(local_total_ms, rows_per_rank, steps, td=None, device=None):
     return ms_per_step, ws * rows_per_rank / ms_per_step * 1e3
 
 
-def time_steps(torch, stream, fn, steps, warmup, barrier):
-    """W untimed + K timed calls of fn, CUDA events on the launching stream; returns total ms (this rank)."""
-    for _ in range(warmup):
-        fn()
-    torch.cuda.synchronize()
-    barrier()
+def time_steps(torch, stream, fn, steps, warmup, barrier, min_load_ms=0.0):
+    """W untimed calls of fn (plus, when min_load_ms is given, further untimed calls until the GPU has been under load
+    that long, so that a clock sampler running beside the loop collects enough samples), then EXACTLY `steps` timed
+    calls bracketed by CUDA events on the launching stream; returns the timed total in ms (this rank)."""
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    with torch.cuda.stream(stream):
+        e0.record(stream)
+        for _ in range(warmup):
+            fn()
+        e1.record(stream)
+    torch.cuda.synchronize()
+    if min_load_ms > 0:
+        per = max(e0.elapsed_time(e1) / max(1, warmup), 1e-3)
+        need = min_load_ms - steps * per
+        for _ in range(int(min(200_000, max(0.0, need) / per))):
+            fn()
+    barrier()
+    torch.cuda.synchronize()
     with torch.cuda.stream(stream):
         e0.record(stream)
         for _ in range(steps):
@@ -131,23 +164,91 @@ def parse_configs(text, c5_scale):
     return out
 
 
-def run_config(cfg, gq, ctx, torch, datagen, plans, gqrun, steps, warmup, scale=1.0, peak=6548.2):
-    """Device-resident timing of one config: whole pipeline (builds + fused scan + finalise) and its scan kernel."""
+def load_digests():
+    with open(os.path.join(ROOT, "tests", "golden", "fullsize_digests.json")) as f:
+        return json.load(f)
+
+
+def load_traffic():
+    path = os.path.join(ROOT, "profiles", "traffic.json")   # dram bytes per launch from the committed ncu captures
+    if os.path.exists(path):
+        with open(path) as f:
+            return json.load(f)
+    return {}
+
+
+def result_columns(torch, res, nkeys):
+    """Output columns of a pipeline as int64 numpy arrays sorted by the first key (group order is unspecified)."""
+    cols = [k.to(torch.int64) for k in res["keys"]] + list(res["aggs"])
+    if nkeys and res["n"] > 1:
+        order = torch.argsort(cols[0])
+        cols = [c[order] for c in cols]
+    return [c.cpu().numpy() for c in cols]
+
+
+def result_rows(torch, res):
+    cols = [k.to(torch.int64).cpu().numpy() for k in res["keys"]] + [a.cpu().numpy() for a in res["aggs"]]
+    return [[int(c[i]) for c in cols] for i in range(res["n"])]
+
+
+def check_parity(torch, cfg, scale, plan, res, digests):
+    """The timed configuration's output against the oracle: C1 (any scale the oracle finishes in seconds) by running
+    the oracle on the same plan; C2-C5 at full size against the oracle-written digests of tests/golden/ (whole table;
+    C3's timed plan is the top-10, compared row by row)."""
+    import golden_util
+    import oracle
+    nkeys = len(plan.get("keys", []))
+    if cfg == 1 and scale <= 4.0:
+        exp = oracle.run_query(plan)
+        got = result_columns(torch, res, nkeys)
+        if nkeys > 1:
+            order = np.lexsort(tuple(got[k] for k in reversed(range(nkeys))))
+            got = [c[order] for c in got]
+        return dict(ok=bool(res["n"] == exp.nrows and all(np.array_equal(g, e) for g, e in zip(got, exp.cols))),
+                    how="oracle.run_query on the same plan, every output row")
+    if scale != 1.0 or f"C{cfg}" not in digests:
+        return dict(ok=None, how="no stored digest for this scale")
+    d = digests[f"C{cfg}"]
+    if plan.get("topk", 0):
+        return dict(ok=bool(result_rows(torch, res) == d["top10"]), how="top-10 rows == oracle's (tests/golden/fullsize_digests.json)")
+    got = result_columns(torch, res, nkeys)
+    ok = res["n"] == d["ngroups"] and golden_util.digest_columns(got) == d["columns"]
+    return dict(ok=bool(ok), how=f"whole table ({d['ngroups']} groups): per-column sum/xor/SHA-256 == oracle-written digests "
+                                 "(tests/golden/fullsize_digests.json)")
+
+
+def run_config(cfg, gq, ctx, torch, datagen, plans, gqrun, steps, warmup, scale=1.0, peak=6548.2, dense=True, hinted=True,
+               detail=False, digests=None, traffic=None, dev=None):
+    """Device-resident timing of one config: whole pipeline (builds + fused scan + finalise). detail=True adds the
+    per-kernel device times of one profiled step, the dominant kernel's roofline, parity and clocks."""
     t0 = time.time()
     tabs = datagen.make_config(cfg, scale=scale)
     plan = plans.PLANS[cfg](tabs, topk=10) if cfg == 3 else plans.PLANS[cfg](tabs)
     gen_s = time.time() - t0
     nrows = len(plan["table"][0])
+    l2 = float(dev["l2_bytes"]) if dev else 126e6
     ncopies = 1
     fact_bytes = sum(c.nbytes for c in plan["table"])
-    if fact_bytes < 2 * 126e6:               # C1: rotate copies so every timed rep reads cold HBM (SURVEY §7.2-1)
-        ncopies = int(np.ceil(3 * 126e6 / fact_bytes)) + 1
-    # planner-style cardinality hints (DESIGN.md "Table sizing"): expected surviving build rows / groups + 10 %
-    hints = {3: [0.55], 4: [0.22, 0.11]}
-    if cfg in hints:
-        for b, h in zip(plan["builds"], hints[cfg]):
-            b["max_rows"] = int(len(b["table"][0]) * h) + 1024
-        plan["max_groups"] = plan["builds"][-1]["max_rows"]
+    if fact_bytes < 2 * l2:                  # C1: rotate copies so every timed rep reads cold HBM (SURVEY §7.2-1)
+        ncopies = int(np.ceil(3 * l2 / fact_bytes)) + 1
+    sizing = "n/a"
+    if plan.get("builds"):
+        # Table sizing (DESIGN D2). "dense": the planner's column statistics (min/max of every build key) select
+        # direct-address tables. "hinted": expected surviving build rows from the predicates' selectivities (uniform
+        # columns: orderdate < 1200 of 2406 values, segment == 1 of 5 values), + 10 %. "upper bound": max_rows = input rows.
+        sel = {3: [1200 / 2406], 4: [1 / 5, (1200 / 2406) * (1 / 5)]}[cfg]
+        if dense:
+            sizing = "direct-address tables from min/max statistics of the build keys (GQ_F_DENSE_KEYS)"
+            for b in plan["builds"]:
+                k = b["table"][b["key"]]
+                b["dense_range"] = (int(k.min()), int(k.max()))
+        elif hinted:
+            sizing = "hash tables sized from predicate selectivities + 10 %"
+            for b, s in zip(plan["builds"], sel):
+                b["max_rows"] = int(len(b["table"][0]) * s * 1.1) + 1024
+            plan["max_groups"] = plan["builds"][-1]["max_rows"]
+        else:
+            sizing = "hash tables sized for every build input row (no selectivity knowledge)"
     if cfg == 5:
         plan["max_groups"] = int(datagen.ROWS[5]["keys"] * scale)
     build_cols = [gqrun.dev(b["table"]) for b in plan.get("builds", [])]
@@ -175,16 +276,41 @@ def run_config(cfg, gq, ctx, torch, datagen, plans, gqrun, steps, warmup, scale=
     l0 = ctx.launch_count()
     step(); ctx.sync()
     launches_per_step = ctx.launch_count() - l0
-    ms = time_steps(torch, ctx.stream, step, steps, warmup, lambda: None) / steps
+    sampler = ClockSampler(dev["index"] if dev else 0).start() if detail else None
+    ms = time_steps(torch, ctx.stream, step, steps, warmup, lambda: None, MIN_LOAD_MS if detail else 0.0) / steps
+    clocks = sampler.stop() if sampler else None
     ctx.sync()
     alg = ALG_BYTES_PER_ROW[cfg] * nrows + build_bytes
     out = dict(rows=nrows, ms_per_step=ms, rows_per_s=nrows / ms * 1e3, alg_gb=alg / 1e9, gbs=alg / ms / 1e6,
                frac_of_measured=alg / ms / 1e6 / peak, frac_of_8000=alg / ms / 1e6 / 8000.0,
-               launches_per_step=launches_per_step, scale=scale, cold_copies=ncopies, gen_s=round(gen_s, 2))
-    if cfg == 1:   # L2-warm figure, labelled as such
+               launches_per_step=launches_per_step, scale=scale, cold_copies=ncopies, gen_s=round(gen_s, 2), table_sizing=sizing)
+    if detail:
+        out["clocks"] = clocks
+        # one profiled step: every kernel (group) bracketed by CUDA events on the context's stream
+        ctx.profile(True)
+        step()
+        kernels = ctx.profile_read()
+        ctx.profile(False)
+        out["kernels_ms"] = [[n, round(t, 5)] for n, t in kernels]
+        scans = [(t, n) for n, t in kernels if n.startswith("gq_scan") or n == "gq_psa"]
+        dom_ms, dom_name = max(scans) if scans else max((t, n) for n, t in kernels)
+        # algorithmic bytes of the dominant kernel's launch: the fact batch it streams (B/row x rows)
+        dom_alg = ALG_BYTES_PER_ROW[cfg] * nrows
+        tr = (traffic or {}).get(f"C{cfg}") if scale == 1.0 else None
+        out["roofline"] = dict(bound="hbm", kernel=dom_name, kernel_ms=dom_ms, kernel_share_of_step=dom_ms / sum(t for _, t in kernels),
+                               algorithmic_bytes_per_launch=dom_alg, achieved=dom_alg / dom_ms / 1e6, peak=peak, unit="GB/s",
+                               frac=dom_alg / dom_ms / 1e6 / peak, frac_of_nominal_8000=dom_alg / dom_ms / 1e6 / 8000.0,
+                               traffic=tr, how="CUDA events around the launch (gq_profile), one step after the timed loop")
+        res = state["pipes"][(state["i"] - 1) % ncopies].result()
+        out["parity_vs_oracle"] = check_parity(torch, cfg, scale, plan, res, digests or {})
+    if cfg == 1:   # L2-warm figure, labelled as such; and the same kernel on two tiles: launch + set-up + merge tail
         def warm():
             state["pipes"][0].run()
         out["ms_l2_warm"] = time_steps(torch, ctx.stream, warm, steps, warmup, lambda: None) / steps
+        if detail:
+            small = gqrun.prepare(ctx, plan, [], cols=[c[:2048] for c in fact[0]], out_capacity=plan["max_groups"])
+            small.run(); ctx.sync()
+            out["ms_fixed_cost_2048_rows"] = time_steps(torch, ctx.stream, small.run, steps, warmup, lambda: None) / steps
     return out, plan, state
 
 
@@ -215,32 +341,34 @@ def run_standalone_ops(gq, ctx, torch, datagen, plans, gqrun, steps, warmup):
     b = p3["builds"][0]
     bcols = gqrun.dev(b["table"])
     nb = len(b["table"][0])
-    hint = int(nb * 0.55) + 1024
-    tb = ctx.hash_build(bcols, preds=b["preds"], key=0, unique=True, max_rows=hint)
-    ws = tb.workspace
-
-    def build():
-        ctx.hash_build(bcols, preds=b["preds"], key=0, unique=True, max_rows=hint, workspace=ws)
-    ms = time_steps(torch, ctx.stream, build, steps, warmup, lambda: None) / steps
-    out["hash_build_c3_dim"] = dict(rows=nb, ms=ms, rows_per_s=nb / ms * 1e3, gbs=12 * nb / ms / 1e6,
-                                    note="table init + scan + CAS inserts (7.48 M of 15 M rows pass the filter)")
-    tb = ctx.hash_build(bcols, preds=b["preds"], key=0, unique=True, max_rows=hint, workspace=ws)
     fcols = gqrun.dev(p3["table"])
     nf = len(p3["table"][0])
     pexprs = [[("col", 0)], p3["exprs"][0]]
     pcap = nf // 3
     pouts = [torch.empty(pcap, dtype=torch.int64, device="cuda") for _ in pexprs]
+    for label, kw in (("hashed", dict(max_rows=int(nb * 1200 / 2406 * 1.1) + 1024)),
+                      ("dense", dict(dense_range=(int(b["table"][0].min()), int(b["table"][0].max()))))):
+        tb = ctx.hash_build(bcols, preds=b["preds"], key=0, unique=True, **kw)
+        ws = tb.workspace
 
-    def probe():
-        count.zero_()
-        ctx.hash_probe(fcols, p3["preds"], [(tb, 0)], pexprs, capacity=pcap, outs=pouts, count=count)
-    ms = time_steps(torch, ctx.stream, probe, steps, warmup, lambda: None) / steps
-    ctx.sync()
-    out["hash_probe_c3_fact"] = dict(rows=nf, out_rows=int(count.item()), ms=ms, rows_per_s=nf / ms * 1e3,
-                                     gbs=(28 * nf + 16 * int(count.item())) / ms / 1e6)
+        def build():
+            return ctx.hash_build(bcols, preds=b["preds"], key=0, unique=True, workspace=ws, **kw)
+        ms = time_steps(torch, ctx.stream, build, steps, warmup, lambda: None) / steps
+        out[f"hash_build_c3_dim_{label}"] = dict(rows=nb, ms=ms, rows_per_s=nb / ms * 1e3, gbs=12 * nb / ms / 1e6,
+                                                 note="table init + scan + inserts (7.48 M of 15 M rows pass the filter)")
+        tb = build()
+
+        def probe():
+            count.zero_()
+            ctx.hash_probe(fcols, p3["preds"], [(tb, 0)], pexprs, capacity=pcap, outs=pouts, count=count)
+        ms = time_steps(torch, ctx.stream, probe, steps, warmup, lambda: None) / steps
+        ctx.sync()
+        out[f"hash_probe_c3_fact_{label}"] = dict(rows=nf, out_rows=int(count.item()), ms=ms, rows_per_s=nf / ms * 1e3,
+                                                  gbs=(28 * nf + 16 * int(count.item())) / ms / 1e6)
     return out
 
 
+# ---------------------------------------------------------------------------------------------- CPU baselines
 def oracle_rate(plans, datagen, cfg, sample_rows, reps=1):
     """The oracle as it stands, single thread, on a bounded sample of the workload (rows/s)."""
     import oracle
@@ -256,33 +384,63 @@ def oracle_rate(plans, datagen, cfg, sample_rows, reps=1):
     return n / best, n, best
 
 
+def oracle_rate_threads(plans, datagen, nthreads):
+    """The same oracle sharded over the host cores: C2's 60 M rows cut into `nthreads` row ranges, one oracle call per
+    range on its own thread (the C call releases the GIL), the partial (SUM, COUNT) rows added — Partial -> Final of a
+    key-less aggregation. Its result must equal the single-thread oracle's before its time is reported."""
+    import oracle
+    from concurrent.futures import ThreadPoolExecutor
+    plan = plans.PLANS[2](datagen.make_config(2))
+    n = len(plan["table"][0])
+    whole = oracle.run_query(plan)
+    cuts = [n * i // nthreads for i in range(nthreads + 1)]
+    parts = [dict(plan, table=[np.ascontiguousarray(c[a:b]) for c in plan["table"]]) for a, b in zip(cuts, cuts[1:])]
+    best, res = None, None
+    with ThreadPoolExecutor(nthreads) as ex:
+        for _ in range(3):
+            t0 = time.perf_counter()
+            rs = list(ex.map(oracle.run_query, parts))
+            dt = time.perf_counter() - t0
+            if best is None or dt < best:
+                best, res = dt, rs
+    tot = [int(np.sum(np.array([int(r.cols[c][0]) for r in res], dtype=np.int64))) for c in range(len(whole.cols))]
+    equal = all(tot[c] == int(whole.cols[c][0]) for c in range(len(whole.cols)))
+    return n / best, best, equal
+
+
 def main_reference(args):
-    """--impl reference: the CPU oracle (this tier's reference arm) on the box's host cores, rank 0 only."""
+    """--impl reference: the CPU oracle (this tier's reference arm) on the box's host cores, rank 0 only. Same config
+    as the repo's arm (C2, 60 M rows); each step runs the oracle over a bounded sample of those rows sized so that the
+    whole --steps K run ends within a few minutes (all 60 M rows when K is small enough)."""
     ws, rank, _ = dist()
     if rank != 0:
         return
+    import oracle
     import plans
     from paper_2606_24647_b200 import datagen
-    sample = 12_000_000
-    for _ in range(args.warmup):
-        oracle_rate(plans, datagen, 2, 1_000_000)
+    full = datagen.ROWS[2]["fact"]
+    plan = plans.PLANS[2](datagen.make_config(2))
+    calib = dict(plan, table=[np.ascontiguousarray(c[:2_000_000]) for c in plan["table"]])
     t0 = time.perf_counter()
-    rows = 0
+    oracle.run_query(calib)
+    rate0 = 2_000_000 / (time.perf_counter() - t0)
+    sample = int(min(full, max(1_000_000, rate0 * 150.0 / max(1, args.steps + args.warmup))))
+    sub = plan if sample == full else dict(plan, table=[np.ascontiguousarray(c[:sample]) for c in plan["table"]])
+    for _ in range(args.warmup):
+        oracle.run_query(sub)
+    t0 = time.perf_counter()
     for _ in range(args.steps):
-        r, n, dt = oracle_rate(plans, datagen, 2, sample)
-        rows += n
+        oracle.run_query(sub)
     total = time.perf_counter() - t0
-    import oracle  # timed part only
-    # generation is inside oracle_rate but outside its timed region; recompute pure oracle time
-    rate, n, dt = oracle_rate(plans, datagen, 2, sample, reps=max(1, args.steps))
+    rate = sample * args.steps / total
+    what = f"first {sample} of the 60000000 rows of the seeded C2 table per step" if sample < full else "all 60000000 rows per step"
     line = dict(impl="reference", metric=METRIC, value=rate, unit="rows/s", n_gpus=args.gpus, steps=args.steps,
-                warmup=args.warmup, ms_per_step=dt * 1e3, higher_is_better=True, scaling="weak", vs_baseline=None,
-                dtype="int64", data="synthetic",
-                config=dict(workload="C2 selective filter + global SUM(price*discount), 60M-row fact (BASELINE configs[1])",
-                            sample=f"first {n} rows of the seeded C2 table per step"),
-                cpu_baseline=dict(value=rate, unit="rows/s", cores=1, kind="oracle",
-                                  sample=f"{n} rows of C2, best of {max(1, args.steps)}"),
-                e2e=dict(value=rate, unit="rows/s", h2d_bytes_per_step=0, d2h_bytes_per_step=0), gpu_launches=0)
+                warmup=args.warmup, ms_per_step=total / args.steps * 1e3, higher_is_better=True, scaling="weak",
+                vs_baseline=None, dtype="int64", data="synthetic",
+                config=dict(workload=WORKLOAD, rows=full, l2=L2_NOTE),
+                cpu_baseline=dict(value=rate, unit="rows/s", cores=1, kind="oracle", sample=what),
+                e2e=dict(value=rate, unit="rows/s", h2d_bytes_per_step=0, d2h_bytes_per_step=0), gpu_launches=0,
+                host=host_info())
     print(json.dumps(line))
 
 
@@ -297,7 +455,8 @@ def main():
                     "NxS = config N at S times its rows (C1x64: the low-cardinality pipeline at steady state)")
     ap.add_argument("--c5-scale", type=float, default=1.0)
     ap.add_argument("--no-cpu-baseline", action="store_true")
-    ap.add_argument("--no-headline", action="store_true", help="profiling aid: only the --configs entries, printed as JSON")
+    ap.add_argument("--only-configs", action="store_true", help="skip the C2 headline: print only the --configs records "
+                    "(the ncu captures under profiles/ name this command)")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3)
     if args.impl == "reference":
@@ -327,15 +486,40 @@ def main():
     dev_index = lr if ws > 1 else 0
     ctx = gq.Context(dev_index)
     peak, peak_src = peaks()
+    props = torch.cuda.get_device_properties(dev_index)
+    dev = dict(index=dev_index, name=props.name, sms=int(props.multi_processor_count), l2_bytes=int(props.L2_cache_size),
+               mem_bytes=int(props.total_memory))
+    digests, traffic = load_digests(), load_traffic()
+    cfg_steps = max(5, min(20, args.steps))
 
-    if args.no_headline:
+    def extra_configs():
         per_config = {}
         for label, cfg, sc in parse_configs(args.configs, args.c5_scale):
-            out, _, _ = run_config(cfg, gq, ctx, torch, datagen, plans, gqrun, args.steps, args.warmup, scale=sc, peak=peak)
-            per_config[label] = out
+            try:
+                out, _, _ = run_config(cfg, gq, ctx, torch, datagen, plans, gqrun, cfg_steps, 3, scale=sc, peak=peak, detail=True,
+                                       digests=digests, traffic=traffic, dev=dev)
+                per_config[label] = out
+                torch.cuda.empty_cache()
+                if cfg in (3, 4) and sc == 1.0:   # the same pipeline on hash tables: sized from selectivities, and for every input row
+                    alt = {}
+                    for name, kw in (("hashed_hinted", dict(dense=False, hinted=True)), ("hashed_upper_bound", dict(dense=False, hinted=False))):
+                        o2, _, _ = run_config(cfg, gq, ctx, torch, datagen, plans, gqrun, 5, 3, scale=sc, peak=peak, dev=dev, **kw)
+                        alt[name] = dict(ms_per_step=o2["ms_per_step"], table_sizing=o2["table_sizing"], launches_per_step=o2["launches_per_step"])
+                        torch.cuda.empty_cache()
+                    out["other_table_sizings"] = alt
+            except Exception as e:  # a failing extra config must not hide the headline number
+                per_config[label] = dict(error=str(e)[:300])
+            torch.cuda.empty_cache()
         if "ops" in args.configs.split(","):
-            per_config["standalone_ops"] = run_standalone_ops(gq, ctx, torch, datagen, plans, gqrun, args.steps, args.warmup)
-        print(json.dumps(dict(per_config=per_config)))
+            try:
+                per_config["standalone_ops"] = run_standalone_ops(gq, ctx, torch, datagen, plans, gqrun, 10, 3)
+            except Exception as e:
+                per_config["standalone_ops"] = dict(error=str(e)[:300])
+            torch.cuda.empty_cache()
+        return per_config
+
+    if args.only_configs:
+        print(json.dumps(dict(per_config=extra_configs(), device=dev)))
         return
 
     # ---------------- headline: C2, device-resident ----------------
@@ -347,13 +531,9 @@ def main():
     l0 = ctx.launch_count()
     pipe.run(); ctx.sync()
     launches_per_step = ctx.launch_count() - l0
-    import oracle  # parity of the timed configuration against the oracle (full 60 M rows)
-    exp = oracle.run_query(plan) if (rank == 0 and not args.no_cpu_baseline) else None
-    res = pipe.result()
-    parity = None if exp is None else bool(res["n"] == 1 and all(int(a[0]) == int(e[0]) for a, e in zip(res["aggs"], exp.cols)))
-    sampler = ClockSampler(dev_index)
-    sampler.start()
-    total_ms = time_steps(torch, ctx.stream, pipe.run, args.steps, args.warmup, barrier)
+    parity = check_parity(torch, 2, 1.0, plan, pipe.result(), digests) if rank == 0 else None
+    sampler = ClockSampler(dev_index).start()
+    total_ms = time_steps(torch, ctx.stream, pipe.run, args.steps, args.warmup, barrier, MIN_LOAD_MS)
     clocks = sampler.stop()
     # dominant kernel alone: further batches into an existing aggregation state launch only the fused scan kernel
     st = ctx.aggregate(None, cols, preds=plan["preds"], exprs=plan["exprs"], keys=[], aggs=plan["aggs"], max_groups=1)
@@ -365,15 +545,11 @@ def main():
     ms_per_step, value = whole_job_value(total_ms, nrows, args.steps, td if ws > 1 else None, "cuda")
     alg_bytes = ALG_BYTES_PER_ROW[2] * nrows + 16
     achieved = alg_bytes / scan_ms / 1e6
-    traffic = None
-    tpath = os.path.join(ROOT, "profiles", "traffic.json")   # dram bytes per launch from the committed ncu capture
-    if os.path.exists(tpath):
-        with open(tpath) as f:
-            traffic = json.load(f).get("c2_scan_dram_bytes_per_launch")
-    roofline = dict(bound="hbm", kernel="gq_scan (C2 fused filter+project+global aggregate)", achieved=achieved,
-                    peak=peak, unit="GB/s", frac=achieved / peak, traffic=traffic, peak_source=peak_src,
+    roofline = dict(bound="hbm", kernel="gq_scan:global (C2 fused filter+project+global aggregate; the step's only launch)",
+                    achieved=achieved, peak=peak, unit="GB/s", frac=achieved / peak, traffic=traffic.get("C2"), peak_source=peak_src,
                     algorithmic_bytes_per_launch=alg_bytes, kernel_ms=scan_ms, frac_of_nominal_8000=achieved / 8000.0,
-                    read_probe_gbs=(1 << 30) / probe_ms / 1e6)
+                    read_probe_gbs=(1 << 30) / probe_ms / 1e6,
+                    traffic_source="dram__bytes_read.sum + dram__bytes_write.sum of this kernel, committed ncu capture (profiles/traffic.json)")
 
     # ---------------- end to end: HOST buffers through the C ABI ----------------
     e2e = None
@@ -386,9 +562,8 @@ def main():
         for _ in range(k):
             hp.run_host()
         e2e_ms = (time.perf_counter() - t0) / k * 1e3     # run_host returns after the results landed on the host
-        r = hp.result()
-        if exp is not None:
-            parity = parity and all(int(a[0]) == int(e[0]) for a, e in zip(r["aggs"], exp.cols))
+        if parity is not None and parity["ok"]:
+            parity["ok"] = bool(result_rows(torch, hp.result()) == result_rows(torch, pipe.result()))   # e2e path: same row
         e2e = dict(value=ws * nrows / e2e_ms * 1e3, unit="rows/s", h2d_bytes_per_step=int(sum(c.nbytes for c in plan["table"])),
                    d2h_bytes_per_step=8 * (1 + len(plan["aggs"])), ms_per_step=e2e_ms,
                    how="gq_pipeline_host: pinned host columns, 8 Mi-row chunks, H2D overlapped with the scan")
@@ -399,36 +574,52 @@ def main():
     if ws == 1 and args.configs:
         del cols, pipe, st, probe_t
         torch.cuda.empty_cache()
-        for label, cfg, sc in parse_configs(args.configs, args.c5_scale):
+        per_config = extra_configs()
+        # end to end for a join pipeline too: C3 with its build side device-resident, the 60 M-row fact table on the host
+        if "C3" in per_config:
             try:
-                out, _, _ = run_config(cfg, gq, ctx, torch, datagen, plans, gqrun, max(5, min(20, args.steps)), 3, scale=sc, peak=peak)
-                per_config[label] = out
-            except Exception as e:  # a failing extra config must not hide the headline number
-                per_config[label] = dict(error=str(e)[:300])
-            torch.cuda.empty_cache()
-
-        if "ops" in args.configs.split(","):
-            try:
-                per_config["standalone_ops"] = run_standalone_ops(gq, ctx, torch, datagen, plans, gqrun, 10, 3)
+                t3 = datagen.make_config(3)
+                p3 = plans.plan_c3(t3, topk=10)
+                for b in p3["builds"]:
+                    kk = b["table"][b["key"]]
+                    b["dense_range"] = (int(kk.min()), int(kk.max()))
+                tables = gqrun.build_tables(ctx, p3)
+                h3 = [torch.from_numpy(np.ascontiguousarray(c)).pin_memory() for c in p3["table"]]
+                hp3 = gqrun.prepare(ctx, p3, tables, cols=h3, out_capacity=10)
+                hp3.run_host(); hp3.run_host()
+                t0 = time.perf_counter()
+                for _ in range(3):
+                    hp3.run_host()
+                ms3 = (time.perf_counter() - t0) / 3 * 1e3
+                per_config["C3"]["e2e"] = dict(
+                    value=len(p3["table"][0]) / ms3 * 1e3, unit="rows/s", ms_per_step=ms3,
+                    h2d_bytes_per_step=int(sum(c.nbytes for c in p3["table"])), d2h_bytes_per_step=8 + 10 * 8 * 3,
+                    parity_vs_oracle=bool(result_rows(torch, hp3.result()) == digests["C3"]["top10"]),
+                    how="gq_pipeline_host: fact columns in pinned host memory, build-side table device-resident")
+                del h3, hp3, tables
+                torch.cuda.empty_cache()
             except Exception as e:
-                per_config["standalone_ops"] = dict(error=str(e)[:300])
-            torch.cuda.empty_cache()
+                per_config["C3"]["e2e"] = dict(error=str(e)[:300])
 
-    # ---------------- CPU baseline: the oracle on this box's host cores ----------------
-    cpu = None
+    # ---------------- CPU baselines: the oracle on this box's host cores ----------------
+    cpu, cpu_threads, host = None, None, host_info()
     if rank == 0 and not args.no_cpu_baseline:
         rate, n, dt = oracle_rate(plans, datagen, 2, 60_000_000, reps=3)
         cpu = dict(value=rate, unit="rows/s", cores=1, kind="oracle", sample=f"all {n} rows of C2, best of 3 ({dt:.2f} s each)",
                    host_cores=os.cpu_count())
+        nt = os.cpu_count() or 1
+        trate, tdt, equal = oracle_rate_threads(plans, datagen, nt)
+        cpu_threads = dict(value=trate if equal else None, unit="rows/s", cores=nt,
+                           kind="oracle sharded over row ranges, one thread each; partial rows added",
+                           sample=f"all {n} rows of C2, best of 3 ({tdt:.2f} s each)", equals_single_thread_oracle=bool(equal))
     if rank == 0:
         line = dict(metric=METRIC, value=value, unit="rows/s", n_gpus=ws, steps=args.steps, warmup=args.warmup,
                     ms_per_step=ms_per_step, higher_is_better=True, scaling="weak", vs_baseline=None, dtype="int64",
-                    data="synthetic",
-                    config=dict(workload="C2 selective filter + global SUM(price*discount), 60M-row fact (BASELINE configs[1])",
-                                rows=nrows, l2="inputs (1.68 GB) larger than L2 (126 MB): every iteration reads HBM",
-                                parallelism="replicas only" if ws > 1 else "1 GPU", parity_vs_oracle=parity),
-                    roofline=roofline, cpu_baseline=cpu, e2e=e2e, gpu_launches=launches_per_step * args.steps,
-                    launches_per_step=launches_per_step, clocks=clocks, per_config=per_config)
+                    data="synthetic", config=dict(workload=WORKLOAD, rows=nrows, l2=L2_NOTE),
+                    parallelism="replicas only" if ws > 1 else "1 GPU", parity_vs_oracle=parity,
+                    roofline=roofline, cpu_baseline=cpu, cpu_baseline_threads=cpu_threads, host=host, device=dev, e2e=e2e,
+                    gpu_launches=launches_per_step * args.steps, launches_per_step=launches_per_step, clocks=clocks,
+                    per_config=per_config)
         print(json.dumps(line))
     if ws > 1:
         td.destroy_process_group()

@@ -22,7 +22,8 @@
  *                are read during the call only.
  *   Ownership  : the caller owns all columns, outputs and workspaces and must keep them alive until the enqueued work
  *                has completed on the context's stream. The library owns only small host handles and the context's
- *                few hundred bytes of device scratch. No call allocates or frees device memory after gq_create.
+ *                few KB of device scratch (sticky error, ticket and merge table of the fused finalisers). No call
+ *                allocates or frees device memory after gq_create.
  *   Alignment  : column and output pointers 16-byte aligned; workspaces 256-byte aligned.
  *   Types      : signed int8 / int32 / int64 columns, no NULLs, no strings, no floating point input.
  *                All arithmetic is wrapping two's-complement int64; aggregates and COUNT are int64.
@@ -50,7 +51,8 @@ typedef enum {
   GQ_ERR_CUDA = 5,                 /* CUDA runtime error: see gq_last_cuda_error */
   GQ_ERR_DUPLICATE_KEY = 6,        /* GQ_F_UNIQUE_KEYS asserted but a duplicate build key was seen (sticky) */
   GQ_ERR_COMPILE = 7,              /* plan-time kernel compilation failed: see gq_last_message */
-  GQ_ERR_DEPENDENT_KEY = 8         /* GQ_F_CHECK_DEPENDENT: a key declared dependent took two values in one group (sticky) */
+  GQ_ERR_DEPENDENT_KEY = 8,        /* GQ_F_CHECK_DEPENDENT: a key declared dependent took two values in one group (sticky) */
+  GQ_ERR_KEY_RANGE = 9             /* GQ_F_DENSE_KEYS: a build key outside [key_min, key_max] was seen (sticky) */
 } gq_status;
 
 typedef enum { GQ_I8 = 1, GQ_I32 = 2, GQ_I64 = 3 } gq_dtype;
@@ -73,9 +75,17 @@ typedef struct { gq_aggop op; int32_t expr; /* index into exprs[]; ignored for C
 
 enum {
   GQ_F_UNIQUE_KEYS = 1u << 0,      /* gq_build_desc: caller asserts unique build keys; VERIFIED on device, never trusted */
-  GQ_F_CHECK_DEPENDENT = 1u << 1   /* gq_agg_desc: debug check of `ndependent`: every row compares its
+  GQ_F_CHECK_DEPENDENT = 1u << 1,  /* gq_agg_desc: debug check of `ndependent`: every row compares its
                                       dependent key with the one stored for its group; a mismatch sets the sticky
                                       GQ_ERR_DEPENDENT_KEY instead of silently merging two groups */
+  GQ_F_DENSE_KEYS = 1u << 2        /* gq_build_desc: the planner knows (column min/max statistics) that every build key
+                                      lies in [key_min, key_max] and the range is not much larger than the row count:
+                                      the table becomes a DIRECT-ADDRESS table — a membership bitmap plus a payload
+                                      array indexed by key - key_min; no hashing, no probing, a probe that misses costs
+                                      one bit test in an L2-resident bitmap ("the query planner should choose the
+                                      operator implementation based on ... the expected input"). Requires
+                                      GQ_F_UNIQUE_KEYS. VERIFIED on device: a key outside the range sets the sticky
+                                      GQ_ERR_KEY_RANGE, a repeated key GQ_ERR_DUPLICATE_KEY */
 };
 enum { GQ_MAX_PREDS = 16, GQ_MAX_TOKS = 32, GQ_MAX_EXPRS = 8, GQ_MAX_AGGS = 8, GQ_MAX_PROBES = 4, GQ_MAX_PAYLOAD = 3,
        GQ_MAX_KEYS = 2, GQ_MAX_COLS = 32, GQ_MAX_TOPK = 32, GQ_SIDE_SLOTS = 64 };
@@ -112,12 +122,16 @@ typedef struct {
   const gq_probe_step* probes; int32_t nprobes;  /* chained joins: rows must match these tables before insertion */
   int32_t key_col;                               /* int64-widened key column (may be a payload of a probe step) */
   const int32_t* payload_cols; int32_t npayload; /* stored beside the key, handed to probers */
-  uint32_t flags;                                /* GQ_F_UNIQUE_KEYS */
+  uint32_t flags;                                /* GQ_F_UNIQUE_KEYS, GQ_F_DENSE_KEYS */
+  int64_t key_min, key_max;                      /* GQ_F_DENSE_KEYS: inclusive key range (ignored otherwise) */
 } gq_build_desc;
 /* Open addressing, linear probing, 64-bit CAS; capacity = max_build_rows / load slots rounded up to a multiple of
  * 1024 (not to a power of two: slot = multiply-shift range reduction of the hash), load = 0.4 for tables that fit L2 and
  * 0.7 for larger ones; read in 32-byte (key-only) or 64-byte (key + payload) buckets. */
 gq_status gq_hash_build_workspace(int64_t max_build_rows, int32_t npayload, size_t* bytes);
+/* Workspace of a GQ_F_DENSE_KEYS table: header + bitmap of (key_max - key_min + 1) bits + that many payload rows.
+ * gq_hash_build ignores max_build_rows for such a table. */
+gq_status gq_hash_build_workspace_dense(int64_t key_min, int64_t key_max, int32_t npayload, size_t* bytes);
 /* *table == NULL: creates the table in d_workspace (enqueues its initialisation) and inserts the batch.
  * *table != NULL: inserts a further batch (same schema and desc; d_workspace/bytes/max_build_rows ignored). */
 gq_status gq_hash_build(gq_ctx*, gq_table** table, void* d_workspace, size_t bytes, int64_t max_build_rows,
@@ -210,18 +224,30 @@ gq_status gq_precompile_build(const gq_batch* in, const gq_build_desc*, char* h_
 gq_status gq_precompile_materialise(const gq_batch* in, const gq_pred* preds, int32_t npred, const gq_probe_step* probes,
                                     int32_t nprobes, const gq_expr* exprs, int32_t nexpr, char* h_msg, size_t msg_bytes);
 /* Host-only table handle carrying just the schema (payload dtypes, flags) for precompilation. */
-gq_status gq_table_describe(gq_table** out, const gq_dtype* payload_dtypes, int32_t npayload, uint32_t flags);
+gq_status gq_table_describe(gq_table** out, const gq_dtype* payload_dtypes, int32_t npayload, uint32_t flags);   /* flags: GQ_F_UNIQUE_KEYS, GQ_F_DENSE_KEYS */
 
 /* ---- measurement helper ---------------------------------------------------------------------------------------- */
 /* Read-only streaming sum over `bytes` bytes (16-byte aligned, multiple of 16): the practical read roofline probe of
  * SURVEY §7.1 step 5. *d_out (DEVICE uint64) receives the wrapping sum of the 64-bit words. */
 gq_status gq_read_probe(gq_ctx*, const void* d_data, size_t bytes, uint64_t* d_out);
 
+/* ---- per-kernel timing (the operator-level breakdown the paper reports, Fig. 5/6) ----------------------- */
+/* enable != 0: from now on every kernel (or small kernel group) this context launches is bracketed by a pair of CUDA
+ * events on its stream (a few microseconds each; leave it off inside timed loops and CUDA-graph capture). */
+gq_status gq_profile(gq_ctx*, int32_t enable);
+/* Blocks until the stream is idle, then returns the number of entries recorded since the last read (<= max_entries):
+ * h_ms[i] = device milliseconds of entry i, h_names = their names separated by '\n' (HOST buffers). -1 on error. */
+int32_t gq_profile_read(gq_ctx*, char* h_names, size_t names_bytes, float* h_ms, int32_t max_entries);
+
 /* ---- planner knobs --------------------------------------------------------------------------------------------- */
 /* Process-wide thresholds a planner may override ("the query planner should choose the operator
  * implementation based on both the expected input and the available resources"). Names:
  *   "part_min_table_mb"  group-by tables at least this large take the radix-partitioned path (default 256)
  *   "part_min_rows"      ... when the first batch has at least this many rows (default 16 Mi)
+ *   "hot_min_rows"       batches at least this large are sampled for heavy hitters (default 4 Mi)
+ *   "psa_max_log2_partitions"  cap on the pass-A partitions of the partitioned shared-memory aggregation (default 14);
+ *                        key ranges beyond it are resolved by sub-passes of pass B
+ *   "psa_threads"        512 / 1024 threads per CTA in pass B (default 1024), 0 = default
  * Unknown names return GQ_ERR_INVALID_ARG. A negative value restores the default. */
 gq_status gq_set_option(const char* h_name, int64_t value);
 

@@ -61,6 +61,20 @@ WsLayout ws_layout(int64_t capacity, int slot_words, int nside) {
 // several GPUs; cudaSetDevice is a no-op when nothing changes).
 inline void use_device(gq_ctx* ctx) { if (ctx) cudaSetDevice(ctx->device); }
 
+// gq_profile: brackets the kernel launches enqueued while it is alive with a pair of events on the context's stream.
+struct ProfScope {
+  gq_ctx* c; int i = -1;
+  ProfScope(gq_ctx* ctx, const char* name) : c(ctx) {
+    if (!c || !c->prof) return;
+    i = (int)c->prof_names.size();
+    while ((int)c->prof_ev.size() < 2 * (i + 1)) { cudaEvent_t e; if (cudaEventCreate(&e) != cudaSuccess) { i = -1; return; } c->prof_ev.push_back(e); }
+    c->prof_names.push_back(name);
+    cudaEventRecord(c->prof_ev[2 * i], c->stream);
+  }
+  ~ProfScope() { if (i >= 0) cudaEventRecord(c->prof_ev[2 * i + 1], c->stream); }
+};
+#define PROF(ctx, name, call) (ProfScope(ctx, name), (call))
+
 gq_status check_batch(gq_ctx* ctx, const gq_batch* b) {
   use_device(ctx);
   if (!b || b->ncols < 0 || b->ncols > GQ_MAX_COLS || b->nrows < 0 || (b->ncols > 0 && !b->cols))
@@ -107,6 +121,7 @@ gq_status fill_common(gq_ctx* ctx, GqScanSpec* sp, const gq_batch* in, const gq_
     ps.npayload = t->npayload;
     for (int p = 0; p < GQ_MAX_PAYLOAD; ++p) ps.pay_dtype[p] = t->payload_dtype[p];
     ps.unique = (t->flags & GQ_F_UNIQUE_KEYS) != 0;
+    ps.dense = (t->flags & GQ_F_DENSE_KEYS) != 0;
     ps.slot_words = join_slot_words(t->npayload);
     if (ps.key_col < 0 || ps.key_col >= row_width(*sp)) return fail(ctx, GQ_ERR_INVALID_ARG, "probe key column out of range");
     sp->probes.push_back(ps);
@@ -147,7 +162,7 @@ std::string signature(const GqScanSpec& sp) {
   s += 'p';
   for (const gq_pred& p : sp.preds) { put(p.col); put(p.op); }
   s += 'j';
-  for (const GqProbeSpec& p : sp.probes) { put(p.key_col); put(p.npayload); put(p.unique); for (int i = 0; i < p.npayload; ++i) put(p.pay_dtype[i]); }
+  for (const GqProbeSpec& p : sp.probes) { put(p.key_col); put(p.npayload); put(p.unique); put(p.dense); for (int i = 0; i < p.npayload; ++i) put(p.pay_dtype[i]); }
   s += 'e';
   for (const auto& e : sp.exprs) { for (const gq_xtok& t : e) { put(t.op); if (t.op == GQ_X_COL) put(t.arg); } s += ';'; }
   s += 'k';
@@ -156,7 +171,7 @@ std::string signature(const GqScanSpec& sp) {
   for (const gq_agg& a : sp.aggs) { put(a.op); put(a.expr); }
   put(sp.lc_cap); put(sp.lc_key_bits); put(sp.target_sw); put(sp.build_key_col);
   for (int c : sp.payload_cols) put(c);
-  put(sp.unique); put(sp.hot); put(sp.check_dep); put(sp.fused_final); put(sp.direct_step); put(sp.direct_aw); put(sp.direct_touch);
+  put(sp.unique); put(sp.dense_target); put(sp.hot); put(sp.check_dep); put(sp.fused_final); put(sp.direct_step); put(sp.direct_aw); put(sp.direct_touch);
   put(sp.part_rw); put(sp.part_states); for (int e : sp.part_exprs) put(e);
   s += 'c';
   std::vector<long long> kv; std::vector<int> ki;
@@ -253,6 +268,9 @@ gq_status run_scan(gq_ctx* ctx, const GqScanSpec& sp, const gq_batch* in, const 
   const int64_t ntiles = in->nrows / kern.tile_rows;
   int grid = (int)std::max<int64_t>(1, std::min<int64_t>(ctx->num_sms, ntiles));
   void* args[] = {(void*)P};
+  static const char* const kname[] = {"gq_scan:global", "gq_scan:lowcard", "gq_scan:highcard", "gq_scan:build", "gq_scan:materialise",
+                                      "gq_scan:direct", "gq_scan:partition", "gq_scan:scatter"};
+  ProfScope ps(ctx, kname[sp.consumer]);
   cudaError_t e = cudaLaunchKernel((const void*)kern.fn, dim3((unsigned)grid), dim3((unsigned)kern.threads), args,
                                    (size_t)kern.smem_bytes, ctx->stream);
   if (e != cudaSuccess) return cuda_fail(ctx, e, "launch of fused scan kernel");
@@ -275,8 +293,8 @@ gq_status gq_create(gq_ctx** out, int device, void* cuda_stream) {
   c->stream = (cudaStream_t)cuda_stream;
   int sms = 0;
   if (cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, device) == cudaSuccess && sms > 0) c->num_sms = sms;
-  e = cudaMalloc((void**)&c->d_err, 256);
-  if (e == cudaSuccess) e = cudaMemset(c->d_err, 0, 256);
+  e = cudaMalloc((void**)&c->d_err, 256 + GQ_GTAB_BYTES);
+  if (e == cudaSuccess) e = cudaMemset(c->d_err, 0, 256 + GQ_GTAB_BYTES);
   if (e == cudaSuccess) e = cudaMallocHost((void**)&c->h_err, 256);
   if (e != cudaSuccess) { if (c->d_err) cudaFree(c->d_err); delete c; return GQ_ERR_CUDA; }
   *c->h_err = 0;
@@ -288,6 +306,7 @@ gq_status gq_destroy(gq_ctx* c) {
   if (!c) return GQ_ERR_INVALID_ARG;
   cudaFree(c->d_err);
   cudaFreeHost(c->h_err);
+  for (cudaEvent_t e : c->prof_ev) cudaEventDestroy(e);
   if (c->copy_stream) cudaStreamDestroy(c->copy_stream);
   if (c->ev_start) cudaEventDestroy(c->ev_start);
   for (int i = 0; i < 2; ++i) { if (c->ev_copied[i]) cudaEventDestroy(c->ev_copied[i]); if (c->ev_consumed[i]) cudaEventDestroy(c->ev_consumed[i]); }
@@ -305,14 +324,16 @@ gq_status gq_sync(gq_ctx* c) {
   if (code == 0) return GQ_OK;
   c->msg = code == GQ_ERR_CAPACITY ? "device: hash table or output capacity exceeded"
          : code == GQ_ERR_DUPLICATE_KEY ? "device: duplicate build key under GQ_F_UNIQUE_KEYS"
-         : code == GQ_ERR_DEPENDENT_KEY ? "device: a key declared dependent (ndependent) took two values within one group" : "device error";
+         : code == GQ_ERR_DEPENDENT_KEY ? "device: a key declared dependent (ndependent) took two values within one group"
+         : code == GQ_ERR_KEY_RANGE ? "device: a build key outside the declared range of a GQ_F_DENSE_KEYS table" : "device error";
   return (gq_status)code;
 }
 
 gq_status gq_clear_error(gq_ctx* c) {
   if (!c) return GQ_ERR_INVALID_ARG;
   use_device(c);
-  cudaError_t e = cudaMemsetAsync(c->d_err, 0, sizeof(int), c->stream);
+  // (also the ticket and the merge table of the fused finaliser: a kernel that stopped on the error may have left them set)
+  cudaError_t e = cudaMemsetAsync(c->d_err, 0, 256 + GQ_GTAB_BYTES, c->stream);
   return e == cudaSuccess ? GQ_OK : cuda_fail(c, e, "gq_clear_error");
 }
 
@@ -327,6 +348,7 @@ const char* gq_status_str(gq_status s) {
     case GQ_ERR_DUPLICATE_KEY: return "GQ_ERR_DUPLICATE_KEY";
     case GQ_ERR_COMPILE: return "GQ_ERR_COMPILE";
     case GQ_ERR_DEPENDENT_KEY: return "GQ_ERR_DEPENDENT_KEY";
+    case GQ_ERR_KEY_RANGE: return "GQ_ERR_KEY_RANGE";
   }
   return "GQ_ERR_UNKNOWN";
 }
@@ -376,6 +398,25 @@ gq_status gq_hash_build_workspace(int64_t max_build_rows, int32_t npayload, size
   return GQ_OK;
 }
 
+// Direct-address table (GQ_F_DENSE_KEYS): [header 256 B][bitmap, one bit per key of the range][payload rows]
+struct DenseLayout { int64_t range; size_t bitmap_off, bitmap_bytes, pay_off, total; };
+static bool dense_layout(int64_t key_min, int64_t key_max, int npayload, DenseLayout* L) {
+  if (key_max < key_min || (uint64_t)key_max - (uint64_t)key_min >= (1ULL << 36)) return false;
+  L->range = (int64_t)((uint64_t)key_max - (uint64_t)key_min + 1);
+  L->bitmap_off = 256;
+  L->bitmap_bytes = align_up((size_t)((L->range + 31) / 32) * 4, 256);
+  L->pay_off = L->bitmap_off + L->bitmap_bytes;
+  L->total = L->pay_off + align_up((size_t)L->range * (size_t)npayload * 8, 256);
+  return true;
+}
+
+gq_status gq_hash_build_workspace_dense(int64_t key_min, int64_t key_max, int32_t npayload, size_t* bytes) {
+  DenseLayout L;
+  if (!bytes || npayload < 0 || npayload > GQ_MAX_PAYLOAD || !dense_layout(key_min, key_max, npayload, &L)) return GQ_ERR_INVALID_ARG;
+  *bytes = L.total;
+  return GQ_OK;
+}
+
 static gq_status build_spec(gq_ctx* ctx, GqScanSpec* sp, const gq_batch* in, const gq_build_desc* d) {
   gq_status st = fill_common(ctx, sp, in, d->preds, d->npred, d->probes, d->nprobes, nullptr, 0);
   if (st != GQ_OK) return st;
@@ -388,6 +429,9 @@ static gq_status build_spec(gq_ctx* ctx, GqScanSpec* sp, const gq_batch* in, con
   sp->payload_cols.assign(d->payload_cols, d->payload_cols + d->npayload);
   for (int c : sp->payload_cols) if (c < 0 || c >= w) return fail(ctx, GQ_ERR_INVALID_ARG, "payload column out of range");
   sp->unique = (d->flags & GQ_F_UNIQUE_KEYS) != 0;
+  if (d->flags & ~(uint32_t)(GQ_F_UNIQUE_KEYS | GQ_F_DENSE_KEYS)) return fail(ctx, GQ_ERR_INVALID_ARG, "unknown gq_build_desc flags");
+  sp->dense_target = (d->flags & GQ_F_DENSE_KEYS) != 0;
+  if (sp->dense_target && !sp->unique) return fail(ctx, GQ_ERR_INVALID_ARG, "GQ_F_DENSE_KEYS requires GQ_F_UNIQUE_KEYS");
   sp->target_sw = join_slot_words(d->npayload);
   return GQ_OK;
 }
@@ -401,7 +445,27 @@ gq_status gq_hash_build(gq_ctx* ctx, gq_table** table, void* d_ws, size_t bytes,
   st = build_spec(ctx, &sp, in, d);
   if (st != GQ_OK) return st;
   gq_table* t = *table;
-  if (!t) {
+  if (!t && sp.dense_target) {
+    DenseLayout L;
+    if (!d_ws || !aligned(d_ws, 256)) return fail(ctx, GQ_ERR_INVALID_ARG, "bad workspace");
+    if (!dense_layout(d->key_min, d->key_max, d->npayload, &L)) return fail(ctx, GQ_ERR_INVALID_ARG, "bad dense key range");
+    if (bytes < L.total) return fail(ctx, GQ_ERR_WORKSPACE_TOO_SMALL, "hash-build workspace too small");
+    t = new gq_table();
+    t->capacity = L.range; t->dense = true; t->key_min = d->key_min;
+    t->npayload = d->npayload;
+    for (int p = 0; p < d->npayload; ++p) t->payload_dtype[p] = row_dtype(sp, d->payload_cols[p]);
+    t->flags = d->flags;
+    t->max_rows = L.range;
+    t->dev.slots = (unsigned long long*)((char*)d_ws + L.pay_off);
+    t->dev.mask = (unsigned long long)(L.range - 1);
+    t->dev.header = (long long*)d_ws;
+    t->dev.side = (unsigned long long*)((char*)d_ws + L.bitmap_off);
+    t->dev.slot_words = d->npayload; t->dev.flags = d->flags; t->dev.base = d->key_min;
+    cudaError_t e = cudaMemsetAsync(d_ws, 0, L.bitmap_off + L.bitmap_bytes, ctx->stream);   // header + bitmap; payload rows need no init
+    if (e != cudaSuccess) { delete t; return cuda_fail(ctx, e, "dense table init"); }
+    { GqScanSpec c = sp; c.nrows_hint = 0; t->build_sig = signature(c) + "|" + std::to_string(d->key_min) + ":" + std::to_string(d->key_max); }
+    *table = t;
+  } else if (!t) {
     if (!d_ws || !aligned(d_ws, 256) || max_build_rows < 0) return fail(ctx, GQ_ERR_INVALID_ARG, "bad workspace");
     const int sw = sp.target_sw;
     const int64_t cap = join_capacity(max_build_rows, sw);
@@ -424,14 +488,16 @@ gq_status gq_hash_build(gq_ctx* ctx, gq_table** table, void* d_ws, size_t bytes,
     unsigned long long pat[16];
     for (int i = 0; i < 16; ++i) pat[i] = 0;
     pat[0] = GQ_EMPTY_KEY;
-    cudaError_t e = gq_launch_init_table(ctx->stream, t->dev.slots, cap, sw, pat, t->dev.side, GQ_SIDE_SLOTS, t->dev.header, 0, ctx->num_sms);
+    cudaError_t e = PROF(ctx, "gq_k_init_table", gq_launch_init_table(ctx->stream, t->dev.slots, cap, sw, pat, t->dev.side, GQ_SIDE_SLOTS, t->dev.header, 0, ctx->num_sms));
     if (e != cudaSuccess) { delete t; return cuda_fail(ctx, e, "table init"); }
     ++ctx->launches;
     { GqScanSpec c = sp; c.nrows_hint = 0; t->build_sig = signature(c); }
     *table = t;
   } else {
     GqScanSpec c = sp; c.nrows_hint = 0;
-    if (t->describe_only || signature(c) != t->build_sig) return fail(ctx, GQ_ERR_INVALID_ARG, "batch schema/desc differs from the table's first batch");
+    std::string sg = signature(c);
+    if (t->dense) sg += "|" + std::to_string(d->key_min) + ":" + std::to_string(d->key_max);
+    if (t->describe_only || sg != t->build_sig) return fail(ctx, GQ_ERR_INVALID_ARG, "batch schema/desc differs from the table's first batch");
     if (t->finished) return fail(ctx, GQ_ERR_INVALID_ARG, "table already finished");
   }
   GqParams P;
@@ -474,7 +540,9 @@ gq_status gq_table_describe(gq_table** out, const gq_dtype* payload_dtypes, int3
   t->describe_only = true;
   t->npayload = npayload;
   for (int p = 0; p < npayload; ++p) { if (!dtype_ok(payload_dtypes[p])) { delete t; return GQ_ERR_INVALID_ARG; } t->payload_dtype[p] = payload_dtypes[p]; }
+  if ((flags & GQ_F_DENSE_KEYS) && !(flags & GQ_F_UNIQUE_KEYS)) { delete t; return GQ_ERR_INVALID_ARG; }
   t->flags = flags;
+  t->dense = (flags & GQ_F_DENSE_KEYS) != 0;
   *out = t;
   return GQ_OK;
 }
@@ -741,12 +809,13 @@ gq_status gq_hash_aggregate(gq_ctx* ctx, gq_aggstate** state, void* d_ws, size_t
     cudaError_t e;
     if (dp.step >= 0) {
       a->direct = true; a->dtab = d->probes[dp.step].table->dev; a->dcap = dp.cap; a->daw = dp.aw; a->dtouch = dp.touch;
+      a->ddense = d->probes[dp.step].table->dense; a->dnpay = d->probes[dp.step].table->npayload;
       a->dep_pay = dp.dep_pay;
       a->dev.header = (long long*)d_ws;
       a->dacc = (unsigned long long*)((char*)d_ws + 256);
       for (int i = 0; i < d->naggs; ++i)
         pat[i] = d->aggs[i].op == GQ_MIN ? 0x7FFFFFFFFFFFFFFFULL : d->aggs[i].op == GQ_MAX ? 0x8000000000000000ULL : 0ULL;
-      e = gq_launch_init_table(ctx->stream, a->dacc, dp.cap + 1, dp.aw, pat, a->dacc, 0, a->dev.header, 0, ctx->num_sms);
+      e = PROF(ctx, "gq_k_init_table", gq_launch_init_table(ctx->stream, a->dacc, dp.cap + 1, dp.aw, pat, a->dacc, 0, a->dev.header, 0, ctx->num_sms));
     } else {
       const int64_t cap = agg_capacity(d->max_groups, d->nkeys);
       const int sw = sp.target_sw;
@@ -783,7 +852,7 @@ gq_status gq_hash_aggregate(gq_ctx* ctx, gq_aggstate** state, void* d_ws, size_t
       for (int i = 0; i < d->naggs; ++i)
         pat[1 + d->ndependent + i] = d->aggs[i].op == GQ_MIN ? 0x7FFFFFFFFFFFFFFFULL : d->aggs[i].op == GQ_MAX ? 0x8000000000000000ULL : 0ULL;
       // a key-less aggregation has exactly one group, present even with no input rows (S9): header[1] = 1
-      e = gq_launch_init_table(ctx->stream, a->dev.slots, cap, sw, pat, a->dev.side, 1, a->dev.header, d->nkeys == 0 ? 1 : 0, ctx->num_sms);
+      e = PROF(ctx, "gq_k_init_table", gq_launch_init_table(ctx->stream, a->dev.slots, cap, sw, pat, a->dev.side, 1, a->dev.header, d->nkeys == 0 ? 1 : 0, ctx->num_sms));
     }
     if (e != cudaSuccess) { delete a; return cuda_fail(ctx, e, "aggregate state init"); }
     ++ctx->launches;
@@ -810,8 +879,8 @@ gq_status gq_hash_aggregate(gq_ctx* ctx, gq_aggstate** state, void* d_ws, size_t
   if (sp.hot && a->hot && in->nrows >= g_hot_min_rows.load()) {   // heavy-hitter pass over a strided sample of the key column
     int nl = 0;
     const gq_column& kc = in->cols[sp.key_cols[0]];
-    cudaError_t e = gq_launch_hot_keys(ctx->stream, kc.data, (int)kc.dtype, in->nrows, a->hot_table, GQ_HOT_SLOTS, GQ_HOT_SAMPLE,
-                                       GQ_HOT_THRESHOLD, a->hot, GQ_HOT_MAX, ctx->num_sms, &nl);
+    cudaError_t e = PROF(ctx, "gq_k_hot_keys(4)", gq_launch_hot_keys(ctx->stream, kc.data, (int)kc.dtype, in->nrows, a->hot_table, GQ_HOT_SLOTS, GQ_HOT_SAMPLE,
+                                       GQ_HOT_THRESHOLD, a->hot, GQ_HOT_MAX, ctx->num_sms, &nl));
     if (e != cudaSuccess) return cuda_fail(ctx, e, "heavy-hitter sampling");
     ctx->launches += nl;
     P.hot = a->hot;
@@ -833,7 +902,7 @@ gq_status gq_hash_aggregate(gq_ctx* ctx, gq_aggstate** state, void* d_ws, size_t
     for (int i = 0; i < a->naggs; ++i) { pb.op[i] = (int)a->agg_op[i]; pb.src[i] = pp.src[i]; }
     pb.check_dep = a->check_dep ? 1 : 0;
     pb.err = ctx->d_err;
-    e = gq_launch_part_upsert(ctx->stream, pb, ctx->num_sms);
+    e = PROF(ctx, "gq_k_part_upsert", gq_launch_part_upsert(ctx->stream, pb, ctx->num_sms));
     if (e != cudaSuccess) return cuda_fail(ctx, e, "partitioned upsert");
     ++ctx->launches;
     return GQ_OK;
@@ -859,6 +928,7 @@ gq_status gq_hash_aggregate_finish(gq_ctx* ctx, gq_aggstate* a, void* const* out
   if (a->direct) {
     p.direct = 1; p.capacity = a->dcap; p.dacc = a->dacc; p.daw = a->daw; p.dtouch = a->dtouch; p.dep_pay = a->dep_pay;
     p.jslots = a->dtab.slots; p.jside = a->dtab.side; p.jsw = a->dtab.slot_words;
+    p.jdense = a->ddense ? 1 : 0; p.jbase = a->dtab.base; p.jnpay = a->dnpay;
   }
   p.nkeys = a->nkeys; p.ndep = a->ndep; p.naggs = a->naggs;
   for (int k = 0; k < a->nkeys; ++k) {
@@ -880,7 +950,7 @@ gq_status gq_hash_aggregate_finish(gq_ctx* ctx, gq_aggstate* a, void* const* out
   cudaError_t e = cudaMemsetAsync(d_out_ngroups, 0, 8, ctx->stream);
   if (e != cudaSuccess) return cuda_fail(ctx, e, "memset ngroups");
   int nl = 0;
-  e = gq_launch_finalise(ctx->stream, p, ctx->num_sms, &nl);
+  e = PROF(ctx, "gq_k_finalise/topk", gq_launch_finalise(ctx->stream, p, ctx->num_sms, &nl));
   if (e != cudaSuccess) return cuda_fail(ctx, e, "finalise");
   ctx->launches += nl;
   return GQ_OK;
@@ -982,7 +1052,7 @@ static gq_status run_psa(gq_ctx* ctx, const gq_plan* plan, GqScanSpec sp, const 
     if (sp.check_dep) pat[1] = GQ_DEP_UNSET;
     for (int i = 0; i < d->naggs; ++i)
       pat[1 + d->ndependent + i] = d->aggs[i].op == GQ_MIN ? 0x7FFFFFFFFFFFFFFFULL : d->aggs[i].op == GQ_MAX ? 0x8000000000000000ULL : 0ULL;
-    e = gq_launch_init_table(ctx->stream, mt.slots, pp.merge_cap, sp.target_sw, pat, mt.side, 1, mt.header, 0, ctx->num_sms);
+    e = PROF(ctx, "gq_k_init_table", gq_launch_init_table(ctx->stream, mt.slots, pp.merge_cap, sp.target_sw, pat, mt.side, 1, mt.header, 0, ctx->num_sms));
     if (e != cudaSuccess) return cuda_fail(ctx, e, "merge table init");
     ++ctx->launches;
   }
@@ -1000,8 +1070,8 @@ static gq_status run_psa(gq_ctx* ctx, const gq_plan* plan, GqScanSpec sp, const 
     int nl = 0;
     const gq_column& kc = in->cols[sp.key_cols[0]];
     long long* hot = (long long*)(ws + pp.off_hot);
-    e = gq_launch_hot_keys(ctx->stream, kc.data, (int)kc.dtype, in->nrows, (unsigned long long*)(ws + pp.off_hot + 4096), GQ_HOT_SLOTS,
-                           GQ_HOT_SAMPLE, GQ_HOT_THRESHOLD, hot, GQ_HOT_MAX, ctx->num_sms, &nl);
+    e = PROF(ctx, "gq_k_hot_keys(4)", gq_launch_hot_keys(ctx->stream, kc.data, (int)kc.dtype, in->nrows, (unsigned long long*)(ws + pp.off_hot + 4096), GQ_HOT_SLOTS,
+                           GQ_HOT_SAMPLE, GQ_HOT_THRESHOLD, hot, GQ_HOT_MAX, ctx->num_sms, &nl));
     if (e != cudaSuccess) return cuda_fail(ctx, e, "heavy-hitter sampling");
     ctx->launches += nl;
     P.hot = hot;
@@ -1012,8 +1082,8 @@ static gq_status run_psa(gq_ctx* ctx, const gq_plan* plan, GqScanSpec sp, const 
   GqPsaDirParams dp{};
   dp.pcount = U(pp.off_pcount); dp.pstart = U(pp.off_pstart); dp.items = U(pp.off_items); dp.item_seg = U(pp.off_itemseg);
   dp.nitems = U(pp.off_zero) + 1; dp.npart = pp.npart; dp.seg_chunks = pp.seg_chunks; dp.err = ctx->d_err; dp.max_items = pp.max_items; dp.nsub = 1u << pp.log2sub;
-  e = gq_launch_psa_dir(ctx->stream, dp);
-  if (e == cudaSuccess) e = gq_launch_psa_fill(ctx->stream, U(pp.off_info), U(pp.off_ncta), (int)grid, slab, U(pp.off_pstart), U(pp.off_pfill), U(pp.off_plist));
+  e = PROF(ctx, "gq_k_psa_dir", gq_launch_psa_dir(ctx->stream, dp));
+  if (e == cudaSuccess) e = PROF(ctx, "gq_k_psa_fill", gq_launch_psa_fill(ctx->stream, U(pp.off_info), U(pp.off_ncta), (int)grid, slab, U(pp.off_pstart), U(pp.off_pfill), U(pp.off_plist)));
   if (e != cudaSuccess) return cuda_fail(ctx, e, "partition directory");
   ctx->launches += 2;
   CachedKernel* pk = nullptr;
@@ -1028,7 +1098,7 @@ static gq_status run_psa(gq_ctx* ctx, const gq_plan* plan, GqScanSpec sp, const 
   B.nitems = U(pp.off_zero) + 1; B.work = U(pp.off_zero); B.err = ctx->d_err; B.merge = mt; B.seg_chunks = pp.seg_chunks;
   B.hshift = 64 - pp.log2npart; B.log2sub = pp.log2sub; B.fin = F;
   void* args[] = {(void*)&B};
-  e = cudaLaunchKernel((const void*)kern.fn, dim3((unsigned)ctx->num_sms), dim3((unsigned)kern.threads), args, (size_t)kern.smem_bytes, ctx->stream);
+  e = PROF(ctx, "gq_psa", cudaLaunchKernel((const void*)kern.fn, dim3((unsigned)ctx->num_sms), dim3((unsigned)kern.threads), args, (size_t)kern.smem_bytes, ctx->stream));
   if (e != cudaSuccess) return cuda_fail(ctx, e, "launch of the partitioned aggregation kernel");
   ++ctx->launches;
   // groups of split partitions: appended to the same dense output
@@ -1042,7 +1112,7 @@ static gq_status run_psa(gq_ctx* ctx, const gq_plan* plan, GqScanSpec sp, const 
   for (int v = 0; v < F.navg; ++v) { fp.avg_sum[v] = F.avg_sum[v]; fp.avg_cnt[v] = F.avg_cnt[v]; fp.out_avg[v] = F.out_avg[v]; }
   fp.out_capacity = F.out_capacity; fp.out_n = F.out_n; fp.err = ctx->d_err;
   int nl = 0;
-  e = gq_launch_finalise(ctx->stream, fp, ctx->num_sms, &nl);
+  e = PROF(ctx, "gq_k_finalise/topk", gq_launch_finalise(ctx->stream, fp, ctx->num_sms, &nl));
   if (e != cudaSuccess) return cuda_fail(ctx, e, "merge table finalise");
   ctx->launches += nl;
   return GQ_OK;
@@ -1073,6 +1143,7 @@ gq_status gq_pipeline(gq_ctx* ctx, const gq_plan* plan, void* d_ws, size_t bytes
     if (st != GQ_OK) return st;
     P.fin.part = (long long*)((char*)d_ws + L.fused_off);
     P.fin.ticket = (unsigned*)(ctx->d_err + 16);
+    P.fin.gtab = (unsigned long long*)((char*)ctx->d_err + 256);
     return run_scan(ctx, sp, plan->in, d->probes, &P);
   }
   // One large batch into a group-by table far larger than L2: partitioned shared-memory aggregation
@@ -1097,10 +1168,34 @@ gq_status gq_pipeline(gq_ctx* ctx, const gq_plan* plan, void* d_ws, size_t bytes
 gq_status gq_read_probe(gq_ctx* ctx, const void* d_data, size_t bytes, uint64_t* d_out) {
   if (!ctx || !d_data || !d_out || !aligned(d_data, 16) || bytes % 16) return GQ_ERR_INVALID_ARG;
   use_device(ctx);
-  cudaError_t e = gq_launch_read_probe(ctx->stream, d_data, bytes, (unsigned long long*)d_out, ctx->num_sms);
+  cudaError_t e = PROF(ctx, "gq_k_read_probe", gq_launch_read_probe(ctx->stream, d_data, bytes, (unsigned long long*)d_out, ctx->num_sms));
   if (e != cudaSuccess) return cuda_fail(ctx, e, "read probe");
   ++ctx->launches;
   return GQ_OK;
+}
+
+gq_status gq_profile(gq_ctx* ctx, int32_t enable) {
+  if (!ctx) return GQ_ERR_INVALID_ARG;
+  ctx->prof = enable != 0;
+  ctx->prof_names.clear();
+  return GQ_OK;
+}
+
+int32_t gq_profile_read(gq_ctx* ctx, char* h_names, size_t names_bytes, float* h_ms, int32_t max_entries) {
+  if (!ctx || !h_ms || max_entries < 0) return -1;
+  use_device(ctx);
+  if (cudaStreamSynchronize(ctx->stream) != cudaSuccess) return -1;
+  std::string names;
+  int32_t n = 0;
+  for (size_t i = 0; i < ctx->prof_names.size() && n < max_entries; ++i, ++n) {
+    float ms = 0.f;
+    if (cudaEventElapsedTime(&ms, ctx->prof_ev[2 * i], ctx->prof_ev[2 * i + 1]) != cudaSuccess) ms = -1.f;
+    h_ms[n] = ms;
+    names += ctx->prof_names[i]; names += '\n';
+  }
+  if (h_names && names_bytes) { strncpy(h_names, names.c_str(), names_bytes - 1); h_names[names_bytes - 1] = 0; }
+  ctx->prof_names.clear();
+  return n;
 }
 
 gq_status gq_set_option(const char* h_name, int64_t value) {
@@ -1123,8 +1218,12 @@ const int64_t GQ_HOST_CHUNK_ALIGN = 30720;   // lcm of the tile sizes the plan c
 struct HostLayout { size_t agg_off, agg_bytes, topk_off, stage_off[2], stage_col_off[GQ_MAX_COLS], stage_bytes, out_off, out_key_off[2],
                     out_agg_off[GQ_MAX_AGGS], out_avg_off[GQ_MAX_AGGS], n_off, total; };
 gq_status host_layout(const gq_plan* plan, int64_t chunk_rows, int64_t out_capacity, HostLayout* L) {
+  // plan-aware state size for one chunk-sized batch: direct aggregation (group key = key of a probed unique table) is
+  // taken exactly as in gq_pipeline, so the end-to-end path runs the same fused kernels as the device-resident one
   size_t aggb = 0;
-  gq_status st = gq_hash_aggregate_workspace(plan->agg.max_groups, plan->agg.nkeys, plan->agg.naggs, &aggb);
+  gq_batch shape = *plan->in;
+  shape.nrows = std::min<int64_t>(plan->in->nrows, chunk_rows);
+  gq_status st = gq_hash_aggregate_workspace_for(&shape, &plan->agg, &aggb);
   if (st != GQ_OK) return st;
   size_t off = 0;
   L->agg_off = 0; L->agg_bytes = aggb; off = align_up(aggb, 256);

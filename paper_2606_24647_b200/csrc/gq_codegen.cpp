@@ -221,7 +221,8 @@ static gq_status emit_linear(Gen& g, const GqScanSpec& sp, std::ostringstream& o
     const std::string S = std::to_string(s);
     const std::string karr = as_array(ps.key_col);
     o << "  u64 pi" << S << "[GQ_R]; i64 py" << S << "[GQ_R][" << (ps.npayload > 0 ? ps.npayload : 1) << "];\n";
-    o << "  gq_probe_rows<" << ps.slot_words << ", " << ps.npayload << ">(P.probe[" << S << "], " << karr << ", live, pi" << S
+    if (ps.dense) o << "  gq_dense_probe_rows<" << ps.npayload << ">(P.probe[" << S << "], " << karr << ", live, pi" << S << ", py" << S << ");\n";
+    else o << "  gq_probe_rows<" << ps.slot_words << ", " << ps.npayload << ">(P.probe[" << S << "], " << karr << ", live, pi" << S
       << ", py" << S << ");\n";
     o << "  (void)pi" << S << "; (void)py" << S << ";\n";
   }
@@ -335,7 +336,8 @@ static gq_status emit_linear(Gen& g, const GqScanSpec& sp, std::ostringstream& o
         for (int p = 0; p < np; ++p) o << "    bpay[j][" << p << "] = " << g.val(sp.payload_cols[(size_t)p]) << ";\n";
         o << "  }\n";
       }
-      o << "  cx.ninserted += gq_insert_rows<" << sp.target_sw << ", " << np << ">(P.target, " << karr << ", live, bpay, "
+      if (sp.dense_target) o << "  cx.ninserted += gq_dense_insert_rows<" << np << ">(P.target, " << karr << ", live, bpay, P.err);\n";
+      else o << "  cx.ninserted += gq_insert_rows<" << sp.target_sw << ", " << np << ">(P.target, " << karr << ", live, bpay, "
         << (sp.unique ? "true" : "false") << ", P.err);\n";
       break;
     }
@@ -513,6 +515,14 @@ gq_status gq_codegen(const GqScanSpec& sp, GqKernelInfo* out, std::string* msg) 
       ind += "  ";
       o << ind << "const GqTableDev& T" << s << " = P.probe[" << s << "];\n";
       o << ind << "const i64 pk" << s << " = " << g.val(ps.key_col) << ";\n";
+      if (ps.dense) {   // direct-address table: at most one match, found with one bit test
+        o << ind << "for (int n" << s << " = 0; n" << s << " < 1; ++n" << s << ") {\n";
+        ind += "  ";
+        o << ind << "u64 i" << s << ";\n" << ind << "if (!gq_dense_find(T" << s << ", pk" << s << ", &i" << s << ")) break;\n";
+        for (int p = 0; p < ps.npayload; ++p)
+          o << ind << "const i64 y" << s << "_" << p << " = (i64)__ldg(T" << s << ".slots + i" << s << " * " << ps.npayload << " + " << p << ");\n";
+        continue;
+      }
       o << ind << "const bool sd" << s << " = ((u64)pk" << s << " == GQ_EMPTY);\n";
       o << ind << "i64 ns" << s << " = 0; if (sd" << s << ") ns" << s << " = gq_min(T" << s << ".header[1], GQ_SIDE_SLOTS);\n";
       o << ind << "u64 i" << s << " = gq_slot0(T" << s << ", pk" << s << ");\n";
@@ -574,7 +584,8 @@ gq_status gq_codegen(const GqScanSpec& sp, GqKernelInfo* out, std::string* msg) 
         for (int p = 0; p < np; ++p) o << (p ? ", " : "") << g.val(sp.payload_cols[(size_t)p]);
         if (np == 0) o << "0";
         o << "};\n";
-        o << ind << "if (gq_ht_insert<" << sp.target_sw << ", " << np << ">(P.target, " << g.val(sp.build_key_col) << ", pay, "
+        if (sp.dense_target) o << ind << "if (gq_dense_insert<" << np << ">(P.target, " << g.val(sp.build_key_col) << ", pay, P.err)) ++cx.ninserted;\n";
+        else o << ind << "if (gq_ht_insert<" << sp.target_sw << ", " << np << ">(P.target, " << g.val(sp.build_key_col) << ", pay, "
           << (sp.unique ? "true" : "false") << ", P.err)) ++cx.ninserted;\n";
         break;
       }

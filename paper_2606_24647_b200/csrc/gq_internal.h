@@ -15,6 +15,8 @@
 #define GQ_MAXOUT 12
 #define GQ_SMEM_LIMIT 232448   // 227 KB opt-in dynamic shared memory per CTA on sm_100
 #define GQ_DEFAULT_SMS 148     // B200; used only when a plan is compiled ahead of time without a device attached
+#define GQ_GTAB_SLOTS 64        // merge table of the fused low-cardinality finaliser: 64 slots of 16 words {state, key, aggregates}
+#define GQ_GTAB_BYTES (256 + GQ_GTAB_SLOTS * 128)
 #define GQ_DEP_UNSET 0x8000000000000001ULL   // dependent-key word of a slot nobody has stored yet (GQ_F_CHECK_DEPENDENT)
 
 enum { GQ_C_GLOBAL = 0, GQ_C_LOWCARD = 1, GQ_C_HIGHCARD = 2, GQ_C_BUILD = 3, GQ_C_MATERIALISE = 4, GQ_C_DIRECT = 5, GQ_C_PARTITION = 6, GQ_C_SCATTER = 7 };
@@ -29,10 +31,13 @@ struct GqTableDev {
   int slot_words;
   unsigned flags;
   unsigned bshift;             // log2(slots per 32-byte bucket) for join tables, 0 for aggregation tables
+  long long base;              // direct-address (GQ_F_DENSE_KEYS) tables: key_min; slots = payload rows, side = bitmap,
+                               // mask = range size - 1
 };
 struct GqFinal {
   long long* part;
   unsigned* ticket;
+  unsigned long long* gtab;
   void* out_key[2];
   long long* out_agg[8];
   double* out_avg[8];
@@ -72,12 +77,16 @@ struct GqParams {
 struct gq_ctx {
   int device = 0;
   cudaStream_t stream = nullptr;
-  int* d_err = nullptr;        // sticky device error; d_err + 16 = ticket counter of the fused finaliser
+  int* d_err = nullptr;        // sticky device error; d_err + 16 = ticket counter of the fused finaliser;
+                               // (char*)d_err + 256 = merge table of the fused low-cardinality finaliser (GQ_GTAB_BYTES)
   int* h_err = nullptr;        // pinned mirror
   int num_sms = GQ_DEFAULT_SMS;
   int last_cuda = 0;
   int64_t launches = 0;
   std::string msg;
+  bool prof = false;           // gq_profile: every kernel launch group is bracketed by a pair of events
+  std::vector<cudaEvent_t> prof_ev;      //   2 events per recorded group (reused across reads)
+  std::vector<std::string> prof_names;   //   names of the groups recorded since the last gq_profile_read
   cudaStream_t copy_stream = nullptr;   // gq_pipeline_host: H2D copies overlap the scan of the previous chunk
   cudaEvent_t ev_copied[2] = {nullptr, nullptr}, ev_consumed[2] = {nullptr, nullptr}, ev_start = nullptr;
 };
@@ -90,6 +99,8 @@ struct gq_table {
   gq_dtype payload_dtype[GQ_MAX_PAYLOAD] = {GQ_I64, GQ_I64, GQ_I64};
   uint32_t flags = 0;
   int64_t max_rows = 0;
+  bool dense = false;          // GQ_F_DENSE_KEYS: direct-address table over [key_min, key_min + capacity)
+  int64_t key_min = 0;
   std::string build_sig;       // shape signature of the first batch (later batches must match)
   cudaEvent_t ready = nullptr; // recorded by gq_hash_build_finish
   cudaStream_t build_stream = nullptr;
@@ -109,6 +120,7 @@ struct gq_aggstate {
   bool check_dep = false;      // GQ_F_CHECK_DEPENDENT
   bool direct = false;         // aggregate words indexed by the slot of a probed unique table (no keys stored)
   GqTableDev dtab{};           //   that table
+  bool ddense = false; int dnpay = 0;   //   ... is a direct-address table with dnpay payload words per row
   int64_t dcap = 0;            //   its capacity (the accumulator array has dcap + 1 slots: the last is the side entry)
   int daw = 0, dtouch = -1, dep_pay = -1;   // words per accumulator slot, word that marks a touched slot, payload = dep key
   unsigned long long* dacc = nullptr;
@@ -127,6 +139,7 @@ struct GqProbeSpec {
   int npayload;
   gq_dtype pay_dtype[GQ_MAX_PAYLOAD];
   bool unique;
+  bool dense;                  // direct-address table (GQ_F_DENSE_KEYS)
   int slot_words;
 };
 struct GqScanSpec {
@@ -151,6 +164,7 @@ struct GqScanSpec {
   int build_key_col = 0;                          // BUILD
   std::vector<int> payload_cols;
   bool unique = false;
+  bool dense_target = false;                      // BUILD into a direct-address table
   bool hot = false;                               // HIGHCARD: per-CTA shared-memory aggregation of hot keys
   bool check_dep = false;                         // GQ_F_CHECK_DEPENDENT: every row verifies the dependent key
   int num_sms = GQ_DEFAULT_SMS;                   // tiling heuristics: SM count of the context's device
@@ -184,6 +198,7 @@ struct GqFinaliseParams {
   // direct mode: groups = touched accumulator slots; keys / dependent key come from the join table
   int direct; const unsigned long long* dacc; int daw, dtouch, dep_pay;
   const unsigned long long* jslots; const unsigned long long* jside; int jsw;
+  int jdense; long long jbase; int jnpay;        // direct-address join table: key = jbase + i, payload row i of jnpay words
   int nkeys, ndep, naggs;
   int key_bits[2]; int key_dtype[2];
   void* out_key[2]; long long* out_agg[GQ_MAX_AGGS];

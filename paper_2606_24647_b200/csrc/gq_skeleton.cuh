@@ -32,6 +32,7 @@ typedef unsigned int u32;
 #define GQ_MAXK 48
 #define GQ_MAXOUT 12
 #define GQ_SIDE_SLOTS 64
+#define GQ_GTAB_SLOTS 64
 
 #define GQ_C_GLOBAL 0
 #define GQ_C_LOWCARD 1
@@ -45,6 +46,7 @@ typedef unsigned int u32;
 #define GQ_E_CAPACITY 3
 #define GQ_E_DUPLICATE 6
 #define GQ_E_DEPENDENT 8
+#define GQ_E_KEYRANGE 9
 
 #define GQ_OP_SUM 0
 #define GQ_OP_MIN 1
@@ -61,14 +63,19 @@ struct GqTableDev {
   int slot_words;
   u32 flags;
   u32 bshift;        // log2(slots per 32-byte bucket): probe sequences start on a bucket boundary (join tables)
+  i64 base;          // direct-address table (GQ_F_DENSE_KEYS): key_min; then slots = payload rows [range][NPAY],
+                     // side = membership bitmap (u32 words), mask = range size - 1
 };
 
 // Outputs of the finaliser fused into the scan kernel (gq_pipeline over one batch, LOWCARD / GLOBAL consumers): every
-// CTA writes its partial groups to `part`, takes a ticket, and the last CTA merges all partials and emits the dense
-// result (keys, aggregates, AVG, group count) — no separate init / finalise launches. Must match gq_internal.h.
+// CTA folds its partial groups into a small context-owned table (LOWCARD: find-or-claim by key, then RED) or writes its
+// partial aggregates to `part` (GLOBAL), takes a ticket, and the last CTA emits the dense result (keys, aggregates, AVG,
+// group count) and leaves table and ticket zeroed — no separate init / finalise launches. Must match gq_internal.h.
 struct GqFinal {
-  i64* part;                    // [grid][G][1 + NAGG] (LOWCARD) or [grid][NAGG] (GLOBAL), then [grid] group counts
+  i64* part;                    // GLOBAL: [grid][NAGG] per-CTA partial aggregates
   u32* ticket;                  // context-owned counter, zero between kernels (reset by the last CTA)
+  u64* gtab;                    // LOWCARD: context-owned merge table, all states zero between kernels: word 0 = groups
+                                //   claimed, then from word 32 GQ_GTAB_SLOTS slots of 16 words {state, key, aggregates}
   void* out_key[2];
   i64* out_agg[8];
   double* out_avg[8];
@@ -149,6 +156,15 @@ __device__ __forceinline__ u64 gq_ld_relaxed(const u64* p) {               // se
   u64 v;
   asm volatile("ld.relaxed.gpu.global.u64 %0, [%1];" : "=l"(v) : "l"(p) : "memory");
   return v;
+}
+
+__device__ __forceinline__ u64 gq_ld_acquire(const u64* p) {
+  u64 v;
+  asm volatile("ld.acquire.gpu.global.u64 %0, [%1];" : "=l"(v) : "l"(p) : "memory");
+  return v;
+}
+__device__ __forceinline__ void gq_st_release(u64* p, u64 v) {
+  asm volatile("st.release.gpu.global.u64 [%0], %1;" ::"l"(p), "l"(v) : "memory");
 }
 
 // ---------------------------------------------------------------------------------------------- wrapping int64
@@ -412,6 +428,57 @@ __device__ __forceinline__ void gq_upsert_rows(const GqTableDev& T, const i64 (&
           k[j] = gq_ld_relaxed(T.slots + idx[j] * SW);
         }
       }
+    }
+  }
+}
+
+// ---- direct-address join tables (GQ_F_DENSE_KEYS; SURVEY 8(f) NEXT-3 "dense-key array mode"): the planner
+// declared the build keys' range, so slot = key - key_min: HashBuild sets a bit in a membership bitmap (atomicOr: a bit
+// found set is a duplicate key) and stores the payload row; HashProbe is one bit test (the bitmap of a 15 M-key
+// range is 1.9 MB: L2-resident, so the probes that miss never reach DRAM) plus, on a hit, the payload row. The
+// matched slot index (key - key_min) serves direct aggregation exactly like a hash-table slot index.
+template <int NPAY>
+__device__ __forceinline__ bool gq_dense_insert(const GqTableDev& T, i64 key, const i64* pay, int* err) {
+  const u64 idx = (u64)key - (u64)T.base;
+  if (idx > T.mask) { gq_set_err(err, GQ_E_KEYRANGE); return false; }
+  const u32 bit = 1u << (u32)(idx & 31);
+  const u32 old = atomicOr((u32*)T.side + (idx >> 5), bit);
+  if (old & bit) { gq_set_err(err, GQ_E_DUPLICATE); return false; }
+#pragma unroll
+  for (int p = 0; p < NPAY; ++p) T.slots[idx * NPAY + p] = (u64)pay[p];
+  return true;
+}
+template <int NPAY>
+__device__ __forceinline__ int gq_dense_insert_rows(const GqTableDev& T, const i64 (&key)[GQ_R], const bool (&live)[GQ_R],
+                                                    const i64 (&pay)[GQ_R][NPAY > 0 ? NPAY : 1], int* err) {
+  int n = 0;
+#pragma unroll
+  for (int j = 0; j < GQ_R; ++j)
+    if (live[j] && gq_dense_insert<NPAY>(T, key[j], pay[j], err)) ++n;
+  return n;
+}
+__device__ __forceinline__ bool gq_dense_find(const GqTableDev& T, i64 key, u64* idx) {
+  *idx = (u64)key - (u64)T.base;
+  if (*idx > T.mask) return false;
+  return (__ldg((const u32*)T.side + (*idx >> 5)) >> (u32)(*idx & 31)) & 1u;
+}
+template <int NPAY>
+__device__ __forceinline__ void gq_dense_probe_rows(const GqTableDev& T, const i64 (&key)[GQ_R], bool (&live)[GQ_R],
+                                                    u64 (&idx)[GQ_R], i64 (&pay)[GQ_R][NPAY > 0 ? NPAY : 1]) {
+  u32 wv[GQ_R];
+#pragma unroll
+  for (int j = 0; j < GQ_R; ++j) {                      // the bitmap words of all rows in flight together
+    idx[j] = (u64)key[j] - (u64)T.base;
+    live[j] = live[j] && idx[j] <= T.mask;
+    wv[j] = live[j] ? __ldg((const u32*)T.side + (idx[j] >> 5)) : 0u;
+  }
+#pragma unroll
+  for (int j = 0; j < GQ_R; ++j) live[j] = live[j] && ((wv[j] >> (u32)(idx[j] & 31)) & 1u);
+#pragma unroll
+  for (int j = 0; j < GQ_R; ++j) {
+    if (live[j]) {
+#pragma unroll
+      for (int p = 0; p < NPAY; ++p) pay[j][p] = (i64)__ldg(T.slots + idx[j] * NPAY + p);
     }
   }
 }

@@ -155,7 +155,16 @@ extern "C" __global__ void __launch_bounds__(GQ_NT + 32, 1) gq_scan(const __grid
   __syncthreads();
   if (*err_seen != 0) {
 #if GQ_FUSED_FINAL
-    if (tid == 0) { const u32 t = atomicAdd(P.fin.ticket, 1u); if (t == gridDim.x - 1) *P.fin.ticket = 0; }
+    if (tid == 0) {   // keep ticket (and merge table) zeroed for the next kernel
+      const u32 t = atomicAdd(P.fin.ticket, 1u);
+      if (t == gridDim.x - 1) {
+        *P.fin.ticket = 0;
+#if GQ_CONSUMER == GQ_C_LOWCARD
+        P.fin.gtab[0] = 0;
+        for (int i = 0; i < GQ_GTAB_SLOTS; ++i) P.fin.gtab[32 + i * 16] = 0;
+#endif
+      }
+    }
 #endif
     return;
   }
@@ -286,74 +295,71 @@ extern "C" __global__ void __launch_bounds__(GQ_NT + 32, 1) gq_scan(const __grid
       }
     }
 #else
-    // ---- finaliser fused into the scan: partials -> global scratch -> ticket -> last CTA merges and emits
-    constexpr int PW = 1 + GQ_NAGG;                      // words per partial group: key, aggregates
-    i64* mypart = P.fin.part + (i64)blockIdx.x * GQ_LC_G * PW;
-    i64* pn = P.fin.part + (i64)gridDim.x * GQ_LC_G * PW;
+    // ---- finaliser fused into the scan: CTA-level reduction -> the CTA's <= GQ_LC_G groups are folded into
+    // the context-owned merge table (find-or-claim by key: the claimer stores its values and publishes the slot, later
+    // CTAs RED theirs in) -> ticket -> the last CTA only reads the table, emits and zeroes it. Replaces "every CTA
+    // writes its partials, the last one folds grid x G of them" (C1: that tail was 6 of 18 us).
     i64* fin = (i64*)(gq_smem + GQ_CONS_OFF + GQ_LC_FIN_OFF);
     for (int p0 = warp; p0 < ng * GQ_NAGG; p0 += 4 * GQ_NWARP) {
       i64 v[4];
       gq_lc_reduce4(cx, p0, ng * GQ_NAGG, lane, v);
 #pragma unroll
-      for (int u = 0; u < 4; ++u) {
-        const int p = p0 + u * GQ_NWARP;
-        if (lane == 0 && p < ng * GQ_NAGG) {
-          const int g = p / GQ_NAGG, a = p % GQ_NAGG;
-          mypart[g * PW + 1 + a] = v[u];
-          if (a == 0) mypart[g * PW] = cx.lc_gkey[g];
+      for (int u = 0; u < 4; ++u)
+        if (lane == 0 && p0 + u * GQ_NWARP < ng * GQ_NAGG) fin[p0 + u * GQ_NWARP] = v[u];
+    }
+    gq_consumer_barrier();
+    u64* gt = P.fin.gtab;
+    if (tid < ng) {
+      const i64 key = cx.lc_gkey[tid];
+      u32 h = (u32)gq_hash(key, 64 - 6);
+      bool done = false;
+      for (int n = 0; n < GQ_GTAB_SLOTS && !done; ++n, h = (h + 1) & (GQ_GTAB_SLOTS - 1)) {
+        u64* s = gt + 32 + h * 16;
+        u64 st = gq_ld_acquire(s);
+        if (st == 0) {
+          st = atomicCAS(s, 0ULL, 1ULL);
+          if (st == 0) {                                   // claimed: store key and values, then publish
+            s[1] = (u64)key;
+#pragma unroll
+            for (int a = 0; a < GQ_NAGG; ++a) s[2 + a] = (u64)fin[tid * GQ_NAGG + a];
+            gq_st_release(s, 2ULL);
+            if (atomicAdd(gt, 1ULL) >= (u64)GQ_LC_G) gq_set_err(P.err, GQ_E_CAPACITY);   // more distinct keys than max_groups
+            done = true;
+            break;
+          }
+        }
+        while (st == 1) st = gq_ld_acquire(s);             // being published by another CTA
+        if (s[1] == (u64)key) {
+#pragma unroll
+          for (int a = 0; a < GQ_NAGG; ++a) gq_red(GQ_AGG_OP(a), s + 2 + a, fin[tid * GQ_NAGG + a]);
+          done = true;
         }
       }
+      if (!done) gq_set_err(P.err, GQ_E_CAPACITY);
     }
-    if (tid == 0) pn[blockIdx.x] = ng;
     gq_consumer_barrier();
     if (tid == 0) { __threadfence(); cx.lc_n[3] = (atomicAdd(P.fin.ticket, 1u) == gridDim.x - 1); }
     gq_consumer_barrier();
     if (((volatile int*)cx.lc_n)[3]) {
-      // (writers fenced before taking their ticket; the partials are read with ld.cg after the CTA barrier above)
+      // (every CTA fenced its table updates before taking its ticket; the table is read with ld.cg)
+      __threadfence();
+      if (tid < GQ_GTAB_SLOTS) {                            // warps 0 and 1: one slot per lane
+        u64* s = gt + 32 + tid * 16;
+        const bool have = __ldcg((const i64*)s) == 2;
+        const u32 m = __ballot_sync(0xffffffffu, have);
+        if (tid == 31) cx.lc_n[2] = __popc(m);            // groups in slots 0..31 (lc_n[2] is free by now)
+        asm volatile("bar.sync 2, 64;" ::: "memory");
+        const int row = (tid >= 32 ? ((volatile int*)cx.lc_n)[2] : 0) + __popc(m & ((1u << lane) - 1u));
+        if (have) {
+          i64 vals[GQ_NAGG];
 #pragma unroll
-      for (int a = 0; a < GQ_NAGG; ++a)
-        for (int g = 0; g < GQ_LC_G; ++g) cx.lc_acc[(g * GQ_NAGG + a) * GQ_NT + tid] = gq_identity(GQ_AGG_OP(a));
-      // fold every CTA's partial groups into this CTA's private cells: one (CTA, group) pair per thread and round,
-      // the loads of four rounds issued together (group ids are those of THIS CTA's key table)
-      const int npairs = (int)gridDim.x * GQ_LC_G;
-      for (int p0 = 0; p0 < npairs; p0 += 4 * GQ_NT) {   // uniform bounds: the slow path needs converged warps
-        i64 w[4][PW];
-        i64 nb[4];
-#pragma unroll
-        for (int u = 0; u < 4; ++u) {
-          const int p = p0 + u * GQ_NT + tid;
-          const int pc = p < npairs ? p : 0;
-          nb[u] = gq_ldcg(pn + pc / GQ_LC_G);
-#pragma unroll
-          for (int i = 0; i < PW; ++i) w[u][i] = gq_ldcg(P.fin.part + (i64)pc * PW + i);   // stale beyond the CTA's count
+          for (int a = 0; a < GQ_NAGG; ++a) vals[a] = __ldcg((const i64*)s + 2 + a);
+          if (row < P.fin.out_capacity) gq_fin_emit(P.fin, row, __ldcg((const i64*)s + 1), vals);
+          else gq_set_err(P.err, GQ_E_CAPACITY);
+          s[0] = 0;
         }
-#pragma unroll
-        for (int u = 0; u < 4; ++u) {
-          const int p = p0 + u * GQ_NT + tid;
-          const bool have = p < npairs && (p % GQ_LC_G) < (int)nb[u];
-          int grp = have ? gq_lc_find(cx, w[u][0]) : 0;
-          if (__any_sync(0xffffffffu, have && grp < 0)) grp = gq_lc_slow(cx, w[u][0], have && grp < 0, grp, P.err);
-          if (have) {
-#pragma unroll
-            for (int a = 0; a < GQ_NAGG; ++a) gq_lc_update(GQ_AGG_OP(a), cx, grp, a, w[u][1 + a]);
-          }
-        }
+        if (tid == 63) { *P.fin.out_n = row + (have ? 1 : 0); gt[0] = 0; *P.fin.ticket = 0; }
       }
-      gq_consumer_barrier();
-      const int ng2 = min(((volatile int*)cx.lc_n)[0], GQ_LC_G);
-      for (int p0 = warp; p0 < ng2 * GQ_NAGG; p0 += 4 * GQ_NWARP) {
-        i64 v[4];
-        gq_lc_reduce4(cx, p0, ng2 * GQ_NAGG, lane, v);
-#pragma unroll
-        for (int u = 0; u < 4; ++u)
-          if (lane == 0 && p0 + u * GQ_NWARP < ng2 * GQ_NAGG) fin[p0 + u * GQ_NWARP] = v[u];
-      }
-      gq_consumer_barrier();
-      if (tid < ng2) {
-        if (tid < P.fin.out_capacity) gq_fin_emit(P.fin, tid, cx.lc_gkey[tid], fin + tid * GQ_NAGG);
-        else gq_set_err(P.err, GQ_E_CAPACITY);
-      }
-      if (tid == 0) { *P.fin.out_n = ng2; *P.fin.ticket = 0; }
     }
 #endif
   }

@@ -66,6 +66,12 @@ __device__ __forceinline__ bool gq_group_at(const GqFinaliseParams& P, i64 i, Gq
   if (P.direct) {
     const u64* acc = P.dacc + i * P.daw;
     if (acc[P.dtouch] == 0) return false;
+    if (P.jdense) {   // direct-address join table: the key is the slot index, the dependent key a word of payload row i
+      g->key = (u64)(P.jbase + i);
+      g->dep = P.jslots + i * P.jnpay + (P.dep_pay > 0 ? P.dep_pay : 0);
+      g->agg = acc;
+      return i < P.capacity;
+    }
     const u64* js = i < P.capacity ? P.jslots + i * P.jsw : P.jside;
     g->key = i < P.capacity ? js[0] : GQ_EMPTY_KEY;
     g->dep = js + 1 + (P.dep_pay > 0 ? P.dep_pay : 0);

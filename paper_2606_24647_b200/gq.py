@@ -28,8 +28,9 @@ _XOP = dict(col=0, const=1, add=2, sub=3, mul=4)
 _AGG = dict(sum=0, min=1, max=2, count=3)
 F_UNIQUE_KEYS = 1
 F_CHECK_DEPENDENT = 2
+F_DENSE_KEYS = 4
 STATUS = ["GQ_OK", "GQ_ERR_INVALID_ARG", "GQ_ERR_UNSUPPORTED", "GQ_ERR_CAPACITY", "GQ_ERR_WORKSPACE_TOO_SMALL",
-          "GQ_ERR_CUDA", "GQ_ERR_DUPLICATE_KEY", "GQ_ERR_COMPILE", "GQ_ERR_DEPENDENT_KEY"]
+          "GQ_ERR_CUDA", "GQ_ERR_DUPLICATE_KEY", "GQ_ERR_COMPILE", "GQ_ERR_DEPENDENT_KEY", "GQ_ERR_KEY_RANGE"]
 
 # every symbol include/gq.h declares (tests check that the library exports all of them)
 SYMBOLS = ["gq_create", "gq_destroy", "gq_sync", "gq_clear_error", "gq_status_str", "gq_last_cuda_error",
@@ -38,7 +39,7 @@ SYMBOLS = ["gq_create", "gq_destroy", "gq_sync", "gq_clear_error", "gq_status_st
            "gq_hash_aggregate_workspace", "gq_hash_aggregate_workspace_for", "gq_hash_aggregate", "gq_topk_scratch_bytes", "gq_hash_aggregate_finish",
            "gq_aggstate_destroy", "gq_pipeline_workspace", "gq_pipeline", "gq_pipeline_host_workspace",
            "gq_pipeline_host", "gq_set_kernel_cache_dir", "gq_precompile_pipeline", "gq_precompile_build", "gq_precompile_materialise",
-           "gq_table_describe", "gq_read_probe", "gq_set_option"]
+           "gq_table_describe", "gq_read_probe", "gq_set_option", "gq_hash_build_workspace_dense", "gq_profile", "gq_profile_read"]
 
 
 class GqError(RuntimeError):
@@ -78,7 +79,7 @@ class _Probe(C.Structure):
 class _BuildDesc(C.Structure):
     _fields_ = [("preds", C.POINTER(_Pred)), ("npred", C.c_int32), ("probes", C.POINTER(_Probe)),
                 ("nprobes", C.c_int32), ("key_col", C.c_int32), ("payload_cols", C.POINTER(C.c_int32)),
-                ("npayload", C.c_int32), ("flags", C.c_uint32)]
+                ("npayload", C.c_int32), ("flags", C.c_uint32), ("key_min", C.c_int64), ("key_max", C.c_int64)]
 
 
 class _AggDesc(C.Structure):
@@ -117,6 +118,7 @@ def lib():
         L.gq_filter_project.argtypes = [C.c_void_p, C.POINTER(_Batch), C.POINTER(_Pred), C.c_int32, C.POINTER(_Expr),
                                         C.c_int32, C.POINTER(C.c_void_p), C.c_int64, C.c_void_p]
         L.gq_hash_build_workspace.argtypes = [C.c_int64, C.c_int32, C.POINTER(C.c_size_t)]
+        L.gq_hash_build_workspace_dense.argtypes = [C.c_int64, C.c_int64, C.c_int32, C.POINTER(C.c_size_t)]
         L.gq_hash_build.argtypes = [C.c_void_p, C.POINTER(C.c_void_p), C.c_void_p, C.c_size_t, C.c_int64,
                                     C.POINTER(_Batch), C.POINTER(_BuildDesc)]
         L.gq_hash_build_finish.argtypes = [C.c_void_p, C.c_void_p]
@@ -147,6 +149,9 @@ def lib():
         L.gq_table_describe.argtypes = [C.POINTER(C.c_void_p), C.POINTER(C.c_int), C.c_int32, C.c_uint32]
         L.gq_read_probe.argtypes = [C.c_void_p, C.c_void_p, C.c_size_t, C.c_void_p]
         L.gq_set_option.argtypes = [C.c_char_p, C.c_int64]
+        L.gq_profile.argtypes = [C.c_void_p, C.c_int32]
+        L.gq_profile_read.argtypes = [C.c_void_p, C.c_char_p, C.c_size_t, C.POINTER(C.c_float), C.c_int32]
+        L.gq_profile_read.restype = C.c_int32
         _lib = L
     return _lib
 
@@ -224,11 +229,13 @@ class _M:
         return _AggDesc(pr, npr, pb, npb, ee, ne, kk, nk, int(ndependent), aa, len(aggs), int(max_groups),
                         F_CHECK_DEPENDENT if check_dependent else 0)
 
-    def build_desc(self, preds, probes, key, payload, unique):
+    def build_desc(self, preds, probes, key, payload, unique, dense_range=None):
         pr, npr = self.preds(preds)
         pb, npb = self.probes(probes)
         pay, npay = self.ints(payload)
-        return _BuildDesc(pr, npr, pb, npb, int(key), pay, npay, F_UNIQUE_KEYS if unique else 0)
+        lo, hi = (int(dense_range[0]), int(dense_range[1])) if dense_range is not None else (0, 0)
+        return _BuildDesc(pr, npr, pb, npb, int(key), pay, npay,
+                          (F_UNIQUE_KEYS if unique else 0) | (F_DENSE_KEYS if dense_range is not None else 0), lo, hi)
 
     def avgs(self, avgs):
         aa = (_Avg * max(1, len(avgs)))()
@@ -256,11 +263,11 @@ class Table:
             pass
 
 
-def describe_table(payload_dtypes=(), unique=False) -> Table:
+def describe_table(payload_dtypes=(), unique=False, dense=False) -> Table:
     """Schema-only table handle for ahead-of-time kernel compilation (no device memory)."""
     h = C.c_void_p()
     arr = (C.c_int * max(1, len(payload_dtypes)))(*payload_dtypes)
-    st = lib().gq_table_describe(C.byref(h), arr, len(payload_dtypes), F_UNIQUE_KEYS if unique else 0)
+    st = lib().gq_table_describe(C.byref(h), arr, len(payload_dtypes), (F_UNIQUE_KEYS if unique else 0) | (F_DENSE_KEYS if dense else 0))
     if st:
         raise GqError(st)
     return Table(h, None, payload_dtypes)
@@ -364,16 +371,20 @@ class Context:
 
     # ---- HashBuild ----
     def hash_build(self, cols, preds=(), probes=(), key=0, payload=(), unique=False, max_rows=None, table=None,
-                   finish=True, workspace=None):
-        """workspace: a uint8 CUDA tensor to (re)use for the table instead of allocating one."""
+                   finish=True, workspace=None, dense_range=None):
+        """workspace: a uint8 CUDA tensor to (re)use for the table instead of allocating one.
+        dense_range=(key_min, key_max): GQ_F_DENSE_KEYS, a direct-address table over that key range."""
         with torch.cuda.stream(self.stream):
             m = _M()
             b = m.batch(cols)
-            d = m.build_desc(preds, probes, key, payload, unique)
+            d = m.build_desc(preds, probes, key, payload, unique, dense_range)
             if table is None:
                 max_rows = int(b.nrows if max_rows is None else max_rows)
                 nbytes = C.c_size_t()
-                self._check(self.L.gq_hash_build_workspace(max_rows, len(payload), C.byref(nbytes)))
+                if dense_range is not None:
+                    self._check(self.L.gq_hash_build_workspace_dense(int(dense_range[0]), int(dense_range[1]), len(payload), C.byref(nbytes)))
+                else:
+                    self._check(self.L.gq_hash_build_workspace(max_rows, len(payload), C.byref(nbytes)))
                 ws = workspace if workspace is not None else self._ws(nbytes.value)
                 if ws.numel() < nbytes.value + 256:
                     raise ValueError("workspace tensor too small")
@@ -388,6 +399,19 @@ class Context:
             if finish:
                 self._check(self.L.gq_hash_build_finish(self.h, table.handle))
         return table
+
+    def profile(self, enable=True):
+        """gq_profile: bracket every kernel launch of this context with CUDA events (off in timed loops)."""
+        self._check(self.L.gq_profile(self.h, 1 if enable else 0))
+
+    def profile_read(self, max_entries=256):
+        """-> [(kernel name, ms)] recorded since the last read; waits for the stream."""
+        names = C.create_string_buffer(64 * max_entries)
+        ms = (C.c_float * max_entries)()
+        n = self.L.gq_profile_read(self.h, names, len(names), ms, max_entries)
+        if n < 0:
+            raise GqError(5, "gq_profile_read")
+        return list(zip(names.value.decode().split("\n")[:n], [float(ms[i]) for i in range(n)]))
 
     def table_count(self, table) -> torch.Tensor:
         out = torch.zeros(1, dtype=torch.int64, device=self.device)
@@ -542,10 +566,10 @@ def precompile_materialise(col_dtypes, nrows, preds=(), probes=(), exprs=()):
     return buf.value.decode()
 
 
-def precompile_build(col_dtypes, nrows, preds=(), probes=(), key=0, payload=(), unique=False):
+def precompile_build(col_dtypes, nrows, preds=(), probes=(), key=0, payload=(), unique=False, dense_range=None):
     m = _M()
     b = m.batch([None] * len(col_dtypes), dtypes=list(col_dtypes), nrows=int(nrows))
-    d = m.build_desc(preds, probes, key, payload, unique)
+    d = m.build_desc(preds, probes, key, payload, unique, dense_range)
     buf = C.create_string_buffer(8192)
     st = lib().gq_precompile_build(C.byref(b), C.byref(d), buf, 8192)
     if st:

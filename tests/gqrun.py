@@ -21,7 +21,7 @@ def build_tables(ctx, plan, device_tables=None, workspaces=None):
         probes = [(tables[bi], kc) for bi, kc in b.get("probes", [])]
         tables.append(ctx.hash_build(cols, preds=b.get("preds", []), probes=probes, key=b["key"],
                                      payload=b.get("payload", []), unique=b.get("unique", False),
-                                     max_rows=b.get("max_rows"), workspace=ws))
+                                     max_rows=b.get("max_rows"), workspace=ws, dense_range=b.get("dense_range")))
     return tables
 
 

@@ -86,6 +86,31 @@ def test_plan_compiler_covers_probes_of_duplicate_key_tables(gq):
     assert os.path.exists(gq.precompile_materialise([I64, I64], 1_000_000, probes=[(multi, 0)], exprs=[[col(2)], [col(1)]]))
 
 
+def test_plan_compiler_covers_direct_address_tables(gq):
+    # GQ_F_DENSE_KEYS tables (bitmap + payload rows indexed by key - key_min): build, probe in both row-code forms,
+    # direct aggregation through the matched index; the flag needs GQ_F_UNIQUE_KEYS
+    I8, I32, I64 = gq.I8, gq.I32, gq.I64
+    col = lambda i: ("col", i)
+    dense, multi = gq.describe_table([I32], unique=True, dense=True), gq.describe_table([I32], unique=False)
+    ag = [("sum", 0), ("count",)]
+    assert os.path.exists(gq.precompile_build([I64, I32], 1_000_000, preds=[(1, "lt", 5)], key=0, payload=[1], unique=True,
+                                              dense_range=(1, 1_000_000)))
+    assert os.path.exists(gq.precompile_build([I64, I64, I32], 1_000_000, probes=[(multi, 0)], key=1, payload=[2], unique=True,
+                                              dense_range=(-5, 5)))
+    for kw in (dict(keys=[], max_groups=1), dict(keys=[1], max_groups=6), dict(keys=[0], max_groups=100_000),
+               dict(keys=[0, 3], ndependent=1, max_groups=100_000)):
+        assert os.path.exists(gq.precompile_pipeline([I64, I8, I64], 1_000_000, probes=[(dense, 0)], exprs=[[col(2)]], aggs=ag, **kw))
+    assert os.path.exists(gq.precompile_pipeline([I64, I64, I64], 1_000_000, probes=[(multi, 0), (dense, 1)], exprs=[[col(2)]],
+                                                 keys=[1], aggs=ag, max_groups=100_000))
+    assert os.path.exists(gq.precompile_materialise([I64, I64], 1_000_000, probes=[(dense, 0)], exprs=[[col(2)], [col(1)]]))
+    with pytest.raises(gq.GqError):
+        gq.precompile_build([I64], 100, key=0, unique=False, dense_range=(0, 10))
+    n = C.c_size_t()
+    L = gq.lib()
+    assert L.gq_hash_build_workspace_dense(1, 15_000_000, 1, C.byref(n)) == 0 and n.value >= 15_000_000 // 8 + 15_000_000 * 8
+    assert L.gq_hash_build_workspace_dense(5, 4, 0, C.byref(n)) == 1
+
+
 def test_options(gq):
     L = gq.lib()
     assert L.gq_set_option(b"part_min_rows", 4096) == 0 and L.gq_set_option(b"part_min_rows", -1) == 0

@@ -252,6 +252,84 @@ def test_fused_pipeline_over_duplicate_key_build_large_and_chained(ctx):
     run(plan, ctx)
 
 
+# ------------------------------------------------------------------ direct-address (dense-key) join tables
+def _with_dense(plan, ranges):
+    import copy
+    q = copy.copy(plan)
+    q["builds"] = [dict(b, dense_range=r) if r is not None else b for b, r in zip(plan["builds"], ranges)]
+    return q
+
+
+@pytest.mark.parametrize("cfg", [3, 4])
+def test_direct_address_tables_config_shapes(ctx, cfg):
+    # C3 / C4 with the planner's column statistics (min/max of the build keys) declared: bitmap membership, payload rows
+    # and the direct aggregation indexed by key - key_min; the hashed route on the same plan must agree (both == oracle)
+    t = datagen.make_config(cfg, scale=0.01)
+    plan = plans.PLANS[cfg](t)
+    dense = _with_dense(plan, [(int(b["table"][b["key"]].min()), int(b["table"][b["key"]].max())) for b in plan["builds"]])
+    run(dense, ctx)
+    run(plan, ctx)
+    if cfg == 3:
+        top = dict(dense, topk=10, topk_agg=0)
+        exp, got = run(top, ctx)
+        assert got["n"] == 10
+
+
+def test_direct_address_tables_adversarial(ctx):
+    import gqrun
+    from paper_2606_24647_b200 import gq
+    rng = np.random.default_rng(51)
+    # keys around zero incl. negatives, range much wider than the rows present, probes far outside the range (wrap-around of
+    # key - key_min), payload that is the dependent group key, a ragged fact tail
+    nb, nf = 20_001, 300_007
+    bkeys = (rng.permutation(60_000)[:nb].astype(np.int64) - 30_000)
+    attr = rng.integers(-1000, 1000, nb).astype(np.int32)
+    bsel = rng.integers(0, 2, nb).astype(np.int8)
+    fk = rng.integers(-40_000, 40_000, nf).astype(np.int64)
+    fk[::97] = I64_MIN; fk[1::97] = np.iinfo(np.int64).max
+    v = rng.integers(-5000, 5000, nf).astype(np.int64)
+    b = dict(table=[bkeys, attr, bsel], preds=[(2, "eq", 1)], key=0, payload=[1], unique=True, dense_range=(-30_000, 29_999))
+    for keys, ndep, mg in (([0, 2], 1, nb), ([0], 0, nb), ([], 0, 1), ([2], 0, 2100)):
+        plan = dict(builds=[b], table=[fk, v], preds=[], probes=[(0, 0)], exprs=[[("col", 1)], [("col", 1), ("col", 2), ("mul",)]],
+                    keys=keys, ndependent=ndep, aggs=[("sum", 0), ("min", 1), ("max", 0), ("count",)], max_groups=mg)
+        exp, got = run(plan, ctx)
+        assert exp.nrows > 0
+    # materialising probe (inner join as output columns) through a dense table
+    tb = ctx.hash_build(gqrun.dev(b["table"]), preds=b["preds"], key=0, payload=[1], unique=True, dense_range=b["dense_range"])
+    assert int(ctx.table_count(tb).item()) == int((bsel == 1).sum())
+    outs, count = ctx.hash_probe(gqrun.dev([fk, v]), [], [(tb, 0)], [[("col", 0)], [("col", 2)], [("col", 1)]], capacity=nf)
+    ctx.sync()
+    n = int(count.item())
+    got = np.stack([o[:n].cpu().numpy() for o in outs], 1)
+    pairs = oracle.join_pairs([bkeys, attr, bsel], [(2, "eq", 1)], 0, [fk, v], [], 0)
+    ref = np.stack([fk[pairs.cols[0]], attr[pairs.cols[1]].astype(np.int64), v[pairs.cols[0]]], 1)
+    assert n == pairs.nrows > 0 and np.array_equal(got[np.lexsort(got.T[::-1])], ref[np.lexsort(ref.T[::-1])])
+    # streaming batches into one dense table; a multiset step in front of a dense step (one-row-at-a-time row code)
+    h = gqrun.dev(b["table"])
+    tb2 = ctx.hash_build([c[:7008] for c in h], preds=b["preds"], key=0, payload=[1], unique=True, dense_range=b["dense_range"], finish=False)
+    ctx.hash_build([c[7008:] for c in h], preds=b["preds"], key=0, payload=[1], unique=True, dense_range=b["dense_range"], table=tb2)
+    assert int(ctx.table_count(tb2).item()) == int((bsel == 1).sum())
+    mkey = rng.integers(0, 300, 5000).astype(np.int64)
+    mval = rng.integers(-30_000, 30_000, 5000).astype(np.int64)
+    f2 = rng.integers(0, 320, 50_000).astype(np.int64)
+    plan = dict(builds=[dict(table=[mkey, mval], preds=[], key=0, payload=[1], unique=False), b], table=[f2, v[:50_000]], preds=[],
+                probes=[(0, 0), (1, 2)], exprs=[[("col", 1), ("col", 3), ("add",)]], keys=[2], aggs=[("sum", 0), ("count",)], max_groups=nb)
+    run(plan, ctx)
+    # the declarations are verified on the device: a key outside the range, a repeated key
+    c2 = gq.Context()
+    c2.hash_build(gqrun.dev([bkeys]), key=0, unique=True, dense_range=(-30_000, 20_000))
+    with pytest.raises(gq.GqError) as e:
+        c2.sync()
+    assert e.value.status == 9                                  # GQ_ERR_KEY_RANGE
+    c2.clear_error(); c2.sync()
+    dup = bkeys.copy(); dup[5] = dup[9000]
+    c2.hash_build(gqrun.dev([dup]), key=0, unique=True, dense_range=(-30_000, 29_999))
+    with pytest.raises(gq.GqError) as e:
+        c2.sync()
+    assert e.value.status == 6                                  # GQ_ERR_DUPLICATE_KEY
+    c2.clear_error(); c2.sync()
+
+
 def test_check_dependent_flag_catches_a_false_declaration(ctx):
     # S17: a key declared functionally dependent is stored, not hashed. With GQ_F_CHECK_DEPENDENT a false declaration
     # is a sticky error instead of silently merged groups; a true one gives the oracle's tuple-grouped result.
