@@ -189,6 +189,18 @@ gq_status gq_hash_aggregate_finish(gq_ctx*, gq_aggstate*, void* const* out_key_c
                                    int64_t* d_out_ngroups);
 gq_status gq_aggstate_destroy(gq_aggstate*);
 
+/* ---- OrderBy / TopN (PAPER.md:138 and Fig. 2: CudfOrderBy, TopN) ----------------------------- */
+/* Sorts the rows of a batch by key columns: lexicographic with keys[0] most significant, ascending or descending per
+ * key, signed comparison, ties broken by input row position (a STABLE sort: the result is unique). Writes the first
+ * min(limit, nrows) rows (limit <= 0: all): d_out_index[i] (int64, may be NULL) = input row number of output row i, and,
+ * when out_cols != NULL, out_cols[c][i] = column c of that row with the input column's dtype (an entry may be NULL).
+ * nkeys == 0 keeps the input order. Method: LSD radix sort of (sortable key, row) pairs, one key column at a time;
+ * limit << nrows first selects the candidate rows with a two-level radix select on keys[0]. nrows <= 2^31. */
+typedef struct { int32_t col; int32_t descending; } gq_sort_key;
+gq_status gq_order_by_workspace(int64_t nrows, size_t* bytes);
+gq_status gq_order_by(gq_ctx*, const gq_batch* in, const gq_sort_key* keys, int32_t nkeys, int64_t limit, void* d_workspace,
+                      size_t bytes, int64_t* d_out_index, void* const* out_cols);
+
 /* ---- Fused pipeline: scan -> filter -> probe t1..tk -> project -> aggregate -> finalise ------- */
 typedef struct {
   const gq_batch* in; gq_agg_desc agg;

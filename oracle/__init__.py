@@ -37,6 +37,10 @@ class _Table(C.Structure):
     _fields_ = [("cols", C.POINTER(_Col)), ("ncols", C.c_int32), ("nrows", C.c_int64)]
 
 
+class _SortKey(C.Structure):
+    _fields_ = [("col", C.c_int32), ("descending", C.c_int32)]
+
+
 class _Pred(C.Structure):
     _fields_ = [("col", C.c_int32), ("op", C.c_int32), ("lo", C.c_int64), ("hi", C.c_int64)]
 
@@ -92,6 +96,8 @@ def lib():
             f.restype = C.c_void_p
             f.argtypes = [C.POINTER(_Table), C.POINTER(_Pred), C.c_int32, C.c_int32,
                           C.POINTER(_Table), C.POINTER(_Pred), C.c_int32, C.c_int32]
+        L.ocl_order_by.restype = C.c_void_p
+        L.ocl_order_by.argtypes = [C.POINTER(_Table), C.POINTER(_SortKey), C.c_int32, C.c_int64]
         L.ocl_result_nrows.restype = C.c_int64
         L.ocl_result_nrows.argtypes = [C.c_void_p]
         L.ocl_result_ncols.restype = C.c_int32
@@ -213,6 +219,16 @@ def join_pairs(build_table, bpreds, bkey, probe_table, ppreds, pkey, bruteforce=
     pp, npp = _preds(ppreds, keep)
     f = lib().ocl_join_pairs_bruteforce if bruteforce else lib().ocl_join_pairs
     return Result(f(C.byref(bt), bp, nbp, int(bkey), C.byref(pt), pp, npp, int(pkey)))
+
+
+def order_by(table, keys, limit=0) -> Result:
+    """keys = [(column, descending)]; -> Result with cols[0] = input row numbers in order, then the gathered columns."""
+    keep = _Keep()
+    t = _table(table, keep)
+    kk = (_SortKey * max(1, len(keys)))()
+    for i, (c, d) in enumerate(keys):
+        kk[i] = _SortKey(int(c), 1 if d else 0)
+    return Result(lib().ocl_order_by(C.byref(t), kk, len(keys), int(limit)))
 
 
 def avg(s: int, c: int) -> float:

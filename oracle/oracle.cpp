@@ -289,6 +289,30 @@ ocl_result* ocl_join_pairs_bruteforce(const ocl_table* build, const ocl_pred* bp
   return pairs_result(pairs);
 }
 
+ocl_result* ocl_order_by(const ocl_table* in, const ocl_sort_key* keys, int32_t nkeys, int64_t limit) {
+  if (!in || nkeys < 0 || (nkeys > 0 && !keys)) return nullptr;
+  for (int32_t k = 0; k < nkeys; ++k) if (keys[k].col < 0 || keys[k].col >= in->ncols) return nullptr;
+  std::vector<int64_t> order((size_t)in->nrows);
+  for (int64_t r = 0; r < in->nrows; ++r) order[(size_t)r] = r;
+  std::stable_sort(order.begin(), order.end(), [&](int64_t a, int64_t b) {
+    for (int32_t k = 0; k < nkeys; ++k) {
+      const int64_t x = cell(in->cols[keys[k].col], a), y = cell(in->cols[keys[k].col], b);
+      if (x != y) return keys[k].descending ? x > y : x < y;
+    }
+    return false;                                          // equal key tuples: stable_sort keeps input order
+  });
+  const int64_t n = (limit <= 0 || limit > in->nrows) ? in->nrows : limit;
+  ocl_result* res = new ocl_result();
+  res->nrows = n;
+  res->input_rows = in->nrows;
+  res->cols.assign((size_t)in->ncols + 1, std::vector<int64_t>((size_t)n));
+  for (int64_t i = 0; i < n; ++i) {
+    res->cols[0][(size_t)i] = order[(size_t)i];
+    for (int32_t c = 0; c < in->ncols; ++c) res->cols[(size_t)c + 1][(size_t)i] = cell(in->cols[c], order[(size_t)i]);
+  }
+  return res;
+}
+
 int64_t ocl_result_nrows(const ocl_result* r) { return r->nrows; }
 int32_t ocl_result_ncols(const ocl_result* r) { return (int32_t)r->cols.size(); }
 const int64_t* ocl_result_col(const ocl_result* r, int32_t c) { return r->cols[(size_t)c].data(); }

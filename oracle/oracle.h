@@ -57,6 +57,13 @@ ocl_result* ocl_join_pairs(const ocl_table* build, const ocl_pred* bpreds, int32
 ocl_result* ocl_join_pairs_bruteforce(const ocl_table* build, const ocl_pred* bpreds, int32_t nbpred, int32_t bkey,
                                       const ocl_table* probe, const ocl_pred* ppreds, int32_t nppred, int32_t pkey);
 
+/* ORDER BY ... LIMIT (PAPER.md:138 OrderBy / TopN): the definition written out — rows compared
+ * lexicographically over the key columns (keys[0] first; signed values; descending keys compare reversed), ties keep
+ * input order (std::stable_sort). Result: column 0 = input row numbers of the first min(limit, nrows) rows in order
+ * (limit <= 0: all rows), then every input column gathered in that order (widened to int64). */
+typedef struct { int32_t col; int32_t descending; } ocl_sort_key;
+ocl_result* ocl_order_by(const ocl_table* in, const ocl_sort_key* keys, int32_t nkeys, int64_t limit);
+
 int64_t ocl_result_nrows(const ocl_result*);              /* groups / output rows / pairs */
 int32_t ocl_result_ncols(const ocl_result*);              /* keys then aggregates (query); exprs; 2 (pairs) */
 const int64_t* ocl_result_col(const ocl_result*, int32_t c);

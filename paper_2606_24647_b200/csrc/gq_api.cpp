@@ -1174,6 +1174,34 @@ gq_status gq_read_probe(gq_ctx* ctx, const void* d_data, size_t bytes, uint64_t*
   return GQ_OK;
 }
 
+// ------------------------------------------------------------------------------------------------ OrderBy / TopN
+gq_status gq_order_by_workspace(int64_t nrows, size_t* bytes) {
+  if (!bytes || nrows < 0 || nrows > (1LL << 31)) return GQ_ERR_INVALID_ARG;
+  *bytes = gq_sort_workspace_bytes(nrows);
+  return GQ_OK;
+}
+
+gq_status gq_order_by(gq_ctx* ctx, const gq_batch* in, const gq_sort_key* keys, int32_t nkeys, int64_t limit, void* d_ws, size_t bytes,
+                      int64_t* d_out_index, void* const* out_cols) {
+  if (!ctx) return GQ_ERR_INVALID_ARG;
+  gq_status st = check_batch(ctx, in);
+  if (st != GQ_OK) return st;
+  if (in->nrows > (1LL << 31)) return fail(ctx, GQ_ERR_UNSUPPORTED, "gq_order_by: more than 2^31 rows");
+  if (nkeys < 0 || nkeys > GQ_MAX_COLS || (nkeys > 0 && !keys)) return fail(ctx, GQ_ERR_INVALID_ARG, "bad sort keys");
+  for (int k = 0; k < nkeys; ++k)
+    if (keys[k].col < 0 || keys[k].col >= in->ncols) return fail(ctx, GQ_ERR_INVALID_ARG, "sort key column out of range");
+  if (!d_out_index && !out_cols) return fail(ctx, GQ_ERR_INVALID_ARG, "no outputs");
+  if (!d_ws || !aligned(d_ws, 256)) return fail(ctx, GQ_ERR_INVALID_ARG, "bad workspace");
+  if (bytes < gq_sort_workspace_bytes(in->nrows)) return fail(ctx, GQ_ERR_WORKSPACE_TOO_SMALL, "order-by workspace too small");
+  if (in->nrows == 0) return GQ_OK;
+  int nl = 0;
+  cudaError_t e = PROF(ctx, "gq_order_by", gq_launch_order_by(ctx->stream, ctx->num_sms, in, keys, nkeys, limit, (char*)d_ws,
+                                                               (long long*)d_out_index, out_cols, &nl));
+  if (e != cudaSuccess) return cuda_fail(ctx, e, "order by");
+  ctx->launches += nl;
+  return GQ_OK;
+}
+
 gq_status gq_profile(gq_ctx* ctx, int32_t enable) {
   if (!ctx) return GQ_ERR_INVALID_ARG;
   ctx->prof = enable != 0;

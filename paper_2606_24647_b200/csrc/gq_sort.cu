@@ -1,0 +1,284 @@
+// gq_sort.cu — OrderBy / TopN over a device-resident column batch (Fig. 2: the
+// plan's CudfOrderBy / TopN operators). Plan-independent sm_100a kernels, compiled by nvcc into libgq.so.
+//
+// Order: lexicographic over the key columns (keys[0] most significant), ascending or descending per key, signed
+// comparison, ties broken by input row position — i.e. a STABLE sort, so the result is unique and compared bit-exactly
+// with the oracle's std::stable_sort.
+//
+// Method: least-significant-digit radix sort of (64-bit sortable key, 32-bit row index) pairs, 8 bits per pass, one
+// key column at a time from the least significant column to the most significant (a stable sort by the more
+// significant column keeps the order the less significant ones produced). Per column: one gather builds the sortable
+// keys (sign bit flipped; all bits inverted for descending), then one pass per byte of the column's width:
+//   histogram  — a fixed grid of GQ_SORT_BLOCKS CTAs, each owning a contiguous range of tiles, counts its digits;
+//   scan       — one CTA turns the [digit][CTA] counts into exclusive offsets (digit-major: stable across CTAs);
+//   scatter    — every CTA walks its range again in order; inside a tile ranks are stable: the warp's lanes with equal
+//                digits are found with MATCH.ANY, warps are ordered through per-warp digit counts in shared memory.
+// TopN (limit << rows): two histogram levels over the top 24 bits of the most significant key select a threshold
+// bucket on the device; only rows at or before it (>= limit of them, more only with ties) are compacted and sorted.
+// Everything is stream-ordered; the number of candidate rows stays in device memory (no host synchronisation).
+#include <algorithm>
+
+#include "gq_internal.h"
+
+typedef unsigned long long u64;
+typedef long long i64;
+typedef unsigned int u32;
+
+#define GQ_SORT_THREADS 256
+#define GQ_SORT_ITEMS 8
+#define GQ_SORT_TILE (GQ_SORT_THREADS * GQ_SORT_ITEMS)
+#define GQ_SORT_WARPS (GQ_SORT_THREADS / 32)
+#define GQ_SEL_BINS 4096
+
+// Sortable image of a signed column value of `bytes` bytes: unsigned order == requested order.
+__device__ __forceinline__ u64 gq_sort_image(i64 v, int bytes, int desc) {
+  const int bits = 8 * bytes;
+  u64 u = (u64)v ^ (1ULL << (bits - 1));
+  if (bits < 64) u &= (1ULL << bits) - 1;
+  if (desc) u = bits < 64 ? (~u & ((1ULL << bits) - 1)) : ~u;
+  return u;
+}
+__device__ __forceinline__ i64 gq_sort_load(const void* col, int dtype, i64 r) {
+  return dtype == GQ_I8 ? (i64)((const signed char*)col)[r] : dtype == GQ_I32 ? (i64)((const int*)col)[r] : ((const i64*)col)[r];
+}
+__device__ __forceinline__ u32 gq_sort_n(const u32* d_n) { return *(volatile const u32*)d_n; }
+
+// range of tiles owned by a CTA: contiguous, whole tiles
+__device__ __forceinline__ void gq_sort_range(u32 n, u32* lo, u32* hi) {
+  const u32 ntiles = (n + GQ_SORT_TILE - 1) / GQ_SORT_TILE;
+  const u32 per = (ntiles + gridDim.x - 1) / gridDim.x;
+  const u64 a = (u64)blockIdx.x * per * GQ_SORT_TILE, b = a + (u64)per * GQ_SORT_TILE;
+  *lo = (u32)(a < n ? a : n);
+  *hi = (u32)(b < n ? b : n);
+}
+
+__global__ void gq_k_sort_iota(u32* idx, u32 n, u32* d_n) {
+  for (u32 i = blockIdx.x * blockDim.x + threadIdx.x; i < n; i += gridDim.x * blockDim.x) idx[i] = i;
+  if (blockIdx.x == 0 && threadIdx.x == 0) *d_n = n;
+}
+
+__global__ void gq_k_sort_keys(const void* col, int dtype, int bytes, int desc, const u32* idx, const u32* d_n, u64* keys) {
+  const u32 n = gq_sort_n(d_n);
+  for (u32 i = blockIdx.x * blockDim.x + threadIdx.x; i < n; i += gridDim.x * blockDim.x)
+    keys[i] = col ? gq_sort_image(gq_sort_load(col, dtype, (i64)idx[i]), bytes, desc) : (u64)idx[i];   // col == null: the row index itself
+}
+
+__global__ void __launch_bounds__(GQ_SORT_THREADS) gq_k_sort_hist(const u64* keys, const u32* d_n, int shift, u32* hist) {
+  __shared__ u32 h[256];
+  h[threadIdx.x] = 0;
+  __syncthreads();
+  u32 lo, hi;
+  gq_sort_range(gq_sort_n(d_n), &lo, &hi);
+  for (u32 i = lo + threadIdx.x; i < hi; i += GQ_SORT_THREADS) atomicAdd(&h[(keys[i] >> shift) & 255], 1u);
+  __syncthreads();
+  hist[threadIdx.x * gridDim.x + blockIdx.x] = h[threadIdx.x];      // [digit][CTA]
+}
+
+// exclusive scan of hist in [digit][CTA] order, in place; one CTA of 1024 threads
+__global__ void __launch_bounds__(1024) gq_k_sort_scan(u32* hist, int total) {
+  __shared__ u32 part[1024];
+  const int t = threadIdx.x;
+  const int per = (total + 1023) / 1024;
+  const int lo = t * per, hi = min(total, lo + per);
+  u32 s = 0;
+  for (int i = lo; i < hi; ++i) s += hist[i];
+  part[t] = s;
+  __syncthreads();
+  for (int o = 1; o < 1024; o <<= 1) {
+    const u32 v = t >= o ? part[t - o] : 0;
+    __syncthreads();
+    part[t] += v;
+    __syncthreads();
+  }
+  u32 run = part[t] - s;
+  for (int i = lo; i < hi; ++i) { const u32 c = hist[i]; hist[i] = run; run += c; }
+}
+
+__global__ void __launch_bounds__(GQ_SORT_THREADS) gq_k_sort_scatter(const u64* kin, const u32* iin, u64* kout, u32* iout, const u32* d_n,
+                                                                    int shift, const u32* hist) {
+  __shared__ u32 binoff[256];                       // next output position of every digit for this CTA
+  __shared__ u32 wcnt[GQ_SORT_WARPS][256];          // per round: items of a digit in every warp (only touched entries are used)
+  const int t = threadIdx.x, lane = t & 31, warp = t >> 5;
+  binoff[t] = hist[t * gridDim.x + blockIdx.x];
+  for (int w = 0; w < GQ_SORT_WARPS; ++w) wcnt[w][t] = 0;
+  __syncthreads();
+  u32 lo, hi;
+  gq_sort_range(gq_sort_n(d_n), &lo, &hi);
+  for (u32 base = lo; base < hi; base += GQ_SORT_THREADS) {          // one round = 256 consecutive items, in order
+    const u32 i = base + t;
+    const bool have = i < hi;
+    const u64 k = have ? kin[i] : 0;
+    const u32 ix = have ? iin[i] : 0;
+    const u32 d = (u32)(k >> shift) & 255u;
+    const u32 peers = __match_any_sync(0xffffffffu, have ? d : 256u + (u32)lane);   // lanes of this warp with my digit
+    const u32 rank = __popc(peers & ((1u << lane) - 1u));
+    const bool leader = have && rank == 0;
+    if (leader) wcnt[warp][d] = __popc(peers);
+    __syncthreads();
+    u32 before = 0, total = 0;
+    if (have) {
+#pragma unroll
+      for (int w = 0; w < GQ_SORT_WARPS; ++w) { const u32 c = wcnt[w][d]; if (w < warp) before += c; total += c; }
+    }
+    const u32 pos = binoff[d] + before + rank;
+    __syncthreads();                                                 // every thread has read binoff / wcnt of this round
+    if (have) { kout[pos] = k; iout[pos] = ix; }
+    if (leader) {
+      wcnt[warp][d] = 0;
+      if (before == 0) binoff[d] += total;                           // exactly one leader per digit: the first warp holding it
+    }
+    __syncthreads();
+  }
+}
+
+// ---- TopN candidate selection on the most significant key ----
+struct GqSelParams {
+  const void* col; int dtype, bytes, desc; u32 n; u64 limit;
+  u32* hist1; u32* hist2; u32* ctl;   // ctl[0] = threshold bucket level 1, ctl[1] = level 2, ctl[2] = candidates (cursor)
+};
+__device__ __forceinline__ u64 gq_sel_top(const GqSelParams& P, u32 r) {   // sortable image left-aligned in 64 bits
+  return gq_sort_image(gq_sort_load(P.col, P.dtype, (i64)r), P.bytes, P.desc) << (64 - 8 * P.bytes);
+}
+__global__ void __launch_bounds__(256) gq_k_sel_hist(const __grid_constant__ GqSelParams P, int level) {
+  __shared__ u32 h[GQ_SEL_BINS];
+  for (int i = threadIdx.x; i < GQ_SEL_BINS; i += 256) h[i] = 0;
+  __syncthreads();
+  const u32 t1 = level == 2 ? P.ctl[0] : 0;
+  for (u32 r = blockIdx.x * 256 + threadIdx.x; r < P.n; r += gridDim.x * 256) {
+    const u64 u = gq_sel_top(P, r);
+    if (level == 1) atomicAdd(&h[u >> 52], 1u);
+    else if ((u32)(u >> 52) == t1) atomicAdd(&h[(u >> 40) & (GQ_SEL_BINS - 1)], 1u);
+  }
+  __syncthreads();
+  u32* g = level == 1 ? P.hist1 : P.hist2;
+  for (int i = threadIdx.x; i < GQ_SEL_BINS; i += 256) if (h[i]) atomicAdd(&g[i], h[i]);
+}
+// one thread walks the 4096 counts (a few microseconds): threshold = first bucket at which the running count reaches the limit
+__global__ void gq_k_sel_pick(const __grid_constant__ GqSelParams P, int level) {
+  if (threadIdx.x != 0 || blockIdx.x != 0) return;
+  const u32* h = level == 1 ? P.hist1 : P.hist2;
+  u64 need = P.limit;
+  if (level == 2) { u64 below = 0; for (u32 b = 0; b < P.ctl[0]; ++b) below += P.hist1[b]; need = P.limit > below ? P.limit - below : 1; }
+  u64 run = 0;
+  u32 b = 0;
+  for (; b < GQ_SEL_BINS - 1; ++b) { run += h[b]; if (run >= need) break; }
+  P.ctl[level - 1] = b;
+}
+__global__ void __launch_bounds__(256) gq_k_sel_compact(const __grid_constant__ GqSelParams P, u32* idx) {
+  const u32 t1 = P.ctl[0], t2 = P.ctl[1];
+  for (u32 r0 = blockIdx.x * 256; r0 < P.n; r0 += gridDim.x * 256) {
+    const u32 r = r0 + threadIdx.x;
+    bool take = false;
+    if (r < P.n) {
+      const u64 u = gq_sel_top(P, r);
+      const u32 b1 = (u32)(u >> 52), b2 = (u32)(u >> 40) & (GQ_SEL_BINS - 1);
+      take = b1 < t1 || (b1 == t1 && b2 <= t2);
+    }
+    const u32 m = __ballot_sync(0xffffffffu, take);
+    u32 base = 0;
+    if ((threadIdx.x & 31) == 0 && m) base = atomicAdd(&P.ctl[2], (u32)__popc(m));
+    base = __shfl_sync(0xffffffffu, base, 0);
+    if (take) idx[base + __popc(m & ((1u << (threadIdx.x & 31)) - 1u))] = r;   // any order: the rows are sorted by index first
+  }
+}
+
+struct GqEmitParams {
+  const u32* idx; const u32* d_n; u64 limit; i64* out_index;
+  int ncols; const void* col[GQ_MAX_COLS]; void* out[GQ_MAX_COLS]; int dtype[GQ_MAX_COLS];
+};
+__global__ void gq_k_sort_emit(const __grid_constant__ GqEmitParams P) {
+  const u64 n = min((u64)gq_sort_n(P.d_n), P.limit);
+  for (u64 i = blockIdx.x * (u64)blockDim.x + threadIdx.x; i < n; i += (u64)gridDim.x * blockDim.x) {
+    const i64 r = (i64)P.idx[i];
+    if (P.out_index) P.out_index[i] = r;
+    for (int c = 0; c < P.ncols; ++c) {
+      if (!P.out[c]) continue;
+      if (P.dtype[c] == GQ_I8) ((signed char*)P.out[c])[i] = ((const signed char*)P.col[c])[r];
+      else if (P.dtype[c] == GQ_I32) ((int*)P.out[c])[i] = ((const int*)P.col[c])[r];
+      else ((i64*)P.out[c])[i] = ((const i64*)P.col[c])[r];
+    }
+  }
+}
+
+// ---- host side ----
+struct GqSortLayout { size_t keys[2], idx[2], hist, sel1, sel2, ctl, total; int nblk; };
+static GqSortLayout gq_sort_layout(i64 nrows, int num_sms) {
+  GqSortLayout L;
+  auto al = [](size_t v) { return (v + 255) / 256 * 256; };
+  L.nblk = std::max(1, std::min(num_sms * 4, 1024));
+  size_t off = 0;
+  const size_t n = (size_t)std::max<i64>(1, nrows);
+  for (int b = 0; b < 2; ++b) { L.keys[b] = off; off += al(n * 8); }
+  for (int b = 0; b < 2; ++b) { L.idx[b] = off; off += al(n * 4); }
+  L.hist = off; off += al((size_t)256 * 1024 * 4);
+  L.sel1 = off; off += al(GQ_SEL_BINS * 4);
+  L.sel2 = off; off += al(GQ_SEL_BINS * 4);
+  L.ctl = off; off += 256;
+  L.total = off;
+  return L;
+}
+size_t gq_sort_workspace_bytes(i64 nrows) { return gq_sort_layout(nrows, GQ_MAX_SMS).total; }
+
+cudaError_t gq_launch_order_by(cudaStream_t s, int num_sms, const gq_batch* in, const gq_sort_key* keys, int nkeys, i64 limit, char* ws,
+                               i64* out_index, void* const* out_cols, int* nlaunches) {
+  const GqSortLayout L = gq_sort_layout(in->nrows, GQ_MAX_SMS);
+  const int nblk = std::max(1, std::min(num_sms * 4, 1024));
+  const u32 n = (u32)in->nrows;
+  const u64 lim = limit <= 0 || limit > in->nrows ? (u64)in->nrows : (u64)limit;
+  u64* kbuf[2] = {(u64*)(ws + L.keys[0]), (u64*)(ws + L.keys[1])};
+  u32* ibuf[2] = {(u32*)(ws + L.idx[0]), (u32*)(ws + L.idx[1])};
+  u32* hist = (u32*)(ws + L.hist);
+  u32* ctl = (u32*)(ws + L.ctl);
+  u32* d_n = ctl + 8;
+  int nl = 0, cur = 0;
+  const int gs = std::max(1, std::min<int>(num_sms * 8, (int)((n + 255) / 256)));
+  auto dtype_bytes = [](int t) { return t == GQ_I8 ? 1 : t == GQ_I32 ? 4 : 8; };
+  auto passes = [&](int bytes) {                     // LSD passes over the low `bytes` bytes of kbuf[cur]
+    for (int b = 0; b < bytes; ++b) {
+      gq_k_sort_hist<<<nblk, GQ_SORT_THREADS, 0, s>>>(kbuf[cur], d_n, 8 * b, hist);
+      gq_k_sort_scan<<<1, 1024, 0, s>>>(hist, 256 * nblk);
+      gq_k_sort_scatter<<<nblk, GQ_SORT_THREADS, 0, s>>>(kbuf[cur], ibuf[cur], kbuf[cur ^ 1], ibuf[cur ^ 1], d_n, 8 * b, hist);
+      cur ^= 1;
+      nl += 3;
+    }
+  };
+  cudaError_t e = cudaSuccess;
+  const bool topn = nkeys > 0 && lim * 8 < (u64)n && n >= (1u << 16);
+  if (topn) {
+    e = cudaMemsetAsync(ws + L.sel1, 0, L.total - L.sel1, s);   // both histograms and the control words
+    if (e != cudaSuccess) return e;
+    GqSelParams sp;
+    const gq_column& c0 = in->cols[keys[0].col];
+    sp.col = c0.data; sp.dtype = (int)c0.dtype; sp.bytes = dtype_bytes((int)c0.dtype); sp.desc = keys[0].descending ? 1 : 0;
+    sp.n = n; sp.limit = lim; sp.hist1 = (u32*)(ws + L.sel1); sp.hist2 = (u32*)(ws + L.sel2); sp.ctl = ctl;
+    for (int level = 1; level <= 2; ++level) {
+      gq_k_sel_hist<<<gs, 256, 0, s>>>(sp, level);
+      gq_k_sel_pick<<<1, 32, 0, s>>>(sp, level);
+    }
+    gq_k_sel_compact<<<gs, 256, 0, s>>>(sp, ibuf[0]);
+    nl += 5;
+    e = cudaMemcpyAsync(d_n, ctl + 2, 4, cudaMemcpyDeviceToDevice, s);
+    if (e != cudaSuccess) return e;
+    // candidates were appended in any order: sort them by row index first (the least significant "key" of a stable sort)
+    gq_k_sort_keys<<<gs, 256, 0, s>>>(nullptr, 0, 4, 0, ibuf[0], d_n, kbuf[0]);
+    ++nl;
+    passes(4);
+  } else {
+    gq_k_sort_iota<<<gs, 256, 0, s>>>(ibuf[0], n, d_n);
+    ++nl;
+  }
+  for (int k = nkeys - 1; k >= 0; --k) {
+    const gq_column& c = in->cols[keys[k].col];
+    gq_k_sort_keys<<<gs, 256, 0, s>>>(c.data, (int)c.dtype, dtype_bytes((int)c.dtype), keys[k].descending ? 1 : 0, ibuf[cur], d_n, kbuf[cur]);
+    ++nl;
+    passes(dtype_bytes((int)c.dtype));
+  }
+  GqEmitParams ep;
+  ep.idx = ibuf[cur]; ep.d_n = d_n; ep.limit = lim; ep.out_index = out_index; ep.ncols = in->ncols;
+  for (int c = 0; c < in->ncols; ++c) { ep.col[c] = in->cols[c].data; ep.out[c] = out_cols ? out_cols[c] : nullptr; ep.dtype[c] = (int)in->cols[c].dtype; }
+  const int ge = std::max(1, std::min<int>(num_sms * 8, (int)((lim + 255) / 256)));
+  gq_k_sort_emit<<<ge, 256, 0, s>>>(ep);
+  ++nl;
+  *nlaunches = nl;
+  return cudaGetLastError();
+}

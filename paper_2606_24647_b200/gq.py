@@ -39,7 +39,7 @@ SYMBOLS = ["gq_create", "gq_destroy", "gq_sync", "gq_clear_error", "gq_status_st
            "gq_hash_aggregate_workspace", "gq_hash_aggregate_workspace_for", "gq_hash_aggregate", "gq_topk_scratch_bytes", "gq_hash_aggregate_finish",
            "gq_aggstate_destroy", "gq_pipeline_workspace", "gq_pipeline", "gq_pipeline_host_workspace",
            "gq_pipeline_host", "gq_set_kernel_cache_dir", "gq_precompile_pipeline", "gq_precompile_build", "gq_precompile_materialise",
-           "gq_table_describe", "gq_read_probe", "gq_set_option", "gq_hash_build_workspace_dense", "gq_profile", "gq_profile_read"]
+           "gq_table_describe", "gq_read_probe", "gq_set_option", "gq_hash_build_workspace_dense", "gq_profile", "gq_profile_read", "gq_order_by_workspace", "gq_order_by"]
 
 
 class GqError(RuntimeError):
@@ -70,6 +70,10 @@ class _Expr(C.Structure):
 
 class _Agg(C.Structure):
     _fields_ = [("op", C.c_int), ("expr", C.c_int32)]
+
+
+class _SortKey(C.Structure):
+    _fields_ = [("col", C.c_int32), ("descending", C.c_int32)]
 
 
 class _Probe(C.Structure):
@@ -149,6 +153,9 @@ def lib():
         L.gq_table_describe.argtypes = [C.POINTER(C.c_void_p), C.POINTER(C.c_int), C.c_int32, C.c_uint32]
         L.gq_read_probe.argtypes = [C.c_void_p, C.c_void_p, C.c_size_t, C.c_void_p]
         L.gq_set_option.argtypes = [C.c_char_p, C.c_int64]
+        L.gq_order_by_workspace.argtypes = [C.c_int64, C.POINTER(C.c_size_t)]
+        L.gq_order_by.argtypes = [C.c_void_p, C.POINTER(_Batch), C.POINTER(_SortKey), C.c_int32, C.c_int64, C.c_void_p, C.c_size_t,
+                                  C.c_void_p, C.POINTER(C.c_void_p)]
         L.gq_profile.argtypes = [C.c_void_p, C.c_int32]
         L.gq_profile_read.argtypes = [C.c_void_p, C.c_char_p, C.c_size_t, C.POINTER(C.c_float), C.c_int32]
         L.gq_profile_read.restype = C.c_int32
@@ -399,6 +406,28 @@ class Context:
             if finish:
                 self._check(self.L.gq_hash_build_finish(self.h, table.handle))
         return table
+
+    # ---- OrderBy / TopN ----
+    def order_by(self, cols, keys, limit=0, gather=True, workspace=None):
+        """keys = [(column, descending)]. -> (index int64[n_out], [gathered columns] or None); n_out = min(limit, nrows)."""
+        with torch.cuda.stream(self.stream):
+            m = _M()
+            b = m.batch(cols)
+            n = int(b.nrows)
+            nout = n if limit <= 0 or limit > n else int(limit)
+            kk = (_SortKey * max(1, len(keys)))()
+            for i, (c, d) in enumerate(keys):
+                kk[i] = _SortKey(int(c), 1 if d else 0)
+            m.keep.append(kk)
+            nbytes = C.c_size_t()
+            self._check(self.L.gq_order_by_workspace(n, C.byref(nbytes)))
+            ws = workspace if workspace is not None else self._ws(nbytes.value)
+            index = self._empty(nout, torch.int64)
+            outs = [self._empty(nout, c.dtype) for c in cols] if gather else None
+            self._check(self.L.gq_order_by(self.h, C.byref(b), kk, len(keys), int(limit), self._ws_ptr(ws), nbytes.value,
+                                           index.data_ptr(), m.ptrs(outs) if gather else None))
+            self._last_ws = ws
+        return index[:nout], ([o[:nout] for o in outs] if gather else None)
 
     def profile(self, enable=True):
         """gq_profile: bracket every kernel launch of this context with CUDA events (off in timed loops)."""

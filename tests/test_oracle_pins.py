@@ -288,3 +288,40 @@ def test_no_overflow_in_configs():
     for cfg, sc in [(1, 0.05), (3, 0.001), (5, 0.0001)]:
         t = datagen.make_config(cfg, scale=sc)
         assert not oracle.run_query(plans.PLANS[cfg](t)).overflow
+
+
+# ------------------------------------------------------------------ ORDER BY / LIMIT
+def test_T8_order_by_worked_example_with_ties():
+    t = table(G["T8"]["cols"], G["T8"]["rows"])
+    cols = [t["a"], t["b"]]
+    r = oracle.order_by(cols, [tuple(k) for k in G["T8"]["keys"]])
+    assert list(r.cols[0]) == G["T8"]["expect_index"] and list(r.cols[1]) == G["T8"]["expect_a"] and list(r.cols[2]) == G["T8"]["expect_b"]
+    assert list(oracle.order_by(cols, [tuple(k) for k in G["T8"]["keys"]], limit=4).cols[0]) == G["T8"]["expect_index_limit4"]
+    assert list(oracle.order_by(cols, [tuple(k) for k in G["T8"]["keys_b_desc_only"]]).cols[0]) == G["T8"]["expect_index_b_desc"]
+    assert list(oracle.order_by(cols, []).cols[0]) == list(range(6))                # no keys: input order
+
+
+def test_order_by_equals_numpy_lexsort():
+    # an independent library routine: np.lexsort is stable and sorts by the LAST key first; a descending signed key is
+    # its bitwise complement (-x - 1: order reversed, no overflow at INT64_MIN)
+    rng = np.random.default_rng(81)
+    n = 20_000
+    a = rng.integers(-4, 4, n).astype(np.int8)
+    b = rng.integers(-50, 50, n).astype(np.int32)
+    c = rng.integers(-2**62, 2**62, n).astype(np.int64)
+    c[::7] = c[0]; c[5] = np.iinfo(np.int64).min; c[6] = np.iinfo(np.int64).max
+    for keys in ([(0, False)], [(0, True), (1, False)], [(2, True)], [(1, True), (0, True), (2, False)]):
+        r = oracle.order_by([a, b, c], keys)
+        cols = [a, b, c]
+        lex = [np.arange(n)] + [(~cols[k].astype(np.int64) if d else cols[k].astype(np.int64)) for k, d in reversed(keys)]
+        want = np.lexsort(tuple(lex))
+        assert np.array_equal(r.cols[0], want)
+        for j in range(3):
+            assert np.array_equal(r.cols[1 + j], cols[j][want].astype(np.int64))
+        lim = oracle.order_by([a, b, c], keys, limit=137)
+        assert lim.nrows == 137 and np.array_equal(lim.cols[0], want[:137])
+    # invariants: a permutation; adjacent rows are in order
+    r = oracle.order_by([a, b, c], [(1, False), (2, True)])
+    assert np.array_equal(np.sort(r.cols[0]), np.arange(n))
+    kb, kc = r.cols[2], r.cols[3]
+    assert np.all((kb[:-1] < kb[1:]) | ((kb[:-1] == kb[1:]) & (kc[:-1] >= kc[1:])))
