@@ -78,6 +78,12 @@ enum {
   GQ_F_CHECK_DEPENDENT = 1u << 1,  /* gq_agg_desc: debug check of `ndependent`: every row compares its
                                       dependent key with the one stored for its group; a mismatch sets the sticky
                                       GQ_ERR_DEPENDENT_KEY instead of silently merging two groups */
+  GQ_F_FINAL_MODE = 1u << 3,       /* gq_agg_desc: aggregation mode Final ("aggregation modes"): the input rows
+                                      are INTERMEDIATE results — the output rows of earlier (Partial) aggregations over the
+                                      same keys and aggregates, e.g. gathered from several streams or workers. SUM / MIN /
+                                      MAX combine the partial values; a GQ_COUNT_STAR aggregate names through `expr` the
+                                      expression that holds the partial counts and SUMS them. Mode Partial needs no flag:
+                                      its output (without derived AVG columns) is the intermediate form */
   GQ_F_DENSE_KEYS = 1u << 2        /* gq_build_desc: the planner knows (column min/max statistics) that every build key
                                       lies in [key_min, key_max] and the range is not much larger than the row count:
                                       the table becomes a DIRECT-ADDRESS table — a membership bitmap plus a payload
@@ -161,7 +167,7 @@ typedef struct {
   const gq_agg* aggs; int32_t naggs;
   int64_t max_groups;  /* capacity bound (exceeding it => GQ_ERR_CAPACITY); <= 64 selects the low-cardinality path
                           (per-thread cells in shared memory) */
-  uint32_t flags;      /* GQ_F_CHECK_DEPENDENT */
+  uint32_t flags;      /* GQ_F_CHECK_DEPENDENT, GQ_F_FINAL_MODE */
 } gq_agg_desc;
 gq_status gq_hash_aggregate_workspace(int64_t max_groups, int32_t nkeys, int32_t naggs, size_t* bytes);
 /* Plan-aware size: at least the size above; larger when the plan qualifies for DIRECT aggregation — the single hashed
@@ -188,6 +194,18 @@ gq_status gq_hash_aggregate_finish(gq_ctx*, gq_aggstate*, void* const* out_key_c
                                    int64_t out_capacity, int32_t topk, int32_t topk_agg, void* d_topk_scratch,
                                    int64_t* d_out_ngroups);
 gq_status gq_aggstate_destroy(gq_aggstate*);
+/* Partial -> Final between two live states (e.g. one per stream, Fig. 3): folds every group of `src` into `dst`
+ * (same keys and aggregates; direct-aggregation states must share their join table). `src` is left unchanged. Enqueued
+ * on ctx's stream: the caller orders it after the work that filled `src` (same context, or gq_sync on the other). */
+gq_status gq_aggstate_merge(gq_ctx*, gq_aggstate* dst, const gq_aggstate* src);
+/* *d_count (DEVICE int64) = groups currently in the state (enqueued). */
+gq_status gq_aggstate_count(gq_ctx*, const gq_aggstate*, int64_t* d_count);
+/* Growth ("dynamic hash table expansion"): re-hashes a high-cardinality state into a larger table in a
+ * new workspace of gq_hash_aggregate_workspace(new_max_groups, ...) bytes; stream-ordered, no host synchronisation. The
+ * old workspace may be released once this call's work has completed. A planner needs no device round trip to decide:
+ * the groups of a state never exceed the rows fed to it, so it grows the state when that bound passes max_groups
+ * (or after reading gq_aggstate_count at a pipeline boundary). */
+gq_status gq_aggstate_rehash(gq_ctx*, gq_aggstate*, void* d_new_workspace, size_t bytes, int64_t new_max_groups);
 
 /* ---- OrderBy / TopN (PAPER.md:138 and Fig. 2: CudfOrderBy, TopN) ----------------------------- */
 /* Sorts the rows of a batch by key columns: lexicographic with keys[0] most significant, ascending or descending per

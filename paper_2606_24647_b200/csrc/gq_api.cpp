@@ -589,8 +589,10 @@ gq_status agg_spec(gq_ctx* ctx, GqScanSpec* sp, const gq_batch* in, const gq_agg
   if (bits > 64) return fail(ctx, GQ_ERR_UNSUPPORTED, "packed key wider than 64 bits: declare trailing keys dependent (ndependent)");
   sp->ndep = d->ndependent;
   sp->aggs.assign(d->aggs, d->aggs + d->naggs);
-  for (const gq_agg& a : sp->aggs) {
+  for (gq_agg& a : sp->aggs) {
     if ((int)a.op < 0 || (int)a.op > (int)GQ_COUNT_STAR) return fail(ctx, GQ_ERR_INVALID_ARG, "bad aggregate op");
+    // mode Final: the rows are intermediate results; a COUNT is the SUM of the partial counts in `expr`
+    if ((d->flags & GQ_F_FINAL_MODE) && a.op == GQ_COUNT_STAR) a.op = GQ_SUM;
     if (a.op != GQ_COUNT_STAR && (a.expr < 0 || a.expr >= d->nexpr)) return fail(ctx, GQ_ERR_INVALID_ARG, "aggregate names a missing expression");
   }
   sp->target_sw = agg_slot_words(d->ndependent, d->naggs);
@@ -602,7 +604,7 @@ gq_status agg_spec(gq_ctx* ctx, GqScanSpec* sp, const gq_batch* in, const gq_agg
   for (const GqProbeSpec& ps : sp->probes) all_unique = all_unique && ps.unique;
   sp->hot = sp->consumer == GQ_C_HIGHCARD && d->nkeys == 1 && d->ndependent == 0 && sp->key_cols[0] < in->ncols &&
             agg_has_hot_area(d->max_groups, d->nkeys) && all_unique;
-  if (d->flags & ~(uint32_t)GQ_F_CHECK_DEPENDENT) return fail(ctx, GQ_ERR_INVALID_ARG, "unknown gq_agg_desc flags");
+  if (d->flags & ~(uint32_t)(GQ_F_CHECK_DEPENDENT | GQ_F_FINAL_MODE)) return fail(ctx, GQ_ERR_INVALID_ARG, "unknown gq_agg_desc flags");
   sp->check_dep = (d->flags & GQ_F_CHECK_DEPENDENT) != 0 && d->ndependent > 0;
   return GQ_OK;
 }
@@ -908,6 +910,86 @@ gq_status gq_hash_aggregate(gq_ctx* ctx, gq_aggstate** state, void* d_ws, size_t
     return GQ_OK;
   }
   return run_scan(ctx, sp, in, d->probes, &P);
+}
+
+// ---- Partial -> Final between states, group count, growth ----
+static bool same_shape(const gq_aggstate* a, const gq_aggstate* b) {
+  if (a->nkeys != b->nkeys || a->ndep != b->ndep || a->naggs != b->naggs || a->direct != b->direct) return false;
+  for (int k = 0; k < a->nkeys; ++k) if (a->key_dtype[k] != b->key_dtype[k] || a->key_bits[k] != b->key_bits[k]) return false;
+  for (int i = 0; i < a->naggs; ++i) {
+    const bool sa = a->agg_op[i] == GQ_SUM || a->agg_op[i] == GQ_COUNT_STAR, sb = b->agg_op[i] == GQ_SUM || b->agg_op[i] == GQ_COUNT_STAR;
+    if (sa != sb || (!sa && a->agg_op[i] != b->agg_op[i])) return false;
+  }
+  return true;
+}
+static gq_status merge_into(gq_ctx* ctx, const gq_aggstate* src, unsigned long long* dslots, unsigned long long dmask,
+                            unsigned long long* dside, long long* dheader, bool check_dep) {
+  int op[GQ_MAX_AGGS];
+  for (int i = 0; i < src->naggs; ++i) op[i] = (int)src->agg_op[i];
+  cudaError_t e = src->direct
+      ? PROF(ctx, "gq_k_merge", gq_launch_merge(ctx->stream, src->dacc, src->dcap, nullptr, nullptr, dslots, 0, nullptr, nullptr, 0, 0, src->naggs, op, 0, 1,
+                                                src->daw, ctx->d_err, ctx->num_sms))
+      : PROF(ctx, "gq_k_merge", gq_launch_merge(ctx->stream, src->dev.slots, src->capacity, src->dev.side, src->dev.header, dslots, dmask, dside, dheader,
+                                                src->dev.slot_words, src->ndep, src->naggs, op, check_dep ? 1 : 0, 0, 0, ctx->d_err, ctx->num_sms));
+  if (e != cudaSuccess) return cuda_fail(ctx, e, "state merge");
+  ++ctx->launches;
+  return GQ_OK;
+}
+
+gq_status gq_aggstate_merge(gq_ctx* ctx, gq_aggstate* dst, const gq_aggstate* src) {
+  if (!ctx || !dst || !src || dst == src) return GQ_ERR_INVALID_ARG;
+  use_device(ctx);
+  if (!same_shape(dst, src)) return fail(ctx, GQ_ERR_INVALID_ARG, "states differ in keys or aggregates");
+  if (dst->direct && (dst->dtab.slots != src->dtab.slots || dst->daw != src->daw || dst->dcap != src->dcap))
+    return fail(ctx, GQ_ERR_INVALID_ARG, "direct-aggregation states over different join tables cannot be merged");
+  if (dst->direct) return merge_into(ctx, src, dst->dacc, 0, nullptr, nullptr, false);
+  return merge_into(ctx, src, dst->dev.slots, dst->dev.mask, dst->dev.side, dst->dev.header, dst->check_dep);
+}
+
+gq_status gq_aggstate_count(gq_ctx* ctx, const gq_aggstate* a, int64_t* d_count) {
+  if (!ctx || !a || !d_count) return GQ_ERR_INVALID_ARG;
+  use_device(ctx);
+  cudaError_t e = a->direct
+      ? PROF(ctx, "gq_k_count_groups", gq_launch_count_groups(ctx->stream, a->dacc, a->dcap, 0, a->dev.header, 1, a->daw, a->dtouch, (long long*)d_count, ctx->num_sms))
+      : PROF(ctx, "gq_k_count_groups", gq_launch_count_groups(ctx->stream, a->dev.slots, a->capacity, a->dev.slot_words, a->dev.header, 0, 0, 0,
+                                                               (long long*)d_count, ctx->num_sms));
+  if (e != cudaSuccess) return cuda_fail(ctx, e, "group count");
+  ++ctx->launches;
+  return GQ_OK;
+}
+
+gq_status gq_aggstate_rehash(gq_ctx* ctx, gq_aggstate* a, void* d_new_ws, size_t bytes, int64_t new_max_groups) {
+  if (!ctx || !a || !d_new_ws || !aligned(d_new_ws, 256)) return GQ_ERR_INVALID_ARG;
+  use_device(ctx);
+  if (a->direct || a->lowcard || a->nkeys == 0) return fail(ctx, GQ_ERR_UNSUPPORTED, "only hashed high-cardinality states grow");
+  if (new_max_groups <= a->max_groups) return fail(ctx, GQ_ERR_INVALID_ARG, "new_max_groups must exceed the state's");
+  const int64_t cap = agg_capacity(new_max_groups, a->nkeys);
+  const int sw = a->dev.slot_words;
+  size_t hot_off = 0;
+  if (bytes < agg_ws_bytes(cap, sw, new_max_groups, a->nkeys, &hot_off)) return fail(ctx, GQ_ERR_WORKSPACE_TOO_SMALL, "rehash workspace too small");
+  WsLayout w = ws_layout(cap, sw, 1);
+  GqTableDev nt = a->dev;
+  nt.slots = (unsigned long long*)((char*)d_new_ws + w.slots_off);
+  nt.mask = (unsigned long long)(cap - 1);
+  nt.header = (long long*)d_new_ws;
+  nt.side = (unsigned long long*)((char*)d_new_ws + w.side_off);
+  nt.shift = 64 - log2i(cap);
+  unsigned long long pat[16];
+  for (int i = 0; i < 16; ++i) pat[i] = 0;
+  pat[0] = GQ_EMPTY_KEY;
+  if (a->check_dep) pat[1] = GQ_DEP_UNSET;
+  for (int i = 0; i < a->naggs; ++i)
+    pat[1 + a->ndep + i] = a->agg_op[i] == GQ_MIN ? 0x7FFFFFFFFFFFFFFFULL : a->agg_op[i] == GQ_MAX ? 0x8000000000000000ULL : 0ULL;
+  cudaError_t e = PROF(ctx, "gq_k_init_table", gq_launch_init_table(ctx->stream, nt.slots, cap, sw, pat, nt.side, 1, nt.header, 0, ctx->num_sms));
+  if (e != cudaSuccess) return cuda_fail(ctx, e, "rehash table init");
+  ++ctx->launches;
+  gq_status st = merge_into(ctx, a, nt.slots, nt.mask, nt.side, nt.header, a->check_dep);
+  if (st != GQ_OK) return st;
+  a->dev = nt; a->capacity = cap; a->max_groups = new_max_groups;
+  a->hot = (long long*)((char*)d_new_ws + hot_off);
+  a->hot_table = (unsigned long long*)((char*)d_new_ws + hot_off + 4096);
+  a->part = nullptr; a->pcur = nullptr;   // the record buffers lived in the old workspace: later batches aggregate in one pass
+  return GQ_OK;
 }
 
 size_t gq_topk_scratch_bytes(void) { return gq_topk_scratch_bytes_impl(); }

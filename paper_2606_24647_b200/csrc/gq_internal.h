@@ -221,6 +221,11 @@ struct GqPartParams {
   int* err;
 };
 cudaError_t gq_launch_part_upsert(cudaStream_t s, const GqPartParams& p, int num_sms);
+cudaError_t gq_launch_merge(cudaStream_t s, const unsigned long long* sslots, long long scap, const unsigned long long* sside, const long long* sheader,
+                            unsigned long long* dslots, unsigned long long dmask, unsigned long long* dside, long long* dheader, int sw, int ndep,
+                            int naggs, const int* op, int check_dep, int direct, int daw, int* err, int num_sms);
+cudaError_t gq_launch_count_groups(cudaStream_t s, const unsigned long long* slots, long long cap, int sw, const long long* header, int direct, int daw,
+                                   int dtouch, long long* out, int num_sms);
 size_t gq_topk_scratch_bytes_impl();
 // gq_sort.cu
 size_t gq_sort_workspace_bytes(long long nrows);

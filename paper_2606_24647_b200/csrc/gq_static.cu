@@ -431,6 +431,102 @@ cudaError_t gq_launch_part_upsert(cudaStream_t s, const GqPartParams& p, int num
   return cudaGetLastError();
 }
 
+// ------------------------------------------------------------------------------------------------ state merge
+// Partial -> Final between two aggregation states (PAPER.md:154 aggregation modes; Fig. 3: one state per stream; SURVEY
+// §8(f) NEXT-2): every group of `src` is inserted into (or found in) `dst` with the ordinary table protocol and its
+// aggregate words are combined with RED.ADD / RED.MIN / RED.MAX. The same kernel re-hashes a state into a larger table
+// (growth: dst = a freshly initialised table). Direct states (accumulators indexed by the slots of one join table)
+// merge word by word.
+struct GqMergeParams {
+  const u64* sslots; i64 scap; const u64* sside; const i64* sheader;
+  u64* dslots; u64 dmask; u64* dside; i64* dheader;
+  int sw, ndep, naggs, check_dep, direct, daw;
+  int op[GQ_MAX_AGGS + 1];
+  int* err;
+};
+__device__ __forceinline__ void gq_m_red(int op, u64* w, u64 v) {
+  if (op == GQ_MIN) atomicMin((i64*)w, (i64)v);
+  else if (op == GQ_MAX) atomicMax((i64*)w, (i64)v);
+  else atomicAdd(w, v);
+}
+__global__ void __launch_bounds__(256) gq_k_merge(const __grid_constant__ GqMergeParams P) {
+  if (*(volatile int*)P.err != 0) return;
+  const i64 stride = (i64)gridDim.x * blockDim.x;
+  const i64 t0 = (i64)blockIdx.x * blockDim.x + threadIdx.x;
+  if (P.direct) {   // accumulator arrays over the same join table: slot i of src into slot i of dst (untouched slots hold identities)
+    for (i64 i = t0; i <= P.scap; i += stride)
+      for (int a = 0; a < P.daw; ++a) {
+        const u64 v = P.sslots[i * P.daw + a];
+        const int op = a <= P.naggs ? P.op[a] : (int)GQ_SUM;
+        if ((op == GQ_MIN && v == 0x7FFFFFFFFFFFFFFFULL) || (op == GQ_MAX && v == 0x8000000000000000ULL) || ((op == GQ_SUM || op == GQ_COUNT_STAR) && v == 0)) continue;
+        gq_m_red(op, P.dslots + i * P.daw + a, v);
+      }
+    return;
+  }
+  const u64 cap = P.dmask + 1;
+  for (i64 i = t0; i < P.scap; i += stride) {
+    const u64* s = P.sslots + i * P.sw;
+    const u64 key = s[0];
+    if (key == GQ_EMPTY_KEY) continue;
+    u64 x = key;
+    x ^= x >> 32;
+    u64 idx = cap > 1 ? __umul64hi(x * 0x9E3779B97F4A7C15ULL, cap) : 0;
+    u64* slot = nullptr;
+    bool won = false;
+    for (u64 tries = 0; tries <= 2 * cap; ++tries) {
+      u64* d = P.dslots + idx * P.sw;
+      u64 k = gq_p_ld_relaxed(d);
+      if (k == GQ_EMPTY_KEY) { const u64 prev = atomicCAS(d, GQ_EMPTY_KEY, key); if (prev == GQ_EMPTY_KEY) { slot = d; won = true; break; } k = prev; }
+      if (k == key) { slot = d; break; }
+      idx = idx + 1 > P.dmask ? 0 : idx + 1;
+    }
+    if (!slot) { atomicCAS(P.err, 0, (int)GQ_ERR_CAPACITY); continue; }
+    if (P.ndep) {
+      if (P.check_dep) {
+        const u64 prev = atomicCAS(slot + 1, GQ_DEP_UNSET, s[1]);
+        if (prev != GQ_DEP_UNSET && prev != s[1]) atomicCAS(P.err, 0, (int)GQ_ERR_DEPENDENT_KEY);
+      } else if (won) slot[1] = s[1];
+    }
+    for (int a = 0; a < P.naggs; ++a) gq_m_red(P.op[a], slot + 1 + P.ndep + a, s[1 + P.ndep + a]);
+  }
+  // the side slot: the group whose key is the reserved pattern, or THE group of a key-less aggregation
+  if (t0 == 0 && P.sheader[1] != 0) {
+    const i64 prev = (i64)atomicExch((u64*)&P.dheader[1], 1ULL);
+    if (P.ndep && (prev == 0 || P.check_dep)) P.dside[1] = P.sside[1];
+    for (int a = 0; a < P.naggs; ++a) gq_m_red(P.op[a], P.dside + 1 + P.ndep + a, P.sside[1 + P.ndep + a]);
+  }
+}
+__global__ void __launch_bounds__(256) gq_k_count_groups(const u64* slots, i64 cap, int sw, const i64* header, int direct, int daw, int dtouch,
+                                                        i64* out) {
+  i64 n = 0;
+  const i64 stride = (i64)gridDim.x * blockDim.x;
+  for (i64 i = (i64)blockIdx.x * blockDim.x + threadIdx.x; i < cap + (direct ? 1 : 0); i += stride)
+    n += direct ? (slots[i * daw + dtouch] != 0) : (slots[i * sw] != GQ_EMPTY_KEY);
+  for (int o = 16; o > 0; o >>= 1) n += __shfl_xor_sync(0xffffffffu, n, o);
+  if ((threadIdx.x & 31) == 0 && n) atomicAdd((u64*)out, (u64)n);
+  if (!direct && blockIdx.x == 0 && threadIdx.x == 0 && header[1] != 0) atomicAdd((u64*)out, 1ULL);
+}
+cudaError_t gq_launch_merge(cudaStream_t s, const unsigned long long* sslots, long long scap, const unsigned long long* sside, const long long* sheader,
+                            unsigned long long* dslots, unsigned long long dmask, unsigned long long* dside, long long* dheader, int sw, int ndep,
+                            int naggs, const int* op, int check_dep, int direct, int daw, int* err, int num_sms) {
+  GqMergeParams p;
+  p.sslots = sslots; p.scap = scap; p.sside = sside; p.sheader = sheader; p.dslots = dslots; p.dmask = dmask; p.dside = dside; p.dheader = dheader;
+  p.sw = sw; p.ndep = ndep; p.naggs = naggs; p.check_dep = check_dep; p.direct = direct; p.daw = daw; p.err = err;
+  for (int a = 0; a <= GQ_MAX_AGGS; ++a) p.op[a] = a < naggs ? op[a] : (int)GQ_SUM;
+  const i64 work = std::max<i64>(1, scap);
+  const int blocks = (int)std::max<i64>(1, std::min<i64>((work + 255) / 256, (i64)num_sms * 16));
+  gq_k_merge<<<blocks, 256, 0, s>>>(p);
+  return cudaGetLastError();
+}
+cudaError_t gq_launch_count_groups(cudaStream_t s, const unsigned long long* slots, long long cap, int sw, const long long* header, int direct, int daw,
+                                   int dtouch, long long* out, int num_sms) {
+  cudaError_t e = cudaMemsetAsync(out, 0, 8, s);
+  if (e != cudaSuccess) return e;
+  const int blocks = (int)std::max<i64>(1, std::min<i64>((cap + 255) / 256, (i64)num_sms * 16));
+  gq_k_count_groups<<<blocks, 256, 0, s>>>(slots, cap, sw, header, direct, daw, dtouch, out);
+  return cudaGetLastError();
+}
+
 // ------------------------------------------------------------------------------------------------ heavy hitters
 // Skew handling for high-cardinality group-by: before the fused scan of a large batch, a strided
 // sample of the group-key column is counted in a small (key,count) table; keys whose sample count reaches the

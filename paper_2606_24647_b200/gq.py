@@ -29,6 +29,7 @@ _AGG = dict(sum=0, min=1, max=2, count=3)
 F_UNIQUE_KEYS = 1
 F_CHECK_DEPENDENT = 2
 F_DENSE_KEYS = 4
+F_FINAL_MODE = 8
 STATUS = ["GQ_OK", "GQ_ERR_INVALID_ARG", "GQ_ERR_UNSUPPORTED", "GQ_ERR_CAPACITY", "GQ_ERR_WORKSPACE_TOO_SMALL",
           "GQ_ERR_CUDA", "GQ_ERR_DUPLICATE_KEY", "GQ_ERR_COMPILE", "GQ_ERR_DEPENDENT_KEY", "GQ_ERR_KEY_RANGE"]
 
@@ -39,7 +40,8 @@ SYMBOLS = ["gq_create", "gq_destroy", "gq_sync", "gq_clear_error", "gq_status_st
            "gq_hash_aggregate_workspace", "gq_hash_aggregate_workspace_for", "gq_hash_aggregate", "gq_topk_scratch_bytes", "gq_hash_aggregate_finish",
            "gq_aggstate_destroy", "gq_pipeline_workspace", "gq_pipeline", "gq_pipeline_host_workspace",
            "gq_pipeline_host", "gq_set_kernel_cache_dir", "gq_precompile_pipeline", "gq_precompile_build", "gq_precompile_materialise",
-           "gq_table_describe", "gq_read_probe", "gq_set_option", "gq_hash_build_workspace_dense", "gq_profile", "gq_profile_read", "gq_order_by_workspace", "gq_order_by"]
+           "gq_table_describe", "gq_read_probe", "gq_set_option", "gq_hash_build_workspace_dense", "gq_profile", "gq_profile_read", "gq_order_by_workspace", "gq_order_by", "gq_aggstate_merge", "gq_aggstate_count",
+           "gq_aggstate_rehash"]
 
 
 class GqError(RuntimeError):
@@ -153,6 +155,9 @@ def lib():
         L.gq_table_describe.argtypes = [C.POINTER(C.c_void_p), C.POINTER(C.c_int), C.c_int32, C.c_uint32]
         L.gq_read_probe.argtypes = [C.c_void_p, C.c_void_p, C.c_size_t, C.c_void_p]
         L.gq_set_option.argtypes = [C.c_char_p, C.c_int64]
+        L.gq_aggstate_merge.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p]
+        L.gq_aggstate_count.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p]
+        L.gq_aggstate_rehash.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_size_t, C.c_int64]
         L.gq_order_by_workspace.argtypes = [C.c_int64, C.POINTER(C.c_size_t)]
         L.gq_order_by.argtypes = [C.c_void_p, C.POINTER(_Batch), C.POINTER(_SortKey), C.c_int32, C.c_int64, C.c_void_p, C.c_size_t,
                                   C.c_void_p, C.POINTER(C.c_void_p)]
@@ -224,7 +229,7 @@ class _M:
         self.keep += [a, list(tensors)]
         return a
 
-    def agg_desc(self, preds, probes, exprs, keys, ndependent, aggs, max_groups, check_dependent=False):
+    def agg_desc(self, preds, probes, exprs, keys, ndependent, aggs, max_groups, check_dependent=False, final_mode=False):
         pr, npr = self.preds(preds)
         pb, npb = self.probes(probes)
         ee, ne = self.exprs(exprs)
@@ -234,7 +239,7 @@ class _M:
             aa[i] = _Agg(_AGG[a[0]], int(a[1]) if len(a) > 1 and a[1] is not None else 0)
         self.keep.append(aa)
         return _AggDesc(pr, npr, pb, npb, ee, ne, kk, nk, int(ndependent), aa, len(aggs), int(max_groups),
-                        F_CHECK_DEPENDENT if check_dependent else 0)
+                        (F_CHECK_DEPENDENT if check_dependent else 0) | (F_FINAL_MODE if final_mode else 0))
 
     def build_desc(self, preds, probes, key, payload, unique, dense_range=None):
         pr, npr = self.preds(preds)
@@ -450,12 +455,13 @@ class Context:
 
     # ---- HashAggregation (streaming) ----
     def aggregate(self, state, cols, preds=(), probes=(), exprs=(), keys=(), ndependent=0, aggs=(), max_groups=1,
-                  plan_aware_workspace=False, check_dependent=False):
-        """plan_aware_workspace: size the state with gq_hash_aggregate_workspace_for (enables direct aggregation)."""
+                  plan_aware_workspace=False, check_dependent=False, final_mode=False):
+        """plan_aware_workspace: size the state with gq_hash_aggregate_workspace_for (enables direct aggregation).
+        final_mode: GQ_F_FINAL_MODE — the rows are intermediate results; ("count", e) sums the partial counts in expr e."""
         with torch.cuda.stream(self.stream):
             m = _M()
             b = m.batch(cols)
-            d = m.agg_desc(preds, probes, exprs, keys, ndependent, aggs, max_groups, check_dependent)
+            d = m.agg_desc(preds, probes, exprs, keys, ndependent, aggs, max_groups, check_dependent, final_mode)
             if state is None:
                 nbytes = C.c_size_t()
                 if plan_aware_workspace:
@@ -471,6 +477,27 @@ class Context:
                 h = C.c_void_p(state.handle.value)
                 self._check(self.L.gq_hash_aggregate(self.h, C.byref(h), None, 0, C.byref(b), C.byref(d)))
         return state
+
+    def aggregate_merge(self, dst, src):
+        """gq_aggstate_merge: fold the groups of state `src` into state `dst` (Partial -> Final between states)."""
+        with torch.cuda.stream(self.stream):
+            self._check(self.L.gq_aggstate_merge(self.h, dst.handle, src.handle))
+
+    def aggregate_count(self, state) -> torch.Tensor:
+        out = torch.zeros(1, dtype=torch.int64, device=self.device)
+        with torch.cuda.stream(self.stream):
+            self._check(self.L.gq_aggstate_count(self.h, state.handle, out.data_ptr()))
+        return out
+
+    def aggregate_rehash(self, state, new_max_groups):
+        """gq_aggstate_rehash: grow a high-cardinality state into a larger table (new workspace; the old one is kept
+        alive by the state object until the next rehash)."""
+        with torch.cuda.stream(self.stream):
+            nbytes = C.c_size_t()
+            self._check(self.L.gq_hash_aggregate_workspace(int(new_max_groups), len(state.key_dtypes), state.naggs, C.byref(nbytes)))
+            ws = self._ws(nbytes.value)
+            self._check(self.L.gq_aggstate_rehash(self.h, state.handle, self._ws_ptr(ws), nbytes.value, int(new_max_groups)))
+            state.old_workspace, state.workspace = state.workspace, ws
 
     def aggregate_finish(self, state, capacity, avgs=(), topk=0, topk_agg=0):
         with torch.cuda.stream(self.stream):
