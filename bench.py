@@ -238,10 +238,13 @@ def run_config(cfg, gq, ctx, torch, datagen, plans, gqrun, steps, warmup, scale=
         # columns: orderdate < 1200 of 2406 values, segment == 1 of 5 values), + 10 %. "upper bound": max_rows = input rows.
         sel = {3: [1200 / 2406], 4: [1 / 5, (1200 / 2406) * (1 / 5)]}[cfg]
         if dense:
-            sizing = "direct-address tables from min/max statistics of the build keys (GQ_F_DENSE_KEYS)"
-            for b in plan["builds"]:
+            sizing = ("direct-address tables (GQ_F_DENSE_KEYS): key range from min/max statistics of the build keys, "
+                      "rows from predicate selectivities + 10 %")
+            for b, s in zip(plan["builds"], sel):
                 k = b["table"][b["key"]]
                 b["dense_range"] = (int(k.min()), int(k.max()))
+                b["max_rows"] = int(len(k) * s * 1.1) + 1024
+            plan["max_groups"] = plan["builds"][-1]["max_rows"]
         elif hinted:
             sizing = "hash tables sized from predicate selectivities + 10 %"
             for b, s in zip(plan["builds"], sel):
@@ -372,7 +375,7 @@ def run_standalone_ops(gq, ctx, torch, datagen, plans, gqrun, steps, warmup):
     pcap = nf // 3
     pouts = [torch.empty(pcap, dtype=torch.int64, device="cuda") for _ in pexprs]
     for label, kw in (("hashed", dict(max_rows=int(nb * 1200 / 2406 * 1.1) + 1024)),
-                      ("dense", dict(dense_range=(int(b["table"][0].min()), int(b["table"][0].max()))))):
+                      ("dense", dict(dense_range=(int(b["table"][0].min()), int(b["table"][0].max())), max_rows=int(nb * 1200 / 2406 * 1.1) + 1024))):
         tb = ctx.hash_build(bcols, preds=b["preds"], key=0, unique=True, **kw)
         ws = tb.workspace
 
@@ -608,6 +611,7 @@ def main():
                 for b in p3["builds"]:
                     kk = b["table"][b["key"]]
                     b["dense_range"] = (int(kk.min()), int(kk.max()))
+                    b["max_rows"] = int(len(kk) * (1200 / 2406) * 1.1) + 1024
                 tables = gqrun.build_tables(ctx, p3)
                 h3 = [torch.from_numpy(np.ascontiguousarray(c)).pin_memory() for c in p3["table"]]
                 hp3 = gqrun.prepare(ctx, p3, tables, cols=h3, out_capacity=10)

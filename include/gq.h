@@ -87,8 +87,9 @@ enum {
   GQ_F_DENSE_KEYS = 1u << 2        /* gq_build_desc: the planner knows (column min/max statistics) that every build key
                                       lies in [key_min, key_max] and the range is not much larger than the row count:
                                       the table becomes a DIRECT-ADDRESS table — a membership bitmap plus a payload
-                                      array indexed by key - key_min; no hashing, no probing, a probe that misses costs
-                                      one bit test in an L2-resident bitmap ("the query planner should choose the
+                                      array indexed by key - key_min; no hashing, no probing, a probe costs one 8-byte
+                                      load from an L2-resident bitmap (which also yields the key's rank among the build
+                                      keys: the slot index of direct aggregation) ("the query planner should choose the
                                       operator implementation based on ... the expected input"). Requires
                                       GQ_F_UNIQUE_KEYS. VERIFIED on device: a key outside the range sets the sticky
                                       GQ_ERR_KEY_RANGE, a repeated key GQ_ERR_DUPLICATE_KEY */
@@ -135,15 +136,18 @@ typedef struct {
  * 1024 (not to a power of two: slot = multiply-shift range reduction of the hash), load = 0.4 for tables that fit L2 and
  * 0.7 for larger ones; read in 32-byte (key-only) or 64-byte (key + payload) buckets. */
 gq_status gq_hash_build_workspace(int64_t max_build_rows, int32_t npayload, size_t* bytes);
-/* Workspace of a GQ_F_DENSE_KEYS table: header + bitmap of (key_max - key_min + 1) bits + that many payload rows.
- * gq_hash_build ignores max_build_rows for such a table. */
-gq_status gq_hash_build_workspace_dense(int64_t key_min, int64_t key_max, int32_t npayload, size_t* bytes);
+/* Workspace of a GQ_F_DENSE_KEYS table: header + 8 bytes per 32 keys of [key_min, key_max] (membership bits and rank
+ * prefix) + one payload row per key of the range + one word per build row (the key of every rank). max_build_rows bounds
+ * the rows inserted (exceeding it => GQ_ERR_CAPACITY at gq_hash_build_finish); <= 0 means "as many as the range has
+ * keys". Such a table MUST be finished with gq_hash_build_finish before it is probed: that call computes the ranks. */
+gq_status gq_hash_build_workspace_dense(int64_t key_min, int64_t key_max, int64_t max_build_rows, int32_t npayload, size_t* bytes);
 /* *table == NULL: creates the table in d_workspace (enqueues its initialisation) and inserts the batch.
  * *table != NULL: inserts a further batch (same schema and desc; d_workspace/bytes/max_build_rows ignored). */
 gq_status gq_hash_build(gq_ctx*, gq_table** table, void* d_workspace, size_t bytes, int64_t max_build_rows,
                         const gq_batch* in, const gq_build_desc* desc);
 /* "noMoreInput": records an event on the building stream; probing contexts on OTHER streams wait on it (the
- * cross-pipeline synchronisation of PAPER.md:123). No host synchronisation. */
+ * cross-pipeline synchronisation of PAPER.md:123). No host synchronisation. For a GQ_F_DENSE_KEYS table it first
+ * enqueues the rank computation (two small kernels). */
 gq_status gq_hash_build_finish(gq_ctx*, gq_table*);
 /* *d_count (DEVICE int64) = rows inserted so far (enqueued copy). */
 gq_status gq_table_count(gq_ctx*, const gq_table*, int64_t* d_count);

@@ -257,6 +257,7 @@ gq_status run_scan(gq_ctx* ctx, const GqScanSpec& sp, const gq_batch* in, const 
   for (size_t s = 0; s < sp.probes.size(); ++s) {
     const gq_table* t = probes[s].table;
     if (t->describe_only) return fail(ctx, GQ_ERR_INVALID_ARG, "probe step names a describe-only table");
+    if (t->dense && !t->ranked) return fail(ctx, GQ_ERR_INVALID_ARG, "a GQ_F_DENSE_KEYS table must be finished (gq_hash_build_finish) before it is probed");
     P->probe[s] = t->dev;
     if (t->finished && t->build_stream != ctx->stream) {   // cross-pipeline boundary
       cudaError_t e = cudaStreamWaitEvent(ctx->stream, t->ready, 0);
@@ -398,21 +399,27 @@ gq_status gq_hash_build_workspace(int64_t max_build_rows, int32_t npayload, size
   return GQ_OK;
 }
 
-// Direct-address table (GQ_F_DENSE_KEYS): [header 256 B][bitmap, one bit per key of the range][payload rows]
-struct DenseLayout { int64_t range; size_t bitmap_off, bitmap_bytes, pay_off, total; };
-static bool dense_layout(int64_t key_min, int64_t key_max, int npayload, DenseLayout* L) {
-  if (key_max < key_min || (uint64_t)key_max - (uint64_t)key_min >= (1ULL << 36)) return false;
+// Direct-address table (GQ_F_DENSE_KEYS): [header 256 B][bitmap entries, 8 B per 32 keys of the range][payload rows]
+// [key of every rank: max_rows words][scratch of the rank kernels]
+struct DenseLayout { int64_t range, max_rows, nwords; size_t bitmap_off, bitmap_bytes, pay_off, keyrank_off, totals_off, total; };
+static bool dense_layout(int64_t key_min, int64_t key_max, int64_t max_rows, int npayload, DenseLayout* L) {
+  if (key_max < key_min || (uint64_t)key_max - (uint64_t)key_min >= (1ULL << 36) || max_rows < 0) return false;
   L->range = (int64_t)((uint64_t)key_max - (uint64_t)key_min + 1);
+  L->max_rows = std::min<int64_t>(L->range, max_rows > 0 ? max_rows : L->range);   // unique keys: never more rows than keys in the range
+  if (L->max_rows >= (1LL << 32)) return false;
+  L->nwords = (L->range + 31) / 32;
   L->bitmap_off = 256;
-  L->bitmap_bytes = align_up((size_t)((L->range + 31) / 32) * 4, 256);
+  L->bitmap_bytes = align_up((size_t)L->nwords * 8, 256);
   L->pay_off = L->bitmap_off + L->bitmap_bytes;
-  L->total = L->pay_off + align_up((size_t)L->range * (size_t)npayload * 8, 256);
+  L->keyrank_off = L->pay_off + align_up((size_t)L->range * (size_t)npayload * 8, 256);
+  L->totals_off = L->keyrank_off + align_up((size_t)L->max_rows * 8, 256);
+  L->total = L->totals_off + align_up((size_t)((L->nwords + GQ_DENSE_RANK_BLOCK - 1) / GQ_DENSE_RANK_BLOCK) * 4, 256);
   return true;
 }
 
-gq_status gq_hash_build_workspace_dense(int64_t key_min, int64_t key_max, int32_t npayload, size_t* bytes) {
+gq_status gq_hash_build_workspace_dense(int64_t key_min, int64_t key_max, int64_t max_build_rows, int32_t npayload, size_t* bytes) {
   DenseLayout L;
-  if (!bytes || npayload < 0 || npayload > GQ_MAX_PAYLOAD || !dense_layout(key_min, key_max, npayload, &L)) return GQ_ERR_INVALID_ARG;
+  if (!bytes || npayload < 0 || npayload > GQ_MAX_PAYLOAD || !dense_layout(key_min, key_max, max_build_rows, npayload, &L)) return GQ_ERR_INVALID_ARG;
   *bytes = L.total;
   return GQ_OK;
 }
@@ -448,19 +455,21 @@ gq_status gq_hash_build(gq_ctx* ctx, gq_table** table, void* d_ws, size_t bytes,
   if (!t && sp.dense_target) {
     DenseLayout L;
     if (!d_ws || !aligned(d_ws, 256)) return fail(ctx, GQ_ERR_INVALID_ARG, "bad workspace");
-    if (!dense_layout(d->key_min, d->key_max, d->npayload, &L)) return fail(ctx, GQ_ERR_INVALID_ARG, "bad dense key range");
+    if (!dense_layout(d->key_min, d->key_max, max_build_rows, d->npayload, &L)) return fail(ctx, GQ_ERR_INVALID_ARG, "bad dense key range");
     if (bytes < L.total) return fail(ctx, GQ_ERR_WORKSPACE_TOO_SMALL, "hash-build workspace too small");
     t = new gq_table();
     t->capacity = L.range; t->dense = true; t->key_min = d->key_min;
     t->npayload = d->npayload;
     for (int p = 0; p < d->npayload; ++p) t->payload_dtype[p] = row_dtype(sp, d->payload_cols[p]);
     t->flags = d->flags;
-    t->max_rows = L.range;
+    t->max_rows = L.max_rows;
     t->dev.slots = (unsigned long long*)((char*)d_ws + L.pay_off);
     t->dev.mask = (unsigned long long)(L.range - 1);
     t->dev.header = (long long*)d_ws;
     t->dev.side = (unsigned long long*)((char*)d_ws + L.bitmap_off);
     t->dev.slot_words = d->npayload; t->dev.flags = d->flags; t->dev.base = d->key_min;
+    t->keyrank = (unsigned long long*)((char*)d_ws + L.keyrank_off);
+    t->rank_totals = (unsigned*)((char*)d_ws + L.totals_off);
     cudaError_t e = cudaMemsetAsync(d_ws, 0, L.bitmap_off + L.bitmap_bytes, ctx->stream);   // header + bitmap; payload rows need no init
     if (e != cudaSuccess) { delete t; return cuda_fail(ctx, e, "dense table init"); }
     { GqScanSpec c = sp; c.nrows_hint = 0; t->build_sig = signature(c) + "|" + std::to_string(d->key_min) + ":" + std::to_string(d->key_max); }
@@ -509,6 +518,13 @@ gq_status gq_hash_build(gq_ctx* ctx, gq_table** table, void* d_ws, size_t bytes,
 gq_status gq_hash_build_finish(gq_ctx* ctx, gq_table* t) {
   if (!ctx || !t || t->describe_only) return GQ_ERR_INVALID_ARG;
   use_device(ctx);
+  if (t->dense && !t->ranked) {   // all keys are in: rank prefix of every bitmap entry, key of every rank
+    cudaError_t e = PROF(ctx, "gq_k_dense_rank(2)", gq_launch_dense_rank(ctx->stream, t->dev.side, (t->capacity + 31) / 32, t->rank_totals, t->key_min,
+                                                                        t->keyrank, t->max_rows, t->dev.header, ctx->d_err));
+    if (e != cudaSuccess) return cuda_fail(ctx, e, "dense table ranks");
+    ctx->launches += 2;
+    t->ranked = true;
+  }
   if (!t->ready) {
     cudaError_t e = cudaEventCreateWithFlags(&t->ready, cudaEventDisableTiming);
     if (e != cudaSuccess) return cuda_fail(ctx, e, "cudaEventCreate");
@@ -637,7 +653,7 @@ DirectPlan direct_plan(const GqScanSpec& sp, const gq_agg_desc* d, const gq_batc
   const bool hidden = dp.touch < 0;
   if (hidden) dp.touch = d->naggs;
   dp.aw = (int)align_up((size_t)(d->naggs + (hidden ? 1 : 0)), 2);
-  dp.cap = t->capacity;
+  dp.cap = t->dense ? t->max_rows : t->capacity;   // dense: one accumulator slot per build row (slot = rank of the key)
   dp.bytes = 256 + (size_t)(dp.cap + 1) * dp.aw * 8;
   // worthwhile unless the probed table is far larger than a hashed table of max_groups would be
   const size_t hashed = (size_t)agg_capacity(d->max_groups, d->nkeys) * agg_slot_words(d->ndependent, d->naggs) * 8;
@@ -812,6 +828,7 @@ gq_status gq_hash_aggregate(gq_ctx* ctx, gq_aggstate** state, void* d_ws, size_t
     if (dp.step >= 0) {
       a->direct = true; a->dtab = d->probes[dp.step].table->dev; a->dcap = dp.cap; a->daw = dp.aw; a->dtouch = dp.touch;
       a->ddense = d->probes[dp.step].table->dense; a->dnpay = d->probes[dp.step].table->npayload;
+      a->dkeyrank = d->probes[dp.step].table->keyrank;
       a->dep_pay = dp.dep_pay;
       a->dev.header = (long long*)d_ws;
       a->dacc = (unsigned long long*)((char*)d_ws + 256);
@@ -1011,6 +1028,7 @@ gq_status gq_hash_aggregate_finish(gq_ctx* ctx, gq_aggstate* a, void* const* out
     p.direct = 1; p.capacity = a->dcap; p.dacc = a->dacc; p.daw = a->daw; p.dtouch = a->dtouch; p.dep_pay = a->dep_pay;
     p.jslots = a->dtab.slots; p.jside = a->dtab.side; p.jsw = a->dtab.slot_words;
     p.jdense = a->ddense ? 1 : 0; p.jbase = a->dtab.base; p.jnpay = a->dnpay;
+    if (a->ddense) p.jside = a->dkeyrank;
   }
   p.nkeys = a->nkeys; p.ndep = a->ndep; p.naggs = a->naggs;
   for (int k = 0; k < a->nkeys; ++k) {

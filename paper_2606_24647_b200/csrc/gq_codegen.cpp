@@ -518,7 +518,8 @@ gq_status gq_codegen(const GqScanSpec& sp, GqKernelInfo* out, std::string* msg) 
       if (ps.dense) {   // direct-address table: at most one match, found with one bit test
         o << ind << "for (int n" << s << " = 0; n" << s << " < 1; ++n" << s << ") {\n";
         ind += "  ";
-        o << ind << "u64 i" << s << ";\n" << ind << "if (!gq_dense_find(T" << s << ", pk" << s << ", &i" << s << ")) break;\n";
+        o << ind << "u64 i" << s << ", rk" << s << ";\n" << ind << "if (!gq_dense_find(T" << s << ", pk" << s << ", &i" << s << ", &rk" << s << ")) break;\n"
+          << ind << "(void)rk" << s << ";\n";
         for (int p = 0; p < ps.npayload; ++p)
           o << ind << "const i64 y" << s << "_" << p << " = (i64)__ldg(T" << s << ".slots + i" << s << " * " << ps.npayload << " + " << p << ");\n";
         continue;

@@ -101,6 +101,9 @@ struct gq_table {
   int64_t max_rows = 0;
   bool dense = false;          // GQ_F_DENSE_KEYS: direct-address table over [key_min, key_min + capacity)
   int64_t key_min = 0;
+  unsigned long long* keyrank = nullptr;   //   key of every rank (max_rows entries), filled by gq_hash_build_finish
+  unsigned* rank_totals = nullptr;         //   scratch of the rank kernels
+  bool ranked = false;
   std::string build_sig;       // shape signature of the first batch (later batches must match)
   cudaEvent_t ready = nullptr; // recorded by gq_hash_build_finish
   cudaStream_t build_stream = nullptr;
@@ -121,6 +124,7 @@ struct gq_aggstate {
   bool direct = false;         // aggregate words indexed by the slot of a probed unique table (no keys stored)
   GqTableDev dtab{};           //   that table
   bool ddense = false; int dnpay = 0;   //   ... is a direct-address table with dnpay payload words per row
+  const unsigned long long* dkeyrank = nullptr;   //   ... its key-of-rank array (accumulator slot = rank of the key)
   int64_t dcap = 0;            //   its capacity (the accumulator array has dcap + 1 slots: the last is the side entry)
   int daw = 0, dtouch = -1, dep_pay = -1;   // words per accumulator slot, word that marks a touched slot, payload = dep key
   unsigned long long* dacc = nullptr;
@@ -226,6 +230,9 @@ cudaError_t gq_launch_merge(cudaStream_t s, const unsigned long long* sslots, lo
                             int naggs, const int* op, int check_dep, int direct, int daw, int* err, int num_sms);
 cudaError_t gq_launch_count_groups(cudaStream_t s, const unsigned long long* slots, long long cap, int sw, const long long* header, int direct, int daw,
                                    int dtouch, long long* out, int num_sms);
+cudaError_t gq_launch_dense_rank(cudaStream_t s, unsigned long long* entries, long long nwords, unsigned* totals, long long base,
+                                 unsigned long long* keyrank, long long max_rows, long long* header, int* err);
+#define GQ_DENSE_RANK_BLOCK (1024 * 8)   // bitmap entries per CTA of the rank kernels
 size_t gq_topk_scratch_bytes_impl();
 // gq_sort.cu
 size_t gq_sort_workspace_bytes(long long nrows);

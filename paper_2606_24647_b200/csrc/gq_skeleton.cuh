@@ -64,7 +64,7 @@ struct GqTableDev {
   u32 flags;
   u32 bshift;        // log2(slots per 32-byte bucket): probe sequences start on a bucket boundary (join tables)
   i64 base;          // direct-address table (GQ_F_DENSE_KEYS): key_min; then slots = payload rows [range][NPAY],
-                     // side = membership bitmap (u32 words), mask = range size - 1
+                     // side = membership entries {bits, rank prefix} per 32 keys, mask = range size - 1
 };
 
 // Outputs of the finaliser fused into the scan kernel (gq_pipeline over one batch, LOWCARD / GLOBAL consumers): every
@@ -433,16 +433,18 @@ __device__ __forceinline__ void gq_upsert_rows(const GqTableDev& T, const i64 (&
 }
 
 // ---- direct-address join tables (GQ_F_DENSE_KEYS; SURVEY 8(f) NEXT-3 "dense-key array mode"): the planner
-// declared the build keys' range, so slot = key - key_min: HashBuild sets a bit in a membership bitmap (atomicOr: a bit
-// found set is a duplicate key) and stores the payload row; HashProbe is one bit test (the bitmap of a 15 M-key
-// range is 1.9 MB: L2-resident, so the probes that miss never reach DRAM) plus, on a hit, the payload row. The
-// matched slot index (key - key_min) serves direct aggregation exactly like a hash-table slot index.
+// declared the build keys' range, so slot = key - key_min. The membership bitmap is an array of 64-bit entries, one per
+// 32 keys: low word = the 32 membership bits, high word = the number of member keys BEFORE this entry (filled in by
+// gq_hash_build_finish). HashBuild sets a bit (atomicOr: a bit found set is a duplicate key) and stores the payload row at
+// slot; HashProbe is ONE 8-byte load from an L2-resident array (15 M keys: 3.75 MB) — the probes that miss never reach
+// DRAM — plus, on a hit, the payload row. The RANK of the key among the member keys (prefix + popcount) is the slot index
+// handed to direct aggregation, so its accumulator array has one slot per build row, not per key of the range.
 template <int NPAY>
 __device__ __forceinline__ bool gq_dense_insert(const GqTableDev& T, i64 key, const i64* pay, int* err) {
   const u64 idx = (u64)key - (u64)T.base;
   if (idx > T.mask) { gq_set_err(err, GQ_E_KEYRANGE); return false; }
   const u32 bit = 1u << (u32)(idx & 31);
-  const u32 old = atomicOr((u32*)T.side + (idx >> 5), bit);
+  const u32 old = atomicOr((u32*)(T.side + (idx >> 5)), bit);   // (little-endian: the low word of the entry)
   if (old & bit) { gq_set_err(err, GQ_E_DUPLICATE); return false; }
 #pragma unroll
   for (int p = 0; p < NPAY; ++p) T.slots[idx * NPAY + p] = (u64)pay[p];
@@ -457,23 +459,31 @@ __device__ __forceinline__ int gq_dense_insert_rows(const GqTableDev& T, const i
     if (live[j] && gq_dense_insert<NPAY>(T, key[j], pay[j], err)) ++n;
   return n;
 }
-__device__ __forceinline__ bool gq_dense_find(const GqTableDev& T, i64 key, u64* idx) {
+// one row: *idx = key - key_min (payload row), *rank = position among the member keys
+__device__ __forceinline__ bool gq_dense_find(const GqTableDev& T, i64 key, u64* idx, u64* rank) {
   *idx = (u64)key - (u64)T.base;
   if (*idx > T.mask) return false;
-  return (__ldg((const u32*)T.side + (*idx >> 5)) >> (u32)(*idx & 31)) & 1u;
+  const u64 e = __ldg(T.side + (*idx >> 5));
+  const u32 bits = (u32)e, sh = (u32)(*idx & 31);
+  *rank = (e >> 32) + __popc(bits & ((1u << sh) - 1u));
+  return (bits >> sh) & 1u;
 }
 template <int NPAY>
 __device__ __forceinline__ void gq_dense_probe_rows(const GqTableDev& T, const i64 (&key)[GQ_R], bool (&live)[GQ_R],
-                                                    u64 (&idx)[GQ_R], i64 (&pay)[GQ_R][NPAY > 0 ? NPAY : 1]) {
-  u32 wv[GQ_R];
+                                                    u64 (&rank)[GQ_R], i64 (&pay)[GQ_R][NPAY > 0 ? NPAY : 1]) {
+  u64 e[GQ_R], idx[GQ_R];
 #pragma unroll
-  for (int j = 0; j < GQ_R; ++j) {                      // the bitmap words of all rows in flight together
+  for (int j = 0; j < GQ_R; ++j) {                      // the bitmap entries of all rows in flight together
     idx[j] = (u64)key[j] - (u64)T.base;
     live[j] = live[j] && idx[j] <= T.mask;
-    wv[j] = live[j] ? __ldg((const u32*)T.side + (idx[j] >> 5)) : 0u;
+    e[j] = live[j] ? __ldg(T.side + (idx[j] >> 5)) : 0ULL;
   }
 #pragma unroll
-  for (int j = 0; j < GQ_R; ++j) live[j] = live[j] && ((wv[j] >> (u32)(idx[j] & 31)) & 1u);
+  for (int j = 0; j < GQ_R; ++j) {
+    const u32 bits = (u32)e[j], sh = (u32)(idx[j] & 31);
+    live[j] = live[j] && ((bits >> sh) & 1u);
+    rank[j] = (e[j] >> 32) + __popc(bits & ((1u << sh) - 1u));
+  }
 #pragma unroll
   for (int j = 0; j < GQ_R; ++j) {
     if (live[j]) {

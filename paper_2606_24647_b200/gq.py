@@ -124,7 +124,7 @@ def lib():
         L.gq_filter_project.argtypes = [C.c_void_p, C.POINTER(_Batch), C.POINTER(_Pred), C.c_int32, C.POINTER(_Expr),
                                         C.c_int32, C.POINTER(C.c_void_p), C.c_int64, C.c_void_p]
         L.gq_hash_build_workspace.argtypes = [C.c_int64, C.c_int32, C.POINTER(C.c_size_t)]
-        L.gq_hash_build_workspace_dense.argtypes = [C.c_int64, C.c_int64, C.c_int32, C.POINTER(C.c_size_t)]
+        L.gq_hash_build_workspace_dense.argtypes = [C.c_int64, C.c_int64, C.c_int64, C.c_int32, C.POINTER(C.c_size_t)]
         L.gq_hash_build.argtypes = [C.c_void_p, C.POINTER(C.c_void_p), C.c_void_p, C.c_size_t, C.c_int64,
                                     C.POINTER(_Batch), C.POINTER(_BuildDesc)]
         L.gq_hash_build_finish.argtypes = [C.c_void_p, C.c_void_p]
@@ -394,7 +394,7 @@ class Context:
                 max_rows = int(b.nrows if max_rows is None else max_rows)
                 nbytes = C.c_size_t()
                 if dense_range is not None:
-                    self._check(self.L.gq_hash_build_workspace_dense(int(dense_range[0]), int(dense_range[1]), len(payload), C.byref(nbytes)))
+                    self._check(self.L.gq_hash_build_workspace_dense(int(dense_range[0]), int(dense_range[1]), max_rows, len(payload), C.byref(nbytes)))
                 else:
                     self._check(self.L.gq_hash_build_workspace(max_rows, len(payload), C.byref(nbytes)))
                 ws = workspace if workspace is not None else self._ws(nbytes.value)

@@ -107,8 +107,9 @@ def test_plan_compiler_covers_direct_address_tables(gq):
         gq.precompile_build([I64], 100, key=0, unique=False, dense_range=(0, 10))
     n = C.c_size_t()
     L = gq.lib()
-    assert L.gq_hash_build_workspace_dense(1, 15_000_000, 1, C.byref(n)) == 0 and n.value >= 15_000_000 // 8 + 15_000_000 * 8
-    assert L.gq_hash_build_workspace_dense(5, 4, 0, C.byref(n)) == 1
+    assert L.gq_hash_build_workspace_dense(1, 15_000_000, 8_000_000, 1, C.byref(n)) == 0
+    assert n.value >= 15_000_000 // 4 + 15_000_000 * 8 + 8_000_000 * 8
+    assert L.gq_hash_build_workspace_dense(5, 4, 0, 0, C.byref(n)) == 1
 
 
 def test_options(gq):

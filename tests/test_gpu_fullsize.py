@@ -52,11 +52,14 @@ def _gpu(plan, ctx, out_capacity=None):
     return got
 
 
-def _dense(plan):
-    """The plan with every build declared GQ_F_DENSE_KEYS over the min/max of its key column (bench.py's statistics)."""
-    for b in plan["builds"]:
+def _dense(plan, sel):
+    """bench.py's timed configuration: every build declared GQ_F_DENSE_KEYS over the min/max of its key column (column
+    statistics), its row bound from the predicates' selectivities + 10 %."""
+    for b, s in zip(plan["builds"], sel):
         k = b["table"][b["key"]]
         b["dense_range"] = (int(k.min()), int(k.max()))
+        b["max_rows"] = int(len(k) * s * 1.1) + 1024
+    plan["max_groups"] = plan["builds"][-1]["max_rows"]
     return plan
 
 
@@ -108,7 +111,7 @@ def test_c3_full_size(ctx):
     plan_ub = plans.plan_c3(t)
     _check_digest(3, _gpu(plan_ub, ctx))
     # bench.py's timed configuration: a direct-address table from the build key's min/max statistics (GQ_F_DENSE_KEYS)
-    plan_d = _dense(plans.plan_c3(t))
+    plan_d = _dense(plans.plan_c3(t), [1200 / 2406])
     _check_digest(3, _gpu(plan_d, ctx))
     top = _gpu(dict(plan_d, topk=10, topk_agg=0), ctx, out_capacity=10)
     assert [[int(c[i]) for c in top["cols"]] for i in range(top["n"])] == DIGESTS["C3"]["top10"]
@@ -141,7 +144,7 @@ def test_c4_full_size(ctx):
     _sample_check(plan, got, 2, rows_of, np.random.default_rng(4))
     _check_digest(4, got)                                                              # the whole 1.3 M-row table
     _check_digest(4, _gpu(plans.plan_c4(t), ctx))                                      # upper-bound sizing: same table
-    _check_digest(4, _gpu(_dense(plans.plan_c4(t)), ctx))                              # bench.py's configuration: direct-address tables
+    _check_digest(4, _gpu(_dense(plans.plan_c4(t), [1 / 5, (1200 / 2406) / 5]), ctx))                              # bench.py's configuration: direct-address tables
 
 
 def test_c5_full_size(ctx):

@@ -306,7 +306,8 @@ def test_direct_address_tables_adversarial(ctx):
     assert n == pairs.nrows > 0 and np.array_equal(got[np.lexsort(got.T[::-1])], ref[np.lexsort(ref.T[::-1])])
     # streaming batches into one dense table; a multiset step in front of a dense step (one-row-at-a-time row code)
     h = gqrun.dev(b["table"])
-    tb2 = ctx.hash_build([c[:7008] for c in h], preds=b["preds"], key=0, payload=[1], unique=True, dense_range=b["dense_range"], finish=False)
+    tb2 = ctx.hash_build([c[:7008] for c in h], preds=b["preds"], key=0, payload=[1], unique=True, dense_range=b["dense_range"], finish=False,
+                         max_rows=nb)                              # the row bound covers ALL batches (default: this batch's rows)
     ctx.hash_build([c[7008:] for c in h], preds=b["preds"], key=0, payload=[1], unique=True, dense_range=b["dense_range"], table=tb2)
     assert int(ctx.table_count(tb2).item()) == int((bsel == 1).sum())
     mkey = rng.integers(0, 300, 5000).astype(np.int64)
@@ -328,6 +329,14 @@ def test_direct_address_tables_adversarial(ctx):
         c2.sync()
     assert e.value.status == 6                                  # GQ_ERR_DUPLICATE_KEY
     c2.clear_error(); c2.sync()
+    c2.hash_build(gqrun.dev([bkeys]), key=0, unique=True, dense_range=(-30_000, 29_999), max_rows=100)
+    with pytest.raises(gq.GqError) as e:                        # more build rows than max_build_rows promised
+        c2.sync()
+    assert e.value.status == 3                                  # GQ_ERR_CAPACITY
+    c2.clear_error(); c2.sync()
+    tb3 = c2.hash_build(gqrun.dev([bkeys]), key=0, unique=True, dense_range=(-30_000, 29_999), finish=False)
+    with pytest.raises(gq.GqError):                             # probing a dense table before gq_hash_build_finish
+        c2.hash_probe(gqrun.dev([fk, v]), [], [(tb3, 0)], [[("col", 0)]], capacity=nf)
 
 
 def test_check_dependent_flag_catches_a_false_declaration(ctx):
