@@ -232,7 +232,7 @@ cudaError_t gq_launch_count_groups(cudaStream_t s, const unsigned long long* slo
                                    int dtouch, long long* out, int num_sms);
 cudaError_t gq_launch_dense_rank(cudaStream_t s, unsigned long long* entries, long long nwords, unsigned* totals, long long base,
                                  unsigned long long* keyrank, long long max_rows, long long* header, int* err);
-#define GQ_DENSE_RANK_BLOCK (1024 * 8)   // bitmap entries per CTA of the rank kernels
+#define GQ_DENSE_RANK_BLOCK 1024         // bitmap entries per CTA of the rank kernels
 size_t gq_topk_scratch_bytes_impl();
 // gq_sort.cu
 size_t gq_sort_workspace_bytes(long long nrows);

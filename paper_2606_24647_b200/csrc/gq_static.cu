@@ -436,23 +436,21 @@ cudaError_t gq_launch_part_upsert(cudaStream_t s, const GqPartParams& p, int num
 // gq_hash_build_finish of a direct-address table: the high word of every bitmap entry := number of member keys before
 // it, header[2] := member keys; keyrank[r] := key of rank r (read by the finalisers of direct aggregation). Two
 // kernels: per-CTA totals, then every CTA sums the totals before it and scans its own entries.
-#define GQ_RANK_THREADS 1024
-#define GQ_RANK_PER 8
+#define GQ_RANK_THREADS 1024                               // one bitmap entry per thread (gq_internal.h GQ_DENSE_RANK_BLOCK)
 __global__ void __launch_bounds__(GQ_RANK_THREADS) gq_k_dense_rank_totals(const u64* entries, i64 nwords, unsigned* totals) {
   __shared__ unsigned warp_sum[GQ_RANK_THREADS / 32];
-  const i64 w0 = ((i64)blockIdx.x * GQ_RANK_THREADS + threadIdx.x) * GQ_RANK_PER;
-  unsigned c = 0;
-  for (int j = 0; j < GQ_RANK_PER; ++j) if (w0 + j < nwords) c += __popc((unsigned)entries[w0 + j]);
+  const i64 w = (i64)blockIdx.x * GQ_RANK_THREADS + threadIdx.x;
+  unsigned c = w < nwords ? __popc((unsigned)entries[w]) : 0u;
   for (int o = 16; o > 0; o >>= 1) c += __shfl_xor_sync(0xffffffffu, c, o);
   if ((threadIdx.x & 31) == 0) warp_sum[threadIdx.x >> 5] = c;
   __syncthreads();
-  if (threadIdx.x == 0) { unsigned t = 0; for (int w = 0; w < GQ_RANK_THREADS / 32; ++w) t += warp_sum[w]; totals[blockIdx.x] = t; }
+  if (threadIdx.x == 0) { unsigned t = 0; for (int i = 0; i < GQ_RANK_THREADS / 32; ++i) t += warp_sum[i]; totals[blockIdx.x] = t; }
 }
 __global__ void __launch_bounds__(GQ_RANK_THREADS) gq_k_dense_rank_apply(u64* entries, i64 nwords, const unsigned* totals, i64 base, u64* keyrank,
                                                                          i64 max_rows, i64* header, int* err) {
   __shared__ unsigned part[GQ_RANK_THREADS];
   __shared__ unsigned block_base;
-  const int t = threadIdx.x;
+  const int t = threadIdx.x, lane = t & 31;
   unsigned b = 0;
   for (int i = t; i < (int)blockIdx.x; i += GQ_RANK_THREADS) b += totals[i];
   part[t] = b;
@@ -460,37 +458,37 @@ __global__ void __launch_bounds__(GQ_RANK_THREADS) gq_k_dense_rank_apply(u64* en
   for (int o = GQ_RANK_THREADS / 2; o > 0; o >>= 1) { if (t < o) part[t] += part[t + o]; __syncthreads(); }
   if (t == 0) block_base = part[0];
   __syncthreads();
-  const i64 w0 = ((i64)blockIdx.x * GQ_RANK_THREADS + t) * GQ_RANK_PER;
-  unsigned bits[GQ_RANK_PER], c = 0;
-  for (int j = 0; j < GQ_RANK_PER; ++j) { bits[j] = w0 + j < nwords ? (unsigned)entries[w0 + j] : 0u; c += __popc(bits[j]); }
+  const i64 w = (i64)blockIdx.x * GQ_RANK_THREADS + t;
+  const unsigned bits = w < nwords ? (unsigned)entries[w] : 0u;
+  const unsigned c = __popc(bits);
   part[t] = c;
   __syncthreads();
-  for (int o = 1; o < GQ_RANK_THREADS; o <<= 1) {          // inclusive scan of the per-thread counts
+  for (int o = 1; o < GQ_RANK_THREADS; o <<= 1) {          // inclusive scan of the per-entry counts
     const unsigned v = t >= o ? part[t - o] : 0;
     __syncthreads();
     part[t] += v;
     __syncthreads();
   }
-  u64 run = (u64)block_base + part[t] - c;
-  for (int j = 0; j < GQ_RANK_PER; ++j) {
-    if (w0 + j >= nwords) break;
-    entries[w0 + j] = (u64)bits[j] | (run << 32);
-    unsigned m = bits[j];
-    while (m) {                                            // the keys of this entry, in order, at their ranks
-      const int bpos = __ffs(m) - 1;
-      m &= m - 1;
-      if ((i64)run < max_rows) keyrank[run] = (u64)(base + (w0 + j) * 32 + bpos);
-      ++run;
+  const u64 rank0 = (u64)block_base + part[t] - c;         // member keys before this entry
+  if (w < nwords) entries[w] = (u64)bits | (rank0 << 32);
+  // key of every rank: the warp expands its 32 entries one after the other, lane l taking bit l (coalesced stores)
+  for (int k = 0; k < 32; ++k) {
+    const unsigned wb = __shfl_sync(0xffffffffu, bits, k);
+    const u64 wr = __shfl_sync(0xffffffffu, rank0, k);
+    if ((wb >> lane) & 1u) {
+      const u64 r = wr + __popc(wb & ((1u << lane) - 1u));
+      if ((i64)r < max_rows) keyrank[r] = (u64)(base + (w - lane + k) * 32 + lane);
     }
   }
   if (blockIdx.x == gridDim.x - 1 && t == GQ_RANK_THREADS - 1) {
-    header[2] = (i64)run;
-    if ((i64)run > max_rows) atomicCAS(err, 0, (int)GQ_ERR_CAPACITY);   // more build rows than max_build_rows promised
+    const i64 total = (i64)(rank0 + c);
+    header[2] = total;
+    if (total > max_rows) atomicCAS(err, 0, (int)GQ_ERR_CAPACITY);   // more build rows than max_build_rows promised
   }
 }
 cudaError_t gq_launch_dense_rank(cudaStream_t s, unsigned long long* entries, long long nwords, unsigned* totals, long long base,
                                  unsigned long long* keyrank, long long max_rows, long long* header, int* err) {
-  const int blocks = (int)((nwords + GQ_RANK_THREADS * GQ_RANK_PER - 1) / (GQ_RANK_THREADS * GQ_RANK_PER));
+  const int blocks = (int)((nwords + GQ_RANK_THREADS - 1) / GQ_RANK_THREADS);
   gq_k_dense_rank_totals<<<blocks, GQ_RANK_THREADS, 0, s>>>(entries, nwords, totals);
   gq_k_dense_rank_apply<<<blocks, GQ_RANK_THREADS, 0, s>>>(entries, nwords, totals, base, keyrank, max_rows, header, err);
   return cudaGetLastError();
