@@ -473,6 +473,7 @@ def main_reference(args):
 
 
 def main():
+    global MIN_LOAD_MS
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=400)
@@ -483,10 +484,13 @@ def main():
                     "NxS = config N at S times its rows (C1x64: the low-cardinality pipeline at steady state)")
     ap.add_argument("--c5-scale", type=float, default=1.0)
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--min-load-ms", type=float, default=MIN_LOAD_MS, help="untimed warm-up is extended until the GPU has been "
+                    "under load this long (clock samples); 0 keeps launch lists under ncu short")
     ap.add_argument("--only-configs", action="store_true", help="skip the C2 headline: print only the --configs records "
                     "(the ncu captures under profiles/ name this command)")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3)
+    MIN_LOAD_MS = args.min_load_ms
     if args.impl == "reference":
         return main_reference(args)
 
