@@ -176,3 +176,52 @@ def test_state_growth_by_rehash(gqm):
     small = ctx.aggregate(None, [c[:1024] for c in d], exprs=EXPRS, keys=[], aggs=AGGS, max_groups=1)
     with pytest.raises(gqm.GqError):
         ctx.aggregate_rehash(small, 100)
+
+
+def test_degenerate_inputs(gqm):
+    # empty build side, one-key range, every row filtered out, empty states merged: the degenerate cases of the new paths
+    import gqrun
+    import torch
+    from paper_2606_24647_b200 import gq
+    ctx = gqm.Context()
+    rng = np.random.default_rng(65)
+    fk = rng.integers(-3, 4, 10_000).astype(np.int64)
+    v = rng.integers(0, 100, 10_000).astype(np.int64)
+    # (a) dense table whose build batch has no surviving row; range of a single key
+    for bkeys, preds, rng_ in ((np.array([1, 2, 3], np.int64), [(0, "gt", 100)], (0, 5)), (np.array([2], np.int64), [], (2, 2))):
+        b = dict(table=[bkeys], preds=preds, key=0, payload=[], unique=True, dense_range=rng_)
+        plan = dict(builds=[b], table=[fk, v], preds=[], probes=[(0, 0)], exprs=[[("col", 1)]], keys=[0], aggs=[("sum", 0), ("count",)],
+                    max_groups=8)
+        exp = oracle.run_query(plan)
+        got = gqrun.run_query(plan, ctx=ctx)
+        assert got["n"] == exp.nrows and all(np.array_equal(g, e) for g, e in zip(got["cols"], exp.cols))
+    # (b) partitioned shared-memory aggregation with every row filtered out, and with one surviving row
+    try:
+        gq.set_option("part_min_table_mb", 0); gq.set_option("part_min_rows", 4096); gq.set_option("hot_min_rows", 4096)
+        k = rng.integers(0, 1000, 50_000).astype(np.int64)
+        w = np.zeros(50_000, np.int64); w[777] = 5
+        for lim in (9, 3):
+            plan = dict(table=[k, w], preds=[(1, "gt", lim)], exprs=[[("col", 1)]], keys=[0], aggs=[("sum", 0), ("min", 0), ("count",)],
+                        max_groups=100_000)
+            exp = oracle.run_query(plan)
+            got = gqrun.run_query(plan, ctx=ctx)
+            assert got["n"] == exp.nrows == (0 if lim == 9 else 1)
+            assert all(np.array_equal(g, e) for g, e in zip(got["cols"], exp.cols))
+    finally:
+        gq.set_option("part_min_table_mb", -1); gq.set_option("part_min_rows", -1); gq.set_option("hot_min_rows", -1)
+    # (c) merging an empty state, into an empty state; counting an empty state
+    d = gqrun.dev([fk, v])
+    kw = dict(exprs=[[("col", 1)]], keys=[0], aggs=[("sum", 0), ("count",)], max_groups=1000)
+    full = ctx.aggregate(None, d, **kw)
+    empty = ctx.aggregate(None, [c[:0] for c in d], **kw)
+    empty2 = ctx.aggregate(None, [c[:0] for c in d], **kw)
+    assert int(ctx.aggregate_count(empty).item()) == 0
+    ctx.aggregate_merge(full, empty)
+    ctx.aggregate_merge(empty2, full)
+    exp = oracle.run_query(dict(table=[fk, v], **kw))
+    for st in (full, empty2):
+        _equal(exp, *_finish(ctx, st, 1, 100))
+    # (d) order by on a single row and on all-equal keys with limit 1
+    idx, outs = ctx.order_by(gqrun.dev([np.array([7], np.int64)]), [(0, True)])
+    ctx.sync()
+    assert idx.cpu().tolist() == [0] and outs[0].cpu().tolist() == [7]
