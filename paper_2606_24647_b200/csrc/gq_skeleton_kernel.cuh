@@ -83,6 +83,16 @@ __device__ __forceinline__ void gq_lc_reduce4(const GqCtx& cx, int p0, int np, i
 }
 #endif
 
+// One tile into ring stage s: one 1-D TMA bulk copy per referenced column, completion counted on the stage's full barrier.
+__device__ __forceinline__ void gq_produce_tile(const GqParams& P, unsigned char* smem, u64* full_bar, int s, i64 tile, u64 pol) {
+  gq_mbar_expect_tx(&full_bar[s], (u32)GQ_TX_BYTES);
+  unsigned char* st = smem + (size_t)s * GQ_STAGE_BYTES;
+#pragma unroll
+  for (int c = 0; c < GQ_NCOL; ++c)
+    gq_bulk_g2s(st + GQ_COL_OFF(c), (const unsigned char*)P.col[c] + (size_t)tile * GQ_TILE * GQ_COL_BYTES(c),
+                (u32)(GQ_TILE * GQ_COL_BYTES(c)), &full_bar[s], pol);
+}
+
 extern "C" __global__ void __launch_bounds__(GQ_NT + 32, 1) gq_scan(const __grid_constant__ GqParams P) {
   extern __shared__ __align__(128) unsigned char gq_smem[];
   u64* full_bar = (u64*)(gq_smem + GQ_BAR_OFF);
@@ -92,10 +102,16 @@ extern "C" __global__ void __launch_bounds__(GQ_NT + 32, 1) gq_scan(const __grid
   // Sticky error: later kernels are no-ops (gq.h "Errors"). Thread 0 reads the flag once, the CTA decides after the
   // set-up barrier below: every thread sees the same value, and the round trip overlaps the shared-memory set-up.
   volatile int* err_seen = (volatile int*)(gq_smem + GQ_BAR_OFF + 2 * GQ_STAGES * 8);
-  if (tid == 0) {
-    *err_seen = *(volatile int*)P.err;
+  if (tid == 0) *err_seen = *(volatile int*)P.err;
+  // The producer lane initialises the mbarriers and issues the bulk copies of its first GQ_STAGES tiles BEFORE the set-up
+  // barrier: the first TMA round trip (~1.8 us cold) overlaps the error-flag load and the shared-memory set-up.
+  i64 produced = 0;
+  if (tid == GQ_NT) {
     for (int s = 0; s < GQ_STAGES; ++s) { gq_mbar_init(&full_bar[s], 1); gq_mbar_init(&empty_bar[s], GQ_NWARP); }
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    const u64 pol = gq_policy_evict_first();
+    for (i64 tile = blockIdx.x; tile < ntiles && produced < GQ_STAGES; tile += gridDim.x, ++produced)
+      gq_produce_tile(P, gq_smem, full_bar, (int)produced, tile, pol);
   }
   GqCtx cx;
   cx.t = tid;
@@ -154,6 +170,7 @@ extern "C" __global__ void __launch_bounds__(GQ_NT + 32, 1) gq_scan(const __grid
 #endif
   __syncthreads();
   if (*err_seen != 0) {
+    if (tid == GQ_NT) for (i64 i = 0; i < produced; ++i) gq_mbar_wait(&full_bar[i], 0u);   // copies in flight land before the CTA exits
 #if GQ_FUSED_FINAL
     if (tid == 0) {   // keep ticket (and merge table) zeroed for the next kernel
       const u32 t = atomicAdd(P.fin.ticket, 1u);
@@ -173,17 +190,12 @@ extern "C" __global__ void __launch_bounds__(GQ_NT + 32, 1) gq_scan(const __grid
     // ------------------------------------------------------------------ producer warp: TMA bulk copies
     if (tid == GQ_NT) {
       const u64 pol = gq_policy_evict_first();
-      i64 it = 0;
-      for (i64 tile = blockIdx.x; tile < ntiles; tile += gridDim.x, ++it) {
+      i64 it = produced;
+      for (i64 tile = blockIdx.x + produced * gridDim.x; tile < ntiles; tile += gridDim.x, ++it) {
         const int s = (int)(it % GQ_STAGES);
         const u32 ph = (u32)((it / GQ_STAGES) & 1);
-        gq_mbar_wait(&empty_bar[s], ph ^ 1u);            // stage free (first pass through the ring: immediately)
-        gq_mbar_expect_tx(&full_bar[s], (u32)GQ_TX_BYTES);
-        unsigned char* st = gq_smem + (size_t)s * GQ_STAGE_BYTES;
-#pragma unroll
-        for (int c = 0; c < GQ_NCOL; ++c)
-          gq_bulk_g2s(st + GQ_COL_OFF(c), (const unsigned char*)P.col[c] + (size_t)tile * GQ_TILE * GQ_COL_BYTES(c),
-                      (u32)(GQ_TILE * GQ_COL_BYTES(c)), &full_bar[s], pol);
+        gq_mbar_wait(&empty_bar[s], ph ^ 1u);            // the consumers have released the stage
+        gq_produce_tile(P, gq_smem, full_bar, s, tile, pol);
       }
     }
     return;
@@ -313,23 +325,38 @@ extern "C" __global__ void __launch_bounds__(GQ_NT + 32, 1) gq_scan(const __grid
       const i64 key = cx.lc_gkey[tid];
       u32 h = (u32)gq_hash(key, 64 - 6);
       bool done = false;
+#if GQ_LC_KEY32
+      // packed keys narrower than 32 bits travel IN the state word (2 | key << 32): one CAS round trip tells a CTA whether
+      // it claimed the slot, must wait for its publication, found its key, or has to look at the next slot
+      const u64 mine = 2ULL | ((u64)GQ_LC_K32(key) << 32);
+#endif
       for (int n = 0; n < GQ_GTAB_SLOTS && !done; ++n, h = (h + 1) & (GQ_GTAB_SLOTS - 1)) {
         u64* s = gt + 32 + h * 16;
+#if GQ_LC_KEY32
+        u64 st = atomicCAS(s, 0ULL, 1ULL);
+#else
         u64 st = gq_ld_acquire(s);
-        if (st == 0) {
-          st = atomicCAS(s, 0ULL, 1ULL);
-          if (st == 0) {                                   // claimed: store key and values, then publish
-            s[1] = (u64)key;
+        if (st == 0) st = atomicCAS(s, 0ULL, 1ULL);
+#endif
+        if (st == 0) {                                     // claimed: store key and values, then publish
+          s[1] = (u64)key;
 #pragma unroll
-            for (int a = 0; a < GQ_NAGG; ++a) s[2 + a] = (u64)fin[tid * GQ_NAGG + a];
-            gq_st_release(s, 2ULL);
-            if (atomicAdd(gt, 1ULL) >= (u64)GQ_LC_G) gq_set_err(P.err, GQ_E_CAPACITY);   // more distinct keys than max_groups
-            done = true;
-            break;
-          }
+          for (int a = 0; a < GQ_NAGG; ++a) s[2 + a] = (u64)fin[tid * GQ_NAGG + a];
+#if GQ_LC_KEY32
+          gq_st_release(s, mine);
+#else
+          gq_st_release(s, 2ULL);
+#endif
+          atomicAdd(gt, 1ULL);                             // groups claimed (fire and forget; the last CTA checks the bound)
+          done = true;
+          break;
         }
         while (st == 1) st = gq_ld_acquire(s);             // being published by another CTA
+#if GQ_LC_KEY32
+        if (st == mine) {
+#else
         if (s[1] == (u64)key) {
+#endif
 #pragma unroll
           for (int a = 0; a < GQ_NAGG; ++a) gq_red(GQ_AGG_OP(a), s + 2 + a, fin[tid * GQ_NAGG + a]);
           done = true;
@@ -345,20 +372,23 @@ extern "C" __global__ void __launch_bounds__(GQ_NT + 32, 1) gq_scan(const __grid
       __threadfence();
       if (tid < GQ_GTAB_SLOTS) {                            // warps 0 and 1: one slot per lane
         u64* s = gt + 32 + tid * 16;
-        const bool have = __ldcg((const i64*)s) == 2;
+        i64 wd[2 + GQ_NAGG];                                // state, key and values of the slot: all loads in flight together
+#pragma unroll
+        for (int i = 0; i < 2 + GQ_NAGG; ++i) wd[i] = __ldcg((const i64*)s + i);
+        const bool have = ((u64)wd[0] & 3ULL) == 2ULL;
         const u32 m = __ballot_sync(0xffffffffu, have);
         if (tid == 31) cx.lc_n[2] = __popc(m);            // groups in slots 0..31 (lc_n[2] is free by now)
         asm volatile("bar.sync 2, 64;" ::: "memory");
         const int row = (tid >= 32 ? ((volatile int*)cx.lc_n)[2] : 0) + __popc(m & ((1u << lane) - 1u));
         if (have) {
-          i64 vals[GQ_NAGG];
-#pragma unroll
-          for (int a = 0; a < GQ_NAGG; ++a) vals[a] = __ldcg((const i64*)s + 2 + a);
-          if (row < P.fin.out_capacity) gq_fin_emit(P.fin, row, __ldcg((const i64*)s + 1), vals);
+          if (row < P.fin.out_capacity) gq_fin_emit(P.fin, row, wd[1], wd + 2);
           else gq_set_err(P.err, GQ_E_CAPACITY);
           s[0] = 0;
         }
-        if (tid == 63) { *P.fin.out_n = row + (have ? 1 : 0); gt[0] = 0; *P.fin.ticket = 0; }
+        if (tid == 63) {
+          if (row + (have ? 1 : 0) > GQ_LC_G) gq_set_err(P.err, GQ_E_CAPACITY);   // more distinct keys than max_groups
+          *P.fin.out_n = row + (have ? 1 : 0); gt[0] = 0; *P.fin.ticket = 0;
+        }
       }
     }
 #endif
