@@ -809,12 +809,27 @@ __device__ __forceinline__ void gq_lc_update(const int OP, GqCtx& cx, int grp, i
 // SUM/COUNT use two native 32-bit ATOMS.ADD with an explicit carry; MIN/MAX compare first and CAS only to improve.
 #define GQ_HOT_POS 512
 #define GQ_HOT_MAX 256
+// The hot set is bucketised: 128 buckets of 4 keys (GQ_HOT_POS positions for <= GQ_HOT_MAX keys). A key sits in the bucket
+// its hash names unless that bucket was full when it was inserted (then in the next one), so a lookup reads one
+// 32-byte bucket (two LDS.128) and almost always stops there: a bucket with a free position was never full. (The
+// position-by-position linear probe it replaces was a third of pass A's instructions on C5: every row of a warp walked
+// as far as the unluckiest lane.)
+__device__ __forceinline__ u32 gq_hot_bucket(i64 key) { return (u32)gq_hash(key, 64 - 16) & (GQ_HOT_POS / 4 - 1); }
+__device__ __forceinline__ void gq_hot_insert(GqCtx& cx, i64 key) {   // set-up only; keys are distinct
+  u32 b = gq_hot_bucket(key);
+  for (int n = 0; n < GQ_HOT_POS / 4; ++n, b = (b + 1) & (GQ_HOT_POS / 4 - 1))
+    for (int q = 0; q < 4; ++q)
+      if (atomicCAS((u64*)&cx.hot_keys[b * 4 + q], GQ_EMPTY, (u64)key) == GQ_EMPTY) return;
+}
 __device__ __forceinline__ int gq_hot_find(const GqCtx& cx, i64 key) {
-  u32 i = (u32)gq_hash(key, 64 - 16) & (GQ_HOT_POS - 1);
-  for (int n = 0; n < GQ_HOT_POS; ++n, i = (i + 1) & (GQ_HOT_POS - 1)) {
-    const i64 k = cx.hot_keys[i];
-    if (k == key) return (int)i;
-    if ((u64)k == GQ_EMPTY) return -1;
+  u32 b = gq_hot_bucket(key);
+  for (int n = 0; n < GQ_HOT_POS / 4; ++n, b = (b + 1) & (GQ_HOT_POS / 4 - 1)) {
+    const longlong2 k01 = *(const longlong2*)&cx.hot_keys[b * 4], k23 = *(const longlong2*)&cx.hot_keys[b * 4 + 2];
+    if (k01.x == key) return (int)(b * 4);
+    if (k01.y == key) return (int)(b * 4 + 1);
+    if (k23.x == key) return (int)(b * 4 + 2);
+    if (k23.y == key) return (int)(b * 4 + 3);
+    if ((u64)k01.x == GQ_EMPTY || (u64)k01.y == GQ_EMPTY || (u64)k23.x == GQ_EMPTY || (u64)k23.y == GQ_EMPTY) return -1;
   }
   return -1;
 }

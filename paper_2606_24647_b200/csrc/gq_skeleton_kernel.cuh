@@ -160,12 +160,7 @@ extern "C" __global__ void __launch_bounds__(GQ_NT + 32, 1) gq_scan(const __grid
       for (int a = 0; a < GQ_NAGG; ++a) cx.hot_acc[i * GQ_NAGG + a] = (u64)gq_identity(GQ_AGG_OP(a));
     }
     __syncthreads();
-    if (tid < cx.nhot) {   // insert this batch's hot keys into the shared set (distinct by construction)
-      const i64 key = P.hot[32 + tid];
-      u32 i = (u32)gq_hash(key, 64 - 16) & (GQ_HOT_POS - 1);
-      for (int n = 0; n < GQ_HOT_POS; ++n, i = (i + 1) & (GQ_HOT_POS - 1))
-        if (atomicCAS((u64*)&cx.hot_keys[i], GQ_EMPTY, (u64)key) == GQ_EMPTY) break;
-    }
+    if (tid < cx.nhot) gq_hot_insert(cx, P.hot[32 + tid]);   // this batch's hot keys into the shared set (distinct by construction)
   }
 #endif
   __syncthreads();
