@@ -282,6 +282,9 @@ int32_t gq_profile_read(gq_ctx*, char* h_names, size_t names_bytes, float* h_ms,
  *   "psa_max_log2_partitions"  cap on the pass-A partitions of the partitioned shared-memory aggregation (default 14);
  *                        key ranges beyond it are resolved by sub-passes of pass B
  *   "psa_threads"        512 / 1024 threads per CTA in pass B (default 1024), 0 = default
+ *   "dpart_min_acc_mb"   direct aggregations whose accumulator array is at least this large cluster their updates by
+ *                        slice of the array (records appended by the scan, applied slice by slice); default: never
+ *                        (measured slower on C3), a planner may enable it for arrays far beyond L2
  * Unknown names return GQ_ERR_INVALID_ARG. A negative value restores the default. */
 gq_status gq_set_option(const char* h_name, int64_t value);
 

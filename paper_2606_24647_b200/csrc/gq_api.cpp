@@ -668,7 +668,7 @@ DirectPlan direct_plan(const GqScanSpec& sp, const gq_agg_desc* d, const gq_batc
 // an L2-resident table slice. Worth it only for big tables and big batches; thresholds overridable for tests.
 struct PartPlan { bool on = false; int npart = 0, pshift = 0, rw = 0; int64_t pcap = 0; size_t bytes = 0; std::vector<int> exprs; int src[GQ_MAX_AGGS]; };
 // planner knobs (gq_set_option)
-std::atomic<int64_t> g_part_min_table_mb{256}, g_part_min_rows{1 << 24}, g_hot_min_rows{GQ_HOT_MIN_ROWS}, g_psa_max_log2part{GQ_PSA_MAX_LOG2PART}, g_psa_threads{0};
+std::atomic<int64_t> g_part_min_table_mb{256}, g_part_min_rows{1 << 24}, g_hot_min_rows{GQ_HOT_MIN_ROWS}, g_psa_max_log2part{GQ_PSA_MAX_LOG2PART}, g_psa_threads{0}, g_dpart_min_acc_mb{GQ_DPART_OFF};
 PartPlan part_plan(const GqScanSpec& sp, const gq_agg_desc* d, int64_t nrows) {
   PartPlan pp;
   if (sp.consumer != GQ_C_HIGHCARD) return pp;
@@ -691,6 +691,35 @@ PartPlan part_plan(const GqScanSpec& sp, const gq_agg_desc* d, int64_t nrows) {
   }
   pp.rw = (int)align_up((size_t)(1 + d->ndependent + pp.exprs.size()), 4);
   pp.pcap = (nrows / np + nrows / (4 * np) + 1024 + GQ_PART_CHUNK - 1) / GQ_PART_CHUNK * GQ_PART_CHUNK;   // whole chunks
+  pp.bytes = align_up((size_t)np * 8 * GQ_PART_CURSOR_STRIDE, 256) + (size_t)np * (size_t)pp.pcap * pp.rw * 8;
+  pp.on = true;
+  return pp;
+}
+
+// Clustered DIRECT aggregation: when the accumulator array of a direct aggregation is far larger than L2, every RED of the
+// fact scan is a random DRAM read-modify-write (C3: 15.7 M of them bound the scan at 0.64 ms). The same two-pass scheme
+// as above is available: pass A appends (accumulator slot, aggregate inputs) records per 4 MB slice of the array, pass B
+// applies them slice by slice, so the REDs hit L2. Measured on C3 (132 MB of accumulators, 15.7 M records in 32 slices):
+// scan 0.64 -> 0.57 ms but + 0.29 ms for pass B (few, fast-filling slices make the 32-record chunk refills the
+// bottleneck), so it is OFF unless the planner lowers "dpart_min_acc_mb" (tests do).
+PartPlan direct_part_plan(const DirectPlan& dp, const gq_agg_desc* d, int64_t nrows) {
+  PartPlan pp;
+  if (dp.step < 0 || dp.bytes < (size_t)g_dpart_min_acc_mb.load() * (1 << 20) || nrows < g_part_min_rows.load()) return pp;
+  int shift = 0;
+  while (((int64_t)dp.aw * 8 << (shift + 1)) <= (4 << 20)) ++shift;        // slots per slice: 4 MB of accumulators
+  const int64_t np = (dp.cap + 1 + (1LL << shift) - 1) >> shift;
+  if (np < 2 || np > 4096) return pp;
+  pp.npart = (int)np; pp.pshift = shift;
+  for (int a = 0; a < d->naggs; ++a) {
+    pp.src[a] = -1;
+    if (d->aggs[a].op == GQ_COUNT_STAR && !(d->flags & GQ_F_FINAL_MODE)) continue;
+    size_t i = 0;
+    while (i < pp.exprs.size() && pp.exprs[i] != d->aggs[a].expr) ++i;
+    if (i == pp.exprs.size()) pp.exprs.push_back(d->aggs[a].expr);
+    pp.src[a] = 1 + (int)i;
+  }
+  pp.rw = (int)align_up((size_t)(1 + pp.exprs.size()), 4);
+  pp.pcap = (nrows / np + nrows / (4 * np) + 1024 + GQ_PART_CHUNK - 1) / GQ_PART_CHUNK * GQ_PART_CHUNK;
   pp.bytes = align_up((size_t)np * 8 * GQ_PART_CURSOR_STRIDE, 256) + (size_t)np * (size_t)pp.pcap * pp.rw * 8;
   pp.on = true;
   return pp;
@@ -795,8 +824,11 @@ gq_status gq_hash_aggregate_workspace_for(const gq_batch* in, const gq_agg_desc*
   st = agg_spec(&tmp, &sp, in, d, kb, kd);
   if (st != GQ_OK) return st;
   DirectPlan dp = direct_plan(sp, d, in);
-  if (dp.step >= 0) *bytes = std::max(*bytes, dp.bytes);
-  else {
+  if (dp.step >= 0) {
+    *bytes = std::max(*bytes, dp.bytes);
+    PartPlan pp = direct_part_plan(dp, d, in->nrows);
+    if (pp.on) *bytes = align_up(*bytes, 256) + pp.bytes;
+  } else {
     PartPlan pp = part_plan(sp, d, in->nrows);
     if (pp.on) *bytes = align_up(*bytes, 256) + pp.bytes;
   }
@@ -834,6 +866,17 @@ gq_status gq_hash_aggregate(gq_ctx* ctx, gq_aggstate** state, void* d_ws, size_t
       a->dacc = (unsigned long long*)((char*)d_ws + 256);
       for (int i = 0; i < d->naggs; ++i)
         pat[i] = d->aggs[i].op == GQ_MIN ? 0x7FFFFFFFFFFFFFFFULL : d->aggs[i].op == GQ_MAX ? 0x8000000000000000ULL : 0ULL;
+      {
+        PartPlan pp = direct_part_plan(dp, d, in->nrows);
+        size_t hb = 0;
+        gq_hash_aggregate_workspace(d->max_groups, d->nkeys, d->naggs, &hb);
+        const size_t base = align_up(std::max(dp.bytes, hb), 256);   // as gq_hash_aggregate_workspace_for lays it out
+        if (pp.on && bytes >= base + pp.bytes) {   // the plan-aware workspace query made room for the record buffers
+          a->pcur = (unsigned long long*)((char*)d_ws + base);
+          a->part = (unsigned long long*)((char*)d_ws + base + align_up((size_t)pp.npart * 8 * GQ_PART_CURSOR_STRIDE, 256));
+          a->pcap = pp.pcap; a->npart = pp.npart; a->pshift = pp.pshift; a->part_rw = pp.rw; a->part_rows = in->nrows;
+        }
+      }
       e = PROF(ctx, "gq_k_init_table", gq_launch_init_table(ctx->stream, a->dacc, dp.cap + 1, dp.aw, pat, a->dacc, 0, a->dev.header, 0, ctx->num_sms));
     } else {
       const int64_t cap = agg_capacity(d->max_groups, d->nkeys);
@@ -877,8 +920,10 @@ gq_status gq_hash_aggregate(gq_ctx* ctx, gq_aggstate** state, void* d_ws, size_t
     ++ctx->launches;
     *state = a;
   }
+  DirectPlan adp;
   if (a->direct) {
     DirectPlan dp = direct_plan(sp, d, in);
+    adp = dp;
     if (dp.step < 0 || d->probes[dp.step].table->dev.slots != a->dtab.slots || dp.aw != a->daw)
       return fail(ctx, GQ_ERR_INVALID_ARG, "batch schema/desc differs from the state's first batch");
     sp.consumer = GQ_C_DIRECT; sp.direct_step = dp.step; sp.direct_aw = dp.aw; sp.direct_touch = dp.touch == d->naggs;
@@ -903,6 +948,28 @@ gq_status gq_hash_aggregate(gq_ctx* ctx, gq_aggstate** state, void* d_ws, size_t
     if (e != cudaSuccess) return cuda_fail(ctx, e, "heavy-hitter sampling");
     ctx->launches += nl;
     P.hot = a->hot;
+  }
+  if (a->part && a->direct && in->nrows >= g_part_min_rows.load() / 4) {
+    // clustered direct aggregation: pass A appends (slot, inputs) records per slice of the accumulator array, pass B applies them
+    PartPlan pp = direct_part_plan(adp, d, a->part_rows);
+    if (!pp.on || pp.rw != a->part_rw || pp.npart != a->npart) return fail(ctx, GQ_ERR_INVALID_ARG, "batch schema/desc differs from the state's first batch");
+    sp.part_rw = pp.rw; sp.part_exprs = pp.exprs; sp.part_states = 4096;
+    P.part = a->part; P.pcur = a->pcur; P.pcap = a->pcap; P.pshift = a->pshift; P.npart = a->npart;
+    cudaError_t e = cudaMemsetAsync(a->pcur, 0, (size_t)a->npart * 8 * GQ_PART_CURSOR_STRIDE, ctx->stream);
+    if (e != cudaSuccess) return cuda_fail(ctx, e, "partition cursors");
+    gq_status st2 = run_scan(ctx, sp, in, d->probes, &P);
+    if (st2 != GQ_OK) return st2;
+    GqPartParams pb;
+    memset(&pb, 0, sizeof pb);
+    pb.part = a->part; pb.pcur = a->pcur; pb.pcap = a->pcap; pb.npart = a->npart; pb.rw = a->part_rw;
+    pb.slots = a->dacc; pb.mask = 0; pb.sw = a->daw; pb.ndep = 0; pb.naggs = a->naggs;
+    for (int i = 0; i < a->naggs; ++i) { pb.op[i] = (int)sp.aggs[(size_t)i].op; pb.src[i] = pp.src[i]; }
+    pb.direct = 1; pb.touch = sp.direct_touch ? a->naggs : -1;
+    pb.err = ctx->d_err;
+    e = PROF(ctx, "gq_k_part_upsert", gq_launch_part_upsert(ctx->stream, pb, ctx->num_sms));
+    if (e != cudaSuccess) return cuda_fail(ctx, e, "clustered direct aggregation");
+    ++ctx->launches;
+    return GQ_OK;
   }
   if (a->part && !a->direct && in->nrows >= g_part_min_rows.load() / 4) {
     // radix-clustered: pass A appends records per table partition, pass B applies them partition by partition
@@ -1332,6 +1399,7 @@ gq_status gq_set_option(const char* h_name, int64_t value) {
   if (n == "part_min_table_mb") g_part_min_table_mb = value < 0 ? 256 : value;
   else if (n == "part_min_rows") g_part_min_rows = value < 0 ? (1 << 24) : value;
   else if (n == "hot_min_rows") g_hot_min_rows = value < 0 ? GQ_HOT_MIN_ROWS : value;
+  else if (n == "dpart_min_acc_mb") g_dpart_min_acc_mb = value < 0 ? GQ_DPART_OFF : value;
   else if (n == "psa_threads") g_psa_threads = (value == 512 || value == 1024) ? value : 0;
   else if (n == "psa_max_log2_partitions") g_psa_max_log2part = value < 0 ? GQ_PSA_MAX_LOG2PART : value;
   else return GQ_ERR_INVALID_ARG;
@@ -1519,6 +1587,17 @@ gq_status gq_precompile_pipeline(const gq_plan* plan, char* h_msg, size_t msg_by
     f.consumer = GQ_C_DIRECT; f.direct_step = dp.step; f.direct_aw = dp.aw; f.direct_touch = dp.touch == plan->agg.naggs; f.hot = false;
     st = precompile(f, h_msg, msg_bytes);
     if (st != GQ_OK) return st;
+    // the clustered variant (records per slice of the accumulator array): same row code + the append
+    for (int a = 0; a < 1; ++a) {
+      PartPlan pp;
+      for (int i = 0; i < plan->agg.naggs; ++i) {
+        if (plan->agg.aggs[i].op == GQ_COUNT_STAR && !(plan->agg.flags & GQ_F_FINAL_MODE)) continue;
+        if (std::find(pp.exprs.begin(), pp.exprs.end(), plan->agg.aggs[i].expr) == pp.exprs.end()) pp.exprs.push_back(plan->agg.aggs[i].expr);
+      }
+      f.part_rw = (int)align_up((size_t)(1 + pp.exprs.size()), 4); f.part_exprs = pp.exprs; f.part_states = 4096;
+      st = precompile(f, h_msg, msg_bytes);
+      if (st != GQ_OK) return st;
+    }
   }
   return precompile(sp, h_msg, msg_bytes);
 }

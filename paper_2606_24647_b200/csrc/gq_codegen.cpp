@@ -320,6 +320,23 @@ static gq_status emit_linear(Gen& g, const GqScanSpec& sp, std::ostringstream& o
     case GQ_C_DIRECT: {
       // group == matched slot of probe step direct_step (SURVEY §8(d) note on C3): no key compare, no CAS
       if (sp.direct_step < 0 || sp.direct_step >= nprobe || sp.direct_aw < nagg) { if (msg) *msg = "bad direct aggregation spec"; return GQ_ERR_INVALID_ARG; }
+      if (sp.part_rw > 0) {
+        // clustered: append (accumulator slot, aggregate inputs) to the record buffer of the slot's slice of the array
+        // (P.pshift = log2 slots per slice); pass B applies the records slice by slice. Rows that do not fit their
+        // buffer fall through to the in-place REDs below.
+        const int rw = sp.part_rw;
+        o << "  u64 pidx[GQ_R], ppart[GQ_R];\n";
+        o << "  " << LOOP << "{\n    pidx[j] = ~0ULL; ppart[j] = 0;\n    if (live[j]) {\n"
+          << "      ppart[j] = pi" << sp.direct_step << "[j] >> P.pshift;\n      pidx[j] = (u64)gq_part_reserve(P, cx.part_st, ppart[j]);\n    }\n  }\n";
+        o << "  " << LOOP << "if (live[j] && pidx[j] != ~0ULL) {\n    u64* rec = P.part + (ppart[j] * (u64)P.pcap + pidx[j]) * " << rw << ";\n";
+        std::vector<std::string> words;
+        words.push_back("pi" + std::to_string(sp.direct_step) + "[j]");
+        for (int e : sp.part_exprs) words.push_back("(u64)e" + std::to_string(e) + "[j]");
+        while ((int)words.size() < rw) words.push_back("0ULL");
+        for (int w = 0; w < rw; w += 4)
+          o << "    gq_st256(rec + " << w << ", " << words[(size_t)w] << ", " << words[(size_t)w + 1] << ", " << words[(size_t)w + 2] << ", " << words[(size_t)w + 3] << ");\n";
+        o << "    live[j] = false;\n  }\n";
+      }
       o << "  " << LOOP << "if (live[j]) {\n    u64* acc = P.dacc + pi" << sp.direct_step << "[j] * " << sp.direct_aw << ";\n";
       for (int a = 0; a < nagg; ++a)
         o << "    gq_red(" << (int)sp.aggs[(size_t)a].op << ", acc + " << a << ", " << aggval(sp.aggs[(size_t)a]) << ");\n";

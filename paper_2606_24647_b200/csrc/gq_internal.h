@@ -222,6 +222,7 @@ struct GqPartParams {
   unsigned long long* slots; unsigned long long mask; int sw; int ndep; int naggs;
   int op[GQ_MAX_AGGS]; int src[GQ_MAX_AGGS];   // src = record word of the aggregate's input, -1 = COUNT(*)
   int check_dep;
+  int direct, touch;   // direct: record word 0 = accumulator slot of `slots` (sw words per slot, aggregate a at word a); touch = hidden COUNT word or -1
   int* err;
 };
 cudaError_t gq_launch_part_upsert(cudaStream_t s, const GqPartParams& p, int num_sms);
@@ -243,6 +244,7 @@ cudaError_t gq_launch_hot_keys(cudaStream_t s, const void* keycol, int dtype, lo
                                int max_hot, int num_sms, int* nlaunches);
 // ---- partitioned shared-memory aggregation (gq_psa_kernel.cuh, gq_psa.cu) ----
 #define GQ_MAX_SMS 160               // workspace sizing bound for the per-CTA chunk ranges of pass A
+#define GQ_DPART_OFF (1LL << 40)      // accumulator arrays smaller than this many MB are never clustered: off by default
 #define GQ_PSA_MAX_LOG2PART 14        // default cap on pass-A partitions (planner knob "psa_max_log2_partitions")
 #define GQ_PSA_GID_BITS 26           // directory entry = chunk id | records used << 26
 struct GqPsaParams {                 // must match gq_psa_kernel.cuh

@@ -382,6 +382,24 @@ __global__ void __launch_bounds__(GQ_PART_THREADS) gq_k_part_upsert(const __grid
         key[u] = w[u][0];
         live[u] = live[u] && key[u] != GQ_EMPTY_KEY;       // padding of a partly used chunk
       }
+      if (P.direct) {   // clustered direct aggregation: word 0 of a record IS the accumulator slot
+#pragma unroll
+        for (int u = 0; u < GQ_PART_U; ++u) {
+          if (!live[u]) continue;
+          const i64 r = r0 + (i64)u * GQ_PART_THREADS + threadIdx.x;
+          const u64* rec = base + r * P.rw;
+          u64* slot = P.slots + key[u] * P.sw;
+          for (int a = 0; a < P.naggs; ++a) {
+            const int sa = P.src[a];
+            const i64 v = sa < 0 ? 1 : sa == 1 ? (i64)w[u][1] : sa == 2 ? (i64)w[u][2] : sa == 3 ? (i64)w[u][3] : (i64)__ldg(rec + sa);
+            if (P.op[a] == GQ_MIN) atomicMin((i64*)(slot + a), v);
+            else if (P.op[a] == GQ_MAX) atomicMax((i64*)(slot + a), v);
+            else atomicAdd(slot + a, (u64)v);
+          }
+          if (P.touch >= 0) atomicAdd(slot + P.touch, 1ULL);
+        }
+        continue;
+      }
 #pragma unroll
       for (int u = 0; u < GQ_PART_U; ++u) {
         u64 x = key[u];

@@ -487,6 +487,34 @@ def test_partitioned_shared_memory_aggregation_hot_keys_and_sub_passes(ctx, forc
         gq.set_option("hot_min_rows", -1); gq.set_option("psa_max_log2_partitions", -1); gq.set_option("psa_threads", 0)
 
 
+def test_clustered_direct_aggregation(ctx, force_partition):
+    # direct aggregation (group = matched slot / rank of a probed unique table) with its REDs clustered by slice of the
+    # accumulator array: records appended per slice by the scan, applied slice by slice — hashed and direct-address tables,
+    # a dependent key, a plan without COUNT (hidden touch word), MIN/MAX, overflowing record buffers (in-place fallback)
+    from paper_2606_24647_b200 import gq
+    rng = np.random.default_rng(16)
+    try:
+        gq.set_option("dpart_min_acc_mb", 0)
+        for aggs in ([("sum", 0), ("count",)], [("sum", 0), ("min", 0), ("max", 0)]):
+            plan = _join_plan(120_000, 700_001, rng, aggs, with_dep=True)
+            l0 = ctx.launch_count()
+            run(plan, ctx)
+            assert ctx.launch_count() - l0 == 6      # join table init, build, accumulator init, scan + append, apply, finalise
+            dense = dict(plan, builds=[dict(plan["builds"][0], dense_range=(int(plan["builds"][0]["table"][0].min()),
+                                                                           int(plan["builds"][0]["table"][0].max())))])
+            run(dense, ctx)
+        # one key receives 70 % of the rows: its slice's record buffer overflows, the rest is aggregated in place
+        plan = _join_plan(50_000, 600_000, rng, [("sum", 0), ("count",)])
+        hot = plan["builds"][0]["table"][0][plan["builds"][0]["table"][2] == 1][0]
+        fk = plan["table"][0].copy()
+        fk[rng.random(len(fk)) < 0.7] = hot
+        plan["table"][0] = fk
+        exp, got = run(plan, ctx)
+        assert int(got["cols"][-1].max()) > 300_000
+    finally:
+        gq.set_option("dpart_min_acc_mb", -1)
+
+
 def test_partitioned_aggregation_streams_batches(ctx, force_partition):
     import gqrun
     plan = plans.plan_c5(datagen.make_config(5, scale=0.004))
