@@ -55,6 +55,25 @@ __device__ __forceinline__ void gq_fin_emit(const GqFinal& F, i64 row, i64 key, 
 }
 #endif
 
+#if GQ_FUSED_FINAL
+// Aggregate words of the context-owned merge table: a representation whose identity is 0 for every operator.
+__device__ __forceinline__ u64 gq_gt_enc(const int OP, i64 v) {
+  if (OP == GQ_OP_MAX) return (u64)v ^ 0x8000000000000000ULL;          // unsigned order == signed order; INT64_MIN -> 0
+  if (OP == GQ_OP_MIN) return ~((u64)v ^ 0x8000000000000000ULL);       // reversed: the maximum of these is the minimum
+  return (u64)v;
+}
+__device__ __forceinline__ i64 gq_gt_dec(const int OP, u64 w) {
+  if (OP == GQ_OP_MAX) return (i64)(w ^ 0x8000000000000000ULL);
+  if (OP == GQ_OP_MIN) return (i64)(~w ^ 0x8000000000000000ULL);
+  return (i64)w;
+}
+__device__ __forceinline__ u32 gq_atom_add_acq_rel(u32* p, u32 v) {
+  u32 old;
+  asm volatile("atom.acq_rel.gpu.global.add.u32 %0, [%1], %2;" : "=r"(old) : "l"(p), "r"(v) : "memory");
+  return old;
+}
+#endif
+
 #if GQ_CONSUMER == GQ_C_LOWCARD
 // Reduces the GQ_NT private cells of up to four pairs p = group * GQ_NAGG + a (p0, p0 + GQ_NWARP, ...) over the warp's
 // lanes, the four chains interleaved (the loads of one pair alone are a dependent LDS/combine chain); every lane gets
@@ -173,7 +192,7 @@ extern "C" __global__ void __launch_bounds__(GQ_NT + 32, 1) gq_scan(const __grid
         *P.fin.ticket = 0;
 #if GQ_CONSUMER == GQ_C_LOWCARD
         P.fin.gtab[0] = 0;
-        for (int i = 0; i < GQ_GTAB_SLOTS; ++i) P.fin.gtab[32 + i * 16] = 0;
+        for (int i = 0; i < GQ_GTAB_SLOTS * 16; ++i) P.fin.gtab[32 + i] = 0;
 #endif
       }
     }
@@ -321,50 +340,57 @@ extern "C" __global__ void __launch_bounds__(GQ_NT + 32, 1) gq_scan(const __grid
       u32 h = (u32)gq_hash(key, 64 - 6);
       bool done = false;
 #if GQ_LC_KEY32
-      // packed keys narrower than 32 bits travel IN the state word (2 | key << 32): one CAS round trip tells a CTA whether
-      // it claimed the slot, must wait for its publication, found its key, or has to look at the next slot
+      // Packed keys narrower than 32 bits travel IN the slot's first word (2 | key << 32), and the slot's aggregate words
+      // are kept in a form whose identity is ZERO for every operator (gq_gt_enc: MIN/MAX as unsigned maxima of the
+      // biased / complemented value), so a zeroed table is a valid empty table for any plan: ONE CAS round trip tells a
+      // CTA that the slot is (now) its key's and it can RED straight away — no claim/publish wait.
       const u64 mine = 2ULL | ((u64)GQ_LC_K32(key) << 32);
-#endif
       for (int n = 0; n < GQ_GTAB_SLOTS && !done; ++n, h = (h + 1) & (GQ_GTAB_SLOTS - 1)) {
         u64* s = gt + 32 + h * 16;
-#if GQ_LC_KEY32
-        u64 st = atomicCAS(s, 0ULL, 1ULL);
+        const u64 st = atomicCAS(s, 0ULL, mine);
+        if (st != 0 && st != mine) continue;               // another key's slot
+        if (st == 0) s[1] = (u64)key;                      // (read by the last CTA only, after every CTA's fence + ticket)
+#pragma unroll
+        for (int a = 0; a < GQ_NAGG; ++a) {
+          const u64 v = gq_gt_enc(GQ_AGG_OP(a), fin[tid * GQ_NAGG + a]);
+          if (GQ_AGG_OP(a) == GQ_OP_MIN || GQ_AGG_OP(a) == GQ_OP_MAX) atomicMax(s + 2 + a, v);
+          else atomicAdd(s + 2 + a, v);
+        }
+        done = true;
+      }
 #else
+      for (int n = 0; n < GQ_GTAB_SLOTS && !done; ++n, h = (h + 1) & (GQ_GTAB_SLOTS - 1)) {
+        u64* s = gt + 32 + h * 16;
         u64 st = gq_ld_acquire(s);
         if (st == 0) st = atomicCAS(s, 0ULL, 1ULL);
-#endif
         if (st == 0) {                                     // claimed: store key and values, then publish
           s[1] = (u64)key;
 #pragma unroll
-          for (int a = 0; a < GQ_NAGG; ++a) s[2 + a] = (u64)fin[tid * GQ_NAGG + a];
-#if GQ_LC_KEY32
-          gq_st_release(s, mine);
-#else
+          for (int a = 0; a < GQ_NAGG; ++a) s[2 + a] = gq_gt_enc(GQ_AGG_OP(a), fin[tid * GQ_NAGG + a]);
           gq_st_release(s, 2ULL);
-#endif
-          atomicAdd(gt, 1ULL);                             // groups claimed (fire and forget; the last CTA checks the bound)
           done = true;
           break;
         }
         while (st == 1) st = gq_ld_acquire(s);             // being published by another CTA
-#if GQ_LC_KEY32
-        if (st == mine) {
-#else
         if (s[1] == (u64)key) {
-#endif
 #pragma unroll
-          for (int a = 0; a < GQ_NAGG; ++a) gq_red(GQ_AGG_OP(a), s + 2 + a, fin[tid * GQ_NAGG + a]);
+          for (int a = 0; a < GQ_NAGG; ++a) {
+            const u64 v = gq_gt_enc(GQ_AGG_OP(a), fin[tid * GQ_NAGG + a]);
+            if (GQ_AGG_OP(a) == GQ_OP_MIN || GQ_AGG_OP(a) == GQ_OP_MAX) atomicMax(s + 2 + a, v);
+            else atomicAdd(s + 2 + a, v);
+          }
           done = true;
         }
       }
+#endif
       if (!done) gq_set_err(P.err, GQ_E_CAPACITY);
     }
     gq_consumer_barrier();
-    if (tid == 0) { __threadfence(); cx.lc_n[3] = (atomicAdd(P.fin.ticket, 1u) == gridDim.x - 1); }
+    // ticket: release (this CTA's table updates, ordered before by the barrier) and acquire (the last CTA reads the table)
+    if (tid == 0) cx.lc_n[3] = (gq_atom_add_acq_rel(P.fin.ticket, 1u) == gridDim.x - 1);
     gq_consumer_barrier();
     if (((volatile int*)cx.lc_n)[3]) {
-      // (every CTA fenced its table updates before taking its ticket; the table is read with ld.cg)
-      __threadfence();
+      // (the table is read with ld.cg, after thread 0's acquire and the CTA barrier)
       if (tid < GQ_GTAB_SLOTS) {                            // warps 0 and 1: one slot per lane
         u64* s = gt + 32 + tid * 16;
         i64 wd[2 + GQ_NAGG];                                // state, key and values of the slot: all loads in flight together
@@ -376,9 +402,12 @@ extern "C" __global__ void __launch_bounds__(GQ_NT + 32, 1) gq_scan(const __grid
         asm volatile("bar.sync 2, 64;" ::: "memory");
         const int row = (tid >= 32 ? ((volatile int*)cx.lc_n)[2] : 0) + __popc(m & ((1u << lane) - 1u));
         if (have) {
+#pragma unroll
+          for (int a = 0; a < GQ_NAGG; ++a) wd[2 + a] = gq_gt_dec(GQ_AGG_OP(a), (u64)wd[2 + a]);
           if (row < P.fin.out_capacity) gq_fin_emit(P.fin, row, wd[1], wd + 2);
           else gq_set_err(P.err, GQ_E_CAPACITY);
-          s[0] = 0;
+#pragma unroll
+          for (int i = 0; i < 2 + GQ_NAGG; ++i) s[i] = 0;   // a zeroed slot is an empty slot with identity aggregates
         }
         if (tid == 63) {
           if (row + (have ? 1 : 0) > GQ_LC_G) gq_set_err(P.err, GQ_E_CAPACITY);   // more distinct keys than max_groups
