@@ -337,10 +337,11 @@ static gq_status emit_linear(Gen& g, const GqScanSpec& sp, std::ostringstream& o
           o << "    gq_st256(rec + " << w << ", " << words[(size_t)w] << ", " << words[(size_t)w + 1] << ", " << words[(size_t)w + 2] << ", " << words[(size_t)w + 3] << ");\n";
         o << "    live[j] = false;\n  }\n";
       }
+      o << "  const u64 keep = gq_policy_evict_last();\n";
       o << "  " << LOOP << "if (live[j]) {\n    u64* acc = P.dacc + pi" << sp.direct_step << "[j] * " << sp.direct_aw << ";\n";
       for (int a = 0; a < nagg; ++a)
-        o << "    gq_red(" << (int)sp.aggs[(size_t)a].op << ", acc + " << a << ", " << aggval(sp.aggs[(size_t)a]) << ");\n";
-      if (sp.direct_touch) o << "    gq_red(3, acc + " << nagg << ", 1);\n";
+        o << "    gq_red_hint(" << (int)sp.aggs[(size_t)a].op << ", acc + " << a << ", " << aggval(sp.aggs[(size_t)a]) << ", keep);\n";
+      if (sp.direct_touch) o << "    gq_red_hint(3, acc + " << nagg << ", 1, keep);\n";
       o << "  }\n";
       break;
     }

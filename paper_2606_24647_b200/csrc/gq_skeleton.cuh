@@ -513,6 +513,12 @@ __device__ __forceinline__ void gq_red(const int OP, u64* p, i64 v) {
   else if (OP == GQ_OP_MIN) atomicMin((i64*)p, v);
   else atomicMax((i64*)p, v);
 }
+// The same with an L2 cache policy (direct aggregation: the accumulator array should outlive the streamed input in L2).
+__device__ __forceinline__ void gq_red_hint(const int OP, u64* p, i64 v, u64 pol) {
+  if (OP == GQ_OP_SUM || OP == GQ_OP_COUNT) asm volatile("red.global.add.L2::cache_hint.u64 [%0], %1, %2;" ::"l"(p), "l"(v), "l"(pol) : "memory");
+  else if (OP == GQ_OP_MIN) asm volatile("red.global.min.L2::cache_hint.s64 [%0], %1, %2;" ::"l"(p), "l"(v), "l"(pol) : "memory");
+  else asm volatile("red.global.max.L2::cache_hint.s64 [%0], %1, %2;" ::"l"(p), "l"(v), "l"(pol) : "memory");
+}
 __device__ __forceinline__ i64 gq_combine(const int OP, i64 a, i64 b) {
   if (OP == GQ_OP_SUM || OP == GQ_OP_COUNT) return gq_add(a, b);
   if (OP == GQ_OP_MIN) return gq_min(a, b);
