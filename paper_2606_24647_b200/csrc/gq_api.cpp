@@ -1126,11 +1126,9 @@ gq_status gq_hash_aggregate_finish(gq_ctx* ctx, gq_aggstate* a, void* const* out
 gq_status gq_aggstate_destroy(gq_aggstate* a) { if (!a) return GQ_ERR_INVALID_ARG; delete a; return GQ_OK; }
 
 // ------------------------------------------------------------------------------------------------ fused pipeline
-// Scratch of the finaliser fused into the scan kernel: per-CTA partial groups + group counts (<= 256 CTAs).
-static size_t fused_scratch_bytes(const gq_agg_desc* d) {
-  const size_t g = d->nkeys == 0 ? 1 : (size_t)std::min<int64_t>(64, std::max<int64_t>(1, d->max_groups));
-  return align_up(256 * (g * (1 + (size_t)d->naggs) + 1) * 8, 256);
-}
+// Scratch of the finaliser fused into the scan kernel: the per-CTA partial aggregates of a key-less plan (<= 256 CTAs).
+// (Low-cardinality plans merge through the context-owned table instead.)
+static size_t fused_scratch_bytes(const gq_agg_desc* d) { return align_up(256 * (size_t)d->naggs * 8, 256); }
 
 // Offsets inside a pipeline workspace: [aggregation state][top-k scratch][fused-finaliser scratch][partitioned aggregation]
 struct PipeLayout { size_t aggb = 0, topk_off = 0, fused_off = 0, psa_off = 0, total = 0; PsaPlan psa; };
