@@ -92,7 +92,8 @@ enum {
                                       keys: the slot index of direct aggregation) ("the query planner should choose the
                                       operator implementation based on ... the expected input"). Requires
                                       GQ_F_UNIQUE_KEYS. VERIFIED on device: a key outside the range sets the sticky
-                                      GQ_ERR_KEY_RANGE, a repeated key GQ_ERR_DUPLICATE_KEY */
+                                      GQ_ERR_KEY_RANGE at once, a repeated key GQ_ERR_DUPLICATE_KEY at
+                                      gq_hash_build_finish (fewer member keys than rows inserted) */
 };
 enum { GQ_MAX_PREDS = 16, GQ_MAX_TOKS = 32, GQ_MAX_EXPRS = 8, GQ_MAX_AGGS = 8, GQ_MAX_PROBES = 4, GQ_MAX_PAYLOAD = 3,
        GQ_MAX_KEYS = 2, GQ_MAX_COLS = 32, GQ_MAX_TOPK = 32, GQ_SIDE_SLOTS = 64 };

@@ -435,17 +435,18 @@ __device__ __forceinline__ void gq_upsert_rows(const GqTableDev& T, const i64 (&
 // ---- direct-address join tables (GQ_F_DENSE_KEYS; SURVEY 8(f) NEXT-3 "dense-key array mode"): the planner
 // declared the build keys' range, so slot = key - key_min. The membership bitmap is an array of 64-bit entries, one per
 // 32 keys: low word = the 32 membership bits, high word = the number of member keys BEFORE this entry (filled in by
-// gq_hash_build_finish). HashBuild sets a bit (atomicOr: a bit found set is a duplicate key) and stores the payload row at
-// slot; HashProbe is ONE 8-byte load from an L2-resident array (15 M keys: 3.75 MB) — the probes that miss never reach
+// gq_hash_build_finish). HashBuild sets a bit (RED.OR) and stores the payload row at slot (a duplicate key shows at finish:
+// fewer member keys than rows inserted); HashProbe is ONE 8-byte load from an L2-resident array (15 M keys: 3.75 MB) — the probes that miss never reach
 // DRAM — plus, on a hit, the payload row. The RANK of the key among the member keys (prefix + popcount) is the slot index
 // handed to direct aggregation, so its accumulator array has one slot per build row, not per key of the range.
 template <int NPAY>
 __device__ __forceinline__ bool gq_dense_insert(const GqTableDev& T, i64 key, const i64* pay, int* err) {
   const u64 idx = (u64)key - (u64)T.base;
   if (idx > T.mask) { gq_set_err(err, GQ_E_KEYRANGE); return false; }
-  const u32 bit = 1u << (u32)(idx & 31);
-  const u32 old = atomicOr((u32*)(T.side + (idx >> 5)), bit);   // (little-endian: the low word of the entry)
-  if (old & bit) { gq_set_err(err, GQ_E_DUPLICATE); return false; }
+  // Fire-and-forget RED.OR (little-endian: the low word of the entry): no round trip per row. A repeated key sets a bit
+  // that is already set, so the member count computed by gq_hash_build_finish falls short of the rows inserted — the
+  // duplicate is reported there (GQ_ERR_DUPLICATE_KEY), not here.
+  atomicOr((u32*)(T.side + (idx >> 5)), 1u << (u32)(idx & 31));
 #pragma unroll
   for (int p = 0; p < NPAY; ++p) T.slots[idx * NPAY + p] = (u64)pay[p];
   return true;

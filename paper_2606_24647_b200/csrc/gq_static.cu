@@ -502,6 +502,8 @@ __global__ void __launch_bounds__(GQ_RANK_THREADS) gq_k_dense_rank_apply(u64* en
     const i64 total = (i64)(rank0 + c);
     header[2] = total;
     if (total > max_rows) atomicCAS(err, 0, (int)GQ_ERR_CAPACITY);   // more build rows than max_build_rows promised
+    // header[0] = rows the build kernels inserted: more rows than member keys means some key was inserted twice
+    if (*(volatile i64*)&header[0] > total) atomicCAS(err, 0, (int)GQ_ERR_DUPLICATE_KEY);
   }
 }
 cudaError_t gq_launch_dense_rank(cudaStream_t s, unsigned long long* entries, long long nwords, unsigned* totals, long long base,
