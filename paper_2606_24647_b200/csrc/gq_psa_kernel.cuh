@@ -25,8 +25,9 @@
 
 #define GQ_PSA_NW (GQ_PSA_THREADS / 32)            // GQ_PSA_THREADS, GQ_PSA_U (chunks in flight per warp): prelude
 #define GQ_PSA_SLOTS (1 << GQ_PSA_LOG2SLOTS)
-// Groups a table takes before it gives up (load 0.75). The count is checked once per warp and row, so up to
-// GQ_PSA_THREADS further claims may be in flight: a table that fills up completely is caught by the probe loop's guard.
+// Groups a table takes before it gives up (load 0.75). The count is checked once per warp and iteration, so up to
+// GQ_PSA_U x GQ_PSA_THREADS further claims may be in flight: a table that fills up completely is caught by the probe
+// loop's guard.
 #define GQ_PSA_LIMIT (GQ_PSA_SLOTS - GQ_PSA_SLOTS / 4)
 #define GQ_PSA_SW GQ_TARGET_SW
 #define GQ_PSA_RW GQ_PART_RW
@@ -70,7 +71,7 @@ __device__ __forceinline__ u64 gq_psa_init_word(int q) {    // word q of an empt
 // executes it once per round, not once per lane; new groups are counted with one atomic per warp; the updates are
 // straight-line code (SUM/COUNT: a 32-bit ATOMS.ADD and, only when there is a carry or a high word, a second one;
 // MIN/MAX: compare first, CAS only to improve).
-__device__ __forceinline__ void gq_psa_row(u64* tab, u32* ctl, const u64 (&w)[GQ_PSA_RW], bool act, u64 h, int tshift, int* err) {
+__device__ __forceinline__ void gq_psa_row(u64* tab, u32* ctl, const u64 (&w)[GQ_PSA_RW], bool act, u64 h, int tshift, int* err, u32* nwon) {
   const u64 key = w[0];
   u64* slot = nullptr;
   bool won = false, side_won = false;
@@ -78,30 +79,28 @@ __device__ __forceinline__ void gq_psa_row(u64* tab, u32* ctl, const u64 (&w)[GQ
     side_won = atomicExch(&ctl[GQ_PSA_SIDE], 1u) == 0u;
     slot = tab + (size_t)GQ_PSA_SLOTS * GQ_PSA_SW;
   }
-  bool pend = act && slot == nullptr;
+  // (the overflow flag is read once per row, not per probed slot: a claim made after the table has given up is harmless,
+  // the item is redone anyway)
+  bool pend = act && slot == nullptr && !((volatile u32*)ctl)[GQ_PSA_OVF];
   u32 i = (u32)(h >> (tshift - GQ_PSA_LOG2SLOTS)) & (GQ_PSA_SLOTS - 1);
-  for (int n = 0; __any_sync(0xffffffffu, pend); ++n) {
+  int n = 0;
+  for (; n <= GQ_PSA_SLOTS && __any_sync(0xffffffffu, pend); ++n) {
     if (pend) {
       u64* s = tab + (size_t)i * GQ_PSA_SW;
       const u64 k = *(volatile u64*)s;
       if (k == key) { slot = s; pend = false; }
-      else if (k == GQ_EMPTY) {
-        if (((volatile u32*)ctl)[GQ_PSA_OVF]) pend = false;                 // the table has given up: the item is redone
-        else {
+      else {
+        if (k == GQ_EMPTY) {
           const u64 prev = atomicCAS(s, GQ_EMPTY, key);
           if (prev == GQ_EMPTY) { slot = s; won = true; pend = false; }
           else if (prev == key) { slot = s; pend = false; }
-          else i = (i + 1) & (GQ_PSA_SLOTS - 1);
         }
-      } else i = (i + 1) & (GQ_PSA_SLOTS - 1);
-      if (n > GQ_PSA_SLOTS) { ((volatile u32*)ctl)[GQ_PSA_OVF] = 1u; pend = false; }
+        if (pend) i = (i + 1) & (GQ_PSA_SLOTS - 1);
+      }
     }
   }
-  const u32 wm = __ballot_sync(0xffffffffu, won);
-  if (wm != 0u && (threadIdx.x & 31) == (u32)(__ffs(wm) - 1)) {
-    const u32 c = (u32)__popc(wm);
-    if (atomicAdd(&ctl[GQ_PSA_NG], c) + c > (u32)GQ_PSA_LIMIT) ((volatile u32*)ctl)[GQ_PSA_OVF] = 1u;
-  }
+  if (pend) ((volatile u32*)ctl)[GQ_PSA_OVF] = 1u;       // walked the whole table: it is full
+  *nwon += won ? 1u : 0u;                               // counted once per warp and iteration by the caller
   if (slot != nullptr) {
 #if GQ_NDEP
 #if GQ_CHECK_DEP
@@ -184,7 +183,8 @@ extern "C" __global__ void __launch_bounds__(GQ_PSA_THREADS, 1) gq_psa(const __g
     const u32 item = ctl[GQ_PSA_ITEM];
     if (item >= nitems) break;
     const u32 part = P.items[item], seg = P.item_seg[item] & 0xFFFFFFu, sub = P.item_seg[item] >> 24;
-    const int tshift = P.hshift - P.log2sub;            // the table index comes from the hash bits below partition and sub-pass
+    const int log2sub = P.log2sub;
+    const int tshift = P.hshift - log2sub;              // the table index comes from the hash bits below partition and sub-pass
     const u32 p0 = P.pstart[part], p1 = P.pstart[part + 1];
     const bool split = (p1 - p0) > P.seg_chunks;      // this item is one segment of a heavy partition
     const u32 c0 = split ? p0 + seg * P.seg_chunks : p0;
@@ -222,15 +222,20 @@ extern "C" __global__ void __launch_bounds__(GQ_PSA_THREADS, 1) gq_psa(const __g
                            : "=l"(w[u][q]), "=l"(w[u][q + 1]), "=l"(w[u][q + 2]), "=l"(w[u][q + 3]) : "l"(r + q));
           }
         }
+        u32 nwon = 0;
 #pragma unroll
         for (int u = 0; u < GQ_PSA_U; ++u) {
           const u64 key = w[u][0];
           const u64 h = gq_hash((i64)key, 0);
           bool act = live[u];
-          if (P.log2sub) act = act && (u32)((h >> tshift) & ((1u << P.log2sub) - 1u)) == sub;   // another sub-pass owns this key
+          if (log2sub) act = act && (u32)((h >> tshift) & ((1u << log2sub) - 1u)) == sub;   // another sub-pass owns this key
           if (filt) { const u64 h2 = gq_psa_mix(key); act = act && h2 >= lo && h2 <= hi; }
-          gq_psa_row(tab, ctl, w[u], act, h, tshift, P.err);
+          gq_psa_row(tab, ctl, w[u], act, h, tshift, P.err, &nwon);
         }
+        // new groups of this warp and iteration: one atomic (up to GQ_PSA_U x GQ_PSA_THREADS claims may be uncounted when
+        // the bound is checked; a table that fills up meanwhile is caught by the probe loop's guard)
+        nwon = __reduce_add_sync(0xffffffffu, nwon);
+        if (nwon != 0u && lane == 0 && atomicAdd(&ctl[GQ_PSA_NG], nwon) + nwon > (u32)GQ_PSA_LIMIT) ((volatile u32*)ctl)[GQ_PSA_OVF] = 1u;
       }
       __syncthreads();
       if (ctl[GQ_PSA_OVF]) {
