@@ -168,6 +168,22 @@ __device__ __forceinline__ void gq_psa_emit(const GqFinal& F, i64 row, u64 key, 
   }
 }
 
+// The records of GQ_PSA_U chunks (directory entries e: chunk id | records used << GQ_PSA_GID_BITS), one record per lane.
+__device__ __forceinline__ void gq_psa_load(const GqPsaParams& P, const u32 (&e)[GQ_PSA_U], u64 (&w)[GQ_PSA_U][GQ_PSA_RW], bool (&live)[GQ_PSA_U], int lane) {
+#pragma unroll
+  for (int u = 0; u < GQ_PSA_U; ++u) {
+    live[u] = (u32)lane < (e[u] >> GQ_PSA_GID_BITS);
+    const u64* r = P.rec + ((u64)(e[u] & ((1u << GQ_PSA_GID_BITS) - 1u)) * GQ_PART_CHUNK + lane) * GQ_PSA_RW;
+#pragma unroll
+    for (int q = 0; q < GQ_PSA_RW; q += 4) {
+      w[u][q] = w[u][q + 1] = w[u][q + 2] = w[u][q + 3] = 0;
+      if (live[u])
+        asm volatile("ld.global.nc.L1::no_allocate.v4.u64 {%0, %1, %2, %3}, [%4];"
+                     : "=l"(w[u][q]), "=l"(w[u][q + 1]), "=l"(w[u][q + 2]), "=l"(w[u][q + 3]) : "l"(r + q));
+    }
+  }
+}
+
 extern "C" __global__ void __launch_bounds__(GQ_PSA_THREADS, 1) gq_psa(const __grid_constant__ GqPsaParams P) {
   extern __shared__ __align__(128) unsigned char gq_smem[];
   u64* tab = (u64*)gq_smem;
@@ -208,26 +224,27 @@ extern "C" __global__ void __launch_bounds__(GQ_PSA_THREADS, 1) gq_psa(const __g
       // (the directory entries of the NEXT iteration are fetched while this one is processed: the record addresses depend on
       // them, and two dependent global round trips per iteration were 18 % of the kernel's stall samples)
       u32 en[GQ_PSA_U];
+      u64 wn[GQ_PSA_U][GQ_PSA_RW];                       // records of the NEXT iteration, loaded while this one is processed
+      bool liven[GQ_PSA_U];
+      const u32 stride = GQ_PSA_NW * GQ_PSA_U, b0 = c0 + warp * GQ_PSA_U;
 #pragma unroll
-      for (int u = 0; u < GQ_PSA_U; ++u) { const u32 ci = c0 + warp * GQ_PSA_U + u; en[u] = ci < c1 ? __ldg(P.plist + ci) : 0u; }
-      for (u32 b = c0 + warp * GQ_PSA_U; b < c1; b += GQ_PSA_NW * GQ_PSA_U) {
+      for (int u = 0; u < GQ_PSA_U; ++u) { const u32 ci = b0 + u; en[u] = ci < c1 ? __ldg(P.plist + ci) : 0u; }
+      gq_psa_load(P, en, wn, liven, lane);
+#pragma unroll
+      for (int u = 0; u < GQ_PSA_U; ++u) { const u32 ci = b0 + stride + u; en[u] = ci < c1 ? __ldg(P.plist + ci) : 0u; }
+      for (u32 b = b0; b < c1; b += stride) {
         if (((volatile u32*)ctl)[GQ_PSA_OVF]) break;
         u64 w[GQ_PSA_U][GQ_PSA_RW];
         bool live[GQ_PSA_U];
 #pragma unroll
         for (int u = 0; u < GQ_PSA_U; ++u) {
-          const u32 e = en[u];
-          const u32 cn = b + GQ_PSA_NW * GQ_PSA_U + u;
-          en[u] = cn < c1 ? __ldg(P.plist + cn) : 0u;
-          live[u] = (u32)lane < (e >> GQ_PSA_GID_BITS);
-          const u64* r = P.rec + ((u64)(e & ((1u << GQ_PSA_GID_BITS) - 1u)) * GQ_PART_CHUNK + lane) * GQ_PSA_RW;
-          if (live[u]) {
+          live[u] = liven[u];
 #pragma unroll
-            for (int q = 0; q < GQ_PSA_RW; q += 4)
-              asm volatile("ld.global.nc.L1::no_allocate.v4.u64 {%0, %1, %2, %3}, [%4];"
-                           : "=l"(w[u][q]), "=l"(w[u][q + 1]), "=l"(w[u][q + 2]), "=l"(w[u][q + 3]) : "l"(r + q));
-          }
+          for (int q = 0; q < GQ_PSA_RW; ++q) w[u][q] = wn[u][q];
         }
+        gq_psa_load(P, en, wn, liven, lane);               // iteration b + stride (entries fetched one iteration ago)
+#pragma unroll
+        for (int u = 0; u < GQ_PSA_U; ++u) { const u32 cn = b + 2 * stride + u; en[u] = cn < c1 ? __ldg(P.plist + cn) : 0u; }
         u32 nwon = 0;
 #pragma unroll
         for (int u = 0; u < GQ_PSA_U; ++u) {
