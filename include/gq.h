@@ -283,6 +283,9 @@ int32_t gq_profile_read(gq_ctx*, char* h_names, size_t names_bytes, float* h_ms,
  *   "psa_max_log2_partitions"  cap on the pass-A partitions of the partitioned shared-memory aggregation (default 14);
  *                        key ranges beyond it are resolved by sub-passes of pass B
  *   "psa_threads"        512 / 1024 threads per CTA in pass B (default 1024), 0 = default
+ *   "psa_cluster"        2 (default): pass A of the partitioned shared-memory aggregation runs as thread-block clusters of
+ *                        two CTAs that share the open record chunk of every partition through distributed shared
+ *                        memory (half as many partly written record lines compete for L2); 1 = every CTA on its own
  *   "dpart_min_acc_mb"   direct aggregations whose accumulator array is at least this large cluster their updates by
  *                        slice of the array (records appended by the scan, applied slice by slice); default: never
  *                        (measured slower on C3), a planner may enable it for arrays far beyond L2

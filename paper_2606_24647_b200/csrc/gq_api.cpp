@@ -172,7 +172,7 @@ std::string signature(const GqScanSpec& sp) {
   put(sp.lc_cap); put(sp.lc_key_bits); put(sp.target_sw); put(sp.build_key_col);
   for (int c : sp.payload_cols) put(c);
   put(sp.unique); put(sp.dense_target); put(sp.hot); put(sp.check_dep); put(sp.fused_final); put(sp.direct_step); put(sp.direct_aw); put(sp.direct_touch);
-  put(sp.part_rw); put(sp.part_states); for (int e : sp.part_exprs) put(e);
+  put(sp.part_rw); put(sp.part_states); put(sp.cluster); for (int e : sp.part_exprs) put(e);
   s += 'c';
   std::vector<long long> kv; std::vector<int> ki;
   collect_consts(sp, &kv, &ki);
@@ -240,6 +240,20 @@ gq_status get_psa_kernel_info(const GqScanSpec& sp, int log2slots, const int* sr
   return GQ_OK;
 }
 
+// CTAs of a persistent grid of clusters that are co-resident (a cluster of 4 does not pack all 148 SMs of a B200).
+int cluster_grid(gq_ctx* ctx, const GqKernel& kern) {
+  cudaLaunchConfig_t cfg = {};
+  cfg.gridDim = dim3((unsigned)(ctx->num_sms / kern.cluster * kern.cluster)); cfg.blockDim = dim3((unsigned)kern.threads);
+  cfg.dynamicSmemBytes = (size_t)kern.smem_bytes;
+  cudaLaunchAttribute at[1];
+  at[0].id = cudaLaunchAttributeClusterDimension;
+  at[0].val.clusterDim.x = (unsigned)kern.cluster; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
+  cfg.attrs = at; cfg.numAttrs = 1;
+  int nc = 0;
+  if (cudaOccupancyMaxActiveClusters(&nc, (const void*)kern.fn, &cfg) != cudaSuccess || nc < 1) return ctx->num_sms / kern.cluster * kern.cluster;
+  return std::min(ctx->num_sms / kern.cluster, nc) * kern.cluster;
+}
+
 // Codegen (cached) -> JIT (cached) -> parameters -> launch of one fused scan kernel.
 gq_status run_scan(gq_ctx* ctx, const GqScanSpec& sp, const gq_batch* in, const gq_probe_step* probes,
                    GqParams* P /* target/acc/out/out_count pre-filled */) {
@@ -268,12 +282,23 @@ gq_status run_scan(gq_ctx* ctx, const GqScanSpec& sp, const gq_batch* in, const 
   if (in->nrows == 0) return GQ_OK;   // empty batches are legal no-ops (S9)
   const int64_t ntiles = in->nrows / kern.tile_rows;
   int grid = (int)std::max<int64_t>(1, std::min<int64_t>(ctx->num_sms, ntiles));
+  if (kern.cluster > 1) grid = std::max(kern.cluster, std::min(grid, cluster_grid(ctx, kern)) / kern.cluster * kern.cluster);   // whole, co-resident clusters
   void* args[] = {(void*)P};
   static const char* const kname[] = {"gq_scan:global", "gq_scan:lowcard", "gq_scan:highcard", "gq_scan:build", "gq_scan:materialise",
                                       "gq_scan:direct", "gq_scan:partition", "gq_scan:scatter"};
   ProfScope ps(ctx, kname[sp.consumer]);
-  cudaError_t e = cudaLaunchKernel((const void*)kern.fn, dim3((unsigned)grid), dim3((unsigned)kern.threads), args,
-                                   (size_t)kern.smem_bytes, ctx->stream);
+  cudaError_t e;
+  if (kern.cluster > 1) {   // thread-block clusters: the CTAs of a cluster reach each other's shared memory
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3((unsigned)grid); cfg.blockDim = dim3((unsigned)kern.threads);
+    cfg.dynamicSmemBytes = (size_t)kern.smem_bytes; cfg.stream = ctx->stream;
+    cudaLaunchAttribute at[1];
+    at[0].id = cudaLaunchAttributeClusterDimension;
+    at[0].val.clusterDim.x = (unsigned)kern.cluster; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
+    cfg.attrs = at; cfg.numAttrs = 1;
+    e = cudaLaunchKernelExC(&cfg, (const void*)kern.fn, args);
+  } else
+    e = cudaLaunchKernel((const void*)kern.fn, dim3((unsigned)grid), dim3((unsigned)kern.threads), args, (size_t)kern.smem_bytes, ctx->stream);
   if (e != cudaSuccess) return cuda_fail(ctx, e, "launch of fused scan kernel");
   ++ctx->launches;
   return GQ_OK;
@@ -668,7 +693,7 @@ DirectPlan direct_plan(const GqScanSpec& sp, const gq_agg_desc* d, const gq_batc
 // an L2-resident table slice. Worth it only for big tables and big batches; thresholds overridable for tests.
 struct PartPlan { bool on = false; int npart = 0, pshift = 0, rw = 0; int64_t pcap = 0; size_t bytes = 0; std::vector<int> exprs; int src[GQ_MAX_AGGS]; };
 // planner knobs (gq_set_option)
-std::atomic<int64_t> g_part_min_table_mb{256}, g_part_min_rows{1 << 24}, g_hot_min_rows{GQ_HOT_MIN_ROWS}, g_psa_max_log2part{GQ_PSA_MAX_LOG2PART}, g_psa_threads{0}, g_dpart_min_acc_mb{GQ_DPART_OFF};
+std::atomic<int64_t> g_part_min_table_mb{256}, g_part_min_rows{1 << 24}, g_hot_min_rows{GQ_HOT_MIN_ROWS}, g_psa_max_log2part{GQ_PSA_MAX_LOG2PART}, g_psa_threads{0}, g_dpart_min_acc_mb{GQ_DPART_OFF}, g_psa_cluster{2};
 PartPlan part_plan(const GqScanSpec& sp, const gq_agg_desc* d, int64_t nrows) {
   PartPlan pp;
   if (sp.consumer != GQ_C_HIGHCARD) return pp;
@@ -739,6 +764,9 @@ struct PsaPlan {
   size_t off_zero = 0, zero_bytes = 0, off_pcount = 0, off_pfill = 0, off_pstart = 0, off_items = 0, off_itemseg = 0, off_ncta = 0,
          off_info = 0, off_plist = 0, off_merge = 0, merge_bytes = 0, off_hot = 0, off_rec = 0, bytes = 0;
 };
+// Pass A runs as thread-block clusters of 2 (74 clusters pack a B200's 148 SMs exactly) whose CTAs share the open chunk of
+// every partition: half as many open record lines compete for L2 (DESIGN 5.4). Planner knob "psa_cluster": 1 = off.
+int psa_cluster(int num_sms, int npart) { const int c = (int)g_psa_cluster.load(); return (c > 1 && num_sms >= c && npart % c == 0) ? c : 1; }
 const int64_t GQ_PSA_MAX_TILE = 4096;   // upper bound of the scan kernel's tile (rows): bounds a CTA's share of the rows
 PsaPlan psa_plan(const GqScanSpec& sp, const gq_agg_desc* d, int64_t nrows, int topk) {
   PsaPlan pp;
@@ -1190,14 +1218,24 @@ static gq_status run_psa(gq_ctx* ctx, const gq_plan* plan, GqScanSpec sp, const 
   const gq_agg_desc* d = &plan->agg;
   const gq_batch* in = plan->in;
   sp.consumer = GQ_C_SCATTER; sp.hot = pp.hot; sp.part_rw = pp.rw; sp.part_exprs = pp.exprs; sp.part_states = pp.npart;
+  sp.cluster = psa_cluster(ctx->num_sms, pp.npart);
   CachedKernel* ck = nullptr;
   gq_status st = get_kernel_info(sp, &ck, &ctx->msg);
   if (st != GQ_OK) return st;
   const int64_t tile = ck->info.tile_rows;
   if (tile > GQ_PSA_MAX_TILE || ctx->num_sms > GQ_MAX_SMS) return fail(ctx, GQ_ERR_UNSUPPORTED, "internal: scatter tile/grid exceeds the workspace bound");
-  const int64_t grid = std::max<int64_t>(1, std::min<int64_t>(ctx->num_sms, in->nrows / tile));
-  const int64_t slab = (in->nrows / grid + 2 * tile) / GQ_PART_CHUNK + pp.npart + 2;
-  if (grid * slab > pp.chunks_bound || slab >= (1LL << 20)) return fail(ctx, GQ_ERR_UNSUPPORTED, "internal: chunk range bound");
+  const int cl = sp.cluster;
+  int64_t grid = std::max<int64_t>(1, std::min<int64_t>(ctx->num_sms, in->nrows / tile));
+  if (cl > 1) {                                                                    // as run_scan rounds it
+    GqKernel kq;
+    st = load_kernel(ctx, ck, &kq);
+    if (st != GQ_OK) return st;
+    grid = std::max<int64_t>(cl, std::min<int64_t>(grid, cluster_grid(ctx, kq)) / cl * cl);
+  }
+  // chunk ids are handed out per writer: a CTA, or a cluster whose CTAs share the partitions' open chunks
+  const int64_t writers = grid / cl;
+  const int64_t slab = cl * ((in->nrows / grid + 2 * tile) / GQ_PART_CHUNK) + pp.npart + 2;
+  if (writers * slab > pp.chunks_bound || slab >= (1LL << 20)) return fail(ctx, GQ_ERR_UNSUPPORTED, "internal: chunk range bound");
   cudaError_t e = cudaMemsetAsync(ws + pp.off_zero, 0, pp.zero_bytes, ctx->stream);
   if (e == cudaSuccess) e = cudaMemsetAsync(F.out_n, 0, 8, ctx->stream);
   if (e != cudaSuccess) return cuda_fail(ctx, e, "partitioned aggregation: memset");
@@ -1248,7 +1286,7 @@ static gq_status run_psa(gq_ctx* ctx, const gq_plan* plan, GqScanSpec sp, const 
   dp.pcount = U(pp.off_pcount); dp.pstart = U(pp.off_pstart); dp.items = U(pp.off_items); dp.item_seg = U(pp.off_itemseg);
   dp.nitems = U(pp.off_zero) + 1; dp.npart = pp.npart; dp.seg_chunks = pp.seg_chunks; dp.err = ctx->d_err; dp.max_items = pp.max_items; dp.nsub = 1u << pp.log2sub;
   e = PROF(ctx, "gq_k_psa_dir", gq_launch_psa_dir(ctx->stream, dp));
-  if (e == cudaSuccess) e = PROF(ctx, "gq_k_psa_fill", gq_launch_psa_fill(ctx->stream, U(pp.off_info), U(pp.off_ncta), (int)grid, slab, U(pp.off_pstart), U(pp.off_pfill), U(pp.off_plist)));
+  if (e == cudaSuccess) e = PROF(ctx, "gq_k_psa_fill", gq_launch_psa_fill(ctx->stream, U(pp.off_info), U(pp.off_ncta), (int)writers, slab, U(pp.off_pstart), U(pp.off_pfill), U(pp.off_plist)));
   if (e != cudaSuccess) return cuda_fail(ctx, e, "partition directory");
   ctx->launches += 2;
   CachedKernel* pk = nullptr;
@@ -1397,6 +1435,7 @@ gq_status gq_set_option(const char* h_name, int64_t value) {
   if (n == "part_min_table_mb") g_part_min_table_mb = value < 0 ? 256 : value;
   else if (n == "part_min_rows") g_part_min_rows = value < 0 ? (1 << 24) : value;
   else if (n == "hot_min_rows") g_hot_min_rows = value < 0 ? GQ_HOT_MIN_ROWS : value;
+  else if (n == "psa_cluster") g_psa_cluster = value == 1 ? 1 : 2;   // (clusters of 4 were measured: 132 co-resident CTAs, pass A 9.5 -> 10.9 ms)
   else if (n == "dpart_min_acc_mb") g_dpart_min_acc_mb = value < 0 ? GQ_DPART_OFF : value;
   else if (n == "psa_threads") g_psa_threads = (value == 512 || value == 1024) ? value : 0;
   else if (n == "psa_max_log2_partitions") g_psa_max_log2part = value < 0 ? GQ_PSA_MAX_LOG2PART : value;
@@ -1571,6 +1610,7 @@ gq_status gq_precompile_pipeline(const gq_plan* plan, char* h_msg, size_t msg_by
     if (pa.on) {
       GqScanSpec f = sp;
       f.consumer = GQ_C_SCATTER; f.hot = pa.hot; f.part_rw = pa.rw; f.part_exprs = pa.exprs; f.part_states = pa.npart;
+      f.cluster = psa_cluster(GQ_DEFAULT_SMS, pa.npart);
       st = precompile(f, h_msg, msg_bytes);
       if (st != GQ_OK) return st;
       std::string msg, path;

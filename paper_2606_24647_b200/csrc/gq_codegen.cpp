@@ -439,7 +439,7 @@ gq_status gq_codegen(const GqScanSpec& sp, GqKernelInfo* out, std::string* msg) 
   if (sp.part_rw > 0) {   // partition state words (+ the CTA's chunk counter)
     if (sp.part_states < 1 || sp.part_states > 16384) { if (msg) *msg = "bad partition count"; return GQ_ERR_INVALID_ARG; }
     part_state_off = (cons_bytes + 127) / 128 * 128;
-    cons_bytes = part_state_off + sp.part_states * 4LL + 64;
+    cons_bytes = part_state_off + (sp.part_states / std::max(1, sp.cluster)) * 4LL + 64;   // a cluster's CTAs split the state words
   }
   int r = tablebound ? 4 : 2, stages = 0;
   // small inputs: smaller tiles so that every SM still gets several tiles
@@ -461,6 +461,7 @@ gq_status gq_codegen(const GqScanSpec& sp, GqKernelInfo* out, std::string* msg) 
   o << "// generated by gq_codegen — plan-shape specialised prelude\n";
   // (part of the source, hence of the kernel's identity: two plans that differ only in their shared-memory carve-up,
   // e.g. in the number of partition state words, must not share a cached kernel and its launch configuration)
+  o << "#define GQ_SC_CLUSTER " << (sp.consumer == GQ_C_SCATTER ? std::max(1, sp.cluster) : 1) << "\n";
   o << "#define GQ_SMEM_BYTES " << (stages * stage_bytes + 2 * stages * 8 + 64 + cons_bytes + 128) << "\n";
   o << "#define GQ_NCOL " << ncol << "\n#define GQ_NT " << nt << "\n#define GQ_R " << r << "\n#define GQ_STAGES "
     << stages << "\n#define GQ_STAGE_BYTES " << stage_bytes << "\n#define GQ_CONSUMER " << sp.consumer << "\n";
@@ -634,6 +635,7 @@ gq_status gq_codegen(const GqScanSpec& sp, GqKernelInfo* out, std::string* msg) 
   out->hash = hb;
   out->threads = nt + 32;
   out->tile_rows = nt * r;
+  out->cluster = sp.consumer == GQ_C_SCATTER ? std::max(1, sp.cluster) : 1;
   out->smem_bytes = (int)(stages * stage_bytes + 2 * stages * 8 + 64 + cons_bytes + 128);
   out->cols = g.cols;
   out->consts = g.consts;

@@ -171,6 +171,7 @@ struct GqScanSpec {
   bool dense_target = false;                      // BUILD into a direct-address table
   bool hot = false;                               // HIGHCARD: per-CTA shared-memory aggregation of hot keys
   bool check_dep = false;                         // GQ_F_CHECK_DEPENDENT: every row verifies the dependent key
+  int cluster = 1;                                // SCATTER: CTAs per thread-block cluster sharing the partitions' open chunks
   int num_sms = GQ_DEFAULT_SMS;                   // tiling heuristics: SM count of the context's device
   int64_t nrows_hint = 0;                         // tiling heuristic only
 };
@@ -182,6 +183,7 @@ struct GqKernelInfo {
   int threads = 0;             // GQ_NT + 32
   int smem_bytes = 0;
   int tile_rows = 0;
+  int cluster = 1;             // thread-block cluster size the kernel must be launched with
   std::vector<int> cols;       // compacted column list: original input column index per kernel column
   std::vector<long long> consts;  // values for GqParams::k
 };
@@ -191,7 +193,7 @@ gq_status gq_codegen(const GqScanSpec& spec, GqKernelInfo* out, std::string* msg
 gq_status gq_codegen_psa(const GqScanSpec& spec, int log2slots, const int* src, int threads, GqKernelInfo* out, std::string* msg);
 int gq_dtype_bytes(gq_dtype t);
 // gq_jit.cpp
-struct GqKernel { cudaKernel_t fn = nullptr; int threads = 0; int smem_bytes = 0; int tile_rows = 0; };
+struct GqKernel { cudaKernel_t fn = nullptr; int threads = 0; int smem_bytes = 0; int tile_rows = 0; int cluster = 1; };
 gq_status gq_jit_compile_to_cache(const GqKernelInfo& info, std::string* cubin_path, std::string* msg);
 gq_status gq_jit_get(const GqKernelInfo& info, int device, GqKernel* out, std::string* msg, int* cuda_err);
 void gq_jit_set_cache_dir(const char* path);

@@ -134,7 +134,7 @@ gq_status gq_jit_get(const GqKernelInfo& info, int device, GqKernel* out, std::s
     if (msg) *msg = std::string("loading generated kernel: ") + cudaGetErrorString(e);
     return GQ_ERR_CUDA;
   }
-  GqKernel k; k.fn = fn; k.threads = info.threads; k.smem_bytes = info.smem_bytes; k.tile_rows = info.tile_rows;
+  GqKernel k; k.fn = fn; k.threads = info.threads; k.smem_bytes = info.smem_bytes; k.tile_rows = info.tile_rows; k.cluster = info.cluster;
   g_loaded[lkey] = k;
   *out = k;
   return GQ_OK;

@@ -159,9 +159,14 @@ extern "C" __global__ void __launch_bounds__(GQ_NT + 32, 1) gq_scan(const __grid
 #endif
 #if GQ_PART_RW
   cx.part_st = (u32*)(gq_smem + GQ_CONS_OFF + GQ_PART_STATE_OFF);
-  for (int i = tid; i < (int)P.npart; i += GQ_NT + 32) cx.part_st[i] = GQ_PART_CHUNK;   // no open chunk yet
+#if GQ_SC_CLUSTER > 1
+  const int nstate = (int)P.npart / GQ_SC_CLUSTER;         // this CTA holds the words of the partitions p with p mod cluster size == its rank
+#else
+  const int nstate = (int)P.npart;
+#endif
+  for (int i = tid; i < nstate; i += GQ_NT + 32) cx.part_st[i] = GQ_PART_CHUNK;   // no open chunk yet
 #if GQ_CONSUMER == GQ_C_SCATTER
-  cx.sc_next = cx.part_st + P.npart;
+  cx.sc_next = cx.part_st + nstate;
   if (tid == 0) *cx.sc_next = 0;
 #endif
 #endif
@@ -183,8 +188,15 @@ extern "C" __global__ void __launch_bounds__(GQ_NT + 32, 1) gq_scan(const __grid
   }
 #endif
   __syncthreads();
+#if GQ_SC_CLUSTER > 1
+  gq_cluster_sync();                                     // the peers' state words are initialised before anybody reserves through them
+#endif
   if (*err_seen != 0) {
     if (tid == GQ_NT) for (i64 i = 0; i < produced; ++i) gq_mbar_wait(&full_bar[i], 0u);   // copies in flight land before the CTA exits
+#if GQ_SC_CLUSTER > 1
+    __syncwarp();
+    gq_cluster_sync();                                   // a peer that did not see the error may still reserve through this CTA's words
+#endif
 #if GQ_FUSED_FINAL
     if (tid == 0) {   // keep ticket (and merge table) zeroed for the next kernel
       const u32 t = atomicAdd(P.fin.ticket, 1u);
@@ -212,6 +224,10 @@ extern "C" __global__ void __launch_bounds__(GQ_NT + 32, 1) gq_scan(const __grid
         gq_produce_tile(P, gq_smem, full_bar, s, tile, pol);
       }
     }
+#if GQ_SC_CLUSTER > 1
+    __syncwarp();
+    gq_cluster_sync();                                   // the cluster's final barrier (see the SCATTER epilogue)
+#endif
     return;
   }
 
@@ -432,6 +448,20 @@ extern "C" __global__ void __launch_bounds__(GQ_NT + 32, 1) gq_scan(const __grid
   }
 #endif
 #if GQ_CONSUMER == GQ_C_SCATTER
+#if GQ_SC_CLUSTER > 1
+  {   // every CTA of the cluster has stopped reserving: each records how far the part-filled chunks of ITS partitions got
+    __syncwarp();
+    gq_cluster_sync();
+    const u32 rank = gq_cluster_rank();
+    const u64 cbase = (u64)gq_cluster_id() * (u64)P.sc_slab;
+    for (int q = tid; q < nstate; q += GQ_NT) {
+      const u32 v = cx.part_st[q];
+      const u32 used = v & 0xFFFu;
+      if (used < GQ_PART_CHUNK) P.sc_info[cbase + (v >> 12)] = (((u32)q * GQ_SC_CLUSTER + rank) << 8) | used;
+    }
+    if (tid == 0 && rank == 0) { const u32 n = *cx.sc_next; P.sc_ncta[gq_cluster_id()] = n < (u32)P.sc_slab ? n : (u32)P.sc_slab; }
+  }
+#else
   {   // record how far this CTA's part-filled chunks got, and how many chunks it opened
     gq_consumer_barrier();
     for (int p = tid; p < (int)P.npart; p += GQ_NT) {
@@ -441,6 +471,7 @@ extern "C" __global__ void __launch_bounds__(GQ_NT + 32, 1) gq_scan(const __grid
     }
     if (tid == 0) { const u32 n = *cx.sc_next; P.sc_ncta[blockIdx.x] = n < (u32)P.sc_slab ? n : (u32)P.sc_slab; }
   }
+#endif
 #elif GQ_PART_RW
   {   // pad the unused slots of this CTA's open chunks with EMPTY-key records (pass B skips them)
     gq_consumer_barrier();

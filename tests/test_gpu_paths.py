@@ -475,8 +475,9 @@ def test_partitioned_shared_memory_aggregation_hot_keys_and_sub_passes(ctx, forc
                 aggs=[("sum", 0), ("sum", 1), ("min", 0), ("max", 0), ("count",)], max_groups=300_000)
     try:
         gq.set_option("hot_min_rows", 4096)
-        for lp in (14, 6, 5):
+        for lp, cl in ((14, 2), (6, 2), (5, 1), (14, 1)):           # with and without thread-block clusters in pass A
             gq.set_option("psa_max_log2_partitions", lp)
+            gq.set_option("psa_cluster", cl)
             for th in (512, 1024):
                 gq.set_option("psa_threads", th)
                 l0 = ctx.launch_count()
@@ -485,6 +486,7 @@ def test_partitioned_shared_memory_aggregation_hot_keys_and_sub_passes(ctx, forc
                 assert int(got["cols"][-1].max()) > 100_000
     finally:
         gq.set_option("hot_min_rows", -1); gq.set_option("psa_max_log2_partitions", -1); gq.set_option("psa_threads", 0)
+        gq.set_option("psa_cluster", 2)
 
 
 def test_clustered_direct_aggregation(ctx, force_partition):
