@@ -621,51 +621,67 @@ __device__ __forceinline__ u32 gq_dsm_add(u32 a, u32 v) {
 __device__ __forceinline__ void gq_cluster_sync() {   // every thread of every CTA of the cluster, warps converged
   asm volatile("barrier.cluster.arrive.release.aligned;\nbarrier.cluster.wait.acquire.aligned;" ::: "memory");
 }
-// As gq_scatter_reserve below, on the cluster's shared state: st / next are THIS CTA's arrays; partition p's word is word
-// p / GQ_SC_CLUSTER of CTA p mod GQ_SC_CLUSTER, the chunk counter is CTA 0's; chunk ids of cluster c are
+// The state words live in the cluster's distributed shared memory: st / next are THIS CTA's arrays; partition p's word is
+// word p / GQ_SC_CLUSTER of CTA p mod GQ_SC_CLUSTER, the chunk counter is CTA 0's; chunk ids of cluster c are
 // [c * sc_slab, (c + 1) * sc_slab).
-__device__ __forceinline__ u64 gq_scatter_reserve(const GqParams& P, u32* st, u32* next, u32 p) {
-  const u32 a = gq_mapa(gq_smem_addr(st + p / GQ_SC_CLUSTER), p % GQ_SC_CLUSTER);
-  const u64 cbase = (u64)gq_cluster_id() * (u64)P.sc_slab;
-  for (;;) {
-    const u32 v0 = gq_dsm_ld(a);
-    if ((v0 & 0xFFFu) > GQ_PART_CHUNK) { __nanosleep(20); continue; }   // the next chunk is being opened
-    const u32 v = gq_dsm_add(a, 1u);
-    const u32 used = v & 0xFFFu;
-    if (used < GQ_PART_CHUNK) return (cbase + (v >> 12)) * GQ_PART_CHUNK + used;
-    if (used == GQ_PART_CHUNK) {                           // this thread opens the next chunk and takes its first slot
-      const u32 c = gq_dsm_add(gq_mapa(gq_smem_addr(next), 0u), 1u);
-      if ((i64)c >= P.sc_slab) { gq_set_err(P.err, GQ_E_CAPACITY); gq_dsm_st(a, v & ~0xFFFu); return ~0ULL; }
-      const u64 gid = cbase + c;
-      P.sc_info[gid] = (p << 8) | GQ_PART_CHUNK;           // assumed full; part-filled chunks are fixed up at the end
-      atomicAdd(P.sc_count + p, 1u);
-      gq_dsm_st(a, (c << 12) | 1u);
-      return gid * GQ_PART_CHUNK;
-    }
-  }
-}
+__device__ __forceinline__ u32 gq_sc_word(u32* st, u32 p) { return gq_mapa(gq_smem_addr(st + p / GQ_SC_CLUSTER), p % GQ_SC_CLUSTER); }
+__device__ __forceinline__ u32 gq_sc_ld(u32 a) { return gq_dsm_ld(a); }
+__device__ __forceinline__ u32 gq_sc_add(u32 a) { return gq_dsm_add(a, 1u); }
+__device__ __forceinline__ void gq_sc_st(u32 a, u32 v) { gq_dsm_st(a, v); }
+__device__ __forceinline__ u32 gq_sc_next(u32* next) { return gq_dsm_add(gq_mapa(gq_smem_addr(next), 0u), 1u); }
+__device__ __forceinline__ u64 gq_sc_base(const GqParams& P) { return (u64)gq_cluster_id() * (u64)P.sc_slab; }
 #else
-__device__ __forceinline__ u64 gq_scatter_reserve(const GqParams& P, u32* st, u32* next, u32 p) {
+__device__ __forceinline__ u32 gq_sc_word(u32* st, u32 p) { return gq_smem_addr(st + p); }
+__device__ __forceinline__ u32 gq_sc_ld(u32 a) {
+  u32 v;
+  asm volatile("ld.volatile.shared.u32 %0, [%1];" : "=r"(v) : "r"(a) : "memory");
+  return v;
+}
+__device__ __forceinline__ u32 gq_sc_add(u32 a) {
+  u32 o;
+  asm volatile("atom.shared.add.u32 %0, [%1], 1;" : "=r"(o) : "r"(a) : "memory");
+  return o;
+}
+__device__ __forceinline__ void gq_sc_st(u32 a, u32 v) { asm volatile("st.volatile.shared.u32 [%0], %1;" ::"r"(a), "r"(v) : "memory"); }
+__device__ __forceinline__ u32 gq_sc_next(u32* next) { return atomicAdd(next, 1u); }
+__device__ __forceinline__ u64 gq_sc_base(const GqParams& P) { return (u64)blockIdx.x * (u64)P.sc_slab; }
+#endif
+// A reservation is ONE atomic increment of the partition's word (a "ticket"): used < GQ_PART_CHUNK is a slot of the open
+// chunk, used == GQ_PART_CHUNK makes this thread the opener of the next chunk (it takes the first slot and stores the
+// new word), used > GQ_PART_CHUNK means the chunk is being opened: poll with loads, then draw again. A thread adds at
+// most one stray increment per opening, so the 12-bit field cannot overflow (2 x 1024 threads + 32 < 4096). The three
+// phases are separate calls so that a thread's GQ_R tickets are in flight together (half of them are remote shared-memory
+// atomics in a cluster) and so that every opener acts before anybody polls (no waiting cycle between rows).
+__device__ __forceinline__ u32 gq_scatter_ticket(u32* st, u32 p) { return gq_sc_add(gq_sc_word(st, p)); }
+__device__ __forceinline__ u64 gq_scatter_open(const GqParams& P, u32 a, u32* next, u32 p, u32 v) {
+  const u32 c = gq_sc_next(next);
+  if ((i64)c >= P.sc_slab) { gq_set_err(P.err, GQ_E_CAPACITY); gq_sc_st(a, v & ~0xFFFu); return ~0ULL; }
+  const u64 gid = gq_sc_base(P) + c;
+  P.sc_info[gid] = (p << 8) | GQ_PART_CHUNK;               // assumed full; part-filled chunks are fixed up at the end
+  atomicAdd(P.sc_count + p, 1u);
+  gq_sc_st(a, (c << 12) | 1u);
+  return gid * GQ_PART_CHUNK;
+}
+// phase 2 (openers only): returns true when this ticket was the opener's; idx = the record index (or ~0: out of chunks)
+__device__ __forceinline__ bool gq_scatter_opener(const GqParams& P, u32* st, u32* next, u32 p, u32 v, u64& idx) {
+  if ((v & 0xFFFu) != GQ_PART_CHUNK) return false;
+  idx = gq_scatter_open(P, gq_sc_word(st, p), next, p, v);
+  return true;
+}
+// phase 3 (everybody else)
+__device__ __forceinline__ u64 gq_scatter_take(const GqParams& P, u32* st, u32* next, u32 p, u32 v) {
+  u32 used = v & 0xFFFu;
+  if (used < GQ_PART_CHUNK) return (gq_sc_base(P) + (v >> 12)) * GQ_PART_CHUNK + used;
+  const u32 a = gq_sc_word(st, p);
   for (;;) {
-    const u32 v0 = ((volatile u32*)st)[p];
-    if ((v0 & 0xFFFu) > GQ_PART_CHUNK) { __nanosleep(20); continue; }   // the next chunk is being opened (a few cycles)
-    const u32 v = atomicAdd(&st[p], 1u);
-    const u32 used = v & 0xFFFu;
-    if (used < GQ_PART_CHUNK) return ((u64)blockIdx.x * (u64)P.sc_slab + (v >> 12)) * GQ_PART_CHUNK + used;
-    if (used == GQ_PART_CHUNK) {                           // this thread opens the next chunk and takes its first slot
-      const u32 c = atomicAdd(next, 1u);
-      if ((i64)c >= P.sc_slab) { gq_set_err(P.err, GQ_E_CAPACITY); ((volatile u32*)st)[p] = v & ~0xFFFu; return ~0ULL; }
-      const u64 gid = (u64)blockIdx.x * (u64)P.sc_slab + c;
-      P.sc_info[gid] = (p << 8) | GQ_PART_CHUNK;           // assumed full; part-filled chunks are fixed up at the end
-      atomicAdd(P.sc_count + p, 1u);
-      __threadfence_block();
-      ((volatile u32*)st)[p] = (c << 12) | 1u;
-      return gid * GQ_PART_CHUNK;
-    }
+    while ((gq_sc_ld(a) & 0xFFFu) > GQ_PART_CHUNK) __nanosleep(20);   // the next chunk is being opened
+    v = gq_sc_add(a);
+    used = v & 0xFFFu;
+    if (used < GQ_PART_CHUNK) return (gq_sc_base(P) + (v >> 12)) * GQ_PART_CHUNK + used;
+    if (used == GQ_PART_CHUNK) return gq_scatter_open(P, a, next, p, v);
   }
 }
 
-#endif
 
 // ---------------------------------------------------------------------------------------------- row sources
 // A tile staged in shared memory by the producer, or the ragged tail read from global memory.

@@ -342,6 +342,16 @@ extern "C" __global__ void __launch_bounds__(GQ_NT + 32, 1) gq_scan(const __grid
     // CTAs RED theirs in) -> ticket -> the last CTA only reads the table, emits and zeroes it. Replaces "every CTA
     // writes its partials, the last one folds grid x G of them" (C1: that tail was 6 of 18 us).
     i64* fin = (i64*)(gq_smem + GQ_CONS_OFF + GQ_LC_FIN_OFF);
+    u64* gt = P.fin.gtab;
+#if GQ_LC_KEY32
+    // The first find-or-claim CAS of every group goes out BEFORE the CTA-level reduction and is consumed after it: its
+    // round trip to L2 (0.7 us) hides behind the reduction instead of following it.
+    u64 st0 = 0;
+    if (tid < ng) {
+      const i64 key = cx.lc_gkey[tid];
+      st0 = atomicCAS(gt + 32 + (u32)gq_hash(key, 64 - 6) * 16, 0ULL, 2ULL | ((u64)GQ_LC_K32(key) << 32));
+    }
+#endif
     for (int p0 = warp; p0 < ng * GQ_NAGG; p0 += 4 * GQ_NWARP) {
       i64 v[4];
       gq_lc_reduce4(cx, p0, ng * GQ_NAGG, lane, v);
@@ -350,7 +360,6 @@ extern "C" __global__ void __launch_bounds__(GQ_NT + 32, 1) gq_scan(const __grid
         if (lane == 0 && p0 + u * GQ_NWARP < ng * GQ_NAGG) fin[p0 + u * GQ_NWARP] = v[u];
     }
     gq_consumer_barrier();
-    u64* gt = P.fin.gtab;
     if (tid < ng) {
       const i64 key = cx.lc_gkey[tid];
       u32 h = (u32)gq_hash(key, 64 - 6);
@@ -363,7 +372,7 @@ extern "C" __global__ void __launch_bounds__(GQ_NT + 32, 1) gq_scan(const __grid
       const u64 mine = 2ULL | ((u64)GQ_LC_K32(key) << 32);
       for (int n = 0; n < GQ_GTAB_SLOTS && !done; ++n, h = (h + 1) & (GQ_GTAB_SLOTS - 1)) {
         u64* s = gt + 32 + h * 16;
-        const u64 st = atomicCAS(s, 0ULL, mine);
+        const u64 st = n == 0 ? st0 : atomicCAS(s, 0ULL, mine);
         if (st != 0 && st != mine) continue;               // another key's slot
         if (st == 0) s[1] = (u64)key;                      // (read by the last CTA only, after every CTA's fence + ticket)
 #pragma unroll
