@@ -105,6 +105,9 @@ typedef struct gq_aggstate gq_aggstate; /* group-by hash table (host handle; sto
 /* ---- context ------------------------------------------------------------------------------------------------- */
 /* cuda_stream: a cudaStream_t (e.g. torch.cuda.current_stream().cuda_stream), 0 = legacy default stream. */
 gq_status gq_create(gq_ctx** out, int device, void* cuda_stream);
+/* gq_create allocates and gq_destroy frees a small device block (error word, merge table) and a pinned host word: like any
+   cudaMalloc / cudaFree they must not run while a stream of the process is being captured into a CUDA graph. Every other
+   call only enqueues work on the context's stream and can be captured. */
 gq_status gq_destroy(gq_ctx*);
 /* Blocks the HOST until the stream is idle (the pipeline boundary); returns the sticky device error. */
 gq_status gq_sync(gq_ctx*);

@@ -606,7 +606,7 @@ bool agg_has_hot_area(int64_t max_groups, int nkeys) { return nkeys > 0 && max_g
 size_t agg_ws_bytes(int64_t cap, int sw, int64_t max_groups, int nkeys, size_t* hot_off) {
   size_t base = align_up(ws_layout(cap, sw, 1).total, 256);
   if (hot_off) *hot_off = base;
-  return base + (agg_has_hot_area(max_groups, nkeys) ? 4096 + (size_t)GQ_HOT_SLOTS * 16 : 0);
+  return base + (agg_has_hot_area(max_groups, nkeys) ? GQ_HOT_LIST_BYTES + (size_t)GQ_HOT_SLOTS * 16 : 0);
 }
 
 gq_status agg_spec(gq_ctx* ctx, GqScanSpec* sp, const gq_batch* in, const gq_agg_desc* d, int key_bits[2],
@@ -809,7 +809,7 @@ PsaPlan psa_plan(const GqScanSpec& sp, const gq_agg_desc* d, int64_t nrows, int 
   // a partition is "heavy" (cut into segments for several CTAs) when it is far above the average AND a sizeable share of all work
   pp.seg_chunks = (uint32_t)std::max<int64_t>(std::max<int64_t>(64, pp.chunks_bound / 512), 4 * pp.chunks_bound / pp.npart);
   pp.max_items = (uint32_t)((pp.npart + 2 * (pp.chunks_bound / pp.seg_chunks) + 2) << pp.log2sub);
-  pp.merge_cap = table_capacity(std::min<int64_t>(std::max<int64_t>(1, d->max_groups), (pp.chunks_bound / pp.seg_chunks + 1) * limit) + GQ_HOT_MAX);
+  pp.merge_cap = table_capacity(std::min<int64_t>(std::max<int64_t>(1, d->max_groups), (pp.chunks_bound / pp.seg_chunks + 1) * limit) + GQ_HOT_MAX_SCATTER);
   size_t off = 0;
   auto take = [&off](size_t b) { size_t o = off; off += align_up(b, 256); return o; };
   pp.off_zero = take(256);                                   // [0] work cursor, [1] item count
@@ -824,7 +824,7 @@ PsaPlan psa_plan(const GqScanSpec& sp, const gq_agg_desc* d, int64_t nrows, int 
   pp.off_plist = take((size_t)pp.chunks_bound * 4);
   pp.merge_bytes = ws_layout(pp.merge_cap, sw, 1).total;
   pp.off_merge = take(pp.merge_bytes);
-  if (pp.hot) pp.off_hot = take(4096 + (size_t)GQ_HOT_SLOTS * 16);   // hot list + heavy-hitter sample table
+  if (pp.hot) pp.off_hot = take(GQ_HOT_LIST_BYTES + (size_t)GQ_HOT_SLOTS * 16);   // hot list + heavy-hitter sample table
   pp.off_rec = take((size_t)pp.chunks_bound * GQ_PART_CHUNK * pp.rw * 8);
   pp.bytes = off;
   pp.on = true;
@@ -917,7 +917,7 @@ gq_status gq_hash_aggregate(gq_ctx* ctx, gq_aggstate** state, void* d_ws, size_t
       }
       if (agg_has_hot_area(d->max_groups, d->nkeys)) {
         a->hot = (long long*)((char*)d_ws + hot_off);
-        a->hot_table = (unsigned long long*)((char*)d_ws + hot_off + 4096);
+        a->hot_table = (unsigned long long*)((char*)d_ws + hot_off + GQ_HOT_LIST_BYTES);
       }
       {
         PartPlan pp = part_plan(sp, d, in->nrows);
@@ -971,7 +971,7 @@ gq_status gq_hash_aggregate(gq_ctx* ctx, gq_aggstate** state, void* d_ws, size_t
   if (sp.hot && a->hot && in->nrows >= g_hot_min_rows.load()) {   // heavy-hitter pass over a strided sample of the key column
     int nl = 0;
     const gq_column& kc = in->cols[sp.key_cols[0]];
-    cudaError_t e = PROF(ctx, "gq_k_hot_keys(4)", gq_launch_hot_keys(ctx->stream, kc.data, (int)kc.dtype, in->nrows, a->hot_table, GQ_HOT_SLOTS, GQ_HOT_SAMPLE,
+    cudaError_t e = PROF(ctx, "gq_k_hot_keys(5)", gq_launch_hot_keys(ctx->stream, kc.data, (int)kc.dtype, in->nrows, a->hot_table, GQ_HOT_SLOTS, GQ_HOT_SAMPLE,
                                        GQ_HOT_THRESHOLD, a->hot, GQ_HOT_MAX, ctx->num_sms, &nl));
     if (e != cudaSuccess) return cuda_fail(ctx, e, "heavy-hitter sampling");
     ctx->launches += nl;
@@ -1099,7 +1099,7 @@ gq_status gq_aggstate_rehash(gq_ctx* ctx, gq_aggstate* a, void* d_new_ws, size_t
   if (st != GQ_OK) return st;
   a->dev = nt; a->capacity = cap; a->max_groups = new_max_groups;
   a->hot = (long long*)((char*)d_new_ws + hot_off);
-  a->hot_table = (unsigned long long*)((char*)d_new_ws + hot_off + 4096);
+  a->hot_table = (unsigned long long*)((char*)d_new_ws + hot_off + GQ_HOT_LIST_BYTES);
   a->part = nullptr; a->pcur = nullptr;   // the record buffers lived in the old workspace: later batches aggregate in one pass
   return GQ_OK;
 }
@@ -1273,8 +1273,8 @@ static gq_status run_psa(gq_ctx* ctx, const gq_plan* plan, GqScanSpec sp, const 
     int nl = 0;
     const gq_column& kc = in->cols[sp.key_cols[0]];
     long long* hot = (long long*)(ws + pp.off_hot);
-    e = PROF(ctx, "gq_k_hot_keys(4)", gq_launch_hot_keys(ctx->stream, kc.data, (int)kc.dtype, in->nrows, (unsigned long long*)(ws + pp.off_hot + 4096), GQ_HOT_SLOTS,
-                           GQ_HOT_SAMPLE, GQ_HOT_THRESHOLD, hot, GQ_HOT_MAX, ctx->num_sms, &nl));
+    e = PROF(ctx, "gq_k_hot_keys(5)", gq_launch_hot_keys(ctx->stream, kc.data, (int)kc.dtype, in->nrows, (unsigned long long*)(ws + pp.off_hot + GQ_HOT_LIST_BYTES), GQ_HOT_SLOTS,
+                           GQ_HOT_SAMPLE, GQ_HOT_THRESHOLD_SCATTER, hot, GQ_HOT_MAX_SCATTER, ctx->num_sms, &nl));
     if (e != cudaSuccess) return cuda_fail(ctx, e, "heavy-hitter sampling");
     ctx->launches += nl;
     P.hot = hot;

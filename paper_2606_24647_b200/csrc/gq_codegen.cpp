@@ -236,10 +236,12 @@ static gq_status emit_linear(Gen& g, const GqScanSpec& sp, std::ostringstream& o
   // hot keys of a skewed batch (DESIGN 5.4): rows whose key is in the batch's hot list are aggregated in CTA-shared
   // memory and leave the row set; the CTA flushes its partial groups once, at the end of the kernel
   auto emit_hot = [&]() {
-    o << "#if GQ_HOT\n  if (cx.nhot > 0) {\n  " << LOOP << "if (live[j]) {\n      const int hp = gq_hot_find(cx, tkey[j]);\n"
-      << "      if (hp >= 0) {\n";
+    o << "#if GQ_HOT\n  if (cx.nhot > 0) {\n  int hpos[GQ_R];\n  " << LOOP << "hpos[j] = live[j] ? gq_hot_find(cx, tkey[j]) : -1;\n"
+      << "  " << LOOP << "{\n      const int hp = hpos[j];\n      if (hp >= 0) {\n";
     for (int a = 0; a < nagg; ++a)
-      o << "        gq_hot_update(" << (int)sp.aggs[(size_t)a].op << ", cx, hp, " << a << ", " << aggval(sp.aggs[(size_t)a]) << ");\n";
+      o << "        const u64 hg" << a << " = gq_hot_issue(" << (int)sp.aggs[(size_t)a].op << ", cx, hp, " << a << ", " << aggval(sp.aggs[(size_t)a]) << ");\n";
+    for (int a = 0; a < nagg; ++a)
+      o << "        gq_hot_finish(" << (int)sp.aggs[(size_t)a].op << ", cx, hp, " << a << ", " << aggval(sp.aggs[(size_t)a]) << ", hg" << a << ");\n";
     o << "        cx.hot_touched[hp] = 1;\n        live[j] = false;\n      }\n    }\n  }\n#endif\n";
   };
   switch (sp.consumer) {
@@ -439,7 +441,17 @@ gq_status gq_codegen(const GqScanSpec& sp, GqKernelInfo* out, std::string* msg) 
   bool all_unique = true;
   for (const GqProbeSpec& ps : sp.probes) all_unique = all_unique && ps.unique;
   const bool use_hot = sp.hot && (sp.consumer == GQ_C_HIGHCARD || sp.consumer == GQ_C_PARTITION || sp.consumer == GQ_C_SCATTER) && all_unique;   // linear mode only
-  if (use_hot) cons_bytes = 512 * 8 + 512LL * nagg * 8 + 512 * 4 + 256;
+  // hot set: 512 positions (<= 256 keys); pass A takes 2048 (<= 1536 keys: on a Zipf(1) key column every doubling of the
+  // hot set keeps another 4 % of the rows out of the record stream) when a 3-stage ring of one-row-per-thread tiles
+  // still fits beside it and the partition state words
+  int hot_pos = 512;
+  if (use_hot && sp.consumer == GQ_C_SCATTER) {
+    long long st1 = 0;
+    for (int c : g.cols) st1 += ((long long)nt * gq_dtype_bytes(sp.in_dtype[(size_t)c]) + 127) / 128 * 128;
+    const long long hb = 2048LL * (8 + 8 * nagg + 4) + 256 + 128 + (sp.part_states / std::max(1, sp.cluster)) * 4LL + 64;
+    if (GQ_SMEM_LIMIT - hb - 2 * 4 * 8 - 64 - 128 >= 3 * st1) hot_pos = 2048;
+  }
+  if (use_hot) cons_bytes = hot_pos * 8LL + (long long)hot_pos * nagg * 8 + hot_pos * 4LL + 256;
   long long part_state_off = 0;
   if (sp.part_rw > 0) {   // partition state words (+ the CTA's chunk counter)
     if (sp.part_states < 1 || sp.part_states > 16384) { if (msg) *msg = "bad partition count"; return GQ_ERR_INVALID_ARG; }
@@ -466,6 +478,7 @@ gq_status gq_codegen(const GqScanSpec& sp, GqKernelInfo* out, std::string* msg) 
   o << "// generated by gq_codegen — plan-shape specialised prelude\n";
   // (part of the source, hence of the kernel's identity: two plans that differ only in their shared-memory carve-up,
   // e.g. in the number of partition state words, must not share a cached kernel and its launch configuration)
+  if (use_hot) o << "#define GQ_HOT_POS " << hot_pos << "\n#define GQ_HOT_MAX " << (hot_pos == 2048 ? 1536 : 256) << "\n";
   o << "#define GQ_SC_CLUSTER " << (sp.consumer == GQ_C_SCATTER ? std::max(1, sp.cluster) : 1) << "\n";
   o << "#define GQ_SMEM_BYTES " << (stages * stage_bytes + 2 * stages * 8 + 64 + cons_bytes + 128) << "\n";
   o << "#define GQ_NCOL " << ncol << "\n#define GQ_NT " << nt << "\n#define GQ_R " << r << "\n#define GQ_STAGES "

@@ -260,9 +260,12 @@ struct GqPsaDirParams {
 cudaError_t gq_launch_psa_dir(cudaStream_t s, const GqPsaDirParams& p);
 cudaError_t gq_launch_psa_fill(cudaStream_t s, const unsigned* info, const unsigned* ncta, int nctas, long long slab,
                                const unsigned* pstart, unsigned* pfill, unsigned* plist);
-#define GQ_HOT_MAX 256               // hot keys per batch (shared-memory set of 2*GQ_HOT_MAX positions per CTA)
+#define GQ_HOT_MAX 256               // hot keys per batch of the global-table paths (shared set of 512 positions per CTA)
+#define GQ_HOT_MAX_SCATTER 1536      // ... of pass A of the partitioned aggregation (2048 positions, when they fit shared memory)
+#define GQ_HOT_LIST_BYTES 16384      // hot list: 32 header words + keys
 #define GQ_HOT_SAMPLE (1LL << 19)    // sampled rows
 #define GQ_HOT_SLOTS (1LL << 20)     // (key,count) sample table slots (16 B each)
-#define GQ_HOT_THRESHOLD 128         // sample count that makes a key hot (share >= 2^-12)
+#define GQ_HOT_THRESHOLD 128         // sample count that makes a key hot (share >= 2^-12): global-table paths
+#define GQ_HOT_THRESHOLD_SCATTER 16  // ... pass A: every row kept out of the record stream pays (share >= 2^-15)
 #define GQ_HOT_MIN_ROWS (1LL << 22)  // batches smaller than this skip the heavy-hitter pass
 #endif

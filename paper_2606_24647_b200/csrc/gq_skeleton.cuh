@@ -882,9 +882,11 @@ __device__ __forceinline__ void gq_lc_update(const int OP, GqCtx& cx, int grp, i
 // are accumulated in CTA-shared memory and flushed to the global table once per CTA, instead of hammering one L2
 // address with hundreds of millions of atomics. 64-bit shared atomics are CAS loops on sm_100 (ATOMS.CAST.SPIN), so
 // SUM/COUNT use two native 32-bit ATOMS.ADD with an explicit carry; MIN/MAX compare first and CAS only to improve.
-#define GQ_HOT_POS 512
+#ifndef GQ_HOT_POS      // (set by the plan compiler: 512 positions for <= 256 keys; pass A of the partitioned aggregation
+#define GQ_HOT_POS 512  // takes 2048 positions for <= 1536 keys when they fit beside a 3-stage ring)
 #define GQ_HOT_MAX 256
-// The hot set is bucketised: 128 buckets of 4 keys (GQ_HOT_POS positions for <= GQ_HOT_MAX keys). A key sits in the bucket
+#endif
+// The hot set is bucketised: GQ_HOT_POS / 4 buckets of 4 keys (GQ_HOT_POS positions for <= GQ_HOT_MAX keys). A key sits in the bucket
 // its hash names unless that bucket was full when it was inserted (then in the next one), so a lookup reads one
 // 32-byte bucket (two LDS.128) and almost always stops there: a bucket with a free position was never full. (The
 // position-by-position linear probe it replaces was a third of pass A's instructions on C5: every row of a warp walked
@@ -908,16 +910,22 @@ __device__ __forceinline__ int gq_hot_find(const GqCtx& cx, i64 key) {
   }
   return -1;
 }
-__device__ __forceinline__ void gq_hot_update(const int OP, GqCtx& cx, int pos, int a, i64 v) {
+// A hot row's update in two phases, so that the shared-memory round trips of its aggregates overlap: gq_hot_issue sends
+// the low-word add (SUM / COUNT) or reads the cell (MIN / MAX) and returns what came back; gq_hot_finish propagates the
+// carry / runs the compare-and-swap loop.
+__device__ __forceinline__ u64 gq_hot_issue(const int OP, GqCtx& cx, int pos, int a, i64 v) {
+  u64* cell = cx.hot_acc + pos * GQ_NAGG + a;
+  if (OP == GQ_OP_SUM || OP == GQ_OP_COUNT) return (u64)atomicAdd((u32*)cell, (u32)(u64)v);
+  return *(volatile u64*)cell;
+}
+__device__ __forceinline__ void gq_hot_finish(const int OP, GqCtx& cx, int pos, int a, i64 v, u64 got) {
   u64* cell = cx.hot_acc + pos * GQ_NAGG + a;
   if (OP == GQ_OP_SUM || OP == GQ_OP_COUNT) {
-    u32* w = (u32*)cell;
-    const u32 lo = (u32)(u64)v, hi = (u32)((u64)v >> 32);
-    const u32 old = atomicAdd(w, lo);
+    const u32 lo = (u32)(u64)v, hi = (u32)((u64)v >> 32), old = (u32)got;
     const u32 up = hi + ((u32)(old + lo) < old ? 1u : 0u);   // carry out of the low word belongs to THIS addition
-    if (up) atomicAdd(w + 1, up);
+    if (up) atomicAdd((u32*)cell + 1, up);
   } else {
-    i64 cur = *(volatile i64*)cell;
+    i64 cur = (i64)got;
     while (OP == GQ_OP_MIN ? v < cur : v > cur) {
       const i64 prev = (i64)atomicCAS(cell, (u64)cur, (u64)v);
       if (prev == cur) break;

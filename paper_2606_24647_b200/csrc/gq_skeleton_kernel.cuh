@@ -184,7 +184,7 @@ extern "C" __global__ void __launch_bounds__(GQ_NT + 32, 1) gq_scan(const __grid
       for (int a = 0; a < GQ_NAGG; ++a) cx.hot_acc[i * GQ_NAGG + a] = (u64)gq_identity(GQ_AGG_OP(a));
     }
     __syncthreads();
-    if (tid < cx.nhot) gq_hot_insert(cx, P.hot[32 + tid]);   // this batch's hot keys into the shared set (distinct by construction)
+    for (int i = tid; i < cx.nhot; i += GQ_NT + 32) gq_hot_insert(cx, P.hot[32 + i]);   // this batch's hot keys into the shared set (distinct by construction)
   }
 #endif
   __syncthreads();

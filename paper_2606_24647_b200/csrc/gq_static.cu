@@ -656,19 +656,21 @@ __global__ void gq_k_hot_hist(const u64* table, i64 nslots, u64 threshold, i64* 
   if (b < 1) b = 1;
   atomicAdd((u64*)&hot[b], 1ULL);
 }
-__global__ void gq_k_hot_select(const u64* table, i64 nslots, u64 threshold, i64* hot, int max_hot) {
+// pass 0 takes every key at or above the raised threshold (at most max_hot of them, by construction); pass 1 fills the
+// list up with keys of the bin just below it (sample counts within a factor of two of one another: any subset will do).
+__global__ void gq_k_hot_select(const u64* table, i64 nslots, u64 threshold, i64* hot, int max_hot, int pass) {
   const i64 i = (i64)blockIdx.x * blockDim.x + threadIdx.x;
   if (i >= nslots) return;
   const u64 k = table[i * 2];
   const u64 c = table[i * 2 + 1];
   if (k == GQ_EMPTY_KEY || c < threshold) return;
-  u64 t = threshold;                          // every thread derives the same raised threshold from the histogram
+  u64 t = threshold, lo = threshold;          // every thread derives the same raised threshold from the histogram
   i64 above = 0;
   for (int b = 31; b >= 1; --b) {
     above += hot[b];
-    if (above > max_hot) { const u64 tb = 1ULL << (b + 1); if (tb > t) t = tb; break; }
+    if (above > max_hot) { const u64 tb = 1ULL << (b + 1); if (tb > t) { t = tb; lo = tb >> 1; if (lo < threshold) lo = threshold; } break; }
   }
-  if (c < t) return;
+  if (pass == 0 ? c < t : (c >= t || c < lo)) return;
   i64 idx = (i64)atomicAdd((u64*)hot, 1ULL);
   if (idx < max_hot) hot[32 + idx] = (i64)k;
 }
@@ -686,7 +688,8 @@ cudaError_t gq_launch_hot_keys(cudaStream_t s, const void* keycol, int dtype, i6
   gq_k_hot_sample<<<(unsigned)((nsample + 255) / 256), 256, 0, s>>>(keycol, dtype, nrows, stride, nsample, table,
                                                                    (u64)(nslots - 1), shift);
   gq_k_hot_hist<<<(unsigned)((nslots + 255) / 256), 256, 0, s>>>(table, nslots, threshold, hot);
-  gq_k_hot_select<<<(unsigned)((nslots + 255) / 256), 256, 0, s>>>(table, nslots, threshold, hot, max_hot);
-  *nlaunches = 4;
+  gq_k_hot_select<<<(unsigned)((nslots + 255) / 256), 256, 0, s>>>(table, nslots, threshold, hot, max_hot, 0);
+  gq_k_hot_select<<<(unsigned)((nslots + 255) / 256), 256, 0, s>>>(table, nslots, threshold, hot, max_hot, 1);
+  *nlaunches = 5;
   return cudaGetLastError();
 }

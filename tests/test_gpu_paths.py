@@ -482,8 +482,14 @@ def test_partitioned_shared_memory_aggregation_hot_keys_and_sub_passes(ctx, forc
                 gq.set_option("psa_threads", th)
                 l0 = ctx.launch_count()
                 exp, got = run(plan, ctx)
-                assert ctx.launch_count() - l0 == 10     # + table init and three kernels of the heavy-hitter sampling
+                assert ctx.launch_count() - l0 == 11     # + table init and four kernels of the heavy-hitter sampling
                 assert int(got["cols"][-1].max()) > 100_000
+        # more keys reach the sampling threshold than the hot set holds (3000 equally frequent keys + a long tail): the
+        # selection raises its threshold past all of them and fills the list from the bin below it
+        gq.set_option("psa_max_log2_partitions", -1); gq.set_option("psa_threads", 0)
+        k2 = rng.integers(0, 3000, n).astype(np.int64) * 11 - 5000
+        k2[::7] = rng.integers(10**6, 10**6 + 200_000, len(k2[::7]))
+        run(dict(plan, table=[k2, v, w]), ctx)
     finally:
         gq.set_option("hot_min_rows", -1); gq.set_option("psa_max_log2_partitions", -1); gq.set_option("psa_threads", 0)
         gq.set_option("psa_cluster", 2)
@@ -554,11 +560,18 @@ def test_pipeline_is_cuda_graph_capturable():
         p.run()
         c.sync()
         g = torch.cuda.CUDAGraph()
-        with torch.cuda.graph(g, stream=s):
-            tables = gqrun.build_tables(c, plan, device_tables=bcols, workspaces=ws)
-            pr, _ = p.m.probes([(tables[bi], kc) for bi, kc in plan["probes"]])
-            p.plan.agg.probes = pr
-            p.run()
+        # (no cyclic garbage collection inside the capture: a context of an earlier test collected there would cudaFree,
+        # which invalidates a capture in progress)
+        import gc
+        gc.collect(); gc.disable()
+        try:
+            with torch.cuda.graph(g, stream=s):
+                tables = gqrun.build_tables(c, plan, device_tables=bcols, workspaces=ws)
+                pr, _ = p.m.probes([(tables[bi], kc) for bi, kc in plan["probes"]])
+                p.plan.agg.probes = pr
+                p.run()
+        finally:
+            gc.enable()
         for _ in range(3):
             for a in p.aggs:
                 a.zero_()
