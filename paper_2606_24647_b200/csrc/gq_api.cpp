@@ -814,7 +814,7 @@ PsaPlan psa_plan(const GqScanSpec& sp, const gq_agg_desc* d, int64_t nrows, int 
   auto take = [&off](size_t b) { size_t o = off; off += align_up(b, 256); return o; };
   pp.off_zero = take(256);                                   // [0] work cursor, [1] item count
   pp.off_pcount = take((size_t)pp.npart * 4);
-  pp.off_pfill = take((size_t)pp.npart * 4);
+  pp.off_pfill = take((size_t)pp.npart * 4 * GQ_PSA_FILL_STRIDE);   // one fill cursor per 32-byte sector
   pp.zero_bytes = off;                                       // zeroed before every run
   pp.off_pstart = take((size_t)(pp.npart + 1) * 4);
   pp.off_items = take((size_t)pp.max_items * 4);

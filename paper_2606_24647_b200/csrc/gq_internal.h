@@ -258,6 +258,7 @@ struct GqPsaDirParams {
   int* err; unsigned max_items; unsigned nsub;
 };
 cudaError_t gq_launch_psa_dir(cudaStream_t s, const GqPsaDirParams& p);
+#define GQ_PSA_FILL_STRIDE 8   // words between the fill cursors of two partitions (atomics on one L2 sector serialise)
 cudaError_t gq_launch_psa_fill(cudaStream_t s, const unsigned* info, const unsigned* ncta, int nctas, long long slab,
                                const unsigned* pstart, unsigned* pfill, unsigned* plist);
 #define GQ_HOT_MAX 256               // hot keys per batch of the global-table paths (shared set of 512 positions per CTA)

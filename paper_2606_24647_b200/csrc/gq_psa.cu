@@ -18,8 +18,13 @@ __global__ void __launch_bounds__(GQ_DIR_THREADS) gq_k_psa_dir(const __grid_cons
   const int t = threadIdx.x;
   const int per = (P.npart + GQ_DIR_THREADS - 1) / GQ_DIR_THREADS;
   const int lo = t * per, hi = min(P.npart, lo + per);
+  // (npart <= 16384: a thread's <= 16 counts are read once, all loads in flight together, and kept in registers)
+  u32 cnt[16];
+#pragma unroll
+  for (int i = 0; i < 16; ++i) cnt[i] = (i < per && lo + i < hi) ? P.pcount[lo + i] : 0u;
   u32 s = 0;
-  for (int p = lo; p < hi; ++p) s += P.pcount[p];
+#pragma unroll
+  for (int i = 0; i < 16; ++i) s += cnt[i];
   part_sum[t] = s;
   if (t < 3) cls_n[t] = 0;
   __syncthreads();
@@ -31,12 +36,14 @@ __global__ void __launch_bounds__(GQ_DIR_THREADS) gq_k_psa_dir(const __grid_cons
   }
   const u32 total = part_sum[GQ_DIR_THREADS - 1];
   u32 run = part_sum[t] - s;
-  for (int p = lo; p < hi; ++p) { P.pstart[p] = run; run += P.pcount[p]; }
+#pragma unroll
+  for (int i = 0; i < 16; ++i) if (i < per && lo + i < hi) { P.pstart[lo + i] = run; run += cnt[i]; }
   if (t == 0) P.pstart[P.npart] = total;
   const u32 big = 4 * (total / (u32)P.npart) + 64;
   auto cls = [&](u32 n) { return n > P.seg_chunks ? 0 : n > big ? 1 : 2; };
-  for (int p = lo; p < hi; ++p) {
-    const u32 n = P.pcount[p];
+#pragma unroll
+  for (int i = 0; i < 16; ++i) {
+    const u32 n = cnt[i];
     if (n) atomicAdd(&cls_n[cls(n)], (n > P.seg_chunks ? (n + P.seg_chunks - 1) / P.seg_chunks : 1u) * P.nsub);
   }
   __syncthreads();
@@ -47,8 +54,10 @@ __global__ void __launch_bounds__(GQ_DIR_THREADS) gq_k_psa_dir(const __grid_cons
   }
   __syncthreads();
   if (cls_n[0] + cls_n[1] + cls_n[2] > P.max_items) return;
-  for (int p = lo; p < hi; ++p) {
-    const u32 n = P.pcount[p];
+#pragma unroll
+  for (int i = 0; i < 16; ++i) {
+    const u32 n = cnt[i];
+    const int p = lo + i;
     if (!n) continue;
     const u32 k = n > P.seg_chunks ? (n + P.seg_chunks - 1) / P.seg_chunks : 1u;
     const u32 at = atomicAdd(&cls_cur[cls(n)], k * P.nsub);   // the sub-passes of a segment are neighbours in the queue: the
@@ -58,6 +67,7 @@ __global__ void __launch_bounds__(GQ_DIR_THREADS) gq_k_psa_dir(const __grid_cons
   }
 }
 cudaError_t gq_launch_psa_dir(cudaStream_t s, const GqPsaDirParams& p) {
+  if (p.npart > 16 * GQ_DIR_THREADS) return cudaErrorInvalidValue;   // a thread keeps its <= 16 counts in registers
   gq_k_psa_dir<<<1, GQ_DIR_THREADS, 0, s>>>(p);
   return cudaGetLastError();
 }
@@ -68,17 +78,22 @@ __global__ void __launch_bounds__(256) gq_k_psa_fill(const u32* info, const u32*
                                                      u32* plist) {
   const u32 c = blockIdx.y;
   const u32 n = ncta[c];
-  for (u32 l = blockIdx.x * blockDim.x + threadIdx.x; l < n; l += gridDim.x * blockDim.x) {
-    const u64 gid = (u64)c * (u64)slab + l;
-    const u32 e = info[gid];
-    const u32 p = e >> 8, used = e & 0xFFu;
-    const u32 pos = atomicAdd(&pfill[p], 1u);
-    plist[pstart[p] + pos] = (u32)gid | (used << GQ_PSA_GID_BITS);
+  // four chunks per thread and iteration: the kernel is a chain of dependent L2 round trips (word -> counter -> start ->
+  // store), so it is the number of chains in flight that sets its speed
+  for (u32 l0 = (blockIdx.x * blockDim.x + threadIdx.x) * 4u; l0 < n; l0 += gridDim.x * blockDim.x * 4u) {
+    const u64 gid0 = (u64)c * (u64)slab + l0;
+    u32 e[4], pos[4], st[4];
+#pragma unroll
+    for (int u = 0; u < 4; ++u) e[u] = l0 + u < n ? info[gid0 + u] : 0u;
+#pragma unroll
+    for (int u = 0; u < 4; ++u) if (l0 + u < n) { pos[u] = atomicAdd(&pfill[(e[u] >> 8) * GQ_PSA_FILL_STRIDE], 1u); st[u] = pstart[e[u] >> 8]; }
+#pragma unroll
+    for (int u = 0; u < 4; ++u) if (l0 + u < n) plist[st[u] + pos[u]] = (u32)(gid0 + u) | ((e[u] & 0xFFu) << GQ_PSA_GID_BITS);
   }
 }
 cudaError_t gq_launch_psa_fill(cudaStream_t s, const u32* info, const u32* ncta, int nctas, long long slab, const u32* pstart,
                                u32* pfill, u32* plist) {
-  const unsigned bx = (unsigned)std::min<long long>(64, std::max<long long>(1, (slab + 255) / 256));
+  const unsigned bx = (unsigned)std::min<long long>(64, std::max<long long>(1, (slab + 1023) / 1024));
   gq_k_psa_fill<<<dim3(bx, (unsigned)nctas), 256, 0, s>>>(info, ncta, slab, pstart, pfill, plist);
   return cudaGetLastError();
 }
