@@ -1435,7 +1435,7 @@ gq_status gq_set_option(const char* h_name, int64_t value) {
   if (n == "part_min_table_mb") g_part_min_table_mb = value < 0 ? 256 : value;
   else if (n == "part_min_rows") g_part_min_rows = value < 0 ? (1 << 24) : value;
   else if (n == "hot_min_rows") g_hot_min_rows = value < 0 ? GQ_HOT_MIN_ROWS : value;
-  else if (n == "psa_cluster") g_psa_cluster = value == 1 ? 1 : 2;   // (clusters of 4 were measured: 132 co-resident CTAs, pass A 9.5 -> 10.9 ms)
+  else if (n == "psa_cluster") g_psa_cluster = value == 1 ? 1 : 2;   // (clusters of 4 were measured twice: 132 co-resident CTAs, pass A 9.5 -> 10.9 ms, later 7.6 -> 8.7 ms)
   else if (n == "dpart_min_acc_mb") g_dpart_min_acc_mb = value < 0 ? GQ_DPART_OFF : value;
   else if (n == "psa_threads") g_psa_threads = (value == 512 || value == 1024) ? value : 0;
   else if (n == "psa_max_log2_partitions") g_psa_max_log2part = value < 0 ? GQ_PSA_MAX_LOG2PART : value;

@@ -204,6 +204,63 @@ __device__ __forceinline__ void gq_list_feed(GqCand& mine, const GqCand& c, bool
 #define GQ_TOPK_BLOCKS 592
 #define GQ_TOPK_WARPS 8
 #define GQ_TOPK_UNROLL 4
+// scratch layout: [GQ_TOPK_BLOCKS][32] GqCand lists | [GQ_TOPK_BOUND_BLOCKS] i64 sample maxima | [GQ_TOPK_BLOCKS] int entries per list
+#define GQ_TOPK_BOUND_BLOCKS 64
+#define GQ_TOPK_BOUND_PER 16
+#define GQ_TOPK_NONE ((i64)0x8000000000000000LL)
+__device__ __forceinline__ i64* gq_topk_maxima(const GqFinaliseParams& P) { return (i64*)((GqCand*)P.scratch + 32 * GQ_TOPK_BLOCKS); }
+__device__ __forceinline__ int* gq_topk_counts(const GqFinaliseParams& P) { return (int*)(gq_topk_maxima(P) + GQ_TOPK_BOUND_BLOCKS); }
+// validity and ordering aggregate of slot i (loaded unconditionally: several of these are in flight per thread)
+__device__ __forceinline__ void gq_topk_peek(const GqFinaliseParams& P, i64 i, u64& tv, i64& vv) {
+  const i64 ii = i < P.capacity ? i : 0;
+  if (P.direct) { tv = P.dacc[ii * P.daw + P.dtouch]; vv = (i64)P.dacc[ii * P.daw + P.topk_agg]; }
+  else {
+    const u64* sl = P.slots + ii * P.slot_words;
+    tv = sl[0] != GQ_EMPTY_KEY; vv = (i64)sl[1 + P.ndep + P.topk_agg];
+  }
+  if (i >= P.capacity) tv = 0;
+}
+// pass 0: an admission bound for pass 1. Every block takes the maximum of the ordering aggregate over a strided sample of
+// the table; the k-th largest of the GQ_TOPK_BOUND_BLOCKS maxima is a value that at least k groups reach, so no group
+// below it can be among the first k. (Without it every warp of pass 1 fills and sorts a list of its own first: the scan
+// was bound by shuffles, 97 us for 132 MB on C3.)
+__global__ void __launch_bounds__(256) gq_k_topk_bound(const __grid_constant__ GqFinaliseParams P) {
+  __shared__ i64 wmax[8];
+  const i64 nt = (i64)GQ_TOPK_BOUND_BLOCKS * 256;
+  const i64 t = (i64)blockIdx.x * 256 + threadIdx.x;
+  i64 stride = P.capacity / (nt * GQ_TOPK_BOUND_PER);
+  if (stride < 1) stride = 1;
+  u64 tv[GQ_TOPK_BOUND_PER];
+  i64 vv[GQ_TOPK_BOUND_PER];
+#pragma unroll
+  for (int u = 0; u < GQ_TOPK_BOUND_PER; ++u) gq_topk_peek(P, ((i64)u * nt + t) * stride, tv[u], vv[u]);
+  i64 best = GQ_TOPK_NONE;
+#pragma unroll
+  for (int u = 0; u < GQ_TOPK_BOUND_PER; ++u) if (tv[u] != 0 && vv[u] > best) best = vv[u];
+  for (int o = 16; o > 0; o >>= 1) { const i64 x = __shfl_xor_sync(0xffffffffu, best, o); if (x > best) best = x; }
+  if ((threadIdx.x & 31) == 0) wmax[threadIdx.x >> 5] = best;
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    for (int w = 1; w < 8; ++w) if (wmax[w] > best) best = wmax[w];
+    gq_topk_maxima(P)[blockIdx.x] = best;
+  }
+}
+// the k-th largest of the sample maxima (GQ_TOPK_NONE = "no bound" when fewer than k blocks saw a group); warp-uniform
+__device__ __forceinline__ i64 gq_topk_bound_value(const GqFinaliseParams& P, int lane) {
+  const i64* M = gq_topk_maxima(P);
+  const i64 m0 = M[lane], m1 = M[lane + 32];
+  int c0 = 0, c1 = 0;
+  for (int j = 0; j < 32; ++j) {
+    const i64 a = __shfl_sync(0xffffffffu, m0, j), b = __shfl_sync(0xffffffffu, m1, j);
+    c0 += (a >= m0) + (b >= m0);
+    c1 += (a >= m1) + (b >= m1);
+  }
+  i64 best = GQ_TOPK_NONE;
+  if (c0 >= P.topk && m0 > best) best = m0;
+  if (c1 >= P.topk && m1 > best) best = m1;
+  for (int o = 16; o > 0; o >>= 1) { const i64 x = __shfl_xor_sync(0xffffffffu, best, o); if (x > best) best = x; }
+  return best;
+}
 // pass 1: every warp scans a strided share of the table (GQ_TOPK_UNROLL chunks of 32 slots in flight) and keeps its
 // own best list; lists go to scratch.
 __global__ void __launch_bounds__(GQ_TOPK_WARPS * 32, 4) gq_k_topk_scan(const __grid_constant__ GqFinaliseParams P) {
@@ -221,27 +278,26 @@ __global__ void __launch_bounds__(GQ_TOPK_WARPS * 32, 4) gq_k_topk_scan(const __
     if (lane == 0 && gq_group_at(P, si, &g)) { c = gq_make_cand(P, g, si); want = true; }
     gq_list_feed(mine, c, want, lane, kth);
   }
+  // admission bound, warp-uniform: the larger of pass 0's bound and the value of the list's k-th entry; refreshed after
+  // every insertion, so the common iteration is two loads, a compare and a vote
+  i64 bound = gq_topk_bound_value(P, lane);
+  {
+    const GqCand w0 = gq_cand_shfl(mine, kth);
+    if (w0.valid && w0.val > bound) bound = w0.val;
+  }
   for (i64 i0 = gw * 32; i0 < P.capacity; i0 += nw * 32 * GQ_TOPK_UNROLL) {
     // validity word and ordering aggregate of GQ_TOPK_UNROLL slots, loaded unconditionally (all in flight together);
     // the full candidate (keys) is only built for the few slots that can still enter the list
     u64 tv[GQ_TOPK_UNROLL];
     i64 vv[GQ_TOPK_UNROLL];
 #pragma unroll
-    for (int u = 0; u < GQ_TOPK_UNROLL; ++u) {
-      const i64 i = i0 + (i64)u * nw * 32 + lane;
-      const i64 ii = i < P.capacity ? i : 0;
-      if (P.direct) { tv[u] = P.dacc[ii * P.daw + P.dtouch]; vv[u] = (i64)P.dacc[ii * P.daw + P.topk_agg]; }
-      else {
-        const u64* sl = P.slots + ii * P.slot_words;
-        tv[u] = sl[0] != GQ_EMPTY_KEY; vv[u] = (i64)sl[1 + P.ndep + P.topk_agg];
-      }
-      if (i >= P.capacity) tv[u] = 0;
-    }
+    for (int u = 0; u < GQ_TOPK_UNROLL; ++u) gq_topk_peek(P, i0 + (i64)u * nw * 32 + lane, tv[u], vv[u]);
 #pragma unroll
     for (int u = 0; u < GQ_TOPK_UNROLL; ++u) {
+      bool want = tv[u] != 0 && vv[u] >= bound;
+      if (!__any_sync(0xffffffffu, want)) continue;
       const i64 i = i0 + (i64)u * nw * 32 + lane;
       const GqCand worst = gq_cand_shfl(mine, kth);
-      bool want = tv[u] != 0 && (!worst.valid || vv[u] >= worst.val);
       GqCand c; c.valid = 0; c.val = 0; c.k0 = 0; c.k1 = 0; c.slot = -1;
       if (want) {
         GqGroupRef g;
@@ -249,6 +305,8 @@ __global__ void __launch_bounds__(GQ_TOPK_WARPS * 32, 4) gq_k_topk_scan(const __
         if (want) { c = gq_make_cand(P, g, i); want = gq_better(c, worst); }
       }
       gq_list_feed(mine, c, want, lane, kth);
+      const GqCand w1 = gq_cand_shfl(mine, kth);
+      if (w1.valid && w1.val > bound) bound = w1.val;
     }
   }
   // merge the block's GQ_TOPK_WARPS lists into one (warp 0), so pass 2 sees one list per block
@@ -262,6 +320,8 @@ __global__ void __launch_bounds__(GQ_TOPK_WARPS * 32, 4) gq_k_topk_scan(const __
       gq_list_feed(mine, c, c.valid && lane <= kth && gq_better(c, worst), lane, kth);   // entries behind the k-th of a sorted list cannot matter
     }
     ((GqCand*)P.scratch)[(i64)blockIdx.x * 32 + lane] = mine;
+    const unsigned have = __ballot_sync(0xffffffffu, mine.valid != 0 && lane <= kth);
+    if (lane == 0) gq_topk_counts(P)[blockIdx.x] = __popc(have);
   }
 }
 // pass 2: one block; every warp merges a strided share of the per-block lists (two lists in flight), warp 0 merges the
@@ -274,15 +334,19 @@ __global__ void __launch_bounds__(GQ_TOPK_MERGE_WARPS * 32) gq_k_topk_merge(cons
   const int kth = P.topk - 1;
   const GqCand* in = (const GqCand*)P.scratch;
   GqCand mine; mine.valid = 0; mine.val = 0; mine.k0 = 0; mine.k1 = 0; mine.slot = -1;
-  for (i64 l = warp; l < nlists; l += 2 * GQ_TOPK_MERGE_WARPS) {
-    const i64 l2 = l + GQ_TOPK_MERGE_WARPS;
-    GqCand c0 = in[l * 32 + lane], c1;
-    c1.valid = 0; c1.val = 0; c1.k0 = 0; c1.k1 = 0; c1.slot = -1;
-    if (l2 < nlists) c1 = in[l2 * 32 + lane];
-    GqCand worst = gq_cand_shfl(mine, kth);
-    gq_list_feed(mine, c0, c0.valid && lane <= kth && gq_better(c0, worst), lane, kth);
-    worst = gq_cand_shfl(mine, kth);
-    gq_list_feed(mine, c1, c1.valid && lane <= kth && gq_better(c1, worst), lane, kth);
+  // lists l = warp, warp + 32, ...: lane j looks at the entry count of the j-th of them, the warp visits the non-empty ones
+  // (with pass 0's bound most blocks admit nothing)
+  const int* cnt = gq_topk_counts(P);
+  for (i64 base = warp; base < nlists; base += 32 * GQ_TOPK_MERGE_WARPS) {
+    const i64 lj = base + (i64)lane * GQ_TOPK_MERGE_WARPS;
+    unsigned m = __ballot_sync(0xffffffffu, lj < nlists && cnt[lj] > 0);
+    while (m) {
+      const int j = __ffs(m) - 1;
+      m &= m - 1;
+      const GqCand c0 = in[(base + (i64)j * GQ_TOPK_MERGE_WARPS) * 32 + lane];
+      const GqCand worst = gq_cand_shfl(mine, kth);
+      gq_list_feed(mine, c0, c0.valid && lane <= kth && gq_better(c0, worst), lane, kth);
+    }
   }
   sh[warp][lane] = mine;
   __syncthreads();
@@ -302,13 +366,14 @@ __global__ void __launch_bounds__(GQ_TOPK_MERGE_WARPS * 32) gq_k_topk_merge(cons
   if (lane == 0) *P.out_n = n;
 }
 
-size_t gq_topk_scratch_bytes_impl() { return sizeof(GqCand) * 32 * GQ_TOPK_BLOCKS; }
+size_t gq_topk_scratch_bytes_impl() { return sizeof(GqCand) * 32 * GQ_TOPK_BLOCKS + 8 * GQ_TOPK_BOUND_BLOCKS + 4 * GQ_TOPK_BLOCKS; }
 
 cudaError_t gq_launch_finalise(cudaStream_t s, const GqFinaliseParams& p, int num_sms, int* nlaunches) {
   if (p.topk > 0) {
+    gq_k_topk_bound<<<GQ_TOPK_BOUND_BLOCKS, 256, 0, s>>>(p);
     gq_k_topk_scan<<<GQ_TOPK_BLOCKS, GQ_TOPK_WARPS * 32, 0, s>>>(p);
     gq_k_topk_merge<<<1, GQ_TOPK_MERGE_WARPS * 32, 0, s>>>(p, (i64)GQ_TOPK_BLOCKS);
-    *nlaunches = 2;
+    *nlaunches = 3;
   } else {
     i64 nb = (p.capacity + GQ_FIN_THREADS * GQ_FIN_PER - 1) / (GQ_FIN_THREADS * GQ_FIN_PER);
     int blocks = (int)std::max<i64>(1, std::min<i64>(nb, (i64)num_sms * 8));
