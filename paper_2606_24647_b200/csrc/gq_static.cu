@@ -208,6 +208,7 @@ __device__ __forceinline__ void gq_list_feed(GqCand& mine, const GqCand& c, bool
 #define GQ_TOPK_BOUND_BLOCKS 64
 #define GQ_TOPK_BOUND_PER 16
 #define GQ_TOPK_NONE ((i64)0x8000000000000000LL)
+#define GQ_TOPK_RANK_MAX 1024   // entries the merge ranks by counting (4 x 8 B each in the merge's shared memory)
 __device__ __forceinline__ i64* gq_topk_maxima(const GqFinaliseParams& P) { return (i64*)((GqCand*)P.scratch + 32 * GQ_TOPK_BLOCKS); }
 __device__ __forceinline__ int* gq_topk_counts(const GqFinaliseParams& P) { return (int*)(gq_topk_maxima(P) + GQ_TOPK_BOUND_BLOCKS); }
 // validity and ordering aggregate of slot i (loaded unconditionally: several of these are in flight per thread)
@@ -329,10 +330,57 @@ __global__ void __launch_bounds__(GQ_TOPK_WARPS * 32, 4) gq_k_topk_scan(const __
 #define GQ_TOPK_MERGE_WARPS 32
 __global__ void __launch_bounds__(GQ_TOPK_MERGE_WARPS * 32) gq_k_topk_merge(const __grid_constant__ GqFinaliseParams P, i64 nlists) {
   if (*(volatile int*)P.err != 0) return;
-  __shared__ GqCand sh[GQ_TOPK_MERGE_WARPS][32];
+  __shared__ __align__(16) unsigned char shbuf[sizeof(GqCand) * 32 * GQ_TOPK_MERGE_WARPS];
+  __shared__ int s_off[GQ_TOPK_BLOCKS + 1], s_wsum[GQ_TOPK_MERGE_WARPS];
+  GqCand (*sh)[32] = (GqCand (*)[32])shbuf;
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   const int kth = P.topk - 1;
   const GqCand* in = (const GqCand*)P.scratch;
+  // ---- few entries in all lists together (the usual case with pass 0's bound: a few hundred): gather them in shared
+  // memory, every thread counts how many entries come before its own, ranks below k are output rows. (Feeding them
+  // through sorted warp lists is a chain of ~60 dependent shuffle instructions per entry: 25 us.)
+  {
+    const int t = threadIdx.x;
+    const int c = t < nlists ? gq_topk_counts(P)[t] : 0;   // (nlists = GQ_TOPK_BLOCKS <= blockDim.x)
+    int incl = c;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) { const int x = __shfl_up_sync(0xffffffffu, incl, o); if (lane >= o) incl += x; }
+    if (lane == 31) s_wsum[warp] = incl;
+    __syncthreads();
+    int before = 0;
+    for (int w = 0; w < warp; ++w) before += s_wsum[w];
+    if (t < nlists) s_off[t] = before + incl - c;
+    if (t == GQ_TOPK_MERGE_WARPS * 32 - 1) s_off[nlists] = before + incl;
+    __syncthreads();
+    const int n = s_off[nlists];
+    if (n <= GQ_TOPK_RANK_MAX) {
+      i64* sv = (i64*)shbuf; i64* sk0 = sv + GQ_TOPK_RANK_MAX; i64* sk1 = sk0 + GQ_TOPK_RANK_MAX; i64* ss = sk1 + GQ_TOPK_RANK_MAX;
+      for (int l = warp; l < nlists; l += GQ_TOPK_MERGE_WARPS) {
+        const int o = s_off[l];
+        if (lane < s_off[l + 1] - o) {
+          const GqCand e = in[(i64)l * 32 + lane];
+          sv[o + lane] = e.val; sk0[o + lane] = e.k0; sk1[o + lane] = e.k1; ss[o + lane] = e.slot;
+        }
+      }
+      __syncthreads();
+      if (t < n) {
+        const i64 v = sv[t], k0 = sk0[t], k1 = sk1[t];
+        int rank = 0;
+        for (int j = 0; j < n; ++j) {
+          const i64 a = sv[j], b0 = sk0[j], b1 = sk1[j];
+          rank += (a != v) ? (a > v) : (b0 != k0) ? (b0 < k0) : (b1 < k1);
+        }
+        if (rank < P.topk) {
+          GqGroupRef g;
+          if (rank < P.out_capacity) { gq_group_at(P, ss[t], &g); gq_emit_group(P, g, rank); }
+          else atomicCAS(P.err, 0, (int)GQ_ERR_CAPACITY);
+        }
+      }
+      if (t == 0) *P.out_n = min(n, P.topk);
+      return;
+    }
+    __syncthreads();
+  }
   GqCand mine; mine.valid = 0; mine.val = 0; mine.k0 = 0; mine.k1 = 0; mine.slot = -1;
   // lists l = warp, warp + 32, ...: lane j looks at the entry count of the j-th of them, the warp visits the non-empty ones
   // (with pass 0's bound most blocks admit nothing)
@@ -340,22 +388,38 @@ __global__ void __launch_bounds__(GQ_TOPK_MERGE_WARPS * 32) gq_k_topk_merge(cons
   for (i64 base = warp; base < nlists; base += 32 * GQ_TOPK_MERGE_WARPS) {
     const i64 lj = base + (i64)lane * GQ_TOPK_MERGE_WARPS;
     unsigned m = __ballot_sync(0xffffffffu, lj < nlists && cnt[lj] > 0);
-    while (m) {
-      const int j = __ffs(m) - 1;
-      m &= m - 1;
-      const GqCand c0 = in[(base + (i64)j * GQ_TOPK_MERGE_WARPS) * 32 + lane];
-      const GqCand worst = gq_cand_shfl(mine, kth);
-      gq_list_feed(mine, c0, c0.valid && lane <= kth && gq_better(c0, worst), lane, kth);
+    while (m) {                                            // four lists in flight: the loads are what this loop waits for
+      GqCand c[4];
+#pragma unroll
+      for (int u = 0; u < 4; ++u) {
+        c[u].valid = 0; c[u].val = 0; c[u].k0 = 0; c[u].k1 = 0; c[u].slot = -1;
+        if (m) {
+          const int j = __ffs(m) - 1;
+          m &= m - 1;
+          c[u] = in[(base + (i64)j * GQ_TOPK_MERGE_WARPS) * 32 + lane];
+        }
+      }
+#pragma unroll
+      for (int u = 0; u < 4; ++u) {
+        const GqCand worst = gq_cand_shfl(mine, kth);
+        gq_list_feed(mine, c[u], c[u].valid && lane <= kth && gq_better(c[u], worst), lane, kth);
+      }
     }
   }
+  // the warps' lists are merged pairwise (5 rounds of <= k insertions each; one warp taking the 31 others in turn was
+  // 310 dependent insertions, most of this kernel's time)
   sh[warp][lane] = mine;
   __syncthreads();
-  if (warp != 0) return;
-  for (int w = 1; w < GQ_TOPK_MERGE_WARPS; ++w) {
-    GqCand c = sh[w][lane];
-    GqCand worst = gq_cand_shfl(mine, kth);
-    gq_list_feed(mine, c, c.valid && lane <= kth && gq_better(c, worst), lane, kth);   // entries behind the k-th of a sorted list cannot matter
+  for (int step = 1; step < GQ_TOPK_MERGE_WARPS; step <<= 1) {
+    if ((warp & (2 * step - 1)) == 0) {
+      GqCand c = sh[warp + step][lane];
+      GqCand worst = gq_cand_shfl(mine, kth);
+      gq_list_feed(mine, c, c.valid && lane <= kth && gq_better(c, worst), lane, kth);   // entries behind the k-th of a sorted list cannot matter
+      sh[warp][lane] = mine;
+    }
+    __syncthreads();
   }
+  if (warp != 0) return;
   unsigned have = __ballot_sync(0xffffffffu, mine.valid != 0);
   int n = min(__popc(have), P.topk);
   if (lane < n) {

@@ -82,6 +82,26 @@ def test_direct_topk(ctx):
     run(plan, ctx, out_capacity=10)
 
 
+@pytest.mark.parametrize("k", [1, 10, 32])
+def test_topk_admission_bound_ties_and_both_merge_paths(ctx, k):
+    # top-k finaliser: (a) every group has the same ordering aggregate — the sampled admission bound equals that value,
+    # every warp list of pass 1 fills up and the merge takes its sorted-list path, the key order decides; (b) distinct
+    # values over a table far larger than the sample — few entries survive the bound, the merge ranks them by counting;
+    # (c) fewer groups than k
+    rng = np.random.default_rng(70 + k)
+    n = 400_000
+    keys = rng.permutation(1 << 21)[:n].astype(np.int64) - 5000
+    ones = np.ones(n, np.int64)
+    plan = dict(table=[keys, ones], preds=[], exprs=[[("col", 1)]], keys=[0], aggs=[("sum", 0), ("count",)],
+                max_groups=n, topk=k, topk_agg=0)
+    exp, got = run(plan, ctx, out_capacity=k)
+    assert np.array_equal(got["cols"][0], np.sort(keys)[:k])
+    vals = rng.integers(-10**12, 10**12, n).astype(np.int64)
+    vals[rng.integers(0, n, 50)] = vals.max()                      # ties at the top
+    run(dict(plan, table=[keys, vals]), ctx, out_capacity=k)
+    run(dict(plan, table=[keys[:5], vals[:5]], max_groups=8), ctx, out_capacity=k)
+
+
 def test_join_table_at_full_load_and_all_misses(ctx):
     rng = np.random.default_rng(8)
     nb = 50_000
