@@ -448,10 +448,10 @@ gq_status gq_codegen(const GqScanSpec& sp, GqKernelInfo* out, std::string* msg) 
   if (use_hot && sp.consumer == GQ_C_SCATTER) {
     long long st1 = 0;
     for (int c : g.cols) st1 += ((long long)nt * gq_dtype_bytes(sp.in_dtype[(size_t)c]) + 127) / 128 * 128;
-    const long long hb = 2048LL * (8 + 8 * nagg + 4) + 256 + 128 + (sp.part_states / std::max(1, sp.cluster)) * 4LL + 64;
+    const long long hb = 2048LL * (8 + 8 * nagg + 4) + 2048 / 4 + 256 + 128 + (sp.part_states / std::max(1, sp.cluster)) * 4LL + 64;
     if (GQ_SMEM_LIMIT - hb - 2 * 4 * 8 - 64 - 128 >= 3 * st1) hot_pos = 2048;
   }
-  if (use_hot) cons_bytes = hot_pos * 8LL + (long long)hot_pos * nagg * 8 + hot_pos * 4LL + 256;
+  if (use_hot) cons_bytes = hot_pos * 8LL + (long long)hot_pos * nagg * 8 + hot_pos * 4LL + hot_pos / 4 + 256;   // keys, accumulators, touched, bucket overflow flags
   long long part_state_off = 0;
   if (sp.part_rw > 0) {   // partition state words (+ the CTA's chunk counter)
     if (sp.part_states < 1 || sp.part_states > 16384) { if (msg) *msg = "bad partition count"; return GQ_ERR_INVALID_ARG; }

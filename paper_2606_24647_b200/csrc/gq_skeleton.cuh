@@ -717,6 +717,7 @@ struct GqCtx {
   i64* hot_keys;                        // HIGHCARD + GQ_HOT: shared set of this batch's hot keys [GQ_HOT_POS]
   u64* hot_acc;                         //   CTA-shared accumulators [GQ_HOT_POS][GQ_NAGG]
   int* hot_touched;                     //   entry received at least one row
+  unsigned char* hot_ovf;               //   bucket was full when a key that hashes to it was inserted [GQ_HOT_POS / 4]
   int nhot;
   int t;
 };
@@ -894,19 +895,25 @@ __device__ __forceinline__ void gq_lc_update(const int OP, GqCtx& cx, int grp, i
 __device__ __forceinline__ u32 gq_hot_bucket(i64 key) { return (u32)gq_hash(key, 64 - 16) & (GQ_HOT_POS / 4 - 1); }
 __device__ __forceinline__ void gq_hot_insert(GqCtx& cx, i64 key) {   // set-up only; keys are distinct
   u32 b = gq_hot_bucket(key);
-  for (int n = 0; n < GQ_HOT_POS / 4; ++n, b = (b + 1) & (GQ_HOT_POS / 4 - 1))
+  for (int n = 0; n < GQ_HOT_POS / 4; ++n, b = (b + 1) & (GQ_HOT_POS / 4 - 1)) {
     for (int q = 0; q < 4; ++q)
       if (atomicCAS((u64*)&cx.hot_keys[b * 4 + q], GQ_EMPTY, (u64)key) == GQ_EMPTY) return;
+    cx.hot_ovf[b] = 1;                                  // the key moves on: lookups that miss here must too
+  }
 }
+// A lookup reads one 32-byte bucket and its overflow flag and stops there unless a key was ever turned away from that
+// bucket. (Stopping at the first bucket with an EMPTY position instead cost four more 64-bit compares per row, and at
+// 75 % load most rows — the misses — walked on into a second bucket: a quarter of pass A's instructions on C5.)
 __device__ __forceinline__ int gq_hot_find(const GqCtx& cx, i64 key) {
   u32 b = gq_hot_bucket(key);
   for (int n = 0; n < GQ_HOT_POS / 4; ++n, b = (b + 1) & (GQ_HOT_POS / 4 - 1)) {
     const longlong2 k01 = *(const longlong2*)&cx.hot_keys[b * 4], k23 = *(const longlong2*)&cx.hot_keys[b * 4 + 2];
+    const unsigned char ovf = cx.hot_ovf[b];
     if (k01.x == key) return (int)(b * 4);
     if (k01.y == key) return (int)(b * 4 + 1);
     if (k23.x == key) return (int)(b * 4 + 2);
     if (k23.y == key) return (int)(b * 4 + 3);
-    if ((u64)k01.x == GQ_EMPTY || (u64)k01.y == GQ_EMPTY || (u64)k23.x == GQ_EMPTY || (u64)k23.y == GQ_EMPTY) return -1;
+    if (!ovf) return -1;
   }
   return -1;
 }

@@ -174,12 +174,14 @@ extern "C" __global__ void __launch_bounds__(GQ_NT + 32, 1) gq_scan(const __grid
   cx.hot_keys = (i64*)(gq_smem + GQ_CONS_OFF);
   cx.hot_acc = (u64*)(cx.hot_keys + GQ_HOT_POS);
   cx.hot_touched = (int*)(cx.hot_acc + GQ_HOT_POS * GQ_NAGG);
+  cx.hot_ovf = (unsigned char*)(cx.hot_touched + GQ_HOT_POS);
   cx.nhot = 0;
   if (P.hot) { const i64 n = P.hot[0]; cx.nhot = (int)(n < GQ_HOT_MAX ? n : GQ_HOT_MAX); }
   if (cx.nhot > 0) {
     for (int i = tid; i < GQ_HOT_POS; i += GQ_NT + 32) {
       cx.hot_keys[i] = (i64)GQ_EMPTY;
       cx.hot_touched[i] = 0;
+      if (i < GQ_HOT_POS / 4) cx.hot_ovf[i] = 0;
 #pragma unroll
       for (int a = 0; a < GQ_NAGG; ++a) cx.hot_acc[i * GQ_NAGG + a] = (u64)gq_identity(GQ_AGG_OP(a));
     }
