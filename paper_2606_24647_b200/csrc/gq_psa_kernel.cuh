@@ -109,22 +109,31 @@ __device__ __forceinline__ void gq_psa_row(u64* tab, u32* ctl, const u64 (&w)[GQ
     if (won || side_won) *(volatile u64*)(slot + 1) = w[1];
 #endif
 #endif
+    // two phases, so that the shared-memory round trips of the row's aggregates overlap: first every low-word add goes
+    // out and every MIN/MAX cell is read, then the carries and the compare-and-swap loops
+    u64 got[GQ_NAGG];
+#pragma unroll
+    for (int a = 0; a < GQ_NAGG; ++a) {
+      const int op = GQ_AGG_OP(a);
+      u64* cell = slot + 1 + GQ_NDEP + a;
+      if (op == GQ_OP_COUNT) got[a] = (u64)atomicAdd((u32*)cell, 1u);
+      else if (op == GQ_OP_SUM) got[a] = (u64)atomicAdd((u32*)cell, (u32)w[GQ_AGG_SRC(a)]);
+      else got[a] = *(volatile u64*)cell;
+    }
 #pragma unroll
     for (int a = 0; a < GQ_NAGG; ++a) {
       const int op = GQ_AGG_OP(a);
       u64* cell = slot + 1 + GQ_NDEP + a;
       if (op == GQ_OP_COUNT) {
-        const u32 old = atomicAdd((u32*)cell, 1u);
-        if (old == 0xFFFFFFFFu) atomicAdd((u32*)cell + 1, 1u);
+        if ((u32)got[a] == 0xFFFFFFFFu) atomicAdd((u32*)cell + 1, 1u);
       } else if (op == GQ_OP_SUM) {
         const u64 v = w[GQ_AGG_SRC(a)];
-        const u32 lo = (u32)v, hi = (u32)(v >> 32);
-        const u32 old = atomicAdd((u32*)cell, lo);
+        const u32 lo = (u32)v, hi = (u32)(v >> 32), old = (u32)got[a];
         const u32 up = hi + ((u32)(old + lo) < old ? 1u : 0u);   // the carry out of the low word belongs to THIS addition
         if (up) atomicAdd((u32*)cell + 1, up);
       } else {
         const i64 v = (i64)w[GQ_AGG_SRC(a)];
-        i64 cur = *(volatile i64*)cell;
+        i64 cur = (i64)got[a];
         while (op == GQ_OP_MIN ? v < cur : v > cur) {
           const i64 prev = (i64)atomicCAS(cell, (u64)cur, (u64)v);
           if (prev == cur) break;
