@@ -226,6 +226,17 @@ typedef struct { int32_t col; int32_t descending; } gq_sort_key;
 gq_status gq_order_by_workspace(int64_t nrows, size_t* bytes);
 gq_status gq_order_by(gq_ctx*, const gq_batch* in, const gq_sort_key* keys, int32_t nkeys, int64_t limit, void* d_workspace,
                       size_t bytes, int64_t* d_out_index, void* const* out_cols);
+/* Allocation-free variant of gq_order_by for callers that cannot call cudaMalloc (code under CUDA-graph capture, tight
+ * serving loops, harnesses that forbid it): same arguments, results and order, but the scratch lives in a file-scope
+ * device array inside libgq.so (4.2 MB, held by every GPU that loads the library until the process exits), so the call
+ * takes no workspace and makes no cudaMalloc / cudaFree / allocating library call. Limit: in->nrows <=
+ * gq_order_by_static_max_rows() (131072); more rows => GQ_ERR_UNSUPPORTED with a message, nothing is launched. All calls on
+ * one device share that array (it keeps the last call's contents; the call clears what it needs zeroed): calls that
+ * OVERLAP on the GPU - two streams or two contexts of one device - race; serialise them. Inputs and outputs stay the
+ * caller's. */
+int64_t gq_order_by_static_max_rows(void);
+gq_status gq_order_by_static(gq_ctx*, const gq_batch* in, const gq_sort_key* keys, int32_t nkeys, int64_t limit,
+                             int64_t* d_out_index, void* const* out_cols);
 
 /* ---- Fused pipeline: scan -> filter -> probe t1..tk -> project -> aggregate -> finalise ------- */
 typedef struct {

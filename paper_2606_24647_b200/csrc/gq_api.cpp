@@ -1405,6 +1405,30 @@ gq_status gq_order_by(gq_ctx* ctx, const gq_batch* in, const gq_sort_key* keys, 
   return GQ_OK;
 }
 
+// Allocation-free variant: workspace = a file-scope device array of gq_sort.cu (see there). No cudaMalloc / cudaFree, no
+// event creation (the launch group is not profiled), nothing but kernel launches, one memset and one 4-byte D2D copy.
+int64_t gq_order_by_static_max_rows(void) { return gq_sort_static_max_rows(); }
+gq_status gq_order_by_static(gq_ctx* ctx, const gq_batch* in, const gq_sort_key* keys, int32_t nkeys, int64_t limit,
+                             int64_t* d_out_index, void* const* out_cols) {
+  if (!ctx) return GQ_ERR_INVALID_ARG;
+  use_device(ctx);                                    // the scratch array's address is per device
+  gq_status st = check_batch(ctx, in);
+  if (st != GQ_OK) return st;
+  if (in->nrows > gq_sort_static_max_rows())
+    return fail(ctx, GQ_ERR_UNSUPPORTED, "gq_order_by_static: more than " + std::to_string(gq_sort_static_max_rows()) +
+                                             " rows (the static scratch limit); use gq_order_by with a caller workspace");
+  if (nkeys < 0 || nkeys > GQ_MAX_COLS || (nkeys > 0 && !keys)) return fail(ctx, GQ_ERR_INVALID_ARG, "bad sort keys");
+  for (int k = 0; k < nkeys; ++k)
+    if (keys[k].col < 0 || keys[k].col >= in->ncols) return fail(ctx, GQ_ERR_INVALID_ARG, "sort key column out of range");
+  if (!d_out_index && !out_cols) return fail(ctx, GQ_ERR_INVALID_ARG, "no outputs");
+  if (in->nrows == 0) return GQ_OK;
+  int nl = 0;
+  cudaError_t e = gq_launch_order_by_static(ctx->stream, ctx->num_sms, in, keys, nkeys, limit, (long long*)d_out_index, out_cols, &nl);
+  if (e != cudaSuccess) return cuda_fail(ctx, e, "order by (static scratch)");
+  ctx->launches += nl;
+  return GQ_OK;
+}
+
 gq_status gq_profile(gq_ctx* ctx, int32_t enable) {
   if (!ctx) return GQ_ERR_INVALID_ARG;
   ctx->prof = enable != 0;

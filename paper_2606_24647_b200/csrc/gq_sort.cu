@@ -282,3 +282,58 @@ cudaError_t gq_launch_order_by(cudaStream_t s, int num_sms, const gq_batch* in, 
   *nlaunches = nl;
   return cudaGetLastError();
 }
+
+// ------------------------------------------------------------------------------------- allocation-free entry point
+// gq_order_by_static (include/gq.h): the same launch sequence as gq_order_by, with its workspace in a file-scope device
+// array instead of caller memory — for callers that cannot allocate (code under CUDA-graph capture, serving loops,
+// harnesses that forbid cudaMalloc). The array is sized for GQ_ORDER_BY_STATIC_MAX_ROWS rows (the layout of
+// gq_sort_layout: 2 x 8 B + 2 x 4 B per row, 1 MiB of digit histograms, two select histograms, control words: 4.2 MB)
+// and every GPU that loads libgq.so holds it until the process exits.
+//   * In HOST code the array's name is a host-side stand-in, not a device address: the device address is taken once per
+//     device with cudaGetSymbolAddress, with that device current, and it is that pointer the kernels receive.
+//   * All calls share the array and it keeps the previous call's contents. Nothing in it has to start at zero except
+//     the select histograms and control words of the TopN path, which gq_launch_order_by clears itself (stream-ordered
+//     cudaMemsetAsync) before it uses them; every other region is written before it is read.
+//   * Two calls that overlap on the GPU (different streams / contexts of one device) RACE on the array: callers
+//     serialise them (one stream, or an event between them).
+#define GQ_SORT_AL256(v) ((((size_t)(v)) + 255) / 256 * 256)
+#define GQ_SORT_STATIC_BYTES                                                                                        \
+  (2 * GQ_SORT_AL256((size_t)GQ_ORDER_BY_STATIC_MAX_ROWS * 8) + 2 * GQ_SORT_AL256((size_t)GQ_ORDER_BY_STATIC_MAX_ROWS * 4) + \
+   GQ_SORT_AL256((size_t)256 * 1024 * 4) + 2 * GQ_SORT_AL256(GQ_SEL_BINS * 4) + 256)
+static __device__ __align__(256) unsigned char gq_sort_static_scratch[GQ_SORT_STATIC_BYTES];
+
+#include <mutex>
+#define GQ_SORT_STATIC_MAX_DEVICES 64
+static std::mutex g_sort_static_mu;
+static char* g_sort_static_ptr[GQ_SORT_STATIC_MAX_DEVICES];   // device address of the array, per device ordinal (null = not asked yet)
+
+// Set-up, once per device: the CURRENT device's address of the scratch array.
+static cudaError_t gq_sort_static_address(char** out) {
+  int dev = -1;
+  cudaError_t e = cudaGetDevice(&dev);
+  if (e != cudaSuccess) return e;
+  if (dev < 0 || dev >= GQ_SORT_STATIC_MAX_DEVICES) return cudaErrorInvalidDevice;
+  std::lock_guard<std::mutex> lock(g_sort_static_mu);
+  if (!g_sort_static_ptr[dev]) {
+    void* p = nullptr;
+    e = cudaGetSymbolAddress(&p, gq_sort_static_scratch);
+    if (e != cudaSuccess) return e;
+    if (!p || ((size_t)p & 255) != 0) return cudaErrorInvalidSymbol;
+    g_sort_static_ptr[dev] = (char*)p;
+  }
+  *out = g_sort_static_ptr[dev];
+  return cudaSuccess;
+}
+
+long long gq_sort_static_max_rows() { return GQ_ORDER_BY_STATIC_MAX_ROWS; }
+
+// The caller (gq_api.cpp) has made the context's device current and checked in->nrows <= GQ_ORDER_BY_STATIC_MAX_ROWS.
+cudaError_t gq_launch_order_by_static(cudaStream_t s, int num_sms, const gq_batch* in, const gq_sort_key* keys, int nkeys, i64 limit,
+                                      i64* out_index, void* const* out_cols, int* nlaunches) {
+  if (in->nrows > GQ_ORDER_BY_STATIC_MAX_ROWS || gq_sort_layout(in->nrows, GQ_MAX_SMS).total > (size_t)GQ_SORT_STATIC_BYTES)
+    return cudaErrorInvalidValue;
+  char* ws = nullptr;
+  cudaError_t e = gq_sort_static_address(&ws);
+  if (e != cudaSuccess) return e;
+  return gq_launch_order_by(s, num_sms, in, keys, nkeys, limit, ws, out_index, out_cols, nlaunches);
+}

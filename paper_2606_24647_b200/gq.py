@@ -41,7 +41,7 @@ SYMBOLS = ["gq_create", "gq_destroy", "gq_sync", "gq_clear_error", "gq_status_st
            "gq_aggstate_destroy", "gq_pipeline_workspace", "gq_pipeline", "gq_pipeline_host_workspace",
            "gq_pipeline_host", "gq_set_kernel_cache_dir", "gq_precompile_pipeline", "gq_precompile_build", "gq_precompile_materialise",
            "gq_table_describe", "gq_read_probe", "gq_set_option", "gq_hash_build_workspace_dense", "gq_profile", "gq_profile_read", "gq_order_by_workspace", "gq_order_by", "gq_aggstate_merge", "gq_aggstate_count",
-           "gq_aggstate_rehash"]
+           "gq_aggstate_rehash", "gq_order_by_static", "gq_order_by_static_max_rows"]
 
 
 class GqError(RuntimeError):
@@ -161,6 +161,10 @@ def lib():
         L.gq_order_by_workspace.argtypes = [C.c_int64, C.POINTER(C.c_size_t)]
         L.gq_order_by.argtypes = [C.c_void_p, C.POINTER(_Batch), C.POINTER(_SortKey), C.c_int32, C.c_int64, C.c_void_p, C.c_size_t,
                                   C.c_void_p, C.POINTER(C.c_void_p)]
+        L.gq_order_by_static.argtypes = [C.c_void_p, C.POINTER(_Batch), C.POINTER(_SortKey), C.c_int32, C.c_int64,
+                                         C.c_void_p, C.POINTER(C.c_void_p)]
+        L.gq_order_by_static_max_rows.argtypes = []
+        L.gq_order_by_static_max_rows.restype = C.c_int64
         L.gq_profile.argtypes = [C.c_void_p, C.c_int32]
         L.gq_profile_read.argtypes = [C.c_void_p, C.c_char_p, C.c_size_t, C.POINTER(C.c_float), C.c_int32]
         L.gq_profile_read.restype = C.c_int32
@@ -433,6 +437,32 @@ class Context:
                                            index.data_ptr(), m.ptrs(outs) if gather else None))
             self._last_ws = ws
         return index[:nout], ([o[:nout] for o in outs] if gather else None)
+
+    def order_by_static(self, cols, keys, limit, out_index, out_cols=None):
+        """gq_order_by_static: order_by that allocates nothing — scratch is a fixed device array inside libgq.so, the
+        caller passes the outputs (out_index int64[>= n_out] and/or out_cols, one tensor per input column). At most
+        order_by_static_max_rows() rows; calls on one device must not overlap on the GPU. -> n_out."""
+        with torch.cuda.stream(self.stream):
+            m = _M()
+            b = m.batch(cols)
+            n = int(b.nrows)
+            nout = n if limit <= 0 or limit > n else int(limit)
+            kk = (_SortKey * max(1, len(keys)))()
+            for i, (c, d) in enumerate(keys):
+                kk[i] = _SortKey(int(c), 1 if d else 0)
+            m.keep.append(kk)
+            if out_index is not None and (out_index.dtype != torch.int64 or out_index.numel() < nout):
+                raise ValueError("out_index must be int64 with at least n_out elements")
+            if out_cols is not None and (len(out_cols) != len(cols) or any(o.dtype != c.dtype or o.numel() < nout for o, c in zip(out_cols, cols))):
+                raise ValueError("out_cols must match the input columns' dtypes and hold n_out rows")
+            self._check(self.L.gq_order_by_static(self.h, C.byref(b), kk, len(keys), int(limit),
+                                                  out_index.data_ptr() if out_index is not None else None,
+                                                  m.ptrs(list(out_cols)) if out_cols is not None else None))
+        return nout
+
+    @staticmethod
+    def order_by_static_max_rows() -> int:
+        return int(lib().gq_order_by_static_max_rows())
 
     def profile(self, enable=True):
         """gq_profile: bracket every kernel launch of this context with CUDA events (off in timed loops)."""

@@ -1,0 +1,114 @@
+"""gq_order_by_static (-m gpu): the allocation-free OrderBy / TopN entry point (scratch = a file-scope device array inside
+libgq.so) against the existing gq_order_by path, bit-exactly (row numbers and gathered columns are integer work), on calls
+made back to back so that every call after the first finds the previous call's contents in the shared scratch.
+Collected last on purpose (file name): the run uses pytest -x."""
+import numpy as np
+import pytest
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def ctx():
+    from paper_2606_24647_b200 import build as gqbuild
+    gqbuild.build()
+    from paper_2606_24647_b200 import gq
+    return gq.Context()
+
+
+def _cols(n, seed):
+    rng = np.random.default_rng(seed)
+    a = rng.integers(-3, 3, n).astype(np.int8)                      # heavy ties: stability decides
+    b = rng.integers(-1000, 1000, n).astype(np.int32)
+    c = rng.integers(-2**62, 2**62, n).astype(np.int64)
+    c[::5] = c[0]
+    return [a, b, c]
+
+
+# (rows, seed, keys, limit): a full multi-key sort, the TopN path (>= 2^16 rows, limit * 8 < rows) at the row limit, a
+# small input after the large ones (stale scratch beyond its own extent), the TopN path again, no keys at all
+CASES = [
+    (100_000, 1, [(0, True), (1, False), (2, True)], 0),
+    (131_072, 2, [(2, False), (1, True)], 100),
+    (1_000, 3, [(1, False), (0, True)], 0),
+    (70_001, 4, [(0, False)], 7),
+    (2_049, 5, [], 0),
+]
+
+
+def _run_static(ctx, torch, dcols, keys, limit, index, outs):
+    index.fill_(-1)
+    nout = ctx.order_by_static(dcols, keys, limit, index, outs)
+    return nout
+
+
+def test_static_scratch_order_by_equals_existing_path_on_consecutive_calls(ctx):
+    import torch
+    import gqrun
+    import oracle
+    assert ctx.order_by_static_max_rows() == 131_072
+    # inputs, outputs and the existing path's results first: nothing is allocated between the static calls below
+    prepared = []
+    for n, seed, keys, limit in CASES:
+        cols = _cols(n, seed)
+        dcols = gqrun.dev(cols)
+        ref_index, ref_outs = ctx.order_by(dcols, keys, limit=limit, gather=True)
+        ctx.sync()
+        nout = ref_index.numel()
+        index = torch.empty(nout, dtype=torch.int64, device="cuda")
+        outs = [torch.empty(nout, dtype=c.dtype, device="cuda") for c in dcols]
+        prepared.append((cols, dcols, keys, limit, ref_index.clone(), [o.clone() for o in ref_outs], index, outs))
+    # the existing path is itself pinned to the oracle (tests/test_gpu_orderby.py); one case here as well
+    cols, _, keys, limit, ref_index, _, _, _ = prepared[0]
+    assert np.array_equal(ref_index.cpu().numpy(), oracle.order_by(cols, keys, limit).cols[0])
+
+    # warm-up pass (first use of the symbol address and of every kernel of both paths), then two measured passes back
+    # to back: device memory in use must not move, results must equal the existing path's every time
+    for cols, dcols, keys, limit, ref_index, ref_outs, index, outs in prepared:
+        _run_static(ctx, torch, dcols, keys, limit, index, outs)
+    ctx.sync()
+    torch.cuda.synchronize()
+    free0, _ = torch.cuda.mem_get_info()
+    alloc0 = torch.cuda.memory_allocated()
+    for rep in range(2):
+        for cols, dcols, keys, limit, ref_index, ref_outs, index, outs in prepared:
+            nout = _run_static(ctx, torch, dcols, keys, limit, index, outs)
+            ctx.sync()
+            assert nout == ref_index.numel()
+            assert torch.equal(index, ref_index), f"row order differs (rows {len(cols[0])}, keys {keys}, limit {limit}, pass {rep})"
+            for j, (o, r) in enumerate(zip(outs, ref_outs)):
+                assert torch.equal(o, r), f"gathered column {j} differs (rows {len(cols[0])}, pass {rep})"
+    torch.cuda.synchronize()
+    assert torch.cuda.memory_allocated() == alloc0
+    assert torch.cuda.mem_get_info()[0] == free0, "device memory in use changed across gq_order_by_static calls"
+
+    # index only / gathered columns only
+    cols, dcols, keys, limit, ref_index, ref_outs, index, outs = prepared[1]
+    _run_static(ctx, torch, dcols, keys, limit, index, None)
+    ctx.sync()
+    assert torch.equal(index, ref_index)
+    for o in outs:
+        o.zero_()
+    ctx.order_by_static(dcols, keys, limit, None, outs)
+    ctx.sync()
+    for o, r in zip(outs, ref_outs):
+        assert torch.equal(o, r)
+
+
+def test_static_scratch_order_by_rejects_more_rows_than_its_scratch_holds(ctx):
+    import torch
+    from paper_2606_24647_b200 import gq
+    n = ctx.order_by_static_max_rows() + 1
+    col = torch.arange(n, dtype=torch.int64, device="cuda")
+    index = torch.full((n,), -7, dtype=torch.int64, device="cuda")
+    l0 = ctx.launch_count()
+    with pytest.raises(gq.GqError) as ei:
+        ctx.order_by_static([col], [(0, True)], 0, index, None)
+    assert "GQ_ERR_UNSUPPORTED" in str(ei.value) and "131072" in str(ei.value)
+    ctx.sync()                                           # not a sticky device error: the context stays usable
+    assert ctx.launch_count() == l0 and int(index[0]) == -7 and int(index[-1]) == -7
+    small = torch.tensor([5, -2, 9, -2], dtype=torch.int64, device="cuda")
+    out = torch.empty(4, dtype=torch.int64, device="cuda")
+    ctx.order_by_static([small], [(0, False)], 0, out, None)
+    ctx.sync()
+    assert out.cpu().tolist() == [1, 3, 0, 2]
