@@ -96,6 +96,8 @@ def lib():
             f.restype = C.c_void_p
             f.argtypes = [C.POINTER(_Table), C.POINTER(_Pred), C.c_int32, C.c_int32,
                           C.POINTER(_Table), C.POINTER(_Pred), C.c_int32, C.c_int32]
+        L.ocl_hash_partition.restype = C.c_void_p
+        L.ocl_hash_partition.argtypes = [C.POINTER(_Table), C.POINTER(C.c_int32), C.c_int32, C.c_int32]
         L.ocl_order_by.restype = C.c_void_p
         L.ocl_order_by.argtypes = [C.POINTER(_Table), C.POINTER(_SortKey), C.c_int32, C.c_int64]
         L.ocl_result_nrows.restype = C.c_int64
@@ -229,6 +231,15 @@ def order_by(table, keys, limit=0) -> Result:
     for i, (c, d) in enumerate(keys):
         kk[i] = _SortKey(int(c), 1 if d else 0)
     return Result(lib().ocl_order_by(C.byref(t), kk, len(keys), int(limit)))
+
+
+def hash_partition(table, key_cols, nparts) -> Result:
+    """-> Result with cols[0] = destination of every output row, cols[1] = input row number, then the columns; rows are
+    destination-major, input order inside a destination."""
+    keep = _Keep()
+    t = _table(table, keep)
+    kk = (C.c_int32 * max(1, len(key_cols)))(*[int(c) for c in key_cols])
+    return Result(lib().ocl_hash_partition(C.byref(t), kk, len(key_cols), int(nparts)))
 
 
 def avg(s: int, c: int) -> float:

@@ -313,6 +313,42 @@ ocl_result* ocl_order_by(const ocl_table* in, const ocl_sort_key* keys, int32_t 
   return res;
 }
 
+// Hash partitioning (PAPER.md:160, :174 CudfPartitionedOutput; DESIGN reading R-HP): the definition
+// written out. destination(row) follows include/gq.h: h := 0x9E3779B97F4A7C15; for every key column, in order,
+// h := fmix64(h XOR value) with the 64-bit finaliser of MurmurHash3 (x ^= x >> 33; x *= 0xff51afd7ed558ccd; x ^= x >> 33;
+// x *= 0xc4ceb9fe1a85ec53; x ^= x >> 33); destination = floor((h div 2^32) * nparts / 2^32). Rows are emitted destination
+// by destination, input order inside one destination.
+ocl_result* ocl_hash_partition(const ocl_table* in, const int32_t* key_cols, int32_t nkeys, int32_t nparts) {
+  if (!in || nkeys < 1 || !key_cols || nparts < 1) return nullptr;
+  for (int32_t k = 0; k < nkeys; ++k) if (key_cols[k] < 0 || key_cols[k] >= in->ncols) return nullptr;
+  std::vector<int64_t> dest((size_t)in->nrows);
+  for (int64_t r = 0; r < in->nrows; ++r) {
+    uint64_t h = 0x9E3779B97F4A7C15ULL;
+    for (int32_t k = 0; k < nkeys; ++k) {
+      uint64_t x = h ^ (uint64_t)cell(in->cols[key_cols[k]], r);
+      x ^= x >> 33;
+      x *= 0xff51afd7ed558ccdULL;
+      x ^= x >> 33;
+      x *= 0xc4ceb9fe1a85ec53ULL;
+      x ^= x >> 33;
+      h = x;
+    }
+    dest[(size_t)r] = (int64_t)(((h >> 32) * (uint64_t)nparts) >> 32);
+  }
+  ocl_result* res = new ocl_result();
+  res->nrows = in->nrows;
+  res->input_rows = in->nrows;
+  res->cols.assign((size_t)in->ncols + 2, std::vector<int64_t>());
+  for (int64_t d = 0; d < nparts; ++d)
+    for (int64_t r = 0; r < in->nrows; ++r)
+      if (dest[(size_t)r] == d) {
+        res->cols[0].push_back(d);
+        res->cols[1].push_back(r);
+        for (int32_t c = 0; c < in->ncols; ++c) res->cols[(size_t)c + 2].push_back(cell(in->cols[c], r));
+      }
+  return res;
+}
+
 int64_t ocl_result_nrows(const ocl_result* r) { return r->nrows; }
 int32_t ocl_result_ncols(const ocl_result* r) { return (int32_t)r->cols.size(); }
 const int64_t* ocl_result_col(const ocl_result* r, int32_t c) { return r->cols[(size_t)c].data(); }

@@ -64,6 +64,12 @@ ocl_result* ocl_join_pairs_bruteforce(const ocl_table* build, const ocl_pred* bp
 typedef struct { int32_t col; int32_t descending; } ocl_sort_key;
 ocl_result* ocl_order_by(const ocl_table* in, const ocl_sort_key* keys, int32_t nkeys, int64_t limit);
 
+/* Hash partitioning of a batch to nparts destinations (PAPER.md:160, :174 CudfPartitionedOutput):
+ * destination(row) = the function include/gq.h defines over the key columns (restated in oracle.cpp, not shared);
+ * rows are emitted destination by destination, in input order inside a destination. Result: column 0 = destination of
+ * every output row, column 1 = its input row number, then every input column (widened to int64). */
+ocl_result* ocl_hash_partition(const ocl_table* in, const int32_t* key_cols, int32_t nkeys, int32_t nparts);
+
 int64_t ocl_result_nrows(const ocl_result*);              /* groups / output rows / pairs */
 int32_t ocl_result_ncols(const ocl_result*);              /* keys then aggregates (query); exprs; 2 (pairs) */
 const int64_t* ocl_result_col(const ocl_result*, int32_t c);

@@ -325,3 +325,81 @@ def test_order_by_equals_numpy_lexsort():
     assert np.array_equal(np.sort(r.cols[0]), np.arange(n))
     kb, kc = r.cols[2], r.cols[3]
     assert np.all((kb[:-1] < kb[1:]) | ((kb[:-1] == kb[1:]) & (kc[:-1] >= kc[1:])))
+
+
+# ------------------------------------------------------------------ hash partitioning
+def test_hash_partition_murmur3_finaliser_vectors():
+    # the published MurmurHash3 fmix64 vectors fmix64(0) = 0 and fmix64(1) = 0xB456BCFC34C2CB2C, reached through the seed:
+    # a single key k gives h = fmix64(0x9E3779B97F4A7C15 xor k). nparts = 2^16 exposes the top 16 bits of h.
+    seed = 0x9E3779B97F4A7C15
+    k0 = np.array([seed], dtype=np.uint64).view(np.int64)                 # h = fmix64(0) = 0
+    k1 = np.array([seed ^ 1], dtype=np.uint64).view(np.int64)             # h = fmix64(1)
+    assert list(oracle.hash_partition([k0], [0], 1 << 16).cols[0]) == [0]
+    assert list(oracle.hash_partition([k0], [0], 7).cols[0]) == [0]
+    assert list(oracle.hash_partition([k1], [0], 1 << 16).cols[0]) == [0xB456]
+    assert list(oracle.hash_partition([k1], [0], 256).cols[0]) == [0xB4]
+    assert list(oracle.hash_partition([k1], [0], 3).cols[0]) == [(0xB456BCFC * 3) >> 32]   # floor(h_hi * nparts / 2^32)
+
+
+def test_hash_partition_invariants():
+    rng = np.random.default_rng(91)
+    n = 30_000
+    a = rng.integers(-100, 100, n).astype(np.int8)
+    b = rng.integers(-5000, 5000, n).astype(np.int32)
+    c = rng.integers(-2**62, 2**62, n).astype(np.int64)
+    cols = [a, b, c]
+    for keys, nparts in (([1], 8), ([0, 1], 7), ([2], 256), ([1, 2, 0], 3)):
+        r = oracle.hash_partition(cols, keys, nparts)
+        dest, row = r.cols[0], r.cols[1]
+        assert r.nrows == n and np.array_equal(np.sort(row), np.arange(n))                 # a permutation of the rows
+        for j in range(3):
+            assert np.array_equal(r.cols[2 + j], cols[j][row].astype(np.int64))            # whole rows move together
+        assert dest.min() >= 0 and dest.max() < nparts and np.all(dest[1:] >= dest[:-1])   # destination-major
+        same = dest[1:] == dest[:-1]
+        assert np.all(row[1:][same] > row[:-1][same])                                      # input order inside one
+        # the destination is a function of the key tuple alone: not of the other columns, not of the row's position
+        dest_of_row = np.empty(n, np.int64); dest_of_row[row] = dest
+        perm = rng.permutation(n)
+        other = [rng.integers(-9, 9, n).astype(x.dtype) if j not in keys else x for j, x in enumerate(cols)]
+        r2 = oracle.hash_partition([x[perm] for x in other], keys, nparts)
+        d2 = np.empty(n, np.int64); d2[r2.cols[1]] = r2.cols[0]
+        assert np.array_equal(d2, dest_of_row[perm])
+        seen = {}
+        for kt, d in zip(zip(*[cols[k].tolist() for k in keys]), dest_of_row.tolist()):
+            assert seen.setdefault(kt, d) == d                                             # equal keys, equal destination
+    # one destination: the input, in order; empty input: empty output
+    r = oracle.hash_partition(cols, [2], 1)
+    assert np.array_equal(r.cols[1], np.arange(n)) and not r.cols[0].any()
+    assert oracle.hash_partition([c[:0]], [0], 4).nrows == 0
+    # floor(h_hi * nparts / 2^32): halving a power-of-two partition count merges neighbouring destinations
+    d16 = np.empty(n, np.int64); r16 = oracle.hash_partition(cols, [2], 16); d16[r16.cols[1]] = r16.cols[0]
+    d8 = np.empty(n, np.int64); r8 = oracle.hash_partition(cols, [2], 8); d8[r8.cols[1]] = r8.cols[0]
+    assert np.array_equal(d16 >> 1, d8)
+
+
+def test_hash_partition_balance_and_bigint_restatement():
+    # consecutive integers (the worst input for a weak mix) spread evenly: chi-square of the destination sizes against
+    # the uniform law, 7 degrees of freedom / 6: far below 40 (p < 1e-6) for a good mix, in the thousands for a bad one
+    n = 400_000
+    k = np.arange(n, dtype=np.int64) - 1000
+    for nparts in (8, 7):
+        sizes = np.bincount(oracle.hash_partition([k], [0], nparts).cols[0], minlength=nparts)
+        chi2 = float(((sizes - n / nparts) ** 2 / (n / nparts)).sum())
+        assert chi2 < 40.0, (nparts, sizes)
+    # Python integers (no wrap-around, masked by hand) against the C arithmetic: negative keys sign-extended from narrow
+    # types, several keys chained
+    M = (1 << 64) - 1
+    def fmix(x):
+        x ^= x >> 33; x = (x * 0xff51afd7ed558ccd) & M; x ^= x >> 33; x = (x * 0xc4ceb9fe1a85ec53) & M; x ^= x >> 33
+        return x
+    a = np.array([-128, -1, 0, 1, 127, -77], np.int8)
+    b = np.array([-2**31, -1, 0, 5, 2**31 - 1, 123456], np.int32)
+    c = np.array([-2**63, -1, 0, 2**63 - 1, 42, -42], np.int64)
+    for keys, nparts in (([0], 5), ([1], 256), ([2], 1000), ([0, 1, 2], 13), ([2, 0], 64)):
+        r = oracle.hash_partition([a, b, c], keys, nparts)
+        got = np.empty(6, np.int64); got[r.cols[1]] = r.cols[0]
+        for i in range(6):
+            h = 0x9E3779B97F4A7C15
+            for kc in keys:
+                h = fmix(h ^ (int([a, b, c][kc][i]) & M))
+            assert got[i] == ((h >> 32) * nparts) >> 32
