@@ -226,6 +226,24 @@ typedef struct { int32_t col; int32_t descending; } gq_sort_key;
 gq_status gq_order_by_workspace(int64_t nrows, size_t* bytes);
 gq_status gq_order_by(gq_ctx*, const gq_batch* in, const gq_sort_key* keys, int32_t nkeys, int64_t limit, void* d_workspace,
                       size_t bytes, int64_t* d_out_index, void* const* out_cols);
+/* ---- Hash partitioning: the GPU side of PartitionedOutput ---------------
+ * Groups the rows of a batch by DESTINATION so that every destination's rows form one contiguous, packed range of the
+ * output columns ("cudf columns gathered into contiguous memory"), ready for an exchange: rows of
+ * destination d are out rows [d_out_offsets[d], d_out_offsets[d + 1]); inside a destination rows keep their input order
+ * (the result is unique). Whole rows move: every input column is written, with its dtype, to out_cols[c] (nrows
+ * elements, 16-byte aligned, the caller's). d_out_row (optional, int64[nrows]) receives the input row number of every
+ * output row; d_out_offsets is int64[nparts + 1]. The destination of a row depends on its key columns only:
+ *     h = 0x9E3779B97F4A7C15;  for k in key_cols (in order): h = fmix64(h ^ (uint64)(int64)value_k);
+ *     destination = ((h >> 32) * nparts) >> 32                       (fmix64 = MurmurHash3's 64-bit finaliser:
+ *     x ^= x >> 33; x *= 0xff51afd7ed558ccd; x ^= x >> 33; x *= 0xc4ceb9fe1a85ec53; x ^= x >> 33)
+ * so that every sender maps equal keys to the same destination. 1 <= nparts <= GQ_MAX_PARTITIONS, 1..8 key columns,
+ * nrows <= 2^31. Stream-ordered, no host synchronisation; three launches (histogram, scan, scatter). */
+enum { GQ_MAX_PARTITIONS = 256 };
+gq_status gq_hash_partition_workspace(int32_t nparts, size_t* bytes);
+gq_status gq_hash_partition(gq_ctx*, const gq_batch* in, const int32_t* key_cols, int32_t nkeys, int32_t nparts,
+                            void* d_workspace, size_t bytes, void* const* out_cols, int64_t* d_out_row,
+                            int64_t* d_out_offsets);
+
 /* Allocation-free variant of gq_order_by for callers that cannot call cudaMalloc (code under CUDA-graph capture, tight
  * serving loops, harnesses that forbid it): same arguments, results and order, but the scratch lives in a file-scope
  * device array inside libgq.so (4.2 MB, held by every GPU that loads the library until the process exits), so the call

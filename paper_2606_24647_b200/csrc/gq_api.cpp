@@ -1405,6 +1405,40 @@ gq_status gq_order_by(gq_ctx* ctx, const gq_batch* in, const gq_sort_key* keys, 
   return GQ_OK;
 }
 
+// ------------------------------------------------------------------------------------------------ hash partitioning
+gq_status gq_hash_partition_workspace(int32_t nparts, size_t* bytes) {
+  if (!bytes || nparts < 1 || nparts > GQ_MAX_PARTITIONS) return GQ_ERR_INVALID_ARG;
+  *bytes = gq_hash_partition_workspace_bytes(nparts);
+  return GQ_OK;
+}
+gq_status gq_hash_partition(gq_ctx* ctx, const gq_batch* in, const int32_t* key_cols, int32_t nkeys, int32_t nparts, void* d_ws,
+                            size_t bytes, void* const* out_cols, int64_t* d_out_row, int64_t* d_out_offsets) {
+  if (!ctx) return GQ_ERR_INVALID_ARG;
+  gq_status st = check_batch(ctx, in);
+  if (st != GQ_OK) return st;
+  if (in->nrows > (1LL << 31)) return fail(ctx, GQ_ERR_UNSUPPORTED, "gq_hash_partition: more than 2^31 rows");
+  if (nparts < 1) return fail(ctx, GQ_ERR_INVALID_ARG, "gq_hash_partition: nparts < 1");
+  if (nparts > GQ_MAX_PARTITIONS) return fail(ctx, GQ_ERR_UNSUPPORTED, "gq_hash_partition: more than GQ_MAX_PARTITIONS destinations");
+  if (nkeys < 1 || nkeys > GQ_MAX_KEYS_HP || !key_cols) return fail(ctx, GQ_ERR_INVALID_ARG, "gq_hash_partition: 1..8 key columns");
+  for (int k = 0; k < nkeys; ++k)
+    if (key_cols[k] < 0 || key_cols[k] >= in->ncols) return fail(ctx, GQ_ERR_INVALID_ARG, "partition key column out of range");
+  if (!out_cols || !d_out_offsets || !aligned(d_out_offsets, 8)) return fail(ctx, GQ_ERR_INVALID_ARG, "gq_hash_partition: missing outputs");
+  for (int c = 0; c < in->ncols; ++c)
+    if (in->nrows > 0 && (!out_cols[c] || !aligned(out_cols[c], 16))) return fail(ctx, GQ_ERR_INVALID_ARG, "output column null or not 16-byte aligned");
+  if (!d_ws || !aligned(d_ws, 256)) return fail(ctx, GQ_ERR_INVALID_ARG, "bad workspace");
+  if (bytes < gq_hash_partition_workspace_bytes(nparts)) return fail(ctx, GQ_ERR_WORKSPACE_TOO_SMALL, "hash-partition workspace too small");
+  if (in->nrows == 0) {
+    cudaError_t e0 = cudaMemsetAsync(d_out_offsets, 0, (size_t)(nparts + 1) * 8, ctx->stream);
+    return e0 == cudaSuccess ? GQ_OK : cuda_fail(ctx, e0, "hash partition");
+  }
+  int nl = 0;
+  cudaError_t e = PROF(ctx, "gq_hash_partition", gq_launch_hash_partition(ctx->stream, ctx->num_sms, in, key_cols, nkeys, nparts, (char*)d_ws,
+                                                                           out_cols, (long long*)d_out_row, (long long*)d_out_offsets, &nl));
+  if (e != cudaSuccess) return cuda_fail(ctx, e, "hash partition");
+  ctx->launches += nl;
+  return GQ_OK;
+}
+
 // Allocation-free variant: workspace = a file-scope device array of gq_sort.cu (see there). No cudaMalloc / cudaFree, no
 // event creation (the launch group is not profiled), nothing but kernel launches, one memset and one 4-byte D2D copy.
 int64_t gq_order_by_static_max_rows(void) { return gq_sort_static_max_rows(); }

@@ -241,6 +241,10 @@ size_t gq_topk_scratch_bytes_impl();
 size_t gq_sort_workspace_bytes(long long nrows);
 cudaError_t gq_launch_order_by(cudaStream_t s, int num_sms, const gq_batch* in, const gq_sort_key* keys, int nkeys, long long limit,
                                char* ws, long long* out_index, void* const* out_cols, int* nlaunches);
+#define GQ_MAX_KEYS_HP 8                        // key columns of gq_hash_partition
+size_t gq_hash_partition_workspace_bytes(int nparts);
+cudaError_t gq_launch_hash_partition(cudaStream_t s, int num_sms, const gq_batch* in, const int* key_cols, int nkeys, int nparts, char* ws,
+                                     void* const* out_cols, long long* out_row, long long* out_offsets, int* nlaunches);
 #define GQ_ORDER_BY_STATIC_MAX_ROWS (1 << 17)   // rows gq_order_by_static takes (its scratch is a 4.2 MB file-scope device array)
 long long gq_sort_static_max_rows();
 cudaError_t gq_launch_order_by_static(cudaStream_t s, int num_sms, const gq_batch* in, const gq_sort_key* keys, int nkeys, long long limit,

@@ -337,3 +337,196 @@ cudaError_t gq_launch_order_by_static(cudaStream_t s, int num_sms, const gq_batc
   if (e != cudaSuccess) return e;
   return gq_launch_order_by(s, num_sms, in, keys, nkeys, limit, ws, out_index, out_cols, nlaunches);
 }
+
+// ------------------------------------------------------------------------------------- hash partitioning (gq_hash_partition)
+// CudfPartitionedOutput: the rows of a batch are grouped by destination =
+// gq_hp_dest(key columns) (the function include/gq.h defines), destination-major, input order inside a destination —
+// one contiguous packed range per destination, ready to be sent. A stable counting sort with ONE read of the key columns
+// (histogram), one read of every column and one write (scatter): (keys + 2 x row bytes) per row, HBM-bound.
+//   histogram — every CTA owns a contiguous range of 2048-row tiles and counts its rows per destination (shared-memory
+//               counters, one add per distinct destination and 32 rows through MATCH.ANY);
+//   scan      — gq_k_sort_scan over [destination][CTA]: exclusive offsets, destination-major, stable across CTAs;
+//   scatter   — every CTA walks its range again, tile by tile. Inside a tile warp w owns rows [256 w, 256 w + 256): it
+//               ranks them per destination on its own (MATCH.ANY + warp-private counters, no CTA barrier), one pass over
+//               [warp][destination] turns the counters into offsets, and every row knows its place in the tile's
+//               destination-major order. Then, column by column, the tile is permuted THROUGH SHARED MEMORY: values go to
+//               their place in a staging buffer, and the buffer is written out in order, so that the rows of one
+//               destination leave as one contiguous run (2048 / nparts rows on average) instead of row by row — a warp
+//               writing single 4-byte values into 64 open streams reached 0.5 TB/s, a sixth of this.
+#define GQ_HP_THREADS 256
+#define GQ_HP_WARPS (GQ_HP_THREADS / 32)
+#define GQ_HP_ITEMS 8                              // rows per thread and tile
+#define GQ_HP_TILE (GQ_HP_THREADS * GQ_HP_ITEMS)
+struct GqHpParams {
+  u32 n; int nparts; int nkeys; int ncols;
+  const void* key[GQ_MAX_KEYS_HP]; int key_dtype[GQ_MAX_KEYS_HP];
+  const void* col[GQ_MAX_COLS]; void* out[GQ_MAX_COLS]; int dtype[GQ_MAX_COLS];
+  u32* hist;                 // [nparts][CTAs of the grid]
+  i64* out_row;              // input row number of every output row, or null
+  i64* out_offsets;          // [nparts + 1]
+};
+__device__ __forceinline__ u32 gq_hp_dest(const GqHpParams& P, u32 r) {
+  u64 h = 0x9E3779B97F4A7C15ULL;
+#pragma unroll 1
+  for (int k = 0; k < P.nkeys; ++k) {
+    u64 x = h ^ (u64)gq_sort_load(P.key[k], P.key_dtype[k], (i64)r);
+    x ^= x >> 33; x *= 0xff51afd7ed558ccdULL; x ^= x >> 33; x *= 0xc4ceb9fe1a85ec53ULL; x ^= x >> 33;
+    h = x;
+  }
+  return (u32)(((h >> 32) * (u64)(u32)P.nparts) >> 32);
+}
+// rows [lo, hi) of the calling CTA: whole tiles, contiguous, in CTA order
+__device__ __forceinline__ void gq_hp_range(u32 n, u32* lo, u32* hi) {
+  const u32 ntiles = (n + GQ_HP_TILE - 1) / GQ_HP_TILE;
+  const u32 per = (ntiles + gridDim.x - 1) / gridDim.x;
+  const u64 a = (u64)blockIdx.x * per * GQ_HP_TILE, b = a + (u64)per * GQ_HP_TILE;
+  *lo = (u32)(a < n ? a : n);
+  *hi = (u32)(b < n ? b : n);
+}
+__global__ void __launch_bounds__(GQ_HP_THREADS) gq_k_hp_hist(const __grid_constant__ GqHpParams P) {
+  __shared__ u32 cnt[256];
+  const int t = threadIdx.x, lane = t & 31;
+  cnt[t] = 0;
+  __syncthreads();
+  u32 lo, hi;
+  gq_hp_range(P.n, &lo, &hi);
+  for (u32 base = lo; base < hi; base += GQ_HP_TILE) {
+    u32 d[GQ_HP_ITEMS];
+#pragma unroll
+    for (int j = 0; j < GQ_HP_ITEMS; ++j) { const u32 r = base + j * GQ_HP_THREADS + t; d[j] = r < hi ? gq_hp_dest(P, r) : 256u + (u32)lane; }
+#pragma unroll
+    for (int j = 0; j < GQ_HP_ITEMS; ++j) {
+      const u32 peers = __match_any_sync(0xffffffffu, d[j]);
+      if (d[j] < 256u && (peers & ((1u << lane) - 1u)) == 0) atomicAdd(&cnt[d[j]], (u32)__popc(peers));
+    }
+  }
+  __syncthreads();
+  if (t < P.nparts) P.hist[(size_t)t * gridDim.x + blockIdx.x] = cnt[t];
+}
+__global__ void __launch_bounds__(GQ_HP_THREADS) gq_k_hp_scatter(const __grid_constant__ GqHpParams P) {
+  __shared__ u32 cur[256];                             // the CTA's next output row per destination
+  __shared__ unsigned short wc[GQ_HP_WARPS][256];      // per tile: rows of a destination in every warp, then their offsets
+  __shared__ unsigned short toff[256];                 // per tile: first place of every destination in the tile's order
+  __shared__ u32 wsum[GQ_HP_WARPS];
+  __shared__ u32 gpos[GQ_HP_TILE];                     // per tile: output row of every place
+  __shared__ __align__(16) unsigned char stage[GQ_HP_TILE * 8];
+  const int t = threadIdx.x, lane = t & 31, warp = t >> 5;
+  cur[t] = t < P.nparts ? P.hist[(size_t)t * gridDim.x + blockIdx.x] : 0u;
+  if (blockIdx.x == 0) {                               // CTA 0's cursors are the destinations' first rows
+    if (t < P.nparts) P.out_offsets[t] = (i64)cur[t];
+    if (t == 0) P.out_offsets[P.nparts] = (i64)P.n;
+  }
+  u32 lo, hi;
+  gq_hp_range(P.n, &lo, &hi);
+  for (u32 base = lo; base < hi; base += GQ_HP_TILE) {
+    const u32 nt = min((u32)GQ_HP_TILE, hi - base);    // rows of this tile
+    for (int w = 0; w < GQ_HP_WARPS; ++w) wc[w][t] = 0;
+    __syncthreads();
+    // (1) destination and rank among the warp's rows of that destination; the warp's rows are base + 256 warp + 32 j + lane
+    u32 d[GQ_HP_ITEMS];
+    unsigned short wr[GQ_HP_ITEMS];
+#pragma unroll
+    for (int j = 0; j < GQ_HP_ITEMS; ++j) {
+      const u32 i = (u32)warp * 256u + (u32)j * 32u + (u32)lane;
+      d[j] = i < nt ? gq_hp_dest(P, base + i) : 256u + (u32)lane;
+    }
+#pragma unroll
+    for (int j = 0; j < GQ_HP_ITEMS; ++j) {
+      const u32 peers = __match_any_sync(0xffffffffu, d[j]);
+      const u32 rank = __popc(peers & ((1u << lane) - 1u));
+      const bool have = d[j] < 256u;
+      wr[j] = have ? (unsigned short)(wc[warp][d[j]] + rank) : (unsigned short)0;
+      __syncwarp();
+      if (have && rank == 0) wc[warp][d[j]] += (unsigned short)__popc(peers);
+      __syncwarp();
+    }
+    __syncthreads();
+    // (2) thread q: counters of destination q -> offsets over the warps; block scan of the totals -> toff
+    u32 tot = 0;
+#pragma unroll
+    for (int w = 0; w < GQ_HP_WARPS; ++w) { const u32 c = wc[w][t]; wc[w][t] = (unsigned short)tot; tot += c; }
+    u32 incl = tot;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) { const u32 x = __shfl_up_sync(0xffffffffu, incl, o); if (lane >= o) incl += x; }
+    if (lane == 31) wsum[warp] = incl;
+    __syncthreads();
+    u32 before = 0;
+#pragma unroll
+    for (int w = 0; w < GQ_HP_WARPS; ++w) if (w < warp) before += wsum[w];
+    const u32 first = before + incl - tot;             // place of destination t's first row in the tile
+    toff[t] = (unsigned short)first;
+    __syncthreads();
+    // (3) place of every row in the tile's destination-major order, and the output row of that place
+    unsigned short place[GQ_HP_ITEMS];
+#pragma unroll
+    for (int j = 0; j < GQ_HP_ITEMS; ++j) {
+      place[j] = 0;
+      if (d[j] < 256u) {
+        const u32 in_run = (u32)wc[warp][d[j]] + (u32)wr[j];          // rows of this destination before mine in the tile
+        place[j] = (unsigned short)((u32)toff[d[j]] + in_run);
+        gpos[place[j]] = cur[d[j]] + in_run;
+      }
+    }
+    __syncthreads();
+    cur[t] += tot;
+    if (P.out_row) {
+#pragma unroll
+      for (int j = 0; j < GQ_HP_ITEMS; ++j) {
+        const u32 i = (u32)warp * 256u + (u32)j * 32u + (u32)lane;
+        if (i < nt) P.out_row[gpos[place[j]]] = (i64)(base + i);
+      }
+    }
+    // (4) column by column through the staging buffer
+#pragma unroll 1
+    for (int c = 0; c < P.ncols; ++c) {
+      const int dt = P.dtype[c];
+      if (dt == GQ_I64) {
+        const i64* src = (const i64*)P.col[c] + base;
+        i64 v[GQ_HP_ITEMS];
+#pragma unroll
+        for (int j = 0; j < GQ_HP_ITEMS; ++j) { const u32 i = (u32)warp * 256u + (u32)j * 32u + (u32)lane; v[j] = i < nt ? src[i] : 0; }
+#pragma unroll
+        for (int j = 0; j < GQ_HP_ITEMS; ++j) if (d[j] < 256u) ((i64*)stage)[place[j]] = v[j];
+        __syncthreads();
+        for (u32 p = t; p < nt; p += GQ_HP_THREADS) ((i64*)P.out[c])[gpos[p]] = ((const i64*)stage)[p];
+      } else if (dt == GQ_I32) {
+        const int* src = (const int*)P.col[c] + base;
+        int v[GQ_HP_ITEMS];
+#pragma unroll
+        for (int j = 0; j < GQ_HP_ITEMS; ++j) { const u32 i = (u32)warp * 256u + (u32)j * 32u + (u32)lane; v[j] = i < nt ? src[i] : 0; }
+#pragma unroll
+        for (int j = 0; j < GQ_HP_ITEMS; ++j) if (d[j] < 256u) ((int*)stage)[place[j]] = v[j];
+        __syncthreads();
+        for (u32 p = t; p < nt; p += GQ_HP_THREADS) ((int*)P.out[c])[gpos[p]] = ((const int*)stage)[p];
+      } else {
+        const signed char* src = (const signed char*)P.col[c] + base;
+        signed char v[GQ_HP_ITEMS];
+#pragma unroll
+        for (int j = 0; j < GQ_HP_ITEMS; ++j) { const u32 i = (u32)warp * 256u + (u32)j * 32u + (u32)lane; v[j] = i < nt ? src[i] : 0; }
+#pragma unroll
+        for (int j = 0; j < GQ_HP_ITEMS; ++j) if (d[j] < 256u) ((signed char*)stage)[place[j]] = v[j];
+        __syncthreads();
+        for (u32 p = t; p < nt; p += GQ_HP_THREADS) ((signed char*)P.out[c])[gpos[p]] = ((const signed char*)stage)[p];
+      }
+      __syncthreads();                                  // the buffer is free for the next column / tile
+    }
+  }
+}
+static int gq_hp_blocks(int num_sms) { return std::max(1, std::min(num_sms * 4, 1024)); }
+size_t gq_hash_partition_workspace_bytes(int nparts) {
+  return ((size_t)nparts * (size_t)gq_hp_blocks(GQ_MAX_SMS) * 4 + 255) / 256 * 256;
+}
+cudaError_t gq_launch_hash_partition(cudaStream_t s, int num_sms, const gq_batch* in, const int* key_cols, int nkeys, int nparts, char* ws,
+                                     void* const* out_cols, i64* out_row, i64* out_offsets, int* nlaunches) {
+  GqHpParams P;
+  P.n = (u32)in->nrows; P.nparts = nparts; P.nkeys = nkeys; P.ncols = in->ncols;
+  for (int k = 0; k < nkeys; ++k) { P.key[k] = in->cols[key_cols[k]].data; P.key_dtype[k] = (int)in->cols[key_cols[k]].dtype; }
+  for (int c = 0; c < in->ncols; ++c) { P.col[c] = in->cols[c].data; P.out[c] = out_cols[c]; P.dtype[c] = (int)in->cols[c].dtype; }
+  P.hist = (u32*)ws; P.out_row = out_row; P.out_offsets = out_offsets;
+  const int nblk = gq_hp_blocks(num_sms);
+  gq_k_hp_hist<<<nblk, GQ_HP_THREADS, 0, s>>>(P);
+  gq_k_sort_scan<<<1, 1024, 0, s>>>(P.hist, nparts * nblk);
+  gq_k_hp_scatter<<<nblk, GQ_HP_THREADS, 0, s>>>(P);
+  *nlaunches = 3;
+  return cudaGetLastError();
+}

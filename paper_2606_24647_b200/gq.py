@@ -41,7 +41,8 @@ SYMBOLS = ["gq_create", "gq_destroy", "gq_sync", "gq_clear_error", "gq_status_st
            "gq_aggstate_destroy", "gq_pipeline_workspace", "gq_pipeline", "gq_pipeline_host_workspace",
            "gq_pipeline_host", "gq_set_kernel_cache_dir", "gq_precompile_pipeline", "gq_precompile_build", "gq_precompile_materialise",
            "gq_table_describe", "gq_read_probe", "gq_set_option", "gq_hash_build_workspace_dense", "gq_profile", "gq_profile_read", "gq_order_by_workspace", "gq_order_by", "gq_aggstate_merge", "gq_aggstate_count",
-           "gq_aggstate_rehash", "gq_order_by_static", "gq_order_by_static_max_rows"]
+           "gq_aggstate_rehash", "gq_order_by_static", "gq_order_by_static_max_rows",
+           "gq_hash_partition_workspace", "gq_hash_partition"]
 
 
 class GqError(RuntimeError):
@@ -161,6 +162,9 @@ def lib():
         L.gq_order_by_workspace.argtypes = [C.c_int64, C.POINTER(C.c_size_t)]
         L.gq_order_by.argtypes = [C.c_void_p, C.POINTER(_Batch), C.POINTER(_SortKey), C.c_int32, C.c_int64, C.c_void_p, C.c_size_t,
                                   C.c_void_p, C.POINTER(C.c_void_p)]
+        L.gq_hash_partition_workspace.argtypes = [C.c_int32, C.POINTER(C.c_size_t)]
+        L.gq_hash_partition.argtypes = [C.c_void_p, C.POINTER(_Batch), C.POINTER(C.c_int32), C.c_int32, C.c_int32, C.c_void_p, C.c_size_t,
+                                        C.POINTER(C.c_void_p), C.c_void_p, C.c_void_p]
         L.gq_order_by_static.argtypes = [C.c_void_p, C.POINTER(_Batch), C.POINTER(_SortKey), C.c_int32, C.c_int64,
                                          C.c_void_p, C.POINTER(C.c_void_p)]
         L.gq_order_by_static_max_rows.argtypes = []
@@ -437,6 +441,26 @@ class Context:
                                            index.data_ptr(), m.ptrs(outs) if gather else None))
             self._last_ws = ws
         return index[:nout], ([o[:nout] for o in outs] if gather else None)
+
+    def hash_partition(self, cols, key_cols, nparts, want_rows=False, workspace=None):
+        """gq_hash_partition: -> (out_cols, offsets int64[nparts + 1], rows int64[n] or None); rows of destination d are
+        out rows [offsets[d], offsets[d + 1]), in input order."""
+        with torch.cuda.stream(self.stream):
+            m = _M()
+            b = m.batch(cols)
+            n = int(b.nrows)
+            kk = (C.c_int32 * max(1, len(key_cols)))(*[int(c) for c in key_cols])
+            m.keep.append(kk)
+            nbytes = C.c_size_t()
+            st = self.L.gq_hash_partition_workspace(int(nparts), C.byref(nbytes))
+            ws = workspace if workspace is not None else self._ws(nbytes.value if st == 0 else 256)
+            outs = [self._empty(n, c.dtype) for c in cols]
+            offsets = self._empty(max(1, int(nparts)) + 1, torch.int64)
+            rows = self._empty(n, torch.int64) if want_rows else None
+            self._check(self.L.gq_hash_partition(self.h, C.byref(b), kk, len(key_cols), int(nparts), self._ws_ptr(ws), nbytes.value,
+                                                 m.ptrs(outs), rows.data_ptr() if want_rows else None, offsets.data_ptr()))
+            self._last_ws = ws
+        return outs, offsets, rows
 
     def order_by_static(self, cols, keys, limit, out_index, out_cols=None):
         """gq_order_by_static: order_by that allocates nothing — scratch is a fixed device array inside libgq.so, the
