@@ -362,7 +362,23 @@ def run_standalone_ops(gq, ctx, torch, datagen, plans, gqrun, steps, warmup):
     ctx.sync()
     out["filter_project_c2"] = dict(rows=n, out_rows=int(count.item()), ms=ms, rows_per_s=n / ms * 1e3,
                                     gbs=(28 * n + 16 * int(count.item())) / ms / 1e6)
-    del cols, outs
+    del outs
+    # gq_hash_partition (PartitionedOutput): the C2 table to 8 / 64 destinations by its int64 price
+    # column (column 3: > 10^6 distinct values); algorithmic bytes = key column once (histogram) + every column read and written once (scatter)
+    pouts = [torch.empty_like(c) for c in cols]
+    for nparts in (8, 64):
+        _, poff, _ = ctx.hash_partition(cols, [3], nparts, outs=pouts)
+        pws = ctx._last_ws
+
+        def part():
+            ctx.hash_partition(cols, [3], nparts, workspace=pws, outs=pouts, offsets=poff)
+        ms = time_steps(torch, ctx.stream, part, steps, warmup, lambda: None) / steps
+        ctx.sync()
+        sizes = (poff[1:] - poff[:-1]).cpu().tolist()
+        out[f"hash_partition_c2_{nparts}"] = dict(rows=n, destinations=nparts, ms=ms, rows_per_s=n / ms * 1e3,
+                                                  algorithmic_bytes=(8 + 2 * 28) * n, gbs=(8 + 2 * 28) * n / ms / 1e6,
+                                                  rows_min=int(min(sizes)), rows_max=int(max(sizes)), rows_total=int(sum(sizes)))
+    del cols, pouts
     torch.cuda.empty_cache()
     t3 = datagen.make_config(3)
     p3 = plans.plan_c3(t3)

@@ -357,6 +357,9 @@ cudaError_t gq_launch_order_by_static(cudaStream_t s, int num_sms, const gq_batc
 #define GQ_HP_WARPS (GQ_HP_THREADS / 32)
 #define GQ_HP_ITEMS 8                              // rows per thread and tile
 #define GQ_HP_TILE (GQ_HP_THREADS * GQ_HP_ITEMS)
+#ifndef GQ_HP_CTAS_PER_SM
+#define GQ_HP_CTAS_PER_SM 4
+#endif
 struct GqHpParams {
   u32 n; int nparts; int nkeys; int ncols;
   const void* key[GQ_MAX_KEYS_HP]; int key_dtype[GQ_MAX_KEYS_HP];
@@ -365,15 +368,34 @@ struct GqHpParams {
   i64* out_row;              // input row number of every output row, or null
   i64* out_offsets;          // [nparts + 1]
 };
-__device__ __forceinline__ u32 gq_hp_dest(const GqHpParams& P, u32 r) {
-  u64 h = 0x9E3779B97F4A7C15ULL;
+// Destinations of the calling thread's GQ_HP_ITEMS rows r0 + j * stride (rows >= hi get the invalid value 256 + lane, a
+// different one per lane). Key column by key column: all of the thread's loads of a column are issued before the first
+// hash step uses one (a row-at-a-time loop left ONE load in flight per thread: the histogram ran at 1.6 TB/s).
+template <typename T>
+__device__ __forceinline__ void gq_hp_mix(const void* col, u32 r0, u32 stride, u32 hi, u64 (&h)[GQ_HP_ITEMS]) {
+  T v[GQ_HP_ITEMS];
+#pragma unroll
+  for (int j = 0; j < GQ_HP_ITEMS; ++j) { const u32 r = r0 + (u32)j * stride; v[j] = r < hi ? ((const T*)col)[r] : (T)0; }
+#pragma unroll
+  for (int j = 0; j < GQ_HP_ITEMS; ++j) {
+    u64 x = h[j] ^ (u64)(i64)v[j];
+    x ^= x >> 33; x *= 0xff51afd7ed558ccdULL; x ^= x >> 33; x *= 0xc4ceb9fe1a85ec53ULL; x ^= x >> 33;
+    h[j] = x;
+  }
+}
+__device__ __forceinline__ void gq_hp_dests(const GqHpParams& P, u32 r0, u32 stride, u32 hi, int lane, u32 (&d)[GQ_HP_ITEMS]) {
+  u64 h[GQ_HP_ITEMS];
+#pragma unroll
+  for (int j = 0; j < GQ_HP_ITEMS; ++j) h[j] = 0x9E3779B97F4A7C15ULL;
 #pragma unroll 1
   for (int k = 0; k < P.nkeys; ++k) {
-    u64 x = h ^ (u64)gq_sort_load(P.key[k], P.key_dtype[k], (i64)r);
-    x ^= x >> 33; x *= 0xff51afd7ed558ccdULL; x ^= x >> 33; x *= 0xc4ceb9fe1a85ec53ULL; x ^= x >> 33;
-    h = x;
+    if (P.key_dtype[k] == GQ_I64) gq_hp_mix<i64>(P.key[k], r0, stride, hi, h);
+    else if (P.key_dtype[k] == GQ_I32) gq_hp_mix<int>(P.key[k], r0, stride, hi, h);
+    else gq_hp_mix<signed char>(P.key[k], r0, stride, hi, h);
   }
-  return (u32)(((h >> 32) * (u64)(u32)P.nparts) >> 32);
+#pragma unroll
+  for (int j = 0; j < GQ_HP_ITEMS; ++j)
+    d[j] = r0 + (u32)j * stride < hi ? (u32)(((h[j] >> 32) * (u64)(u32)P.nparts) >> 32) : 256u + (u32)lane;
 }
 // rows [lo, hi) of the calling CTA: whole tiles, contiguous, in CTA order
 __device__ __forceinline__ void gq_hp_range(u32 n, u32* lo, u32* hi) {
@@ -384,26 +406,45 @@ __device__ __forceinline__ void gq_hp_range(u32 n, u32* lo, u32* hi) {
   *hi = (u32)(b < n ? b : n);
 }
 __global__ void __launch_bounds__(GQ_HP_THREADS) gq_k_hp_hist(const __grid_constant__ GqHpParams P) {
-  __shared__ u32 cnt[256];
-  const int t = threadIdx.x, lane = t & 31;
-  cnt[t] = 0;
+  __shared__ u32 cnt[GQ_HP_WARPS][256];              // warp-private counters: an add only meets the adds of its own warp
+  const int t = threadIdx.x, lane = t & 31, warp = t >> 5;
+  for (int w = 0; w < GQ_HP_WARPS; ++w) cnt[w][t] = 0;
   __syncthreads();
   u32 lo, hi;
   gq_hp_range(P.n, &lo, &hi);
   for (u32 base = lo; base < hi; base += GQ_HP_TILE) {
     u32 d[GQ_HP_ITEMS];
+    gq_hp_dests(P, base + (u32)t, GQ_HP_THREADS, hi, lane, d);
 #pragma unroll
-    for (int j = 0; j < GQ_HP_ITEMS; ++j) { const u32 r = base + j * GQ_HP_THREADS + t; d[j] = r < hi ? gq_hp_dest(P, r) : 256u + (u32)lane; }
-#pragma unroll
-    for (int j = 0; j < GQ_HP_ITEMS; ++j) {
-      const u32 peers = __match_any_sync(0xffffffffu, d[j]);
-      if (d[j] < 256u && (peers & ((1u << lane) - 1u)) == 0) atomicAdd(&cnt[d[j]], (u32)__popc(peers));
-    }
+    for (int j = 0; j < GQ_HP_ITEMS; ++j) if (d[j] < 256u) atomicAdd(&cnt[warp][d[j]], 1u);
   }
   __syncthreads();
-  if (t < P.nparts) P.hist[(size_t)t * gridDim.x + blockIdx.x] = cnt[t];
+  if (t < P.nparts) {
+    u32 s = 0;
+#pragma unroll
+    for (int w = 0; w < GQ_HP_WARPS; ++w) s += cnt[w][t];
+    P.hist[(size_t)t * gridDim.x + blockIdx.x] = s;
+  }
 }
-__global__ void __launch_bounds__(GQ_HP_THREADS) gq_k_hp_scatter(const __grid_constant__ GqHpParams P) {
+// the calling thread's GQ_HP_ITEMS values of column c (rows base + 256 warp + 32 j + lane of a tile of nt rows), as raw words
+__device__ __forceinline__ void gq_hp_load(const GqHpParams& P, int c, u32 base, u32 nt, int warp, int lane, u64 (&v)[GQ_HP_ITEMS]) {
+  const int dt = P.dtype[c];
+  const u32 i0 = (u32)warp * 256u + (u32)lane;
+  if (dt == GQ_I64) {
+    const u64* src = (const u64*)P.col[c] + base;
+#pragma unroll
+    for (int j = 0; j < GQ_HP_ITEMS; ++j) { const u32 i = i0 + (u32)j * 32u; v[j] = i < nt ? src[i] : 0ULL; }
+  } else if (dt == GQ_I32) {
+    const u32* src = (const u32*)P.col[c] + base;
+#pragma unroll
+    for (int j = 0; j < GQ_HP_ITEMS; ++j) { const u32 i = i0 + (u32)j * 32u; v[j] = i < nt ? (u64)src[i] : 0ULL; }
+  } else {
+    const unsigned char* src = (const unsigned char*)P.col[c] + base;
+#pragma unroll
+    for (int j = 0; j < GQ_HP_ITEMS; ++j) { const u32 i = i0 + (u32)j * 32u; v[j] = i < nt ? (u64)src[i] : 0ULL; }
+  }
+}
+__global__ void __launch_bounds__(GQ_HP_THREADS, GQ_HP_CTAS_PER_SM) gq_k_hp_scatter(const __grid_constant__ GqHpParams P) {
   __shared__ u32 cur[256];                             // the CTA's next output row per destination
   __shared__ unsigned short wc[GQ_HP_WARPS][256];      // per tile: rows of a destination in every warp, then their offsets
   __shared__ unsigned short toff[256];                 // per tile: first place of every destination in the tile's order
@@ -425,11 +466,7 @@ __global__ void __launch_bounds__(GQ_HP_THREADS) gq_k_hp_scatter(const __grid_co
     // (1) destination and rank among the warp's rows of that destination; the warp's rows are base + 256 warp + 32 j + lane
     u32 d[GQ_HP_ITEMS];
     unsigned short wr[GQ_HP_ITEMS];
-#pragma unroll
-    for (int j = 0; j < GQ_HP_ITEMS; ++j) {
-      const u32 i = (u32)warp * 256u + (u32)j * 32u + (u32)lane;
-      d[j] = i < nt ? gq_hp_dest(P, base + i) : 256u + (u32)lane;
-    }
+    gq_hp_dests(P, base + (u32)warp * 256u + (u32)lane, 32u, base + nt, lane, d);
 #pragma unroll
     for (int j = 0; j < GQ_HP_ITEMS; ++j) {
       const u32 peers = __match_any_sync(0xffffffffu, d[j]);
@@ -476,43 +513,33 @@ __global__ void __launch_bounds__(GQ_HP_THREADS) gq_k_hp_scatter(const __grid_co
         if (i < nt) P.out_row[gpos[place[j]]] = (i64)(base + i);
       }
     }
-    // (4) column by column through the staging buffer
+    // (4) column by column through the staging buffer. A column's values are loaded as raw 64-bit words one column AHEAD:
+    // the loads of column c + 1 are in flight while column c is written out (the registers are free once c is staged).
+    u64 v[GQ_HP_ITEMS];
+    gq_hp_load(P, 0, base, nt, warp, lane, v);
 #pragma unroll 1
     for (int c = 0; c < P.ncols; ++c) {
       const int dt = P.dtype[c];
       if (dt == GQ_I64) {
-        const i64* src = (const i64*)P.col[c] + base;
-        i64 v[GQ_HP_ITEMS];
 #pragma unroll
-        for (int j = 0; j < GQ_HP_ITEMS; ++j) { const u32 i = (u32)warp * 256u + (u32)j * 32u + (u32)lane; v[j] = i < nt ? src[i] : 0; }
-#pragma unroll
-        for (int j = 0; j < GQ_HP_ITEMS; ++j) if (d[j] < 256u) ((i64*)stage)[place[j]] = v[j];
-        __syncthreads();
-        for (u32 p = t; p < nt; p += GQ_HP_THREADS) ((i64*)P.out[c])[gpos[p]] = ((const i64*)stage)[p];
+        for (int j = 0; j < GQ_HP_ITEMS; ++j) if (d[j] < 256u) ((u64*)stage)[place[j]] = v[j];
       } else if (dt == GQ_I32) {
-        const int* src = (const int*)P.col[c] + base;
-        int v[GQ_HP_ITEMS];
 #pragma unroll
-        for (int j = 0; j < GQ_HP_ITEMS; ++j) { const u32 i = (u32)warp * 256u + (u32)j * 32u + (u32)lane; v[j] = i < nt ? src[i] : 0; }
-#pragma unroll
-        for (int j = 0; j < GQ_HP_ITEMS; ++j) if (d[j] < 256u) ((int*)stage)[place[j]] = v[j];
-        __syncthreads();
-        for (u32 p = t; p < nt; p += GQ_HP_THREADS) ((int*)P.out[c])[gpos[p]] = ((const int*)stage)[p];
+        for (int j = 0; j < GQ_HP_ITEMS; ++j) if (d[j] < 256u) ((u32*)stage)[place[j]] = (u32)v[j];
       } else {
-        const signed char* src = (const signed char*)P.col[c] + base;
-        signed char v[GQ_HP_ITEMS];
 #pragma unroll
-        for (int j = 0; j < GQ_HP_ITEMS; ++j) { const u32 i = (u32)warp * 256u + (u32)j * 32u + (u32)lane; v[j] = i < nt ? src[i] : 0; }
-#pragma unroll
-        for (int j = 0; j < GQ_HP_ITEMS; ++j) if (d[j] < 256u) ((signed char*)stage)[place[j]] = v[j];
-        __syncthreads();
-        for (u32 p = t; p < nt; p += GQ_HP_THREADS) ((signed char*)P.out[c])[gpos[p]] = ((const signed char*)stage)[p];
+        for (int j = 0; j < GQ_HP_ITEMS; ++j) if (d[j] < 256u) ((unsigned char*)stage)[place[j]] = (unsigned char)v[j];
       }
+      if (c + 1 < P.ncols) gq_hp_load(P, c + 1, base, nt, warp, lane, v);
+      __syncthreads();
+      if (dt == GQ_I64) { for (u32 p = t; p < nt; p += GQ_HP_THREADS) ((u64*)P.out[c])[gpos[p]] = ((const u64*)stage)[p]; }
+      else if (dt == GQ_I32) { for (u32 p = t; p < nt; p += GQ_HP_THREADS) ((u32*)P.out[c])[gpos[p]] = ((const u32*)stage)[p]; }
+      else { for (u32 p = t; p < nt; p += GQ_HP_THREADS) ((unsigned char*)P.out[c])[gpos[p]] = ((const unsigned char*)stage)[p]; }
       __syncthreads();                                  // the buffer is free for the next column / tile
     }
   }
 }
-static int gq_hp_blocks(int num_sms) { return std::max(1, std::min(num_sms * 4, 1024)); }
+static int gq_hp_blocks(int num_sms) { return std::max(1, std::min(num_sms * GQ_HP_CTAS_PER_SM, 1024)); }
 size_t gq_hash_partition_workspace_bytes(int nparts) {
   return ((size_t)nparts * (size_t)gq_hp_blocks(GQ_MAX_SMS) * 4 + 255) / 256 * 256;
 }

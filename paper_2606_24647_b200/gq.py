@@ -442,7 +442,7 @@ class Context:
             self._last_ws = ws
         return index[:nout], ([o[:nout] for o in outs] if gather else None)
 
-    def hash_partition(self, cols, key_cols, nparts, want_rows=False, workspace=None):
+    def hash_partition(self, cols, key_cols, nparts, want_rows=False, workspace=None, outs=None, offsets=None):
         """gq_hash_partition: -> (out_cols, offsets int64[nparts + 1], rows int64[n] or None); rows of destination d are
         out rows [offsets[d], offsets[d + 1]), in input order."""
         with torch.cuda.stream(self.stream):
@@ -454,8 +454,8 @@ class Context:
             nbytes = C.c_size_t()
             st = self.L.gq_hash_partition_workspace(int(nparts), C.byref(nbytes))
             ws = workspace if workspace is not None else self._ws(nbytes.value if st == 0 else 256)
-            outs = [self._empty(n, c.dtype) for c in cols]
-            offsets = self._empty(max(1, int(nparts)) + 1, torch.int64)
+            outs = outs if outs is not None else [self._empty(n, c.dtype) for c in cols]
+            offsets = offsets if offsets is not None else self._empty(max(1, int(nparts)) + 1, torch.int64)
             rows = self._empty(n, torch.int64) if want_rows else None
             self._check(self.L.gq_hash_partition(self.h, C.byref(b), kk, len(key_cols), int(nparts), self._ws_ptr(ws), nbytes.value,
                                                  m.ptrs(outs), rows.data_ptr() if want_rows else None, offsets.data_ptr()))
