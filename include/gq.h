@@ -244,6 +244,27 @@ gq_status gq_hash_partition(gq_ctx*, const gq_batch* in, const int32_t* key_cols
                             void* d_workspace, size_t bytes, void* const* out_cols, int64_t* d_out_row,
                             int64_t* d_out_offsets);
 
+/* The same partitioning FUSED WITH ITS TRANSFER, in two phases (exchange "without requiring the transfer
+ * to the host memory"; over NVLink the scatter's stores ARE the transfer - no packed send buffer, no separate
+ * all-to-all):
+ *   gq_hash_partition_count       histogram + scan; d_out_counts[d] (int64[nparts]) = rows this batch holds for
+ *                                 destination d. The senders exchange their counts; receiver d lays the senders out one
+ *                                 after the other, which gives every sender the row where its run starts in d's buffers.
+ *   gq_hash_partition_scatter_to  the scatter of THE SAME batch, keys, nparts and workspace (it reuses the scanned
+ *                                 histogram: call it after _count, on the same stream, with nothing in between that
+ *                                 touches the workspace). Rows of destination d are written, in input order, to rows
+ *                                 d_dst_row0[d], d_dst_row0[d] + 1, ... of d's own column buffers: d_dst_cols is a
+ *                                 DEVICE array of nparts * ncols pointers, column c of destination d at [d * ncols + c],
+ *                                 each 16-byte aligned and writable from this GPU - local memory, or another GPU's memory
+ *                                 mapped into this process (peer access / IPC / symmetric memory); d_dst_row0 is a
+ *                                 DEVICE int64[nparts]. A destination buffer holds < 2^32 rows.
+ * The receiver may read its buffers once every sender's scatter has completed (an event / barrier of the caller's). */
+gq_status gq_hash_partition_count(gq_ctx*, const gq_batch* in, const int32_t* key_cols, int32_t nkeys, int32_t nparts,
+                                  void* d_workspace, size_t bytes, int64_t* d_out_counts);
+gq_status gq_hash_partition_scatter_to(gq_ctx*, const gq_batch* in, const int32_t* key_cols, int32_t nkeys, int32_t nparts,
+                                       void* d_workspace, size_t bytes, void* const* d_dst_cols,
+                                       const int64_t* d_dst_row0);
+
 /* Allocation-free variant of gq_order_by for callers that cannot call cudaMalloc (code under CUDA-graph capture, tight
  * serving loops, harnesses that forbid it): same arguments, results and order, but the scratch lives in a file-scope
  * device array inside libgq.so (4.2 MB, held by every GPU that loads the library until the process exits), so the call

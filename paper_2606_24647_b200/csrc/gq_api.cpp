@@ -1439,6 +1439,52 @@ gq_status gq_hash_partition(gq_ctx* ctx, const gq_batch* in, const int32_t* key_
   return GQ_OK;
 }
 
+static gq_status hp_check(gq_ctx* ctx, const gq_batch* in, const int32_t* key_cols, int32_t nkeys, int32_t nparts, void* d_ws, size_t bytes) {
+  gq_status st = check_batch(ctx, in);
+  if (st != GQ_OK) return st;
+  if (in->nrows > (1LL << 31)) return fail(ctx, GQ_ERR_UNSUPPORTED, "gq_hash_partition: more than 2^31 rows");
+  if (nparts < 1) return fail(ctx, GQ_ERR_INVALID_ARG, "gq_hash_partition: nparts < 1");
+  if (nparts > GQ_MAX_PARTITIONS) return fail(ctx, GQ_ERR_UNSUPPORTED, "gq_hash_partition: more than GQ_MAX_PARTITIONS destinations");
+  if (nkeys < 1 || nkeys > GQ_MAX_KEYS_HP || !key_cols) return fail(ctx, GQ_ERR_INVALID_ARG, "gq_hash_partition: 1..8 key columns");
+  for (int k = 0; k < nkeys; ++k)
+    if (key_cols[k] < 0 || key_cols[k] >= in->ncols) return fail(ctx, GQ_ERR_INVALID_ARG, "partition key column out of range");
+  if (!d_ws || !aligned(d_ws, 256)) return fail(ctx, GQ_ERR_INVALID_ARG, "bad workspace");
+  if (bytes < gq_hash_partition_workspace_bytes(nparts)) return fail(ctx, GQ_ERR_WORKSPACE_TOO_SMALL, "hash-partition workspace too small");
+  return GQ_OK;
+}
+gq_status gq_hash_partition_count(gq_ctx* ctx, const gq_batch* in, const int32_t* key_cols, int32_t nkeys, int32_t nparts, void* d_ws,
+                                  size_t bytes, int64_t* d_out_counts) {
+  if (!ctx) return GQ_ERR_INVALID_ARG;
+  gq_status st = hp_check(ctx, in, key_cols, nkeys, nparts, d_ws, bytes);
+  if (st != GQ_OK) return st;
+  if (!d_out_counts || !aligned(d_out_counts, 8)) return fail(ctx, GQ_ERR_INVALID_ARG, "gq_hash_partition_count: missing output");
+  if (in->nrows == 0) {
+    cudaError_t e0 = cudaMemsetAsync(d_out_counts, 0, (size_t)nparts * 8, ctx->stream);
+    return e0 == cudaSuccess ? GQ_OK : cuda_fail(ctx, e0, "hash partition count");
+  }
+  int nl = 0;
+  cudaError_t e = PROF(ctx, "gq_hash_partition_count", gq_launch_hash_partition_count(ctx->stream, ctx->num_sms, in, key_cols, nkeys, nparts,
+                                                                                       (char*)d_ws, (long long*)d_out_counts, &nl));
+  if (e != cudaSuccess) return cuda_fail(ctx, e, "hash partition count");
+  ctx->launches += nl;
+  return GQ_OK;
+}
+gq_status gq_hash_partition_scatter_to(gq_ctx* ctx, const gq_batch* in, const int32_t* key_cols, int32_t nkeys, int32_t nparts, void* d_ws,
+                                       size_t bytes, void* const* d_dst_cols, const int64_t* d_dst_row0) {
+  if (!ctx) return GQ_ERR_INVALID_ARG;
+  gq_status st = hp_check(ctx, in, key_cols, nkeys, nparts, d_ws, bytes);
+  if (st != GQ_OK) return st;
+  if (!d_dst_cols || !aligned(d_dst_cols, 8) || !d_dst_row0 || !aligned(d_dst_row0, 8))
+    return fail(ctx, GQ_ERR_INVALID_ARG, "gq_hash_partition_scatter_to: missing destination tables");
+  if (in->nrows == 0) return GQ_OK;
+  int nl = 0;
+  cudaError_t e = PROF(ctx, "gq_hash_partition_scatter_to", gq_launch_hash_partition_scatter_to(ctx->stream, ctx->num_sms, in, key_cols, nkeys, nparts,
+                                                                                                 (char*)d_ws, d_dst_cols, (const long long*)d_dst_row0, &nl));
+  if (e != cudaSuccess) return cuda_fail(ctx, e, "hash partition scatter");
+  ctx->launches += nl;
+  return GQ_OK;
+}
+
 // Allocation-free variant: workspace = a file-scope device array of gq_sort.cu (see there). No cudaMalloc / cudaFree, no
 // event creation (the launch group is not profiled), nothing but kernel launches, one memset and one 4-byte D2D copy.
 int64_t gq_order_by_static_max_rows(void) { return gq_sort_static_max_rows(); }

@@ -245,6 +245,10 @@ cudaError_t gq_launch_order_by(cudaStream_t s, int num_sms, const gq_batch* in, 
 size_t gq_hash_partition_workspace_bytes(int nparts);
 cudaError_t gq_launch_hash_partition(cudaStream_t s, int num_sms, const gq_batch* in, const int* key_cols, int nkeys, int nparts, char* ws,
                                      void* const* out_cols, long long* out_row, long long* out_offsets, int* nlaunches);
+cudaError_t gq_launch_hash_partition_count(cudaStream_t s, int num_sms, const gq_batch* in, const int* key_cols, int nkeys, int nparts, char* ws,
+                                           long long* counts, int* nlaunches);
+cudaError_t gq_launch_hash_partition_scatter_to(cudaStream_t s, int num_sms, const gq_batch* in, const int* key_cols, int nkeys, int nparts,
+                                                char* ws, void* const* d_dst, const long long* d_row0, int* nlaunches);
 #define GQ_ORDER_BY_STATIC_MAX_ROWS (1 << 17)   // rows gq_order_by_static takes (its scratch is a 4.2 MB file-scope device array)
 long long gq_sort_static_max_rows();
 cudaError_t gq_launch_order_by_static(cudaStream_t s, int num_sms, const gq_batch* in, const gq_sort_key* keys, int nkeys, long long limit,

@@ -366,7 +366,10 @@ struct GqHpParams {
   const void* col[GQ_MAX_COLS]; void* out[GQ_MAX_COLS]; int dtype[GQ_MAX_COLS];
   u32* hist;                 // [nparts][CTAs of the grid]
   i64* out_row;              // input row number of every output row, or null
-  i64* out_offsets;          // [nparts + 1]
+  i64* out_offsets;          // [nparts + 1] (or null)
+  // peer variant (gq_hash_partition_scatter_to): destination d's column c is written through dst[d * ncols + c], starting
+  // at row dst_row0[d] of that buffer — the buffers may live in ANOTHER GPU's memory (peer-mapped over NVLink)
+  void* const* dst; const i64* dst_row0;
 };
 // Destinations of the calling thread's GQ_HP_ITEMS rows r0 + j * stride (rows >= hi get the invalid value 256 + lane, a
 // different one per lane). Key column by key column: all of the thread's loads of a column are issued before the first
@@ -444,6 +447,7 @@ __device__ __forceinline__ void gq_hp_load(const GqHpParams& P, int c, u32 base,
     for (int j = 0; j < GQ_HP_ITEMS; ++j) { const u32 i = i0 + (u32)j * 32u; v[j] = i < nt ? (u64)src[i] : 0ULL; }
   }
 }
+template <bool PEER>
 __global__ void __launch_bounds__(GQ_HP_THREADS, GQ_HP_CTAS_PER_SM) gq_k_hp_scatter(const __grid_constant__ GqHpParams P) {
   __shared__ u32 cur[256];                             // the CTA's next output row per destination
   __shared__ unsigned short wc[GQ_HP_WARPS][256];      // per tile: rows of a destination in every warp, then their offsets
@@ -451,10 +455,14 @@ __global__ void __launch_bounds__(GQ_HP_THREADS, GQ_HP_CTAS_PER_SM) gq_k_hp_scat
   __shared__ u32 wsum[GQ_HP_WARPS];
   __shared__ u32 gpos[GQ_HP_TILE];                     // per tile: output row of every place
   __shared__ __align__(16) unsigned char stage[GQ_HP_TILE * 8];
+  __shared__ unsigned char pdst[PEER ? GQ_HP_TILE : 1];   // peer variant: destination of every place
   const int t = threadIdx.x, lane = t & 31, warp = t >> 5;
   cur[t] = t < P.nparts ? P.hist[(size_t)t * gridDim.x + blockIdx.x] : 0u;
-  if (blockIdx.x == 0) {                               // CTA 0's cursors are the destinations' first rows
-    if (t < P.nparts) P.out_offsets[t] = (i64)cur[t];
+  if (PEER) {   // cursor = row inside the DESTINATION's buffer: dst_row0[d] + (row among this sender's rows for d); < 2^32
+    if (t < P.nparts) cur[t] = cur[t] - P.hist[(size_t)t * gridDim.x] + (u32)P.dst_row0[t];
+  }
+  if (blockIdx.x == 0 && P.out_offsets) {              // CTA 0's cursors are the destinations' first rows
+    if (t < P.nparts) P.out_offsets[t] = (i64)P.hist[(size_t)t * gridDim.x];
     if (t == 0) P.out_offsets[P.nparts] = (i64)P.n;
   }
   u32 lo, hi;
@@ -502,6 +510,7 @@ __global__ void __launch_bounds__(GQ_HP_THREADS, GQ_HP_CTAS_PER_SM) gq_k_hp_scat
         const u32 in_run = (u32)wc[warp][d[j]] + (u32)wr[j];          // rows of this destination before mine in the tile
         place[j] = (unsigned short)((u32)toff[d[j]] + in_run);
         gpos[place[j]] = cur[d[j]] + in_run;
+        if (PEER) pdst[place[j]] = (unsigned char)d[j];
       }
     }
     __syncthreads();
@@ -532,9 +541,18 @@ __global__ void __launch_bounds__(GQ_HP_THREADS, GQ_HP_CTAS_PER_SM) gq_k_hp_scat
       }
       if (c + 1 < P.ncols) gq_hp_load(P, c + 1, base, nt, warp, lane, v);
       __syncthreads();
-      if (dt == GQ_I64) { for (u32 p = t; p < nt; p += GQ_HP_THREADS) ((u64*)P.out[c])[gpos[p]] = ((const u64*)stage)[p]; }
-      else if (dt == GQ_I32) { for (u32 p = t; p < nt; p += GQ_HP_THREADS) ((u32*)P.out[c])[gpos[p]] = ((const u32*)stage)[p]; }
-      else { for (u32 p = t; p < nt; p += GQ_HP_THREADS) ((unsigned char*)P.out[c])[gpos[p]] = ((const unsigned char*)stage)[p]; }
+      if (!PEER) {
+        if (dt == GQ_I64) { for (u32 p = t; p < nt; p += GQ_HP_THREADS) ((u64*)P.out[c])[gpos[p]] = ((const u64*)stage)[p]; }
+        else if (dt == GQ_I32) { for (u32 p = t; p < nt; p += GQ_HP_THREADS) ((u32*)P.out[c])[gpos[p]] = ((const u32*)stage)[p]; }
+        else { for (u32 p = t; p < nt; p += GQ_HP_THREADS) ((unsigned char*)P.out[c])[gpos[p]] = ((const unsigned char*)stage)[p]; }
+      } else {                                          // the run of destination d goes to d's own buffer (peer memory)
+        for (u32 p = t; p < nt; p += GQ_HP_THREADS) {
+          void* o = (void*)__ldg((const unsigned long long*)P.dst + (size_t)pdst[p] * P.ncols + c);
+          if (dt == GQ_I64) ((u64*)o)[gpos[p]] = ((const u64*)stage)[p];
+          else if (dt == GQ_I32) ((u32*)o)[gpos[p]] = ((const u32*)stage)[p];
+          else ((unsigned char*)o)[gpos[p]] = ((const unsigned char*)stage)[p];
+        }
+      }
       __syncthreads();                                  // the buffer is free for the next column / tile
     }
   }
@@ -549,11 +567,48 @@ cudaError_t gq_launch_hash_partition(cudaStream_t s, int num_sms, const gq_batch
   P.n = (u32)in->nrows; P.nparts = nparts; P.nkeys = nkeys; P.ncols = in->ncols;
   for (int k = 0; k < nkeys; ++k) { P.key[k] = in->cols[key_cols[k]].data; P.key_dtype[k] = (int)in->cols[key_cols[k]].dtype; }
   for (int c = 0; c < in->ncols; ++c) { P.col[c] = in->cols[c].data; P.out[c] = out_cols[c]; P.dtype[c] = (int)in->cols[c].dtype; }
-  P.hist = (u32*)ws; P.out_row = out_row; P.out_offsets = out_offsets;
+  P.hist = (u32*)ws; P.out_row = out_row; P.out_offsets = out_offsets; P.dst = nullptr; P.dst_row0 = nullptr;
   const int nblk = gq_hp_blocks(num_sms);
   gq_k_hp_hist<<<nblk, GQ_HP_THREADS, 0, s>>>(P);
   gq_k_sort_scan<<<1, 1024, 0, s>>>(P.hist, nparts * nblk);
-  gq_k_hp_scatter<<<nblk, GQ_HP_THREADS, 0, s>>>(P);
+  gq_k_hp_scatter<false><<<nblk, GQ_HP_THREADS, 0, s>>>(P);
   *nlaunches = 3;
+  return cudaGetLastError();
+}
+// Two-phase variant for a partition fused with its transfer: (1) count — histogram + scan, rows per destination to
+// d_counts; the caller exchanges the counts and derives where this sender's rows start in every destination's buffers;
+// (2) scatter_to — the scatter of the SAME batch (the scanned histogram is still in ws), every destination's run written
+// through that destination's own column pointers (peer-mapped memory of another GPU: the stores travel over NVLink
+// while the next tile is being permuted — no packed send buffer, no separate all-to-all).
+__global__ void gq_k_hp_counts(const u32* hist, int nblk, int nparts, u32 n, i64* counts) {
+  const int d = blockIdx.x * blockDim.x + threadIdx.x;
+  if (d >= nparts) return;
+  const u32 a = hist[(size_t)d * nblk], b = d + 1 < nparts ? hist[(size_t)(d + 1) * nblk] : n;
+  counts[d] = (i64)(b - a);
+}
+static void gq_hp_fill(GqHpParams& P, const gq_batch* in, const int* key_cols, int nkeys, int nparts, char* ws) {
+  P.n = (u32)in->nrows; P.nparts = nparts; P.nkeys = nkeys; P.ncols = in->ncols;
+  for (int k = 0; k < nkeys; ++k) { P.key[k] = in->cols[key_cols[k]].data; P.key_dtype[k] = (int)in->cols[key_cols[k]].dtype; }
+  for (int c = 0; c < in->ncols; ++c) { P.col[c] = in->cols[c].data; P.out[c] = nullptr; P.dtype[c] = (int)in->cols[c].dtype; }
+  P.hist = (u32*)ws; P.out_row = nullptr; P.out_offsets = nullptr; P.dst = nullptr; P.dst_row0 = nullptr;
+}
+cudaError_t gq_launch_hash_partition_count(cudaStream_t s, int num_sms, const gq_batch* in, const int* key_cols, int nkeys, int nparts, char* ws,
+                                           i64* counts, int* nlaunches) {
+  GqHpParams P;
+  gq_hp_fill(P, in, key_cols, nkeys, nparts, ws);
+  const int nblk = gq_hp_blocks(num_sms);
+  gq_k_hp_hist<<<nblk, GQ_HP_THREADS, 0, s>>>(P);
+  gq_k_sort_scan<<<1, 1024, 0, s>>>(P.hist, nparts * nblk);
+  gq_k_hp_counts<<<1, 256, 0, s>>>(P.hist, nblk, nparts, P.n, counts);
+  *nlaunches = 3;
+  return cudaGetLastError();
+}
+cudaError_t gq_launch_hash_partition_scatter_to(cudaStream_t s, int num_sms, const gq_batch* in, const int* key_cols, int nkeys, int nparts,
+                                                char* ws, void* const* d_dst, const i64* d_row0, int* nlaunches) {
+  GqHpParams P;
+  gq_hp_fill(P, in, key_cols, nkeys, nparts, ws);
+  P.dst = d_dst; P.dst_row0 = d_row0;
+  gq_k_hp_scatter<true><<<gq_hp_blocks(num_sms), GQ_HP_THREADS, 0, s>>>(P);
+  *nlaunches = 1;
   return cudaGetLastError();
 }

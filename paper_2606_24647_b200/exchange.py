@@ -57,3 +57,42 @@ def hash_exchange(ctx, cols, key_cols, group=None):
     outs, offsets, _ = ctx.hash_partition(cols, key_cols, world)
     with torch.cuda.stream(ctx.stream):
         return exchange_partitioned(outs, offsets, group)
+
+
+def exchange_layout(counts, group=None):
+    """Phase between gq_hash_partition_count and gq_hash_partition_scatter_to: all ranks share their per-destination row
+    counts (one all-gather of world int64s per rank); receiver d lays the senders out one after the other. counts:
+    int64[world] tensor of this rank. -> (row0 int64[world] CPU tensor: the row of destination d's buffers where THIS
+    rank's run starts; recv_counts int64[world] CPU tensor: rows every sender will write into THIS rank's buffers)."""
+    world, rank = td.get_world_size(group), td.get_rank(group)
+    c = counts.detach().to(torch.int64).reshape(-1)
+    if c.numel() != world:
+        raise ValueError(f"counts must hold world_size = {world} entries, got {c.numel()}")
+    allc = torch.empty(world * world, dtype=torch.int64, device=c.device)
+    td.all_gather_into_tensor(allc, c.contiguous(), group=group)
+    m = allc.cpu().reshape(world, world)                     # [sender][destination]
+    row0 = m[:rank].sum(dim=0) if rank > 0 else torch.zeros(world, dtype=torch.int64)
+    return row0, m[:, rank].clone()
+
+
+def hash_exchange_fused(ctx, cols, key_cols, peer_cols, group=None):
+    """Partition fused with its transfer (gq.h: gq_hash_partition_count / _scatter_to): no packed send buffer and no
+    all-to-all of the data — after the counts have been shared, the scatter kernel stores every destination's run
+    straight into that destination's receive buffers. peer_cols[d][c]: destination d's buffer for column c as a tensor
+    THIS process can write — on several GPUs the peers' memory mapped over NVLink (CUDA IPC / symmetric memory; peer_cols
+    [rank] are this rank's own buffers), allocated by the caller with room for what exchange_layout announces.
+    -> recv_counts (CPU int64[world]): rows[sum(recv_counts[:s]) ...] of this rank's buffers came from sender s. On return
+    every rank's scatter has completed (stream synchronised, then a barrier): the receive buffers may be read."""
+    world = td.get_world_size(group)
+    if len(peer_cols) != world or any(len(p) != len(cols) for p in peer_cols):
+        raise ValueError("peer_cols must be [world_size][number of columns]")
+    counts, ws = ctx.hash_partition_count(cols, key_cols, world)
+    row0, recv_counts = exchange_layout(counts, group)
+    for d in range(world):
+        need = int(row0[d]) + int(counts[d])
+        if any(t.numel() < need or t.dtype != c.dtype for t, c in zip(peer_cols[d], cols)):
+            raise ValueError(f"destination {d}: receive buffers too small or of the wrong dtype (need {need} rows)")
+    ctx.hash_partition_scatter_to(cols, key_cols, world, ws, peer_cols, row0.to(cols[0].device))
+    ctx.sync()
+    td.barrier(group=group)
+    return recv_counts

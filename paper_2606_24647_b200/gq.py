@@ -42,7 +42,7 @@ SYMBOLS = ["gq_create", "gq_destroy", "gq_sync", "gq_clear_error", "gq_status_st
            "gq_pipeline_host", "gq_set_kernel_cache_dir", "gq_precompile_pipeline", "gq_precompile_build", "gq_precompile_materialise",
            "gq_table_describe", "gq_read_probe", "gq_set_option", "gq_hash_build_workspace_dense", "gq_profile", "gq_profile_read", "gq_order_by_workspace", "gq_order_by", "gq_aggstate_merge", "gq_aggstate_count",
            "gq_aggstate_rehash", "gq_order_by_static", "gq_order_by_static_max_rows",
-           "gq_hash_partition_workspace", "gq_hash_partition"]
+           "gq_hash_partition_workspace", "gq_hash_partition", "gq_hash_partition_count", "gq_hash_partition_scatter_to"]
 
 
 class GqError(RuntimeError):
@@ -165,6 +165,10 @@ def lib():
         L.gq_hash_partition_workspace.argtypes = [C.c_int32, C.POINTER(C.c_size_t)]
         L.gq_hash_partition.argtypes = [C.c_void_p, C.POINTER(_Batch), C.POINTER(C.c_int32), C.c_int32, C.c_int32, C.c_void_p, C.c_size_t,
                                         C.POINTER(C.c_void_p), C.c_void_p, C.c_void_p]
+        L.gq_hash_partition_count.argtypes = [C.c_void_p, C.POINTER(_Batch), C.POINTER(C.c_int32), C.c_int32, C.c_int32, C.c_void_p, C.c_size_t,
+                                              C.c_void_p]
+        L.gq_hash_partition_scatter_to.argtypes = [C.c_void_p, C.POINTER(_Batch), C.POINTER(C.c_int32), C.c_int32, C.c_int32, C.c_void_p,
+                                                   C.c_size_t, C.c_void_p, C.c_void_p]
         L.gq_order_by_static.argtypes = [C.c_void_p, C.POINTER(_Batch), C.POINTER(_SortKey), C.c_int32, C.c_int64,
                                          C.c_void_p, C.POINTER(C.c_void_p)]
         L.gq_order_by_static_max_rows.argtypes = []
@@ -461,6 +465,36 @@ class Context:
                                                  m.ptrs(outs), rows.data_ptr() if want_rows else None, offsets.data_ptr()))
             self._last_ws = ws
         return outs, offsets, rows
+
+    def hash_partition_count(self, cols, key_cols, nparts, workspace=None):
+        """Phase 1 of the fused partition + transfer: -> (counts int64[nparts] on the device, workspace to pass on)."""
+        with torch.cuda.stream(self.stream):
+            m = _M()
+            b = m.batch(cols)
+            kk = (C.c_int32 * max(1, len(key_cols)))(*[int(c) for c in key_cols])
+            m.keep.append(kk)
+            nbytes = C.c_size_t()
+            st = self.L.gq_hash_partition_workspace(int(nparts), C.byref(nbytes))
+            ws = workspace if workspace is not None else self._ws(nbytes.value if st == 0 else 256)
+            counts = self._empty(max(1, int(nparts)), torch.int64)
+            self._check(self.L.gq_hash_partition_count(self.h, C.byref(b), kk, len(key_cols), int(nparts), self._ws_ptr(ws), nbytes.value,
+                                                       counts.data_ptr()))
+        return counts, ws
+
+    def hash_partition_scatter_to(self, cols, key_cols, nparts, workspace, dst_cols, dst_row0):
+        """Phase 2: scatter the same batch; dst_cols[d][c] = destination d's buffer for column c (a tensor this GPU can
+        write: local or peer-mapped), dst_row0 = int64[nparts] device tensor of first rows."""
+        with torch.cuda.stream(self.stream):
+            m = _M()
+            b = m.batch(cols)
+            kk = (C.c_int32 * max(1, len(key_cols)))(*[int(c) for c in key_cols])
+            m.keep.append(kk)
+            nbytes = C.c_size_t()
+            self._check(self.L.gq_hash_partition_workspace(int(nparts), C.byref(nbytes)))
+            ptrs = torch.tensor([int(t.data_ptr()) for d in dst_cols for t in d], dtype=torch.int64).to(self.device, non_blocking=False)
+            self._check(self.L.gq_hash_partition_scatter_to(self.h, C.byref(b), kk, len(key_cols), int(nparts), self._ws_ptr(workspace),
+                                                            nbytes.value, ptrs.data_ptr(), dst_row0.data_ptr()))
+            self._last_ptrs = ptrs
 
     def order_by_static(self, cols, keys, limit, out_index, out_cols=None):
         """gq_order_by_static: order_by that allocates nothing — scratch is a fixed device array inside libgq.so, the

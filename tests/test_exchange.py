@@ -58,7 +58,10 @@ def _worker(rank, world, port, out):
                 exchange.exchange_partitioned([torch.zeros(8, dtype=torch.int64)], off, None)
             except ValueError:
                 bad += 1
-        out.put((rank, [g.numpy() for g in got], counts.tolist(), [c.copy() for c in final.cols], bad))
+        # (4) layout of the fused variant: every rank announces its counts, gets the first row of its runs
+        mine = torch.from_numpy(np.diff(offsets).astype(np.int64))
+        row0, rc = exchange.exchange_layout(mine, None)
+        out.put((rank, [g.numpy() for g in got], counts.tolist(), [c.copy() for c in final.cols], bad, row0.tolist(), rc.tolist()))
         td.barrier()
     finally:
         td.destroy_process_group()
@@ -87,8 +90,10 @@ def test_two_ranks_exchange_rows_and_partial_groups():
     whole_part = oracle.hash_partition([whole.cols[0]], [0], WORLD)
     owner = np.empty(whole.nrows, np.int64); owner[whole_part.cols[1]] = whole_part.cols[0]
     seen = 0
-    for rank, got, counts, final_cols, bad in res:
+    cm = np.array([[int((dests[s] == d).sum()) for d in range(WORLD)] for s in range(WORLD)])     # [sender][destination]
+    for rank, got, counts, final_cols, bad, row0, rc in res:
         assert bad == 3
+        assert row0 == (np.cumsum(cm, axis=0) - cm)[rank].tolist() and rc == cm[:, rank].tolist()
         assert counts == [int((dests[s] == rank).sum()) for s in range(WORLD)]
         for j in range(4):                                 # rows by sender, input order inside a sender, whole rows together
             want = np.concatenate([tables[s][j][dests[s] == rank] for s in range(WORLD)])

@@ -123,3 +123,49 @@ def test_partitions_feed_partial_to_final_aggregation(ctx):
             assert np.array_equal(got["cols"][j], whole.cols[j][sel]), f"destination {d}, column {j}"
         seen += got["n"]
     assert seen == whole.nrows
+
+
+def test_count_then_scatter_into_destination_buffers(ctx):
+    # the fused partition + transfer protocol on one GPU: three "senders" (batches) count, the counts are laid out per
+    # destination (sender after sender: what an exchange of counts gives every rank), then every sender scatters straight
+    # into the destinations' own buffers — separate allocations here, peer-mapped memory on several GPUs. Destination d
+    # must end up with exactly the oracle's rows of destination d: by sender, input order inside a sender.
+    import torch
+    import gqrun
+    rng = np.random.default_rng(21)
+    nparts, sizes = 5, (70_001, 4_097, 33)
+    senders = []
+    for i, n in enumerate(sizes):
+        cols = _cols(n, 300 + i)
+        cols[2][::3] = cols[2][0]                                   # repeated keys across senders meet on one destination
+        senders.append(cols)
+    keys = [2, 0]
+    dcols = [gqrun.dev(c) for c in senders]
+    counts, wss = [], []
+    for dc in dcols:
+        c, ws = ctx.hash_partition_count(dc, keys, nparts)
+        counts.append(c); wss.append(ws)
+    ctx.sync()
+    cm = torch.stack(counts).cpu().numpy()                           # [sender][destination]
+    exp = [oracle.hash_partition(c, keys, nparts) for c in senders]
+    for s, e in enumerate(exp):
+        assert np.array_equal(cm[s], np.bincount(e.cols[0], minlength=nparts))
+    row0 = np.cumsum(cm, axis=0) - cm                                # first row of sender s in destination d's buffers
+    total = cm.sum(axis=0)
+    dst = [[torch.full((int(total[d]) + 16,), -99, dtype=c.dtype, device="cuda") for c in dcols[0]] for d in range(nparts)]
+    for s, dc in enumerate(dcols):
+        ctx.hash_partition_scatter_to(dc, keys, nparts, wss[s], dst, torch.from_numpy(row0[s].copy()).cuda())
+    ctx.sync()
+    for d in range(nparts):
+        for j in range(4):
+            want = np.concatenate([e.cols[2 + j][e.cols[0] == d] for e in exp])
+            got = dst[d][j].cpu().numpy().astype(np.int64)
+            assert np.array_equal(got[:len(want)], want), f"destination {d}, column {j}"
+            assert np.all(got[len(want):] == -99)                    # nothing written past the destination's rows
+    # an empty sender and argument errors
+    from paper_2606_24647_b200 import gq
+    c0, ws0 = ctx.hash_partition_count([t[:0] for t in dcols[0]], keys, nparts)
+    ctx.sync()
+    assert c0.cpu().tolist() == [0] * nparts
+    with pytest.raises(gq.GqError):
+        ctx.hash_partition_count(dcols[0], [9], nparts)

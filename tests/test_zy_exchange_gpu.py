@@ -34,5 +34,14 @@ def test_single_rank_hash_exchange_returns_the_input():
             assert counts.tolist() == [n]
             for g, c in zip(got, cols):
                 assert g.dtype == torch.from_numpy(c[:1]).dtype and np.array_equal(g.cpu().numpy(), c)
+        # the fused variant: counts -> layout (all-gather) -> the scatter stores into the destination's own buffers
+        recv = [[torch.full((n + 8,), -5, dtype=c.dtype, device="cuda") for c in dcols]]
+        for _ in range(2):
+            rc = exchange.hash_exchange_fused(ctx, dcols, [0, 2], recv)
+            assert rc.tolist() == [n]
+            for g, c in zip(recv[0], cols):
+                assert np.array_equal(g[:n].cpu().numpy(), c) and bool((g[n:] == -5).all())
+        with pytest.raises(ValueError):
+            exchange.hash_exchange_fused(ctx, dcols, [0], [[torch.empty(10, dtype=c.dtype, device="cuda") for c in dcols]])
     finally:
         td.destroy_process_group()
