@@ -13,8 +13,8 @@
 //   scan       — one CTA turns the [digit][CTA] counts into exclusive offsets (digit-major: stable across CTAs);
 //   scatter    — every CTA walks its range again in order; inside a tile ranks are stable: the warp's lanes with equal
 //                digits are found with MATCH.ANY, warps are ordered through per-warp digit counts in shared memory.
-// TopN (limit << rows): two histogram levels over the top 24 bits of the most significant key select a threshold
-// bucket on the device; only rows at or before it (>= limit of them, more only with ties) are compacted and sorted.
+// TopN (limit << rows): two 12-bit histogram levels below the common prefix of the most significant key's images select a
+// threshold bucket on the device; only rows at or before it (>= limit of them, more only with ties) are compacted and sorted.
 // Everything is stream-ordered; the number of candidate rows stays in device memory (no host synchronisation).
 #include <algorithm>
 
@@ -74,24 +74,47 @@ __global__ void __launch_bounds__(GQ_SORT_THREADS) gq_k_sort_hist(const u64* key
   hist[threadIdx.x * gridDim.x + blockIdx.x] = h[threadIdx.x];      // [digit][CTA]
 }
 
-// exclusive scan of hist in [digit][CTA] order, in place; one CTA of 1024 threads
-__global__ void __launch_bounds__(1024) gq_k_sort_scan(u32* hist, int total) {
-  __shared__ u32 part[1024];
-  const int t = threadIdx.x;
-  const int per = (total + 1023) / 1024;
-  const int lo = t * per, hi = min(total, lo + per);
-  u32 s = 0;
-  for (int i = lo; i < hi; ++i) s += hist[i];
-  part[t] = s;
+// inclusive scan of one value per thread over a CTA of 1024 threads (warp shuffles + one shared-memory step); returns the
+// inclusive prefix, *total = the CTA's sum. Every thread of the CTA calls it.
+__device__ __forceinline__ u32 gq_block_scan_1024(u32 v, u32* wsum /* [33] shared */, u32* total) {
+  const int t = threadIdx.x, lane = t & 31, warp = t >> 5;
+  u32 incl = v;
+#pragma unroll
+  for (int o = 1; o < 32; o <<= 1) { const u32 x = __shfl_up_sync(0xffffffffu, incl, o); if (lane >= o) incl += x; }
+  __syncthreads();                                   // (wsum may still be read by the previous call)
+  if (lane == 31) wsum[warp] = incl;
   __syncthreads();
-  for (int o = 1; o < 1024; o <<= 1) {
-    const u32 v = t >= o ? part[t - o] : 0;
-    __syncthreads();
-    part[t] += v;
-    __syncthreads();
+  if (warp == 0) {
+    u32 w = wsum[lane], wi = w;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) { const u32 x = __shfl_up_sync(0xffffffffu, wi, o); if (lane >= o) wi += x; }
+    wsum[lane] = wi - w;                              // exclusive prefix of the warp sums
+    if (lane == 31) wsum[32] = wi;
   }
-  u32 run = part[t] - s;
-  for (int i = lo; i < hi; ++i) { const u32 c = hist[i]; hist[i] = run; run += c; }
+  __syncthreads();
+  *total = wsum[32];
+  return incl + wsum[warp];
+}
+// exclusive scan of hist in [digit][CTA] order, in place; one CTA of 1024 threads walks it in chunks of 4096 counters,
+// four consecutive counters per thread (coalesced 16-byte accesses; the first version gave every thread its own
+// contiguous share: strided accesses and a 148-step serial loop, 153 us per pass for 592 CTAs)
+__global__ void __launch_bounds__(1024) gq_k_sort_scan(u32* hist, int total) {
+  __shared__ u32 wsum[33];
+  const int t = threadIdx.x;
+  u32 carry = 0;
+  for (int base = 0; base < total; base += 4096) {
+    const int i = base + 4 * t;
+    u32 v[4];
+    if (i + 3 < total && (total & 3) == 0) { const uint4 q = *(const uint4*)(hist + i); v[0] = q.x; v[1] = q.y; v[2] = q.z; v[3] = q.w; }
+    else { for (int k = 0; k < 4; ++k) v[k] = i + k < total ? hist[i + k] : 0u; }
+    const u32 s = v[0] + v[1] + v[2] + v[3];
+    u32 tot;
+    const u32 excl = gq_block_scan_1024(s, wsum, &tot) - s + carry;
+    const u32 o0 = excl, o1 = o0 + v[0], o2 = o1 + v[1], o3 = o2 + v[2];
+    if (i + 3 < total && (total & 3) == 0) *(uint4*)(hist + i) = make_uint4(o0, o1, o2, o3);
+    else { const u32 o[4] = {o0, o1, o2, o3}; for (int k = 0; k < 4; ++k) if (i + k < total) hist[i + k] = o[k]; }
+    carry += tot;
+  }
 }
 
 __global__ void __launch_bounds__(GQ_SORT_THREADS) gq_k_sort_scatter(const u64* kin, const u32* iin, u64* kout, u32* iout, const u32* d_n,
@@ -139,39 +162,88 @@ struct GqSelParams {
 __device__ __forceinline__ u64 gq_sel_top(const GqSelParams& P, u32 r) {   // sortable image left-aligned in 64 bits
   return gq_sort_image(gq_sort_load(P.col, P.dtype, (i64)r), P.bytes, P.desc) << (64 - 8 * P.bytes);
 }
+// The two 12-bit histogram levels sit directly BELOW the bits all keys share: a pre-pass takes the minimum and maximum of
+// the images (ctl words 16..19: ~min and max, both as atomic maxima over the zeroed control block), their common prefix
+// is skipped. (With the levels fixed at the top 24 bits a column of small non-negative int64 values — prices, counts —
+// fell into ONE bucket, every row became a candidate and TopN cost more than the full sort: 18.6 vs 10.0 ms, 60 M rows.)
+__global__ void __launch_bounds__(256) gq_k_sel_range(const __grid_constant__ GqSelParams P) {
+  u64 lo = ~0ULL, hi = 0;
+  for (u32 r = blockIdx.x * 256 + threadIdx.x; r < P.n; r += gridDim.x * 256) {
+    const u64 u = gq_sel_top(P, r);
+    lo = u < lo ? u : lo;
+    hi = u > hi ? u : hi;
+  }
+  for (int o = 16; o > 0; o >>= 1) {
+    const u64 a = __shfl_xor_sync(0xffffffffu, lo, o), b = __shfl_xor_sync(0xffffffffu, hi, o);
+    lo = a < lo ? a : lo;
+    hi = b > hi ? b : hi;
+  }
+  if ((threadIdx.x & 31) == 0 && lo <= hi) { atomicMax((u64*)(P.ctl + 16), ~lo); atomicMax((u64*)(P.ctl + 18), hi); }
+}
+// shifts of the two levels: level 1 = the 12 bits below the common prefix of all images, level 2 = the 12 below those
+__device__ __forceinline__ void gq_sel_shifts(const GqSelParams& P, int* s1, int* s2) {
+  const u64 lo = ~*(volatile const u64*)(P.ctl + 16), hi = *(volatile const u64*)(P.ctl + 18);
+  const u64 x = lo ^ hi;
+  const int vary = x ? 64 - __clzll((long long)x) : 0;        // bits [0, vary) differ between some two keys
+  *s1 = vary > 12 ? vary - 12 : 0;
+  *s2 = *s1 > 12 ? *s1 - 12 : 0;
+}
 __global__ void __launch_bounds__(256) gq_k_sel_hist(const __grid_constant__ GqSelParams P, int level) {
   __shared__ u32 h[GQ_SEL_BINS];
   for (int i = threadIdx.x; i < GQ_SEL_BINS; i += 256) h[i] = 0;
   __syncthreads();
+  int s1, s2;
+  gq_sel_shifts(P, &s1, &s2);
   const u32 t1 = level == 2 ? P.ctl[0] : 0;
   for (u32 r = blockIdx.x * 256 + threadIdx.x; r < P.n; r += gridDim.x * 256) {
     const u64 u = gq_sel_top(P, r);
-    if (level == 1) atomicAdd(&h[u >> 52], 1u);
-    else if ((u32)(u >> 52) == t1) atomicAdd(&h[(u >> 40) & (GQ_SEL_BINS - 1)], 1u);
+    const u32 b1 = (u32)(u >> s1) & (GQ_SEL_BINS - 1);
+    if (level == 1) atomicAdd(&h[b1], 1u);
+    else if (b1 == t1) atomicAdd(&h[(u32)(u >> s2) & (GQ_SEL_BINS - 1)], 1u);
   }
   __syncthreads();
   u32* g = level == 1 ? P.hist1 : P.hist2;
   for (int i = threadIdx.x; i < GQ_SEL_BINS; i += 256) if (h[i]) atomicAdd(&g[i], h[i]);
 }
-// one thread walks the 4096 counts (a few microseconds): threshold = first bucket at which the running count reaches the limit
-__global__ void gq_k_sel_pick(const __grid_constant__ GqSelParams P, int level) {
-  if (threadIdx.x != 0 || blockIdx.x != 0) return;
+// threshold = the first bucket at which the running count reaches the limit; one CTA of 1024 threads, four buckets each
+// (one thread walking 4096 global counters took 100-165 us)
+__global__ void __launch_bounds__(1024) gq_k_sel_pick(const __grid_constant__ GqSelParams P, int level) {
+  __shared__ u32 wsum[33];
+  __shared__ u32 best;
+  const int t = threadIdx.x;
   const u32* h = level == 1 ? P.hist1 : P.hist2;
   u64 need = P.limit;
-  if (level == 2) { u64 below = 0; for (u32 b = 0; b < P.ctl[0]; ++b) below += P.hist1[b]; need = P.limit > below ? P.limit - below : 1; }
-  u64 run = 0;
-  u32 b = 0;
-  for (; b < GQ_SEL_BINS - 1; ++b) { run += h[b]; if (run >= need) break; }
-  P.ctl[level - 1] = b;
+  if (level == 2) {                                   // rows in the buckets before level 1's threshold are taken anyway
+    const u32 t1 = P.ctl[0];
+    u32 mine = 0;
+    for (int k = 0; k < 4; ++k) if ((u32)(4 * t + k) < t1) mine += P.hist1[4 * t + k];
+    u32 below;
+    gq_block_scan_1024(mine, wsum, &below);
+    need = P.limit > (u64)below ? P.limit - (u64)below : 1;
+  }
+  if (t == 0) best = GQ_SEL_BINS - 1;
+  u32 v[4];
+  for (int k = 0; k < 4; ++k) v[k] = h[4 * t + k];
+  const u32 s = v[0] + v[1] + v[2] + v[3];
+  u32 tot;
+  u64 run = (u64)(gq_block_scan_1024(s, wsum, &tot) - s);      // (counts sum to <= 2^31 rows: 32 bits suffice)
+  for (int k = 0; k < 4; ++k) {
+    run += v[k];
+    if (run >= need) { atomicMin(&best, (u32)(4 * t + k)); break; }
+  }
+  __syncthreads();
+  if (t == 0) P.ctl[level - 1] = best;
 }
 __global__ void __launch_bounds__(256) gq_k_sel_compact(const __grid_constant__ GqSelParams P, u32* idx) {
   const u32 t1 = P.ctl[0], t2 = P.ctl[1];
+  int s1, s2;
+  gq_sel_shifts(P, &s1, &s2);
   for (u32 r0 = blockIdx.x * 256; r0 < P.n; r0 += gridDim.x * 256) {
     const u32 r = r0 + threadIdx.x;
     bool take = false;
     if (r < P.n) {
       const u64 u = gq_sel_top(P, r);
-      const u32 b1 = (u32)(u >> 52), b2 = (u32)(u >> 40) & (GQ_SEL_BINS - 1);
+      const u32 b1 = (u32)(u >> s1) & (GQ_SEL_BINS - 1), b2 = (u32)(u >> s2) & (GQ_SEL_BINS - 1);
       take = b1 < t1 || (b1 == t1 && b2 <= t2);
     }
     const u32 m = __ballot_sync(0xffffffffu, take);
@@ -233,17 +305,20 @@ cudaError_t gq_launch_order_by(cudaStream_t s, int num_sms, const gq_batch* in, 
   int nl = 0, cur = 0;
   const int gs = std::max(1, std::min<int>(num_sms * 8, (int)((n + 255) / 256)));
   auto dtype_bytes = [](int t) { return t == GQ_I8 ? 1 : t == GQ_I32 ? 4 : 8; };
+  const bool topn = nkeys > 0 && lim * 8 < (u64)n && n >= (1u << 16);
+  // TopN sorts its few candidates (how many is known on the device only) with a small grid: the scan and the launches,
+  // not the data, are what its passes cost. (Any grid is correct; many tied candidates just take longer.)
+  const int nb = topn ? std::min(nblk, 16) : nblk;
   auto passes = [&](int bytes) {                     // LSD passes over the low `bytes` bytes of kbuf[cur]
     for (int b = 0; b < bytes; ++b) {
-      gq_k_sort_hist<<<nblk, GQ_SORT_THREADS, 0, s>>>(kbuf[cur], d_n, 8 * b, hist);
-      gq_k_sort_scan<<<1, 1024, 0, s>>>(hist, 256 * nblk);
-      gq_k_sort_scatter<<<nblk, GQ_SORT_THREADS, 0, s>>>(kbuf[cur], ibuf[cur], kbuf[cur ^ 1], ibuf[cur ^ 1], d_n, 8 * b, hist);
+      gq_k_sort_hist<<<nb, GQ_SORT_THREADS, 0, s>>>(kbuf[cur], d_n, 8 * b, hist);
+      gq_k_sort_scan<<<1, 1024, 0, s>>>(hist, 256 * nb);
+      gq_k_sort_scatter<<<nb, GQ_SORT_THREADS, 0, s>>>(kbuf[cur], ibuf[cur], kbuf[cur ^ 1], ibuf[cur ^ 1], d_n, 8 * b, hist);
       cur ^= 1;
       nl += 3;
     }
   };
   cudaError_t e = cudaSuccess;
-  const bool topn = nkeys > 0 && lim * 8 < (u64)n && n >= (1u << 16);
   if (topn) {
     e = cudaMemsetAsync(ws + L.sel1, 0, L.total - L.sel1, s);   // both histograms and the control words
     if (e != cudaSuccess) return e;
@@ -251,9 +326,11 @@ cudaError_t gq_launch_order_by(cudaStream_t s, int num_sms, const gq_batch* in, 
     const gq_column& c0 = in->cols[keys[0].col];
     sp.col = c0.data; sp.dtype = (int)c0.dtype; sp.bytes = dtype_bytes((int)c0.dtype); sp.desc = keys[0].descending ? 1 : 0;
     sp.n = n; sp.limit = lim; sp.hist1 = (u32*)(ws + L.sel1); sp.hist2 = (u32*)(ws + L.sel2); sp.ctl = ctl;
+    gq_k_sel_range<<<gs, 256, 0, s>>>(sp);
+    ++nl;
     for (int level = 1; level <= 2; ++level) {
       gq_k_sel_hist<<<gs, 256, 0, s>>>(sp, level);
-      gq_k_sel_pick<<<1, 32, 0, s>>>(sp, level);
+      gq_k_sel_pick<<<1, 1024, 0, s>>>(sp, level);
     }
     gq_k_sel_compact<<<gs, 256, 0, s>>>(sp, ibuf[0]);
     nl += 5;

@@ -73,6 +73,13 @@ def test_topn_selects_candidates_on_device(ctx):
     for keys, limit in (([(0, True)], 10), ([(0, False)], 1000), ([(1, False), (3, True)], 100), ([(2, True), (0, False)], 4096),
                         ([(1, True)], 100_000), ([(3, False), (1, False)], 1)):
         check(ctx, [wide, narrow, tiny, other], keys, limit=limit)
+    # keys that share a long prefix of bits: small non-negative int64 values (prices, counts), values that differ only in
+    # their low bits, and both with ties at the threshold — the select's two levels start below the common prefix
+    price = rng.integers(0, 10**7, n).astype(np.int64)
+    offset = (2**50 + rng.integers(0, 1000, n)).astype(np.int64)
+    negs = (-(2**40) - rng.integers(0, 5000, n)).astype(np.int64)
+    for keys, limit in (([(0, True)], 100), ([(0, False)], 100), ([(1, False), (0, True)], 64), ([(2, True)], 3000), ([(2, False), (1, True)], 7)):
+        check(ctx, [price, offset, negs, other], keys, limit=limit)
     same = np.full(200_000, 7, np.int64)                            # one key value only: every row is a candidate
     check(ctx, [same, other[:200_000]], [(0, True)], limit=5)
     check(ctx, [same, other[:200_000]], [(0, False), (1, True)], limit=5)
