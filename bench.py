@@ -343,8 +343,8 @@ def run_config(cfg, gq, ctx, torch, datagen, plans, gqrun, steps, warmup, scale=
 
 
 def run_standalone_ops(gq, ctx, torch, datagen, plans, gqrun, steps, warmup):
-    """The standalone, materialising entry points on the C2 / C3 tables: gq_filter_project
-    (ballot/popc compaction), gq_hash_build, gq_hash_probe (inner join materialised as output columns)."""
+    """The standalone entry points on the C2 / C3 tables: gq_filter_project (ballot/popc compaction), gq_hash_partition,
+    gq_order_by, gq_hash_build, gq_hash_probe (inner join materialised as output columns)."""
     out = {}
     t2 = datagen.make_config(2)
     p2 = plans.plan_c2(t2)
@@ -378,7 +378,25 @@ def run_standalone_ops(gq, ctx, torch, datagen, plans, gqrun, steps, warmup):
         out[f"hash_partition_c2_{nparts}"] = dict(rows=n, destinations=nparts, ms=ms, rows_per_s=n / ms * 1e3,
                                                   algorithmic_bytes=(8 + 2 * 28) * n, gbs=(8 + 2 * 28) * n / ms / 1e6,
                                                   rows_min=int(min(sizes)), rows_max=int(max(sizes)), rows_total=int(sum(sizes)))
-    del cols, pouts
+    del pouts
+    # gq_order_by (OrderBy / TopN) on the same table: full stable sort by the int64 price column (row
+    # numbers only / all four columns gathered), by (date desc, price asc), and TopN 100 with the columns gathered
+    for label, keys, limit, gather in (("order_by_c2_int64_index", [(3, False)], 0, False), ("order_by_c2_int64_gather", [(3, False)], 0, True),
+                                       ("order_by_c2_date_desc_price", [(0, True), (3, False)], 0, False),
+                                       ("top100_c2_int64_gather", [(3, True)], 100, True)):
+        ctx.order_by(cols, keys, limit=limit, gather=gather)
+        ows = ctx._last_ws
+        l0 = ctx.launch_count()
+        ctx.order_by(cols, keys, limit=limit, gather=gather, workspace=ows)
+        nl = ctx.launch_count() - l0
+
+        def sort():
+            ctx.order_by(cols, keys, limit=limit, gather=gather, workspace=ows)
+        ms = time_steps(torch, ctx.stream, sort, max(2, steps // 2), 2, lambda: None) / max(2, steps // 2)
+        ctx.sync()
+        out[label] = dict(rows=n, keys=[[c, "desc" if d else "asc"] for c, d in keys], limit=limit, gathered_columns=4 if gather else 0,
+                          ms=ms, rows_per_s=n / ms * 1e3, launches=nl)
+    del cols
     torch.cuda.empty_cache()
     t3 = datagen.make_config(3)
     p3 = plans.plan_c3(t3)

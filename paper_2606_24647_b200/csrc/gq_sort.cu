@@ -58,14 +58,63 @@ __global__ void gq_k_sort_iota(u32* idx, u32 n, u32* d_n) {
   if (blockIdx.x == 0 && threadIdx.x == 0) *d_n = n;
 }
 
-__global__ void gq_k_sort_keys(const void* col, int dtype, int bytes, int desc, const u32* idx, const u32* d_n, u64* keys) {
+// ---- passes that would move nothing are skipped ON THE DEVICE. While the sortable keys of a column are built, the OR of
+// (key xor first key) is collected in the control block (one word per sort column; id GQ_SORT_ROWID = the row-number
+// "column" of the TopN path): a byte of that mask is zero iff all keys agree in that byte, and then the pass over it is
+// the identity. The host still enqueues every pass (it never learns the mask); histogram, scan and scatter of a skipped
+// pass return at once, and since a skipped pass does not swap the two buffers, every kernel derives WHICH buffer holds
+// the data from the masks: parity of the number of non-skipped passes so far. (An int64 price column below 2^24: 3
+// passes instead of 8.)
+#define GQ_SORT_ROWID 32
+#define GQ_SORT_CTL_BYTES 512
+struct GqSortBufs { u64* k[2]; u32* i[2]; const u32* ctl; };
+__device__ __forceinline__ u64 gq_sort_mask(const u32* ctl, int id) { return ((volatile const u64*)ctl)[16 + id]; }
+__device__ __forceinline__ u32 gq_sort_live_bytes(u64 m, int below) {      // parity of the non-zero bytes among bytes [0, below)
+  u32 p = 0;
+  for (int b = 0; b < below; ++b) p ^= ((m >> (8 * b)) & 255ULL) != 0ULL;
+  return p;
+}
+// -> buffer that holds the data when pass `pass` (0..8) of column `id` starts; *live = that pass moves something. All
+// threads of the CTA call it (one shared-memory broadcast).
+__device__ __forceinline__ u32 gq_sort_where(const u32* ctl, int id, int pass, bool* live) {
+  __shared__ u32 sh[2];
+  if (threadIdx.x == 0) {
+    u32 par = 0;
+    for (int c = id + 1; c <= GQ_SORT_ROWID; ++c) par ^= gq_sort_live_bytes(gq_sort_mask(ctl, c), 8);   // columns done before this one
+    const u64 m = id >= 0 ? gq_sort_mask(ctl, id) : 0ULL;
+    par ^= gq_sort_live_bytes(m, pass);
+    sh[0] = par;
+    sh[1] = pass < 8 && ((m >> (8 * pass)) & 255ULL) != 0ULL;
+  }
+  __syncthreads();
+  *live = sh[1] != 0;
+  return sh[0];
+}
+__global__ void gq_k_sort_keys(const void* col, int dtype, int bytes, int desc, GqSortBufs B, const u32* d_n, int id) {
+  bool live;
+  const u32 par = gq_sort_where(B.ctl, id, 0, &live);
+  const u32* idx = B.i[par];
+  u64* keys = B.k[par];
   const u32 n = gq_sort_n(d_n);
-  for (u32 i = blockIdx.x * blockDim.x + threadIdx.x; i < n; i += gridDim.x * blockDim.x)
-    keys[i] = col ? gq_sort_image(gq_sort_load(col, dtype, (i64)idx[i]), bytes, desc) : (u64)idx[i];   // col == null: the row index itself
+  if (n == 0) return;
+  const u64 ref = col ? gq_sort_image(gq_sort_load(col, dtype, (i64)idx[0]), bytes, desc) : (u64)idx[0];
+  u64 diff = 0;
+  for (u32 i = blockIdx.x * blockDim.x + threadIdx.x; i < n; i += gridDim.x * blockDim.x) {
+    const u64 k = col ? gq_sort_image(gq_sort_load(col, dtype, (i64)idx[i]), bytes, desc) : (u64)idx[i];   // col == null: the row index itself
+    keys[i] = k;
+    diff |= k ^ ref;
+  }
+  for (int o = 16; o > 0; o >>= 1) diff |= __shfl_xor_sync(0xffffffffu, diff, o);
+  if ((threadIdx.x & 31) == 0 && diff) atomicOr((u64*)B.ctl + 16 + id, diff);
 }
 
-__global__ void __launch_bounds__(GQ_SORT_THREADS) gq_k_sort_hist(const u64* keys, const u32* d_n, int shift, u32* hist) {
+__global__ void __launch_bounds__(GQ_SORT_THREADS) gq_k_sort_hist(GqSortBufs B, const u32* d_n, int id, int pass, u32* hist) {
   __shared__ u32 h[256];
+  bool live;
+  const u32 par = gq_sort_where(B.ctl, id, pass, &live);
+  if (!live) return;
+  const u64* keys = B.k[par];
+  const int shift = 8 * pass;
   h[threadIdx.x] = 0;
   __syncthreads();
   u32 lo, hi;
@@ -99,9 +148,10 @@ __device__ __forceinline__ u32 gq_block_scan_1024(u32 v, u32* wsum /* [33] share
 // exclusive scan of hist in [digit][CTA] order, in place; one CTA of 1024 threads walks it in chunks of 4096 counters,
 // four consecutive counters per thread (coalesced 16-byte accesses; the first version gave every thread its own
 // contiguous share: strided accesses and a 148-step serial loop, 153 us per pass for 592 CTAs)
-__global__ void __launch_bounds__(1024) gq_k_sort_scan(u32* hist, int total) {
+__global__ void __launch_bounds__(1024) gq_k_sort_scan(u32* hist, int total, const u32* ctl = nullptr, int id = 0, int pass = 0) {
   __shared__ u32 wsum[33];
   const int t = threadIdx.x;
+  if (ctl) { bool live; gq_sort_where(ctl, id, pass, &live); if (!live) return; }   // a skipped pass of the sort
   u32 carry = 0;
   for (int base = 0; base < total; base += 4096) {
     const int i = base + 4 * t;
@@ -126,8 +176,7 @@ __global__ void __launch_bounds__(1024) gq_k_sort_scan(u32* hist, int total) {
 // 60 M pairs; this one 460 us.
 #define GQ_SS_ITEMS 8
 #define GQ_SS_TILE (GQ_SORT_THREADS * GQ_SS_ITEMS)
-__global__ void __launch_bounds__(GQ_SORT_THREADS, 4) gq_k_sort_scatter_staged(const u64* kin, const u32* iin, u64* kout, u32* iout, const u32* d_n,
-                                                                              int shift, const u32* hist) {
+__global__ void __launch_bounds__(GQ_SORT_THREADS, 4) gq_k_sort_scatter_staged(GqSortBufs B, const u32* d_n, int id, int pass, const u32* hist) {
   __shared__ u32 cur[256];
   __shared__ unsigned short wc[GQ_SORT_WARPS][256];
   __shared__ unsigned short toff[256];
@@ -135,6 +184,12 @@ __global__ void __launch_bounds__(GQ_SORT_THREADS, 4) gq_k_sort_scatter_staged(c
   __shared__ u32 gpos[GQ_SS_TILE];
   __shared__ __align__(16) u64 stage[GQ_SS_TILE];
   const int t = threadIdx.x, lane = t & 31, warp = t >> 5;
+  bool live;
+  const u32 par = gq_sort_where(B.ctl, id, pass, &live);
+  if (!live) return;
+  const u64* kin = B.k[par]; const u32* iin = B.i[par];
+  u64* kout = B.k[par ^ 1]; u32* iout = B.i[par ^ 1];
+  const int shift = 8 * pass;
   cur[t] = hist[t * gridDim.x + blockIdx.x];
   u32 lo, hi;
   gq_sort_range(gq_sort_n(d_n), &lo, &hi);
@@ -299,13 +354,15 @@ __global__ void __launch_bounds__(256) gq_k_sel_compact(const __grid_constant__ 
 }
 
 struct GqEmitParams {
-  const u32* idx; const u32* d_n; u64 limit; i64* out_index;
+  const u32* idx[2]; const u32* ctl; const u32* d_n; u64 limit; i64* out_index;
   int ncols; const void* col[GQ_MAX_COLS]; void* out[GQ_MAX_COLS]; int dtype[GQ_MAX_COLS];
 };
 __global__ void gq_k_sort_emit(const __grid_constant__ GqEmitParams P) {
   const u64 n = min((u64)gq_sort_n(P.d_n), P.limit);
+  bool live;
+  const u32* idx = P.idx[gq_sort_where(P.ctl, -1, 0, &live)];       // the buffer the last non-skipped pass wrote
   for (u64 i = blockIdx.x * (u64)blockDim.x + threadIdx.x; i < n; i += (u64)gridDim.x * blockDim.x) {
-    const i64 r = (i64)P.idx[i];
+    const i64 r = (i64)idx[i];
     if (P.out_index) P.out_index[i] = r;
     for (int c = 0; c < P.ncols; ++c) {
       if (!P.out[c]) continue;
@@ -329,7 +386,7 @@ static GqSortLayout gq_sort_layout(i64 nrows, int num_sms) {
   L.hist = off; off += al((size_t)256 * 1024 * 4);
   L.sel1 = off; off += al(GQ_SEL_BINS * 4);
   L.sel2 = off; off += al(GQ_SEL_BINS * 4);
-  L.ctl = off; off += 256;
+  L.ctl = off; off += GQ_SORT_CTL_BYTES;
   L.total = off;
   return L;
 }
@@ -346,23 +403,28 @@ cudaError_t gq_launch_order_by(cudaStream_t s, int num_sms, const gq_batch* in, 
   u32* hist = (u32*)(ws + L.hist);
   u32* ctl = (u32*)(ws + L.ctl);
   u32* d_n = ctl + 8;
-  int nl = 0, cur = 0;
+  int nl = 0;
+  GqSortBufs B;
+  B.k[0] = kbuf[0]; B.k[1] = kbuf[1]; B.i[0] = ibuf[0]; B.i[1] = ibuf[1]; B.ctl = ctl;
   const int gs = std::max(1, std::min<int>(num_sms * 8, (int)((n + 255) / 256)));
   auto dtype_bytes = [](int t) { return t == GQ_I8 ? 1 : t == GQ_I32 ? 4 : 8; };
   const bool topn = nkeys > 0 && lim * 8 < (u64)n && n >= (1u << 16);
   // TopN sorts its few candidates (how many is known on the device only) with a small grid: the scan and the launches,
   // not the data, are what its passes cost. (Any grid is correct; many tied candidates just take longer.)
   const int nb = topn ? std::min(nblk, 16) : nblk;
-  auto passes = [&](int bytes) {                     // LSD passes over the low `bytes` bytes of kbuf[cur]
+  auto passes = [&](int id, int bytes) {             // LSD passes over the low `bytes` bytes of sort column `id`'s keys
     for (int b = 0; b < bytes; ++b) {
-      gq_k_sort_hist<<<nb, GQ_SORT_THREADS, 0, s>>>(kbuf[cur], d_n, 8 * b, hist);
-      gq_k_sort_scan<<<1, 1024, 0, s>>>(hist, 256 * nb);
-      gq_k_sort_scatter_staged<<<nb, GQ_SORT_THREADS, 0, s>>>(kbuf[cur], ibuf[cur], kbuf[cur ^ 1], ibuf[cur ^ 1], d_n, 8 * b, hist);
-      cur ^= 1;
+      gq_k_sort_hist<<<nb, GQ_SORT_THREADS, 0, s>>>(B, d_n, id, b, hist);
+      gq_k_sort_scan<<<1, 1024, 0, s>>>(hist, 256 * nb, ctl, id, b);
+      gq_k_sort_scatter_staged<<<nb, GQ_SORT_THREADS, 0, s>>>(B, d_n, id, b, hist);
       nl += 3;
     }
   };
   cudaError_t e = cudaSuccess;
+  if (!topn) {
+    e = cudaMemsetAsync(ctl, 0, GQ_SORT_CTL_BYTES, s);          // the control words (key masks of the pass skipping)
+    if (e != cudaSuccess) return e;
+  }
   if (topn) {
     e = cudaMemsetAsync(ws + L.sel1, 0, L.total - L.sel1, s);   // both histograms and the control words
     if (e != cudaSuccess) return e;
@@ -381,21 +443,21 @@ cudaError_t gq_launch_order_by(cudaStream_t s, int num_sms, const gq_batch* in, 
     e = cudaMemcpyAsync(d_n, ctl + 2, 4, cudaMemcpyDeviceToDevice, s);
     if (e != cudaSuccess) return e;
     // candidates were appended in any order: sort them by row index first (the least significant "key" of a stable sort)
-    gq_k_sort_keys<<<gs, 256, 0, s>>>(nullptr, 0, 4, 0, ibuf[0], d_n, kbuf[0]);
+    gq_k_sort_keys<<<gs, 256, 0, s>>>(nullptr, 0, 4, 0, B, d_n, GQ_SORT_ROWID);
     ++nl;
-    passes(4);
+    passes(GQ_SORT_ROWID, 4);
   } else {
     gq_k_sort_iota<<<gs, 256, 0, s>>>(ibuf[0], n, d_n);
     ++nl;
   }
   for (int k = nkeys - 1; k >= 0; --k) {
     const gq_column& c = in->cols[keys[k].col];
-    gq_k_sort_keys<<<gs, 256, 0, s>>>(c.data, (int)c.dtype, dtype_bytes((int)c.dtype), keys[k].descending ? 1 : 0, ibuf[cur], d_n, kbuf[cur]);
+    gq_k_sort_keys<<<gs, 256, 0, s>>>(c.data, (int)c.dtype, dtype_bytes((int)c.dtype), keys[k].descending ? 1 : 0, B, d_n, k);
     ++nl;
-    passes(dtype_bytes((int)c.dtype));
+    passes(k, dtype_bytes((int)c.dtype));
   }
   GqEmitParams ep;
-  ep.idx = ibuf[cur]; ep.d_n = d_n; ep.limit = lim; ep.out_index = out_index; ep.ncols = in->ncols;
+  ep.idx[0] = ibuf[0]; ep.idx[1] = ibuf[1]; ep.ctl = ctl; ep.d_n = d_n; ep.limit = lim; ep.out_index = out_index; ep.ncols = in->ncols;
   for (int c = 0; c < in->ncols; ++c) { ep.col[c] = in->cols[c].data; ep.out[c] = out_cols ? out_cols[c] : nullptr; ep.dtype[c] = (int)in->cols[c].dtype; }
   const int ge = std::max(1, std::min<int>(num_sms * 8, (int)((lim + 255) / 256)));
   gq_k_sort_emit<<<ge, 256, 0, s>>>(ep);
@@ -420,7 +482,7 @@ cudaError_t gq_launch_order_by(cudaStream_t s, int num_sms, const gq_batch* in, 
 #define GQ_SORT_AL256(v) ((((size_t)(v)) + 255) / 256 * 256)
 #define GQ_SORT_STATIC_BYTES                                                                                        \
   (2 * GQ_SORT_AL256((size_t)GQ_ORDER_BY_STATIC_MAX_ROWS * 8) + 2 * GQ_SORT_AL256((size_t)GQ_ORDER_BY_STATIC_MAX_ROWS * 4) + \
-   GQ_SORT_AL256((size_t)256 * 1024 * 4) + 2 * GQ_SORT_AL256(GQ_SEL_BINS * 4) + 256)
+   GQ_SORT_AL256((size_t)256 * 1024 * 4) + 2 * GQ_SORT_AL256(GQ_SEL_BINS * 4) + GQ_SORT_CTL_BYTES)
 static __device__ __align__(256) unsigned char gq_sort_static_scratch[GQ_SORT_STATIC_BYTES];
 
 #include <mutex>

@@ -110,3 +110,33 @@ def test_order_by_errors(ctx):
         ctx.order_by(cols, [(3, False)])
     index, outs = ctx.order_by(gqrun.dev([np.zeros(0, np.int64)]), [(0, False)])
     assert index.numel() == 0
+
+
+def test_passes_over_constant_bytes_are_skipped_on_the_device(ctx):
+    # a radix pass over a byte in which all keys agree is skipped by the kernels themselves, and which of the two buffers
+    # holds the data is derived from the keys' bit masks: key columns with 0, 1, 2, 3 and 8 live bytes, in every order,
+    # so that the number of executed passes is odd and even, also on the TopN path and in the static-scratch entry point
+    import torch
+    import gqrun
+    rng = np.random.default_rng(123)
+    n = 150_001
+    const = np.full(n, -12345, np.int64)                                     # no live byte: nothing moves
+    one = rng.integers(0, 200, n).astype(np.int64)                           # 1 live byte
+    two = (2**45 + rng.integers(0, 60_000, n)).astype(np.int64)              # 2 live bytes below a constant prefix
+    three = rng.integers(0, 2**24, n).astype(np.int32)                       # 3 of 4
+    full = rng.integers(-2**63, 2**63 - 1, n).astype(np.int64)               # all 8
+    mid = ((rng.integers(0, 256, n).astype(np.int64) << 24) + 7)             # one live byte in the middle
+    cols = [const, one, two, three, full, mid]
+    for keys in ([(0, False)], [(1, True)], [(2, False)], [(3, True)], [(4, False)], [(5, False)],
+                 [(1, False), (2, True)], [(2, True), (1, False), (0, True)], [(5, True), (3, False)], [(3, False), (5, True), (1, True)],
+                 [(0, True), (4, True)], [(1, False), (5, False), (2, False), (3, False)]):
+        check(ctx, cols, keys)
+        check(ctx, cols, keys, limit=50)                                     # TopN path (n >= 2^16, limit * 8 < n)
+    small = [c[:100_000] for c in cols]
+    dcols = gqrun.dev(small)
+    for keys in ([(0, False)], [(1, True), (5, False)], [(2, False), (3, True), (1, False)]):
+        exp = oracle.order_by(small, keys, 0)
+        index = torch.empty(100_000, dtype=torch.int64, device="cuda")
+        ctx.order_by_static(dcols, keys, 0, index)
+        ctx.sync()
+        assert np.array_equal(index.cpu().numpy(), exp.cols[0])
