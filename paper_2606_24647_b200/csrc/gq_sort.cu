@@ -119,7 +119,13 @@ __global__ void __launch_bounds__(GQ_SORT_THREADS) gq_k_sort_hist(GqSortBufs B, 
   __syncthreads();
   u32 lo, hi;
   gq_sort_range(gq_sort_n(d_n), &lo, &hi);
-  for (u32 i = lo + threadIdx.x; i < hi; i += GQ_SORT_THREADS) atomicAdd(&h[(keys[i] >> shift) & 255], 1u);
+  for (u32 base = lo; base < hi; base += GQ_SORT_TILE) {             // eight loads per thread in flight, then eight adds
+    u64 k[GQ_SORT_ITEMS];
+#pragma unroll
+    for (int j = 0; j < GQ_SORT_ITEMS; ++j) { const u32 i = base + (u32)j * GQ_SORT_THREADS + threadIdx.x; k[j] = i < hi ? keys[i] : 0ULL; }
+#pragma unroll
+    for (int j = 0; j < GQ_SORT_ITEMS; ++j) if (base + (u32)j * GQ_SORT_THREADS + threadIdx.x < hi) atomicAdd(&h[(k[j] >> shift) & 255], 1u);
+  }
   __syncthreads();
   hist[threadIdx.x * gridDim.x + blockIdx.x] = h[threadIdx.x];      // [digit][CTA]
 }
@@ -357,18 +363,40 @@ struct GqEmitParams {
   const u32* idx[2]; const u32* ctl; const u32* d_n; u64 limit; i64* out_index;
   int ncols; const void* col[GQ_MAX_COLS]; void* out[GQ_MAX_COLS]; int dtype[GQ_MAX_COLS];
 };
+// Four output rows per thread: the four row numbers are loaded first, then, column by column, four random reads are in
+// flight per thread (one dependent load after the other left the gather at half of the DRAM random-sector rate).
 __global__ void gq_k_sort_emit(const __grid_constant__ GqEmitParams P) {
   const u64 n = min((u64)gq_sort_n(P.d_n), P.limit);
   bool live;
   const u32* idx = P.idx[gq_sort_where(P.ctl, -1, 0, &live)];       // the buffer the last non-skipped pass wrote
-  for (u64 i = blockIdx.x * (u64)blockDim.x + threadIdx.x; i < n; i += (u64)gridDim.x * blockDim.x) {
-    const i64 r = (i64)idx[i];
-    if (P.out_index) P.out_index[i] = r;
+  const u64 stride = (u64)gridDim.x * blockDim.x;
+  for (u64 i0 = blockIdx.x * (u64)blockDim.x + threadIdx.x; i0 < n; i0 += 4 * stride) {
+    i64 r[4];
+#pragma unroll
+    for (int u = 0; u < 4; ++u) { const u64 i = i0 + u * stride; r[u] = i < n ? (i64)idx[i] : 0; }
+    if (P.out_index) {
+#pragma unroll
+      for (int u = 0; u < 4; ++u) { const u64 i = i0 + u * stride; if (i < n) P.out_index[i] = r[u]; }
+    }
     for (int c = 0; c < P.ncols; ++c) {
       if (!P.out[c]) continue;
-      if (P.dtype[c] == GQ_I8) ((signed char*)P.out[c])[i] = ((const signed char*)P.col[c])[r];
-      else if (P.dtype[c] == GQ_I32) ((int*)P.out[c])[i] = ((const int*)P.col[c])[r];
-      else ((i64*)P.out[c])[i] = ((const i64*)P.col[c])[r];
+      i64 v[4];
+      if (P.dtype[c] == GQ_I8) {
+#pragma unroll
+        for (int u = 0; u < 4; ++u) v[u] = (i64)((const signed char*)P.col[c])[r[u]];
+#pragma unroll
+        for (int u = 0; u < 4; ++u) { const u64 i = i0 + u * stride; if (i < n) ((signed char*)P.out[c])[i] = (signed char)v[u]; }
+      } else if (P.dtype[c] == GQ_I32) {
+#pragma unroll
+        for (int u = 0; u < 4; ++u) v[u] = (i64)((const int*)P.col[c])[r[u]];
+#pragma unroll
+        for (int u = 0; u < 4; ++u) { const u64 i = i0 + u * stride; if (i < n) ((int*)P.out[c])[i] = (int)v[u]; }
+      } else {
+#pragma unroll
+        for (int u = 0; u < 4; ++u) v[u] = ((const i64*)P.col[c])[r[u]];
+#pragma unroll
+        for (int u = 0; u < 4; ++u) { const u64 i = i0 + u * stride; if (i < n) ((i64*)P.out[c])[i] = v[u]; }
+      }
     }
   }
 }
