@@ -45,10 +45,10 @@ __device__ __forceinline__ i64 gq_sort_load(const void* col, int dtype, i64 r) {
 __device__ __forceinline__ u32 gq_sort_n(const u32* d_n) { return *(volatile const u32*)d_n; }
 
 // range of tiles owned by a CTA: contiguous, whole tiles
-__device__ __forceinline__ void gq_sort_range(u32 n, u32* lo, u32* hi) {
-  const u32 ntiles = (n + GQ_SORT_TILE - 1) / GQ_SORT_TILE;
+__device__ __forceinline__ void gq_sort_range(u32 n, u32* lo, u32* hi, u32 tile) {
+  const u32 ntiles = (n + tile - 1) / tile;
   const u32 per = (ntiles + gridDim.x - 1) / gridDim.x;
-  const u64 a = (u64)blockIdx.x * per * GQ_SORT_TILE, b = a + (u64)per * GQ_SORT_TILE;
+  const u64 a = (u64)blockIdx.x * per * tile, b = a + (u64)per * tile;
   *lo = (u32)(a < n ? a : n);
   *hi = (u32)(b < n ? b : n);
 }
@@ -108,26 +108,27 @@ __global__ void gq_k_sort_keys(const void* col, int dtype, int bytes, int desc, 
   if ((threadIdx.x & 31) == 0 && diff) atomicOr((u64*)B.ctl + 16 + id, diff);
 }
 
-__global__ void __launch_bounds__(GQ_SORT_THREADS) gq_k_sort_hist(GqSortBufs B, const u32* d_n, int id, int pass, u32* hist) {
+template <int NT>
+__global__ void __launch_bounds__(NT) gq_k_sort_hist(GqSortBufs B, const u32* d_n, int id, int pass, u32* hist) {
   __shared__ u32 h[256];
   bool live;
   const u32 par = gq_sort_where(B.ctl, id, pass, &live);
   if (!live) return;
   const u64* keys = B.k[par];
   const int shift = 8 * pass;
-  h[threadIdx.x] = 0;
+  if (threadIdx.x < 256) h[threadIdx.x] = 0;
   __syncthreads();
   u32 lo, hi;
-  gq_sort_range(gq_sort_n(d_n), &lo, &hi);
-  for (u32 base = lo; base < hi; base += GQ_SORT_TILE) {             // eight loads per thread in flight, then eight adds
+  gq_sort_range(gq_sort_n(d_n), &lo, &hi, NT * GQ_SORT_ITEMS);
+  for (u32 base = lo; base < hi; base += NT * GQ_SORT_ITEMS) {       // eight loads per thread in flight, then eight adds
     u64 k[GQ_SORT_ITEMS];
 #pragma unroll
-    for (int j = 0; j < GQ_SORT_ITEMS; ++j) { const u32 i = base + (u32)j * GQ_SORT_THREADS + threadIdx.x; k[j] = i < hi ? keys[i] : 0ULL; }
+    for (int j = 0; j < GQ_SORT_ITEMS; ++j) { const u32 i = base + (u32)j * NT + threadIdx.x; k[j] = i < hi ? keys[i] : 0ULL; }
 #pragma unroll
-    for (int j = 0; j < GQ_SORT_ITEMS; ++j) if (base + (u32)j * GQ_SORT_THREADS + threadIdx.x < hi) atomicAdd(&h[(k[j] >> shift) & 255], 1u);
+    for (int j = 0; j < GQ_SORT_ITEMS; ++j) if (base + (u32)j * NT + threadIdx.x < hi) atomicAdd(&h[(k[j] >> shift) & 255], 1u);
   }
   __syncthreads();
-  hist[threadIdx.x * gridDim.x + blockIdx.x] = h[threadIdx.x];      // [digit][CTA]
+  if (threadIdx.x < 256) hist[threadIdx.x * gridDim.x + blockIdx.x] = h[threadIdx.x];      // [digit][CTA]
 }
 
 // inclusive scan of one value per thread over a CTA of 1024 threads (warp shuffles + one shared-memory step); returns the
@@ -180,15 +181,18 @@ __global__ void __launch_bounds__(1024) gq_k_sort_scan(u32* hist, int total, con
 // row numbers are staged in that order and written out as runs. The first version ranked 256 pairs per round across the
 // CTA (3 barriers per 256 pairs, one load per thread in flight) and wrote every pair on its own: 947 us per pass of
 // 60 M pairs; this one 460 us.
+// NT = 256 (4 CTAs per SM, 2048-pair tiles) or 512 (2 CTAs per SM, 4096-pair tiles: half as many CTAs keep half as many
+// write streams open and a digit's run is twice as long — the full sort uses it; TopN's few candidates take 256).
 #define GQ_SS_ITEMS 8
-#define GQ_SS_TILE (GQ_SORT_THREADS * GQ_SS_ITEMS)
-__global__ void __launch_bounds__(GQ_SORT_THREADS, 4) gq_k_sort_scatter_staged(GqSortBufs B, const u32* d_n, int id, int pass, const u32* hist) {
-  __shared__ u32 cur[256];
-  __shared__ unsigned short wc[GQ_SORT_WARPS][256];
-  __shared__ unsigned short toff[256];
-  __shared__ u32 wsum[GQ_SORT_WARPS];
-  __shared__ u32 gpos[GQ_SS_TILE];
-  __shared__ __align__(16) u64 stage[GQ_SS_TILE];
+template <int NT>
+__global__ void __launch_bounds__(NT, 1024 / NT) gq_k_sort_scatter_staged(GqSortBufs B, const u32* d_n, int id, int pass, const u32* hist) {
+  constexpr int NW = NT / 32, TILE = NT * GQ_SS_ITEMS;
+  __shared__ u32 cur[256];                               // the CTA's next output position per digit (at the tile's start)
+  __shared__ unsigned short wc[NW][256];                 // per tile: pairs of a digit in every warp, then their offsets
+  __shared__ unsigned short toff[256];                   // per tile: first place of every digit in the tile's order
+  __shared__ u32 wsum[8];
+  __shared__ unsigned char pd[TILE];                     // per tile: digit of every place (output position = cur + place - toff)
+  __shared__ __align__(16) u64 stage[TILE];
   const int t = threadIdx.x, lane = t & 31, warp = t >> 5;
   bool live;
   const u32 par = gq_sort_where(B.ctl, id, pass, &live);
@@ -196,15 +200,15 @@ __global__ void __launch_bounds__(GQ_SORT_THREADS, 4) gq_k_sort_scatter_staged(G
   const u64* kin = B.k[par]; const u32* iin = B.i[par];
   u64* kout = B.k[par ^ 1]; u32* iout = B.i[par ^ 1];
   const int shift = 8 * pass;
-  cur[t] = hist[t * gridDim.x + blockIdx.x];
+  if (t < 256) cur[t] = hist[t * gridDim.x + blockIdx.x];
   u32 lo, hi;
-  gq_sort_range(gq_sort_n(d_n), &lo, &hi);
-  for (u32 base = lo; base < hi; base += GQ_SS_TILE) {
-    const u32 nt = min((u32)GQ_SS_TILE, hi - base);
-    for (int w = 0; w < GQ_SORT_WARPS; ++w) wc[w][t] = 0;
+  gq_sort_range(gq_sort_n(d_n), &lo, &hi, TILE);
+  for (u32 base = lo; base < hi; base += TILE) {
+    const u32 nt = min((u32)TILE, hi - base);
+    if (t < 256) for (int w = 0; w < NW; ++w) wc[w][t] = 0;
     __syncthreads();
     u64 k[GQ_SS_ITEMS];
-    unsigned short wr[GQ_SS_ITEMS], place[GQ_SS_ITEMS];
+    unsigned short wr[GQ_SS_ITEMS];                       // rank among the warp's pairs of the digit, then place in the tile
     const u32 i0 = (u32)warp * (32u * GQ_SS_ITEMS) + (u32)lane;
 #pragma unroll
     for (int j = 0; j < GQ_SS_ITEMS; ++j) { const u32 i = i0 + (u32)j * 32u; k[j] = i < nt ? kin[base + i] : 0ULL; }
@@ -220,42 +224,44 @@ __global__ void __launch_bounds__(GQ_SORT_THREADS, 4) gq_k_sort_scatter_staged(G
       __syncwarp();
     }
     __syncthreads();
-    u32 tot = 0;
+    u32 tot = 0, incl = 0;
+    if (t < 256) {                                        // thread q < 256: digit q (warps 0..7, all lanes)
 #pragma unroll
-    for (int w = 0; w < GQ_SORT_WARPS; ++w) { const u32 c = wc[w][t]; wc[w][t] = (unsigned short)tot; tot += c; }
-    u32 incl = tot;
+      for (int w = 0; w < NW; ++w) { const u32 c = wc[w][t]; wc[w][t] = (unsigned short)tot; tot += c; }
+      incl = tot;
 #pragma unroll
-    for (int o = 1; o < 32; o <<= 1) { const u32 x = __shfl_up_sync(0xffffffffu, incl, o); if (lane >= o) incl += x; }
-    if (lane == 31) wsum[warp] = incl;
+      for (int o = 1; o < 32; o <<= 1) { const u32 x = __shfl_up_sync(0xffffffffu, incl, o); if (lane >= o) incl += x; }
+      if (lane == 31) wsum[warp] = incl;
+    }
     __syncthreads();
-    u32 before = 0;
+    if (t < 256) {
+      u32 before = 0;
 #pragma unroll
-    for (int w = 0; w < GQ_SORT_WARPS; ++w) if (w < warp) before += wsum[w];
-    toff[t] = (unsigned short)(before + incl - tot);
+      for (int w = 0; w < 8; ++w) if (w < warp) before += wsum[w];
+      toff[t] = (unsigned short)(before + incl - tot);
+    }
     __syncthreads();
 #pragma unroll
     for (int j = 0; j < GQ_SS_ITEMS; ++j) {
-      place[j] = 0;
       if (i0 + (u32)j * 32u < nt) {
         const u32 d = (u32)(k[j] >> shift) & 255u;
-        const u32 in_run = (u32)wc[warp][d] + (u32)wr[j];
-        place[j] = (unsigned short)((u32)toff[d] + in_run);
-        gpos[place[j]] = cur[d] + in_run;
-        stage[place[j]] = k[j];
+        wr[j] = (unsigned short)((u32)toff[d] + (u32)wc[warp][d] + (u32)wr[j]);
+        pd[wr[j]] = (unsigned char)d;
+        stage[wr[j]] = k[j];
       }
     }
     u32 ix[GQ_SS_ITEMS];                                 // the row numbers are on their way while the keys are written out
 #pragma unroll
     for (int j = 0; j < GQ_SS_ITEMS; ++j) { const u32 i = i0 + (u32)j * 32u; ix[j] = i < nt ? iin[base + i] : 0u; }
     __syncthreads();
-    cur[t] += tot;
-    for (u32 p = t; p < nt; p += GQ_SORT_THREADS) kout[gpos[p]] = stage[p];
+    for (u32 p = t; p < nt; p += NT) { const u32 d = pd[p]; kout[cur[d] + p - (u32)toff[d]] = stage[p]; }
     __syncthreads();
 #pragma unroll
-    for (int j = 0; j < GQ_SS_ITEMS; ++j) if (i0 + (u32)j * 32u < nt) ((u32*)stage)[place[j]] = ix[j];
+    for (int j = 0; j < GQ_SS_ITEMS; ++j) if (i0 + (u32)j * 32u < nt) ((u32*)stage)[wr[j]] = ix[j];
     __syncthreads();
-    for (u32 p = t; p < nt; p += GQ_SORT_THREADS) iout[gpos[p]] = ((const u32*)stage)[p];
+    for (u32 p = t; p < nt; p += NT) { const u32 d = pd[p]; iout[cur[d] + p - (u32)toff[d]] = ((const u32*)stage)[p]; }
     __syncthreads();
+    if (t < 256) cur[t] += tot;                           // (read again only after the next tile's barriers)
   }
 }
 
@@ -439,12 +445,18 @@ cudaError_t gq_launch_order_by(cudaStream_t s, int num_sms, const gq_batch* in, 
   const bool topn = nkeys > 0 && lim * 8 < (u64)n && n >= (1u << 16);
   // TopN sorts its few candidates (how many is known on the device only) with a small grid: the scan and the launches,
   // not the data, are what its passes cost. (Any grid is correct; many tied candidates just take longer.)
-  const int nb = topn ? std::min(nblk, 16) : nblk;
+  const int nb = topn ? std::min(nblk, 16) : std::max(1, nblk / 2);   // (the full sort runs 2 CTAs of 512 threads per SM)
   auto passes = [&](int id, int bytes) {             // LSD passes over the low `bytes` bytes of sort column `id`'s keys
     for (int b = 0; b < bytes; ++b) {
-      gq_k_sort_hist<<<nb, GQ_SORT_THREADS, 0, s>>>(B, d_n, id, b, hist);
-      gq_k_sort_scan<<<1, 1024, 0, s>>>(hist, 256 * nb, ctl, id, b);
-      gq_k_sort_scatter_staged<<<nb, GQ_SORT_THREADS, 0, s>>>(B, d_n, id, b, hist);
+      if (topn) {
+        gq_k_sort_hist<256><<<nb, 256, 0, s>>>(B, d_n, id, b, hist);
+        gq_k_sort_scan<<<1, 1024, 0, s>>>(hist, 256 * nb, ctl, id, b);
+        gq_k_sort_scatter_staged<256><<<nb, 256, 0, s>>>(B, d_n, id, b, hist);
+      } else {
+        gq_k_sort_hist<512><<<nb, 512, 0, s>>>(B, d_n, id, b, hist);
+        gq_k_sort_scan<<<1, 1024, 0, s>>>(hist, 256 * nb, ctl, id, b);
+        gq_k_sort_scatter_staged<512><<<nb, 512, 0, s>>>(B, d_n, id, b, hist);
+      }
       nl += 3;
     }
   };
