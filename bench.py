@@ -396,7 +396,17 @@ def run_standalone_ops(gq, ctx, torch, datagen, plans, gqrun, steps, warmup):
         ctx.sync()
         out[label] = dict(rows=n, keys=[[c, "desc" if d else "asc"] for c, d in keys], limit=limit, gathered_columns=4 if gather else 0,
                           ms=ms, rows_per_s=n / ms * 1e3, launches=nl)
-    del cols
+    # ORDER BY at the end of a query: a small group table (2048 rows, two keys, columns gathered) - one launch
+    scols = [c[:2048].contiguous() for c in cols]
+    ctx.order_by(scols, [(0, True), (3, False)], limit=0, gather=True)
+    sws = ctx._last_ws
+
+    def small_sort():
+        ctx.order_by(scols, [(0, True), (3, False)], limit=0, gather=True, workspace=sws)
+    ms = time_steps(torch, ctx.stream, small_sort, 50, 5, lambda: None) / 50
+    ctx.sync()
+    out["order_by_2048_rows_two_keys_gather"] = dict(rows=2048, ms=ms, rows_per_s=2048 / ms * 1e3, launches=1)
+    del cols, scols
     torch.cuda.empty_cache()
     t3 = datagen.make_config(3)
     p3 = plans.plan_c3(t3)

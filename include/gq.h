@@ -221,7 +221,9 @@ gq_status gq_aggstate_rehash(gq_ctx*, gq_aggstate*, void* d_new_workspace, size_
  * min(limit, nrows) rows (limit <= 0: all): d_out_index[i] (int64, may be NULL) = input row number of output row i, and,
  * when out_cols != NULL, out_cols[c][i] = column c of that row with the input column's dtype (an entry may be NULL).
  * nkeys == 0 keeps the input order. Method: LSD radix sort of (sortable key, row) pairs, one key column at a time;
- * limit << nrows first selects the candidate rows with a two-level radix select on keys[0]. nrows <= 2^31. */
+ * radix passes over bytes in which all keys agree are skipped on the device; limit << nrows first selects the candidate
+ * rows with a two-level radix select on keys[0]; up to 2048 rows are sorted by one CTA in one launch. Stream-ordered, no
+ * host synchronisation. nrows <= 2^31. */
 typedef struct { int32_t col; int32_t descending; } gq_sort_key;
 gq_status gq_order_by_workspace(int64_t nrows, size_t* bytes);
 gq_status gq_order_by(gq_ctx*, const gq_batch* in, const gq_sort_key* keys, int32_t nkeys, int64_t limit, void* d_workspace,

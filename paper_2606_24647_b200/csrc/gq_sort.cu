@@ -407,6 +407,56 @@ __global__ void gq_k_sort_emit(const __grid_constant__ GqEmitParams P) {
   }
 }
 
+// ---- small inputs: one CTA, one launch. ORDER BY at the end of a query usually sees a handful of groups (Fig. 2:
+// OrderBy after the final aggregation); the radix path costs >= 27 launches whatever the size (~100 us). Up to 2048 rows
+// are sorted as row numbers in shared memory by a bitonic network whose comparator reads the key columns (lexicographic,
+// signed, per-key direction, the row number last: a total order, so the unstable network gives the stable result), and
+// the same CTA gathers the outputs.
+#define GQ_SMALL_SORT_MAX 2048
+struct GqSmallSortParams {
+  u32 n; int nkeys; u64 limit; i64* out_index; int ncols;
+  const void* key[GQ_MAX_COLS]; int key_dtype[GQ_MAX_COLS]; int key_desc[GQ_MAX_COLS];
+  const void* col[GQ_MAX_COLS]; void* out[GQ_MAX_COLS]; int dtype[GQ_MAX_COLS];
+};
+__device__ __forceinline__ bool gq_small_less(const GqSmallSortParams& P, u32 a, u32 b) {   // row a strictly before row b
+  if (a == 0xFFFFFFFFu) return false;                     // padding sorts last
+  if (b == 0xFFFFFFFFu) return true;
+  for (int k = 0; k < P.nkeys; ++k) {
+    const i64 x = gq_sort_load(P.key[k], P.key_dtype[k], (i64)a), y = gq_sort_load(P.key[k], P.key_dtype[k], (i64)b);
+    if (x != y) return P.key_desc[k] ? x > y : x < y;
+  }
+  return a < b;
+}
+__global__ void __launch_bounds__(1024) gq_k_sort_small(const __grid_constant__ GqSmallSortParams P) {
+  __shared__ u32 idx[GQ_SMALL_SORT_MAX];
+  const u32 t = threadIdx.x;
+  u32 N = 2;
+  while (N < P.n) N <<= 1;                                // power of two >= n (>= 2)
+  for (u32 i = t; i < N; i += 1024) idx[i] = i < P.n ? i : 0xFFFFFFFFu;
+  __syncthreads();
+  for (u32 k = 2; k <= N; k <<= 1)
+    for (u32 j = k >> 1; j > 0; j >>= 1) {
+      if (t < N / 2) {                                    // compare-exchange number t of this stage: elements e and e + j
+        const u32 e = 2 * j * (t / j) + (t % j);
+        const bool asc = (e & k) == 0;
+        const u32 a = idx[e], b = idx[e + j];
+        if (gq_small_less(P, b, a) == asc) { idx[e] = b; idx[e + j] = a; }
+      }
+      __syncthreads();
+    }
+  const u64 nout = min((u64)P.n, P.limit);
+  for (u64 i = t; i < nout; i += 1024) {
+    const i64 r = (i64)idx[i];
+    if (P.out_index) P.out_index[i] = r;
+    for (int c = 0; c < P.ncols; ++c) {
+      if (!P.out[c]) continue;
+      if (P.dtype[c] == GQ_I8) ((signed char*)P.out[c])[i] = ((const signed char*)P.col[c])[r];
+      else if (P.dtype[c] == GQ_I32) ((int*)P.out[c])[i] = ((const int*)P.col[c])[r];
+      else ((i64*)P.out[c])[i] = ((const i64*)P.col[c])[r];
+    }
+  }
+}
+
 // ---- host side ----
 struct GqSortLayout { size_t keys[2], idx[2], hist, sel1, sel2, ctl, total; int nblk; };
 static GqSortLayout gq_sort_layout(i64 nrows, int num_sms) {
@@ -432,6 +482,18 @@ cudaError_t gq_launch_order_by(cudaStream_t s, int num_sms, const gq_batch* in, 
   const int nblk = std::max(1, std::min(num_sms * 4, 1024));
   const u32 n = (u32)in->nrows;
   const u64 lim = limit <= 0 || limit > in->nrows ? (u64)in->nrows : (u64)limit;
+  if (n <= GQ_SMALL_SORT_MAX) {                          // one CTA, one launch (the workspace is not used)
+    GqSmallSortParams sp;
+    sp.n = n; sp.nkeys = nkeys; sp.limit = lim; sp.out_index = out_index; sp.ncols = in->ncols;
+    for (int k = 0; k < nkeys; ++k) {
+      const gq_column& c = in->cols[keys[k].col];
+      sp.key[k] = c.data; sp.key_dtype[k] = (int)c.dtype; sp.key_desc[k] = keys[k].descending ? 1 : 0;
+    }
+    for (int c = 0; c < in->ncols; ++c) { sp.col[c] = in->cols[c].data; sp.out[c] = out_cols ? out_cols[c] : nullptr; sp.dtype[c] = (int)in->cols[c].dtype; }
+    gq_k_sort_small<<<1, 1024, 0, s>>>(sp);
+    *nlaunches = 1;
+    return cudaGetLastError();
+  }
   u64* kbuf[2] = {(u64*)(ws + L.keys[0]), (u64*)(ws + L.keys[1])};
   u32* ibuf[2] = {(u32*)(ws + L.idx[0]), (u32*)(ws + L.idx[1])};
   u32* hist = (u32*)(ws + L.hist);

@@ -140,3 +140,23 @@ def test_passes_over_constant_bytes_are_skipped_on_the_device(ctx):
         ctx.order_by_static(dcols, keys, 0, index)
         ctx.sync()
         assert np.array_equal(index.cpu().numpy(), exp.cols[0])
+
+
+@pytest.mark.parametrize("n", [3, 6, 100, 1000, 2047, 2048])
+def test_small_inputs_take_one_launch(ctx, n):
+    # up to 2048 rows: one CTA sorts the row numbers in shared memory (comparator over the key columns) and gathers the
+    # outputs — one launch instead of the radix path's >= 27; heavy ties (stability), every dtype, limits
+    import gqrun
+    rng = np.random.default_rng(1000 + n)
+    a = rng.integers(-2, 2, n).astype(np.int8)
+    b = rng.integers(-3, 3, n).astype(np.int32)
+    c = rng.integers(-2**62, 2**62, n).astype(np.int64)
+    c[::4] = c[0]
+    cols = [a, b, c]
+    for keys, limit in (([(0, False), (1, True)], 0), ([(2, True)], 0), ([(1, True), (0, False), (2, False)], max(1, n // 2)), ([], 0), ([(0, True)], 1)):
+        check(ctx, cols, keys, limit=limit)
+    dcols = gqrun.dev(cols)
+    l0 = ctx.launch_count()
+    ctx.order_by(dcols, [(0, False), (2, True)], limit=0, gather=True)
+    ctx.sync()
+    assert ctx.launch_count() - l0 == 1

@@ -63,24 +63,37 @@ def test_static_scratch_order_by_equals_existing_path_on_consecutive_calls(ctx):
     assert np.array_equal(ref_index.cpu().numpy(), oracle.order_by(cols, keys, limit).cols[0])
 
     # warm-up pass (first use of the symbol address and of every kernel of both paths), then two measured passes back
-    # to back: device memory in use must not move, results must equal the existing path's every time
+    # to back into buffers allocated beforehand. Inside the measured window NOTHING but the static entry point runs (a
+    # torch comparison there could make torch's caching allocator take a new segment from the driver): device memory in
+    # use must not move. The results are compared with the existing path's afterwards.
     for cols, dcols, keys, limit, ref_index, ref_outs, index, outs in prepared:
         _run_static(ctx, torch, dcols, keys, limit, index, outs)
     ctx.sync()
+    results = []
+    for rep in range(2):
+        for cols, dcols, keys, limit, ref_index, ref_outs, index, outs in prepared:
+            results.append((torch.full_like(index, -1), [torch.zeros_like(o) for o in outs]))
     torch.cuda.synchronize()
     free0, _ = torch.cuda.mem_get_info()
     alloc0 = torch.cuda.memory_allocated()
+    it = iter(results)
+    nouts = []
     for rep in range(2):
         for cols, dcols, keys, limit, ref_index, ref_outs, index, outs in prepared:
-            nout = _run_static(ctx, torch, dcols, keys, limit, index, outs)
-            ctx.sync()
-            assert nout == ref_index.numel()
-            assert torch.equal(index, ref_index), f"row order differs (rows {len(cols[0])}, keys {keys}, limit {limit}, pass {rep})"
-            for j, (o, r) in enumerate(zip(outs, ref_outs)):
-                assert torch.equal(o, r), f"gathered column {j} differs (rows {len(cols[0])}, pass {rep})"
+            ridx, routs = next(it)
+            nouts.append(ctx.order_by_static(dcols, keys, limit, ridx, routs))
+    ctx.sync()
     torch.cuda.synchronize()
     assert torch.cuda.memory_allocated() == alloc0
     assert torch.cuda.mem_get_info()[0] == free0, "device memory in use changed across gq_order_by_static calls"
+    it = iter(zip(results, nouts))
+    for rep in range(2):
+        for cols, dcols, keys, limit, ref_index, ref_outs, index, outs in prepared:
+            (ridx, routs), nout = next(it)
+            assert nout == ref_index.numel()
+            assert torch.equal(ridx, ref_index), f"row order differs (rows {len(cols[0])}, keys {keys}, limit {limit}, pass {rep})"
+            for j, (o, r) in enumerate(zip(routs, ref_outs)):
+                assert torch.equal(o, r), f"gathered column {j} differs (rows {len(cols[0])}, pass {rep})"
 
     # index only / gathered columns only
     cols, dcols, keys, limit, ref_index, ref_outs, index, outs = prepared[1]
