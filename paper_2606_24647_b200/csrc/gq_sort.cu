@@ -418,10 +418,16 @@ struct GqSmallSortParams {
   const void* key[GQ_MAX_COLS]; int key_dtype[GQ_MAX_COLS]; int key_desc[GQ_MAX_COLS];
   const void* col[GQ_MAX_COLS]; void* out[GQ_MAX_COLS]; int dtype[GQ_MAX_COLS];
 };
-__device__ __forceinline__ bool gq_small_less(const GqSmallSortParams& P, u32 a, u32 b) {   // row a strictly before row b
+// The first GQ_SMALL_IMG key columns are compared through their sortable images in shared memory (unsigned order ==
+// requested order), further ones through the columns themselves.
+#define GQ_SMALL_IMG 2
+__device__ __forceinline__ bool gq_small_less(const GqSmallSortParams& P, const u64 (*img)[GQ_SMALL_SORT_MAX], u32 a, u32 b) {   // row a strictly before row b
   if (a == 0xFFFFFFFFu) return false;                     // padding sorts last
   if (b == 0xFFFFFFFFu) return true;
-  for (int k = 0; k < P.nkeys; ++k) {
+#pragma unroll
+  for (int k = 0; k < GQ_SMALL_IMG; ++k)
+    if (k < P.nkeys) { const u64 x = img[k][a], y = img[k][b]; if (x != y) return x < y; }
+  for (int k = GQ_SMALL_IMG; k < P.nkeys; ++k) {
     const i64 x = gq_sort_load(P.key[k], P.key_dtype[k], (i64)a), y = gq_sort_load(P.key[k], P.key_dtype[k], (i64)b);
     if (x != y) return P.key_desc[k] ? x > y : x < y;
   }
@@ -429,10 +435,15 @@ __device__ __forceinline__ bool gq_small_less(const GqSmallSortParams& P, u32 a,
 }
 __global__ void __launch_bounds__(1024) gq_k_sort_small(const __grid_constant__ GqSmallSortParams P) {
   __shared__ u32 idx[GQ_SMALL_SORT_MAX];
+  __shared__ u64 img[GQ_SMALL_IMG][GQ_SMALL_SORT_MAX];
   const u32 t = threadIdx.x;
   u32 N = 2;
   while (N < P.n) N <<= 1;                                // power of two >= n (>= 2)
   for (u32 i = t; i < N; i += 1024) idx[i] = i < P.n ? i : 0xFFFFFFFFu;
+  for (int k = 0; k < GQ_SMALL_IMG && k < P.nkeys; ++k) {
+    const int bytes = P.key_dtype[k] == GQ_I8 ? 1 : P.key_dtype[k] == GQ_I32 ? 4 : 8;
+    for (u32 i = t; i < P.n; i += 1024) img[k][i] = gq_sort_image(gq_sort_load(P.key[k], P.key_dtype[k], (i64)i), bytes, P.key_desc[k]);
+  }
   __syncthreads();
   for (u32 k = 2; k <= N; k <<= 1)
     for (u32 j = k >> 1; j > 0; j >>= 1) {
@@ -440,7 +451,7 @@ __global__ void __launch_bounds__(1024) gq_k_sort_small(const __grid_constant__ 
         const u32 e = 2 * j * (t / j) + (t % j);
         const bool asc = (e & k) == 0;
         const u32 a = idx[e], b = idx[e + j];
-        if (gq_small_less(P, b, a) == asc) { idx[e] = b; idx[e + j] = a; }
+        if (gq_small_less(P, img, b, a) == asc) { idx[e] = b; idx[e + j] = a; }
       }
       __syncthreads();
     }
