@@ -697,23 +697,25 @@ __device__ __forceinline__ void gq_hp_dests(const GqHpParams& P, u32 r0, u32 str
     d[j] = r0 + (u32)j * stride < hi ? (u32)(((h[j] >> 32) * (u64)(u32)P.nparts) >> 32) : 256u + (u32)lane;
 }
 // rows [lo, hi) of the calling CTA: whole tiles, contiguous, in CTA order
-__device__ __forceinline__ void gq_hp_range(u32 n, u32* lo, u32* hi) {
-  const u32 ntiles = (n + GQ_HP_TILE - 1) / GQ_HP_TILE;
+__device__ __forceinline__ void gq_hp_range(u32 n, u32* lo, u32* hi, u32 tile) {
+  const u32 ntiles = (n + tile - 1) / tile;
   const u32 per = (ntiles + gridDim.x - 1) / gridDim.x;
-  const u64 a = (u64)blockIdx.x * per * GQ_HP_TILE, b = a + (u64)per * GQ_HP_TILE;
+  const u64 a = (u64)blockIdx.x * per * tile, b = a + (u64)per * tile;
   *lo = (u32)(a < n ? a : n);
   *hi = (u32)(b < n ? b : n);
 }
-__global__ void __launch_bounds__(GQ_HP_THREADS) gq_k_hp_hist(const __grid_constant__ GqHpParams P) {
-  __shared__ u32 cnt[GQ_HP_WARPS][256];              // warp-private counters: an add only meets the adds of its own warp
+template <int NT>
+__global__ void __launch_bounds__(NT) gq_k_hp_hist(const __grid_constant__ GqHpParams P) {
+  constexpr int NW = NT / 32;
+  __shared__ u32 cnt[NW][256];                       // warp-private counters: an add only meets the adds of its own warp
   const int t = threadIdx.x, lane = t & 31, warp = t >> 5;
-  for (int w = 0; w < GQ_HP_WARPS; ++w) cnt[w][t] = 0;
+  if (t < 256) for (int w = 0; w < NW; ++w) cnt[w][t] = 0;
   __syncthreads();
   u32 lo, hi;
-  gq_hp_range(P.n, &lo, &hi);
-  for (u32 base = lo; base < hi; base += GQ_HP_TILE) {
+  gq_hp_range(P.n, &lo, &hi, NT * GQ_HP_ITEMS);
+  for (u32 base = lo; base < hi; base += NT * GQ_HP_ITEMS) {
     u32 d[GQ_HP_ITEMS];
-    gq_hp_dests(P, base + (u32)t, GQ_HP_THREADS, hi, lane, d);
+    gq_hp_dests(P, base + (u32)t, NT, hi, lane, d);
 #pragma unroll
     for (int j = 0; j < GQ_HP_ITEMS; ++j) if (d[j] < 256u) atomicAdd(&cnt[warp][d[j]], 1u);
   }
@@ -721,7 +723,7 @@ __global__ void __launch_bounds__(GQ_HP_THREADS) gq_k_hp_hist(const __grid_const
   if (t < P.nparts) {
     u32 s = 0;
 #pragma unroll
-    for (int w = 0; w < GQ_HP_WARPS; ++w) s += cnt[w][t];
+    for (int w = 0; w < NW; ++w) s += cnt[w][t];
     P.hist[(size_t)t * gridDim.x + blockIdx.x] = s;
   }
 }
@@ -743,79 +745,85 @@ __device__ __forceinline__ void gq_hp_load(const GqHpParams& P, int c, u32 base,
     for (int j = 0; j < GQ_HP_ITEMS; ++j) { const u32 i = i0 + (u32)j * 32u; v[j] = i < nt ? (u64)src[i] : 0ULL; }
   }
 }
-template <bool PEER>
-__global__ void __launch_bounds__(GQ_HP_THREADS, GQ_HP_CTAS_PER_SM) gq_k_hp_scatter(const __grid_constant__ GqHpParams P) {
-  __shared__ u32 cur[256];                             // the CTA's next output row per destination
-  __shared__ unsigned short wc[GQ_HP_WARPS][256];      // per tile: rows of a destination in every warp, then their offsets
+// NT = 256 (4 CTAs per SM, 2048-row tiles) below GQ_HP_WIDE_FROM destinations, 512 (2 CTAs per SM, 4096-row tiles: half as
+// many open write streams, runs twice as long) from there on: C2 table, 256 destinations 2.44 -> 1.72 ms, but 64
+// destinations 1.09 -> 1.17 ms.
+template <int NT, bool PEER>
+__global__ void __launch_bounds__(NT, 1024 / NT) gq_k_hp_scatter(const __grid_constant__ GqHpParams P) {
+  constexpr int NW = NT / 32, TILE = NT * GQ_HP_ITEMS;
+  __shared__ u32 cur[256];                             // the CTA's next output row per destination (at the tile's start)
+  __shared__ unsigned short wc[NW][256];               // per tile: rows of a destination in every warp, then their offsets
   __shared__ unsigned short toff[256];                 // per tile: first place of every destination in the tile's order
-  __shared__ u32 wsum[GQ_HP_WARPS];
-  __shared__ u32 gpos[GQ_HP_TILE];                     // per tile: output row of every place
-  __shared__ __align__(16) unsigned char stage[GQ_HP_TILE * 8];
-  __shared__ unsigned char pdst[PEER ? GQ_HP_TILE : 1];   // peer variant: destination of every place
+  __shared__ u32 wsum[8];
+  __shared__ unsigned char pd[TILE];                   // per tile: destination of every place (output row = cur + place - toff)
+  constexpr bool GPOS = NT == 256;                     // 2048-row tiles also keep the output row of every place (one lookup per
+  __shared__ u32 gpos[GPOS ? TILE : 1];                //  element instead of three; 4096-row tiles have no room for it)
+  __shared__ __align__(16) unsigned char stage[TILE * 8];
   const int t = threadIdx.x, lane = t & 31, warp = t >> 5;
-  cur[t] = t < P.nparts ? P.hist[(size_t)t * gridDim.x + blockIdx.x] : 0u;
-  if (PEER) {   // cursor = row inside the DESTINATION's buffer: dst_row0[d] + (row among this sender's rows for d); < 2^32
-    if (t < P.nparts) cur[t] = cur[t] - P.hist[(size_t)t * gridDim.x] + (u32)P.dst_row0[t];
-  }
-  if (blockIdx.x == 0 && P.out_offsets) {              // CTA 0's cursors are the destinations' first rows
-    if (t < P.nparts) P.out_offsets[t] = (i64)P.hist[(size_t)t * gridDim.x];
-    if (t == 0) P.out_offsets[P.nparts] = (i64)P.n;
+  if (t < 256) {
+    cur[t] = t < P.nparts ? P.hist[(size_t)t * gridDim.x + blockIdx.x] : 0u;
+    if (PEER) {   // cursor = row inside the DESTINATION's buffer: dst_row0[d] + (row among this sender's rows for d); < 2^32
+      if (t < P.nparts) cur[t] = cur[t] - P.hist[(size_t)t * gridDim.x] + (u32)P.dst_row0[t];
+    }
+    if (blockIdx.x == 0 && P.out_offsets) {            // CTA 0's cursors are the destinations' first rows
+      if (t < P.nparts) P.out_offsets[t] = (i64)P.hist[(size_t)t * gridDim.x];
+      if (t == 0) P.out_offsets[P.nparts] = (i64)P.n;
+    }
   }
   u32 lo, hi;
-  gq_hp_range(P.n, &lo, &hi);
-  for (u32 base = lo; base < hi; base += GQ_HP_TILE) {
-    const u32 nt = min((u32)GQ_HP_TILE, hi - base);    // rows of this tile
-    for (int w = 0; w < GQ_HP_WARPS; ++w) wc[w][t] = 0;
+  gq_hp_range(P.n, &lo, &hi, TILE);
+  for (u32 base = lo; base < hi; base += TILE) {
+    const u32 nt = min((u32)TILE, hi - base);          // rows of this tile
+    if (t < 256) for (int w = 0; w < NW; ++w) wc[w][t] = 0;
     __syncthreads();
     // (1) destination and rank among the warp's rows of that destination; the warp's rows are base + 256 warp + 32 j + lane
     u32 d[GQ_HP_ITEMS];
-    unsigned short wr[GQ_HP_ITEMS];
+    unsigned short place[GQ_HP_ITEMS];                 // rank among the warp's rows of the destination, then place in the tile
     gq_hp_dests(P, base + (u32)warp * 256u + (u32)lane, 32u, base + nt, lane, d);
 #pragma unroll
     for (int j = 0; j < GQ_HP_ITEMS; ++j) {
       const u32 peers = __match_any_sync(0xffffffffu, d[j]);
       const u32 rank = __popc(peers & ((1u << lane) - 1u));
       const bool have = d[j] < 256u;
-      wr[j] = have ? (unsigned short)(wc[warp][d[j]] + rank) : (unsigned short)0;
+      place[j] = have ? (unsigned short)(wc[warp][d[j]] + rank) : (unsigned short)0;
       __syncwarp();
       if (have && rank == 0) wc[warp][d[j]] += (unsigned short)__popc(peers);
       __syncwarp();
     }
     __syncthreads();
-    // (2) thread q: counters of destination q -> offsets over the warps; block scan of the totals -> toff
-    u32 tot = 0;
+    // (2) thread q < 256: counters of destination q -> offsets over the warps; block scan of the totals -> toff
+    u32 tot = 0, incl = 0;
+    if (t < 256) {
 #pragma unroll
-    for (int w = 0; w < GQ_HP_WARPS; ++w) { const u32 c = wc[w][t]; wc[w][t] = (unsigned short)tot; tot += c; }
-    u32 incl = tot;
+      for (int w = 0; w < NW; ++w) { const u32 c = wc[w][t]; wc[w][t] = (unsigned short)tot; tot += c; }
+      incl = tot;
 #pragma unroll
-    for (int o = 1; o < 32; o <<= 1) { const u32 x = __shfl_up_sync(0xffffffffu, incl, o); if (lane >= o) incl += x; }
-    if (lane == 31) wsum[warp] = incl;
-    __syncthreads();
-    u32 before = 0;
-#pragma unroll
-    for (int w = 0; w < GQ_HP_WARPS; ++w) if (w < warp) before += wsum[w];
-    const u32 first = before + incl - tot;             // place of destination t's first row in the tile
-    toff[t] = (unsigned short)first;
-    __syncthreads();
-    // (3) place of every row in the tile's destination-major order, and the output row of that place
-    unsigned short place[GQ_HP_ITEMS];
-#pragma unroll
-    for (int j = 0; j < GQ_HP_ITEMS; ++j) {
-      place[j] = 0;
-      if (d[j] < 256u) {
-        const u32 in_run = (u32)wc[warp][d[j]] + (u32)wr[j];          // rows of this destination before mine in the tile
-        place[j] = (unsigned short)((u32)toff[d[j]] + in_run);
-        gpos[place[j]] = cur[d[j]] + in_run;
-        if (PEER) pdst[place[j]] = (unsigned char)d[j];
-      }
+      for (int o = 1; o < 32; o <<= 1) { const u32 x = __shfl_up_sync(0xffffffffu, incl, o); if (lane >= o) incl += x; }
+      if (lane == 31) wsum[warp] = incl;
     }
     __syncthreads();
-    cur[t] += tot;
+    if (t < 256) {
+      u32 before = 0;
+#pragma unroll
+      for (int w = 0; w < 8; ++w) if (w < warp) before += wsum[w];
+      toff[t] = (unsigned short)(before + incl - tot);  // place of destination t's first row in the tile
+    }
+    __syncthreads();
+    // (3) place of every row in the tile's destination-major order
+#pragma unroll
+    for (int j = 0; j < GQ_HP_ITEMS; ++j) {
+      if (d[j] < 256u) {
+        const u32 in_run = (u32)wc[warp][d[j]] + (u32)place[j];        // rows of this destination before mine in the tile
+        place[j] = (unsigned short)((u32)toff[d[j]] + in_run);
+        pd[place[j]] = (unsigned char)d[j];
+        if (GPOS) gpos[place[j]] = cur[d[j]] + in_run;
+      }
+    }
     if (P.out_row) {
 #pragma unroll
       for (int j = 0; j < GQ_HP_ITEMS; ++j) {
         const u32 i = (u32)warp * 256u + (u32)j * 32u + (u32)lane;
-        if (i < nt) P.out_row[gpos[place[j]]] = (i64)(base + i);
+        if (i < nt) P.out_row[cur[d[j]] + (u32)place[j] - (u32)toff[d[j]]] = (i64)(base + i);
       }
     }
     // (4) column by column through the staging buffer. A column's values are loaded as raw 64-bit words one column AHEAD:
@@ -836,26 +844,25 @@ __global__ void __launch_bounds__(GQ_HP_THREADS, GQ_HP_CTAS_PER_SM) gq_k_hp_scat
         for (int j = 0; j < GQ_HP_ITEMS; ++j) if (d[j] < 256u) ((unsigned char*)stage)[place[j]] = (unsigned char)v[j];
       }
       if (c + 1 < P.ncols) gq_hp_load(P, c + 1, base, nt, warp, lane, v);
-      __syncthreads();
-      if (!PEER) {
-        if (dt == GQ_I64) { for (u32 p = t; p < nt; p += GQ_HP_THREADS) ((u64*)P.out[c])[gpos[p]] = ((const u64*)stage)[p]; }
-        else if (dt == GQ_I32) { for (u32 p = t; p < nt; p += GQ_HP_THREADS) ((u32*)P.out[c])[gpos[p]] = ((const u32*)stage)[p]; }
-        else { for (u32 p = t; p < nt; p += GQ_HP_THREADS) ((unsigned char*)P.out[c])[gpos[p]] = ((const unsigned char*)stage)[p]; }
-      } else {                                          // the run of destination d goes to d's own buffer (peer memory)
-        for (u32 p = t; p < nt; p += GQ_HP_THREADS) {
-          void* o = (void*)__ldg((const unsigned long long*)P.dst + (size_t)pdst[p] * P.ncols + c);
-          if (dt == GQ_I64) ((u64*)o)[gpos[p]] = ((const u64*)stage)[p];
-          else if (dt == GQ_I32) ((u32*)o)[gpos[p]] = ((const u32*)stage)[p];
-          else ((unsigned char*)o)[gpos[p]] = ((const unsigned char*)stage)[p];
-        }
+      __syncthreads();                                  // (also: pd of this tile is complete)
+      for (u32 p = t; p < nt; p += NT) {
+        const u32 dd = pd[p];
+        const u32 row = GPOS ? gpos[p] : cur[dd] + p - (u32)toff[dd];
+        void* o = PEER ? (void*)__ldg((const unsigned long long*)P.dst + (size_t)dd * P.ncols + c) : P.out[c];   // PEER: d's own buffer (peer memory)
+        if (dt == GQ_I64) ((u64*)o)[row] = ((const u64*)stage)[p];
+        else if (dt == GQ_I32) ((u32*)o)[row] = ((const u32*)stage)[p];
+        else ((unsigned char*)o)[row] = ((const unsigned char*)stage)[p];
       }
       __syncthreads();                                  // the buffer is free for the next column / tile
     }
+    if (t < 256) cur[t] += tot;                         // (read again only after the next tile's barriers)
   }
 }
-static int gq_hp_blocks(int num_sms) { return std::max(1, std::min(num_sms * GQ_HP_CTAS_PER_SM, 1024)); }
+// 4 CTAs of 256 threads per SM up to GQ_HP_WIDE_FROM destinations, 2 CTAs of 512 threads above
+#define GQ_HP_WIDE_FROM 128
+static int gq_hp_blocks(int num_sms, int nparts) { return std::max(1, std::min(num_sms * (nparts >= GQ_HP_WIDE_FROM ? 2 : 4), 1024)); }
 size_t gq_hash_partition_workspace_bytes(int nparts) {
-  return ((size_t)nparts * (size_t)gq_hp_blocks(GQ_MAX_SMS) * 4 + 255) / 256 * 256;
+  return ((size_t)nparts * (size_t)gq_hp_blocks(GQ_MAX_SMS, 1) * 4 + 255) / 256 * 256;
 }
 cudaError_t gq_launch_hash_partition(cudaStream_t s, int num_sms, const gq_batch* in, const int* key_cols, int nkeys, int nparts, char* ws,
                                      void* const* out_cols, i64* out_row, i64* out_offsets, int* nlaunches) {
@@ -864,10 +871,10 @@ cudaError_t gq_launch_hash_partition(cudaStream_t s, int num_sms, const gq_batch
   for (int k = 0; k < nkeys; ++k) { P.key[k] = in->cols[key_cols[k]].data; P.key_dtype[k] = (int)in->cols[key_cols[k]].dtype; }
   for (int c = 0; c < in->ncols; ++c) { P.col[c] = in->cols[c].data; P.out[c] = out_cols[c]; P.dtype[c] = (int)in->cols[c].dtype; }
   P.hist = (u32*)ws; P.out_row = out_row; P.out_offsets = out_offsets; P.dst = nullptr; P.dst_row0 = nullptr;
-  const int nblk = gq_hp_blocks(num_sms);
-  gq_k_hp_hist<<<nblk, GQ_HP_THREADS, 0, s>>>(P);
+  const int nblk = gq_hp_blocks(num_sms, nparts);
+  if (nparts >= GQ_HP_WIDE_FROM) gq_k_hp_hist<512><<<nblk, 512, 0, s>>>(P); else gq_k_hp_hist<256><<<nblk, 256, 0, s>>>(P);
   gq_k_sort_scan<<<1, 1024, 0, s>>>(P.hist, nparts * nblk);
-  gq_k_hp_scatter<false><<<nblk, GQ_HP_THREADS, 0, s>>>(P);
+  if (nparts >= GQ_HP_WIDE_FROM) gq_k_hp_scatter<512, false><<<nblk, 512, 0, s>>>(P); else gq_k_hp_scatter<256, false><<<nblk, 256, 0, s>>>(P);
   *nlaunches = 3;
   return cudaGetLastError();
 }
@@ -892,8 +899,8 @@ cudaError_t gq_launch_hash_partition_count(cudaStream_t s, int num_sms, const gq
                                            i64* counts, int* nlaunches) {
   GqHpParams P;
   gq_hp_fill(P, in, key_cols, nkeys, nparts, ws);
-  const int nblk = gq_hp_blocks(num_sms);
-  gq_k_hp_hist<<<nblk, GQ_HP_THREADS, 0, s>>>(P);
+  const int nblk = gq_hp_blocks(num_sms, nparts);
+  if (nparts >= GQ_HP_WIDE_FROM) gq_k_hp_hist<512><<<nblk, 512, 0, s>>>(P); else gq_k_hp_hist<256><<<nblk, 256, 0, s>>>(P);
   gq_k_sort_scan<<<1, 1024, 0, s>>>(P.hist, nparts * nblk);
   gq_k_hp_counts<<<1, 256, 0, s>>>(P.hist, nblk, nparts, P.n, counts);
   *nlaunches = 3;
@@ -904,7 +911,8 @@ cudaError_t gq_launch_hash_partition_scatter_to(cudaStream_t s, int num_sms, con
   GqHpParams P;
   gq_hp_fill(P, in, key_cols, nkeys, nparts, ws);
   P.dst = d_dst; P.dst_row0 = d_row0;
-  gq_k_hp_scatter<true><<<gq_hp_blocks(num_sms), GQ_HP_THREADS, 0, s>>>(P);
+  if (nparts >= GQ_HP_WIDE_FROM) gq_k_hp_scatter<512, true><<<gq_hp_blocks(num_sms, nparts), 512, 0, s>>>(P);
+  else gq_k_hp_scatter<256, true><<<gq_hp_blocks(num_sms, nparts), 256, 0, s>>>(P);
   *nlaunches = 1;
   return cudaGetLastError();
 }
