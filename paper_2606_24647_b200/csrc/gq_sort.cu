@@ -448,7 +448,7 @@ __global__ void __launch_bounds__(1024) gq_k_sort_small(const __grid_constant__ 
   for (u32 k = 2; k <= N; k <<= 1)
     for (u32 j = k >> 1; j > 0; j >>= 1) {
       if (t < N / 2) {                                    // compare-exchange number t of this stage: elements e and e + j
-        const u32 e = 2 * j * (t / j) + (t % j);
+        const u32 e = ((t & ~(j - 1u)) << 1) | (t & (j - 1u));   // = 2 j (t / j) + t % j, j a power of two
         const bool asc = (e & k) == 0;
         const u32 a = idx[e], b = idx[e + j];
         if (gq_small_less(P, img, b, a) == asc) { idx[e] = b; idx[e + j] = a; }
