@@ -125,7 +125,8 @@ def test_partitions_feed_partial_to_final_aggregation(ctx):
     assert seen == whole.nrows
 
 
-def test_count_then_scatter_into_destination_buffers(ctx):
+@pytest.mark.parametrize("nparts", [5, 200])
+def test_count_then_scatter_into_destination_buffers(ctx, nparts):
     # the fused partition + transfer protocol on one GPU: three "senders" (batches) count, the counts are laid out per
     # destination (sender after sender: what an exchange of counts gives every rank), then every sender scatters straight
     # into the destinations' own buffers — separate allocations here, peer-mapped memory on several GPUs. Destination d
@@ -133,7 +134,7 @@ def test_count_then_scatter_into_destination_buffers(ctx):
     import torch
     import gqrun
     rng = np.random.default_rng(21)
-    nparts, sizes = 5, (70_001, 4_097, 33)
+    sizes = (70_001, 4_097, 33)                                    # (200 destinations: the 512-thread kernels)
     senders = []
     for i, n in enumerate(sizes):
         cols = _cols(n, 300 + i)
